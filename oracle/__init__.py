@@ -1,0 +1,248 @@
+"""ufnvc oracle -- TEST INFRASTRUCTURE ONLY (see ufnvc_oracle.c header).
+
+Plain CPU chunk decode, steps O1..O9 of SURVEY.md section 8(c), following PAPER.md section 3.1 (chunk decoder
++ frame-specific decoders) and section 3.4 (single-step entropy: sigma for everything in one pass,
+r = AD(sigma), y = r + mu).  The C file holds the loops; this file strings them together in
+the paper's order and keeps every intermediate.  It imports nothing from the product package.
+
+Importers allowed: tests/, __graft_entry__.smoke(), bench.py's cpu_baseline / --impl reference legs.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import math
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_LIBS = {}
+
+
+def _lib(real: str):
+    if real not in _LIBS:
+        path = _build.lib_path(real)
+        if not os.path.exists(path):
+            _build.build()
+        lib = C.CDLL(path)
+        lib.orc_rans_encode_substream.restype = C.c_long
+        lib.orc_rans_decode_substream.restype = C.c_int
+        lib.orc_ideal_bits.restype = C.c_double
+        lib.orc_real_bytes.restype = C.c_int
+        _LIBS[real] = lib
+    return _LIBS[real]
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+class Oracle:
+    """Thin typed wrappers over the C loops.  real = "f64" (default, parity truth) or "f32"."""
+
+    def __init__(self, real: str = "f64"):
+        self.real = real
+        self.lib = _lib(real)
+        self.dt = np.float64 if real == "f64" else np.float32
+        assert self.lib.orc_real_bytes() == np.dtype(self.dt).itemsize
+
+    def arr(self, a):
+        return np.ascontiguousarray(a, dtype=self.dt)
+
+    # ---- layers (planar [C][H][W]) ----
+    def conv2d(self, x, w, b):
+        x, w = self.arr(x), self.arr(w)
+        co, ci, k, _ = w.shape
+        assert x.shape[0] == ci and k in (1, 3)
+        out = np.empty((co,) + x.shape[1:], self.dt)
+        bb = self.arr(b) if b is not None else None
+        self.lib.orc_conv2d(_p(x), C.c_int(ci), C.c_int(x.shape[1]), C.c_int(x.shape[2]), _p(w),
+                            _p(bb) if bb is not None else None, C.c_int(co), C.c_int(k), _p(out))
+        return out
+
+    def dwconv3x3(self, x, w, b):
+        x, w = self.arr(x), self.arr(w)
+        out = np.empty_like(x)
+        bb = self.arr(b) if b is not None else None
+        self.lib.orc_dwconv3x3(_p(x), C.c_int(x.shape[0]), C.c_int(x.shape[1]), C.c_int(x.shape[2]), _p(w),
+                               _p(bb) if bb is not None else None, _p(out))
+        return out
+
+    def pixel_shuffle(self, x, r):
+        x = self.arr(x)
+        c = x.shape[0] // (r * r)
+        assert c * r * r == x.shape[0]
+        out = np.empty((c, x.shape[1] * r, x.shape[2] * r), self.dt)
+        self.lib.orc_pixel_shuffle(_p(x), C.c_int(c), C.c_int(x.shape[1]), C.c_int(x.shape[2]), C.c_int(r), _p(out))
+        return out
+
+    def relu(self, x):
+        x = self.arr(x).copy()
+        self.lib.orc_relu(_p(x), C.c_size_t(x.size))
+        return x
+
+    def gelu(self, x):
+        x = self.arr(x).copy()
+        self.lib.orc_gelu(_p(x), C.c_size_t(x.size))
+        return x
+
+    # ---- entropy model pieces ----
+    def build_cdf(self, nb, smin, smax):
+        cdf = np.empty((nb, 256), np.uint32)
+        self.lib.orc_build_cdf(C.c_int(nb), C.c_double(smin), C.c_double(smax), _p(cdf))
+        return cdf
+
+    def bucket_index(self, u, nb, smin, smax):
+        u = self.arr(u)
+        idx = np.empty(u.shape, np.uint8)
+        uc = np.empty_like(u)
+        self.lib.orc_bucket_index(_p(u), C.c_size_t(u.size), C.c_int(nb), C.c_double(smin), C.c_double(smax),
+                                  _p(idx), _p(uc))
+        return idx, uc
+
+    def symbols_from_uniform(self, cdf, idx, u16):
+        idx = np.ascontiguousarray(idx, np.uint8)
+        u16 = np.ascontiguousarray(u16, np.uint16)
+        assert idx.shape == u16.shape
+        sym = np.empty(idx.shape, np.int16)
+        self.lib.orc_symbols_from_uniform(_p(cdf), _p(idx), _p(u16), C.c_size_t(idx.size), _p(sym))
+        return sym
+
+    def rans_encode_substream(self, cdf, idx, sym, W):
+        idx = np.ascontiguousarray(idx, np.uint8).ravel()
+        sym = np.ascontiguousarray(sym, np.int16).ravel()
+        cap = 8 * (W // 32) + (W // 32) * 136 + 2 * sym.size + 64
+        out = np.zeros(cap, np.uint8)
+        n = self.lib.orc_rans_encode_substream(_p(cdf), _p(idx), _p(sym), C.c_size_t(sym.size), C.c_int(W),
+                                               _p(out), C.c_size_t(cap))
+        if n < 0:
+            raise ValueError(f"rANS encode failed ({n})")
+        return out[:n].copy()
+
+    def rans_decode_substream(self, cdf, idx, W, data):
+        idx = np.ascontiguousarray(idx, np.uint8).ravel()
+        data = np.ascontiguousarray(data, np.uint8)
+        sym = np.zeros(idx.size, np.int16)
+        st = self.lib.orc_rans_decode_substream(_p(cdf), _p(idx), C.c_size_t(idx.size), C.c_int(W), _p(data),
+                                                C.c_size_t(data.size), _p(sym))
+        return sym, int(st)
+
+    def ideal_bits(self, cdf, idx, sym):
+        idx = np.ascontiguousarray(idx, np.uint8).ravel()
+        sym = np.ascontiguousarray(sym, np.int16).ravel()
+        return float(self.lib.orc_ideal_bits(_p(cdf), _p(idx), _p(sym), C.c_size_t(sym.size)))
+
+
+# ---------------------------------------------------------------------------------------------
+# geometry (SURVEY.md section 8 notation; R2, R16)
+# ---------------------------------------------------------------------------------------------
+def geometry(cfg):
+    H = -(-cfg.height // 16) * 16
+    W = -(-cfg.width // 16) * 16
+    h, w = H // 16, W // 16
+    return dict(H=H, W=W, h=h, w=w, h_z=-(-h // 4), w_z=-(-w // 4), n_sub=-(-h // cfg.rows_per_substream))
+
+
+# ---------------------------------------------------------------------------------------------
+# the path, in the paper's order
+# ---------------------------------------------------------------------------------------------
+def entropy_params(orc: Oracle, cfg, weights, z):
+    """O1 + O2 (one forward pass gives the scale of every element and the mean).
+    z: int [C_z][h_z][w_z].  Returns mu, u = clamped ln sigma, idx, each [C_y][h][w]."""
+    g = geometry(cfg)
+    x0 = orc.arr(z)
+    x1 = orc.relu(orc.conv2d(x0, weights["hyper.0.w"], weights["hyper.0.b"]))
+    x2 = orc.relu(orc.conv2d(x1, weights["hyper.1.w"], weights["hyper.1.b"]))
+    x3 = orc.conv2d(x2, weights["hyper.2.w"], weights["hyper.2.b"])
+    ps = orc.pixel_shuffle(x3, 4)[:, :g["h"], :g["w"]]
+    mu = np.ascontiguousarray(ps[:cfg.c_y])
+    idx, u = orc.bucket_index(np.ascontiguousarray(ps[cfg.c_y:]), cfg.n_buckets, cfg.scale_min, cfg.scale_max)
+    return mu, u, idx
+
+
+def _stream_order(a_chw, r0, r1):
+    """planar [C][h][w] rows [r0,r1) -> stream order (row, col, channel) [R9]."""
+    return np.ascontiguousarray(np.transpose(a_chw[:, r0:r1, :], (1, 2, 0))).ravel()
+
+
+def encode_chunk(orc: Oracle, cfg, cdf, idx, sym):
+    """Test-fixture ENCODER (mirror of O4).  idx, sym planar [C_y][h][w].  Returns (bytes, sub_off[n_sub+1])."""
+    g = geometry(cfg)
+    parts, off = [], [0]
+    for s in range(g["n_sub"]):
+        r0, r1 = s * cfg.rows_per_substream, min((s + 1) * cfg.rows_per_substream, g["h"])
+        b = orc.rans_encode_substream(cdf, _stream_order(idx, r0, r1), _stream_order(sym, r0, r1),
+                                      cfg.lanes_per_substream)
+        parts.append(b)
+        off.append(off[-1] + b.size)
+    return np.concatenate(parts), np.asarray(off, np.uint32)
+
+
+def decode_symbols(orc: Oracle, cfg, cdf, idx, bits, sub_off):
+    """O4 (arithmetic decoding of all partitions in one consolidated step, scale only)."""
+    g = geometry(cfg)
+    sym = np.zeros((cfg.c_y, g["h"], g["w"]), np.int16)
+    status = 0
+    for s in range(g["n_sub"]):
+        r0, r1 = s * cfg.rows_per_substream, min((s + 1) * cfg.rows_per_substream, g["h"])
+        ss, st = orc.rans_decode_substream(cdf, _stream_order(idx, r0, r1), cfg.lanes_per_substream,
+                                           bits[int(sub_off[s]):int(sub_off[s + 1])])
+        sym[:, r0:r1, :] = np.transpose(ss.reshape(r1 - r0, g["w"], cfg.c_y), (2, 0, 1))
+        status = status or st
+    return sym, status
+
+
+def synthesis(orc: Oracle, cfg, weights, yhat, keep=False):
+    """O6..O9: cross-frame unfold, shared trunk of DC blocks, T frame-specific
+    decoders, clamp + crop.  yhat [C_y][h][w].  Returns frames [T][3][height][width] (+ taps)."""
+    taps = {}
+    f0 = orc.conv2d(yhat, weights["xframe.w"], weights["xframe.b"])            # O6: [T*C_t][h][w]
+    frames = np.empty((cfg.T, 3, cfg.height, cfg.width), orc.dt)
+    if keep:
+        taps["F0"] = f0.reshape(cfg.T, cfg.c_trunk, *f0.shape[1:]).copy()
+        taps["trunk"] = []
+        taps["stage"] = [[] for _ in range(cfg.T)]
+    for t in range(cfg.T):
+        x = np.ascontiguousarray(f0[t * cfg.c_trunk:(t + 1) * cfg.c_trunk])
+        for k in range(cfg.n_trunk_blocks):                                    # O7, same weights for every t [R15]
+            d = orc.dwconv3x3(x, weights[f"trunk.{k}.dw.w"], weights[f"trunk.{k}.dw.b"])
+            e = orc.gelu(orc.conv2d(d, weights[f"trunk.{k}.pw1.w"], weights[f"trunk.{k}.pw1.b"]))
+            x = x + orc.conv2d(e, weights[f"trunk.{k}.pw2.w"], weights[f"trunk.{k}.pw2.b"])
+        if keep:
+            taps["trunk"].append(x.copy())
+        for s in range(4):                                                     # O8 [R10]
+            a = orc.conv2d(x, weights[f"dec.{t}.{s}.w"], weights[f"dec.{t}.{s}.b"])
+            if s < 3:
+                a = orc.gelu(a)
+            x = orc.pixel_shuffle(a, 2)
+            if keep and s < 3:
+                taps["stage"][t].append(x.copy())
+        frames[t] = np.clip(x, 0.0, 1.0)[:, :cfg.height, :cfg.width]           # O9 [R16]
+    return frames, taps
+
+
+def chunk_decode(orc: Oracle, cfg, weights, z, bits, sub_off, idx_override=None, mu_override=None, keep=False):
+    """One chunk, O1..O9.  z [C_z][h_z][w_z]; bits uint8; sub_off [n_sub+1] byte offsets into bits."""
+    mu, u, idx = entropy_params(orc, cfg, weights, z)
+    if idx_override is not None:
+        idx = np.ascontiguousarray(idx_override, np.uint8)
+    if mu_override is not None:
+        mu = orc.arr(mu_override)
+    cdf = orc.build_cdf(cfg.n_buckets, cfg.scale_min, cfg.scale_max)          # O3
+    sym, status = decode_symbols(orc, cfg, cdf, idx, bits, sub_off)            # O4
+    yhat = sym.astype(orc.dt) + mu                                             # O5
+    frames, taps = synthesis(orc, cfg, weights, yhat, keep=keep)
+    return dict(mu=mu, u=u, idx=idx, sym=sym, status=status, yhat=yhat, frames=frames, taps=taps)
+
+
+def make_stream(orc: Oracle, cfg, weights, z, u16_hwc, idx_override=None):
+    """Fixture: what an encoder would have produced for this z -- run the prior net (O1, O2), draw r from the
+    quantised tables by inverse CDF with the given 16-bit uniforms [h][w][C_y] (R7), encode (mirror of O4)."""
+    mu, u, idx = entropy_params(orc, cfg, weights, z)
+    if idx_override is not None:
+        idx = np.ascontiguousarray(idx_override, np.uint8)
+    cdf = orc.build_cdf(cfg.n_buckets, cfg.scale_min, cfg.scale_max)
+    sym = orc.symbols_from_uniform(cdf, idx, np.transpose(u16_hwc, (2, 0, 1)))
+    bits, sub_off = encode_chunk(orc, cfg, cdf, idx, sym)
+    return dict(mu=mu, u=u, idx=idx, sym=sym, bits=bits, sub_off=sub_off, cdf=cdf)

@@ -1,0 +1,220 @@
+"""Seeded synthetic inputs for the chunk-decode path.
+
+This module is shared by the CUDA path's callers (tests, bench.py) and by the oracle's
+callers (tests).  It holds NONE of the method's arithmetic: it only names the five
+BASELINE.json workloads and draws raw random numbers (weights, the hyper-latent z, 16-bit
+uniforms from which each side derives its own symbols, and exact-law (mu, ln sigma) maps
+for the entropy-only mode).  Neither `oracle/` nor `csrc/` imports it.
+
+Stand-in statement: the paper measures on UVG / MCL-JCV / HEVC B-E natural video
+ with trained weights; neither is available, so everything below is random
+with the shapes of BASELINE.json:configs.
+"""
+from __future__ import annotations
+
+import dataclasses
+import math
+import zlib
+
+import numpy as np
+
+
+@dataclasses.dataclass(frozen=True)
+class ChunkConfig:
+    """Mirror of `ufnvc_config` (include/ufnvc.h) plus the seed and the input laws."""
+    name: str
+    seed: int
+    T: int
+    height: int
+    width: int
+    c_y: int
+    c_z: int
+    c_hyper: int
+    c_trunk: int
+    n_trunk_blocks: int
+    trunk_expand: int
+    dec_channels: tuple
+    n_buckets: int = 64
+    scale_min: float = 0.11
+    scale_max: float = 20.0
+    rows_per_substream: int = 4
+    lanes_per_substream: int = 128
+    n_chunks: int = 1
+    weight_dtype: int = 1          # 0 = fp32, 1 = bf16
+    mu_law: str = "normal"         # "normal": N(0,1); "uniform": U(-2,2)
+    sigma_hi: float = 20.0         # ln sigma ~ U[ln scale_min, ln sigma_hi] (moment-matched, see make_weights)
+
+    # derived geometry (SURVEY.md section 8 notation)
+    @property
+    def H(self):  # padded frame height
+        return -(-self.height // 16) * 16
+
+    @property
+    def W(self):
+        return -(-self.width // 16) * 16
+
+    @property
+    def h(self):
+        return self.H // 16
+
+    @property
+    def w(self):
+        return self.W // 16
+
+    @property
+    def h_z(self):
+        return -(-self.h // 4)
+
+    @property
+    def w_z(self):
+        return -(-self.w // 4)
+
+    @property
+    def n_sub(self):
+        return -(-self.h // self.rows_per_substream)
+
+    @property
+    def n_symbols(self):
+        return self.c_y * self.h * self.w
+
+    def macs_per_chunk(self) -> int:
+        """Algorithmic multiply-accumulates of one chunk decode."""
+        hz, wz, P = self.h_z, self.w_z, self.h * self.w
+        m = hz * wz * 9 * (self.c_z * self.c_hyper + self.c_hyper * self.c_hyper
+                           + self.c_hyper * 2 * self.c_y * 16)
+        m += P * self.c_y * self.T * self.c_trunk
+        m += self.n_trunk_blocks * self.T * P * (9 * self.c_trunk
+                                                 + 2 * self.c_trunk * self.c_trunk * self.trunk_expand)
+        pix = P
+        for s in range(4):
+            ci, co = self.dec_channels[s], self.dec_channels[s + 1]
+            m += self.T * pix * 9 * ci * 4 * co
+            pix *= 4
+        return m
+
+
+_DEC = (256, 192, 128, 64, 3)
+
+CONFIGS = {
+    1: ChunkConfig("cfg1-tiny", 0, 2, 64, 64, 32, 16, 32, 64, 0, 4, (64, 48, 32, 16, 3),
+                   lanes_per_substream=32, weight_dtype=0, mu_law="uniform"),
+    2: ChunkConfig("cfg2-480p", 1, 4, 480, 832, 128, 64, 128, 256, 4, 4, _DEC),
+    3: ChunkConfig("cfg3-1080p", 2, 8, 1080, 1920, 128, 64, 128, 256, 6, 4, _DEC),
+    4: ChunkConfig("cfg4-1080p-4xT16", 3, 16, 1080, 1920, 192, 64, 128, 256, 6, 4, _DEC,
+                   lanes_per_substream=192, n_chunks=4, sigma_hi=2.0),
+    5: ChunkConfig("cfg5-4k", 4, 8, 2160, 3840, 128, 64, 128, 256, 8, 4, _DEC),
+}
+
+
+def crop_config(cfg: ChunkConfig, height: int, width: int, name: str | None = None) -> ChunkConfig:
+    """Same layer plan on a smaller frame (used for bounded CPU-baseline samples and mid-size parity)."""
+    return dataclasses.replace(cfg, height=height, width=width,
+                               name=name or f"{cfg.name}-crop{width}x{height}")
+
+
+def round_to_bf16(a: np.ndarray) -> np.ndarray:
+    """fp32 array -> nearest-even bf16 value, returned as fp32 (so both sides consume identical weights)."""
+    u = np.ascontiguousarray(a, dtype=np.float32).view(np.uint32)
+    r = ((u >> 16) & 1) + np.uint32(0x7FFF)
+    return ((u + r) & np.uint32(0xFFFF0000)).view(np.float32)
+
+
+def _rng(cfg: ChunkConfig, tag: str) -> np.random.Generator:
+    return np.random.default_rng(np.random.SeedSequence([cfg.seed, zlib.crc32(tag.encode())]))
+
+
+def _ln_sigma_moments(cfg: ChunkConfig):
+    lo, hi = math.log(cfg.scale_min), math.log(cfg.sigma_hi)
+    return 0.5 * (lo + hi), (hi - lo) / math.sqrt(12.0)
+
+
+def _second_moment_yhat(cfg: ChunkConfig) -> float:
+    # E[y^2] for y = r + mu, r ~ N(0, sigma^2) rounded, ln sigma uniform: closed form of E[sigma^2].
+    lo, hi = cfg.scale_min, cfg.sigma_hi
+    e_s2 = (hi * hi - lo * lo) / (2.0 * math.log(hi / lo))
+    var_mu = 1.0 if cfg.mu_law == "normal" else 4.0 / 3.0
+    return e_s2 + 1.0 / 12.0 + var_mu
+
+
+def make_weights(cfg: ChunkConfig) -> dict:
+    """Canonical-layout weights: conv [C_out][C_in][kh][kw] fp32 (bf16-representable when
+    weight_dtype == 1), biases fp32.  Kaiming-normal with analytic gains (R3/R11):
+    no data-dependent calibration, so no side has to run the net to make its own inputs."""
+    out = {}
+
+    def conv(name, co, ci, k, gain2, bias_std=0.02, bias_mean=0.0):
+        rng = _rng(cfg, name)
+        fan_in = ci * k * k
+        w = rng.normal(0.0, math.sqrt(gain2 / fan_in), size=(co, ci, k, k)).astype(np.float32)
+        b = (bias_mean + rng.normal(0.0, bias_std, size=(co,))).astype(np.float32)
+        out[name + ".w"] = round_to_bf16(w) if cfg.weight_dtype == 1 else w
+        out[name + ".b"] = b
+
+    # hyper-decoder (O1): z ~ round(N(0,4)) so E[z^2] ~ 4.08; ReLU + gain 2 keeps E[x^2] ~ 4.08.
+    # `edge` = mean fraction of the 9 taps that fall inside a zero-padded h_z x w_z map (pure geometry):
+    # dividing the gain by it keeps the mean variance on tiny maps (config 1 has a 1x1 z).
+    edge = ((3 * cfg.h_z - 2) / (3 * cfg.h_z)) * ((3 * cfg.w_z - 2) / (3 * cfg.w_z))
+    conv("hyper.0", cfg.c_hyper, cfg.c_z, 3, 2.0 / edge)
+    conv("hyper.1", cfg.c_hyper, cfg.c_hyper, 3, 2.0 / edge)
+    # head: channels after pixel-shuffle x4: [0,C_y) = mu, [C_y,2C_y) = ln sigma.  Pre-shuffle
+    # channel o = c*16 + 4i + j  ->  rows [0, 16 C_y) feed mu, the rest feed ln sigma.
+    m_u, s_u = _ln_sigma_moments(cfg)
+    s_mu = 1.0 if cfg.mu_law == "normal" else 2.0 / math.sqrt(3.0)
+    ex2 = 4.08
+    name = "hyper.2"
+    rng = _rng(cfg, name)
+    co, ci = 2 * cfg.c_y * 16, cfg.c_hyper
+    w = rng.normal(0.0, 1.0, size=(co, ci, 3, 3)) / math.sqrt(ci * 9 * ex2 * edge)
+    half = cfg.c_y * 16
+    w[:half] *= s_mu
+    w[half:] *= s_u
+    b = rng.normal(0.0, 0.02, size=(co,))
+    b[half:] += m_u
+    w = w.astype(np.float32)
+    out[name + ".w"] = round_to_bf16(w) if cfg.weight_dtype == 1 else w
+    out[name + ".b"] = b.astype(np.float32)
+
+    # cross-frame unfold (O6): gain so that E[F0^2] ~ 1.
+    conv("xframe", cfg.T * cfg.c_trunk, cfg.c_y, 1, 1.0 / _second_moment_yhat(cfg))
+    # trunk (O7): shared over t; W2 scaled by 1/B so the residual stream stays O(1).
+    ce = cfg.c_trunk * cfg.trunk_expand
+    for k in range(cfg.n_trunk_blocks):
+        conv(f"trunk.{k}.dw", cfg.c_trunk, 1, 3, 1.0)
+        conv(f"trunk.{k}.pw1", ce, cfg.c_trunk, 1, 2.0)
+        conv(f"trunk.{k}.pw2", cfg.c_trunk, ce, 1, 1.0 / max(1, cfg.n_trunk_blocks))
+    # frame-specific decoders (O8): distinct weights per frame index t.
+    for t in range(cfg.T):
+        for s in range(4):
+            ci, co = cfg.dec_channels[s], cfg.dec_channels[s + 1]
+            if s < 3:
+                conv(f"dec.{t}.{s}", 4 * co, ci, 3, 2.0)
+            else:   # linear output stage: mean 0.5, std ~0.2 (input second moment ~1.5)
+                conv(f"dec.{t}.{s}", 4 * co, ci, 3, 0.04 / 1.5, bias_std=0.02, bias_mean=0.5)
+    return out
+
+
+def make_z(cfg: ChunkConfig) -> np.ndarray:
+    """Hyper-latent z: round(N(0, 2^2)) clipped to +-15, int16 [n_chunks][C_z][h_z][w_z]."""
+    rng = _rng(cfg, "z")
+    z = np.rint(rng.normal(0.0, 2.0, size=(cfg.n_chunks, cfg.c_z, cfg.h_z, cfg.w_z)))
+    return np.clip(z, -15, 15).astype(np.int16)
+
+
+def make_uniform16(cfg: ChunkConfig) -> np.ndarray:
+    """One uniform 16-bit draw per latent element, [n_chunks][h][w][C_y] (stream order).
+    Each side turns it into a symbol by inverse-CDF on ITS OWN quantised table (R7)."""
+    rng = _rng(cfg, "u16")
+    return rng.integers(0, 1 << 16, size=(cfg.n_chunks, cfg.h, cfg.w, cfg.c_y), dtype=np.uint16)
+
+
+def make_exact_law_params(cfg: ChunkConfig):
+    """Entropy-only mode: mu and ln sigma drawn EXACTLY from the laws BASELINE.json states,
+    [n_chunks][h][w][C_y] fp32 each."""
+    rng = _rng(cfg, "exact")
+    shape = (cfg.n_chunks, cfg.h, cfg.w, cfg.c_y)
+    if cfg.mu_law == "normal":
+        mu = rng.normal(0.0, 1.0, size=shape)
+    else:
+        mu = rng.uniform(-2.0, 2.0, size=shape)
+    u = rng.uniform(math.log(cfg.scale_min), math.log(cfg.sigma_hi), size=shape)
+    return mu.astype(np.float32), u.astype(np.float32)
