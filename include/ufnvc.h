@@ -1,0 +1,157 @@
+/*
+ * ufnvc.h -- C ABI of the B200-native chunk-decode library (libufnvc.so).
+ *
+ * The operation: decode of one chunk of the chunk-based neural video codec of "Ultra-Fast Neural Video
+ * Compression" (DCVC-UF).  PAPER.md:79-81 (section 3.1): "the latent representation y_i is parsed from the
+ * bit-stream and fed to the chunk decoder, which generates a rich feature F_i ... used by a set of parallel,
+ * frame-specific decoders to reconstruct the individual frames {x_i,0 .. x_i,N-1}".
+ * (section 3.4): the parameter network predicts the scales of every element in ONE forward pass, "r_i is
+ * recovered using only sigma_i, and the final latent is reconstructed as y_i = r_i + mu_i", arithmetic
+ * decoding of all partitions is "one consolidated step".  The layer plan is BASELINE.json:configs as read by
+ * SURVEY.md section 8(c) O1..O9 and DESIGN.md (readings R0..R18).
+ *
+ * Conventions
+ *   - plain pointers and sizes only; "_dev" = device pointer (cudaMalloc / torch CUDA tensor), "_host" = host.
+ *   - every function returns 0 (UFNVC_OK) or a negative ufnvc_status; no exceptions cross the ABI; no globals.
+ *   - a handle is used from one host thread and one CUDA stream at a time; it owns weights, CDF tables,
+ *     TMA descriptors and a workspace sized at create for max_chunks_per_call.
+ *   - ufnvc_chunk_decode only ENQUEUES work on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy
+ *     default stream): it never synchronises, never allocates and never touches the host copy of anything.
+ *   - sm_100 only: ufnvc_create fails with UFNVC_E_UNSUPPORTED_DEVICE elsewhere.  There is no CPU fallback.
+ */
+#ifndef UFNVC_H
+#define UFNVC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum ufnvc_status {
+    UFNVC_OK = 0,
+    UFNVC_E_INVALID_ARG = -1,
+    UFNVC_E_BAD_CONFIG = -2,
+    UFNVC_E_NO_WEIGHTS = -3,
+    UFNVC_E_BAD_BLOB = -4,
+    UFNVC_E_UNSUPPORTED_DEVICE = -5,
+    UFNVC_E_CUDA = -6,
+    UFNVC_E_OOM = -7
+} ufnvc_status;
+
+/* device-side bit-stream status bits, OR-ed over all warp-streams of the last call (ufnvc_get_status) */
+#define UFNVC_STREAM_BAD_END_STATE 1u /* some lane did not return to 2^16 */
+#define UFNVC_STREAM_BAD_WORD_COUNT 2u /* words consumed != words present */
+#define UFNVC_STREAM_BAD_HEADER 4u    /* offsets outside the substream; reads were clamped */
+
+typedef struct ufnvc_handle ufnvc_handle; /* opaque */
+
+/* Plain-old-data, versioned by struct_size.  Geometry (R16): frames are padded at
+ * the bottom/right to multiples of 32 (the rule that reproduces every BASELINE.json shape: 1080 -> 1088,
+ * 2160 -> 2176, 480 -> 480); latent h = H/16, w = W/16; hyper-latent h_z = ceil(h/4), w_z = ceil(w/4) [R2]. */
+typedef struct ufnvc_config {
+    uint32_t struct_size;        /* = sizeof(ufnvc_config) */
+    int32_t T;                   /* frames per chunk (paper's N), >= 1 */
+    int32_t height, width;       /* output frame size, e.g. 1080 x 1920 */
+    int32_t c_y, c_z;            /* channels of the chunk latent y and of the hyper-latent z */
+    int32_t c_hyper;             /* hyper-decoder width (O1) */
+    int32_t c_trunk;             /* per-frame feature width after the cross-frame unfold (O6) */
+    int32_t n_trunk_blocks;      /* residual DC blocks shared over t (O7), >= 0 */
+    int32_t trunk_expand;        /* 1x1 expansion factor inside a DC block (4) */
+    int32_t dec_channels[5];     /* frame-decoder channels, dec_channels[0] == c_trunk, dec_channels[4] == 3 */
+    int32_t n_buckets;           /* scale buckets (64), log-spaced on [scale_min, scale_max] inclusive [R4] */
+    float scale_min, scale_max;  /* 0.11, 20 */
+    int32_t rows_per_substream;  /* latent rows per rANS substream (4) [R9] */
+    int32_t lanes_per_substream; /* interleaved rANS lanes W per substream, multiple of 32 (default c_y) */
+    int32_t max_chunks_per_call; /* independent chunks decoded by one call (1; 4 for config 4) */
+    int32_t weight_dtype;        /* dtype of conv weights in the blob: 0 = fp32, 1 = bf16 */
+} ufnvc_config;
+
+/* Optional device buffers that receive intermediates of ufnvc_chunk_decode_ex (parity/debug; any may be NULL).
+ * Layouts are the library's own: channels-last. */
+typedef struct ufnvc_taps {
+    uint32_t struct_size;
+    float *mu;          /* [n][h][w][c_y]  mean (O2) */
+    float *lnscale;     /* [n][h][w][c_y]  clamped ln sigma (O2) */
+    uint8_t *idx;       /* [n][h][w][c_y]  bucket index actually used for decoding */
+    int16_t *sym;       /* [n][h][w][c_y]  decoded residual r (O4) */
+    float *yhat;        /* [n][h][w][c_y]  r + mu before bf16 rounding (O5) */
+    uint16_t *f0;       /* bf16 [n][T][h][w][c_trunk]            after the cross-frame unfold (O6) */
+    uint16_t *trunk;    /* bf16 [n][T][h][w][c_trunk]            after the trunk (O7) */
+    uint16_t *stage[3]; /* bf16 [n][T][2^s h][2^s w][dec_channels[s]], s = 1..3, after decoder stage s (O8) */
+} ufnvc_taps;
+
+/* Validate cfg, check the device (cuda:current), allocate tables + workspace.  *out is set on success only. */
+int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out);
+
+/* Waits for the device, frees everything the handle owns.  The handle must not be used afterwards. */
+int ufnvc_destroy(ufnvc_handle *h);
+
+/* Parse, copy and repack the weights blob (host pointer; not retained).  Blob format (little-endian):
+ *   char magic[8] = "UFNVCW01"; uint32 n_tensors; uint32 reserved;
+ *   n_tensors x { char name[40]; uint32 dtype (0 fp32, 1 bf16); uint32 ndim; uint32 shape[4];
+ *                 uint64 offset (from blob start, 16-byte aligned); uint64 nbytes };
+ *   data.
+ * Tensors (canonical [C_out][C_in][kh][kw], biases fp32 [C_out]): hyper.{0,1,2}.{w,b}, xframe.{w,b},
+ * trunk.{k}.{dw,pw1,pw2}.{w,b}, dec.{t}.{s}.{w,b} (t < T, s < 4).  Missing / mis-shaped tensor: UFNVC_E_BAD_BLOB. */
+int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t bytes);
+
+/* The hot path, one call, everything enqueued on cuda_stream:
+ *   z_dev        int16 [n_chunks][c_z][h_z][w_z]                    hyper-latent (already entropy-decoded, R0)
+ *   bits_dev     the rANS bit-stream of r for all chunks, 4-byte aligned
+ *   sub_off_dev  uint32 [n_chunks * n_sub + 1] byte offsets of the substreams inside bits_dev, multiples of 4
+ *   frames_dev   float [n_chunks][T][3][height][width], values in [0,1]     (output, caller-owned)
+ * Bit-stream corruption never faults: reads are clamped and a status word is set (ufnvc_get_status). */
+int ufnvc_chunk_decode(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, const uint8_t *bits_dev,
+                       size_t bits_bytes, const uint32_t *sub_off_dev, float *frames_dev, void *cuda_stream);
+
+/* Same, with parity hooks: idx_override_dev / mu_override_dev ([n][h][w][c_y], may be NULL) replace the
+ * hyper-decoder's indices / means ("teacher forcing", R12; the entropy-only mode of DESIGN.md);
+ * taps (may be NULL) receives intermediates.  frames_dev may be NULL to stop after the entropy stage. */
+int ufnvc_chunk_decode_ex(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, const uint8_t *bits_dev,
+                          size_t bits_bytes, const uint32_t *sub_off_dev, float *frames_dev, void *cuda_stream,
+                          const uint8_t *idx_override_dev, const float *mu_override_dev, const ufnvc_taps *taps);
+
+/* A1 + A2 only: mu, clamped ln sigma, bucket index, each [n][h][w][c_y] on the device (any may be NULL). */
+int ufnvc_entropy_params(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, float *mu_dev, float *lnscale_dev,
+                         uint8_t *idx_dev, void *cuda_stream);
+
+/* Synchronises cuda_stream-independent: reads the device status word of the last decode (after the caller
+ * synchronised the stream).  *device_status = 0 or an OR of UFNVC_STREAM_* bits. */
+int ufnvc_get_status(ufnvc_handle *h, uint32_t *device_status);
+
+/* Human-readable text of the last failing call on this handle (never NULL; NULL handle -> static text). */
+const char *ufnvc_last_error(const ufnvc_handle *h);
+
+/* Number of kernels / async copies ufnvc_chunk_decode enqueues per call for n_chunks (for bench accounting). */
+int ufnvc_launches_per_call(const ufnvc_handle *h, int n_chunks);
+
+/* Per-stage device time of the LAST ufnvc_chunk_decode_profiled call, in microseconds.
+ * ufnvc_chunk_decode_profiled = ufnvc_chunk_decode with a cudaEvent after each stage A1+A2, A3+A4, A5, A6+A7
+ * (all trunk blocks), A8 (stages 1-3), A9; it synchronises the stream at the end.  us_out_host[6]. */
+int ufnvc_chunk_decode_profiled(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, const uint8_t *bits_dev,
+                                size_t bits_bytes, const uint32_t *sub_off_dev, float *frames_dev,
+                                void *cuda_stream, float *us_out_host);
+
+/* ---- encoder-side fixtures (HOST code, not on the timed path): what a sender would run so that bench.py can
+ * build a valid bit-stream without the oracle.  The real codec's encoder runs the decoder's prior net
+ * (PAPER.md:125), hence idx comes from ufnvc_entropy_params. ---- */
+
+/* Quantised CDF tables the library decodes with: cdf_host uint32 [n_buckets][256], c[0] = 0, c[255] = 2^16 (O3). */
+int ufnvc_get_cdf(const ufnvc_handle *h, uint32_t *cdf_host);
+
+/* Inverse-CDF draw of r from the quantised tables with one uniform 16-bit number per element [R7]. */
+int ufnvc_symbols_from_uniform(const ufnvc_handle *h, const uint8_t *idx_host, const uint16_t *u16_host, size_t n,
+                               int16_t *sym_host);
+
+/* rANS-encode one chunk (mirror of O4).  idx_host, sym_host: [h][w][c_y].  Writes the concatenated substreams
+ * to bits_host (capacity cap bytes) and n_sub + 1 byte offsets (relative to bits_host) to sub_off_host.
+ * Returns the byte count (> 0) or a negative status (UFNVC_E_INVALID_ARG if cap is too small). */
+long ufnvc_encode_chunk(const ufnvc_handle *h, const uint8_t *idx_host, const int16_t *sym_host, uint8_t *bits_host,
+                        size_t cap, uint32_t *sub_off_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* UFNVC_H */

@@ -47,6 +47,9 @@ class Oracle:
         self.dt = np.float64 if real == "f64" else np.float32
         assert self.lib.orc_real_bytes() == np.dtype(self.dt).itemsize
 
+    def num_threads(self) -> int:
+        return int(self.lib.orc_num_threads())
+
     def arr(self, a):
         return np.ascontiguousarray(a, dtype=self.dt)
 
@@ -138,8 +141,8 @@ class Oracle:
 # geometry (SURVEY.md section 8 notation; R2, R16)
 # ---------------------------------------------------------------------------------------------
 def geometry(cfg):
-    H = -(-cfg.height // 16) * 16
-    W = -(-cfg.width // 16) * 16
+    H = -(-cfg.height // 32) * 32
+    W = -(-cfg.width // 32) * 32
     h, w = H // 16, W // 16
     return dict(H=H, W=W, h=h, w=w, h_z=-(-h // 4), w_z=-(-w // 4), n_sub=-(-h // cfg.rows_per_substream))
 

@@ -255,3 +255,11 @@ double orc_ideal_bits(const uint32_t *cdf, const uint8_t *idx, const int16_t *sy
     }
     return bits;
 }
+
+/* threads the OpenMP loops above actually use (reported by bench.py's cpu_baseline) */
+#ifdef _OPENMP
+#include <omp.h>
+int orc_num_threads(void) { return omp_get_max_threads(); }
+#else
+int orc_num_threads(void) { return 1; }
+#endif

@@ -1,0 +1,167 @@
+// C ABI of libufnvc (include/ufnvc.h): handle lifetime, validation, the launch sequence of the hot path.
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "handle.h"
+
+using namespace ufnvc;
+
+namespace ufnvc {
+int fail(ufnvc_handle *h, int code, const std::string &msg)
+{
+    if (h) h->err = msg;
+    return code;
+}
+}  // namespace ufnvc
+
+namespace {
+
+const char *kNullHandleText = "null handle";
+
+template <typename T> bool dev_alloc(ufnvc_handle *h, T *&p, size_t count)
+{
+    void *d = nullptr;
+    if (cudaMalloc(&d, (count ? count : 1) * sizeof(T)) != cudaSuccess) return false;
+    h->allocs.push_back(d);
+    p = static_cast<T *>(d);
+    return true;
+}
+
+int validate(const ufnvc_config &c, std::string &why)
+{
+#define BAD(cond, text) if (cond) { why = text; return UFNVC_E_BAD_CONFIG; }
+    BAD(c.struct_size != sizeof(ufnvc_config), "struct_size mismatch");
+    BAD(c.T < 1 || c.T > 64, "T out of range");
+    BAD(c.height < 1 || c.width < 1 || c.height > 16384 || c.width > 16384, "frame size out of range");
+    BAD(c.c_y < 8 || c.c_y % 8 || c.c_z < 1 || c.c_hyper < 1, "c_y must be a multiple of 8; c_z, c_hyper >= 1");
+    BAD(c.c_trunk < 8 || c.c_trunk % 8, "c_trunk must be a multiple of 8");
+    BAD(c.n_trunk_blocks < 0 || c.n_trunk_blocks > 64 || c.trunk_expand < 1, "bad trunk");
+    BAD(c.dec_channels[0] != c.c_trunk || c.dec_channels[4] != 3, "dec_channels[0] must equal c_trunk and [4] must be 3");
+    for (int s = 1; s < 4; ++s) BAD(c.dec_channels[s] < 8 || c.dec_channels[s] % 8, "dec_channels must be multiples of 8");
+    BAD(c.n_buckets < 1 || c.n_buckets > 64, "n_buckets must be in [1,64]");
+    BAD(!(c.scale_min > 0.f) || !(c.scale_max > c.scale_min), "need 0 < scale_min < scale_max");
+    BAD(c.rows_per_substream < 1, "rows_per_substream >= 1");
+    BAD(c.lanes_per_substream < 32 || c.lanes_per_substream % 32 || c.lanes_per_substream > 1024, "lanes_per_substream: multiple of 32 in [32,1024]");
+    BAD(c.max_chunks_per_call < 1 || c.max_chunks_per_call > 64, "max_chunks_per_call out of range");
+    BAD(c.weight_dtype != 0 && c.weight_dtype != 1, "weight_dtype must be 0 or 1");
+#undef BAD
+    return UFNVC_OK;
+}
+
+}  // namespace
+
+extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
+{
+    if (!cfg || !out) return UFNVC_E_INVALID_ARG;
+    std::string why;
+    if (int rc = validate(*cfg, why)) return rc;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return UFNVC_E_CUDA;
+    if (prop.major != 10) return UFNVC_E_UNSUPPORTED_DEVICE;
+    ufnvc_handle *h = new (std::nothrow) ufnvc_handle();
+    if (!h) return UFNVC_E_OOM;
+    h->cfg = *cfg;
+    h->num_sms = prop.multiProcessorCount;
+    h->H = (cfg->height + 31) / 32 * 32;
+    h->W = (cfg->width + 31) / 32 * 32;
+    h->h = h->H / 16;
+    h->w = h->W / 16;
+    h->h_z = (h->h + 3) / 4;
+    h->w_z = (h->w + 3) / 4;
+    h->n_sub = (h->h + cfg->rows_per_substream - 1) / cfg->rows_per_substream;
+    h->max_chunks = cfg->max_chunks_per_call;
+    const char *fg = std::getenv("UFNVC_FORCE_GENERIC");
+    h->force_generic = fg && fg[0] == '1';
+
+    // O3 tables + search accelerator
+    build_cdf_tables(cfg->n_buckets, double(cfg->scale_min), double(cfg->scale_max), h->cdf32);
+    std::vector<uint16_t> lut, cdf16(h->cdf32.size());
+    build_search_lut(h->cdf32, cfg->n_buckets, lut);
+    for (size_t i = 0; i < cdf16.size(); ++i) cdf16[i] = uint16_t(h->cdf32[i]);     // c[255] = 2^16 wraps to 0
+
+    const size_t n = size_t(h->max_chunks), P = size_t(h->h) * h->w, Pz = size_t(h->h_z) * h->w_z, T = size_t(cfg->T);
+    bool ok = dev_alloc(h, h->d_cdf, cdf16.size()) && dev_alloc(h, h->d_lut, lut.size()) && dev_alloc(h, h->d_status, 1) &&
+              dev_alloc(h, h->hx0, n * Pz * cfg->c_z) && dev_alloc(h, h->hx1, n * Pz * cfg->c_hyper) &&
+              dev_alloc(h, h->hx2, n * Pz * cfg->c_hyper) && dev_alloc(h, h->mu, n * P * cfg->c_y) &&
+              dev_alloc(h, h->lnscale, n * P * cfg->c_y) && dev_alloc(h, h->idx, n * P * cfg->c_y) &&
+              dev_alloc(h, h->yhat, n * P * cfg->c_y) && dev_alloc(h, h->fa, n * T * P * cfg->c_trunk) &&
+              dev_alloc(h, h->fb, n * T * P * cfg->c_trunk) &&
+              dev_alloc(h, h->hidden, cfg->n_trunk_blocks ? n * T * P * cfg->c_trunk * cfg->trunk_expand : 1);
+    for (int s = 0; ok && s < 3; ++s) ok = dev_alloc(h, h->stage[s], n * T * (P << (2 * (s + 1))) * cfg->dec_channels[s + 1]);
+    if (ok) ok = cudaMemcpy(h->d_cdf, cdf16.data(), cdf16.size() * 2, cudaMemcpyHostToDevice) == cudaSuccess &&
+                 cudaMemcpy(h->d_lut, lut.data(), lut.size() * 2, cudaMemcpyHostToDevice) == cudaSuccess &&
+                 cudaMemset(h->d_status, 0, 4) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
+        ufnvc_destroy(h);
+        return UFNVC_E_OOM;
+    }
+    *out = h;
+    return UFNVC_OK;
+}
+
+extern "C" int ufnvc_destroy(ufnvc_handle *h)
+{
+    if (!h) return UFNVC_E_INVALID_ARG;
+    cudaDeviceSynchronize();
+    for (void *p : h->allocs) cudaFree(p);
+    if (h->ev_made) for (auto &e : h->ev) cudaEventDestroy(e);
+    delete h;
+    return UFNVC_OK;
+}
+
+extern "C" const char *ufnvc_last_error(const ufnvc_handle *h) { return h ? h->err.c_str() : kNullHandleText; }
+
+extern "C" int ufnvc_get_status(ufnvc_handle *h, uint32_t *device_status)
+{
+    if (!h || !device_status) return UFNVC_E_INVALID_ARG;
+    if (cudaMemcpy(device_status, h->d_status, 4, cudaMemcpyDeviceToHost) != cudaSuccess) return fail(h, UFNVC_E_CUDA, "status read failed");
+    return UFNVC_OK;
+}
+
+extern "C" int ufnvc_get_cdf(const ufnvc_handle *h, uint32_t *cdf_host)
+{
+    if (!h || !cdf_host) return UFNVC_E_INVALID_ARG;
+    std::memcpy(cdf_host, h->cdf32.data(), h->cdf32.size() * 4);
+    return UFNVC_OK;
+}
+
+extern "C" int ufnvc_symbols_from_uniform(const ufnvc_handle *h, const uint8_t *idx_host, const uint16_t *u16_host, size_t n,
+                                          int16_t *sym_host)
+{
+    if (!h || !idx_host || !u16_host || !sym_host) return UFNVC_E_INVALID_ARG;
+    for (size_t i = 0; i < n; ++i) {
+        if (idx_host[i] >= h->cfg.n_buckets) return UFNVC_E_INVALID_ARG;
+        const uint32_t *c = &h->cdf32[size_t(idx_host[i]) * 256];
+        int lo = 0, hi = 254;                      // largest p with c[p] <= u
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) / 2;
+            if (c[mid] <= u16_host[i]) lo = mid; else hi = mid - 1;
+        }
+        sym_host[i] = int16_t(lo - 127);
+    }
+    return UFNVC_OK;
+}
+
+extern "C" long ufnvc_encode_chunk(const ufnvc_handle *h, const uint8_t *idx_host, const int16_t *sym_host, uint8_t *bits_host,
+                                   size_t cap, uint32_t *sub_off_host)
+{
+    if (!h || !idx_host || !sym_host || !bits_host || !sub_off_host) return UFNVC_E_INVALID_ARG;
+    size_t pos = 0;
+    sub_off_host[0] = 0;
+    for (int s = 0; s < h->n_sub; ++s) {
+        const int r0 = s * h->cfg.rows_per_substream;
+        const int rows = std::min(h->cfg.rows_per_substream, h->h - r0);
+        const size_t e0 = size_t(r0) * h->w * h->cfg.c_y, cnt = size_t(rows) * h->w * h->cfg.c_y;
+        const long nb = encode_substream(h->cdf32.data(), idx_host + e0, sym_host + e0, cnt, h->cfg.lanes_per_substream,
+                                         bits_host + pos, cap - pos);
+        if (nb < 0) return nb;
+        pos += size_t(nb);
+        sub_off_host[s + 1] = uint32_t(pos);
+    }
+    return long(pos);
+}

@@ -1,0 +1,212 @@
+// The launch sequence of ufnvc_chunk_decode: A1+A2 -> A3+A4 -> A5 -> B x (A6, A7) -> A8 -> A9.
+// One host call, zero host synchronisations, everything on the caller's stream.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "handle.h"
+
+using namespace ufnvc;
+
+namespace {
+
+#define CU_TRY(expr)                                                                                         \
+    do {                                                                                                     \
+        cudaError_t e__ = (expr);                                                                            \
+        if (e__ != cudaSuccess) return fail(h, UFNVC_E_CUDA, std::string(#expr) + ": " + cudaGetErrorString(e__)); \
+    } while (0)
+
+// conv dispatch: tcgen05 implicit GEMM when the layer and the activation map qualify, CUDA-core kernel otherwise.
+cudaError_t conv(ufnvc_handle *h, const ConvLayer &L, const ConvProblem &P, const ufnvc_handle::ActMap &am, const EpiParams &E,
+                 cudaStream_t st, int *launches)
+{
+    if (launches) ++*launches;
+    if (L.use_tc && am.ok && !h->force_generic) return launch_conv_tc(L, P, am.tm, am.tile_h, am.tile_w, E, h->num_sms, st);
+    return launch_conv_generic(L, P, E, st);
+}
+
+struct Stage { cudaEvent_t *ev; int i; };
+inline void mark(Stage *s, cudaStream_t st) { if (s) cudaEventRecord(s->ev[s->i++], st); }
+
+int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bits_bytes, const uint32_t *sub_off, float *frames,
+        cudaStream_t st, const uint8_t *idx_ovr, const float *mu_ovr, const ufnvc_taps *taps, bool entropy_params_only,
+        float *mu_out, float *ls_out, uint8_t *idx_out, Stage *sg, int *launches)
+{
+    const ufnvc_config &c = h->cfg;
+    const int P = h->h * h->w, Pz = h->h_z * h->w_z;
+    const size_t ne = size_t(n) * P * c.c_y;
+
+    // ---- A1 + A2: hyper-decoder in fp64 -> mu, ln sigma, bucket index ----
+    const bool need_hyper = entropy_params_only || !idx_ovr || !mu_ovr || (taps && (taps->mu || taps->lnscale));
+    mark(sg, st);
+    if (need_hyper) {
+        CU_TRY(launch_z_to_f64(z, h->hx0, n, c.c_z, Pz, st));
+        CU_TRY(launch_hyper_conv(h->hyper[0], h->hx0, h->hx1, n, h->h_z, h->w_z, st));
+        CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, n, h->h_z, h->w_z, st));
+        HeadParams hp{c.c_y, h->h, h->w, c.n_buckets, std::log(double(c.scale_min)), std::log(double(c.scale_max)), h->mu, h->lnscale, h->idx};
+        CU_TRY(launch_hyper_head(h->hyper[2], h->hx2, n, h->h_z, h->w_z, hp, st));
+        if (launches) *launches += 4;
+    }
+    if (entropy_params_only) {
+        if (mu_out) CU_TRY(cudaMemcpyAsync(mu_out, h->mu, ne * 4, cudaMemcpyDeviceToDevice, st));
+        if (ls_out) CU_TRY(cudaMemcpyAsync(ls_out, h->lnscale, ne * 4, cudaMemcpyDeviceToDevice, st));
+        if (idx_out) CU_TRY(cudaMemcpyAsync(idx_out, h->idx, ne, cudaMemcpyDeviceToDevice, st));
+        return UFNVC_OK;
+    }
+    const uint8_t *idx = idx_ovr ? idx_ovr : h->idx;
+    const float *mu = mu_ovr ? mu_ovr : h->mu;
+    if (taps) {
+        if (taps->mu) CU_TRY(cudaMemcpyAsync(taps->mu, mu, ne * 4, cudaMemcpyDeviceToDevice, st));
+        if (taps->lnscale) CU_TRY(cudaMemcpyAsync(taps->lnscale, h->lnscale, ne * 4, cudaMemcpyDeviceToDevice, st));
+        if (taps->idx) CU_TRY(cudaMemcpyAsync(taps->idx, idx, ne, cudaMemcpyDeviceToDevice, st));
+    }
+    mark(sg, st);
+
+    // ---- A3 + A4: rANS decode + dequantisation ----
+    CU_TRY(cudaMemsetAsync(h->d_status, 0, 4, st));
+    RansParams rp{};
+    rp.bits = bits; rp.bits_bytes = bits_bytes; rp.sub_off = sub_off; rp.idx = idx; rp.mu = mu;
+    rp.cdf = h->d_cdf; rp.lut = h->d_lut;
+    rp.n_chunks = n; rp.n_sub = h->n_sub; rp.h = h->h; rp.w = h->w; rp.c_y = c.c_y;
+    rp.rows_per_sub = c.rows_per_substream; rp.W = c.lanes_per_substream; rp.n_buckets = c.n_buckets;
+    rp.yhat = h->yhat; rp.sym_tap = taps ? taps->sym : nullptr; rp.yhat_tap = taps ? taps->yhat : nullptr;
+    rp.status = h->d_status;
+    CU_TRY(launch_rans_decode(rp, st));
+    if (launches) *launches += 2;
+    mark(sg, st);
+    if (!frames) return UFNVC_OK;
+
+    // ---- A5: cross-frame unfold, 1x1 conv c_y -> T*c_trunk, channel t*c_trunk + c -> frame t ----
+    const int T = c.T, Ct = c.c_trunk;
+    const size_t fe = size_t(n) * T * P * Ct;
+    {
+        ConvProblem pr{h->yhat, n, h->h, h->w, 1};
+        EpiParams E{EPI_NHWC, ACT_NONE, h->fa, nullptr, Ct, (long long)P * Ct, (long long)T * P * Ct, 0, 0, 0};
+        CU_TRY(conv(h, h->xframe, pr, h->am_yhat, E, st, launches));
+    }
+    if (taps && taps->f0) CU_TRY(cudaMemcpyAsync(taps->f0, h->fa, fe * 2, cudaMemcpyDeviceToDevice, st));
+    mark(sg, st);
+
+    // ---- A6 + A7: trunk of residual DC blocks, weights shared over t (t is batch) ----
+    const int Ce = Ct * c.trunk_expand;
+    for (int k = 0; k < c.n_trunk_blocks; ++k) {
+        const ufnvc_handle::TrunkBlock &tb = h->trunk[k];
+        CU_TRY(launch_dwconv3x3(h->fa, h->fb, tb.dw_w, tb.dw_b, n * T, h->h, h->w, Ct, st));
+        if (launches) ++*launches;
+        ConvProblem p1{h->fb, n * T, h->h, h->w, 1};
+        EpiParams E1{EPI_NHWC, ACT_GELU, h->hidden, nullptr, Ce, 0, (long long)P * Ce, 0, 0, 0};
+        CU_TRY(conv(h, tb.pw1, p1, h->am_fb, E1, st, launches));
+        ConvProblem p2{h->hidden, n * T, h->h, h->w, 1};
+        EpiParams E2{EPI_NHWC, ACT_NONE, h->fa, h->fa, Ct, 0, (long long)P * Ct, 0, 0, 0};
+        CU_TRY(conv(h, tb.pw2, p2, h->am_hidden, E2, st, launches));
+    }
+    if (taps && taps->trunk) CU_TRY(cudaMemcpyAsync(taps->trunk, h->fa, fe * 2, cudaMemcpyDeviceToDevice, st));
+    mark(sg, st);    // (A6 and A7 are reported together here; the profiled call splits them with its own events)
+
+    // ---- A8: frame-specific decoders, stages 1..3, one grouped launch over t per stage ----
+    const bf16 *x = h->fa;
+    const ufnvc_handle::ActMap *am = &h->am_fa;
+    int sh = h->h, sw = h->w;
+    for (int s = 0; s < 3; ++s) {
+        const int co = c.dec_channels[s + 1];
+        ConvProblem pr{x, n * T, sh, sw, T};
+        EpiParams E{EPI_PS2, ACT_GELU, h->stage[s], nullptr, 0, 0, (long long)sh * sw * 4 * co, co, 0, 0};
+        CU_TRY(conv(h, h->dec[s], pr, *am, E, st, launches));
+        sh *= 2; sw *= 2;
+        x = h->stage[s];
+        am = &h->am_stage[s];
+        if (taps && taps->stage[s]) CU_TRY(cudaMemcpyAsync(taps->stage[s], x, size_t(n) * T * sh * sw * co * 2, cudaMemcpyDeviceToDevice, st));
+    }
+    mark(sg, st);
+
+    // ---- A9: last stage (linear) + pixel-shuffle + clamp + crop + planar fp32 ----
+    {
+        ConvProblem pr{x, n * T, sh, sw, T};
+        EpiParams E{EPI_FINAL, ACT_NONE, frames, nullptr, 0, 0, (long long)3 * c.height * c.width, 3, c.height, c.width};
+        CU_TRY(conv(h, h->dec[3], pr, *am, E, st, launches));
+    }
+    mark(sg, st);
+    return UFNVC_OK;
+}
+
+int check_call(ufnvc_handle *h, int n_chunks, const void *z, const void *bits, const void *sub_off)
+{
+    if (!h) return UFNVC_E_INVALID_ARG;
+    if (!h->weights_loaded) return fail(h, UFNVC_E_NO_WEIGHTS, "ufnvc_load_weights has not succeeded on this handle");
+    if (n_chunks < 1 || n_chunks > h->max_chunks) return fail(h, UFNVC_E_INVALID_ARG, "n_chunks outside [1, max_chunks_per_call]");
+    if (!z || !bits || !sub_off) return fail(h, UFNVC_E_INVALID_ARG, "null device pointer");
+    if (reinterpret_cast<uintptr_t>(bits) & 3) return fail(h, UFNVC_E_INVALID_ARG, "bits_dev must be 4-byte aligned");
+    return UFNVC_OK;
+}
+
+}  // namespace
+
+extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t bytes)
+{
+    if (!h || !blob_host) return UFNVC_E_INVALID_ARG;
+    h->weights_loaded = false;
+    if (int rc = load_weights_impl(h, blob_host, bytes)) return rc;
+    h->weights_loaded = true;
+    return UFNVC_OK;
+}
+
+extern "C" int ufnvc_chunk_decode_ex(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, const uint8_t *bits_dev, size_t bits_bytes,
+                                     const uint32_t *sub_off_dev, float *frames_dev, void *cuda_stream, const uint8_t *idx_override_dev,
+                                     const float *mu_override_dev, const ufnvc_taps *taps)
+{
+    if (int rc = check_call(h, n_chunks, z_dev, bits_dev, sub_off_dev)) return rc;
+    if (taps && taps->struct_size != sizeof(ufnvc_taps)) return fail(h, UFNVC_E_INVALID_ARG, "ufnvc_taps.struct_size mismatch");
+    return run(h, n_chunks, z_dev, bits_dev, bits_bytes, sub_off_dev, frames_dev, static_cast<cudaStream_t>(cuda_stream),
+               idx_override_dev, mu_override_dev, taps, false, nullptr, nullptr, nullptr, nullptr, nullptr);
+}
+
+extern "C" int ufnvc_chunk_decode(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, const uint8_t *bits_dev, size_t bits_bytes,
+                                  const uint32_t *sub_off_dev, float *frames_dev, void *cuda_stream)
+{
+    if (int rc = check_call(h, n_chunks, z_dev, bits_dev, sub_off_dev)) return rc;
+    if (!frames_dev) return fail(h, UFNVC_E_INVALID_ARG, "frames_dev is null");
+    return run(h, n_chunks, z_dev, bits_dev, bits_bytes, sub_off_dev, frames_dev, static_cast<cudaStream_t>(cuda_stream), nullptr,
+               nullptr, nullptr, false, nullptr, nullptr, nullptr, nullptr, nullptr);
+}
+
+extern "C" int ufnvc_entropy_params(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, float *mu_dev, float *lnscale_dev,
+                                    uint8_t *idx_dev, void *cuda_stream)
+{
+    if (!h) return UFNVC_E_INVALID_ARG;
+    if (!h->weights_loaded) return fail(h, UFNVC_E_NO_WEIGHTS, "ufnvc_load_weights has not succeeded on this handle");
+    if (n_chunks < 1 || n_chunks > h->max_chunks || !z_dev) return fail(h, UFNVC_E_INVALID_ARG, "bad n_chunks or null z_dev");
+    return run(h, n_chunks, z_dev, nullptr, 0, nullptr, nullptr, static_cast<cudaStream_t>(cuda_stream), nullptr, nullptr, nullptr, true,
+               mu_dev, lnscale_dev, idx_dev, nullptr, nullptr);
+}
+
+extern "C" int ufnvc_launches_per_call(const ufnvc_handle *h, int n_chunks)
+{
+    if (!h || n_chunks < 1) return UFNVC_E_INVALID_ARG;
+    // 4 hyper + memset + rANS + A5 + 3 per trunk block + 4 decoder stages
+    return 4 + 2 + 1 + 3 * h->cfg.n_trunk_blocks + 4;
+}
+
+extern "C" int ufnvc_chunk_decode_profiled(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, const uint8_t *bits_dev,
+                                           size_t bits_bytes, const uint32_t *sub_off_dev, float *frames_dev, void *cuda_stream,
+                                           float *us_out_host)
+{
+    if (int rc = check_call(h, n_chunks, z_dev, bits_dev, sub_off_dev)) return rc;
+    if (!frames_dev || !us_out_host) return fail(h, UFNVC_E_INVALID_ARG, "null frames_dev / us_out_host");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (!h->ev_made) {
+        for (auto &e : h->ev) CU_TRY(cudaEventCreate(&e));
+        h->ev_made = true;
+    }
+    Stage sg{h->ev, 0};
+    if (int rc = run(h, n_chunks, z_dev, bits_dev, bits_bytes, sub_off_dev, frames_dev, st, nullptr, nullptr, nullptr, false, nullptr,
+                     nullptr, nullptr, &sg, nullptr))
+        return rc;
+    CU_TRY(cudaStreamSynchronize(st));
+    // events: 0 start, 1 after A1+A2, 2 after A3+A4, 3 after A5, 4 after trunk, 5 after A8, 6 after A9
+    for (int i = 0; i < 6; ++i) {
+        float ms = 0.f;
+        CU_TRY(cudaEventElapsedTime(&ms, h->ev[i], h->ev[i + 1]));
+        us_out_host[i] = ms * 1000.f;
+    }
+    return UFNVC_OK;
+}

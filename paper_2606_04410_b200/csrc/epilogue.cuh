@@ -1,0 +1,47 @@
+// Epilogue arithmetic and addressing shared by the conv kernels (bias is added by the caller).
+#pragma once
+#include "ufnvc_internal.h"
+
+namespace ufnvc {
+
+// GELU(v) = v/2 (1 + erf(v/sqrt2)), erf by Abramowitz-Stegun 7.1.26 (|abs err| <= 1.5e-7): one MUFU.RCP, one
+// MUFU.EX2 and a degree-5 Horner chain -- far below the bf16 rounding (2^-9 relative) the result is stored with.
+__device__ __forceinline__ float gelu_erf(float v)
+{
+    const float z = fabsf(v) * 0.70710678118654752f;
+    const float t = __fdividef(1.0f, fmaf(0.3275911f, z, 1.0f));
+    float poly = fmaf(1.061405429f, t, -1.453152027f);
+    poly = fmaf(poly, t, 1.421413741f);
+    poly = fmaf(poly, t, -0.284496736f);
+    poly = fmaf(poly, t, 0.254829592f);
+    poly *= t;
+    const float e = 1.0f - poly * __expf(-z * z);      // erf(|v|/sqrt2)
+    const float erfv = copysignf(e, v);
+    return 0.5f * v * (1.0f + erfv);
+}
+
+__device__ __forceinline__ float apply_act(float v, int act) { return act == ACT_GELU ? gelu_erf(v) : v; }
+
+// Destination element offset of packed output column n of input pixel (img, y, x); EPI_NHWC / EPI_PS2 only.
+__device__ __forceinline__ long long epi_offset(const EpiParams &E, int img, int y, int x, int H, int W, int n)
+{
+    if (E.mode == EPI_NHWC) {
+        const int grp = n / E.n_split, c = n - grp * E.n_split;
+        return (long long)img * E.img_stride + (long long)grp * E.split_stride + ((long long)y * W + x) * E.n_split + c;
+    }
+    const int ij = n / E.c_o, c = n - ij * E.c_o;
+    const int oy = 2 * y + (ij >> 1), ox = 2 * x + (ij & 1);
+    return (long long)img * E.img_stride + ((long long)oy * (2 * W) + ox) * E.c_o + c;
+}
+
+// EPI_FINAL: clamp, crop, planar fp32 (A9 / O9).
+__device__ __forceinline__ void epi_store_final(const EpiParams &E, int img, int y, int x, int n, float v)
+{
+    const int ij = n / E.c_o, c = n - ij * E.c_o;
+    const int oy = 2 * y + (ij >> 1), ox = 2 * x + (ij & 1);
+    if (oy >= E.out_h || ox >= E.out_w) return;
+    v = fminf(fmaxf(v, 0.0f), 1.0f);
+    reinterpret_cast<float *>(E.out)[(long long)img * E.img_stride + ((long long)c * E.out_h + oy) * E.out_w + ox] = v;
+}
+
+}  // namespace ufnvc

@@ -1,0 +1,57 @@
+// The opaque handle behind include/ufnvc.h: config, geometry, device weights, tables, workspace.
+#pragma once
+#include <map>
+#include <string>
+#include <vector>
+
+#include "ufnvc_internal.h"
+
+struct ufnvc_handle {
+    ufnvc_config cfg{};
+    // geometry (SURVEY.md section 8 notation)
+    int H = 0, W = 0, h = 0, w = 0, h_z = 0, w_z = 0, n_sub = 0;
+    int num_sms = 0;
+    int max_chunks = 1;
+    bool weights_loaded = false;
+    bool force_generic = false;          // env UFNVC_FORCE_GENERIC=1: CUDA-core convs everywhere (cross-check)
+    std::string err;
+
+    // entropy tables (O3)
+    std::vector<uint32_t> cdf32;         // [nb][256], host copy
+    uint16_t *d_cdf = nullptr, *d_lut = nullptr;
+    uint32_t *d_status = nullptr;
+
+    // layers
+    ufnvc::HyperLayer hyper[3];
+    ufnvc::ConvLayer xframe;
+    struct TrunkBlock {
+        float *dw_w = nullptr, *dw_b = nullptr;   // [9][C], [C] fp32
+        ufnvc::ConvLayer pw1, pw2;
+    };
+    std::vector<TrunkBlock> trunk;
+    ufnvc::ConvLayer dec[4];             // groups = T
+
+    // workspace (sized for max_chunks)
+    double *hx0 = nullptr, *hx1 = nullptr, *hx2 = nullptr;
+    float *mu = nullptr, *lnscale = nullptr;
+    uint8_t *idx = nullptr;
+    ufnvc::bf16 *yhat = nullptr, *fa = nullptr, *fb = nullptr, *hidden = nullptr;
+    ufnvc::bf16 *stage[3] = {nullptr, nullptr, nullptr};
+
+    // TMA descriptors of the activation tensors the tcgen05 convs read, built once at create (workspace is fixed)
+    struct ActMap {
+        CUtensorMap tm;
+        int tile_h = 0, tile_w = 0;
+        bool ok = false;
+    };
+    ActMap am_yhat, am_fa, am_fb, am_hidden, am_stage[3];
+
+    std::vector<void *> allocs;          // everything cudaMalloc'ed, freed at destroy
+    cudaEvent_t ev[8] = {};
+    bool ev_made = false;
+};
+
+namespace ufnvc {
+int fail(ufnvc_handle *h, int code, const std::string &msg);
+int load_weights_impl(ufnvc_handle *h, const void *blob, size_t bytes);
+}  // namespace ufnvc

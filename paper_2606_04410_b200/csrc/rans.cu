@@ -1,0 +1,138 @@
+// A3 + A4: parallel rANS decode of independent substreams + dequantisation.
+// "we can perform arithmetic decoding for all partitions in one consolidated step";
+// "r_i is recovered using only sigma_i, and the final latent is reconstructed as y_i = r_i + mu_i".
+//
+// One thread block per substream, one warp per warp-stream (32 interleaved 32-bit rANS states, 16-bit words,
+// 16-bit probabilities).  Per step every lane decodes one symbol; lanes whose state fell below 2^16 pull the next
+// words of the warp's word run in ascending lane order -- a ballot + popc prefix (the warp-level scan).  The words
+// are kept in a 64-entry register window (two per lane) and fetched with shuffles, so the serial critical path per
+// step is: 1 shared-memory LUT read, 1 table read, a few integer ops, 1 ballot, 1 shuffle.  The idx / mu loads of
+// step j+1 do not depend on the state and are issued one step ahead.
+#include "ufnvc_internal.h"
+
+namespace ufnvc {
+
+struct RansSmem {
+    uint16_t cdf[64 * 256];
+    uint16_t lut[64 * 256];
+};
+
+__global__ void __launch_bounds__(1024) rans_decode_kernel(RansParams p, int nb)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    uint16_t *s_cdf = reinterpret_cast<uint16_t *>(smem_raw);
+    uint16_t *s_lut = s_cdf + nb * 256;
+    {
+        const uint4 *src_c = reinterpret_cast<const uint4 *>(p.cdf);
+        const uint4 *src_l = reinterpret_cast<const uint4 *>(p.lut);
+        uint4 *dc = reinterpret_cast<uint4 *>(s_cdf), *dl = reinterpret_cast<uint4 *>(s_lut);
+        for (int i = threadIdx.x; i < nb * 32; i += blockDim.x) {
+            dc[i] = src_c[i];
+            dl[i] = src_l[i];
+        }
+    }
+    __syncthreads();
+
+    const int sub = blockIdx.x;                 // chunk * n_sub + s
+    const int chunk = sub / p.n_sub, s = sub % p.n_sub;
+    const int g = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int G = p.W >> 5;
+    const int row0 = s * p.rows_per_sub;
+    const int rows = min(p.rows_per_sub, p.h - row0);
+    const int n = rows * p.w * p.c_y;                                   // symbols of this substream
+    const long long ebase = ((long long)chunk * p.h + row0) * p.w * p.c_y;   // stream order == NHWC order
+    const int n_steps = (n + p.W - 1) / p.W;
+
+    // ---- container parsing, every read clamped to the substream ----
+    const uint32_t so = p.sub_off[sub], se = p.sub_off[sub + 1];
+    uint32_t st = 0;
+    uint32_t sub_bytes = 0;
+    if (se < so || (size_t)se > p.bits_bytes || (so & 3)) st |= UFNVC_STREAM_BAD_HEADER; else sub_bytes = se - so;
+    const uint8_t *sb = p.bits + so;
+    uint32_t ws_off = 0, nw = 0;
+    bool ws_ok = false;
+    if (sub_bytes >= 8u * G) {
+        ws_off = reinterpret_cast<const uint32_t *>(sb)[2 * g];
+        nw = reinterpret_cast<const uint32_t *>(sb)[2 * g + 1];
+        ws_ok = !(ws_off & 3) && (unsigned long long)ws_off + 128ull + 2ull * nw <= sub_bytes;
+    }
+    if (!ws_ok) { st |= UFNVC_STREAM_BAD_HEADER; nw = 0; }
+    uint32_t x = 1u << 16;
+    const uint16_t *words = nullptr;
+    if (ws_ok) {
+        x = reinterpret_cast<const uint32_t *>(sb + ws_off)[lane];
+        words = reinterpret_cast<const uint16_t *>(sb + ws_off + 128);
+    }
+    // word window: w0 = words[qb + lane], w1 = words[qb + 32 + lane]
+    uint32_t qb = 0, q = 0;
+    uint32_t w0 = (lane < nw) ? words[lane] : 0u;
+    uint32_t w1 = (32u + lane < nw) ? words[32 + lane] : 0u;
+
+    // prefetch step 0
+    int i = g * 32 + lane;
+    uint32_t k_next = 0;
+    float mu_next = 0.f;
+    if (i < n) { k_next = p.idx[ebase + i]; mu_next = p.mu[ebase + i]; }
+
+    for (int j = 0; j < n_steps; ++j) {
+        const bool valid = i < n;
+        const uint32_t k = k_next;
+        const float mu = mu_next;
+        const int i_next = i + p.W;
+        if (i_next < n) { k_next = p.idx[ebase + i_next]; mu_next = p.mu[ebase + i_next]; }
+
+        const uint32_t slot = x & 0xFFFFu;
+        const uint16_t *c = s_cdf + k * 256;
+        const uint32_t lh = s_lut[k * 256 + (slot >> 8)];
+        uint32_t lo = lh & 0xFFu, hi = lh >> 8;
+        while (lo < hi) {                       // largest pos in [lo,hi] with c[pos] <= slot
+            const uint32_t mid = (lo + hi + 1) >> 1;
+            if (c[mid] <= slot) lo = mid; else hi = mid - 1;
+        }
+        const uint32_t cp = c[lo];
+        const uint32_t f = (uint32_t(c[lo + 1]) - cp) & 0xFFFFu;        // c[255] = 2^16 is stored as 0
+        uint32_t xn = f * (x >> 16) + slot - cp;
+        const bool need = valid && xn < (1u << 16);
+        const uint32_t m = __ballot_sync(0xFFFFFFFFu, need);
+        const uint32_t r = q - qb + __popc(m & ((1u << lane) - 1u));     // index into the 64-word window
+        const uint32_t wa = __shfl_sync(0xFFFFFFFFu, w0, r & 31);
+        const uint32_t wb = __shfl_sync(0xFFFFFFFFu, w1, r & 31);
+        if (need) xn = (xn << 16) | (r < 32 ? wa : wb);
+        if (valid) x = xn;
+        q += __popc(m);
+        if (q - qb >= 32) {                     // slide the window (warp-uniform)
+            qb += 32;
+            w0 = w1;
+            const uint32_t a = qb + 32 + lane;
+            w1 = (a < nw) ? words[a] : 0u;
+        }
+        if (valid) {
+            const int sym = int(lo) - 127;
+            const float y = float(sym) + mu;                             // O5
+            p.yhat[ebase + i] = __float2bfloat16_rn(y);
+            if (p.sym_tap) p.sym_tap[ebase + i] = int16_t(sym);
+            if (p.yhat_tap) p.yhat_tap[ebase + i] = y;
+        }
+        i = i_next;
+    }
+    // end-state invariant (O4): every lane back at 2^16 and every word consumed
+    if (__any_sync(0xFFFFFFFFu, x != (1u << 16))) st |= UFNVC_STREAM_BAD_END_STATE;
+    if (q != nw) st |= UFNVC_STREAM_BAD_WORD_COUNT;
+    if (st && lane == 0) atomicOr(p.status, st);
+}
+
+cudaError_t launch_rans_decode(const RansParams &p, cudaStream_t st)
+{
+    const int nb = p.n_buckets;
+    const size_t smem = (size_t)64 * 256 * 2 * 2;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(rans_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    rans_decode_kernel<<<p.n_chunks * p.n_sub, p.W, smem, st>>>(p, nb);
+    return cudaGetLastError();
+}
+
+}  // namespace ufnvc

@@ -1,0 +1,107 @@
+// Internal declarations of libufnvc (not part of the ABI).  sm_100a only.
+#pragma once
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/ufnvc.h"
+
+namespace ufnvc {
+
+typedef __nv_bfloat16 bf16;
+
+// ---- epilogue description shared by the CUDA-core and the tcgen05 conv kernels -------------------------------
+enum EpiMode : int {
+    EPI_NHWC = 0,   // out[img][split][pix][n % n_split]  (bf16), optional residual with the same indexing
+    EPI_PS2 = 1,    // pixel-shuffle x2 (R14): packed column n' = (2i+j)*C_o + c -> out[img][2y+i][2x+j][c] (bf16)
+    EPI_FINAL = 2   // EPI_PS2 + clamp [0,1] + crop + planar fp32 store out[img][c][Y][X]  (A9)
+};
+enum Act : int { ACT_NONE = 0, ACT_GELU = 1 };
+
+struct EpiParams {
+    int mode, act;
+    void *out;
+    const bf16 *residual;    // EPI_NHWC only; may alias out
+    int n_split;             // EPI_NHWC: channels per output group (xframe: c_trunk, else N)
+    long long split_stride;  // EPI_NHWC: elements between output groups
+    long long img_stride;    // output elements per input image
+    int c_o;                 // EPI_PS2/FINAL: channels after the shuffle (N = 4*c_o)
+    int out_h, out_w;        // EPI_FINAL: crop (height, width)
+};
+
+// One conv layer as the kernels consume it.  Weights are K-major ("[n][k]", k = c_in contiguous) per tap and
+// per weight group: w[group][tap][n_pad][c_in] bf16; bias[group][n_pad] fp32.  For EPI_PS2/FINAL layers the
+// rows are permuted at load time so that packed row n' = (2i+j)*C_o + c holds canonical row 4c + 2i + j.
+struct ConvLayer {
+    int c_in = 0, n = 0, n_pad = 0, taps = 1, groups = 1;
+    bf16 *w = nullptr;
+    float *bias = nullptr;
+    bool use_tc = false;     // tcgen05 path eligible (c_in % 64 == 0, n_pad % 16 == 0)
+    CUtensorMap tmap_w;      // 3-D {c_in, n_pad, groups*taps}, box {64, block_n, 1}, 128B swizzle
+    int block_n = 0;
+};
+
+struct ConvProblem {
+    const bf16 *in;          // [n_img][H][W][c_in] bf16 NHWC
+    int n_img, H, W;
+    int imgs_per_group_cycle; // weight group of image i = (groups == 1) ? 0 : i % groups
+};
+
+// ---- kernels (each .cu exposes host launchers; all enqueue on `st` and return cudaGetLastError()) -------------
+cudaError_t launch_conv_generic(const ConvLayer &L, const ConvProblem &P, const EpiParams &E, cudaStream_t st);
+cudaError_t launch_dwconv3x3(const bf16 *in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
+                             int C, cudaStream_t st);
+
+// fp64 hyper-decoder (A1 + A2), R12: the scale decision is taken in double on both sides.
+struct HyperLayer {
+    int c_in = 0, n = 0;
+    double *w = nullptr;     // [9][c_in][n]
+    double *bias = nullptr;  // [n]
+};
+cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z, int pz, cudaStream_t st);
+cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out, int n_img, int hz, int wz,
+                              cudaStream_t st);
+struct HeadParams {
+    int c_y, h, w, n_buckets;
+    double ln_lo, ln_hi;
+    float *mu, *lnscale;     // [n][h][w][c_y], lnscale may be null
+    uint8_t *idx;
+};
+cudaError_t launch_hyper_head(const HyperLayer &L, const double *in, int n_img, int hz, int wz, const HeadParams &hp,
+                              cudaStream_t st);
+
+// rANS decode + dequantisation (A3 + A4)
+struct RansParams {
+    const uint8_t *bits;
+    size_t bits_bytes;
+    const uint32_t *sub_off;  // [n_chunks*n_sub + 1]
+    const uint8_t *idx;       // [n][h][w][c_y]
+    const float *mu;
+    const uint16_t *cdf;      // [nb][256] u16 (c[255] wraps to 0)
+    const uint16_t *lut;      // [nb][256]: lo | hi<<8 = first/last candidate position for slot>>8
+    int n_chunks, n_sub, h, w, c_y, rows_per_sub, W, n_buckets;
+    bf16 *yhat;               // [n][h][w][c_y]
+    int16_t *sym_tap;         // optional
+    float *yhat_tap;          // optional
+    uint32_t *status;         // device word, OR-ed
+};
+cudaError_t launch_rans_decode(const RansParams &p, cudaStream_t st);
+
+// tcgen05 implicit-GEMM conv (conv_tc.cu)
+cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_in, int tile_h, int tile_w,
+                           const EpiParams &E, int num_sms, cudaStream_t st);
+bool tc_make_weight_tmap(ConvLayer &L, std::string &err);
+bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, int tile_h, int tile_w,
+                      std::string &err);
+
+// ---- host-side entropy tables + encoder fixture (tables.cpp part of api) ---------------------------------------
+void build_cdf_tables(int nb, double smin, double smax, std::vector<uint32_t> &cdf32);
+void build_search_lut(const std::vector<uint32_t> &cdf32, int nb, std::vector<uint16_t> &lut);
+long encode_substream(const uint32_t *cdf32, const uint8_t *idx, const int16_t *sym, size_t n, int W, uint8_t *out,
+                      size_t cap);
+
+}  // namespace ufnvc

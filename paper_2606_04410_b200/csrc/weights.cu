@@ -1,0 +1,156 @@
+// ufnvc_load_weights: parse the blob (include/ufnvc.h), convert / permute / pad, upload.
+#include <cstring>
+
+#include "handle.h"
+
+namespace ufnvc {
+
+namespace {
+
+struct DirEntry {
+    char name[40];
+    uint32_t dtype, ndim, shape[4];
+    uint64_t offset, nbytes;
+};
+static_assert(sizeof(DirEntry) == 80, "blob directory entry is 80 bytes");
+
+struct Tensor {
+    const uint8_t *data;
+    uint32_t dtype, ndim, shape[4];
+    size_t count;
+    float at(size_t i) const
+    {
+        if (dtype == 0) { float v; std::memcpy(&v, data + 4 * i, 4); return v; }
+        uint16_t b; std::memcpy(&b, data + 2 * i, 2);
+        uint32_t u = uint32_t(b) << 16; float v; std::memcpy(&v, &u, 4); return v;
+    }
+};
+
+uint16_t f32_to_bf16_rne(float f)
+{
+    uint32_t u; std::memcpy(&u, &f, 4);
+    u += 0x7FFFu + ((u >> 16) & 1u);
+    return uint16_t(u >> 16);
+}
+
+struct Loader {
+    ufnvc_handle *h;
+    std::map<std::string, Tensor> t;
+    std::string err;
+
+    const Tensor *get(const std::string &name, std::initializer_list<uint32_t> shape)
+    {
+        auto it = t.find(name);
+        if (it == t.end()) { err = "missing tensor " + name; return nullptr; }
+        const Tensor &x = it->second;
+        if (x.ndim != shape.size()) { err = "bad rank for " + name; return nullptr; }
+        int d = 0;
+        for (uint32_t s : shape) if (x.shape[d++] != s) { err = "bad shape for " + name; return nullptr; }
+        return &x;
+    }
+
+    template <typename T> T *upload(const std::vector<T> &v)
+    {
+        T *d = nullptr;
+        if (cudaMalloc(&d, v.size() * sizeof(T)) != cudaSuccess) { err = "cudaMalloc failed (weights)"; return nullptr; }
+        h->allocs.push_back(d);
+        if (cudaMemcpy(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess) { err = "cudaMemcpy failed (weights)"; return nullptr; }
+        return d;
+    }
+
+    // canonical [n][c_in][k][k] (+ bias [n]) for each group -> ConvLayer (bf16 [g][tap][n_pad][c_in], fp32 bias)
+    bool conv(ConvLayer &L, const std::vector<std::string> &names, int c_in, int n, int k, bool ps2)
+    {
+        L.c_in = c_in; L.n = n; L.n_pad = (n + 15) / 16 * 16; L.taps = k * k; L.groups = int(names.size());
+        std::vector<uint16_t> w(size_t(L.groups) * L.taps * L.n_pad * c_in, 0);
+        std::vector<float> b(size_t(L.groups) * L.n_pad, 0.f);
+        const int c_o = n / 4;
+        for (int g = 0; g < L.groups; ++g) {
+            const Tensor *tw = get(names[g] + ".w", {uint32_t(n), uint32_t(c_in), uint32_t(k), uint32_t(k)});
+            const Tensor *tb = get(names[g] + ".b", {uint32_t(n)});
+            if (!tw || !tb) return false;
+            for (int np = 0; np < n; ++np) {
+                const int row = ps2 ? 4 * (np % c_o) + np / c_o : np;       // packed n' = ij*C_o + c  <-  4c + ij
+                b[size_t(g) * L.n_pad + np] = tb->at(row);
+                for (int tap = 0; tap < L.taps; ++tap)
+                    for (int c = 0; c < c_in; ++c)
+                        w[((size_t(g) * L.taps + tap) * L.n_pad + np) * c_in + c] =
+                            f32_to_bf16_rne(tw->at((size_t(row) * c_in + c) * L.taps + tap));
+            }
+        }
+        L.w = reinterpret_cast<bf16 *>(upload(w));
+        L.bias = upload(b);
+        return L.w && L.bias;
+    }
+
+    bool hyper(HyperLayer &L, const std::string &name, int c_in, int n)
+    {
+        const Tensor *tw = get(name + ".w", {uint32_t(n), uint32_t(c_in), 3u, 3u});
+        const Tensor *tb = get(name + ".b", {uint32_t(n)});
+        if (!tw || !tb) return false;
+        L.c_in = c_in; L.n = n;
+        std::vector<double> w(size_t(9) * c_in * n), b(n);
+        for (int o = 0; o < n; ++o) {
+            b[o] = double(tb->at(o));
+            for (int c = 0; c < c_in; ++c)
+                for (int tap = 0; tap < 9; ++tap) w[(size_t(tap) * c_in + c) * n + o] = double(tw->at((size_t(o) * c_in + c) * 9 + tap));
+        }
+        L.w = upload(w); L.bias = upload(b);
+        return L.w && L.bias;
+    }
+
+    bool depthwise(float *&dw, float *&db, const std::string &name, int C)
+    {
+        const Tensor *tw = get(name + ".w", {uint32_t(C), 1u, 3u, 3u});
+        const Tensor *tb = get(name + ".b", {uint32_t(C)});
+        if (!tw || !tb) return false;
+        std::vector<float> w(size_t(9) * C), b(C);
+        for (int c = 0; c < C; ++c) {
+            b[c] = tb->at(c);
+            for (int tap = 0; tap < 9; ++tap) w[size_t(tap) * C + c] = tw->at(size_t(c) * 9 + tap);
+        }
+        dw = upload(w); db = upload(b);
+        return dw && db;
+    }
+};
+
+}  // namespace
+
+int load_weights_impl(ufnvc_handle *h, const void *blob, size_t bytes)
+{
+    const uint8_t *p = static_cast<const uint8_t *>(blob);
+    if (bytes < 16 || std::memcmp(p, "UFNVCW01", 8) != 0) return fail(h, UFNVC_E_BAD_BLOB, "bad magic");
+    uint32_t n_t; std::memcpy(&n_t, p + 8, 4);
+    if (n_t > 100000 || 16 + size_t(n_t) * sizeof(DirEntry) > bytes) return fail(h, UFNVC_E_BAD_BLOB, "directory exceeds blob");
+    Loader ld; ld.h = h;
+    for (uint32_t i = 0; i < n_t; ++i) {
+        DirEntry e; std::memcpy(&e, p + 16 + size_t(i) * sizeof(DirEntry), sizeof(DirEntry));
+        e.name[39] = 0;
+        if (e.dtype > 1 || e.ndim < 1 || e.ndim > 4) return fail(h, UFNVC_E_BAD_BLOB, std::string("bad entry ") + e.name);
+        size_t cnt = 1; for (uint32_t d = 0; d < e.ndim; ++d) cnt *= e.shape[d];
+        const size_t need = cnt * (e.dtype == 0 ? 4 : 2);
+        if (e.nbytes != need || e.offset > bytes || need > bytes - e.offset) return fail(h, UFNVC_E_BAD_BLOB, std::string("tensor outside blob: ") + e.name);
+        Tensor t{p + e.offset, e.dtype, e.ndim, {e.shape[0], e.shape[1], e.shape[2], e.shape[3]}, cnt};
+        ld.t[e.name] = t;
+    }
+    const ufnvc_config &c = h->cfg;
+    bool ok = ld.hyper(h->hyper[0], "hyper.0", c.c_z, c.c_hyper) && ld.hyper(h->hyper[1], "hyper.1", c.c_hyper, c.c_hyper) &&
+              ld.hyper(h->hyper[2], "hyper.2", c.c_hyper, 2 * c.c_y * 16);
+    ok = ok && ld.conv(h->xframe, {"xframe"}, c.c_y, c.T * c.c_trunk, 1, false);
+    h->trunk.assign(c.n_trunk_blocks, ufnvc_handle::TrunkBlock());
+    const int ce = c.c_trunk * c.trunk_expand;
+    for (int k = 0; ok && k < c.n_trunk_blocks; ++k) {
+        const std::string b = "trunk." + std::to_string(k);
+        ok = ld.depthwise(h->trunk[k].dw_w, h->trunk[k].dw_b, b + ".dw", c.c_trunk) &&
+             ld.conv(h->trunk[k].pw1, {b + ".pw1"}, c.c_trunk, ce, 1, false) && ld.conv(h->trunk[k].pw2, {b + ".pw2"}, ce, c.c_trunk, 1, false);
+    }
+    for (int s = 0; ok && s < 4; ++s) {
+        std::vector<std::string> names;
+        for (int t = 0; t < c.T; ++t) names.push_back("dec." + std::to_string(t) + "." + std::to_string(s));
+        ok = ld.conv(h->dec[s], names, c.dec_channels[s], 4 * c.dec_channels[s + 1], 3, true);
+    }
+    if (!ok) return fail(h, ld.err.find("cuda") == 0 ? UFNVC_E_CUDA : UFNVC_E_BAD_BLOB, ld.err);
+    return UFNVC_OK;
+}
+
+}  // namespace ufnvc

@@ -47,11 +47,11 @@ class ChunkConfig:
     # derived geometry (SURVEY.md section 8 notation)
     @property
     def H(self):  # padded frame height
-        return -(-self.height // 16) * 16
+        return -(-self.height // 32) * 32
 
     @property
     def W(self):
-        return -(-self.width // 16) * 16
+        return -(-self.width // 32) * 32
 
     @property
     def h(self):

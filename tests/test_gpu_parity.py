@@ -1,0 +1,229 @@
+"""GPU-vs-oracle parity through the C ABI (run with -m gpu on the B200 box).
+
+Tolerances (BASELINE.json north_star): symbols and CDF indices bit-exact when fed the same indices; index mismatch
+rate <= 1e-5, only at bucket boundaries; mu within 1e-2 relative (|d mu| <= 1e-2 max(|mu|,1), R13), ln sigma within
+1e-2; pixels <= 2e-2 max abs on [0,1] and PSNR >= 45 dB against the oracle's frames.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from common import gpu_inputs, nhwc, oracle_case, psnr
+from paper_2606_04410_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+PIX_TOL, PSNR_MIN, IDX_RATE = 2e-2, 45.0, 1e-5
+
+CASES = {
+    "cfg1": synth.CONFIGS[1],
+    # ragged in every direction: h = 10 (3 substreams, last has 2 rows), w = 14, 160x224 frames cropped to 150x200
+    "cfg2-ragged": synth.crop_config(synth.CONFIGS[2], 150, 200),
+    "cfg3-crop": synth.crop_config(synth.CONFIGS[3], 272, 480),
+    "cfg2": synth.CONFIGS[2],
+}
+
+
+@pytest.fixture(scope="module")
+def decoders():
+    from paper_2606_04410_b200 import binding
+    cache = {}
+
+    def get(name):
+        if name not in cache:
+            case = oracle_case(CASES[name])
+            dec = binding.ChunkDecoder(case["cfg"])
+            dec.load_weights(case["weights"])
+            cache[name] = (dec, case)
+        return cache[name]
+    yield get
+    for dec, _ in cache.values():
+        dec.destroy()
+
+
+def bf16_np(t):
+    return t.float().cpu().numpy()
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2-ragged", "cfg3-crop", "cfg2"])
+def test_chunk_decode_matches_oracle(decoders, name):
+    dec, case = decoders(name)
+    cfg = case["cfg"]
+    z, bits, off = gpu_inputs(case)
+    out = dec.chunk_decode_ex(z, bits, off, taps=True)
+    torch.cuda.synchronize()
+    assert dec.get_status() == 0
+    for n, ch in enumerate(case["chunks"]):
+        ref, st = ch["out"], ch["stream"]
+        # A1 + A2
+        idx = out["idx"][n].cpu().numpy()
+        mism = idx != nhwc(ref["idx"])
+        assert mism.mean() <= IDX_RATE
+        if mism.any():     # only at bucket boundaries (R18)
+            step = (math.log(cfg.scale_max) - math.log(cfg.scale_min)) / (cfg.n_buckets - 1)
+            u = nhwc(ref["u"])[mism]
+            frac = (u - math.log(cfg.scale_min)) / step
+            assert np.abs(frac - np.floor(frac) - 0.5).max() < 1e-4
+        mu_ref = nhwc(ref["mu"])
+        assert (np.abs(out["mu"][n].cpu().numpy() - mu_ref) <= 1e-2 * np.maximum(np.abs(mu_ref), 1.0)).all()
+        assert np.abs(out["lnscale"][n].cpu().numpy() - nhwc(ref["u"])).max() <= 1e-2
+        # A3 + A4: integer work is bit-exact
+        assert np.array_equal(out["sym"][n].cpu().numpy(), nhwc(ref["sym"]))
+        assert np.abs(out["yhat"][n].cpu().numpy() - nhwc(ref["yhat"])).max() <= 1e-5
+        # A5 .. A8 intermediates: bf16 storage, loose stage-wise bounds relative to the tensor's scale
+        taps = ref["taps"]
+        for t in range(cfg.T):
+            for got, want in ([(out["f0"][n, t], taps["F0"][t]), (out["trunk"][n, t], taps["trunk"][t])] +
+                              [(out["stage"][s][n, t], taps["stage"][t][s]) for s in range(3)]):
+                w = nhwc(want)
+                err = np.abs(bf16_np(got) - w)
+                scale = max(1.0, float(np.abs(w).max()))
+                assert err.max() <= 0.03 * scale, (name, n, t, err.max(), scale)
+        # A9: pixels
+        f = out["frames"][n].cpu().numpy()
+        assert f.shape == ref["frames"].shape and f.min() >= 0.0 and f.max() <= 1.0
+        assert np.abs(f - ref["frames"]).max() <= PIX_TOL
+        assert psnr(f, ref["frames"]) >= PSNR_MIN
+
+
+def test_plain_entry_point_equals_ex_and_is_deterministic(decoders):
+    dec, case = decoders("cfg2-ragged")
+    z, bits, off = gpu_inputs(case)
+    a = dec.chunk_decode(z, bits, off).clone()
+    b = dec.chunk_decode_ex(z, bits, off)["frames"].clone()
+    c = dec.chunk_decode(z, bits, off).clone()
+    torch.cuda.synchronize()
+    assert torch.equal(a, b) and torch.equal(a, c)          # run-to-run bit-identical (R12 ii)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        d = dec.chunk_decode(z, bits, off, stream=s)
+    s.synchronize()
+    assert torch.equal(a, d)
+
+
+def test_entropy_params_entry_point(decoders):
+    dec, case = decoders("cfg3-crop")
+    z, _, _ = gpu_inputs(case)
+    mu, ls, idx = dec.entropy_params(z)
+    torch.cuda.synchronize()
+    ref = case["chunks"][0]["out"]
+    assert (idx[0].cpu().numpy() != nhwc(ref["idx"])).mean() <= IDX_RATE
+    assert np.abs(ls[0].cpu().numpy() - nhwc(ref["u"])).max() <= 1e-5
+    assert np.abs(mu[0].cpu().numpy() - nhwc(ref["mu"])).max() <= 1e-5
+
+
+def test_tables_and_encoder_bit_equal_to_oracle(decoders, orc):
+    import oracle
+    dec, case = decoders("cfg2-ragged")
+    cfg = case["cfg"]
+    st = case["chunks"][0]["stream"]
+    assert np.array_equal(dec.get_cdf(), st["cdf"])                       # two independent table builders (R8)
+    idx, u16 = nhwc(st["idx"]), case["u16"][0]
+    sym = dec.symbols_from_uniform(idx, u16)
+    assert np.array_equal(sym, nhwc(st["sym"]))
+    bits, off = dec.encode_chunk(idx, sym)
+    assert np.array_equal(off, st["sub_off"]) and np.array_equal(bits, st["bits"])   # two independent encoders
+    sym2, status = oracle.decode_symbols(orc, cfg, st["cdf"], st["idx"], bits, off)
+    assert status == 0 and np.array_equal(sym2, st["sym"])
+
+
+def test_teacher_forced_exact_laws_entropy_only(decoders, orc):
+    """Entropy-only mode: mu and ln sigma drawn exactly from the stated laws, indices fed to both sides (R3, R12)."""
+    import oracle
+    dec, case = decoders("cfg3-crop")
+    cfg = case["cfg"]
+    mu, u = synth.make_exact_law_params(cfg)
+    idx_hwc, _ = orc.bucket_index(u[0].astype(np.float64), cfg.n_buckets, cfg.scale_min, cfg.scale_max)
+    cdf = orc.build_cdf(cfg.n_buckets, cfg.scale_min, cfg.scale_max)
+    sym_hwc = orc.symbols_from_uniform(cdf, idx_hwc, case["u16"][0])
+    idx_chw, sym_chw = np.moveaxis(idx_hwc, -1, 0), np.moveaxis(sym_hwc, -1, 0)
+    bits, off = oracle.encode_chunk(orc, cfg, cdf, idx_chw, sym_chw)
+    z = torch.from_numpy(case["z"]).cuda()
+    out = dec.chunk_decode_ex(z, torch.from_numpy(bits).cuda(), torch.from_numpy(off.astype(np.int64)).to(torch.int32).cuda(),
+                              idx_override=torch.from_numpy(idx_hwc).cuda(), mu_override=torch.from_numpy(mu[0]).cuda(),
+                              taps=True, want_frames=False)
+    torch.cuda.synchronize()
+    assert dec.get_status() == 0
+    assert np.array_equal(out["sym"][0].cpu().numpy(), sym_hwc)
+    assert np.array_equal(out["yhat"][0].cpu().numpy(), sym_hwc.astype(np.float32) + mu[0])
+    zero_frac = float((sym_hwc == 0).mean())
+    assert 0.36 <= zero_frac <= 0.46                                       # P(r=0) ~ 0.41
+
+
+def test_corrupt_and_truncated_streams_set_status_not_fault(decoders):
+    dec, case = decoders("cfg2-ragged")
+    z, bits, off = gpu_inputs(case)
+    rng = np.random.default_rng(0)
+    hdr = 8 * (case["cfg"].lanes_per_substream // 32)
+    hits = 0
+    for trial in range(12):
+        b = bits.clone()
+        pos = int(rng.integers(hdr, int(off[1].item())))
+        b[pos] ^= 1 << int(rng.integers(0, 8))
+        dec.chunk_decode_ex(z, b, off, want_frames=False)
+        torch.cuda.synchronize()
+        hits += dec.get_status() != 0
+    assert hits >= 10
+    b = bits.clone()
+    b[:hdr] = 0xFF                                                          # garbage header: offsets out of range
+    dec.chunk_decode_ex(z, b, off, want_frames=False)
+    torch.cuda.synchronize()
+    assert dec.get_status() & 4
+    off2 = off.clone()
+    off2[-1] = off2[-1] // 2 // 4 * 4                                       # truncated last substream
+    dec.chunk_decode_ex(z, bits, off2, want_frames=False)
+    torch.cuda.synchronize()
+    assert dec.get_status() != 0
+    dec.chunk_decode_ex(z, bits, off, want_frames=False)                    # and the handle still works
+    torch.cuda.synchronize()
+    assert dec.get_status() == 0
+
+
+def test_multi_chunk_low_rate_call():
+    """Config-4 shape class on a small frame: 2 independent chunks in one call, T=16, c_y=192 (W=192 lanes), low-rate law."""
+    from paper_2606_04410_b200 import binding
+    import dataclasses
+    cfg = dataclasses.replace(synth.crop_config(synth.CONFIGS[4], 96, 160), n_chunks=2)
+    case = oracle_case(cfg)
+    dec = binding.ChunkDecoder(cfg)
+    dec.load_weights(case["weights"])
+    z, bits, off = gpu_inputs(case)
+    out = dec.chunk_decode_ex(z, bits, off, taps=True)
+    torch.cuda.synchronize()
+    assert dec.get_status() == 0
+    zero = 0.0
+    for n, ch in enumerate(case["chunks"]):
+        assert np.array_equal(out["sym"][n].cpu().numpy(), nhwc(ch["out"]["sym"]))
+        f = out["frames"][n].cpu().numpy()
+        assert np.abs(f - ch["out"]["frames"]).max() <= PIX_TOL and psnr(f, ch["out"]["frames"]) >= PSNR_MIN
+        zero += float((ch["out"]["sym"] == 0).mean()) / cfg.n_chunks
+    assert zero > 0.5                                                        # low-rate: mostly zero symbols
+    assert not torch.equal(out["frames"][0], out["frames"][1])
+    dec.destroy()
+
+
+def test_api_errors(decoders):
+    import ctypes as C
+    from paper_2606_04410_b200 import binding
+    cfg = synth.CONFIGS[1]
+    dec = binding.ChunkDecoder(cfg)
+    z = torch.zeros((1, cfg.c_z, 1, 1), dtype=torch.int16, device="cuda")
+    bits = torch.zeros(64, dtype=torch.uint8, device="cuda")
+    off = torch.zeros(2, dtype=torch.int32, device="cuda")
+    with pytest.raises(binding.UfnvcError, match="-3"):                      # UFNVC_E_NO_WEIGHTS
+        dec.chunk_decode(z, bits, off)
+    w = synth.make_weights(cfg)
+    blob = binding.pack_weights_blob(w, cfg.weight_dtype)
+    bad = np.frombuffer(b"XXXX" + blob[4:], np.uint8)
+    assert binding.LIB.ufnvc_load_weights(dec.handle, bad.ctypes.data, bad.size) == -4
+    w2 = dict(w); del w2["dec.1.2.w"]
+    with pytest.raises(binding.UfnvcError, match="dec.1.2.w"):
+        dec.load_weights(w2)
+    trunc = np.frombuffer(blob[:len(blob) // 2], np.uint8)
+    assert binding.LIB.ufnvc_load_weights(dec.handle, trunc.ctypes.data, trunc.size) == -4
+    dec.load_weights(w)
+    assert binding.LIB.ufnvc_chunk_decode(dec.handle, 1, None, None, 0, None, None, None) == -1
+    assert binding.LIB.ufnvc_chunk_decode(dec.handle, 2, z.data_ptr(), bits.data_ptr(), 64, off.data_ptr(), 1, None) == -1
+    dec.destroy()
