@@ -61,7 +61,7 @@ typedef struct ufnvc_config {
     int32_t trunk_expand;        /* 1x1 expansion factor inside a DC block (4) */
     int32_t dec_channels[5];     /* frame-decoder channels, dec_channels[0] == c_trunk, dec_channels[4] == 3 */
     int32_t n_buckets;           /* scale buckets (64), log-spaced on [scale_min, scale_max] inclusive [R4] */
-    float scale_min, scale_max;  /* 0.11, 20 */
+    double scale_min, scale_max; /* 0.11, 20 (double: both the tables and the bucket rule depend on them) */
     int32_t rows_per_substream;  /* latent rows per rANS substream (4) [R9] */
     int32_t lanes_per_substream; /* interleaved rANS lanes W per substream, multiple of 32 (default c_y) */
     int32_t max_chunks_per_call; /* independent chunks decoded by one call (1; 4 for config 4) */

@@ -24,7 +24,7 @@ class ufnvc_config(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("T", C.c_int32), ("height", C.c_int32), ("width", C.c_int32),
                 ("c_y", C.c_int32), ("c_z", C.c_int32), ("c_hyper", C.c_int32), ("c_trunk", C.c_int32),
                 ("n_trunk_blocks", C.c_int32), ("trunk_expand", C.c_int32), ("dec_channels", C.c_int32 * 5),
-                ("n_buckets", C.c_int32), ("scale_min", C.c_float), ("scale_max", C.c_float),
+                ("n_buckets", C.c_int32), ("scale_min", C.c_double), ("scale_max", C.c_double),
                 ("rows_per_substream", C.c_int32), ("lanes_per_substream", C.c_int32),
                 ("max_chunks_per_call", C.c_int32), ("weight_dtype", C.c_int32)]
 

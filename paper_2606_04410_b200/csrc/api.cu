@@ -42,7 +42,7 @@ int validate(const ufnvc_config &c, std::string &why)
     BAD(c.dec_channels[0] != c.c_trunk || c.dec_channels[4] != 3, "dec_channels[0] must equal c_trunk and [4] must be 3");
     for (int s = 1; s < 4; ++s) BAD(c.dec_channels[s] < 8 || c.dec_channels[s] % 8, "dec_channels must be multiples of 8");
     BAD(c.n_buckets < 1 || c.n_buckets > 64, "n_buckets must be in [1,64]");
-    BAD(!(c.scale_min > 0.f) || !(c.scale_max > c.scale_min), "need 0 < scale_min < scale_max");
+    BAD(!(c.scale_min > 0.0) || !(c.scale_max > c.scale_min), "need 0 < scale_min < scale_max");
     BAD(c.rows_per_substream < 1, "rows_per_substream >= 1");
     BAD(c.lanes_per_substream < 32 || c.lanes_per_substream % 32 || c.lanes_per_substream > 1024, "lanes_per_substream: multiple of 32 in [32,1024]");
     BAD(c.max_chunks_per_call < 1 || c.max_chunks_per_call > 64, "max_chunks_per_call out of range");
@@ -78,7 +78,7 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     h->force_generic = fg && fg[0] == '1';
 
     // O3 tables + search accelerator
-    build_cdf_tables(cfg->n_buckets, double(cfg->scale_min), double(cfg->scale_max), h->cdf32);
+    build_cdf_tables(cfg->n_buckets, cfg->scale_min, cfg->scale_max, h->cdf32);
     std::vector<uint16_t> lut, cdf16(h->cdf32.size());
     build_search_lut(h->cdf32, cfg->n_buckets, lut);
     for (size_t i = 0; i < cdf16.size(); ++i) cdf16[i] = uint16_t(h->cdf32[i]);     // c[255] = 2^16 wraps to 0

@@ -43,7 +43,7 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
         CU_TRY(launch_z_to_f64(z, h->hx0, n, c.c_z, Pz, st));
         CU_TRY(launch_hyper_conv(h->hyper[0], h->hx0, h->hx1, n, h->h_z, h->w_z, st));
         CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, n, h->h_z, h->w_z, st));
-        HeadParams hp{c.c_y, h->h, h->w, c.n_buckets, std::log(double(c.scale_min)), std::log(double(c.scale_max)), h->mu, h->lnscale, h->idx};
+        HeadParams hp{c.c_y, h->h, h->w, c.n_buckets, std::log(c.scale_min), std::log(c.scale_max), h->mu, h->lnscale, h->idx};
         CU_TRY(launch_hyper_head(h->hyper[2], h->hx2, n, h->h_z, h->w_z, hp, st));
         if (launches) *launches += 4;
     }
