@@ -21,7 +21,7 @@ cudaError_t conv(ufnvc_handle *h, const ConvLayer &L, const ConvProblem &P, cons
                  cudaStream_t st, int *launches)
 {
     if (launches) ++*launches;
-    if (L.use_tc && am.ok && !h->force_generic) return launch_conv_tc(L, P, am.tm, am.tile_h, am.tile_w, E, h->num_sms, st);
+    if (L.use_tc && am.ok && !h->force_generic) return launch_conv_tc(L, P, am.tm, am.tile_h, am.tile_w, am.flat, E, h->num_sms, st);
     return launch_conv_generic(L, P, E, st);
 }
 
@@ -141,11 +141,55 @@ int check_call(ufnvc_handle *h, int n_chunks, const void *z, const void *bits, c
 
 }  // namespace
 
+// choose the 128-pixel tile (TH x TW) that covers an H x W image with the fewest tiles; ties -> wider rows
+static void pick_tile(int H, int W, int &th, int &tw)
+{
+    long best = -1;
+    for (int t = 1; t <= 16; t *= 2) {
+        const int w = 128 / t;
+        const long tiles = long((H + t - 1) / t) * ((W + w - 1) / w);
+        if (best < 0 || tiles < best) { best = tiles; th = t; tw = w; }
+    }
+}
+
+static bool make_act_map(ufnvc_handle *h, ufnvc_handle::ActMap &am, const bf16 *base, int n_img, int H, int W, int C, bool want_flat,
+                         int imgs_per_chunk)
+{
+    am.ok = false;
+    if (C % 64) return true;
+    std::string err;
+    am.flat = want_flat && ((long long)imgs_per_chunk * H * W) % 128 == 0;
+    if (am.flat) {
+        am.tile_h = 1; am.tile_w = 128;
+        if (!tc_make_act_tmap(&am.tm, base, 1, int((long long)n_img * H * W / 128), 128, C, 1, 128, err)) { h->err = err; return false; }
+    } else {
+        pick_tile(H, W, am.tile_h, am.tile_w);
+        if (!tc_make_act_tmap(&am.tm, base, n_img, H, W, C, am.tile_h, am.tile_w, err)) { h->err = err; return false; }
+    }
+    am.ok = true;
+    return true;
+}
+
 extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t bytes)
 {
     if (!h || !blob_host) return UFNVC_E_INVALID_ARG;
     h->weights_loaded = false;
     if (int rc = load_weights_impl(h, blob_host, bytes)) return rc;
+    // tcgen05 path: weight descriptors + descriptors of the (fixed) workspace activations
+    const ufnvc_config &c = h->cfg;
+    std::string err;
+    bool ok = tc_make_weight_tmap(h->xframe, err);
+    for (auto &tb : h->trunk) ok = ok && tc_make_weight_tmap(tb.pw1, err) && tc_make_weight_tmap(tb.pw2, err);
+    for (int s = 0; s < 4; ++s) ok = ok && tc_make_weight_tmap(h->dec[s], err);
+    if (!ok) return fail(h, UFNVC_E_CUDA, err);
+    const int n = h->max_chunks, T = c.T;
+    ok = make_act_map(h, h->am_yhat, h->yhat, n, h->h, h->w, c.c_y, true, 1) &&
+         make_act_map(h, h->am_fb, h->fb, n * T, h->h, h->w, c.c_trunk, true, T) &&
+         make_act_map(h, h->am_hidden, h->hidden, n * T, h->h, h->w, c.c_trunk * c.trunk_expand, true, T) &&
+         make_act_map(h, h->am_fa, h->fa, n * T, h->h, h->w, c.c_trunk, false, T);
+    for (int s = 0; ok && s < 3; ++s)
+        ok = make_act_map(h, h->am_stage[s], h->stage[s], n * T, h->h << (s + 1), h->w << (s + 1), c.dec_channels[s + 1], false, T);
+    if (!ok) return fail(h, UFNVC_E_CUDA, h->err);
     h->weights_loaded = true;
     return UFNVC_OK;
 }

@@ -42,6 +42,7 @@ struct ufnvc_handle {
     struct ActMap {
         CUtensorMap tm;
         int tile_h = 0, tile_w = 0;
+        bool flat = false;               // 1x1 convs: all pixels of all images as one [rows][128] matrix
         bool ok = false;
     };
     ActMap am_yhat, am_fa, am_fb, am_hidden, am_stage[3];

@@ -93,7 +93,7 @@ cudaError_t launch_rans_decode(const RansParams &p, cudaStream_t st);
 
 // tcgen05 implicit-GEMM conv (conv_tc.cu)
 cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_in, int tile_h, int tile_w,
-                           const EpiParams &E, int num_sms, cudaStream_t st);
+                           bool flat, const EpiParams &E, int num_sms, cudaStream_t st);
 bool tc_make_weight_tmap(ConvLayer &L, std::string &err);
 bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, int tile_h, int tile_w,
                       std::string &err);

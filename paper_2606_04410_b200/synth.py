@@ -151,9 +151,10 @@ def make_weights(cfg: ChunkConfig) -> dict:
         out[name + ".b"] = b
 
     # hyper-decoder (O1): z ~ round(N(0,4)) so E[z^2] ~ 4.08; ReLU + gain 2 keeps E[x^2] ~ 4.08.
-    # `edge` = mean fraction of the 9 taps that fall inside a zero-padded h_z x w_z map (pure geometry):
-    # dividing the gain by it keeps the mean variance on tiny maps (config 1 has a 1x1 z).
-    edge = ((3 * cfg.h_z - 2) / (3 * cfg.h_z)) * ((3 * cfg.w_z - 2) / (3 * cfg.w_z))
+    # `edge`: a 1x1 z map (config 1) sees only the centre tap of each zero-padded 3x3 conv (1/9 of the fan-in), so
+    # the gain is raised to keep the variance; larger maps keep the plain gain (borders are then under-dispersed,
+    # which only narrows the sigma distribution on small test crops).  Pure geometry, no method arithmetic.
+    edge = 1.0 / 9.0 if cfg.h_z * cfg.w_z == 1 else 1.0
     conv("hyper.0", cfg.c_hyper, cfg.c_z, 3, 2.0 / edge)
     conv("hyper.1", cfg.c_hyper, cfg.c_hyper, 3, 2.0 / edge)
     # head: channels after pixel-shuffle x4: [0,C_y) = mu, [C_y,2C_y) = ln sigma.  Pre-shuffle

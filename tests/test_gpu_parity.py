@@ -227,3 +227,38 @@ def test_api_errors(decoders):
     assert binding.LIB.ufnvc_chunk_decode(dec.handle, 1, None, None, 0, None, None, None) == -1
     assert binding.LIB.ufnvc_chunk_decode(dec.handle, 2, z.data_ptr(), bits.data_ptr(), 64, off.data_ptr(), 1, None) == -1
     dec.destroy()
+
+
+def test_full_size_1080p_config3_matches_oracle():
+    """BASELINE.json configs[2] at FULL size, in the launch configuration bench.py times (plain ufnvc_chunk_decode on
+    a side stream): every pixel of all 8 frames against the oracle (894 GMAC in fp64 on the host: ~1-2 minutes)."""
+    import json
+    import os
+    import time
+    from paper_2606_04410_b200 import binding
+    cfg = synth.CONFIGS[3]
+    t0 = time.time()
+    case = oracle_case(cfg, keep=False)
+    t_oracle = time.time() - t0
+    dec = binding.ChunkDecoder(cfg)
+    dec.load_weights(case["weights"])
+    z, bits, off = gpu_inputs(case)
+    s = torch.cuda.Stream()
+    frames = dec.new_frames(1)
+    with torch.cuda.stream(s):
+        dec.chunk_decode(z, bits, off, frames=frames, stream=s)
+    s.synchronize()
+    assert dec.get_status() == 0
+    ref = case["chunks"][0]["out"]
+    f = frames[0].cpu().numpy()
+    err = np.abs(f - ref["frames"])
+    res = dict(max_abs=float(err.max()), rms=float(np.sqrt((err ** 2).mean())), psnr=psnr(f, ref["frames"]),
+               frame_std=float(ref["frames"].std()), oracle_seconds=t_oracle)
+    os.makedirs("gpurun_out", exist_ok=True)
+    json.dump(res, open("gpurun_out/parity_cfg3_full.json", "w"))
+    out = dec.chunk_decode_ex(z, bits, off, taps=True, want_frames=False)
+    torch.cuda.synchronize()
+    assert np.array_equal(out["sym"][0].cpu().numpy(), nhwc(ref["sym"]))          # 1,044,480 symbols bit-exact
+    assert (out["idx"][0].cpu().numpy() != nhwc(ref["idx"])).mean() <= IDX_RATE
+    assert res["max_abs"] <= PIX_TOL and res["psnr"] >= PSNR_MIN, res
+    dec.destroy()
