@@ -133,7 +133,10 @@ def _second_moment_yhat(cfg: ChunkConfig) -> float:
     lo, hi = cfg.scale_min, cfg.sigma_hi
     e_s2 = (hi * hi - lo * lo) / (2.0 * math.log(hi / lo))
     var_mu = 1.0 if cfg.mu_law == "normal" else 4.0 / 3.0
-    return e_s2 + 1.0 / 12.0 + var_mu
+    # R8 gives every one of the 255 symbols a frequency >= 1/2^16; drawing r from the QUANTISED table (R7) therefore
+    # adds sum_r r^2 / 2^16 = 2 * (127*128*255/6) / 65536 = 21.08 to E[r^2] whatever sigma is.
+    floor_mass = 2.0 * (127 * 128 * 255 / 6.0) / 65536.0
+    return e_s2 + 1.0 / 12.0 + var_mu + floor_mass
 
 
 def make_weights(cfg: ChunkConfig) -> dict:
