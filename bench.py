@@ -118,7 +118,7 @@ def run_reference(args):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2606_04410_b200 import binding, synth
+    from paper_2606_04410_b200 import binding, replicas, synth
 
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -177,10 +177,7 @@ def run_ours(args):
         barrier()
         t_wall = time.perf_counter() - t_wall
     total_ms = sum(step_ms)
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = replicas.max_over_ranks(total_ms, dev)
     frames_per_step = n * cfg.T
     value = world * frames_per_step * args.steps / (total_ms / 1e3)
 
@@ -206,10 +203,7 @@ def run_ours(args):
         e2e_step()
     barrier()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = replicas.max_over_ranks(e2e_s, dev)
     e2e_val = world * frames_per_step * e2e_steps / e2e_s
     h2d = z_pin.numel() * 2 + bits_pin.numel() + off_pin.numel() * 4
     d2h = out_pin.numel() * 4
