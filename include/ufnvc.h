@@ -63,7 +63,7 @@ typedef struct ufnvc_config {
     int32_t n_buckets;           /* scale buckets (64), log-spaced on [scale_min, scale_max] inclusive [R4] */
     double scale_min, scale_max; /* 0.11, 20 (double: both the tables and the bucket rule depend on them) */
     int32_t rows_per_substream;  /* latent rows per rANS substream (4) [R9] */
-    int32_t lanes_per_substream; /* interleaved rANS lanes W per substream, multiple of 32 (default c_y) */
+    int32_t lanes_per_substream; /* interleaved rANS lanes W per substream, multiple of 32 in [32,512] (default c_y) */
     int32_t max_chunks_per_call; /* independent chunks decoded by one call (1; 4 for config 4) */
     int32_t weight_dtype;        /* dtype of conv weights in the blob: 0 = fp32, 1 = bf16 */
 } ufnvc_config;

@@ -44,7 +44,7 @@ int validate(const ufnvc_config &c, std::string &why)
     BAD(c.n_buckets < 1 || c.n_buckets > 64, "n_buckets must be in [1,64]");
     BAD(!(c.scale_min > 0.0) || !(c.scale_max > c.scale_min), "need 0 < scale_min < scale_max");
     BAD(c.rows_per_substream < 1, "rows_per_substream >= 1");
-    BAD(c.lanes_per_substream < 32 || c.lanes_per_substream % 32 || c.lanes_per_substream > 1024, "lanes_per_substream: multiple of 32 in [32,1024]");
+    BAD(c.lanes_per_substream < 32 || c.lanes_per_substream % 32 || c.lanes_per_substream > 512, "lanes_per_substream: multiple of 32 in [32,512]");
     BAD(c.max_chunks_per_call < 1 || c.max_chunks_per_call > 64, "max_chunks_per_call out of range");
     BAD(c.weight_dtype != 0 && c.weight_dtype != 1, "weight_dtype must be 0 or 1");
 #undef BAD
@@ -76,6 +76,8 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     h->max_chunks = cfg->max_chunks_per_call;
     const char *fg = std::getenv("UFNVC_FORCE_GENERIC");
     h->force_generic = fg && fg[0] == '1';
+    const char *hl = std::getenv("UFNVC_HALO");
+    h->use_halo = !(hl && hl[0] == '0');
 
     // O3 tables + search accelerator
     build_cdf_tables(cfg->n_buckets, cfg->scale_min, cfg->scale_max, h->cdf32);
@@ -86,7 +88,7 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     const size_t n = size_t(h->max_chunks), P = size_t(h->h) * h->w, Pz = size_t(h->h_z) * h->w_z, T = size_t(cfg->T);
     bool ok = dev_alloc(h, h->d_cdf, cdf16.size()) && dev_alloc(h, h->d_lut, lut.size()) && dev_alloc(h, h->d_status, 1) &&
               dev_alloc(h, h->hx0, n * Pz * cfg->c_z) && dev_alloc(h, h->hx1, n * Pz * cfg->c_hyper) &&
-              dev_alloc(h, h->hx2, n * Pz * cfg->c_hyper) && dev_alloc(h, h->mu, n * P * cfg->c_y) &&
+              dev_alloc(h, h->hx2, n * Pz * cfg->c_hyper) && dev_alloc(h, h->hpart, 9 * n * Pz * cfg->c_hyper) && dev_alloc(h, h->mu, n * P * cfg->c_y) &&
               dev_alloc(h, h->lnscale, n * P * cfg->c_y) && dev_alloc(h, h->idx, n * P * cfg->c_y) &&
               dev_alloc(h, h->yhat, n * P * cfg->c_y) && dev_alloc(h, h->fa, n * T * P * cfg->c_trunk) &&
               dev_alloc(h, h->fb, n * T * P * cfg->c_trunk) &&

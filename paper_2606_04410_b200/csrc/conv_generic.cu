@@ -93,84 +93,94 @@ cudaError_t launch_conv_generic(const ConvLayer &L, const ConvProblem &P, const 
     return cudaGetLastError();
 }
 
-// ---- A6: depthwise 3x3, zero pad, bias.  HBM-bound: each thread owns 8 channels (one 16-byte
-// vector) of a run of DW_X horizontally adjacent pixels and slides a 3-column register window, so every input
-// vector is loaded 3 times (once per output row it feeds; the row neighbours hit L1/L2), and stored once.
-constexpr int DW_X = 4;
+// ---- A6: depthwise 3x3, zero pad, bias.  HBM-bound.  A thread owns 8 channels (one 16-byte vector)
+// of one pixel column x and walks down a segment of rows: each input row is loaded once as 3 vectors (x-1, x, x+1;
+// the side columns are L1 hits, loaded by the neighbouring warps of the block) and scattered into three rolling
+// accumulators (output rows r-1, r, r+1), so a row of outputs costs 3 vector loads and 1 store.  For C = 256 a warp is
+// exactly one pixel (512 contiguous bytes).
+__device__ __forceinline__ void dw_unpack(const uint4 &v, float (&f)[8])
+{
+    const __nv_bfloat162 *h = reinterpret_cast<const __nv_bfloat162 *>(&v);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) { const float2 t = __bfloat1622float2(h[e]); f[2 * e] = t.x; f[2 * e + 1] = t.y; }
+}
 
 __global__ void __launch_bounds__(256) dwconv3x3_kernel(const bf16 *__restrict__ in, bf16 *__restrict__ out,
                                                         const float *__restrict__ w9c, const float *__restrict__ bias,
-                                                        int n_img, int H, int W, int C)
+                                                        int n_img, int H, int W, int C, int rows_per_seg, int n_seg)
 {
-    const int cv = C / 8;                               // channel vectors per pixel
-    const int xr = (W + DW_X - 1) / DW_X;               // pixel runs per row
-    const long long total = (long long)n_img * H * xr * cv;
-    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
-        const int c8 = int(t % cv);
-        long long r = t / cv;
-        const int xrun = int(r % xr); r /= xr;
-        const int y = int(r % H);
-        const int img = int(r / H);
-        const int c0 = c8 * 8, x0 = xrun * DW_X;
-        float wv[9][8], bv[8];
+    const int cv = C / 8;
+    const long long total = (long long)n_img * n_seg * W * cv;
+    const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t >= total) return;
+    const int c8 = int(t % cv);
+    long long r = t / cv;
+    const int x = int(r % W); r /= W;
+    const int seg = int(r % n_seg);
+    const int img = int(r / n_seg);
+    const int c0 = c8 * 8;
+    const int y0 = seg * rows_per_seg, y1 = min(H, y0 + rows_per_seg);      // output rows [y0, y1)
+
+    float wv[9][8], bv[8];
 #pragma unroll
-        for (int k = 0; k < 9; ++k) {
-            const float4 lo = *reinterpret_cast<const float4 *>(w9c + k * C + c0);
-            const float4 hi = *reinterpret_cast<const float4 *>(w9c + k * C + c0 + 4);
-            wv[k][0] = lo.x; wv[k][1] = lo.y; wv[k][2] = lo.z; wv[k][3] = lo.w;
-            wv[k][4] = hi.x; wv[k][5] = hi.y; wv[k][6] = hi.z; wv[k][7] = hi.w;
-        }
-        {
-            const float4 lo = *reinterpret_cast<const float4 *>(bias + c0), hi = *reinterpret_cast<const float4 *>(bias + c0 + 4);
-            bv[0] = lo.x; bv[1] = lo.y; bv[2] = lo.z; bv[3] = lo.w; bv[4] = hi.x; bv[5] = hi.y; bv[6] = hi.z; bv[7] = hi.w;
-        }
-        const bf16 *img_in = in + (long long)img * H * W * C;
-        float acc[DW_X][8];
+    for (int k = 0; k < 9; ++k) {
+        const float4 lo = __ldg(reinterpret_cast<const float4 *>(w9c + k * C + c0));
+        const float4 hi = __ldg(reinterpret_cast<const float4 *>(w9c + k * C + c0 + 4));
+        wv[k][0] = lo.x; wv[k][1] = lo.y; wv[k][2] = lo.z; wv[k][3] = lo.w;
+        wv[k][4] = hi.x; wv[k][5] = hi.y; wv[k][6] = hi.z; wv[k][7] = hi.w;
+    }
+    {
+        const float4 lo = __ldg(reinterpret_cast<const float4 *>(bias + c0)), hi = __ldg(reinterpret_cast<const float4 *>(bias + c0 + 4));
+        bv[0] = lo.x; bv[1] = lo.y; bv[2] = lo.z; bv[3] = lo.w; bv[4] = hi.x; bv[5] = hi.y; bv[6] = hi.z; bv[7] = hi.w;
+    }
+    const bf16 *img_in = in + (long long)img * H * W * C + c0;
+    bf16 *img_out = out + (long long)img * H * W * C + c0;
+    const bool has_l = x > 0, has_r = x + 1 < W;
+
+    float accP[8], accC[8], accN[8];            // outputs rows ir-1, ir, ir+1 while input row ir is being added
 #pragma unroll
-        for (int i = 0; i < DW_X; ++i)
+    for (int e = 0; e < 8; ++e) { accP[e] = bv[e]; accC[e] = bv[e]; accN[e] = bv[e]; }
+
+    for (int ir = y0 - 1; ir <= y1; ++ir) {     // input rows feeding outputs [y0, y1)
+        if (ir >= 0 && ir < H) {
+            const bf16 *row = img_in + ((long long)ir * W + x) * C;
+            const uint4 z4 = make_uint4(0, 0, 0, 0);
+            const uint4 vl = has_l ? __ldg(reinterpret_cast<const uint4 *>(row - C)) : z4;
+            const uint4 vc = __ldg(reinterpret_cast<const uint4 *>(row));
+            const uint4 vr = has_r ? __ldg(reinterpret_cast<const uint4 *>(row + C)) : z4;
+            float fl[8], fc[8], fr[8];
+            dw_unpack(vl, fl); dw_unpack(vc, fc); dw_unpack(vr, fr);
 #pragma unroll
-            for (int e = 0; e < 8; ++e) acc[i][e] = bv[e];
-#pragma unroll
-        for (int dy = 0; dy < 3; ++dy) {
-            const int yy = y + dy - 1;
-            if (yy < 0 || yy >= H) continue;
-#pragma unroll
-            for (int xi = 0; xi < DW_X + 2; ++xi) {     // input column x0 - 1 + xi feeds outputs xi-2 .. xi
-                const int xx = x0 - 1 + xi;
-                if (xx < 0 || xx >= W) continue;
-                const uint4 v = *reinterpret_cast<const uint4 *>(img_in + ((long long)yy * W + xx) * C + c0);
-                const bf16 *ve = reinterpret_cast<const bf16 *>(&v);
-                float f[8];
-#pragma unroll
-                for (int e = 0; e < 8; ++e) f[e] = __bfloat162float(ve[e]);
-#pragma unroll
-                for (int dx = 0; dx < 3; ++dx) {
-                    const int oi = xi - dx;             // output index whose tap dx reads this column
-                    if (oi < 0 || oi >= DW_X) continue;
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) acc[oi][e] = fmaf(wv[dy * 3 + dx][e], f[e], acc[oi][e]);
-                }
+            for (int e = 0; e < 8; ++e) {
+                // input row ir is kernel row 2 of output ir-1, row 1 of output ir, row 0 of output ir+1
+                accP[e] = fmaf(wv[6][e], fl[e], fmaf(wv[7][e], fc[e], fmaf(wv[8][e], fr[e], accP[e])));
+                accC[e] = fmaf(wv[3][e], fl[e], fmaf(wv[4][e], fc[e], fmaf(wv[5][e], fr[e], accC[e])));
+                accN[e] = fmaf(wv[0][e], fl[e], fmaf(wv[1][e], fc[e], fmaf(wv[2][e], fr[e], accN[e])));
             }
         }
-#pragma unroll
-        for (int i = 0; i < DW_X; ++i) {
-            if (x0 + i >= W) continue;
+        const int oy = ir - 1;                  // output row oy is complete once input row oy+1 = ir has been added
+        if (oy >= y0 && oy < y1) {
             uint4 o;
-            bf16 *oe = reinterpret_cast<bf16 *>(&o);
+            __nv_bfloat162 *oe = reinterpret_cast<__nv_bfloat162 *>(&o);
 #pragma unroll
-            for (int e = 0; e < 8; ++e) oe[e] = __float2bfloat16_rn(acc[i][e]);
-            *reinterpret_cast<uint4 *>(out + (((long long)img * H + y) * W + x0 + i) * C + c0) = o;
+            for (int e = 0; e < 4; ++e) oe[e] = __floats2bfloat162_rn(accP[2 * e], accP[2 * e + 1]);
+            *reinterpret_cast<uint4 *>(img_out + ((long long)oy * W + x) * C) = o;
         }
+#pragma unroll
+        for (int e = 0; e < 8; ++e) { accP[e] = accC[e]; accC[e] = accN[e]; accN[e] = bv[e]; }
     }
 }
 
 cudaError_t launch_dwconv3x3(const bf16 *in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
                              int C, cudaStream_t st)
 {
-    const long long total = (long long)n_img * H * ((W + DW_X - 1) / DW_X) * (C / 8);
-    long long blocks = (total + 255) / 256;
-    if (blocks > 148LL * 64) blocks = 148LL * 64;
-    dwconv3x3_kernel<<<(unsigned)blocks, 256, 0, st>>>(in, out, w9c, bias, n_img, H, W, C);
+    // segment length: the shortest of {H, 16, 8} rows that still gives >= ~32 warps per SM (148 SMs)
+    int rows = H;
+    const long long per_row_threads = (long long)n_img * W * (C / 8);
+    while (rows > 8 && per_row_threads * ((H + rows - 1) / rows) < 148LL * 32 * 32) rows = (rows + 1) / 2;
+    const int n_seg = (H + rows - 1) / rows;
+    const long long total = per_row_threads * n_seg;
+    dwconv3x3_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(in, out, w9c, bias, n_img, H, W, C, rows, n_seg);
     return cudaGetLastError();
 }
 

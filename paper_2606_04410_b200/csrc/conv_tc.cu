@@ -27,11 +27,12 @@ constexpr int kStages = 4;
 constexpr int kTileM = 128;
 constexpr int kSlabK = 64;                       // bf16 channels per smem row = 128 bytes = one swizzle span
 constexpr int kABytes = kTileM * kSlabK * 2;     // 16 KB
-constexpr int kThreads = 192;
+constexpr int kThreads = 320;                    // warp 0 TMA, warp 1 MMA, warps 2..9 epilogue
 constexpr uint32_t kSpinLimit = 1u << 28;
 
 struct TcParams {
     int n_img_m, Hm, Wm;          // activation as the TMA map sees it (flattened for 1x1 convs)
+    int flat, tw_shift;           // flat: rows of 128 consecutive pixels; tw_shift = log2(TW)
     int tiles_y, tiles_x, TH, TW;
     int H, W;                     // real image dims: global pixel -> (img, y, x) for the epilogue
     int taps, slabs;              // k-blocks per tile = taps * slabs
@@ -162,6 +163,117 @@ __device__ __forceinline__ TileCoord tile_coord(const TcParams &p, int tile)
     return c;
 }
 
+// 8 epilogue warps: warp w reads TMEM lanes 32*(w%4) .. +31 (a hardware rule), and the two warps of a lane quadrant
+// split the 32-column chunks between them (even / odd), so every SM sub-partition holds two epilogue warps and the
+// tcgen05.ld / MUFU latencies of one hide behind the other.  tcgen05.ld -> bias -> act -> store, per tile of the
+// persistent schedule; tfull0 / tempty0 are the smem addresses of the first of two consecutive mbarriers each.
+template <int MODE>
+__device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_base, uint32_t tfull0, uint32_t tempty0,
+                                               int warp, int lane)
+{
+    const int quad = warp & 3;
+    const int half = (warp - 2) >> 2;                             // 0: even 32-column chunks, 1: odd ones
+    const int m = quad * 32 + lane;                               // accumulator row = pixel inside the tile
+    const int my = m >> p.tw_shift, mx = m & (p.TW - 1);          // TW is a power of two
+    const unsigned P = unsigned(p.H) * unsigned(p.W);
+    int it = 0;
+    for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x, ++it) {
+        const TileCoord tc = tile_coord(p, tile);
+        const int acc = it & 1;
+        const uint32_t acc_phase = (it >> 1) & 1;
+        const int ym = tc.y0 + my, xm = tc.x0 + mx;
+        const bool inb = ym < p.Hm && xm < p.Wm;
+        int img = tc.img, y = ym, x = xm;
+        if (p.flat) {                                             // map-space row of 128 pixels -> real (img, y, x)
+            const unsigned gp = unsigned(ym) * 128u + unsigned(xm);
+            img = int(gp / P);
+            const unsigned rem = gp - unsigned(img) * P;
+            y = int(rem / unsigned(p.W));
+            x = int(rem - unsigned(y) * unsigned(p.W));
+        }
+        const int grp = p.groups == 1 ? 0 : img % p.groups;
+        const float *bias = p.bias + (long long)grp * p.n_pad + tc.nt * p.BN;
+        mbar_wait(tfull0 + 8u * acc, acc_phase);
+        tc_fence_after();
+        const uint32_t t_row = tmem_base + (uint32_t(quad * 32) << 16) + uint32_t(acc * p.BN);
+        if (MODE == EPI_FINAL) {
+            if (half == 0) {
+                uint32_t v[16];
+                tmem_ld16(t_row, v);
+                if (inb) {
+                    if (p.E.c_o == 3 && p.n_real == 12 && !(p.E.out_w & 1)) {
+                        // packed column n = (2i + j) * 3 + c -> out[img][c][2y + i][2x + j]: j = 0, 1 are one float2
+                        float *base = reinterpret_cast<float *>(p.E.out) + (long long)img * p.E.img_stride;
+                        const int ox = 2 * x;
+                        if (ox < p.E.out_w) {
+#pragma unroll
+                            for (int i = 0; i < 2; ++i) {
+                                const int oy = 2 * y + i;
+                                if (oy >= p.E.out_h) continue;
+#pragma unroll
+                                for (int c = 0; c < 3; ++c) {
+                                    const int n0 = (2 * i) * 3 + c, n1 = (2 * i + 1) * 3 + c;
+                                    float2 o2;
+                                    o2.x = fminf(fmaxf(__uint_as_float(v[n0]) + __ldg(bias + n0), 0.0f), 1.0f);
+                                    o2.y = fminf(fmaxf(__uint_as_float(v[n1]) + __ldg(bias + n1), 0.0f), 1.0f);
+                                    *reinterpret_cast<float2 *>(base + ((long long)c * p.E.out_h + oy) * p.E.out_w + ox) = o2;
+                                }
+                            }
+                        }
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) {
+                            const int n = tc.nt * p.BN + j;
+                            if (n < p.n_real) epi_store_final(p.E, img, y, x, n, __uint_as_float(v[j]) + __ldg(bias + j));
+                        }
+                    }
+                }
+            }
+        } else {
+            for (int c0 = half * 32; c0 < p.BN; c0 += 64) {
+                uint32_t v[32];
+                tmem_ld32(t_row + uint32_t(c0), v);
+                if (!inb) continue;
+                const int n = tc.nt * p.BN + c0;                  // 32 consecutive packed columns, one store run
+                const long long o = epi_offset(p.E, img, y, x, p.H, p.W, n);
+                bf16 *dst = reinterpret_cast<bf16 *>(p.E.out) + o;
+                float f[32];
+#pragma unroll
+                for (int j = 0; j < 32; j += 4) {
+                    const float4 b4 = __ldg(reinterpret_cast<const float4 *>(bias + c0 + j));
+                    f[j] = __uint_as_float(v[j]) + b4.x; f[j + 1] = __uint_as_float(v[j + 1]) + b4.y;
+                    f[j + 2] = __uint_as_float(v[j + 2]) + b4.z; f[j + 3] = __uint_as_float(v[j + 3]) + b4.w;
+                }
+                if (p.E.act == ACT_GELU) {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) f[j] = gelu_fast(f[j]);
+                }
+                if (MODE == EPI_NHWC && p.E.residual) {
+                    const uint4 *rs = reinterpret_cast<const uint4 *>(p.E.residual + o);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const uint4 r4 = rs[q];
+                        const bf16 *re = reinterpret_cast<const bf16 *>(&r4);
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) f[q * 8 + e] += __bfloat162float(re[e]);
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    uint4 o4;
+                    __nv_bfloat162 *oe = reinterpret_cast<__nv_bfloat162 *>(&o4);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) oe[e] = __floats2bfloat162_rn(f[q * 8 + 2 * e], f[q * 8 + 2 * e + 1]);
+                    reinterpret_cast<uint4 *>(dst)[q] = o4;
+                }
+            }
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(tempty0 + 8u * acc);
+    }
+}
+
 template <int MODE>
 __global__ void __launch_bounds__(kThreads, 1)
 conv_tc_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b, const TcParams p)
@@ -188,7 +300,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_a) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_b) : "memory");
         for (int s = 0; s < kStages; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-        for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 4); }
+        for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 8); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) {
@@ -246,80 +358,174 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant
             }
         }
     } else {
-        // ===================== epilogue: 4 warps, warp w owns TMEM lanes 32*(w%4) .. +31 =====================
-        const int quad = warp & 3;
-        const int m = quad * 32 + lane;                               // accumulator row = pixel inside the tile
-        const int P = p.H * p.W;
-        int it = 0;
-        for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x, ++it) {
-            const TileCoord tc = tile_coord(p, tile);
-            const int acc = it & 1;
-            const uint32_t acc_phase = (it >> 1) & 1;
-            const int ym = tc.y0 + m / p.TW, xm = tc.x0 + m % p.TW;
-            const bool inb = ym < p.Hm && xm < p.Wm;
-            // map-space pixel -> real (img, y, x)
-            const long long gp = ((long long)tc.img * p.Hm + ym) * p.Wm + xm;
-            const int img = int(gp / P);
-            const int rem = int(gp - (long long)img * P);
-            const int y = rem / p.W, x = rem - y * p.W;
-            const int grp = p.groups == 1 ? 0 : img % p.groups;
-            const float *bias = p.bias + (long long)grp * p.n_pad + tc.nt * p.BN;
-            mbar_wait(tfull_bar(acc), acc_phase);
-            tc_fence_after();
-            const uint32_t t_row = tmem_base + (uint32_t(quad * 32) << 16) + uint32_t(acc * p.BN);
-            if (MODE == EPI_FINAL) {
-                uint32_t v[16];
-                tmem_ld16(t_row, v);
-                if (inb) {
-#pragma unroll
-                    for (int j = 0; j < 16; ++j) {
-                        const int n = tc.nt * p.BN + j;
-                        if (n < p.n_real) epi_store_final(p.E, img, y, x, n, __uint_as_float(v[j]) + __ldg(bias + j));
+        epilogue_warps<MODE>(p, tmem_base, tfull_bar(0), tempty_bar(0), warp, lane);
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(tmem_cols) : "memory");
+    }
+}
+
+
+// ---------------------------------------------------------------------------------------------------------------
+// Halo variant for 3x3 convs.  The tile is 16 rows x 8 columns of pixels.  Per 64-channel slab ONE TMA box
+// {64 ch, 10, 18} brings the tile plus its 1-pixel halo (zero-filled outside the image); halo pixel (hy, hx) lands at
+// (hy * 10 + hx) * 128 B, 128B-swizzled relative to the 1024-aligned stage base.  Tap (dy, dx) then needs no data
+// movement at all: its A operand is the same buffer viewed from start + (dy * 10 + dx) * 128 B with a stride of
+// 10 * 128 = 1280 B between 8-row groups (one image row of the tile = one 8-row core-matrix group), because the
+// tensor core applies the 128B swizzle to absolute shared-memory address bits.  L2->SM traffic for A drops from
+// 9 x 16 KB to 22.5 KB per slab -- the first-pass kernel was bound by exactly that traffic.
+// When all weight tiles of a (group, n-tile) fit the B ring (A9: 9 taps x 2 KB) they stay resident across tiles.
+constexpr int kHaloTH = 16, kHaloTW = 8;
+constexpr int kHaloRowPitch = (kHaloTW + 2) * 128;                            // 1280 B
+constexpr int kHaloBytes = (kHaloTH + 2) * (kHaloTW + 2) * 128;              // 23040 B = one TMA box
+constexpr int kHaloStage = (kHaloBytes + 1023) / 1024 * 1024;                // 23552 B
+constexpr int kHaloAStages = 3;
+
+__device__ __forceinline__ uint64_t umma_desc_sw128_sbo(uint32_t saddr, uint32_t sbo_bytes)
+{
+    return uint64_t((saddr & 0x3FFFFu) >> 4) | (uint64_t(1) << 16) | (uint64_t(sbo_bytes >> 4) << 32) | (uint64_t(1) << 46) |
+           (uint64_t(2) << 61);
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(kThreads, 1)
+conv_halo_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b, const TcParams p,
+                 const int nb_stages, const int b_resident)
+{
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t b_bytes = uint32_t(p.BN) * 128u;                             // multiple of 2 KB
+    const uint32_t b_base = smem_base + kHaloAStages * kHaloStage;
+    const uint32_t bar_base = b_base + uint32_t(nb_stages) * b_bytes;
+    auto afull = [&](int s) { return bar_base + 8u * s; };
+    auto aempty = [&](int s) { return bar_base + 8u * (kHaloAStages + s); };
+    const uint32_t misc = bar_base + 8u * (2 * kHaloAStages);
+    const uint32_t tfull0 = misc, tempty0 = misc + 16u, bres_full = misc + 32u, bfree = misc + 40u, tmem_slot = misc + 48u;
+    const uint32_t bbar = misc + 64u;
+    auto bfull = [&](int s) { return bbar + 8u * s; };
+    auto bempty = [&](int s) { return bbar + 8u * (nb_stages + s); };
+    volatile uint32_t *tmem_slot_ptr = reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int btiles = 9 * p.slabs;                                             // weight tiles per output tile
+    uint32_t tmem_cols = 32;
+    while (tmem_cols < uint32_t(2 * p.BN)) tmem_cols <<= 1;
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_a) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_b) : "memory");
+        for (int s = 0; s < kHaloAStages; ++s) { mbar_init(afull(s), 1); mbar_init(aempty(s), 1); }
+        for (int s = 0; s < nb_stages; ++s) { mbar_init(bfull(s), 1); mbar_init(bempty(s), 1); }
+        for (int a = 0; a < 2; ++a) { mbar_init(tfull0 + 8u * a, 1); mbar_init(tempty0 + 8u * a, 8); }
+        mbar_init(bres_full, 1);
+        mbar_init(bfree, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(tmem_cols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    // weight-set key of a tile: resident weights are reloaded only when it changes
+    auto tile_key = [&](const TileCoord &tc) { return (p.groups == 1 ? 0 : tc.img % p.groups) * p.n_tiles + tc.nt; };
+
+    if (warp == 0) {
+        // ===================== TMA producer =====================
+        if (lane == 0) {
+            int sa = 0, sb = 0; uint32_t pa = 0, pb = 0, pfree = 0;
+            int prev_key = -1;
+            for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x) {
+                const TileCoord tc = tile_coord(p, tile);
+                const int grp = p.groups == 1 ? 0 : tc.img % p.groups;
+                if (b_resident) {
+                    const int key = tile_key(tc);
+                    if (key != prev_key) {
+                        if (prev_key >= 0) { mbar_wait(bfree, pfree); pfree ^= 1; }     // MMAs on the old weights retired
+                        mbar_expect_tx(bres_full, uint32_t(btiles) * b_bytes);
+                        for (int bt = 0; bt < btiles; ++bt) {
+                            const int slab = bt / 9, tap = bt - slab * 9;
+                            tma_load_3d(b_base + uint32_t(bt) * b_bytes, &tmap_b, bres_full, slab * kSlabK, tc.nt * p.BN, grp * 9 + tap);
+                        }
+                        prev_key = key;
                     }
                 }
-            } else {
-                for (int c0 = 0; c0 < p.BN; c0 += 32) {
-                    uint32_t v[32];
-                    tmem_ld32(t_row + uint32_t(c0), v);
-                    if (!inb) continue;
-                    const int n = tc.nt * p.BN + c0;                  // 32 consecutive packed columns, one store run
-                    const long long o = epi_offset(p.E, img, y, x, p.H, p.W, n);
-                    bf16 *dst = reinterpret_cast<bf16 *>(p.E.out) + o;
-                    float f[32];
-#pragma unroll
-                    for (int j = 0; j < 32; j += 4) {
-                        const float4 b4 = __ldg(reinterpret_cast<const float4 *>(bias + c0 + j));
-                        f[j] = __uint_as_float(v[j]) + b4.x; f[j + 1] = __uint_as_float(v[j + 1]) + b4.y;
-                        f[j + 2] = __uint_as_float(v[j + 2]) + b4.z; f[j + 3] = __uint_as_float(v[j + 3]) + b4.w;
-                    }
-                    if (p.E.act == ACT_GELU) {
-#pragma unroll
-                        for (int j = 0; j < 32; ++j) f[j] = gelu_erf(f[j]);
-                    }
-                    if (MODE == EPI_NHWC && p.E.residual) {
-                        const uint4 *rs = reinterpret_cast<const uint4 *>(p.E.residual + o);
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            const uint4 r4 = rs[q];
-                            const bf16 *re = reinterpret_cast<const bf16 *>(&r4);
-#pragma unroll
-                            for (int e = 0; e < 8; ++e) f[q * 8 + e] += __bfloat162float(re[e]);
+                for (int slab = 0; slab < p.slabs; ++slab) {
+                    mbar_wait(aempty(sa), pa ^ 1);
+                    mbar_expect_tx(afull(sa), kHaloBytes);
+                    tma_load_4d(smem_base + sa * kHaloStage, &tmap_a, afull(sa), slab * kSlabK, tc.x0 - 1, tc.y0 - 1, tc.img);
+                    if (++sa == kHaloAStages) { sa = 0; pa ^= 1; }
+                    if (!b_resident) {
+                        for (int tap = 0; tap < 9; ++tap) {
+                            mbar_wait(bempty(sb), pb ^ 1);
+                            mbar_expect_tx(bfull(sb), b_bytes);
+                            tma_load_3d(b_base + uint32_t(sb) * b_bytes, &tmap_b, bfull(sb), slab * kSlabK, tc.nt * p.BN, grp * 9 + tap);
+                            if (++sb == nb_stages) { sb = 0; pb ^= 1; }
                         }
-                    }
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        uint4 o4;
-                        __nv_bfloat162 *oe = reinterpret_cast<__nv_bfloat162 *>(&o4);
-#pragma unroll
-                        for (int e = 0; e < 4; ++e) oe[e] = __floats2bfloat162_rn(f[q * 8 + 2 * e], f[q * 8 + 2 * e + 1]);
-                        reinterpret_cast<uint4 *>(dst)[q] = o4;
                     }
                 }
             }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(tempty_bar(acc));
         }
+    } else if (warp == 1) {
+        // ===================== MMA issuer =====================
+        if (lane == 0) {
+            const uint32_t idesc = umma_idesc_bf16(kTileM, p.BN);
+            int sa = 0, sb = 0; uint32_t pa = 0, pb = 0, pres = 0;
+            int prev_key = -1;
+            int it = 0;
+            for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x, ++it) {
+                const TileCoord tc = tile_coord(p, tile);
+                const int acc = it & 1;
+                const uint32_t acc_phase = (it >> 1) & 1;
+                if (b_resident) {
+                    const int key = tile_key(tc);
+                    if (key != prev_key) { mbar_wait(bres_full, pres); pres ^= 1; prev_key = key; }
+                }
+                mbar_wait(tempty0 + 8u * acc, acc_phase ^ 1);
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + uint32_t(acc * p.BN);
+                for (int slab = 0; slab < p.slabs; ++slab) {
+                    mbar_wait(afull(sa), pa);
+                    tc_fence_after();
+                    const uint32_t a_src = smem_base + sa * kHaloStage;
+                    for (int tap = 0; tap < 9; ++tap) {
+                        uint32_t b_src;
+                        if (b_resident) {
+                            b_src = b_base + uint32_t(slab * 9 + tap) * b_bytes;
+                        } else {
+                            mbar_wait(bfull(sb), pb);
+                            tc_fence_after();
+                            b_src = b_base + uint32_t(sb) * b_bytes;
+                        }
+                        const uint32_t a_tap = a_src + uint32_t((tap / 3) * (kHaloTW + 2) + tap % 3) * 128u;
+                        const uint64_t da = umma_desc_sw128_sbo(a_tap, kHaloRowPitch), db = umma_desc_sw128(b_src);
+#pragma unroll
+                        for (int k = 0; k < kSlabK / 16; ++k)
+                            umma_bf16(d_tmem, da + uint64_t(2 * k), db + uint64_t(2 * k), idesc, (slab | tap | k) != 0);
+                        if (!b_resident) {
+                            umma_commit(bempty(sb));
+                            if (++sb == nb_stages) { sb = 0; pb ^= 1; }
+                        }
+                    }
+                    umma_commit(aempty(sa));
+                    if (++sa == kHaloAStages) { sa = 0; pa ^= 1; }
+                }
+                umma_commit(tfull0 + 8u * acc);
+                if (b_resident) {                                               // release the weights if the next tile swaps them
+                    const int next = tile + gridDim.x;
+                    if (next < p.total_tiles && tile_key(tile_coord(p, next)) != prev_key) umma_commit(bfree);
+                }
+            }
+        }
+    } else {
+        epilogue_warps<MODE>(p, tmem_base, tfull0, tempty0, warp, lane);
     }
 
     tc_fence_before();
@@ -390,6 +596,56 @@ bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W
     return encode(tm, base, 4, dims, strides, box, err);
 }
 
+bool tc_make_halo_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, std::string &err)
+{
+    return tc_make_act_tmap(tm, base, n_img, H, W, C, kHaloTH + 2, kHaloTW + 2, err);
+}
+
+cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
+                             cudaStream_t st)
+{
+    if (L.taps != 9) return cudaErrorInvalidValue;
+    TcParams p{};
+    p.H = P.H; p.W = P.W;
+    p.n_img_m = P.n_img; p.Hm = P.H; p.Wm = P.W;
+    p.TH = kHaloTH; p.TW = kHaloTW;
+    p.flat = 0; p.tw_shift = 3;
+    p.tiles_y = (P.H + kHaloTH - 1) / kHaloTH;
+    p.tiles_x = (P.W + kHaloTW - 1) / kHaloTW;
+    p.taps = 9; p.slabs = L.c_in / kSlabK;
+    p.BN = L.block_n; p.n_tiles = L.n_pad / L.block_n; p.n_real = L.n; p.n_pad = L.n_pad;
+    p.groups = L.groups;
+    p.total_tiles = p.n_img_m * p.tiles_y * p.tiles_x * p.n_tiles;
+    p.bias = L.bias;
+    p.E = E;
+    const size_t b_bytes = size_t(L.block_n) * 128;
+    const size_t budget = 227 * 1024 - 1024 - size_t(kHaloAStages) * kHaloStage - 1024;
+    const int btiles = 9 * p.slabs;
+    int nb = int(budget / b_bytes);
+    const int resident = btiles <= nb ? 1 : 0;
+    if (resident) nb = btiles; else if (nb > 8) nb = 8;
+    if (nb < 2) return cudaErrorInvalidValue;
+    const size_t smem = 1024 + size_t(kHaloAStages) * kHaloStage + size_t(nb) * b_bytes + 128 + 16 * size_t(nb) + 64;
+    const int grid = p.total_tiles < num_sms ? p.total_tiles : num_sms;
+    auto launch = [&](auto kern) -> cudaError_t {
+        static thread_local const void *configured[8] = {};
+        bool done = false;
+        for (const void *c : configured) done |= (c == (const void *)kern);
+        if (!done) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+            if (e != cudaSuccess) return e;
+            for (auto &c : configured) if (!c) { c = (const void *)kern; break; }
+        }
+        kern<<<grid, kThreads, smem, st>>>(tmap_halo, L.tmap_w, p, nb, resident);
+        return cudaGetLastError();
+    };
+    switch (E.mode) {
+        case EPI_NHWC: return launch(conv_halo_kernel<EPI_NHWC>);
+        case EPI_PS2: return launch(conv_halo_kernel<EPI_PS2>);
+        default: return launch(conv_halo_kernel<EPI_FINAL>);
+    }
+}
+
 cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_in, int tile_h, int tile_w, bool flat,
                            const EpiParams &E, int num_sms, cudaStream_t st)
 {
@@ -403,6 +659,8 @@ cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUten
         p.n_img_m = P.n_img; p.Hm = P.H; p.Wm = P.W;
     }
     p.TH = tile_h; p.TW = tile_w;
+    p.flat = flat ? 1 : 0;
+    for (p.tw_shift = 0; (1 << p.tw_shift) < tile_w; ++p.tw_shift) {}
     p.tiles_y = (p.Hm + tile_h - 1) / tile_h;
     p.tiles_x = (p.Wm + tile_w - 1) / tile_w;
     p.taps = L.taps; p.slabs = L.c_in / kSlabK;

@@ -21,6 +21,8 @@ cudaError_t conv(ufnvc_handle *h, const ConvLayer &L, const ConvProblem &P, cons
                  cudaStream_t st, int *launches)
 {
     if (launches) ++*launches;
+    if (L.use_tc && L.taps == 9 && am.halo_ok && h->use_halo && !h->force_generic)
+        return launch_conv_halo(L, P, am.tm_halo, E, h->num_sms, st);
     if (L.use_tc && am.ok && !h->force_generic) return launch_conv_tc(L, P, am.tm, am.tile_h, am.tile_w, am.flat, E, h->num_sms, st);
     return launch_conv_generic(L, P, E, st);
 }
@@ -41,8 +43,8 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     mark(sg, st);
     if (need_hyper) {
         CU_TRY(launch_z_to_f64(z, h->hx0, n, c.c_z, Pz, st));
-        CU_TRY(launch_hyper_conv(h->hyper[0], h->hx0, h->hx1, n, h->h_z, h->w_z, st));
-        CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, n, h->h_z, h->w_z, st));
+        CU_TRY(launch_hyper_conv(h->hyper[0], h->hx0, h->hx1, h->hpart, n, h->h_z, h->w_z, st));
+        CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, h->hpart, n, h->h_z, h->w_z, st));
         HeadParams hp{c.c_y, h->h, h->w, c.n_buckets, std::log(c.scale_min), std::log(c.scale_max), h->mu, h->lnscale, h->idx};
         CU_TRY(launch_hyper_head(h->hyper[2], h->hx2, n, h->h_z, h->w_z, hp, st));
         if (launches) *launches += 4;
@@ -156,6 +158,7 @@ static bool make_act_map(ufnvc_handle *h, ufnvc_handle::ActMap &am, const bf16 *
                          int imgs_per_chunk)
 {
     am.ok = false;
+    am.halo_ok = false;
     if (C % 64) return true;
     std::string err;
     am.flat = want_flat && ((long long)imgs_per_chunk * H * W) % 128 == 0;
@@ -165,6 +168,8 @@ static bool make_act_map(ufnvc_handle *h, ufnvc_handle::ActMap &am, const bf16 *
     } else {
         pick_tile(H, W, am.tile_h, am.tile_w);
         if (!tc_make_act_tmap(&am.tm, base, n_img, H, W, C, am.tile_h, am.tile_w, err)) { h->err = err; return false; }
+        if (!tc_make_halo_tmap(&am.tm_halo, base, n_img, H, W, C, err)) { h->err = err; return false; }
+        am.halo_ok = true;
     }
     am.ok = true;
     return true;

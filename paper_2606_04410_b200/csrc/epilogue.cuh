@@ -20,6 +20,23 @@ __device__ __forceinline__ float gelu_erf(float v)
     return 0.5f * v * (1.0f + erfv);
 }
 
+// GELU for the tensor-core epilogues: v/2 (1 + tanh(v (a + b v^2 + c v^4))) with (a, b, c) a least-squares fit of
+// atanh(erf(v/sqrt2))/v weighted by the GELU sensitivity (|fit - erf form| <= 3e-5 on the whole line; the classic
+// 0.044715 tanh form is off by 4.7e-4), and tanh by MUFU.TANH (relative error 2^-11).  6 FMA-pipe instructions + 1 MUFU
+// per element instead of 17 + 2: the epilogue, not the MMAs, bounded the first-pass conv kernels.  v^2 is clamped so
+// the fitted polynomial stays in its monotone range (|v| <= 7; tanh is saturated long before).
+__device__ __forceinline__ float gelu_fast(float v)
+{
+    const float s = fminf(v * v, 49.0f);
+    float pl = fmaf(-3.58006361e-4f, s, 3.70462883e-2f);
+    pl = fmaf(pl, s, 7.97462455e-1f);
+    const float u = v * pl;
+    float t;
+    asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(u));
+    const float hv = 0.5f * v;
+    return fmaf(hv, t, hv);
+}
+
 __device__ __forceinline__ float apply_act(float v, int act) { return act == ACT_GELU ? gelu_erf(v) : v; }
 
 // Destination element offset of packed output column n of input pixel (img, y, x); EPI_NHWC / EPI_PS2 only.

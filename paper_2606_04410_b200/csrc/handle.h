@@ -13,6 +13,7 @@ struct ufnvc_handle {
     int num_sms = 0;
     int max_chunks = 1;
     bool weights_loaded = false;
+    bool use_halo = true;                // env UFNVC_HALO=0: first-pass implicit-GEMM kernel for the 3x3 convs (A/B test)
     bool force_generic = false;          // env UFNVC_FORCE_GENERIC=1: CUDA-core convs everywhere (cross-check)
     std::string err;
 
@@ -32,7 +33,7 @@ struct ufnvc_handle {
     ufnvc::ConvLayer dec[4];             // groups = T
 
     // workspace (sized for max_chunks)
-    double *hx0 = nullptr, *hx1 = nullptr, *hx2 = nullptr;
+    double *hx0 = nullptr, *hx1 = nullptr, *hx2 = nullptr, *hpart = nullptr;
     float *mu = nullptr, *lnscale = nullptr;
     uint8_t *idx = nullptr;
     ufnvc::bf16 *yhat = nullptr, *fa = nullptr, *fb = nullptr, *hidden = nullptr;
@@ -44,6 +45,8 @@ struct ufnvc_handle {
         int tile_h = 0, tile_w = 0;
         bool flat = false;               // 1x1 convs: all pixels of all images as one [rows][128] matrix
         bool ok = false;
+        CUtensorMap tm_halo;             // 3x3 convs: box {64, 10, 18}: a 16 x 8 pixel tile plus halo (conv_halo_kernel)
+        bool halo_ok = false;
     };
     ActMap am_yhat, am_fa, am_fb, am_hidden, am_stage[3];
 

@@ -31,6 +31,32 @@ struct HyperEpi {
     HeadParams hp;
 };
 
+// ReLU -> NHWC double (mode 0), or the head (mode 1): O2 / R14 pixel-shuffle x4 + crop + split + clamp + bucket.
+__device__ __forceinline__ void hyper_epilogue(const HyperEpi &epi, double v, int m, int o, int pz, int wz, int n_out)
+{
+    if (epi.mode == 0) {
+        epi.out[(long long)m * n_out + o] = v > 0.0 ? v : 0.0;
+        return;
+    }
+    // pre-shuffle channel o = c2*16 + 4i + j at z-pixel (zy, zx) -> latent (4zy+i, 4zx+j), channel c2.
+    const HeadParams &hp = epi.hp;
+    const int img = m / pz, p = m % pz, zy = p / wz, zx = p % wz;
+    const int c2 = o >> 4, ly = 4 * zy + ((o >> 2) & 3), lx = 4 * zx + (o & 3);
+    if (ly >= hp.h || lx >= hp.w) return;                                   // crop [R2]
+    if (c2 < hp.c_y) {
+        hp.mu[(((long long)img * hp.h + ly) * hp.w + lx) * hp.c_y + c2] = float(v);
+    } else {
+        const long long e = (((long long)img * hp.h + ly) * hp.w + lx) * hp.c_y + (c2 - hp.c_y);
+        const double u = v < hp.ln_lo ? hp.ln_lo : (v > hp.ln_hi ? hp.ln_hi : v);
+        // same operation order as the definition: floor((nb-1)*(u-lo)/(hi-lo) + 0.5), in double
+        const double t = floor(double(hp.n_buckets - 1) * (u - hp.ln_lo) / (hp.ln_hi - hp.ln_lo) + 0.5);
+        int k = int(t);
+        k = k < 0 ? 0 : (k > hp.n_buckets - 1 ? hp.n_buckets - 1 : k);
+        hp.idx[e] = uint8_t(k);
+        if (hp.lnscale) hp.lnscale[e] = float(u);
+    }
+}
+
 __global__ void __launch_bounds__(256) hyper_conv_kernel(const double *__restrict__ in, const double *__restrict__ wt,
                                                          const double *__restrict__ bias, int n_img, int hz, int wz,
                                                          int c_in, int n_out, HyperEpi epi)
@@ -92,29 +118,115 @@ __global__ void __launch_bounds__(256) hyper_conv_kernel(const double *__restric
         for (int j = 0; j < 4; ++j) {
             const int o = n0 + tx * 4 + j;
             if (o >= n_out) continue;
-            const double v = acc[i][j] + bias[o];
-            if (epi.mode == 0) {
-                epi.out[(long long)m * n_out + o] = v > 0.0 ? v : 0.0;
+            hyper_epilogue(epi, acc[i][j] + bias[o], m, o, pz, wz, n_out);
+        }
+    }
+}
+
+
+// ---- fast path: 64 x 64 tile, 256 threads, 4 x 4 doubles per thread, K step 16, register-prefetch double buffering.
+// Requires c_in % 16 == 0 (a K step never straddles a tap) and n_out % 4 == 0.  DFMA-pipe bound by design: per warp
+// and k, 2 broadcast A vectors + 512 B of conflict-free B feed 512 DFMAs.  SPLIT = true: blockIdx.z = tap, raw partial
+// sums go to part[tap][M][n_out] and hyper_reduce_kernel adds them in tap order (deterministic), for the two small
+// layers that would otherwise occupy 16 CTAs.
+constexpr int FM = 64, FN = 64, FK = 16, FPAD = 2;
+
+template <bool SPLIT>
+__global__ void __launch_bounds__(256) hyper_conv_fast_kernel(const double *__restrict__ in, const double *__restrict__ wt,
+                                                              const double *__restrict__ bias, int n_img, int hz, int wz,
+                                                              int c_in, int n_out, HyperEpi epi, double *__restrict__ part)
+{
+    __shared__ __align__(16) double As[2][FK][FM + FPAD];
+    __shared__ __align__(16) double Bs[2][FK][FN];
+    const int pz = hz * wz;
+    const int M = n_img * pz;
+    const int m0 = blockIdx.x * FM, n0 = blockIdx.y * FN;
+    const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
+
+    // loaders: A 64 px x 16 k (4 consecutive k per thread), B 16 k x 64 n (4 consecutive n per thread)
+    const int a_pix = tid >> 2, a_k = (tid & 3) * 4;
+    const int gm = m0 + a_pix;
+    const int a_img = gm < M ? gm / pz : 0, a_p = gm < M ? gm % pz : 0;
+    const int a_y = a_p / wz, a_x = a_p % wz;
+    const int b_k = tid >> 4, b_n = (tid & 15) * 4;
+    const bool b_ok = n0 + b_n < n_out;
+
+    const int tap_lo = SPLIT ? blockIdx.z : 0, tap_hi = SPLIT ? blockIdx.z + 1 : 9;
+    const int ksteps_per_tap = c_in / FK;
+    const int total_steps = (tap_hi - tap_lo) * ksteps_per_tap;
+
+    double2 ra[2], rb[2];
+    auto gload = [&](int step) {
+        const int tap = tap_lo + step / ksteps_per_tap, k0 = (step % ksteps_per_tap) * FK;
+        const int yy = a_y + tap / 3 - 1, xx = a_x + tap % 3 - 1;
+        const bool a_ok = gm < M && yy >= 0 && yy < hz && xx >= 0 && xx < wz;
+        ra[0] = ra[1] = make_double2(0.0, 0.0);
+        if (a_ok) {
+            const double2 *src = reinterpret_cast<const double2 *>(in + ((long long)a_img * pz + (long long)yy * wz + xx) * c_in + k0 + a_k);
+            ra[0] = src[0]; ra[1] = src[1];
+        }
+        rb[0] = rb[1] = make_double2(0.0, 0.0);
+        if (b_ok) {
+            const double2 *src = reinterpret_cast<const double2 *>(wt + ((long long)tap * c_in + k0 + b_k) * n_out + n0 + b_n);
+            rb[0] = src[0]; rb[1] = src[1];
+        }
+    };
+    auto sstore = [&](int buf) {
+        As[buf][a_k + 0][a_pix] = ra[0].x; As[buf][a_k + 1][a_pix] = ra[0].y;
+        As[buf][a_k + 2][a_pix] = ra[1].x; As[buf][a_k + 3][a_pix] = ra[1].y;
+        *reinterpret_cast<double2 *>(&Bs[buf][b_k][b_n]) = rb[0];
+        *reinterpret_cast<double2 *>(&Bs[buf][b_k][b_n + 2]) = rb[1];
+    };
+
+    double acc[4][4] = {};
+    gload(0);
+    sstore(0);
+    __syncthreads();
+    for (int step = 0; step < total_steps; ++step) {
+        const int buf = step & 1;
+        if (step + 1 < total_steps) gload(step + 1);
+#pragma unroll
+        for (int k = 0; k < FK; ++k) {
+            const double2 a01 = *reinterpret_cast<const double2 *>(&As[buf][k][ty * 4]);
+            const double2 a23 = *reinterpret_cast<const double2 *>(&As[buf][k][ty * 4 + 2]);
+            const double2 b01 = *reinterpret_cast<const double2 *>(&Bs[buf][k][tx * 2]);          // columns 2tx, 2tx+1
+            const double2 b23 = *reinterpret_cast<const double2 *>(&Bs[buf][k][32 + tx * 2]);     // columns 32+2tx, 33+2tx
+            const double a[4] = {a01.x, a01.y, a23.x, a23.y}, b[4] = {b01.x, b01.y, b23.x, b23.y};
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) acc[i][j] = fma(a[i], b[j], acc[i][j]);
+        }
+        if (step + 1 < total_steps) sstore(buf ^ 1);
+        __syncthreads();
+    }
+
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int m = m0 + ty * 4 + i;
+        if (m >= M) continue;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int o = n0 + (j < 2 ? tx * 2 + j : 32 + tx * 2 + (j - 2));
+            if (o >= n_out) continue;
+            if (SPLIT) {
+                part[((long long)blockIdx.z * M + m) * n_out + o] = acc[i][j];
             } else {
-                // O2 / R14: pre-shuffle channel o = c2*16 + 4i + j at z-pixel (zy, zx) -> latent (4zy+i, 4zx+j), c2.
-                const HeadParams &hp = epi.hp;
-                const int img = m / pz, p = m % pz, zy = p / wz, zx = p % wz;
-                const int c2 = o >> 4, ly = 4 * zy + ((o >> 2) & 3), lx = 4 * zx + (o & 3);
-                if (ly >= hp.h || lx >= hp.w) continue;                        // crop [R2]
-                if (c2 < hp.c_y) {
-                    hp.mu[(((long long)img * hp.h + ly) * hp.w + lx) * hp.c_y + c2] = float(v);
-                } else {
-                    const long long e = (((long long)img * hp.h + ly) * hp.w + lx) * hp.c_y + (c2 - hp.c_y);
-                    double u = v < hp.ln_lo ? hp.ln_lo : (v > hp.ln_hi ? hp.ln_hi : v);
-                    // same operation order as the definition: floor((nb-1)*(u-lo)/(hi-lo) + 0.5), in double
-                    const double t = floor(double(hp.n_buckets - 1) * (u - hp.ln_lo) / (hp.ln_hi - hp.ln_lo) + 0.5);
-                    int k = int(t);
-                    k = k < 0 ? 0 : (k > hp.n_buckets - 1 ? hp.n_buckets - 1 : k);
-                    hp.idx[e] = uint8_t(k);
-                    if (hp.lnscale) hp.lnscale[e] = float(u);
-                }
+                hyper_epilogue(epi, acc[i][j] + bias[o], m, o, pz, wz, n_out);
             }
         }
+    }
+}
+
+__global__ void hyper_reduce_kernel(const double *__restrict__ part, const double *__restrict__ bias, double *__restrict__ out,
+                                    long long MN, int n_out)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < MN; i += (long long)gridDim.x * blockDim.x) {
+        double v = part[i];
+#pragma unroll
+        for (int t = 1; t < 9; ++t) v += part[t * MN + i];                   // fixed tap order: run-to-run deterministic
+        v += bias[i % n_out];
+        out[i] = v > 0.0 ? v : 0.0;
     }
 }
 
@@ -126,13 +238,24 @@ cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z
     return cudaGetLastError();
 }
 
-cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out, int n_img, int hz, int wz,
+static bool fast_ok(const HyperLayer &L) { return L.c_in % FK == 0 && L.n % 4 == 0; }
+
+cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out, double *part, int n_img, int hz, int wz,
                               cudaStream_t st)
 {
     HyperEpi e{};
     e.mode = 0;
     e.out = out;
-    dim3 grid((n_img * hz * wz + HM - 1) / HM, (L.n + HN - 1) / HN);
+    const int M = n_img * hz * wz;
+    if (fast_ok(L) && part) {                   // split over the 9 taps, then a deterministic reduce + bias + ReLU
+        dim3 grid((M + FM - 1) / FM, (L.n + FN - 1) / FN, 9);
+        hyper_conv_fast_kernel<true><<<grid, 256, 0, st>>>(in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e, part);
+        const long long MN = (long long)M * L.n;
+        const int blocks = int((MN + 255) / 256 < 1184 ? (MN + 255) / 256 : 1184);
+        hyper_reduce_kernel<<<blocks, 256, 0, st>>>(part, L.bias, out, MN, L.n);
+        return cudaGetLastError();
+    }
+    dim3 grid((M + HM - 1) / HM, (L.n + HN - 1) / HN);
     hyper_conv_kernel<<<grid, 256, 0, st>>>(in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e);
     return cudaGetLastError();
 }
@@ -144,7 +267,13 @@ cudaError_t launch_hyper_head(const HyperLayer &L, const double *in, int n_img, 
     e.mode = 1;
     e.out = nullptr;
     e.hp = hp;
-    dim3 grid((n_img * hz * wz + HM - 1) / HM, (L.n + HN - 1) / HN);
+    const int M = n_img * hz * wz;
+    if (fast_ok(L)) {
+        dim3 grid((M + FM - 1) / FM, (L.n + FN - 1) / FN);
+        hyper_conv_fast_kernel<false><<<grid, 256, 0, st>>>(in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e, nullptr);
+        return cudaGetLastError();
+    }
+    dim3 grid((M + HM - 1) / HM, (L.n + HN - 1) / HN);
     hyper_conv_kernel<<<grid, 256, 0, st>>>(in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e);
     return cudaGetLastError();
 }

@@ -17,7 +17,7 @@ struct RansSmem {
     uint16_t lut[64 * 256];
 };
 
-__global__ void __launch_bounds__(1024) rans_decode_kernel(RansParams p, int nb)
+__global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     uint16_t *s_cdf = reinterpret_cast<uint16_t *>(smem_raw);
@@ -63,24 +63,30 @@ __global__ void __launch_bounds__(1024) rans_decode_kernel(RansParams p, int nb)
         x = reinterpret_cast<const uint32_t *>(sb + ws_off)[lane];
         words = reinterpret_cast<const uint16_t *>(sb + ws_off + 128);
     }
-    // word window: w0 = words[qb + lane], w1 = words[qb + 32 + lane]
+    // word window: w0/w1/w2 = words[qb + {0,32,64} + lane]; a step consumes <= 32 words and starts with q - qb < 32,
+    // so it reads w0/w1 only, and the refill of w2 has a whole window period to land.
     uint32_t qb = 0, q = 0;
     uint32_t w0 = (lane < nw) ? words[lane] : 0u;
     uint32_t w1 = (32u + lane < nw) ? words[32 + lane] : 0u;
+    uint32_t w2 = (64u + lane < nw) ? words[64 + lane] : 0u;
 
-    // prefetch step 0
-    int i = g * 32 + lane;
-    uint32_t k_next = 0;
-    float mu_next = 0.f;
-    if (i < n) { k_next = p.idx[ebase + i]; mu_next = p.mu[ebase + i]; }
-
-    for (int j = 0; j < n_steps; ++j) {
-        const bool valid = i < n;
-        const uint32_t k = k_next;
-        const float mu = mu_next;
-        const int i_next = i + p.W;
-        if (i_next < n) { k_next = p.idx[ebase + i_next]; mu_next = p.mu[ebase + i_next]; }
-
+    // idx / mu do not depend on the decoder state: they are fetched kPre steps ahead into two register banks, so the
+    // serial chain of a step holds no global-memory latency (with a 1-deep prefetch every step waited ~800 cycles).
+    constexpr int kPre = 8;
+    const int i0 = g * 32 + lane;
+    uint32_t kA[kPre], kB[kPre];
+    float mA[kPre], mB[kPre];
+    auto fetch = [&](uint32_t (&kk)[kPre], float (&mm)[kPre], int j0) {
+#pragma unroll
+        for (int s = 0; s < kPre; ++s) {
+            const int ii = i0 + (j0 + s) * p.W;
+            kk[s] = 0; mm[s] = 0.f;
+            if (j0 + s < n_steps && ii < n) { kk[s] = p.idx[ebase + ii]; mm[s] = p.mu[ebase + ii]; }
+        }
+    };
+    auto step = [&](uint32_t k, float mu, int j) {
+        const int i = i0 + j * p.W;
+        const bool valid = j < n_steps && i < n;
         const uint32_t slot = x & 0xFFFFu;
         const uint16_t *c = s_cdf + k * 256;
         const uint32_t lh = s_lut[k * 256 + (slot >> 8)];
@@ -94,7 +100,7 @@ __global__ void __launch_bounds__(1024) rans_decode_kernel(RansParams p, int nb)
         uint32_t xn = f * (x >> 16) + slot - cp;
         const bool need = valid && xn < (1u << 16);
         const uint32_t m = __ballot_sync(0xFFFFFFFFu, need);
-        const uint32_t r = q - qb + __popc(m & ((1u << lane) - 1u));     // index into the 64-word window
+        const uint32_t r = q - qb + __popc(m & ((1u << lane) - 1u));     // index into the window, < 64
         const uint32_t wa = __shfl_sync(0xFFFFFFFFu, w0, r & 31);
         const uint32_t wb = __shfl_sync(0xFFFFFFFFu, w1, r & 31);
         if (need) xn = (xn << 16) | (r < 32 ? wa : wb);
@@ -102,9 +108,9 @@ __global__ void __launch_bounds__(1024) rans_decode_kernel(RansParams p, int nb)
         q += __popc(m);
         if (q - qb >= 32) {                     // slide the window (warp-uniform)
             qb += 32;
-            w0 = w1;
-            const uint32_t a = qb + 32 + lane;
-            w1 = (a < nw) ? words[a] : 0u;
+            w0 = w1; w1 = w2;
+            const uint32_t a = qb + 64 + lane;
+            w2 = (a < nw) ? words[a] : 0u;
         }
         if (valid) {
             const int sym = int(lo) - 127;
@@ -113,7 +119,16 @@ __global__ void __launch_bounds__(1024) rans_decode_kernel(RansParams p, int nb)
             if (p.sym_tap) p.sym_tap[ebase + i] = int16_t(sym);
             if (p.yhat_tap) p.yhat_tap[ebase + i] = y;
         }
-        i = i_next;
+    };
+
+    fetch(kA, mA, 0);
+    for (int j0 = 0; j0 < n_steps; j0 += 2 * kPre) {
+        fetch(kB, mB, j0 + kPre);
+#pragma unroll
+        for (int s = 0; s < kPre; ++s) step(kA[s], mA[s], j0 + s);
+        fetch(kA, mA, j0 + 2 * kPre);
+#pragma unroll
+        for (int s = 0; s < kPre; ++s) step(kB[s], mB[s], j0 + kPre + s);
     }
     // end-state invariant (O4): every lane back at 2^16 and every word consumed
     if (__any_sync(0xFFFFFFFFu, x != (1u << 16))) st |= UFNVC_STREAM_BAD_END_STATE;

@@ -63,8 +63,8 @@ struct HyperLayer {
     double *bias = nullptr;  // [n]
 };
 cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z, int pz, cudaStream_t st);
-cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out, int n_img, int hz, int wz,
-                              cudaStream_t st);
+cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out, double *part, int n_img, int hz, int wz,
+                              cudaStream_t st);   // part: [9][M][n] scratch for the split-tap fast path (may be null)
 struct HeadParams {
     int c_y, h, w, n_buckets;
     double ln_lo, ln_hi;
@@ -94,6 +94,9 @@ cudaError_t launch_rans_decode(const RansParams &p, cudaStream_t st);
 // tcgen05 implicit-GEMM conv (conv_tc.cu)
 cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_in, int tile_h, int tile_w,
                            bool flat, const EpiParams &E, int num_sms, cudaStream_t st);
+cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
+                             cudaStream_t st);
+bool tc_make_halo_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, std::string &err);
 bool tc_make_weight_tmap(ConvLayer &L, std::string &err);
 bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, int tile_h, int tile_w,
                       std::string &err);
