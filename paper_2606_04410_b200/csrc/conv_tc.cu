@@ -117,6 +117,19 @@ __device__ __forceinline__ void umma_commit(uint32_t bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
+// One elected lane of a converged warp.  Unlike `lane == 0`, the compiler knows exactly one thread is active inside the
+// branch, so tcgen05.mma / TMA operands live in uniform registers without a per-instruction "waterfall" loop (with
+// `lane == 0` every UTCHMMA cost ~25 SASS instructions of ELECT / BRA.U.ANY: the A9 kernel was bound by MMA issue).
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred P1;\n\t"
+        "elect.sync _|P1, 0xFFFFFFFF;\n\t"
+        "selp.b32 %0, 1, 0, P1;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 
@@ -314,7 +327,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant
 
     if (warp == 0) {
         // ===================== TMA producer =====================
-        if (lane == 0) {
+        if (elect_one()) {
             int stage = 0; uint32_t phase = 0;
             for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x) {
                 const TileCoord tc = tile_coord(p, tile);
@@ -333,7 +346,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant
         }
     } else if (warp == 1) {
         // ===================== MMA issuer =====================
-        if (lane == 0) {
+        if (elect_one()) {
             const uint32_t idesc = umma_idesc_bf16(kTileM, p.BN);
             int stage = 0; uint32_t phase = 0;
             int it = 0;
@@ -439,7 +452,7 @@ conv_halo_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
 
     if (warp == 0) {
         // ===================== TMA producer =====================
-        if (lane == 0) {
+        if (elect_one()) {
             int sa = 0, sb = 0; uint32_t pa = 0, pb = 0, pfree = 0;
             int prev_key = -1;
             for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x) {
@@ -475,7 +488,7 @@ conv_halo_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
         }
     } else if (warp == 1) {
         // ===================== MMA issuer =====================
-        if (lane == 0) {
+        if (elect_one()) {
             const uint32_t idesc = umma_idesc_bf16(kTileM, p.BN);
             int sa = 0, sb = 0; uint32_t pa = 0, pb = 0, pres = 0;
             int prev_key = -1;
