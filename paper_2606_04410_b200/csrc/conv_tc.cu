@@ -30,7 +30,27 @@ constexpr int kABytes = kTileM * kSlabK * 2;     // 16 KB
 constexpr int kThreads = 320;                    // warp 0 TMA, warp 1 MMA, warps 2..9 epilogue
 constexpr uint32_t kSpinLimit = 1u << 28;
 
+// n / d for 0 <= n < 2^31 as one multiply-high, one add and one shift (Granlund-Montgomery round-up method): the
+// per-tile index arithmetic sits on the single-thread MMA-issue path, where a hardware-emulated division costs ~40
+// dependent instructions.
+struct FastDiv {
+    uint32_t d, mul, shr;
+    __device__ __forceinline__ uint32_t div(uint32_t n) const { return (__umulhi(n, mul) + n) >> shr; }
+    __device__ __forceinline__ void divmod(uint32_t n, uint32_t &q, uint32_t &r) const { q = div(n); r = n - q * d; }
+};
+static FastDiv make_fastdiv(uint32_t d)
+{
+    FastDiv f;
+    f.d = d;
+    uint32_t l = 0;
+    while ((1ull << l) < d) ++l;
+    f.mul = uint32_t(((1ull << 32) * ((1ull << l) - d)) / d + 1);
+    f.shr = l;
+    return f;
+}
+
 struct TcParams {
+    FastDiv fd_ntiles, fd_tx, fd_ty, fd_groups;
     int n_img_m, Hm, Wm;          // activation as the TMA map sees it (flattened for 1x1 convs)
     int flat, tw_shift;           // flat: rows of 128 consecutive pixels; tw_shift = log2(TW)
     int tiles_y, tiles_x, TH, TW;
@@ -113,6 +133,20 @@ __device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t da, uint64_t
         ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
         : "memory");
 }
+// Same, descriptors given as (lo, hi) 32-bit halves: only the 14-bit start-address field of lo changes between MMAs,
+// so the issue loop is one 32-bit add per operand.
+__device__ __forceinline__ void umma_bf16_lh(uint32_t tmem_d, uint32_t a_lo, uint32_t a_hi, uint32_t b_lo, uint32_t b_hi,
+                                             uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\t"
+        "setp.ne.b32 p, %6, 0;\n\t"
+        "mov.b64 da, {%1, %2};\n\t"
+        "mov.b64 db, {%3, %4};\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %5, p;\n\t}"
+        ::"r"(tmem_d), "r"(a_lo), "r"(a_hi), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
 __device__ __forceinline__ void umma_commit(uint32_t bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
@@ -163,16 +197,24 @@ namespace {
 
 // tile index -> (image in map space, tile origin, n tile); n fastest so CTAs running side by side share the A tile in L2
 struct TileCoord { int img, y0, x0, nt; };
+__device__ __forceinline__ int group_of(const TcParams &p, int img)
+{
+    if (p.groups == 1) return 0;
+    uint32_t q, r;
+    p.fd_groups.divmod(uint32_t(img), q, r);
+    return int(r);
+}
 __device__ __forceinline__ TileCoord tile_coord(const TcParams &p, int tile)
 {
     TileCoord c;
-    c.nt = tile % p.n_tiles;
-    int r = tile / p.n_tiles;
-    const int tx = r % p.tiles_x; r /= p.tiles_x;
-    const int ty = r % p.tiles_y;
-    c.img = r / p.tiles_y;
-    c.y0 = ty * p.TH;
-    c.x0 = tx * p.TW;
+    uint32_t r, nt, tx, ty, img;
+    p.fd_ntiles.divmod(uint32_t(tile), r, nt);
+    p.fd_tx.divmod(r, r, tx);
+    p.fd_ty.divmod(r, img, ty);
+    c.nt = int(nt);
+    c.img = int(img);
+    c.y0 = int(ty) * p.TH;
+    c.x0 = int(tx) * p.TW;
     return c;
 }
 
@@ -204,7 +246,7 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
             y = int(rem / unsigned(p.W));
             x = int(rem - unsigned(y) * unsigned(p.W));
         }
-        const int grp = p.groups == 1 ? 0 : img % p.groups;
+        const int grp = group_of(p, img);
         const float *bias = p.bias + (long long)grp * p.n_pad + tc.nt * p.BN;
         mbar_wait(tfull0 + 8u * acc, acc_phase);
         tc_fence_after();
@@ -331,7 +373,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant
             int stage = 0; uint32_t phase = 0;
             for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x) {
                 const TileCoord tc = tile_coord(p, tile);
-                const int grp = p.groups == 1 ? 0 : tc.img % p.groups;
+                const int grp = group_of(p, tc.img);
                 for (int kb = 0; kb < kblocks; ++kb) {
                     const int tap = kb / p.slabs, slab = kb - tap * p.slabs;
                     const int dy = p.taps == 9 ? tap / 3 - 1 : 0, dx = p.taps == 9 ? tap % 3 - 1 : 0;
@@ -404,19 +446,20 @@ __device__ __forceinline__ uint64_t umma_desc_sw128_sbo(uint32_t saddr, uint32_t
            (uint64_t(2) << 61);
 }
 
-template <int MODE>
+template <int MODE, bool RESIDENT>
 __global__ void __launch_bounds__(kThreads, 1)
 conv_halo_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b, const TcParams p,
-                 const int nb_stages, const int b_resident)
+                 const int nb_stages, const int na_stages)
 {
+    constexpr bool b_resident = RESIDENT;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t b_bytes = uint32_t(p.BN) * 128u;                             // multiple of 2 KB
-    const uint32_t b_base = smem_base + kHaloAStages * kHaloStage;
+    const uint32_t b_base = smem_base + na_stages * kHaloStage;
     const uint32_t bar_base = b_base + uint32_t(nb_stages) * b_bytes;
     auto afull = [&](int s) { return bar_base + 8u * s; };
-    auto aempty = [&](int s) { return bar_base + 8u * (kHaloAStages + s); };
-    const uint32_t misc = bar_base + 8u * (2 * kHaloAStages);
+    auto aempty = [&](int s) { return bar_base + 8u * (na_stages + s); };
+    const uint32_t misc = bar_base + 8u * (2 * na_stages);
     const uint32_t tfull0 = misc, tempty0 = misc + 16u, bres_full = misc + 32u, bfree = misc + 40u, tmem_slot = misc + 48u;
     const uint32_t bbar = misc + 64u;
     auto bfull = [&](int s) { return bbar + 8u * s; };
@@ -431,7 +474,7 @@ conv_halo_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_a) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_b) : "memory");
-        for (int s = 0; s < kHaloAStages; ++s) { mbar_init(afull(s), 1); mbar_init(aempty(s), 1); }
+        for (int s = 0; s < na_stages; ++s) { mbar_init(afull(s), 1); mbar_init(aempty(s), 1); }
         for (int s = 0; s < nb_stages; ++s) { mbar_init(bfull(s), 1); mbar_init(bempty(s), 1); }
         for (int a = 0; a < 2; ++a) { mbar_init(tfull0 + 8u * a, 1); mbar_init(tempty0 + 8u * a, 8); }
         mbar_init(bres_full, 1);
@@ -448,7 +491,7 @@ conv_halo_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     const uint32_t tmem_base = *tmem_slot_ptr;
 
     // weight-set key of a tile: resident weights are reloaded only when it changes
-    auto tile_key = [&](const TileCoord &tc) { return (p.groups == 1 ? 0 : tc.img % p.groups) * p.n_tiles + tc.nt; };
+    auto tile_key = [&](const TileCoord &tc) { return group_of(p, tc.img) * p.n_tiles + tc.nt; };
 
     if (warp == 0) {
         // ===================== TMA producer =====================
@@ -457,7 +500,7 @@ conv_halo_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
             int prev_key = -1;
             for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x) {
                 const TileCoord tc = tile_coord(p, tile);
-                const int grp = p.groups == 1 ? 0 : tc.img % p.groups;
+                const int grp = group_of(p, tc.img);
                 if (b_resident) {
                     const int key = tile_key(tc);
                     if (key != prev_key) {
@@ -474,7 +517,7 @@ conv_halo_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
                     mbar_wait(aempty(sa), pa ^ 1);
                     mbar_expect_tx(afull(sa), kHaloBytes);
                     tma_load_4d(smem_base + sa * kHaloStage, &tmap_a, afull(sa), slab * kSlabK, tc.x0 - 1, tc.y0 - 1, tc.img);
-                    if (++sa == kHaloAStages) { sa = 0; pa ^= 1; }
+                    if (++sa == na_stages) { sa = 0; pa ^= 1; }
                     if (!b_resident) {
                         for (int tap = 0; tap < 9; ++tap) {
                             mbar_wait(bempty(sb), pb ^ 1);
@@ -490,11 +533,17 @@ conv_halo_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
         // ===================== MMA issuer =====================
         if (elect_one()) {
             const uint32_t idesc = umma_idesc_bf16(kTileM, p.BN);
+            // descriptor halves: lo = start >> 4 | LBO(1) << 16; hi = SBO >> 4 | version 1 << 14 | SWIZZLE_128B << 29
+            const uint32_t a_hi = uint32_t(kHaloRowPitch >> 4) | (1u << 14) | (2u << 29);
+            const uint32_t b_hi = uint32_t(1024 >> 4) | (1u << 14) | (2u << 29);
+            const uint32_t a_lo0 = ((smem_base & 0x3FFFFu) >> 4) | (1u << 16);
+            const uint32_t b_lo0 = ((b_base & 0x3FFFFu) >> 4) | (1u << 16);
+            const uint32_t b_step = b_bytes >> 4;
             int sa = 0, sb = 0; uint32_t pa = 0, pb = 0, pres = 0;
             int prev_key = -1;
             int it = 0;
+            TileCoord tc = tile_coord(p, blockIdx.x);
             for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x, ++it) {
-                const TileCoord tc = tile_coord(p, tile);
                 const int acc = it & 1;
                 const uint32_t acc_phase = (it >> 1) & 1;
                 if (b_resident) {
@@ -507,33 +556,34 @@ conv_halo_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
                 for (int slab = 0; slab < p.slabs; ++slab) {
                     mbar_wait(afull(sa), pa);
                     tc_fence_after();
-                    const uint32_t a_src = smem_base + sa * kHaloStage;
+                    const uint32_t a_lo = a_lo0 + uint32_t(sa) * (kHaloStage >> 4);
+                    uint32_t b_lo = b_lo0 + uint32_t(slab * 9) * b_step;                 // resident: tile (slab, tap)
+#pragma unroll
                     for (int tap = 0; tap < 9; ++tap) {
-                        uint32_t b_src;
-                        if (b_resident) {
-                            b_src = b_base + uint32_t(slab * 9 + tap) * b_bytes;
-                        } else {
+                        if (!b_resident) {
                             mbar_wait(bfull(sb), pb);
                             tc_fence_after();
-                            b_src = b_base + uint32_t(sb) * b_bytes;
+                            b_lo = b_lo0 + uint32_t(sb) * b_step;
                         }
-                        const uint32_t a_tap = a_src + uint32_t((tap / 3) * (kHaloTW + 2) + tap % 3) * 128u;
-                        const uint64_t da = umma_desc_sw128_sbo(a_tap, kHaloRowPitch), db = umma_desc_sw128(b_src);
+                        const uint32_t a_tap = a_lo + uint32_t(((tap / 3) * (kHaloTW + 2) + tap % 3) * 128 >> 4);
 #pragma unroll
-                        for (int k = 0; k < kSlabK / 16; ++k)
-                            umma_bf16(d_tmem, da + uint64_t(2 * k), db + uint64_t(2 * k), idesc, (slab | tap | k) != 0);
+                        for (int k = 0; k < kSlabK / 16; ++k)                              // 32 bytes = +2 descriptor units
+                            umma_bf16_lh(d_tmem, a_tap + 2 * k, a_hi, b_lo + 2 * k, b_hi, idesc, uint32_t(slab | tap | k));
                         if (!b_resident) {
                             umma_commit(bempty(sb));
                             if (++sb == nb_stages) { sb = 0; pb ^= 1; }
+                        } else {
+                            b_lo += b_step;
                         }
                     }
                     umma_commit(aempty(sa));
-                    if (++sa == kHaloAStages) { sa = 0; pa ^= 1; }
+                    if (++sa == na_stages) { sa = 0; pa ^= 1; }
                 }
                 umma_commit(tfull0 + 8u * acc);
-                if (b_resident) {                                               // release the weights if the next tile swaps them
-                    const int next = tile + gridDim.x;
-                    if (next < p.total_tiles && tile_key(tile_coord(p, next)) != prev_key) umma_commit(bfree);
+                const int next = tile + gridDim.x;
+                if (next < p.total_tiles) {
+                    tc = tile_coord(p, next);
+                    if (b_resident && tile_key(tc) != prev_key) umma_commit(bfree);      // the next tile swaps the weights
                 }
             }
         }
@@ -629,19 +679,24 @@ cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUt
     p.BN = L.block_n; p.n_tiles = L.n_pad / L.block_n; p.n_real = L.n; p.n_pad = L.n_pad;
     p.groups = L.groups;
     p.total_tiles = p.n_img_m * p.tiles_y * p.tiles_x * p.n_tiles;
+    p.fd_ntiles = make_fastdiv(p.n_tiles); p.fd_tx = make_fastdiv(p.tiles_x); p.fd_ty = make_fastdiv(p.tiles_y);
+    p.fd_groups = make_fastdiv(p.groups);
     p.bias = L.bias;
     p.E = E;
     const size_t b_bytes = size_t(L.block_n) * 128;
-    const size_t budget = 227 * 1024 - 1024 - size_t(kHaloAStages) * kHaloStage - 1024;
+    int na = kHaloAStages;
+    const size_t budget = 227 * 1024 - 1024 - size_t(na) * kHaloStage - 1024;
     const int btiles = 9 * p.slabs;
     int nb = int(budget / b_bytes);
     const int resident = btiles <= nb ? 1 : 0;
     if (resident) nb = btiles; else if (nb > 8) nb = 8;
     if (nb < 2) return cudaErrorInvalidValue;
-    const size_t smem = 1024 + size_t(kHaloAStages) * kHaloStage + size_t(nb) * b_bytes + 128 + 16 * size_t(nb) + 64;
+    // small resident weights (A9) leave room: deepen the A ring so more halo loads are in flight per SM
+    while (na < 8 && 1024 + size_t(na + 1) * kHaloStage + size_t(nb) * b_bytes + 2048 <= 227 * 1024) ++na;
+    const size_t smem = 1024 + size_t(na) * kHaloStage + size_t(nb) * b_bytes + 256 + 16 * size_t(nb) + 16 * size_t(na);
     const int grid = p.total_tiles < num_sms ? p.total_tiles : num_sms;
     auto launch = [&](auto kern) -> cudaError_t {
-        static thread_local const void *configured[8] = {};
+        static thread_local const void *configured[16] = {};
         bool done = false;
         for (const void *c : configured) done |= (c == (const void *)kern);
         if (!done) {
@@ -649,13 +704,13 @@ cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUt
             if (e != cudaSuccess) return e;
             for (auto &c : configured) if (!c) { c = (const void *)kern; break; }
         }
-        kern<<<grid, kThreads, smem, st>>>(tmap_halo, L.tmap_w, p, nb, resident);
+        kern<<<grid, kThreads, smem, st>>>(tmap_halo, L.tmap_w, p, nb, na);
         return cudaGetLastError();
     };
     switch (E.mode) {
-        case EPI_NHWC: return launch(conv_halo_kernel<EPI_NHWC>);
-        case EPI_PS2: return launch(conv_halo_kernel<EPI_PS2>);
-        default: return launch(conv_halo_kernel<EPI_FINAL>);
+        case EPI_NHWC: return resident ? launch(conv_halo_kernel<EPI_NHWC, true>) : launch(conv_halo_kernel<EPI_NHWC, false>);
+        case EPI_PS2: return resident ? launch(conv_halo_kernel<EPI_PS2, true>) : launch(conv_halo_kernel<EPI_PS2, false>);
+        default: return resident ? launch(conv_halo_kernel<EPI_FINAL, true>) : launch(conv_halo_kernel<EPI_FINAL, false>);
     }
 }
 
@@ -680,12 +735,14 @@ cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUten
     p.BN = L.block_n; p.n_tiles = L.n_pad / L.block_n; p.n_real = L.n; p.n_pad = L.n_pad;
     p.groups = L.groups;
     p.total_tiles = p.n_img_m * p.tiles_y * p.tiles_x * p.n_tiles;
+    p.fd_ntiles = make_fastdiv(p.n_tiles); p.fd_tx = make_fastdiv(p.tiles_x); p.fd_ty = make_fastdiv(p.tiles_y);
+    p.fd_groups = make_fastdiv(p.groups);
     p.bias = L.bias;
     p.E = E;
     const size_t smem = size_t(kStages) * (kABytes + size_t(L.block_n) * 128) + 1024 + 256;
     const int grid = p.total_tiles < num_sms ? p.total_tiles : num_sms;
     auto launch = [&](auto kern) -> cudaError_t {
-        static thread_local const void *configured[8] = {};
+        static thread_local const void *configured[16] = {};
         bool done = false;
         for (const void *c : configured) done |= (c == (const void *)kern);
         if (!done) {
