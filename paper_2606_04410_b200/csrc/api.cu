@@ -78,6 +78,8 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     h->force_generic = fg && fg[0] == '1';
     const char *hl = std::getenv("UFNVC_HALO");
     h->use_halo = !(hl && hl[0] == '0');
+    const char *ft = std::getenv("UFNVC_FUSED_TRUNK");
+    h->use_fused_trunk = !(ft && ft[0] == '0');
 
     // O3 tables + search accelerator
     build_cdf_tables(cfg->n_buckets, cfg->scale_min, cfg->scale_max, h->cdf32);

@@ -95,6 +95,11 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
         const ufnvc_handle::TrunkBlock &tb = h->trunk[k];
         CU_TRY(launch_dwconv3x3(h->fa, h->fb, tb.dw_w, tb.dw_b, n * T, h->h, h->w, Ct, st));
         if (launches) ++*launches;
+        if (h->use_fused_trunk && tb.fused.ok && !h->force_generic) {
+            CU_TRY(launch_trunk_mlp(tb.fused, tb.pw1, tb.pw2, h->fa, h->fa, (long long)n * T * P, h->num_sms, st));
+            if (launches) ++*launches;
+            continue;
+        }
         ConvProblem p1{h->fb, n * T, h->h, h->w, 1};
         EpiParams E1{EPI_NHWC, ACT_GELU, h->hidden, nullptr, Ce, 0, (long long)P * Ce, 0, 0, 0};
         CU_TRY(conv(h, tb.pw1, p1, h->am_fb, E1, st, launches));
@@ -192,6 +197,8 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
          make_act_map(h, h->am_fb, h->fb, n * T, h->h, h->w, c.c_trunk, true, T) &&
          make_act_map(h, h->am_hidden, h->hidden, n * T, h->h, h->w, c.c_trunk * c.trunk_expand, true, T) &&
          make_act_map(h, h->am_fa, h->fa, n * T, h->h, h->w, c.c_trunk, false, T);
+    for (auto &tb : h->trunk)
+        if (ok && !trunk_make_maps(tb.fused, h->fb, (long long)n * T * h->h * h->w, tb.pw1, tb.pw2, h->err)) ok = false;
     for (int s = 0; ok && s < 3; ++s)
         ok = make_act_map(h, h->am_stage[s], h->stage[s], n * T, h->h << (s + 1), h->w << (s + 1), c.dec_channels[s + 1], false, T);
     if (!ok) return fail(h, UFNVC_E_CUDA, h->err);

@@ -1,0 +1,324 @@
+// A7: the trunk DC block's MLP as ONE tcgen05 kernel ("DC block"):
+//
+//     out = x + W2 * GELU(W1 * d + b1) + b2,      d = depthwise(x) [A6],  256 -> 1024 -> 256, per pixel
+//
+// Unfused, the 1024-wide hidden tensor makes a 268 MB HBM round trip per block and the block is bandwidth-bound
+// (DESIGN.md section 6).  Here a CTA owns 128 pixels and walks the hidden dimension in chunks of 128 columns:
+//
+//   GEMM1(c): Hacc[c&1] (TMEM, 128 x 128 fp32)  = d_tile (smem, 128 x 256)  x  W1[c]^T   (4 slabs x 4 UMMAs, N = 128)
+//   epi(c):   Hacc -> registers -> +b1 -> GELU -> bf16 -> Hs[c&1] (smem, written directly in the K-major SWIZZLE_128B
+//             layout tcgen05.mma reads; fence.proxy.async hands it to the tensor core)
+//   GEMM2(c): Oacc (TMEM, 128 x 256 fp32)      += Hs[c&1] (128 x 128)  x  W2[:, c]^T     (2 slabs x 4 UMMAs, N = 256)
+//
+// The MMA warp issues GEMM1(c+1) before GEMM2(c), so the tensor core always has a GEMM to run while the epilogue warps
+// do the GELU of chunk c.  TMEM: 256 (Oacc) + 2 x 128 (Hacc) = all 512 columns.  Shared memory: d tile 64 KB, Hs
+// 2 x 32 KB, weight ring 3 x 32 KB (W1 and W2 chunks stream through it in the order the MMA warp consumes them).
+// warp 0 = TMA producer, warp 1 = MMA issuer + TMEM allocator, warps 2..9 = epilogue.  Persistent, grid = #SMs.
+#include <cuda.h>
+
+#include "epilogue.cuh"
+#include "tc_ptx.cuh"
+#include "ufnvc_internal.h"
+
+namespace ufnvc {
+
+namespace {
+
+constexpr int kC = 256;                  // trunk width: K of GEMM1, N of GEMM2
+constexpr int kHC = 128;                 // hidden columns per chunk
+constexpr int kTM = 128;                 // pixels per tile
+constexpr int kTrunkThreads = 320;
+constexpr int kWStages = 3;
+constexpr uint32_t kSlab = 16384;        // 128 rows x 128 B
+constexpr uint32_t kWStage = 32768;
+constexpr uint32_t kOffA = 0, kOffHs = 4 * kSlab, kOffW = kOffHs + 4 * kSlab, kOffBar = kOffW + kWStages * kWStage;
+constexpr uint32_t kTrunkSmem = kOffBar + 256 + 1024;        // + alignment slack
+
+struct TrunkParams {
+    int n_tiles, n_chunks, n_px;
+    const float *b1, *b2;                // [hidden], [256]
+    const bf16 *x;                       // residual input  [n_px][256]
+    bf16 *out;                           // [n_px][256] (may alias x: a tile reads its own rows before writing them)
+};
+
+// barrier slots (8 bytes each) from kOffBar
+enum : uint32_t {
+    B_AFULL = 0, B_AEMPTY = 1, B_WFULL = 2, B_WEMPTY = 5, B_HACC_FULL = 8, B_HACC_EMPTY = 10, B_HS_FULL = 12, B_HS_EMPTY = 14,
+    B_OFULL = 16, B_OEMPTY = 17, B_TMEM_SLOT = 18
+};
+
+}  // namespace
+
+namespace {
+
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d)
+{
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi)
+{
+    const __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<const uint32_t *>(&h);
+}
+
+__global__ void __launch_bounds__(kTrunkThreads, 1)
+trunk_mlp_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant__ CUtensorMap tm_w1,
+                 const __grid_constant__ CUtensorMap tm_w2, const TrunkParams p)
+{
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    auto bar = [&](uint32_t slot) { return base + kOffBar + 8u * slot; };
+    volatile uint32_t *tmem_slot_ptr =
+        reinterpret_cast<volatile uint32_t *>(smem_raw + (bar(B_TMEM_SLOT) - smem_u32(smem_raw)));
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int NC = p.n_chunks;
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_d) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_w1) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_w2) : "memory");
+        mbar_init(bar(B_AFULL), 1); mbar_init(bar(B_AEMPTY), 1);
+        for (int s = 0; s < kWStages; ++s) { mbar_init(bar(B_WFULL + s), 1); mbar_init(bar(B_WEMPTY + s), 1); }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bar(B_HACC_FULL + b), 1); mbar_init(bar(B_HACC_EMPTY + b), 8);
+            mbar_init(bar(B_HS_FULL + b), 8);   mbar_init(bar(B_HS_EMPTY + b), 1);
+        }
+        mbar_init(bar(B_OFULL), 1); mbar_init(bar(B_OEMPTY), 8);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(bar(B_TMEM_SLOT)), "r"(512u) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===================== TMA producer: d tile, then W1 / W2 chunks in MMA consumption order =====================
+        if (elect_one()) {
+            int ws = 0; uint32_t wp = 0, ap = 0;
+            auto w_slot = [&]() {                                  // claim the next ring stage; returns its smem address
+                mbar_wait(bar(B_WEMPTY + ws), wp ^ 1);
+                mbar_expect_tx(bar(B_WFULL + ws), kWStage);
+                return base + kOffW + uint32_t(ws) * kWStage;
+            };
+            auto w_next = [&]() { if (++ws == kWStages) { ws = 0; wp ^= 1; } };
+            auto load_w1 = [&](int c) {                            // rows c*128.. of W1, k slabs (2st, 2st+1) per stage
+                for (int st = 0; st < 2; ++st) {
+                    const uint32_t dst = w_slot();
+                    tma_load_2d(dst, &tm_w1, bar(B_WFULL + ws), (2 * st) * 64, c * kHC);
+                    tma_load_2d(dst + kSlab, &tm_w1, bar(B_WFULL + ws), (2 * st + 1) * 64, c * kHC);
+                    w_next();
+                }
+            };
+            auto load_w2 = [&](int c) {                            // all 256 rows of W2, k slab c*128 + st*64 per stage
+                for (int st = 0; st < 2; ++st) {
+                    const uint32_t dst = w_slot();
+                    tma_load_2d(dst, &tm_w2, bar(B_WFULL + ws), c * kHC + st * 64, 0);
+                    w_next();
+                }
+            };
+            for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x) {
+                mbar_wait(bar(B_AEMPTY), ap ^ 1);
+                mbar_expect_tx(bar(B_AFULL), 4 * kSlab);
+                for (int s = 0; s < 4; ++s) tma_load_2d(base + kOffA + s * kSlab, &tm_d, bar(B_AFULL), s * 64, tile * kTM);
+                ap ^= 1;
+                load_w1(0);
+                for (int c = 0; c < NC; ++c) {
+                    if (c + 1 < NC) load_w1(c + 1);
+                    load_w2(c);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer =====================
+        if (elect_one()) {
+            const uint32_t idesc1 = umma_idesc_bf16(kTM, kHC), idesc2 = umma_idesc_bf16(kTM, kC);
+            const uint32_t hi = uint32_t(1024 >> 4) | (1u << 14) | (2u << 29);
+            auto lo = [](uint32_t addr) { return ((addr & 0x3FFFFu) >> 4) | (1u << 16); };
+            const uint32_t a_lo = lo(base + kOffA), hs_lo = lo(base + kOffHs), w_lo = lo(base + kOffW);
+            const uint32_t o_acc = tmem_base, h_acc = tmem_base + kC;
+            int ws = 0; uint32_t wp = 0;
+            uint32_t ph_hacc = 0, ph_hs = 0;                      // bit b = parity of the use count of buffer b
+            auto w_wait = [&]() {
+                mbar_wait(bar(B_WFULL + ws), wp);
+                tc_fence_after();
+                return w_lo + uint32_t(ws) * (kWStage >> 4);
+            };
+            auto w_release = [&]() { umma_commit(bar(B_WEMPTY + ws)); if (++ws == kWStages) { ws = 0; wp ^= 1; } };
+            auto gemm1 = [&](int c) {
+                const int b = c & 1;
+                mbar_wait(bar(B_HACC_EMPTY + b), ((ph_hacc >> b) & 1) ^ 1);
+                ph_hacc ^= 1u << b;
+                tc_fence_after();
+                const uint32_t d = h_acc + uint32_t(b) * kHC;
+#pragma unroll
+                for (int st = 0; st < 2; ++st) {
+                    const uint32_t w = w_wait();
+#pragma unroll
+                    for (int j = 0; j < 2; ++j)
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)
+                            umma_bf16_lh(d, a_lo + uint32_t(2 * st + j) * (kSlab >> 4) + 2 * k, hi, w + uint32_t(j) * (kSlab >> 4) + 2 * k, hi,
+                                         idesc1, uint32_t(st | j | k));
+                    w_release();
+                }
+                umma_commit(bar(B_HACC_FULL + b));
+            };
+            int it = 0;
+            for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x, ++it) {
+                mbar_wait(bar(B_AFULL), it & 1);
+                tc_fence_after();
+                gemm1(0);
+                for (int c = 0; c < NC; ++c) {
+                    if (c + 1 < NC) gemm1(c + 1);
+                    if (c + 1 == NC) umma_commit(bar(B_AEMPTY));          // every GEMM1 of this tile has been issued
+                    const int b = c & 1;
+                    mbar_wait(bar(B_HS_FULL + b), (ph_hs >> b) & 1);
+                    ph_hs ^= 1u << b;
+                    if (c == 0) mbar_wait(bar(B_OEMPTY), (it & 1) ^ 1);  // previous tile's output has left TMEM
+                    tc_fence_after();
+#pragma unroll
+                    for (int st = 0; st < 2; ++st) {
+                        const uint32_t w = w_wait();
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)
+                            umma_bf16_lh(o_acc, hs_lo + uint32_t(2 * b + st) * (kSlab >> 4) + 2 * k, hi, w + 2 * k, hi, idesc2,
+                                         uint32_t(c | st | k));
+                        w_release();
+                    }
+                    umma_commit(bar(B_HS_EMPTY + b));
+                }
+                umma_commit(bar(B_OFULL));
+            }
+        }
+    } else {
+        // ===================== epilogue warps =====================
+        const int quad = warp & 3, half = (warp - 2) >> 2;
+        const int r = quad * 32 + lane;                                   // row of the tile = TMEM lane
+        const uint32_t t_lane = tmem_base + (uint32_t(quad * 32) << 16);
+        uint32_t ph_use = 0;
+        int it = 0;
+        for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x, ++it) {
+            for (int c = 0; c < NC; ++c) {
+                const int b = c & 1;
+                mbar_wait(bar(B_HACC_FULL + b), (ph_use >> b) & 1);
+                mbar_wait(bar(B_HS_EMPTY + b), ((ph_use >> b) & 1) ^ 1);
+                ph_use ^= 1u << b;
+                tc_fence_after();
+                const float *b1 = p.b1 + c * kHC + half * 64;
+                const uint32_t hs_row = base + kOffHs + uint32_t(2 * b + half) * kSlab + uint32_t(r) * 128u;
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    uint32_t v[32];
+                    tmem_ld32(t_lane + kC + uint32_t(b) * kHC + uint32_t(half * 64 + q * 32), v);
+                    uint32_t pk[16];
+#pragma unroll
+                    for (int j = 0; j < 32; j += 4) {
+                        const float4 b4 = __ldg(reinterpret_cast<const float4 *>(b1 + q * 32 + j));
+                        const float f0 = gelu_fast(__uint_as_float(v[j]) + b4.x), f1 = gelu_fast(__uint_as_float(v[j + 1]) + b4.y);
+                        const float f2 = gelu_fast(__uint_as_float(v[j + 2]) + b4.z), f3 = gelu_fast(__uint_as_float(v[j + 3]) + b4.w);
+                        pk[j / 2] = pack_bf16x2(f0, f1);
+                        pk[j / 2 + 1] = pack_bf16x2(f2, f3);
+                    }
+#pragma unroll
+                    for (int jj = 0; jj < 4; ++jj) {                      // 16-byte chunk q*4+jj of the row, 128B-swizzled
+                        const uint32_t chunk = uint32_t(q * 4 + jj) ^ uint32_t(r & 7);
+                        st_shared_v4(hs_row + (chunk << 4), pk[4 * jj], pk[4 * jj + 1], pk[4 * jj + 2], pk[4 * jj + 3]);
+                    }
+                }
+                tc_fence_before();
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) { mbar_arrive(bar(B_HACC_EMPTY + b)); mbar_arrive(bar(B_HS_FULL + b)); }
+            }
+            // ---- output: Oacc + b2 + x -> bf16 ----
+            mbar_wait(bar(B_OFULL), it & 1);
+            tc_fence_after();
+            const long long row = (long long)tile * kTM + r;
+            const bool inb = row < p.n_px;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                uint32_t v[32];
+                const int c0 = half * 128 + q * 32;
+                tmem_ld32(t_lane + uint32_t(c0), v);
+                if (!inb) continue;
+                const uint4 *rs = reinterpret_cast<const uint4 *>(p.x + row * kC + c0);
+                uint4 *dst = reinterpret_cast<uint4 *>(p.out + row * kC + c0);
+#pragma unroll
+                for (int g = 0; g < 4; ++g) {
+                    const uint4 r4 = rs[g];
+                    const __nv_bfloat162 *re = reinterpret_cast<const __nv_bfloat162 *>(&r4);
+                    const float4 ba = __ldg(reinterpret_cast<const float4 *>(p.b2 + c0 + g * 8));
+                    const float4 bb = __ldg(reinterpret_cast<const float4 *>(p.b2 + c0 + g * 8 + 4));
+                    const float bs[8] = {ba.x, ba.y, ba.z, ba.w, bb.x, bb.y, bb.z, bb.w};
+                    uint4 o4;
+                    uint32_t *oe = reinterpret_cast<uint32_t *>(&o4);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const float2 xr = __bfloat1622float2(re[e]);
+                        oe[e] = pack_bf16x2(__uint_as_float(v[g * 8 + 2 * e]) + bs[2 * e] + xr.x,
+                                            __uint_as_float(v[g * 8 + 2 * e + 1]) + bs[2 * e + 1] + xr.y);
+                    }
+                    dst[g] = o4;
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_OEMPTY));
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512u) : "memory");
+    }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------- host side ----------------------------------
+bool trunk_fusable(const ConvLayer &pw1, const ConvLayer &pw2)
+{
+    return pw1.c_in == kC && pw2.n == kC && pw2.n_pad == kC && pw1.n == pw2.c_in && pw1.n_pad == pw1.n && pw1.n % kHC == 0 &&
+           pw1.taps == 1 && pw2.taps == 1 && pw1.groups == 1 && pw2.groups == 1;
+}
+
+bool trunk_make_maps(TrunkMaps &m, const bf16 *d_base, long long n_px, const ConvLayer &pw1, const ConvLayer &pw2, std::string &err)
+{
+    m.ok = false;
+    if (!trunk_fusable(pw1, pw2)) return true;
+    // d: [n_px][256] bf16, box {64 ch, 128 px}; rows past n_px are zero-filled by TMA (ragged last tile)
+    if (!tc_encode_2d(&m.tm_d, d_base, kC, (unsigned long long)n_px, 64, kTM, err)) return false;
+    // W1: [hidden][256] (n rows, k contiguous), box {64, 128}; W2: [256][hidden], box {64, 256}
+    if (!tc_encode_2d(&m.tm_w1, pw1.w, kC, (unsigned long long)pw1.n, 64, kHC, err)) return false;
+    if (!tc_encode_2d(&m.tm_w2, pw2.w, (unsigned long long)pw2.c_in, kC, 64, kC, err)) return false;
+    m.ok = true;
+    return true;
+}
+
+cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const ConvLayer &pw2, const bf16 *x, bf16 *out, long long n_px,
+                             int num_sms, cudaStream_t st)
+{
+    TrunkParams p{};
+    p.n_px = int(n_px);
+    p.n_tiles = int((n_px + kTM - 1) / kTM);
+    p.n_chunks = pw1.n / kHC;
+    p.b1 = pw1.bias; p.b2 = pw2.bias;
+    p.x = x; p.out = out;
+    static thread_local bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(trunk_mlp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kTrunkSmem));
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    const int grid = p.n_tiles < num_sms ? p.n_tiles : num_sms;
+    trunk_mlp_kernel<<<grid, kTrunkThreads, kTrunkSmem, st>>>(m.tm_d, m.tm_w1, m.tm_w2, p);
+    return cudaGetLastError();
+}
+
+}  // namespace ufnvc

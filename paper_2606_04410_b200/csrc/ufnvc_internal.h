@@ -101,6 +101,18 @@ bool tc_make_weight_tmap(ConvLayer &L, std::string &err);
 bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, int tile_h, int tile_w,
                       std::string &err);
 
+bool tc_encode_2d(CUtensorMap *tm, const void *base, unsigned long long dim0, unsigned long long dim1, unsigned box0, unsigned box1,
+                  std::string &err);   // 2-D bf16 map, dim0 contiguous, 128B swizzle, zero OOB fill
+
+// fused trunk MLP (trunk_tc.cu): out = x + W2 GELU(W1 d + b1) + b2 in one kernel, hidden kept on chip
+struct TrunkMaps {
+    CUtensorMap tm_d, tm_w1, tm_w2;
+    bool ok = false;
+};
+bool trunk_make_maps(TrunkMaps &m, const bf16 *d_base, long long n_px, const ConvLayer &pw1, const ConvLayer &pw2, std::string &err);
+cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const ConvLayer &pw2, const bf16 *x, bf16 *out, long long n_px,
+                             int num_sms, cudaStream_t st);
+
 // ---- host-side entropy tables + encoder fixture (tables.cpp part of api) ---------------------------------------
 void build_cdf_tables(int nb, double smin, double smax, std::vector<uint32_t> &cdf32);
 void build_search_lut(const std::vector<uint32_t> &cdf32, int nb, std::vector<uint16_t> &lut);
