@@ -234,23 +234,29 @@ trunk_mlp_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant
                 __syncwarp();
                 if (lane == 0) { mbar_arrive(bar(B_HACC_EMPTY + b)); mbar_arrive(bar(B_HS_FULL + b)); }
             }
-            // ---- output: Oacc + b2 + x -> bf16 ----
-            mbar_wait(bar(B_OFULL), it & 1);
-            tc_fence_after();
+            // ---- output: Oacc + b2 + x -> bf16.  The residual row segment (128 columns = 16 x 16 B) is fetched BEFORE the
+            // wait for the last GEMM2s, so its latency hides behind them: Oacc is single-buffered, which puts this
+            // epilogue on the tile's critical path (fetched after the wait it cost ~60 % of the kernel).
             const long long row = (long long)tile * kTM + r;
             const bool inb = row < p.n_px;
+            uint4 res[16];
+            {
+                const uint4 *rs = reinterpret_cast<const uint4 *>(p.x + row * kC + half * 128);
+#pragma unroll
+                for (int g = 0; g < 16; ++g) res[g] = inb ? rs[g] : make_uint4(0, 0, 0, 0);
+            }
+            mbar_wait(bar(B_OFULL), it & 1);
+            tc_fence_after();
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 uint32_t v[32];
                 const int c0 = half * 128 + q * 32;
                 tmem_ld32(t_lane + uint32_t(c0), v);
                 if (!inb) continue;
-                const uint4 *rs = reinterpret_cast<const uint4 *>(p.x + row * kC + c0);
                 uint4 *dst = reinterpret_cast<uint4 *>(p.out + row * kC + c0);
 #pragma unroll
                 for (int g = 0; g < 4; ++g) {
-                    const uint4 r4 = rs[g];
-                    const __nv_bfloat162 *re = reinterpret_cast<const __nv_bfloat162 *>(&r4);
+                    const __nv_bfloat162 *re = reinterpret_cast<const __nv_bfloat162 *>(&res[q * 4 + g]);
                     const float4 ba = __ldg(reinterpret_cast<const float4 *>(p.b2 + c0 + g * 8));
                     const float4 bb = __ldg(reinterpret_cast<const float4 *>(p.b2 + c0 + g * 8 + 4));
                     const float bs[8] = {ba.x, ba.y, ba.z, ba.w, bb.x, bb.y, bb.z, bb.w};
