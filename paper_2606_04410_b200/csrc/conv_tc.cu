@@ -165,15 +165,20 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
                 const long long o = epi_offset(p.E, img, y, x, p.H, p.W, n);
                 bf16 *dst = reinterpret_cast<bf16 *>(p.E.out) + o;
                 float f[32];
-#pragma unroll
-                for (int j = 0; j < 32; j += 4) {
-                    const float4 b4 = __ldg(reinterpret_cast<const float4 *>(bias + c0 + j));
-                    f[j] = __uint_as_float(v[j]) + b4.x; f[j + 1] = __uint_as_float(v[j + 1]) + b4.y;
-                    f[j + 2] = __uint_as_float(v[j + 2]) + b4.z; f[j + 3] = __uint_as_float(v[j + 3]) + b4.w;
-                }
                 if (p.E.act == ACT_GELU) {
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) f[j] = gelu_fast(f[j]);
+                    for (int j = 0; j < 32; j += 4) {
+                        const float4 b4 = __ldg(reinterpret_cast<const float4 *>(bias + c0 + j));
+                        gelu_bias2(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), b4.x, b4.y, f[j], f[j + 1]);
+                        gelu_bias2(__uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]), b4.z, b4.w, f[j + 2], f[j + 3]);
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 32; j += 4) {
+                        const float4 b4 = __ldg(reinterpret_cast<const float4 *>(bias + c0 + j));
+                        f[j] = __uint_as_float(v[j]) + b4.x; f[j + 1] = __uint_as_float(v[j + 1]) + b4.y;
+                        f[j + 2] = __uint_as_float(v[j + 2]) + b4.z; f[j + 3] = __uint_as_float(v[j + 3]) + b4.w;
+                    }
                 }
                 if (MODE == EPI_NHWC && p.E.residual) {
                     const uint4 *rs = reinterpret_cast<const uint4 *>(p.E.residual + o);

@@ -37,6 +37,49 @@ __device__ __forceinline__ float gelu_fast(float v)
     return fmaf(hv, t, hv);
 }
 
+// Two GELUs at once on the packed-fp32 pipe (sm_100 FADD2 / FMUL2 / FFMA2): (acc0 + b0, acc1 + b1) -> gelu_fast of each.
+// 13 issue slots per PAIR (6 packed FMA-pipe ops, 2 FMNMX, 2 MUFU.TANH, + the bf16 pack done by the caller).
+__device__ __forceinline__ uint64_t f2_pack(float a, float b)
+{
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ void f2_unpack(uint64_t v, float &a, float &b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ uint64_t f2_fma(uint64_t a, uint64_t b, uint64_t c)
+{
+    uint64_t r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ uint64_t f2_mul(uint64_t a, uint64_t b)
+{
+    uint64_t r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ uint64_t f2_add(uint64_t a, uint64_t b)
+{
+    uint64_t r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ void gelu_bias2(float acc0, float acc1, float b0, float b1, float &g0, float &g1)
+{
+    const uint64_t v = f2_add(f2_pack(acc0, acc1), f2_pack(b0, b1));
+    float s0, s1;
+    f2_unpack(f2_mul(v, v), s0, s1);
+    const uint64_t s = f2_pack(fminf(s0, 49.0f), fminf(s1, 49.0f));
+    uint64_t pl = f2_fma(f2_pack(-3.58006361e-4f, -3.58006361e-4f), s, f2_pack(3.70462883e-2f, 3.70462883e-2f));
+    pl = f2_fma(pl, s, f2_pack(7.97462455e-1f, 7.97462455e-1f));
+    float u0, u1, t0, t1;
+    f2_unpack(f2_mul(v, pl), u0, u1);
+    asm("tanh.approx.f32 %0, %1;" : "=f"(t0) : "f"(u0));
+    asm("tanh.approx.f32 %0, %1;" : "=f"(t1) : "f"(u1));
+    const uint64_t hv = f2_mul(v, f2_pack(0.5f, 0.5f));
+    f2_unpack(f2_fma(hv, f2_pack(t0, t1), hv), g0, g1);
+}
+
 __device__ __forceinline__ float apply_act(float v, int act) { return act == ACT_GELU ? gelu_erf(v) : v; }
 
 // Destination element offset of packed output column n of input pixel (img, y, x); EPI_NHWC / EPI_PS2 only.

@@ -218,8 +218,9 @@ trunk_mlp_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant
 #pragma unroll
                     for (int j = 0; j < 32; j += 4) {
                         const float4 b4 = __ldg(reinterpret_cast<const float4 *>(b1 + q * 32 + j));
-                        const float f0 = gelu_fast(__uint_as_float(v[j]) + b4.x), f1 = gelu_fast(__uint_as_float(v[j + 1]) + b4.y);
-                        const float f2 = gelu_fast(__uint_as_float(v[j + 2]) + b4.z), f3 = gelu_fast(__uint_as_float(v[j + 3]) + b4.w);
+                        float f0, f1, f2, f3;
+                        gelu_bias2(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), b4.x, b4.y, f0, f1);
+                        gelu_bias2(__uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]), b4.z, b4.w, f2, f3);
                         pk[j / 2] = pack_bf16x2(f0, f1);
                         pk[j / 2 + 1] = pack_bf16x2(f2, f3);
                     }
