@@ -83,12 +83,14 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
 
     // O3 tables + search accelerator
     build_cdf_tables(cfg->n_buckets, cfg->scale_min, cfg->scale_max, h->cdf32);
-    std::vector<uint16_t> lut, cdf16(h->cdf32.size());
+    std::vector<uint16_t> lut;
+    std::vector<uint32_t> cf(h->cdf32.size(), 0u);
     build_search_lut(h->cdf32, cfg->n_buckets, lut);
-    for (size_t i = 0; i < cdf16.size(); ++i) cdf16[i] = uint16_t(h->cdf32[i]);     // c[255] = 2^16 wraps to 0
+    for (size_t i = 0; i < cf.size(); ++i)                                          // pos 255 is never a symbol
+        if ((i & 255) != 255) cf[i] = h->cdf32[i] | ((h->cdf32[i + 1] - h->cdf32[i]) << 16);
 
     const size_t n = size_t(h->max_chunks), P = size_t(h->h) * h->w, Pz = size_t(h->h_z) * h->w_z, T = size_t(cfg->T);
-    bool ok = dev_alloc(h, h->d_cdf, cdf16.size()) && dev_alloc(h, h->d_lut, lut.size()) && dev_alloc(h, h->d_status, 1) &&
+    bool ok = dev_alloc(h, h->d_cf, cf.size()) && dev_alloc(h, h->d_lut, lut.size()) && dev_alloc(h, h->d_status, 1) &&
               dev_alloc(h, h->hx0, n * Pz * cfg->c_z) && dev_alloc(h, h->hx1, n * Pz * cfg->c_hyper) &&
               dev_alloc(h, h->hx2, n * Pz * cfg->c_hyper) && dev_alloc(h, h->hpart, 9 * n * Pz * cfg->c_hyper) && dev_alloc(h, h->mu, n * P * cfg->c_y) &&
               dev_alloc(h, h->lnscale, n * P * cfg->c_y) && dev_alloc(h, h->idx, n * P * cfg->c_y) &&
@@ -96,7 +98,7 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
               dev_alloc(h, h->fb, n * T * P * cfg->c_trunk) &&
               dev_alloc(h, h->hidden, cfg->n_trunk_blocks ? n * T * P * cfg->c_trunk * cfg->trunk_expand : 1);
     for (int s = 0; ok && s < 3; ++s) ok = dev_alloc(h, h->stage[s], n * T * (P << (2 * (s + 1))) * cfg->dec_channels[s + 1]);
-    if (ok) ok = cudaMemcpy(h->d_cdf, cdf16.data(), cdf16.size() * 2, cudaMemcpyHostToDevice) == cudaSuccess &&
+    if (ok) ok = cudaMemcpy(h->d_cf, cf.data(), cf.size() * 4, cudaMemcpyHostToDevice) == cudaSuccess &&
                  cudaMemcpy(h->d_lut, lut.data(), lut.size() * 2, cudaMemcpyHostToDevice) == cudaSuccess &&
                  cudaMemset(h->d_status, 0, 4) == cudaSuccess;
     if (!ok) {

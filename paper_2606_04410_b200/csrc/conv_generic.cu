@@ -98,14 +98,13 @@ cudaError_t launch_conv_generic(const ConvLayer &L, const ConvProblem &P, const 
 // the side columns are L1 hits, loaded by the neighbouring warps of the block) and scattered into three rolling
 // accumulators (output rows r-1, r, r+1), so a row of outputs costs 3 vector loads and 1 store.  For C = 256 a warp is
 // exactly one pixel (512 contiguous bytes).
-__device__ __forceinline__ void dw_unpack(const uint4 &v, float (&f)[8])
+// bf16x2 word -> packed (lo, hi) fp32 pair for the FFMA2 pipe: 2 integer ops
+__device__ __forceinline__ uint64_t dw_pair(uint32_t w)
 {
-    const __nv_bfloat162 *h = reinterpret_cast<const __nv_bfloat162 *>(&v);
-#pragma unroll
-    for (int e = 0; e < 4; ++e) { const float2 t = __bfloat1622float2(h[e]); f[2 * e] = t.x; f[2 * e + 1] = t.y; }
+    return f2_pack(__uint_as_float(w << 16), __uint_as_float(w & 0xFFFF0000u));
 }
 
-__global__ void __launch_bounds__(256) dwconv3x3_kernel(const bf16 *__restrict__ in, bf16 *__restrict__ out,
+__global__ void __launch_bounds__(256, 2) dwconv3x3_kernel(const bf16 *__restrict__ in, bf16 *__restrict__ out,
                                                         const float *__restrict__ w9c, const float *__restrict__ bias,
                                                         int n_img, int H, int W, int C, int rows_per_seg, int n_seg)
 {
@@ -121,53 +120,65 @@ __global__ void __launch_bounds__(256) dwconv3x3_kernel(const bf16 *__restrict__
     const int c0 = c8 * 8;
     const int y0 = seg * rows_per_seg, y1 = min(H, y0 + rows_per_seg);      // output rows [y0, y1)
 
-    float wv[9][8], bv[8];
+    uint64_t wv[9][4], bv[4];                                               // channel pairs (2e, 2e+1)
 #pragma unroll
     for (int k = 0; k < 9; ++k) {
         const float4 lo = __ldg(reinterpret_cast<const float4 *>(w9c + k * C + c0));
         const float4 hi = __ldg(reinterpret_cast<const float4 *>(w9c + k * C + c0 + 4));
-        wv[k][0] = lo.x; wv[k][1] = lo.y; wv[k][2] = lo.z; wv[k][3] = lo.w;
-        wv[k][4] = hi.x; wv[k][5] = hi.y; wv[k][6] = hi.z; wv[k][7] = hi.w;
+        wv[k][0] = f2_pack(lo.x, lo.y); wv[k][1] = f2_pack(lo.z, lo.w);
+        wv[k][2] = f2_pack(hi.x, hi.y); wv[k][3] = f2_pack(hi.z, hi.w);
     }
     {
         const float4 lo = __ldg(reinterpret_cast<const float4 *>(bias + c0)), hi = __ldg(reinterpret_cast<const float4 *>(bias + c0 + 4));
-        bv[0] = lo.x; bv[1] = lo.y; bv[2] = lo.z; bv[3] = lo.w; bv[4] = hi.x; bv[5] = hi.y; bv[6] = hi.z; bv[7] = hi.w;
+        bv[0] = f2_pack(lo.x, lo.y); bv[1] = f2_pack(lo.z, lo.w); bv[2] = f2_pack(hi.x, hi.y); bv[3] = f2_pack(hi.z, hi.w);
     }
     const bf16 *img_in = in + (long long)img * H * W * C + c0;
     bf16 *img_out = out + (long long)img * H * W * C + c0;
     const bool has_l = x > 0, has_r = x + 1 < W;
-
-    float accP[8], accC[8], accN[8];            // outputs rows ir-1, ir, ir+1 while input row ir is being added
-#pragma unroll
-    for (int e = 0; e < 8; ++e) { accP[e] = bv[e]; accC[e] = bv[e]; accN[e] = bv[e]; }
-
-    for (int ir = y0 - 1; ir <= y1; ++ir) {     // input rows feeding outputs [y0, y1)
-        if (ir >= 0 && ir < H) {
+    const uint4 z4 = make_uint4(0, 0, 0, 0);
+    auto load_row = [&](int ir, uint4 &vl, uint4 &vc, uint4 &vr) {
+        vl = vc = vr = z4;
+        if (ir >= 0 && ir < H && ir <= y1) {
             const bf16 *row = img_in + ((long long)ir * W + x) * C;
-            const uint4 z4 = make_uint4(0, 0, 0, 0);
-            const uint4 vl = has_l ? __ldg(reinterpret_cast<const uint4 *>(row - C)) : z4;
-            const uint4 vc = __ldg(reinterpret_cast<const uint4 *>(row));
-            const uint4 vr = has_r ? __ldg(reinterpret_cast<const uint4 *>(row + C)) : z4;
-            float fl[8], fc[8], fr[8];
-            dw_unpack(vl, fl); dw_unpack(vc, fc); dw_unpack(vr, fr);
+            if (has_l) vl = __ldg(reinterpret_cast<const uint4 *>(row - C));
+            vc = __ldg(reinterpret_cast<const uint4 *>(row));
+            if (has_r) vr = __ldg(reinterpret_cast<const uint4 *>(row + C));
+        }
+    };
+
+    uint64_t accP[4], accC[4], accN[4];         // outputs rows ir-1, ir, ir+1 while input row ir is being added
 #pragma unroll
-            for (int e = 0; e < 8; ++e) {
-                // input row ir is kernel row 2 of output ir-1, row 1 of output ir, row 0 of output ir+1
-                accP[e] = fmaf(wv[6][e], fl[e], fmaf(wv[7][e], fc[e], fmaf(wv[8][e], fr[e], accP[e])));
-                accC[e] = fmaf(wv[3][e], fl[e], fmaf(wv[4][e], fc[e], fmaf(wv[5][e], fr[e], accC[e])));
-                accN[e] = fmaf(wv[0][e], fl[e], fmaf(wv[1][e], fc[e], fmaf(wv[2][e], fr[e], accN[e])));
-            }
+    for (int e = 0; e < 4; ++e) { accP[e] = bv[e]; accC[e] = bv[e]; accN[e] = bv[e]; }
+
+    uint4 nl, nc, nr;
+    load_row(y0 - 1, nl, nc, nr);
+    for (int ir = y0 - 1; ir <= y1; ++ir) {     // input rows feeding outputs [y0, y1); rows outside the image are zeros
+        const uint4 vl = nl, vc = nc, vr = nr;
+        load_row(ir + 1, nl, nc, nr);           // next row's loads are in flight while this row is accumulated
+        const uint32_t *pl = reinterpret_cast<const uint32_t *>(&vl), *pc = reinterpret_cast<const uint32_t *>(&vc),
+                       *pr = reinterpret_cast<const uint32_t *>(&vr);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const uint64_t fl = dw_pair(pl[e]), fc = dw_pair(pc[e]), fr = dw_pair(pr[e]);
+            // input row ir is kernel row 2 of output ir-1, row 1 of output ir, row 0 of output ir+1
+            accP[e] = f2_fma(wv[6][e], fl, f2_fma(wv[7][e], fc, f2_fma(wv[8][e], fr, accP[e])));
+            accC[e] = f2_fma(wv[3][e], fl, f2_fma(wv[4][e], fc, f2_fma(wv[5][e], fr, accC[e])));
+            accN[e] = f2_fma(wv[0][e], fl, f2_fma(wv[1][e], fc, f2_fma(wv[2][e], fr, accN[e])));
         }
         const int oy = ir - 1;                  // output row oy is complete once input row oy+1 = ir has been added
         if (oy >= y0 && oy < y1) {
             uint4 o;
             __nv_bfloat162 *oe = reinterpret_cast<__nv_bfloat162 *>(&o);
 #pragma unroll
-            for (int e = 0; e < 4; ++e) oe[e] = __floats2bfloat162_rn(accP[2 * e], accP[2 * e + 1]);
+            for (int e = 0; e < 4; ++e) {
+                float a, b;
+                f2_unpack(accP[e], a, b);
+                oe[e] = __floats2bfloat162_rn(a, b);
+            }
             *reinterpret_cast<uint4 *>(img_out + ((long long)oy * W + x) * C) = o;
         }
 #pragma unroll
-        for (int e = 0; e < 8; ++e) { accP[e] = accC[e]; accC[e] = accN[e]; accN[e] = bv[e]; }
+        for (int e = 0; e < 4; ++e) { accP[e] = accC[e]; accC[e] = accN[e]; accN[e] = bv[e]; }
     }
 }
 

@@ -68,7 +68,7 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     CU_TRY(cudaMemsetAsync(h->d_status, 0, 4, st));
     RansParams rp{};
     rp.bits = bits; rp.bits_bytes = bits_bytes; rp.sub_off = sub_off; rp.idx = idx; rp.mu = mu;
-    rp.cdf = h->d_cdf; rp.lut = h->d_lut;
+    rp.cf = h->d_cf; rp.lut = h->d_lut;
     rp.n_chunks = n; rp.n_sub = h->n_sub; rp.h = h->h; rp.w = h->w; rp.c_y = c.c_y;
     rp.rows_per_sub = c.rows_per_substream; rp.W = c.lanes_per_substream; rp.n_buckets = c.n_buckets;
     rp.yhat = h->yhat; rp.sym_tap = taps ? taps->sym : nullptr; rp.yhat_tap = taps ? taps->yhat : nullptr;

@@ -20,7 +20,8 @@ struct ufnvc_handle {
 
     // entropy tables (O3)
     std::vector<uint32_t> cdf32;         // [nb][256], host copy
-    uint16_t *d_cdf = nullptr, *d_lut = nullptr;
+    uint32_t *d_cf = nullptr;             // [nb][256]: c[pos] | freq[pos] << 16
+    uint16_t *d_lut = nullptr;
     uint32_t *d_status = nullptr;
 
     // layers

@@ -12,24 +12,18 @@
 
 namespace ufnvc {
 
-struct RansSmem {
-    uint16_t cdf[64 * 256];
-    uint16_t lut[64 * 256];
-};
-
 __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    uint16_t *s_cdf = reinterpret_cast<uint16_t *>(smem_raw);
-    uint16_t *s_lut = s_cdf + nb * 256;
+    // s_cf[k][pos] = c[pos] | freq[pos] << 16 (one 32-bit read gives both; freq <= 65282 fits 16 bits), then the search LUT
+    uint32_t *s_cf = reinterpret_cast<uint32_t *>(smem_raw);
+    uint16_t *s_lut = reinterpret_cast<uint16_t *>(s_cf + nb * 256);
     {
-        const uint4 *src_c = reinterpret_cast<const uint4 *>(p.cdf);
+        const uint4 *src_c = reinterpret_cast<const uint4 *>(p.cf);
         const uint4 *src_l = reinterpret_cast<const uint4 *>(p.lut);
-        uint4 *dc = reinterpret_cast<uint4 *>(s_cdf), *dl = reinterpret_cast<uint4 *>(s_lut);
-        for (int i = threadIdx.x; i < nb * 32; i += blockDim.x) {
-            dc[i] = src_c[i];
-            dl[i] = src_l[i];
-        }
+        uint4 *dc = reinterpret_cast<uint4 *>(s_cf), *dl = reinterpret_cast<uint4 *>(s_lut);
+        for (int i = threadIdx.x; i < nb * 64; i += blockDim.x) dc[i] = src_c[i];
+        for (int i = threadIdx.x; i < nb * 32; i += blockDim.x) dl[i] = src_l[i];
     }
     __syncthreads();
 
@@ -88,15 +82,15 @@ __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
         const int i = i0 + j * p.W;
         const bool valid = j < n_steps && i < n;
         const uint32_t slot = x & 0xFFFFu;
-        const uint16_t *c = s_cdf + k * 256;
+        const uint32_t *c = s_cf + k * 256;
         const uint32_t lh = s_lut[k * 256 + (slot >> 8)];
         uint32_t lo = lh & 0xFFu, hi = lh >> 8;
         while (lo < hi) {                       // largest pos in [lo,hi] with c[pos] <= slot
             const uint32_t mid = (lo + hi + 1) >> 1;
-            if (c[mid] <= slot) lo = mid; else hi = mid - 1;
+            if ((c[mid] & 0xFFFFu) <= slot) lo = mid; else hi = mid - 1;
         }
-        const uint32_t cp = c[lo];
-        const uint32_t f = (uint32_t(c[lo + 1]) - cp) & 0xFFFFu;        // c[255] = 2^16 is stored as 0
+        const uint32_t cf = c[lo];
+        const uint32_t cp = cf & 0xFFFFu, f = cf >> 16;
         uint32_t xn = f * (x >> 16) + slot - cp;
         const bool need = valid && xn < (1u << 16);
         const uint32_t m = __ballot_sync(0xFFFFFFFFu, need);
@@ -139,7 +133,7 @@ __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
 cudaError_t launch_rans_decode(const RansParams &p, cudaStream_t st)
 {
     const int nb = p.n_buckets;
-    const size_t smem = (size_t)64 * 256 * 2 * 2;
+    const size_t smem = (size_t)64 * 256 * (4 + 2);
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(rans_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

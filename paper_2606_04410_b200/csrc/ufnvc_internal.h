@@ -81,7 +81,7 @@ struct RansParams {
     const uint32_t *sub_off;  // [n_chunks*n_sub + 1]
     const uint8_t *idx;       // [n][h][w][c_y]
     const float *mu;
-    const uint16_t *cdf;      // [nb][256] u16 (c[255] wraps to 0)
+    const uint32_t *cf;       // [nb][256]: c[pos] | freq[pos] << 16
     const uint16_t *lut;      // [nb][256]: lo | hi<<8 = first/last candidate position for slot>>8
     int n_chunks, n_sub, h, w, c_y, rows_per_sub, W, n_buckets;
     bf16 *yhat;               // [n][h][w][c_y]

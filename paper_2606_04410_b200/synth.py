@@ -38,7 +38,7 @@ class ChunkConfig:
     scale_min: float = 0.11
     scale_max: float = 20.0
     rows_per_substream: int = 4
-    lanes_per_substream: int = 128
+    lanes_per_substream: int = 512       # rANS lanes W per substream: 16 warp-streams (R9, speed variant)
     n_chunks: int = 1
     weight_dtype: int = 1          # 0 = fp32, 1 = bf16
     mu_law: str = "normal"         # "normal": N(0,1); "uniform": U(-2,2)
@@ -101,7 +101,7 @@ CONFIGS = {
     2: ChunkConfig("cfg2-480p", 1, 4, 480, 832, 128, 64, 128, 256, 4, 4, _DEC),
     3: ChunkConfig("cfg3-1080p", 2, 8, 1080, 1920, 128, 64, 128, 256, 6, 4, _DEC),
     4: ChunkConfig("cfg4-1080p-4xT16", 3, 16, 1080, 1920, 192, 64, 128, 256, 6, 4, _DEC,
-                   lanes_per_substream=192, n_chunks=4, sigma_hi=2.0),
+                   lanes_per_substream=384, n_chunks=4, sigma_hi=2.0),
     5: ChunkConfig("cfg5-4k", 4, 8, 2160, 3840, 128, 64, 128, 256, 8, 4, _DEC),
 }
 

@@ -78,7 +78,7 @@ def _random_case(orc, cdf, n, rng, lo_bucket=0, hi_bucket=NB):
 
 
 @pytest.mark.parametrize("W,n", [(32, 1), (32, 5), (32, 32), (32, 512), (64, 1000), (128, 61440), (128, 26624),
-                                 (128, 13312), (192, 92160), (512, 4097), (32, 33)])
+                                 (128, 13312), (192, 92160), (512, 4097), (32, 33), (512, 61440), (384, 92160)])
 def test_rans_round_trip_end_state_and_size(orc, cdf, W, n):
     rng = np.random.default_rng(n * 31 + W)
     idx, sym = _random_case(orc, cdf, n, rng)
