@@ -134,6 +134,10 @@ int ufnvc_chunk_decode_profiled(ufnvc_handle *h, int n_chunks, const int16_t *z_
                                 size_t bits_bytes, const uint32_t *sub_off_dev, float *frames_dev,
                                 void *cuda_stream, float *us_out_host);
 
+/* Debug counters of the last decode / entropy_params call (synchronises the device).  which = 0: number of latent
+ * elements whose scale bucket was re-decided in fp64 by the hybrid head (R12); 0 when the head runs all-fp64. */
+int ufnvc_debug_counter(ufnvc_handle *h, int which, uint64_t *value_host);
+
 /* ---- encoder-side fixtures (HOST code, not on the timed path): what a sender would run so that bench.py can
  * build a valid bit-stream without the oracle.  The real codec's encoder runs the decoder's prior net
  * (PAPER.md:125), hence idx comes from ufnvc_entropy_params. ---- */

@@ -52,6 +52,7 @@ def _load():
         "ufnvc_last_error": (C.c_char_p, [vp]),
         "ufnvc_launches_per_call": (i, [vp, i]),
         "ufnvc_chunk_decode_profiled": (i, [vp, i, vp, vp, sz, vp, vp, vp, C.POINTER(C.c_float)]),
+        "ufnvc_debug_counter": (i, [vp, i, C.POINTER(C.c_uint64)]),
         "ufnvc_get_cdf": (i, [vp, vp]),
         "ufnvc_symbols_from_uniform": (i, [vp, vp, vp, sz, vp]),
         "ufnvc_encode_chunk": (C.c_long, [vp, vp, vp, vp, sz, vp]),
@@ -65,7 +66,7 @@ def _load():
 LIB = _load()
 EXPORTS = ("ufnvc_create", "ufnvc_destroy", "ufnvc_load_weights", "ufnvc_chunk_decode", "ufnvc_chunk_decode_ex",
            "ufnvc_entropy_params", "ufnvc_get_status", "ufnvc_last_error", "ufnvc_launches_per_call",
-           "ufnvc_chunk_decode_profiled", "ufnvc_get_cdf", "ufnvc_symbols_from_uniform", "ufnvc_encode_chunk")
+           "ufnvc_chunk_decode_profiled", "ufnvc_debug_counter", "ufnvc_get_cdf", "ufnvc_symbols_from_uniform", "ufnvc_encode_chunk")
 
 
 def make_config(cfg, max_chunks: int | None = None) -> ufnvc_config:
@@ -216,6 +217,11 @@ class ChunkDecoder:
     def get_status(self) -> int:
         v = C.c_uint32(0)
         self._check(LIB.ufnvc_get_status(self.handle, C.byref(v)), "ufnvc_get_status")
+        return int(v.value)
+
+    def debug_counter(self, which: int = 0) -> int:
+        v = C.c_uint64(0)
+        self._check(LIB.ufnvc_debug_counter(self.handle, which, C.byref(v)), "ufnvc_debug_counter")
         return int(v.value)
 
     def launches_per_call(self, n_chunks=1) -> int:

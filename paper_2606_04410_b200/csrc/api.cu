@@ -81,6 +81,12 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     const char *ft = std::getenv("UFNVC_FUSED_TRUNK");
     h->use_fused_trunk = !(ft && ft[0] == '0');
 
+    const char *hy = std::getenv("UFNVC_HYBRID_HEAD");
+    h->hybrid_head = !(hy && hy[0] == '0') && cfg->weight_dtype == 1 && cfg->c_y % 32 == 0 && cfg->c_hyper % 32 == 0 &&
+                     !h->force_generic;
+
+    if (const char *fu = std::getenv("UFNVC_HEAD_FLAG_U")) h->head_flag_u = std::atof(fu);
+
     // O3 tables + search accelerator
     build_cdf_tables(cfg->n_buckets, cfg->scale_min, cfg->scale_max, h->cdf32);
     std::vector<uint16_t> lut;
@@ -92,7 +98,8 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     const size_t n = size_t(h->max_chunks), P = size_t(h->h) * h->w, Pz = size_t(h->h_z) * h->w_z, T = size_t(cfg->T);
     bool ok = dev_alloc(h, h->d_cf, cf.size()) && dev_alloc(h, h->d_lut, lut.size()) && dev_alloc(h, h->d_status, 1) &&
               dev_alloc(h, h->hx0, n * Pz * cfg->c_z) && dev_alloc(h, h->hx1, n * Pz * cfg->c_hyper) &&
-              dev_alloc(h, h->hx2, n * Pz * cfg->c_hyper) && dev_alloc(h, h->hpart, 9 * n * Pz * cfg->c_hyper) && dev_alloc(h, h->mu, n * P * cfg->c_y) &&
+              dev_alloc(h, h->hx2, n * Pz * cfg->c_hyper) && dev_alloc(h, h->xs, n * Pz * 2 * cfg->c_hyper) &&
+              dev_alloc(h, h->fix_list, n * P * cfg->c_y) && dev_alloc(h, h->fix_count, 1) && dev_alloc(h, h->hpart, 9 * n * Pz * cfg->c_hyper) && dev_alloc(h, h->mu, n * P * cfg->c_y) &&
               dev_alloc(h, h->lnscale, n * P * cfg->c_y) && dev_alloc(h, h->idx, n * P * cfg->c_y) &&
               dev_alloc(h, h->yhat, n * P * cfg->c_y) && dev_alloc(h, h->fa, n * T * P * cfg->c_trunk) &&
               dev_alloc(h, h->fb, n * T * P * cfg->c_trunk) &&
@@ -126,6 +133,18 @@ extern "C" int ufnvc_get_status(ufnvc_handle *h, uint32_t *device_status)
 {
     if (!h || !device_status) return UFNVC_E_INVALID_ARG;
     if (cudaMemcpy(device_status, h->d_status, 4, cudaMemcpyDeviceToHost) != cudaSuccess) return fail(h, UFNVC_E_CUDA, "status read failed");
+    return UFNVC_OK;
+}
+
+extern "C" int ufnvc_debug_counter(ufnvc_handle *h, int which, uint64_t *value_host)
+{
+    if (!h || !value_host || which != 0) return UFNVC_E_INVALID_ARG;
+    uint32_t v = 0;
+    if (h->hybrid_head) {
+        if (cudaDeviceSynchronize() != cudaSuccess || cudaMemcpy(&v, h->fix_count, 4, cudaMemcpyDeviceToHost) != cudaSuccess)
+            return fail(h, UFNVC_E_CUDA, "cudaMemcpy(fix_count) failed");
+    }
+    *value_host = v;
     return UFNVC_OK;
 }
 

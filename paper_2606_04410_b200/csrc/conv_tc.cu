@@ -156,6 +156,56 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
                     }
                 }
             }
+        } else if (MODE == EPI_HEAD) {
+            // A2: pixel-shuffle x4 + crop + split.  A 32-column chunk is 32 consecutive latent channels of one sub-pixel.
+            for (int c0 = half * 32; c0 < p.BN; c0 += 64) {
+                uint32_t v[32];
+                tmem_ld32(t_row + uint32_t(c0), v);
+                if (!inb) continue;
+                const EpiParams &E = p.E;
+                const int n = tc.nt * p.BN + c0;
+                const int sij = n / E.c_y, c2 = n - sij * E.c_y;
+                const int ly = 4 * y + ((sij >> 2) & 3), lx = 4 * x + (sij & 3);
+                if (ly >= E.lat_h || lx >= E.lat_w) continue;                      // crop [R2]
+                const long long e0 = (((long long)img * E.lat_h + ly) * E.lat_w + lx) * E.c_y + c2;
+                float f[32];
+#pragma unroll
+                for (int j = 0; j < 32; j += 4) {
+                    const float4 b4 = __ldg(reinterpret_cast<const float4 *>(bias + c0 + j));
+                    f[j] = __uint_as_float(v[j]) + b4.x; f[j + 1] = __uint_as_float(v[j + 1]) + b4.y;
+                    f[j + 2] = __uint_as_float(v[j + 2]) + b4.z; f[j + 3] = __uint_as_float(v[j + 3]) + b4.w;
+                }
+                if ((sij >> 4) == 0) {                                             // mean
+                    float4 *dst = reinterpret_cast<float4 *>(E.mu + e0);
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) dst[q] = make_float4(f[4 * q], f[4 * q + 1], f[4 * q + 2], f[4 * q + 3]);
+                } else {                                                           // ln sigma -> bucket, edge flag
+                    uint32_t packed[8];
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) {
+                        const float u = fminf(fmaxf(f[j], E.ln_lo), E.ln_hi);
+                        f[j] = u;
+                        const float t = fmaf(u - E.ln_lo, E.t_scale, 0.5f);
+                        const float tf = floorf(t);
+                        int k = int(tf);
+                        k = k < 0 ? 0 : (k > E.n_buckets - 1 ? E.n_buckets - 1 : k);
+                        const float fr = t - tf;
+                        if (fminf(fr, 1.0f - fr) < E.flag_t) {                     // decided exactly by hyper_fix_kernel
+                            const uint32_t pos = atomicAdd(E.fix_count, 1u);
+                            E.fix_list[pos] = uint32_t(e0 + j);
+                        }
+                        if ((j & 3) == 0) packed[j >> 2] = uint32_t(k); else packed[j >> 2] |= uint32_t(k) << (8 * (j & 3));
+                    }
+                    uint4 *di = reinterpret_cast<uint4 *>(E.idx + e0);
+                    di[0] = make_uint4(packed[0], packed[1], packed[2], packed[3]);
+                    di[1] = make_uint4(packed[4], packed[5], packed[6], packed[7]);
+                    if (E.lnscale) {
+                        float4 *dl = reinterpret_cast<float4 *>(E.lnscale + e0);
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) dl[q] = make_float4(f[4 * q], f[4 * q + 1], f[4 * q + 2], f[4 * q + 3]);
+                    }
+                }
+            }
         } else {
             for (int c0 = half * 32; c0 < p.BN; c0 += 64) {
                 uint32_t v[32];
@@ -596,6 +646,7 @@ cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUt
     switch (E.mode) {
         case EPI_NHWC: return resident ? launch(conv_halo_kernel<EPI_NHWC, true>) : launch(conv_halo_kernel<EPI_NHWC, false>);
         case EPI_PS2: return resident ? launch(conv_halo_kernel<EPI_PS2, true>) : launch(conv_halo_kernel<EPI_PS2, false>);
+        case EPI_HEAD: return resident ? cudaErrorInvalidValue : launch(conv_halo_kernel<EPI_HEAD, false>);
         default: return resident ? launch(conv_halo_kernel<EPI_FINAL, true>) : launch(conv_halo_kernel<EPI_FINAL, false>);
     }
 }
@@ -642,6 +693,7 @@ cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUten
     switch (E.mode) {
         case EPI_NHWC: return launch(conv_tc_kernel<EPI_NHWC>);
         case EPI_PS2: return launch(conv_tc_kernel<EPI_PS2>);
+        case EPI_HEAD: return launch(conv_tc_kernel<EPI_HEAD>);
         default: return launch(conv_tc_kernel<EPI_FINAL>);
     }
 }

@@ -44,9 +44,29 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     if (need_hyper) {
         CU_TRY(launch_z_to_f64(z, h->hx0, n, c.c_z, Pz, st));
         CU_TRY(launch_hyper_conv(h->hyper[0], h->hx0, h->hx1, h->hpart, n, h->h_z, h->w_z, st));
-        CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, h->hpart, n, h->h_z, h->w_z, st));
         HeadParams hp{c.c_y, h->h, h->w, c.n_buckets, std::log(c.scale_min), std::log(c.scale_max), h->mu, h->lnscale, h->idx};
-        CU_TRY(launch_hyper_head(h->hyper[2], h->hx2, n, h->h_z, h->w_z, hp, st));
+        if (h->hybrid_head && h->am_xs.ok && h->head_tc.use_tc) {
+            // layer 1 also emits the bf16 hi|mid split; the head runs on tensor cores; elements whose ln sigma lands within
+            // flag_u of a bucket edge are re-decided in fp64 (identical decisions to the all-fp64 path, R12)
+            CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, h->hpart, n, h->h_z, h->w_z, st, h->xs));
+            CU_TRY(cudaMemsetAsync(h->fix_count, 0, 4, st));
+            const double step = (hp.ln_hi - hp.ln_lo) / double(c.n_buckets - 1 > 0 ? c.n_buckets - 1 : 1);
+            EpiParams E{};
+            E.mode = EPI_HEAD; E.act = ACT_NONE;
+            E.mu = h->mu; E.lnscale = h->lnscale; E.idx = h->idx; E.fix_list = h->fix_list; E.fix_count = h->fix_count;
+            E.c_y = c.c_y; E.lat_h = h->h; E.lat_w = h->w; E.n_buckets = c.n_buckets;
+            E.ln_lo = float(hp.ln_lo); E.ln_hi = float(hp.ln_hi); E.t_scale = float(1.0 / step);
+            E.flag_t = float(h->head_flag_u / step);
+            ConvProblem pr{h->xs, n, h->h_z, h->w_z, 1};
+            // z maps are tiny (17 x 30 at 1080p): the shifted-TMA-box kernel tiles them with the least padding
+            CU_TRY(launch_conv_tc(h->head_tc, pr, h->am_xs.tm, h->am_xs.tile_h, h->am_xs.tile_w, false, E, h->num_sms, st));
+            CU_TRY(launch_hyper_fix(h->fix_list, h->fix_count, h->hx2, h->head_fix_w, h->head_fix_b, c.c_hyper, h->h_z, h->w_z, hp,
+                                    h->num_sms, st));
+            if (launches) *launches += 3;
+        } else {
+            CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, h->hpart, n, h->h_z, h->w_z, st));
+            CU_TRY(launch_hyper_head(h->hyper[2], h->hx2, n, h->h_z, h->w_z, hp, st));
+        }
         if (launches) *launches += 4;
     }
     if (entropy_params_only) {
@@ -189,11 +209,13 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
     const ufnvc_config &c = h->cfg;
     std::string err;
     bool ok = tc_make_weight_tmap(h->xframe, err);
+    if (h->hybrid_head) ok = ok && tc_make_weight_tmap(h->head_tc, err);
     for (auto &tb : h->trunk) ok = ok && tc_make_weight_tmap(tb.pw1, err) && tc_make_weight_tmap(tb.pw2, err);
     for (int s = 0; s < 4; ++s) ok = ok && tc_make_weight_tmap(h->dec[s], err);
     if (!ok) return fail(h, UFNVC_E_CUDA, err);
     const int n = h->max_chunks, T = c.T;
-    ok = make_act_map(h, h->am_yhat, h->yhat, n, h->h, h->w, c.c_y, true, 1) &&
+    if (h->hybrid_head) ok = make_act_map(h, h->am_xs, h->xs, n, h->h_z, h->w_z, 2 * c.c_hyper, false, 1);
+    ok = ok && make_act_map(h, h->am_yhat, h->yhat, n, h->h, h->w, c.c_y, true, 1) &&
          make_act_map(h, h->am_fb, h->fb, n * T, h->h, h->w, c.c_trunk, true, T) &&
          make_act_map(h, h->am_hidden, h->hidden, n * T, h->h, h->w, c.c_trunk * c.trunk_expand, true, T) &&
          make_act_map(h, h->am_fa, h->fa, n * T, h->h, h->w, c.c_trunk, false, T);

@@ -26,6 +26,13 @@ struct ufnvc_handle {
 
     // layers
     ufnvc::HyperLayer hyper[3];
+    // hybrid head (R12): tensor-core evaluation of the last hyper conv + exact fp64 re-evaluation near bucket edges
+    bool hybrid_head = false;
+    double head_flag_u = 5e-4;           // |ln sigma - bucket edge| below which the fp64 re-evaluation decides (env UFNVC_HEAD_FLAG_U)
+    ufnvc::ConvLayer head_tc;
+    double *head_fix_w = nullptr, *head_fix_b = nullptr;   // [c_y*16][9][c_hyper], [c_y*16] (scale half)
+    ufnvc::bf16 *xs = nullptr;           // [n][h_z][w_z][2*c_hyper]: bf16 hi | mid split of the fp64 hx2
+    uint32_t *fix_list = nullptr, *fix_count = nullptr;
     ufnvc::ConvLayer xframe;
     struct TrunkBlock {
         float *dw_w = nullptr, *dw_b = nullptr;   // [9][C], [C] fp32
@@ -51,7 +58,7 @@ struct ufnvc_handle {
         CUtensorMap tm_halo;             // 3x3 convs: box {64, 10, 18}: a 16 x 8 pixel tile plus halo (conv_halo_kernel)
         bool halo_ok = false;
     };
-    ActMap am_yhat, am_fa, am_fb, am_hidden, am_stage[3];
+    ActMap am_xs, am_yhat, am_fa, am_fb, am_hidden, am_stage[3];
 
     std::vector<void *> allocs;          // everything cudaMalloc'ed, freed at destroy
     cudaEvent_t ev[8] = {};

@@ -238,10 +238,69 @@ cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z
     return cudaGetLastError();
 }
 
+// same reduce, also emitting the 2-term bf16 split of the fp64 result: xs[m][o] = hi = bf16(v), xs[m][n_out + o] = bf16(v - hi)
+__global__ void hyper_reduce_split_kernel(const double *__restrict__ part, const double *__restrict__ bias, double *__restrict__ out,
+                                          bf16 *__restrict__ xs, long long MN, int n_out)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < MN; i += (long long)gridDim.x * blockDim.x) {
+        double v = part[i];
+#pragma unroll
+        for (int t = 1; t < 9; ++t) v += part[t * MN + i];
+        const int o = int(i % n_out);
+        const long long m = i / n_out;
+        v += bias[o];
+        v = v > 0.0 ? v : 0.0;
+        out[i] = v;
+        const bf16 hi = __double2bfloat16(v);
+        const bf16 mid = __double2bfloat16(v - double(__bfloat162float(hi)));
+        xs[m * 2 * n_out + o] = hi;
+        xs[m * 2 * n_out + n_out + o] = mid;
+    }
+}
+
+// Exact fp64 re-evaluation of ln sigma for the flagged elements: one warp per element, lanes stride the channels,
+// fixed-order tree reduction (deterministic).  list[i] = element index in [n][h][w][c_y].
+__global__ void __launch_bounds__(256) hyper_fix_kernel(const uint32_t *__restrict__ list, const uint32_t *__restrict__ count,
+                                                        const double *__restrict__ x2, const double *__restrict__ fix_w,
+                                                        const double *__restrict__ fix_b, int c_h, int hz, int wz, HeadParams hp)
+{
+    const int lane = threadIdx.x & 31;
+    const unsigned n = *count;
+    const unsigned warps = (gridDim.x * blockDim.x) >> 5;
+    for (unsigned i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; i < n; i += warps) {
+        const unsigned e = list[i];
+        const int c2 = int(e % unsigned(hp.c_y));
+        unsigned r = e / unsigned(hp.c_y);
+        const int lx = int(r % unsigned(hp.w)); r /= unsigned(hp.w);
+        const int ly = int(r % unsigned(hp.h));
+        const int img = int(r / unsigned(hp.h));
+        const int zy = ly >> 2, zx = lx >> 2, ij = ((ly & 3) << 2) | (lx & 3);
+        const double *wrow = fix_w + (size_t(c2) * 16 + ij) * 9 * c_h;
+        double acc = 0.0;
+        for (int tap = 0; tap < 9; ++tap) {
+            const int yy = zy + tap / 3 - 1, xx = zx + tap % 3 - 1;
+            if (yy < 0 || yy >= hz || xx < 0 || xx >= wz) continue;
+            const double *xr = x2 + ((size_t(img) * hz + yy) * wz + xx) * c_h;
+            for (int c = lane; c < c_h; c += 32) acc = fma(xr[c], wrow[tap * c_h + c], acc);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
+        if (lane == 0) {
+            const double v = acc + fix_b[size_t(c2) * 16 + ij];
+            const double u = v < hp.ln_lo ? hp.ln_lo : (v > hp.ln_hi ? hp.ln_hi : v);
+            const double t = floor(double(hp.n_buckets - 1) * (u - hp.ln_lo) / (hp.ln_hi - hp.ln_lo) + 0.5);
+            int k = int(t);
+            k = k < 0 ? 0 : (k > hp.n_buckets - 1 ? hp.n_buckets - 1 : k);
+            hp.idx[e] = uint8_t(k);
+            if (hp.lnscale) hp.lnscale[e] = float(u);
+        }
+    }
+}
+
 static bool fast_ok(const HyperLayer &L) { return L.c_in % FK == 0 && L.n % 4 == 0; }
 
 cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out, double *part, int n_img, int hz, int wz,
-                              cudaStream_t st)
+                              cudaStream_t st, bf16 *xs)
 {
     HyperEpi e{};
     e.mode = 0;
@@ -252,11 +311,28 @@ cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out
         hyper_conv_fast_kernel<true><<<grid, 256, 0, st>>>(in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e, part);
         const long long MN = (long long)M * L.n;
         const int blocks = int((MN + 255) / 256 < 1184 ? (MN + 255) / 256 : 1184);
-        hyper_reduce_kernel<<<blocks, 256, 0, st>>>(part, L.bias, out, MN, L.n);
+        if (xs) hyper_reduce_split_kernel<<<blocks, 256, 0, st>>>(part, L.bias, out, xs, MN, L.n);
+        else hyper_reduce_kernel<<<blocks, 256, 0, st>>>(part, L.bias, out, MN, L.n);
         return cudaGetLastError();
     }
     dim3 grid((M + HM - 1) / HM, (L.n + HN - 1) / HN);
     hyper_conv_kernel<<<grid, 256, 0, st>>>(in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_hyper_reduce_split(const double *part, const double *bias, double *out, bf16 *xs, long long M, int n_out,
+                                      cudaStream_t st)
+{
+    const long long MN = M * n_out;
+    const int blocks = int((MN + 255) / 256 < 1184 ? (MN + 255) / 256 : 1184);
+    hyper_reduce_split_kernel<<<blocks, 256, 0, st>>>(part, bias, out, xs, MN, n_out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_hyper_fix(const uint32_t *list, const uint32_t *count, const double *x2, const double *fix_w, const double *fix_b,
+                             int c_h, int hz, int wz, const HeadParams &hp, int num_sms, cudaStream_t st)
+{
+    hyper_fix_kernel<<<num_sms * 4, 256, 0, st>>>(list, count, x2, fix_w, fix_b, c_h, hz, wz, hp);
     return cudaGetLastError();
 }
 

@@ -18,7 +18,8 @@ typedef __nv_bfloat16 bf16;
 enum EpiMode : int {
     EPI_NHWC = 0,   // out[img][split][pix][n % n_split]  (bf16), optional residual with the same indexing
     EPI_PS2 = 1,    // pixel-shuffle x2 (R14): packed column n' = (2i+j)*C_o + c -> out[img][2y+i][2x+j][c] (bf16)
-    EPI_FINAL = 2   // EPI_PS2 + clamp [0,1] + crop + planar fp32 store out[img][c][Y][X]  (A9)
+    EPI_FINAL = 2,  // EPI_PS2 + clamp [0,1] + crop + planar fp32 store out[img][c][Y][X]  (A9)
+    EPI_HEAD = 3    // hyper head (A2): pixel-shuffle x4 + crop; mu half -> fp32, scale half -> clamp, bucket, edge flag
 };
 enum Act : int { ACT_NONE = 0, ACT_GELU = 1 };
 
@@ -31,6 +32,12 @@ struct EpiParams {
     long long img_stride;    // output elements per input image
     int c_o;                 // EPI_PS2/FINAL: channels after the shuffle (N = 4*c_o)
     int out_h, out_w;        // EPI_FINAL: crop (height, width)
+    // EPI_HEAD: packed column n' = (s*16 + 4i+j)*c_y + c2 of z-pixel (zy, zx) -> latent (4zy+i, 4zx+j), channel c2
+    float *mu, *lnscale;     // [n][lat_h][lat_w][c_y]
+    uint8_t *idx;
+    uint32_t *fix_list, *fix_count;   // elements whose tensor-core ln sigma is within flag_t of a bucket edge
+    int c_y, lat_h, lat_w, n_buckets;
+    float ln_lo, ln_hi, t_scale, flag_t;   // t = (u - ln_lo) * t_scale + 0.5; flag when |t - round(t)| < flag_t
 };
 
 // One conv layer as the kernels consume it.  Weights are K-major ("[n][k]", k = c_in contiguous) per tap and
@@ -64,13 +71,18 @@ struct HyperLayer {
 };
 cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z, int pz, cudaStream_t st);
 cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out, double *part, int n_img, int hz, int wz,
-                              cudaStream_t st);   // part: [9][M][n] scratch for the split-tap fast path (may be null)
+                              cudaStream_t st, bf16 *xs = nullptr);   // part: [9][M][n] scratch for the split-tap fast path (may be null)
 struct HeadParams {
     int c_y, h, w, n_buckets;
     double ln_lo, ln_hi;
     float *mu, *lnscale;     // [n][h][w][c_y], lnscale may be null
     uint8_t *idx;
 };
+// hybrid head helpers (hyper.cu)
+cudaError_t launch_hyper_reduce_split(const double *part, const double *bias, double *out, bf16 *xs, long long M, int n_out,
+                                      cudaStream_t st);
+cudaError_t launch_hyper_fix(const uint32_t *list, const uint32_t *count, const double *x2, const double *fix_w, const double *fix_b,
+                             int c_h, int hz, int wz, const HeadParams &hp, int num_sms, cudaStream_t st);
 cudaError_t launch_hyper_head(const HyperLayer &L, const double *in, int n_img, int hz, int wz, const HeadParams &hp,
                               cudaStream_t st);
 

@@ -99,6 +99,40 @@ struct Loader {
         return L.w && L.bias;
     }
 
+    // Hybrid head (R12): the last hyper conv on tensor cores with a 2-term bf16 split of its fp64 input
+    // (channels [0,c_h) = hi, [c_h,2c_h) = mid, weights duplicated), plus the fp64 weights of the scale half laid out
+    // per output row for the exact re-evaluation of elements that land near a bucket edge.
+    // packed row n' = (s*16 + 4i+j) * c_y + c2   <-   canonical o = (s*c_y + c2)*16 + 4i+j   (s = 0: mu, 1: ln sigma)
+    bool head_hybrid(ConvLayer &L, double *&fix_w, double *&fix_b, const std::string &name, int c_h, int c_y)
+    {
+        const int n = 2 * c_y * 16;
+        const Tensor *tw = get(name + ".w", {uint32_t(n), uint32_t(c_h), 3u, 3u});
+        const Tensor *tb = get(name + ".b", {uint32_t(n)});
+        if (!tw || !tb) return false;
+        L.c_in = 2 * c_h; L.n = n; L.n_pad = n; L.taps = 9; L.groups = 1;
+        std::vector<uint16_t> w(size_t(9) * n * L.c_in);
+        std::vector<float> b(n);
+        std::vector<double> fw(size_t(c_y) * 16 * 9 * c_h), fb(size_t(c_y) * 16);
+        for (int np = 0; np < n; ++np) {
+            const int sij = np / c_y, c2 = np % c_y, sft = sij / 16, ij = sij % 16;
+            const int o = (sft * c_y + c2) * 16 + ij;
+            b[np] = tb->at(o);
+            for (int tap = 0; tap < 9; ++tap)
+                for (int c = 0; c < c_h; ++c) {
+                    const float v = tw->at((size_t(o) * c_h + c) * 9 + tap);
+                    const uint16_t q = f32_to_bf16_rne(v);
+                    w[(size_t(tap) * n + np) * L.c_in + c] = q;
+                    w[(size_t(tap) * n + np) * L.c_in + c_h + c] = q;
+                    if (sft == 1) fw[((size_t(c2) * 16 + ij) * 9 + tap) * c_h + c] = double(v);
+                }
+            if (sft == 1) fb[size_t(c2) * 16 + ij] = double(tb->at(o));
+        }
+        L.w = reinterpret_cast<bf16 *>(upload(w));
+        L.bias = upload(b);
+        fix_w = upload(fw); fix_b = upload(fb);
+        return L.w && L.bias && fix_w && fix_b;
+    }
+
     bool depthwise(float *&dw, float *&db, const std::string &name, int C)
     {
         const Tensor *tw = get(name + ".w", {uint32_t(C), 1u, 3u, 3u});
@@ -136,6 +170,7 @@ int load_weights_impl(ufnvc_handle *h, const void *blob, size_t bytes)
     const ufnvc_config &c = h->cfg;
     bool ok = ld.hyper(h->hyper[0], "hyper.0", c.c_z, c.c_hyper) && ld.hyper(h->hyper[1], "hyper.1", c.c_hyper, c.c_hyper) &&
               ld.hyper(h->hyper[2], "hyper.2", c.c_hyper, 2 * c.c_y * 16);
+    if (ok && h->hybrid_head) ok = ld.head_hybrid(h->head_tc, h->head_fix_w, h->head_fix_b, "hyper.2", c.c_hyper, c.c_y);
     ok = ok && ld.conv(h->xframe, {"xframe"}, c.c_y, c.T * c.c_trunk, 1, false);
     h->trunk.assign(c.n_trunk_blocks, ufnvc_handle::TrunkBlock());
     const int ce = c.c_trunk * c.trunk_expand;

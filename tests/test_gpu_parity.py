@@ -71,7 +71,8 @@ def test_chunk_decode_matches_oracle(decoders, name):
         assert np.abs(out["lnscale"][n].cpu().numpy() - nhwc(ref["u"])).max() <= 1e-2
         # A3 + A4: integer work is bit-exact
         assert np.array_equal(out["sym"][n].cpu().numpy(), nhwc(ref["sym"]))
-        assert np.abs(out["yhat"][n].cpu().numpy() - nhwc(ref["yhat"])).max() <= 1e-5
+        # yhat = r + mu: r is bit-exact, so yhat inherits mu's tolerance (R13); the tensor-core mean is good to ~3e-5
+        assert np.abs(out["yhat"][n].cpu().numpy() - nhwc(ref["yhat"])).max() <= 1e-4
         # A5 .. A8 intermediates: bf16 storage, loose stage-wise bounds relative to the tensor's scale
         taps = ref["taps"]
         for t in range(cfg.T):
@@ -110,8 +111,10 @@ def test_entropy_params_entry_point(decoders):
     torch.cuda.synchronize()
     ref = case["chunks"][0]["out"]
     assert (idx[0].cpu().numpy() != nhwc(ref["idx"])).mean() <= IDX_RATE
-    assert np.abs(ls[0].cpu().numpy() - nhwc(ref["u"])).max() <= 1e-5
-    assert np.abs(mu[0].cpu().numpy() - nhwc(ref["mu"])).max() <= 1e-5
+    # north_star: mean and scale within 1e-2 relative.  The hybrid head (R12) evaluates both on tensor cores
+    # from a 2-term bf16 split (observed error <= 3e-5) and re-decides only the bucket of near-edge elements in fp64.
+    assert np.abs(ls[0].cpu().numpy() - nhwc(ref["u"])).max() <= 1e-4
+    assert np.abs(mu[0].cpu().numpy() - nhwc(ref["mu"])).max() <= 1e-4
 
 
 def test_tables_and_encoder_bit_equal_to_oracle(decoders, orc):
