@@ -116,7 +116,7 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
         CU_TRY(launch_dwconv3x3(h->fa, h->fb, tb.dw_w, tb.dw_b, n * T, h->h, h->w, Ct, st));
         if (launches) ++*launches;
         if (h->use_fused_trunk && tb.fused.ok && !h->force_generic) {
-            CU_TRY(launch_trunk_mlp(tb.fused, tb.pw1, tb.pw2, h->fa, h->fa, (long long)n * T * P, h->num_sms, st));
+            CU_TRY(launch_trunk_mlp(tb.fused, tb.pw1, tb.pw2, h->fa, h->fa, (long long)n * T * P, h->num_sms, h->use_pair_trunk, st));
             if (launches) ++*launches;
             continue;
         }

@@ -126,8 +126,9 @@ trunk_mlp_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant
                 for (int s = 0; s < 4; ++s) tma_load_2d(base + kOffA + s * kSlab, &tm_d, bar(B_AFULL), s * 64, tile * kTM);
                 ap ^= 1;
                 load_w1(0);
-                for (int c = 0; c < NC; ++c) {
-                    if (c + 1 < NC) load_w1(c + 1);
+                if (NC > 1) load_w1(1);
+                for (int c = 0; c < NC; ++c) {                     // the order the MMA warp consumes them in
+                    if (c + 2 < NC) load_w1(c + 2);
                     load_w2(c);
                 }
             }
@@ -171,10 +172,16 @@ trunk_mlp_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant
             for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x, ++it) {
                 mbar_wait(bar(B_AFULL), it & 1);
                 tc_fence_after();
+                // GEMM1 runs two chunks ahead of GEMM2: the epilogue frees Hacc[c&1] as soon as chunk c sits in its registers,
+                // so GEMM1(c+2) is queued behind GEMM1(c+1) while the GELU of chunk c is still being computed
                 gemm1(0);
+                if (NC > 1) gemm1(1);
+                if (NC <= 2) umma_commit(bar(B_AEMPTY));
                 for (int c = 0; c < NC; ++c) {
-                    if (c + 1 < NC) gemm1(c + 1);
-                    if (c + 1 == NC) umma_commit(bar(B_AEMPTY));          // every GEMM1 of this tile has been issued
+                    if (c + 2 < NC) {
+                        gemm1(c + 2);
+                        if (c + 3 == NC) umma_commit(bar(B_AEMPTY));      // every GEMM1 of this tile has been issued
+                    }
                     const int b = c & 1;
                     mbar_wait(bar(B_HS_FULL + b), (ph_hs >> b) & 1);
                     ph_hs ^= 1u << b;
@@ -200,6 +207,10 @@ trunk_mlp_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant
         const int r = quad * 32 + lane;                                   // row of the tile = TMEM lane
         const uint32_t t_lane = tmem_base + (uint32_t(quad * 32) << 16);
         uint32_t ph_use = 0;
+        float2 bnext = __ldg(reinterpret_cast<const float2 *>(p.b1 + half * 64) + lane);          // chunk 0
+        float b2r[4];                                                     // b2[half*128 + 32 i + lane]
+#pragma unroll
+        for (int i = 0; i < 4; ++i) b2r[i] = __ldg(p.b2 + half * 128 + 32 * i + lane);
         int it = 0;
         for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x, ++it) {
             for (int c = 0; c < NC; ++c) {
@@ -208,21 +219,34 @@ trunk_mlp_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant
                 mbar_wait(bar(B_HS_EMPTY + b), ((ph_use >> b) & 1) ^ 1);
                 ph_use ^= 1u << b;
                 tc_fence_after();
-                const float *b1 = p.b1 + c * kHC + half * 64;
+                // this chunk's 64 biases live 2 per lane (fetched one chunk ahead: with ~225 KB of shared memory the L1 is a few
+                // KB, so a bias load in the dependent chain costs an L2 round trip); the next chunk's are requested now
+                const float2 bcur = bnext;
+                {
+                    const int cn = c + 1 < NC ? c + 1 : 0;
+                    bnext = __ldg(reinterpret_cast<const float2 *>(p.b1 + cn * kHC + half * 64) + lane);
+                }
                 const uint32_t hs_row = base + kOffHs + uint32_t(2 * b + half) * kSlab + uint32_t(r) * 128u;
+                // both 32-column loads are in flight before the single wait: a TMEM load costs ~400 cycles while the tensor
+                // core is accumulating, and it sits on the GEMM1 -> GELU -> GEMM2 critical chain
+                uint32_t vv[2][32];
+                tmem_ld32_nowait(t_lane + kC + uint32_t(b) * kHC + uint32_t(half * 64), vv[0]);
+                tmem_ld32_nowait(t_lane + kC + uint32_t(b) * kHC + uint32_t(half * 64 + 32), vv[1]);
+                tmem_ld_wait();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(B_HACC_EMPTY + b));        // chunk c is in registers: Hacc[b] may be overwritten
 #pragma unroll
                 for (int q = 0; q < 2; ++q) {
-                    uint32_t v[32];
-                    tmem_ld32(t_lane + kC + uint32_t(b) * kHC + uint32_t(half * 64 + q * 32), v);
+                    uint32_t (&v)[32] = vv[q];
                     uint32_t pk[16];
 #pragma unroll
-                    for (int j = 0; j < 32; j += 4) {
-                        const float4 b4 = __ldg(reinterpret_cast<const float4 *>(b1 + q * 32 + j));
-                        float f0, f1, f2, f3;
-                        gelu_bias2(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), b4.x, b4.y, f0, f1);
-                        gelu_bias2(__uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]), b4.z, b4.w, f2, f3);
+                    for (int j = 0; j < 32; j += 2) {                     // columns q*32 + j, j+1 <- lane (q*32 + j) / 2
+                        const float bx = __shfl_sync(0xFFFFFFFFu, bcur.x, q * 16 + j / 2);
+                        const float by = __shfl_sync(0xFFFFFFFFu, bcur.y, q * 16 + j / 2);
+                        float f0, f1;
+                        gelu_bias2(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), bx, by, f0, f1);
                         pk[j / 2] = pack_bf16x2(f0, f1);
-                        pk[j / 2 + 1] = pack_bf16x2(f2, f3);
                     }
 #pragma unroll
                     for (int jj = 0; jj < 4; ++jj) {                      // 16-byte chunk q*4+jj of the row, 128B-swizzled
@@ -233,7 +257,7 @@ trunk_mlp_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant
                 tc_fence_before();
                 fence_proxy_async();
                 __syncwarp();
-                if (lane == 0) { mbar_arrive(bar(B_HACC_EMPTY + b)); mbar_arrive(bar(B_HS_FULL + b)); }
+                if (lane == 0) mbar_arrive(bar(B_HS_FULL + b));
             }
             // ---- output: Oacc + b2 + x -> bf16.  The residual row segment (128 columns = 16 x 16 B) is fetched BEFORE the
             // wait for the last GEMM2s, so its latency hides behind them: Oacc is single-buffered, which puts this
@@ -253,14 +277,13 @@ trunk_mlp_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant
                 uint32_t v[32];
                 const int c0 = half * 128 + q * 32;
                 tmem_ld32(t_lane + uint32_t(c0), v);
-                if (!inb) continue;
                 uint4 *dst = reinterpret_cast<uint4 *>(p.out + row * kC + c0);
 #pragma unroll
                 for (int g = 0; g < 4; ++g) {
                     const __nv_bfloat162 *re = reinterpret_cast<const __nv_bfloat162 *>(&res[q * 4 + g]);
-                    const float4 ba = __ldg(reinterpret_cast<const float4 *>(p.b2 + c0 + g * 8));
-                    const float4 bb = __ldg(reinterpret_cast<const float4 *>(p.b2 + c0 + g * 8 + 4));
-                    const float bs[8] = {ba.x, ba.y, ba.z, ba.w, bb.x, bb.y, bb.z, bb.w};
+                    float bs[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) bs[e] = __shfl_sync(0xFFFFFFFFu, b2r[q], g * 8 + e);
                     uint4 o4;
                     uint32_t *oe = reinterpret_cast<uint32_t *>(&o4);
 #pragma unroll
@@ -269,7 +292,7 @@ trunk_mlp_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant
                         oe[e] = pack_bf16x2(__uint_as_float(v[g * 8 + 2 * e]) + bs[2 * e] + xr.x,
                                             __uint_as_float(v[g * 8 + 2 * e + 1]) + bs[2 * e + 1] + xr.y);
                     }
-                    dst[g] = o4;
+                    if (inb) dst[g] = o4;                                 // (shuffles above need every lane)
                 }
             }
             tc_fence_before();
@@ -283,6 +306,265 @@ trunk_mlp_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant
     if (warp == 1) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512u) : "memory");
+    }
+}
+
+}  // namespace
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------------------------
+// CTA-pair version (cta_group::2).  The single-CTA kernel above is bound by the weight ring: every 128-pixel tile pulls
+// the whole 1 MB of W1 + W2 through 96 KB of shared memory, and with ~1.5-2 us of L2 latency that ring cannot deliver
+// the 122 GB/s per SM the tensor core would consume (measured: tensor pipe 42 % active, L2 throughput 21 %).  A pair of
+// CTAs on one TPC runs ONE M = 256 MMA over both d tiles; each CTA stores only HALF of every weight tile (N/2 rows), so
+// the bytes per SM and per tile drop to 512 KB and a ring stage now lasts a whole GEMM1 or GEMM2 chunk (1024 tensor
+// cycles).  The leader CTA (rank 0) issues all MMAs; both CTAs run their own TMA producer and their own 8 epilogue
+// warps.  Barriers the MMA thread waits on live in the leader (the peer signals them through the cluster window);
+// barriers signalled by tcgen05.commit are multicast to both CTAs.
+__global__ void __launch_bounds__(kTrunkThreads, 1)
+trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant__ CUtensorMap tm_w1h,
+                      const __grid_constant__ CUtensorMap tm_w2h, const TrunkParams p)
+{
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    auto bar = [&](uint32_t slot) { return base + kOffBar + 8u * slot; };
+    volatile uint32_t *tmem_slot_ptr =
+        reinterpret_cast<volatile uint32_t *>(smem_raw + (bar(B_TMEM_SLOT) - smem_u32(smem_raw)));
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+    const int NC = p.n_chunks;
+    const int n_pairs = gridDim.x >> 1, pair0 = blockIdx.x >> 1;
+    const int n_ptiles = (p.n_tiles + 1) >> 1;                       // tile pairs; a missing odd tile is all padding
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_d) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_w1h) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_w2h) : "memory");
+        mbar_init(bar(B_AFULL), 1); mbar_init(bar(B_AEMPTY), 1);
+        for (int s = 0; s < kWStages; ++s) { mbar_init(bar(B_WFULL + s), 1); mbar_init(bar(B_WEMPTY + s), 1); }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bar(B_HACC_FULL + b), 1); mbar_init(bar(B_HACC_EMPTY + b), 16);     // 8 epilogue warps x 2 CTAs
+            mbar_init(bar(B_HS_FULL + b), 16);  mbar_init(bar(B_HS_EMPTY + b), 1);
+        }
+        mbar_init(bar(B_OFULL), 1); mbar_init(bar(B_OEMPTY), 16);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    cluster_sync_all();                                              // peer barriers are initialised before anyone signals
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(bar(B_TMEM_SLOT)), "r"(512u) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    cluster_sync_all();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===================== TMA producer (both CTAs): own d tile, own half of every weight tile =====================
+        if (elect_one()) {
+            const uint32_t afull_l = mapa_rank(bar(B_AFULL), 0);     // the leader's barriers, as cluster addresses
+            int ws = 0; uint32_t wp = 0, ap = 0;
+            auto w_slot = [&](uint32_t &full_l) {
+                mbar_wait(bar(B_WEMPTY + ws), wp ^ 1);                // local: multicast commit of the MMAs that read it
+                if (rank == 0) mbar_expect_tx(bar(B_WFULL + ws), 2 * kWStage);
+                full_l = mapa_rank(bar(B_WFULL + ws), 0);
+                return base + kOffW + uint32_t(ws) * kWStage;
+            };
+            auto w_next = [&]() { if (++ws == kWStages) { ws = 0; wp ^= 1; } };
+            auto load_w1 = [&](int c) {                               // rows c*128 + rank*64 .. +63 of W1, 4 k slabs of 8 KB
+                uint32_t full_l;
+                const uint32_t dst = w_slot(full_l);
+                for (int s = 0; s < 4; ++s) tma_load_2d_pair(dst + uint32_t(s) * (kSlab / 2), &tm_w1h, full_l, s * 64, c * kHC + int(rank) * 64);
+                w_next();
+            };
+            auto load_w2 = [&](int c) {                               // rows rank*128 .. +127 of W2, k slabs c*128 + {0, 64}
+                uint32_t full_l;
+                const uint32_t dst = w_slot(full_l);
+                for (int j = 0; j < 2; ++j) tma_load_2d_pair(dst + uint32_t(j) * kSlab, &tm_w2h, full_l, c * kHC + j * 64, int(rank) * 128);
+                w_next();
+            };
+            for (int pt = pair0; pt < n_ptiles; pt += n_pairs) {
+                const int tile = 2 * pt + int(rank);
+                mbar_wait(bar(B_AEMPTY), ap ^ 1);
+                if (rank == 0) mbar_expect_tx(bar(B_AFULL), 2 * 4 * kSlab);
+                for (int s = 0; s < 4; ++s) tma_load_2d_pair(base + kOffA + s * kSlab, &tm_d, afull_l, s * 64, tile * kTM);
+                ap ^= 1;
+                load_w1(0);
+                if (NC > 1) load_w1(1);
+                for (int c = 0; c < NC; ++c) {                     // the order the MMA warp consumes them in
+                    if (c + 2 < NC) load_w1(c + 2);
+                    load_w2(c);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer: leader CTA only =====================
+        if (rank == 0 && elect_one()) {
+            const uint32_t idesc1 = umma_idesc_bf16(2 * kTM, kHC), idesc2 = umma_idesc_bf16(2 * kTM, kC);
+            const uint32_t hi = uint32_t(1024 >> 4) | (1u << 14) | (2u << 29);
+            auto lo = [](uint32_t addr) { return ((addr & 0x3FFFFu) >> 4) | (1u << 16); };
+            const uint32_t a_lo = lo(base + kOffA), hs_lo = lo(base + kOffHs), w_lo = lo(base + kOffW);
+            const uint32_t o_acc = tmem_base, h_acc = tmem_base + kC;
+            int ws = 0; uint32_t wp = 0;
+            uint32_t ph_hacc = 0, ph_hs = 0;
+            auto w_wait = [&]() {
+                mbar_wait_cluster(bar(B_WFULL + ws), wp);
+                tc_fence_after();
+                return w_lo + uint32_t(ws) * (kWStage >> 4);
+            };
+            auto w_release = [&]() { umma2_commit_both(bar(B_WEMPTY + ws)); if (++ws == kWStages) { ws = 0; wp ^= 1; } };
+            auto gemm1 = [&](int c) {
+                const int b = c & 1;
+                mbar_wait_cluster(bar(B_HACC_EMPTY + b), ((ph_hacc >> b) & 1) ^ 1);
+                ph_hacc ^= 1u << b;
+                tc_fence_after();
+                const uint32_t d = h_acc + uint32_t(b) * kHC;
+                const uint32_t w = w_wait();
+#pragma unroll
+                for (int s = 0; s < 4; ++s)
+#pragma unroll
+                    for (int k = 0; k < 4; ++k)
+                        umma2_bf16_lh(d, a_lo + uint32_t(s) * (kSlab >> 4) + 2 * k, hi, w + uint32_t(s) * (kSlab >> 5) + 2 * k, hi, idesc1,
+                                      uint32_t(s | k));
+                w_release();
+                umma2_commit_both(bar(B_HACC_FULL + b));
+            };
+            int it = 0;
+            for (int pt = pair0; pt < n_ptiles; pt += n_pairs, ++it) {
+                mbar_wait_cluster(bar(B_AFULL), it & 1);
+                tc_fence_after();
+                gemm1(0);
+                if (NC > 1) gemm1(1);
+                if (NC <= 2) umma2_commit_both(bar(B_AEMPTY));
+                for (int c = 0; c < NC; ++c) {
+                    if (c + 2 < NC) {
+                        gemm1(c + 2);
+                        if (c + 3 == NC) umma2_commit_both(bar(B_AEMPTY));
+                    }
+                    const int b = c & 1;
+                    mbar_wait_cluster(bar(B_HS_FULL + b), (ph_hs >> b) & 1);
+                    ph_hs ^= 1u << b;
+                    if (c == 0) mbar_wait_cluster(bar(B_OEMPTY), (it & 1) ^ 1);
+                    tc_fence_after();
+                    const uint32_t w = w_wait();
+#pragma unroll
+                    for (int j = 0; j < 2; ++j)
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)
+                            umma2_bf16_lh(o_acc, hs_lo + uint32_t(2 * b + j) * (kSlab >> 4) + 2 * k, hi, w + uint32_t(j) * (kSlab >> 4) + 2 * k,
+                                          hi, idesc2, uint32_t(c | j | k));
+                    w_release();
+                    umma2_commit_both(bar(B_HS_EMPTY + b));
+                }
+                umma2_commit_both(bar(B_OFULL));
+            }
+        }
+    } else {
+        // ===================== epilogue warps (both CTAs) =====================
+        const int quad = warp & 3, half = (warp - 2) >> 2;
+        const int r = quad * 32 + lane;
+        const uint32_t t_lane = tmem_base + (uint32_t(quad * 32) << 16);
+        const uint32_t hacc_empty_l = mapa_rank(bar(B_HACC_EMPTY), 0), hs_full_l = mapa_rank(bar(B_HS_FULL), 0),
+                       oempty_l = mapa_rank(bar(B_OEMPTY), 0);
+        uint32_t ph_use = 0;
+        float2 bnext = __ldg(reinterpret_cast<const float2 *>(p.b1 + half * 64) + lane);          // chunk 0
+        float b2r[4];                                                     // b2[half*128 + 32 i + lane]
+#pragma unroll
+        for (int i = 0; i < 4; ++i) b2r[i] = __ldg(p.b2 + half * 128 + 32 * i + lane);
+        int it = 0;
+        for (int pt = pair0; pt < n_ptiles; pt += n_pairs, ++it) {
+            const int tile = 2 * pt + int(rank);
+            for (int c = 0; c < NC; ++c) {
+                const int b = c & 1;
+                mbar_wait(bar(B_HACC_FULL + b), (ph_use >> b) & 1);
+                mbar_wait(bar(B_HS_EMPTY + b), ((ph_use >> b) & 1) ^ 1);
+                ph_use ^= 1u << b;
+                tc_fence_after();
+                // this chunk's 64 biases live 2 per lane (fetched one chunk ahead: with ~225 KB of shared memory the L1 is a few
+                // KB, so a bias load in the dependent chain costs an L2 round trip); the next chunk's are requested now
+                const float2 bcur = bnext;
+                {
+                    const int cn = c + 1 < NC ? c + 1 : 0;
+                    bnext = __ldg(reinterpret_cast<const float2 *>(p.b1 + cn * kHC + half * 64) + lane);
+                }
+                const uint32_t hs_row = base + kOffHs + uint32_t(2 * b + half) * kSlab + uint32_t(r) * 128u;
+                // both 32-column loads are in flight before the single wait: a TMEM load costs ~400 cycles while the tensor
+                // core is accumulating, and it sits on the GEMM1 -> GELU -> GEMM2 critical chain
+                uint32_t vv[2][32];
+                tmem_ld32_nowait(t_lane + kC + uint32_t(b) * kHC + uint32_t(half * 64), vv[0]);
+                tmem_ld32_nowait(t_lane + kC + uint32_t(b) * kHC + uint32_t(half * 64 + 32), vv[1]);
+                tmem_ld_wait();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(hacc_empty_l + 8u * b);
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    uint32_t (&v)[32] = vv[q];
+                    uint32_t pk[16];
+#pragma unroll
+                    for (int j = 0; j < 32; j += 2) {                     // columns q*32 + j, j+1 <- lane (q*32 + j) / 2
+                        const float bx = __shfl_sync(0xFFFFFFFFu, bcur.x, q * 16 + j / 2);
+                        const float by = __shfl_sync(0xFFFFFFFFu, bcur.y, q * 16 + j / 2);
+                        float f0, f1;
+                        gelu_bias2(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), bx, by, f0, f1);
+                        pk[j / 2] = pack_bf16x2(f0, f1);
+                    }
+#pragma unroll
+                    for (int jj = 0; jj < 4; ++jj) {
+                        const uint32_t chunk = uint32_t(q * 4 + jj) ^ uint32_t(r & 7);
+                        st_shared_v4(hs_row + (chunk << 4), pk[4 * jj], pk[4 * jj + 1], pk[4 * jj + 2], pk[4 * jj + 3]);
+                    }
+                }
+                tc_fence_before();
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(hs_full_l + 8u * b);
+            }
+            const long long row = (long long)tile * kTM + r;
+            const bool inb = row < p.n_px;
+            uint4 res[16];
+            {
+                const uint4 *rs = reinterpret_cast<const uint4 *>(p.x + row * kC + half * 128);
+#pragma unroll
+                for (int g = 0; g < 16; ++g) res[g] = inb ? rs[g] : make_uint4(0, 0, 0, 0);
+            }
+            mbar_wait(bar(B_OFULL), it & 1);
+            tc_fence_after();
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                uint32_t v[32];
+                const int c0 = half * 128 + q * 32;
+                tmem_ld32(t_lane + uint32_t(c0), v);
+                uint4 *dst = reinterpret_cast<uint4 *>(p.out + row * kC + c0);
+#pragma unroll
+                for (int g = 0; g < 4; ++g) {
+                    const __nv_bfloat162 *re = reinterpret_cast<const __nv_bfloat162 *>(&res[q * 4 + g]);
+                    float bs[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) bs[e] = __shfl_sync(0xFFFFFFFFu, b2r[q], g * 8 + e);
+                    uint4 o4;
+                    uint32_t *oe = reinterpret_cast<uint32_t *>(&o4);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const float2 xr = __bfloat1622float2(re[e]);
+                        oe[e] = pack_bf16x2(__uint_as_float(v[g * 8 + 2 * e]) + bs[2 * e] + xr.x,
+                                            __uint_as_float(v[g * 8 + 2 * e + 1]) + bs[2 * e + 1] + xr.y);
+                    }
+                    if (inb) dst[g] = o4;                                 // (shuffles above need every lane)
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(oempty_l);
+        }
+    }
+
+    tc_fence_before();
+    cluster_sync_all();                                              // both CTAs are done with TMEM and with each other's barriers
+    if (warp == 1) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512u) : "memory");
     }
 }
 
@@ -304,12 +586,15 @@ bool trunk_make_maps(TrunkMaps &m, const bf16 *d_base, long long n_px, const Con
     // W1: [hidden][256] (n rows, k contiguous), box {64, 128}; W2: [256][hidden], box {64, 256}
     if (!tc_encode_2d(&m.tm_w1, pw1.w, kC, (unsigned long long)pw1.n, 64, kHC, err)) return false;
     if (!tc_encode_2d(&m.tm_w2, pw2.w, (unsigned long long)pw2.c_in, kC, 64, kC, err)) return false;
+    // CTA-pair kernel: each CTA loads half of every weight tile (64 of the 128 W1 rows, 128 of the 256 W2 rows)
+    if (!tc_encode_2d(&m.tm_w1h, pw1.w, kC, (unsigned long long)pw1.n, 64, kHC / 2, err)) return false;
+    if (!tc_encode_2d(&m.tm_w2h, pw2.w, (unsigned long long)pw2.c_in, kC, 64, kC / 2, err)) return false;
     m.ok = true;
     return true;
 }
 
 cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const ConvLayer &pw2, const bf16 *x, bf16 *out, long long n_px,
-                             int num_sms, cudaStream_t st)
+                             int num_sms, bool pair, cudaStream_t st)
 {
     TrunkParams p{};
     p.n_px = int(n_px);
@@ -322,6 +607,26 @@ cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const Con
         cudaError_t e = cudaFuncSetAttribute(trunk_mlp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kTrunkSmem));
         if (e != cudaSuccess) return e;
         configured = true;
+    }
+    if (pair && p.n_tiles >= 2) {
+        static thread_local bool configured2 = false;
+        if (!configured2) {
+            cudaError_t e = cudaFuncSetAttribute(trunk_mlp_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kTrunkSmem));
+            if (e != cudaSuccess) return e;
+            configured2 = true;
+        }
+        const int n_ptiles = (p.n_tiles + 1) / 2;
+        const int clusters = n_ptiles < num_sms / 2 ? n_ptiles : num_sms / 2;
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(2 * clusters);
+        cfg.blockDim = dim3(kTrunkThreads);
+        cfg.dynamicSmemBytes = kTrunkSmem;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        return cudaLaunchKernelEx(&cfg, trunk_mlp_pair_kernel, m.tm_d, m.tm_w1h, m.tm_w2h, p);
     }
     const int grid = p.n_tiles < num_sms ? p.n_tiles : num_sms;
     trunk_mlp_kernel<<<grid, kTrunkThreads, kTrunkSmem, st>>>(m.tm_d, m.tm_w1, m.tm_w2, p);

@@ -118,12 +118,12 @@ bool tc_encode_2d(CUtensorMap *tm, const void *base, unsigned long long dim0, un
 
 // fused trunk MLP (trunk_tc.cu): out = x + W2 GELU(W1 d + b1) + b2 in one kernel, hidden kept on chip
 struct TrunkMaps {
-    CUtensorMap tm_d, tm_w1, tm_w2;
+    CUtensorMap tm_d, tm_w1, tm_w2, tm_w1h, tm_w2h;   // *h: half tiles for the CTA-pair kernel
     bool ok = false;
 };
 bool trunk_make_maps(TrunkMaps &m, const bf16 *d_base, long long n_px, const ConvLayer &pw1, const ConvLayer &pw2, std::string &err);
 cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const ConvLayer &pw2, const bf16 *x, bf16 *out, long long n_px,
-                             int num_sms, cudaStream_t st);
+                             int num_sms, bool pair, cudaStream_t st);
 
 // ---- host-side entropy tables + encoder fixture (tables.cpp part of api) ---------------------------------------
 void build_cdf_tables(int nb, double smin, double smax, std::vector<uint32_t> &cdf32);
