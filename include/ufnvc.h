@@ -124,7 +124,8 @@ int ufnvc_get_status(ufnvc_handle *h, uint32_t *device_status);
 /* Human-readable text of the last failing call on this handle (never NULL; NULL handle -> static text). */
 const char *ufnvc_last_error(const ufnvc_handle *h);
 
-/* Number of kernels / async copies ufnvc_chunk_decode enqueues per call for n_chunks (for bench accounting). */
+/* Number of this library's kernels one ufnvc_chunk_decode call enqueues (memsets and copies not counted): the count
+ * recorded by the last decode on this handle, else the default path's. For bench accounting. */
 int ufnvc_launches_per_call(const ufnvc_handle *h, int n_chunks);
 
 /* Per-stage device time of the LAST ufnvc_chunk_decode_profiled call, in microseconds.

@@ -35,6 +35,9 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
         float *mu_out, float *ls_out, uint8_t *idx_out, Stage *sg, int *launches)
 {
     const ufnvc_config &c = h->cfg;
+    int local_launches = 0;                    // kernels of this library enqueued by this call (memsets / copies not counted)
+    if (!launches) launches = &local_launches;
+    struct Publish { ufnvc_handle *h; int *n; ~Publish() { h->last_launches = *n; } } publish{h, launches};
     const int P = h->h * h->w, Pz = h->h_z * h->w_z;
     const size_t ne = size_t(n) * P * c.c_y;
 
@@ -62,12 +65,14 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
             CU_TRY(launch_conv_tc(h->head_tc, pr, h->am_xs.tm, h->am_xs.tile_h, h->am_xs.tile_w, false, E, h->num_sms, st));
             CU_TRY(launch_hyper_fix(h->fix_list, h->fix_count, h->hx2, h->head_fix_w, h->head_fix_b, c.c_hyper, h->h_z, h->w_z, hp,
                                     h->num_sms, st));
-            if (launches) *launches += 3;
+            *launches += 2;                    // head conv + fp64 fix
         } else {
             CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, h->hpart, n, h->h_z, h->w_z, st));
             CU_TRY(launch_hyper_head(h->hyper[2], h->hx2, n, h->h_z, h->w_z, hp, st));
         }
-        if (launches) *launches += 4;
+        auto hyper_kernels = [](const HyperLayer &L) { return (L.c_in % 16 == 0 && L.n % 4 == 0) ? 2 : 1; };   // split-tap + reduce
+        *launches += 1 + hyper_kernels(h->hyper[0]) + hyper_kernels(h->hyper[1]);
+        if (!(h->hybrid_head && h->am_xs.ok && h->head_tc.use_tc)) *launches += 1;
     }
     if (entropy_params_only) {
         if (mu_out) CU_TRY(cudaMemcpyAsync(mu_out, h->mu, ne * 4, cudaMemcpyDeviceToDevice, st));
@@ -94,7 +99,7 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     rp.yhat = h->yhat; rp.sym_tap = taps ? taps->sym : nullptr; rp.yhat_tap = taps ? taps->yhat : nullptr;
     rp.status = h->d_status;
     CU_TRY(launch_rans_decode(rp, st));
-    if (launches) *launches += 2;
+    *launches += 1;                            // rANS decode
     mark(sg, st);
     if (!frames) return UFNVC_OK;
 
@@ -260,8 +265,10 @@ extern "C" int ufnvc_entropy_params(ufnvc_handle *h, int n_chunks, const int16_t
 extern "C" int ufnvc_launches_per_call(const ufnvc_handle *h, int n_chunks)
 {
     if (!h || n_chunks < 1) return UFNVC_E_INVALID_ARG;
-    // 4 hyper + memset + rANS + A5 + 3 per trunk block + 4 decoder stages
-    return 4 + 2 + 1 + 3 * h->cfg.n_trunk_blocks + 4;
+    // kernels counted by the last decode on this handle (the count does not depend on n_chunks); before any decode, the
+    // count of the default path: 7 hyper (hybrid head) + rANS + A5 + (depthwise + fused MLP) per trunk block + 4 stages
+    if (h->last_launches > 0) return h->last_launches;
+    return 7 + 1 + 1 + 2 * h->cfg.n_trunk_blocks + 4;
 }
 
 extern "C" int ufnvc_chunk_decode_profiled(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, const uint8_t *bits_dev,
