@@ -3,6 +3,7 @@
 // the on-device cross-check of the tensor-core path.  Activations NHWC bf16, fp32 accumulate.
 //   out[pix][n] = bias[n] + sum_{tap, c} in[pix + tap][c] * w[group][tap][n][c]
 #include "epilogue.cuh"
+#include "tc_ptx.cuh"
 #include "ufnvc_internal.h"
 
 namespace ufnvc {
@@ -180,6 +181,112 @@ __global__ void __launch_bounds__(256, 2) dwconv3x3_kernel(const bf16 *__restric
 #pragma unroll
         for (int e = 0; e < 4; ++e) { accP[e] = accC[e]; accC[e] = accN[e]; accN[e] = bv[e]; }
     }
+}
+
+// ---- A6, TMA-staged variant (C a multiple of 64).  One block = an 8 x 8 pixel tile of one image, all channels: one
+// TMA box {64 ch, 10, 10} per 64-channel slab brings the tile plus halo into shared memory (zero-filled outside the
+// image = the conv's zero padding), so ~50 KB per block x 4 blocks per SM are in flight without costing a register --
+// the register-only kernel above is latency-bound (16 warps/SM, 8 KB of unique loads in flight, 28 % of HBM peak).
+// Thread (x, c8) then walks down its column with the same rolling 3-row window, reading 3 conflict-free LDS.128 per row.
+constexpr int kDwT = 8;                                   // tile edge (pixels)
+constexpr int kDwHalo = kDwT + 2;
+constexpr uint32_t kDwSlab = ((kDwHalo * kDwHalo * 128 + 1023) / 1024) * 1024;     // 13312 B, 1024-aligned for the swizzle
+
+__global__ void __launch_bounds__(256, 2) dwconv3x3_tma_kernel(const __grid_constant__ CUtensorMap tm_in, bf16 *__restrict__ out,
+                                                             const float *__restrict__ w9c, const float *__restrict__ bias,
+                                                             int H, int W, int C, int tiles_x, int tiles_y)
+{
+    extern __shared__ __align__(1024) uint8_t dw_smem[];
+    const uint32_t base = (smem_u32(dw_smem) + 1023u) & ~1023u;
+    const int slabs = C >> 6;
+    const uint32_t bar = base + uint32_t(slabs) * kDwSlab;
+    int tile = blockIdx.x;
+    const int tx = tile % tiles_x; tile /= tiles_x;
+    const int ty = tile % tiles_y;
+    const int img = tile / tiles_y;
+    const int x0 = tx * kDwT, y0 = ty * kDwT;
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_expect_tx(bar, uint32_t(slabs) * (kDwHalo * kDwHalo * 128));
+        for (int s = 0; s < slabs; ++s) tma_load_4d(base + uint32_t(s) * kDwSlab, &tm_in, bar, s * 64, x0 - 1, y0 - 1, img);
+    }
+    const int cv = C >> 3;
+    const int xl = threadIdx.x / cv, c8 = threadIdx.x % cv;           // column of the tile, 8-channel group
+    const int c0 = c8 * 8;
+    uint64_t wv[9][4], bv[4];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        const float4 lo = __ldg(reinterpret_cast<const float4 *>(w9c + k * C + c0));
+        const float4 hi = __ldg(reinterpret_cast<const float4 *>(w9c + k * C + c0 + 4));
+        wv[k][0] = f2_pack(lo.x, lo.y); wv[k][1] = f2_pack(lo.z, lo.w);
+        wv[k][2] = f2_pack(hi.x, hi.y); wv[k][3] = f2_pack(hi.z, hi.w);
+    }
+    {
+        const float4 lo = __ldg(reinterpret_cast<const float4 *>(bias + c0)), hi = __ldg(reinterpret_cast<const float4 *>(bias + c0 + 4));
+        bv[0] = f2_pack(lo.x, lo.y); bv[1] = f2_pack(lo.z, lo.w); bv[2] = f2_pack(hi.x, hi.y); bv[3] = f2_pack(hi.z, hi.w);
+    }
+    __syncthreads();                                                  // barrier initialised before anyone polls it
+    mbar_wait(bar, 0);
+
+    const uint32_t slab_base = base + uint32_t(c8 >> 3) * kDwSlab;
+    const uint32_t chunk = uint32_t(c8 & 7);
+    auto lds = [&](int hy, int hx) {                                  // halo pixel -> this thread's 16 bytes (128B swizzle)
+        const uint32_t p = uint32_t(hy * kDwHalo + hx);
+        uint4 v;
+        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                     : "r"(slab_base + p * 128u + ((chunk ^ (p & 7u)) << 4)));
+        return v;
+    };
+    uint64_t accP[4], accC[4], accN[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) { accP[e] = bv[e]; accC[e] = bv[e]; accN[e] = bv[e]; }
+    const int ox = x0 + xl;
+    bf16 *col_out = out + (((long long)img * H) * W + ox) * C + c0;
+#pragma unroll
+    for (int hy = 0; hy < kDwHalo; ++hy) {                            // halo row hy = image row y0 - 1 + hy
+        const uint4 vl = lds(hy, xl), vc = lds(hy, xl + 1), vr = lds(hy, xl + 2);
+        const uint32_t *pl = reinterpret_cast<const uint32_t *>(&vl), *pc = reinterpret_cast<const uint32_t *>(&vc),
+                       *pr = reinterpret_cast<const uint32_t *>(&vr);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const uint64_t fl = dw_pair(pl[e]), fc = dw_pair(pc[e]), fr = dw_pair(pr[e]);
+            accP[e] = f2_fma(wv[6][e], fl, f2_fma(wv[7][e], fc, f2_fma(wv[8][e], fr, accP[e])));
+            accC[e] = f2_fma(wv[3][e], fl, f2_fma(wv[4][e], fc, f2_fma(wv[5][e], fr, accC[e])));
+            accN[e] = f2_fma(wv[0][e], fl, f2_fma(wv[1][e], fc, f2_fma(wv[2][e], fr, accN[e])));
+        }
+        if (hy >= 2) {                                                // output row y0 + hy - 2 is complete
+            const int oy = y0 + hy - 2;
+            if (oy < H && ox < W) {
+                uint4 o;
+                __nv_bfloat162 *oe = reinterpret_cast<__nv_bfloat162 *>(&o);
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    float a, b;
+                    f2_unpack(accP[e], a, b);
+                    oe[e] = __floats2bfloat162_rn(a, b);
+                }
+                *reinterpret_cast<uint4 *>(col_out + (long long)oy * W * C) = o;
+            }
+        }
+#pragma unroll
+        for (int e = 0; e < 4; ++e) { accP[e] = accC[e]; accC[e] = accN[e]; accN[e] = bv[e]; }
+    }
+}
+
+cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
+                                 int C, cudaStream_t st)
+{
+    const int tiles_x = (W + kDwT - 1) / kDwT, tiles_y = (H + kDwT - 1) / kDwT;
+    const size_t smem = 1024 + size_t(C >> 6) * kDwSlab + 16;
+    static thread_local bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(dwconv3x3_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dwconv3x3_tma_kernel<<<n_img * tiles_x * tiles_y, C, smem, st>>>(tm_in, out, w9c, bias, H, W, C, tiles_x, tiles_y);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_dwconv3x3(const bf16 *in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,

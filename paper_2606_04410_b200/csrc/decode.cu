@@ -2,6 +2,7 @@
 // One host call, zero host synchronisations, everything on the caller's stream.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 #include "handle.h"
@@ -118,7 +119,8 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     const int Ce = Ct * c.trunk_expand;
     for (int k = 0; k < c.n_trunk_blocks; ++k) {
         const ufnvc_handle::TrunkBlock &tb = h->trunk[k];
-        CU_TRY(launch_dwconv3x3(h->fa, h->fb, tb.dw_w, tb.dw_b, n * T, h->h, h->w, Ct, st));
+        if (h->dw_tma_ok) CU_TRY(launch_dwconv3x3_tma(h->tm_dw, h->fb, tb.dw_w, tb.dw_b, n * T, h->h, h->w, Ct, st));
+        else CU_TRY(launch_dwconv3x3(h->fa, h->fb, tb.dw_w, tb.dw_b, n * T, h->h, h->w, Ct, st));
         if (launches) ++*launches;
         if (h->use_fused_trunk && tb.fused.ok && !h->force_generic) {
             CU_TRY(launch_trunk_mlp(tb.fused, tb.pw1, tb.pw2, h->fa, h->fa, (long long)n * T * P, h->num_sms, h->use_pair_trunk, st));
@@ -224,6 +226,14 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
          make_act_map(h, h->am_fb, h->fb, n * T, h->h, h->w, c.c_trunk, true, T) &&
          make_act_map(h, h->am_hidden, h->hidden, n * T, h->h, h->w, c.c_trunk * c.trunk_expand, true, T) &&
          make_act_map(h, h->am_fa, h->fa, n * T, h->h, h->w, c.c_trunk, false, T);
+    h->dw_tma_ok = false;
+    {
+        const char *dv = std::getenv("UFNVC_DW_TMA");
+        if (ok && c.n_trunk_blocks > 0 && c.c_trunk % 64 == 0 && c.c_trunk <= 256 && !(dv && dv[0] == '0')) {
+            ok = tc_make_act_tmap(&h->tm_dw, h->fa, n * T, h->h, h->w, c.c_trunk, 10, 10, h->err);
+            h->dw_tma_ok = ok;
+        }
+    }
     for (auto &tb : h->trunk)
         if (ok && !trunk_make_maps(tb.fused, h->fb, (long long)n * T * h->h * h->w, tb.pw1, tb.pw2, h->err)) ok = false;
     for (int s = 0; ok && s < 3; ++s)

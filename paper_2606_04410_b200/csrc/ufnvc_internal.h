@@ -63,6 +63,9 @@ cudaError_t launch_conv_generic(const ConvLayer &L, const ConvProblem &P, const 
 cudaError_t launch_dwconv3x3(const bf16 *in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
                              int C, cudaStream_t st);
 
+cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
+                                 int C, cudaStream_t st);   // tm_in: NHWC map of `in` with box {64, 10, 10, 1}
+
 // fp64 hyper-decoder (A1 + A2), R12: the scale decision is taken in double on both sides.
 struct HyperLayer {
     int c_in = 0, n = 0;
