@@ -16,6 +16,8 @@
 // warp 0 = TMA producer, warp 1 = MMA issuer + TMEM allocator, warps 2..9 = epilogue.  Persistent, grid = #SMs.
 #include <cuda.h>
 
+#include <cstdlib>
+
 #include "epilogue.cuh"
 #include "tc_ptx.cuh"
 #include "ufnvc_internal.h"
@@ -322,13 +324,22 @@ namespace {
 // cycles).  The leader CTA (rank 0) issues all MMAs; both CTAs run their own TMA producer and their own 8 epilogue
 // warps.  Barriers the MMA thread waits on live in the leader (the peer signals them through the cluster window);
 // barriers signalled by tcgen05.commit are multicast to both CTAs.
+// TMH = true: the GELU'd hidden chunk goes back into TMEM (bf16, over the fp32 columns it came from) and GEMM2 reads its
+// A operand from there: no 64 KB Hs buffer (the weight ring grows from 3 to 5 stages), and per tile 256 KB of st.shared
+// plus 256 KB of A-operand reads leave the shared-memory port, which TMA writes + MMA operand reads had saturated.
+template <bool TMH>
 __global__ void __launch_bounds__(kTrunkThreads, 1)
 trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant__ CUtensorMap tm_w1h,
                       const __grid_constant__ CUtensorMap tm_w2h, const TrunkParams p)
 {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    auto bar = [&](uint32_t slot) { return base + kOffBar + 8u * slot; };
+    constexpr int NS = TMH ? 5 : 3;                            // weight-ring stages
+    constexpr uint32_t offW = TMH ? kOffHs : kOffW, offBar = offW + NS * kWStage;
+    constexpr uint32_t B_WFULL = 2, B_WEMPTY = B_WFULL + NS, B_HACC_FULL = B_WEMPTY + NS, B_HACC_EMPTY = B_HACC_FULL + 2,
+                       B_HS_FULL = B_HACC_EMPTY + 2, B_HS_EMPTY = B_HS_FULL + 2, B_OFULL = B_HS_EMPTY + 2, B_OEMPTY = B_OFULL + 1,
+                       B_TMEM_SLOT = B_OEMPTY + 1;                     // (shadow the file-scope slots: 3-stage layout)
+    auto bar = [&](uint32_t slot) { return base + offBar + 8u * slot; };
     volatile uint32_t *tmem_slot_ptr =
         reinterpret_cast<volatile uint32_t *>(smem_raw + (bar(B_TMEM_SLOT) - smem_u32(smem_raw)));
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -342,7 +353,7 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_w1h) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_w2h) : "memory");
         mbar_init(bar(B_AFULL), 1); mbar_init(bar(B_AEMPTY), 1);
-        for (int s = 0; s < kWStages; ++s) { mbar_init(bar(B_WFULL + s), 1); mbar_init(bar(B_WEMPTY + s), 1); }
+        for (int s = 0; s < NS; ++s) { mbar_init(bar(B_WFULL + s), 1); mbar_init(bar(B_WEMPTY + s), 1); }
         for (int b = 0; b < 2; ++b) {
             mbar_init(bar(B_HACC_FULL + b), 1); mbar_init(bar(B_HACC_EMPTY + b), 16);     // 8 epilogue warps x 2 CTAs
             mbar_init(bar(B_HS_FULL + b), 16);  mbar_init(bar(B_HS_EMPTY + b), 1);
@@ -369,9 +380,9 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
                 mbar_wait(bar(B_WEMPTY + ws), wp ^ 1);                // local: multicast commit of the MMAs that read it
                 if (rank == 0) mbar_expect_tx(bar(B_WFULL + ws), 2 * kWStage);
                 full_l = mapa_rank(bar(B_WFULL + ws), 0);
-                return base + kOffW + uint32_t(ws) * kWStage;
+                return base + offW + uint32_t(ws) * kWStage;
             };
-            auto w_next = [&]() { if (++ws == kWStages) { ws = 0; wp ^= 1; } };
+            auto w_next = [&]() { if (++ws == NS) { ws = 0; wp ^= 1; } };
             auto load_w1 = [&](int c) {                               // rows c*128 + rank*64 .. +63 of W1, 4 k slabs of 8 KB
                 uint32_t full_l;
                 const uint32_t dst = w_slot(full_l);
@@ -391,9 +402,9 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
                 for (int s = 0; s < 4; ++s) tma_load_2d_pair(base + kOffA + s * kSlab, &tm_d, afull_l, s * 64, tile * kTM);
                 ap ^= 1;
                 load_w1(0);
-                if (NC > 1) load_w1(1);
+                if (!TMH && NC > 1) load_w1(1);
                 for (int c = 0; c < NC; ++c) {                     // the order the MMA warp consumes them in
-                    if (c + 2 < NC) load_w1(c + 2);
+                    if (c + (TMH ? 1 : 2) < NC) load_w1(c + (TMH ? 1 : 2));
                     load_w2(c);
                 }
             }
@@ -404,7 +415,7 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
             const uint32_t idesc1 = umma_idesc_bf16(2 * kTM, kHC), idesc2 = umma_idesc_bf16(2 * kTM, kC);
             const uint32_t hi = uint32_t(1024 >> 4) | (1u << 14) | (2u << 29);
             auto lo = [](uint32_t addr) { return ((addr & 0x3FFFFu) >> 4) | (1u << 16); };
-            const uint32_t a_lo = lo(base + kOffA), hs_lo = lo(base + kOffHs), w_lo = lo(base + kOffW);
+            const uint32_t a_lo = lo(base + kOffA), hs_lo = lo(base + kOffHs), w_lo = lo(base + offW);
             const uint32_t o_acc = tmem_base, h_acc = tmem_base + kC;
             int ws = 0; uint32_t wp = 0;
             uint32_t ph_hacc = 0, ph_hs = 0;
@@ -413,12 +424,14 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
                 tc_fence_after();
                 return w_lo + uint32_t(ws) * (kWStage >> 4);
             };
-            auto w_release = [&]() { umma2_commit_both(bar(B_WEMPTY + ws)); if (++ws == kWStages) { ws = 0; wp ^= 1; } };
+            auto w_release = [&]() { umma2_commit_both(bar(B_WEMPTY + ws)); if (++ws == NS) { ws = 0; wp ^= 1; } };
             auto gemm1 = [&](int c) {
                 const int b = c & 1;
-                mbar_wait_cluster(bar(B_HACC_EMPTY + b), ((ph_hacc >> b) & 1) ^ 1);
-                ph_hacc ^= 1u << b;
-                tc_fence_after();
+                if (!TMH) {                                            // TMH: Hacc[b] is released by GEMM2(c-2), in issue order
+                    mbar_wait_cluster(bar(B_HACC_EMPTY + b), ((ph_hacc >> b) & 1) ^ 1);
+                    ph_hacc ^= 1u << b;
+                    tc_fence_after();
+                }
                 const uint32_t d = h_acc + uint32_t(b) * kHC;
                 const uint32_t w = w_wait();
 #pragma unroll
@@ -434,13 +447,14 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
             for (int pt = pair0; pt < n_ptiles; pt += n_pairs, ++it) {
                 mbar_wait_cluster(bar(B_AFULL), it & 1);
                 tc_fence_after();
+                constexpr int LA = TMH ? 1 : 2;                           // GEMM1 lookahead (chunks)
                 gemm1(0);
-                if (NC > 1) gemm1(1);
-                if (NC <= 2) umma2_commit_both(bar(B_AEMPTY));
+                if (LA == 2 && NC > 1) gemm1(1);
+                if (NC <= LA) umma2_commit_both(bar(B_AEMPTY));
                 for (int c = 0; c < NC; ++c) {
-                    if (c + 2 < NC) {
-                        gemm1(c + 2);
-                        if (c + 3 == NC) umma2_commit_both(bar(B_AEMPTY));
+                    if (c + LA < NC) {
+                        gemm1(c + LA);
+                        if (c + LA + 1 == NC) umma2_commit_both(bar(B_AEMPTY));
                     }
                     const int b = c & 1;
                     mbar_wait_cluster(bar(B_HS_FULL + b), (ph_hs >> b) & 1);
@@ -451,11 +465,16 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
 #pragma unroll
                     for (int j = 0; j < 2; ++j)
 #pragma unroll
-                        for (int k = 0; k < 4; ++k)
-                            umma2_bf16_lh(o_acc, hs_lo + uint32_t(2 * b + j) * (kSlab >> 4) + 2 * k, hi, w + uint32_t(j) * (kSlab >> 4) + 2 * k,
-                                          hi, idesc2, uint32_t(c | j | k));
+                        for (int k = 0; k < 4; ++k) {
+                            if (TMH)     // hidden 64 j + 16 k .. +15 = 8 packed columns at Hacc[b] + 64 j + 8 k (see the GELU warps)
+                                umma2_bf16_ts(o_acc, h_acc + uint32_t(b) * kHC + uint32_t(64 * j + 8 * k), w + uint32_t(j) * (kSlab >> 4) + 2 * k, hi,
+                                              idesc2, uint32_t(c | j | k));
+                            else
+                                umma2_bf16_lh(o_acc, hs_lo + uint32_t(2 * b + j) * (kSlab >> 4) + 2 * k, hi, w + uint32_t(j) * (kSlab >> 4) + 2 * k,
+                                              hi, idesc2, uint32_t(c | j | k));
+                        }
                     w_release();
-                    umma2_commit_both(bar(B_HS_EMPTY + b));
+                    if (!TMH) umma2_commit_both(bar(B_HS_EMPTY + b));
                 }
                 umma2_commit_both(bar(B_OFULL));
             }
@@ -478,7 +497,7 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
             for (int c = 0; c < NC; ++c) {
                 const int b = c & 1;
                 mbar_wait(bar(B_HACC_FULL + b), (ph_use >> b) & 1);
-                mbar_wait(bar(B_HS_EMPTY + b), ((ph_use >> b) & 1) ^ 1);
+                if (!TMH) mbar_wait(bar(B_HS_EMPTY + b), ((ph_use >> b) & 1) ^ 1);
                 ph_use ^= 1u << b;
                 tc_fence_after();
                 // this chunk's 64 biases live 2 per lane (fetched one chunk ahead: with ~225 KB of shared memory the L1 is a few
@@ -491,13 +510,13 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
                 const uint32_t hs_row = base + kOffHs + uint32_t(2 * b + half) * kSlab + uint32_t(r) * 128u;
                 // both 32-column loads are in flight before the single wait: a TMEM load costs ~400 cycles while the tensor
                 // core is accumulating, and it sits on the GEMM1 -> GELU -> GEMM2 critical chain
-                uint32_t vv[2][32];
+                uint32_t vv[2][32], hid[32];
                 tmem_ld32_nowait(t_lane + kC + uint32_t(b) * kHC + uint32_t(half * 64), vv[0]);
                 tmem_ld32_nowait(t_lane + kC + uint32_t(b) * kHC + uint32_t(half * 64 + 32), vv[1]);
                 tmem_ld_wait();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(hacc_empty_l + 8u * b);
+                if (!TMH && lane == 0) mbar_arrive_cluster(hacc_empty_l + 8u * b);
 #pragma unroll
                 for (int q = 0; q < 2; ++q) {
                     uint32_t (&v)[32] = vv[q];
@@ -510,14 +529,23 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
                         gelu_bias2(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), bx, by, f0, f1);
                         pk[j / 2] = pack_bf16x2(f0, f1);
                     }
+                    if (TMH) {
 #pragma unroll
-                    for (int jj = 0; jj < 4; ++jj) {
-                        const uint32_t chunk = uint32_t(q * 4 + jj) ^ uint32_t(r & 7);
-                        st_shared_v4(hs_row + (chunk << 4), pk[4 * jj], pk[4 * jj + 1], pk[4 * jj + 2], pk[4 * jj + 3]);
+                        for (int jj = 0; jj < 16; ++jj) hid[q * 16 + jj] = pk[jj];
+                    } else {
+#pragma unroll
+                        for (int jj = 0; jj < 4; ++jj) {
+                            const uint32_t chunk = uint32_t(q * 4 + jj) ^ uint32_t(r & 7);
+                            st_shared_v4(hs_row + (chunk << 4), pk[4 * jj], pk[4 * jj + 1], pk[4 * jj + 2], pk[4 * jj + 3]);
+                        }
                     }
                 }
+                if (TMH) {      // this warp read fp32 columns [64 half, 64 half + 64) of Hacc[b]; its 64 bf16 go over the first 32 of them
+                    tmem_st32(t_lane + kC + uint32_t(b) * kHC + uint32_t(half * 64), hid);
+                    tmem_st_wait();
+                }
                 tc_fence_before();
-                fence_proxy_async();
+                if (!TMH) fence_proxy_async();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(hs_full_l + 8u * b);
             }
@@ -611,7 +639,8 @@ cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const Con
     if (pair && p.n_tiles >= 2) {
         static thread_local bool configured2 = false;
         if (!configured2) {
-            cudaError_t e = cudaFuncSetAttribute(trunk_mlp_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kTrunkSmem));
+            cudaError_t e = cudaFuncSetAttribute(trunk_mlp_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kTrunkSmem));
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(trunk_mlp_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kTrunkSmem));
             if (e != cudaSuccess) return e;
             configured2 = true;
         }
@@ -626,7 +655,9 @@ cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const Con
         attr[0].id = cudaLaunchAttributeClusterDimension;
         attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
         cfg.attrs = attr; cfg.numAttrs = 1;
-        return cudaLaunchKernelEx(&cfg, trunk_mlp_pair_kernel, m.tm_d, m.tm_w1h, m.tm_w2h, p);
+        static const bool tmh = [] { const char *e = std::getenv("UFNVC_TRUNK_TMEM_HIDDEN"); return !(e && e[0] == '0'); }();
+        return tmh ? cudaLaunchKernelEx(&cfg, trunk_mlp_pair_kernel<true>, m.tm_d, m.tm_w1h, m.tm_w2h, p)
+                   : cudaLaunchKernelEx(&cfg, trunk_mlp_pair_kernel<false>, m.tm_d, m.tm_w1h, m.tm_w2h, p);
     }
     const int grid = p.n_tiles < num_sms ? p.n_tiles : num_sms;
     trunk_mlp_kernel<<<grid, kTrunkThreads, kTrunkSmem, st>>>(m.tm_d, m.tm_w1, m.tm_w2, p);
