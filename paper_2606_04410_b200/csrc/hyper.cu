@@ -276,13 +276,23 @@ __global__ void __launch_bounds__(256) hyper_fix_kernel(const uint32_t *__restri
         const int img = int(r / unsigned(hp.h));
         const int zy = ly >> 2, zx = lx >> 2, ij = ((ly & 3) << 2) | (lx & 3);
         const double *wrow = fix_w + (size_t(c2) * 16 + ij) * 9 * c_h;
-        double acc = 0.0;
+        // lanes stride the channels; 4 independent accumulators (channel blocks) keep the fp64 pipe and the loads busy.
+        // Fixed summation order per element -> run-to-run deterministic.
+        double a4[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
         for (int tap = 0; tap < 9; ++tap) {
             const int yy = zy + tap / 3 - 1, xx = zx + tap % 3 - 1;
             if (yy < 0 || yy >= hz || xx < 0 || xx >= wz) continue;
             const double *xr = x2 + ((size_t(img) * hz + yy) * wz + xx) * c_h;
-            for (int c = lane; c < c_h; c += 32) acc = fma(xr[c], wrow[tap * c_h + c], acc);
+            const double *wr = wrow + tap * c_h;
+            int c = lane;
+            for (; c + 96 < c_h; c += 128) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u) a4[u] = fma(xr[c + 32 * u], wr[c + 32 * u], a4[u]);
+            }
+            for (; c < c_h; c += 32) a4[0] = fma(xr[c], wr[c], a4[0]);
         }
+        double acc = (a4[0] + a4[1]) + (a4[2] + a4[3]);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
         if (lane == 0) {
