@@ -47,7 +47,7 @@ class ClockSampler:
     def __enter__(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                          "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
         except OSError:
@@ -63,11 +63,16 @@ class ClockSampler:
             self.proc.terminate()
             self.th.join(timeout=2)
 
-    def summary(self):
-        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+    def mark(self):
+        """Index of the next sample: bench marks the start and the end of the timed region with it."""
+        return len(self.rows)
+
+    def summary(self, i0=0, i1=None):
+        rows = self.rows[i0:i1] or self.rows          # samples taken DURING the timed region (all, if it was too short)
+        sm = [float(r[0]) for r in rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
         reasons = set()
-        for r in self.rows:
+        for r in rows:
             if len(r) >= 7:
                 for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
                     if v.lower().startswith("active"):
@@ -156,14 +161,15 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- device-resident timing: per-step event pairs on the launching stream, L2 flushed between steps ----
-    with torch.cuda.stream(stream):
-        for _ in range(max(3, args.warmup)):
-            dec.chunk_decode(z, bits, off, frames=frames, stream=stream)
-    barrier()
-    assert dec.get_status() == 0, "bit-stream status"
     step_ms, stage_us = [], []
-    with ClockSampler(local) as clocks:
+    with ClockSampler(local) as clocks:               # started before the warm-up: nvidia-smi takes ~0.2 s to print its first line
+        time.sleep(0.3)
+        with torch.cuda.stream(stream):
+            for _ in range(max(3, args.warmup)):
+                dec.chunk_decode(z, bits, off, frames=frames, stream=stream)
         barrier()
+        assert dec.get_status() == 0, "bit-stream status"
+        i0 = clocks.mark()
         t_wall = time.perf_counter()
         with torch.cuda.stream(stream):
             for _ in range(args.steps):
@@ -176,6 +182,7 @@ def run_ours(args):
                 step_ms.append(e0.elapsed_time(e1))
         barrier()
         t_wall = time.perf_counter() - t_wall
+        i1 = clocks.mark()
     total_ms = sum(step_ms)
     total_ms = replicas.max_over_ranks(total_ms, dev)
     frames_per_step = n * cfg.T
@@ -230,7 +237,7 @@ def run_ours(args):
                 config=dict(workload=cfg.name, T=cfg.T, frame=f"{cfg.width}x{cfg.height}", chunks_per_step=n,
                             l2="flushed between timed steps (256 MiB memset, untimed)", parallelism=f"replicas x{world}",
                             gmac_per_chunk=cfg.macs_per_chunk() / 1e9),
-                clocks=clocks.summary(), gpu_launches=dec.launches_per_call(n) * args.steps,
+                clocks=clocks.summary(i0, i1), gpu_launches=dec.launches_per_call(n) * args.steps,
                 e2e=dict(value=e2e_val, unit="frames/s", h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, steps=e2e_steps),
                 roofline=roofline,
                 cpu_baseline=dict(value=fps_cpu, unit="frames/s", cores=cores, kind="oracle", sample=desc),
@@ -243,7 +250,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=3, help="SURVEY.md config number 1..5 (3 = 1080p headline)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
