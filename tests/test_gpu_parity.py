@@ -104,6 +104,27 @@ def test_plain_entry_point_equals_ex_and_is_deterministic(decoders):
     assert torch.equal(a, d)
 
 
+def test_whole_call_is_cuda_graph_capturable(decoders):
+    """ufnvc_chunk_decode only enqueues (no sync, no allocation): the 25-kernel sequence can be captured once in a CUDA
+    graph and replayed; the replay's frames equal the direct call's bit for bit."""
+    dec, case = decoders("cfg3-crop")
+    z, bits, off = gpu_inputs(case)
+    ref = dec.chunk_decode(z, bits, off).clone()                 # also the warm-up (function attributes are set here)
+    torch.cuda.synchronize()
+    frames = dec.new_frames(1)
+    s = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        g.capture_begin()
+        dec.chunk_decode(z, bits, off, frames=frames, stream=s)
+        g.capture_end()
+    frames.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert dec.get_status() == 0
+    assert torch.equal(frames, ref)
+
+
 def test_entropy_params_entry_point(decoders):
     dec, case = decoders("cfg3-crop")
     z, _, _ = gpu_inputs(case)
