@@ -365,7 +365,7 @@ constexpr int kHaloTH = 16, kHaloTW = 8;
 constexpr int kHaloRowPitch = (kHaloTW + 2) * 128;                            // 1280 B
 constexpr int kHaloBytes = (kHaloTH + 2) * (kHaloTW + 2) * 128;              // 23040 B = one TMA box
 constexpr int kHaloStage = (kHaloBytes + 1023) / 1024 * 1024;                // 23552 B
-constexpr int kHaloAStages = 3;
+constexpr int kHaloAStages = 2;                  // an A halo stage lasts 9 k-blocks; the B ring is what must be deep
 
 __device__ __forceinline__ uint64_t umma_desc_sw128_sbo(uint32_t saddr, uint32_t sbo_bytes)
 {
