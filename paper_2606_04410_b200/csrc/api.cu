@@ -80,6 +80,8 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     h->use_halo = !(hl && hl[0] == '0');
     const char *ft = std::getenv("UFNVC_FUSED_TRUNK");
     h->use_fused_trunk = !(ft && ft[0] == '0');
+    const char *pc = std::getenv("UFNVC_PAIR_CONV");
+    h->use_pair_conv = !(pc && pc[0] == '0');
     const char *pt = std::getenv("UFNVC_PAIR_TRUNK");
     h->use_pair_trunk = !(pt && pt[0] == '0');
 

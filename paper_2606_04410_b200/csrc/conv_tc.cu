@@ -94,9 +94,11 @@ __device__ __forceinline__ TileCoord tile_coord(const TcParams &p, int tile)
 // split the 32-column chunks between them (even / odd), so every SM sub-partition holds two epilogue warps and the
 // tcgen05.ld / MUFU latencies of one hide behind the other.  tcgen05.ld -> bias -> act -> store, per tile of the
 // persistent schedule; tfull0 / tempty0 are the smem addresses of the first of two consecutive mbarriers each.
+// pair_rank >= 0: CTA-pair kernel -- the schedule runs over tile PAIRS (blockIdx.x / 2, stride gridDim.x / 2), this CTA
+// owns x tile 2 * txp + pair_rank, and tempty0 is the LEADER's barrier as a cluster address (relaxed remote arrive).
 template <int MODE>
 __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_base, uint32_t tfull0, uint32_t tempty0,
-                                               int warp, int lane)
+                                               int warp, int lane, int pair_rank = -1)
 {
     const int quad = warp & 3;
     const int half = (warp - 2) >> 2;                             // 0: even 32-column chunks, 1: odd ones
@@ -104,8 +106,10 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
     const int my = m >> p.tw_shift, mx = m & (p.TW - 1);          // TW is a power of two
     const unsigned P = unsigned(p.H) * unsigned(p.W);
     int it = 0;
-    for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x, ++it) {
-        const TileCoord tc = tile_coord(p, tile);
+    const int tile0 = pair_rank < 0 ? int(blockIdx.x) : int(blockIdx.x >> 1), tstride = pair_rank < 0 ? int(gridDim.x) : int(gridDim.x >> 1);
+    for (int tile = tile0; tile < p.total_tiles; tile += tstride, ++it) {
+        TileCoord tc = tile_coord(p, tile);
+        if (pair_rank >= 0) tc.x0 = 2 * tc.x0 + pair_rank * p.TW;
         const int acc = it & 1;
         const uint32_t acc_phase = (it >> 1) & 1;
         const int ym = tc.y0 + my, xm = tc.x0 + mx;
@@ -252,7 +256,7 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
         }
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(tempty0 + 8u * acc);
+        if (lane == 0) { if (pair_rank < 0) mbar_arrive(tempty0 + 8u * acc); else mbar_arrive_cluster(tempty0 + 8u * acc); }
     }
 }
 
@@ -526,6 +530,131 @@ conv_halo_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// CTA-pair halo conv (cta_group::2) for the streamed-weight layers (A8).  Measured on the single-CTA kernel: the MMA
+// thread spent ~60 % of its time waiting for weight stages -- four 32 KB stages buffer 1.1 us of tensor work, about one
+// L2 round trip.  Here two CTAs of a cluster take two x-adjacent tiles of the same image and n-tile (same weights) and
+// run ONE M = 256 MMA; each CTA stores only its half of every weight tile (BN/2 rows = 16 KB), so the same shared memory
+// holds a ring twice as deep in k-blocks and every SM pulls half the weight bytes.  Leader = rank 0 issues the MMAs;
+// barriers it waits on live in its shared memory (the peer's TMA and epilogue warps signal them through the cluster
+// window); tcgen05.commit arrivals are multicast to both CTAs.
+template <int MODE>
+__global__ void __launch_bounds__(kThreads, 1)
+conv_halo_pair_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_bh, const TcParams p,
+                      const int nb_stages, const int na_stages)
+{
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bh_bytes = uint32_t(p.BN) * 64u;                              // this CTA's half of a weight tile
+    const uint32_t b_base = smem_base + na_stages * kHaloStage;
+    const uint32_t bar_base = b_base + uint32_t(nb_stages) * bh_bytes;
+    auto afull = [&](int s) { return bar_base + 8u * s; };
+    auto aempty = [&](int s) { return bar_base + 8u * (na_stages + s); };
+    const uint32_t misc = bar_base + 8u * (2 * na_stages);
+    const uint32_t tfull0 = misc, tempty0 = misc + 16u, tmem_slot = misc + 48u;
+    const uint32_t bbar = misc + 64u;
+    auto bfull = [&](int s) { return bbar + 8u * s; };
+    auto bempty = [&](int s) { return bbar + 8u * (nb_stages + s); };
+    volatile uint32_t *tmem_slot_ptr = reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+    const int pair0 = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+    uint32_t tmem_cols = 32;
+    while (tmem_cols < uint32_t(2 * p.BN)) tmem_cols <<= 1;
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_a) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_bh) : "memory");
+        for (int s = 0; s < na_stages; ++s) { mbar_init(afull(s), 1); mbar_init(aempty(s), 1); }
+        for (int s = 0; s < nb_stages; ++s) { mbar_init(bfull(s), 1); mbar_init(bempty(s), 1); }
+        for (int a = 0; a < 2; ++a) { mbar_init(tfull0 + 8u * a, 1); mbar_init(tempty0 + 8u * a, 16); }     // 8 warps x 2 CTAs
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    cluster_sync_all();
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(tmem_cols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    cluster_sync_all();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===================== TMA producer (both CTAs): own halo tile, own half of every weight tile =====================
+        if (elect_one()) {
+            int sa = 0, sb = 0; uint32_t pa = 0, pb = 0;
+            for (int tile = pair0; tile < p.total_tiles; tile += n_pairs) {
+                TileCoord tc = tile_coord(p, tile);
+                tc.x0 = 2 * tc.x0 + int(rank) * p.TW;                              // may lie past the image: an all-zero tile
+                const int grp = group_of(p, tc.img);
+                for (int slab = 0; slab < p.slabs; ++slab) {
+                    mbar_wait(aempty(sa), pa ^ 1);
+                    if (rank == 0) mbar_expect_tx(afull(sa), 2 * kHaloBytes);
+                    tma_load_4d_pair(smem_base + sa * kHaloStage, &tmap_a, mapa_rank(afull(sa), 0), slab * kSlabK, tc.x0 - 1, tc.y0 - 1, tc.img);
+                    if (++sa == na_stages) { sa = 0; pa ^= 1; }
+                    for (int tap = 0; tap < 9; ++tap) {
+                        mbar_wait(bempty(sb), pb ^ 1);
+                        if (rank == 0) mbar_expect_tx(bfull(sb), 2 * bh_bytes);
+                        tma_load_3d_pair(b_base + uint32_t(sb) * bh_bytes, &tmap_bh, mapa_rank(bfull(sb), 0), slab * kSlabK,
+                                         tc.nt * p.BN + int(rank) * (p.BN >> 1), grp * 9 + tap);
+                        if (++sb == nb_stages) { sb = 0; pb ^= 1; }
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer: leader CTA only =====================
+        if (rank == 0 && elect_one()) {
+            const uint32_t idesc = umma_idesc_bf16(2 * kTileM, p.BN);
+            const uint32_t a_hi = uint32_t(kHaloRowPitch >> 4) | (1u << 14) | (2u << 29);
+            const uint32_t b_hi = uint32_t(1024 >> 4) | (1u << 14) | (2u << 29);
+            const uint32_t a_lo0 = ((smem_base & 0x3FFFFu) >> 4) | (1u << 16);
+            const uint32_t b_lo0 = ((b_base & 0x3FFFFu) >> 4) | (1u << 16);
+            const uint32_t b_step = bh_bytes >> 4;
+            int sa = 0, sb = 0; uint32_t pa = 0, pb = 0;
+            int it = 0;
+            for (int tile = pair0; tile < p.total_tiles; tile += n_pairs, ++it) {
+                const int acc = it & 1;
+                const uint32_t acc_phase = (it >> 1) & 1;
+                mbar_wait_cluster(tempty0 + 8u * acc, acc_phase ^ 1);
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + uint32_t(acc * p.BN);
+                for (int slab = 0; slab < p.slabs; ++slab) {
+                    mbar_wait_cluster(afull(sa), pa);
+                    tc_fence_after();
+                    const uint32_t a_lo = a_lo0 + uint32_t(sa) * (kHaloStage >> 4);
+#pragma unroll
+                    for (int tap = 0; tap < 9; ++tap) {
+                        mbar_wait_cluster(bfull(sb), pb);
+                        tc_fence_after();
+                        const uint32_t b_lo = b_lo0 + uint32_t(sb) * b_step;
+                        const uint32_t a_tap = a_lo + uint32_t(((tap / 3) * (kHaloTW + 2) + tap % 3) * 128 >> 4);
+#pragma unroll
+                        for (int k = 0; k < kSlabK / 16; ++k)
+                            umma2_bf16_lh(d_tmem, a_tap + 2 * k, a_hi, b_lo + 2 * k, b_hi, idesc, uint32_t(slab | tap | k));
+                        umma2_commit_both(bempty(sb));
+                        if (++sb == nb_stages) { sb = 0; pb ^= 1; }
+                    }
+                    umma2_commit_both(aempty(sa));
+                    if (++sa == na_stages) { sa = 0; pa ^= 1; }
+                }
+                umma2_commit_both(tfull0 + 8u * acc);
+            }
+        }
+    } else {
+        epilogue_warps<MODE>(p, tmem_base, tfull0, mapa_rank(tempty0, 0), warp, lane, int(rank));
+    }
+
+    tc_fence_before();
+    cluster_sync_all();
+    if (warp == 1) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(tmem_cols) : "memory");
+    }
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------- host side ----------------------------------
@@ -583,6 +712,12 @@ bool tc_make_weight_tmap(ConvLayer &L, std::string &err)
     cuuint64_t strides[2] = {cuuint64_t(L.c_in) * 2, cuuint64_t(L.c_in) * 2 * L.n_pad};
     cuuint32_t box[3] = {cuuint32_t(kSlabK), cuuint32_t(L.block_n), 1};
     if (!encode(&L.tmap_w, L.w, 3, dims, strides, box, err)) return false;
+    L.has_half_map = false;
+    if (L.taps == 9 && L.block_n % 32 == 0) {                              // CTA-pair kernel: each CTA loads BN/2 rows
+        cuuint32_t boxh[3] = {cuuint32_t(kSlabK), cuuint32_t(L.block_n / 2), 1};
+        if (!encode(&L.tmap_w_half, L.w, 3, dims, strides, boxh, err)) return false;
+        L.has_half_map = true;
+    }
     L.use_tc = true;
     return true;
 }
@@ -598,6 +733,50 @@ bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W
 bool tc_make_halo_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, std::string &err)
 {
     return tc_make_act_tmap(tm, base, n_img, H, W, C, kHaloTH + 2, kHaloTW + 2, err);
+}
+
+cudaError_t launch_conv_halo_pair(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
+                                  cudaStream_t st)
+{
+    if (L.taps != 9 || !L.has_half_map || E.mode != EPI_PS2) return cudaErrorInvalidValue;
+    TcParams p{};
+    p.H = P.H; p.W = P.W;
+    p.n_img_m = P.n_img; p.Hm = P.H; p.Wm = P.W;
+    p.TH = kHaloTH; p.TW = kHaloTW;
+    p.flat = 0; p.tw_shift = 3;
+    p.tiles_y = (P.H + kHaloTH - 1) / kHaloTH;
+    p.tiles_x = ((P.W + kHaloTW - 1) / kHaloTW + 1) / 2;          // tile PAIRS along x; rank r owns x tile 2 txp + r
+    p.taps = 9; p.slabs = L.c_in / kSlabK;
+    p.BN = L.block_n; p.n_tiles = L.n_pad / L.block_n; p.n_real = L.n; p.n_pad = L.n_pad;
+    p.groups = L.groups;
+    p.total_tiles = p.n_img_m * p.tiles_y * p.tiles_x * p.n_tiles;
+    p.fd_ntiles = make_fastdiv(p.n_tiles); p.fd_tx = make_fastdiv(p.tiles_x); p.fd_ty = make_fastdiv(p.tiles_y);
+    p.fd_groups = make_fastdiv(p.groups);
+    p.bias = L.bias;
+    p.E = E;
+    const size_t bh_bytes = size_t(L.block_n) * 64;
+    const int na = kHaloAStages;
+    int nb = int((227 * 1024 - 1024 - size_t(na) * kHaloStage - 2048) / bh_bytes);
+    if (nb > 12) nb = 12;
+    if (nb < 2) return cudaErrorInvalidValue;
+    const size_t smem = 1024 + size_t(na) * kHaloStage + size_t(nb) * bh_bytes + 256 + 16 * size_t(nb) + 16 * size_t(na);
+    static thread_local bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(conv_halo_pair_kernel<EPI_PS2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    const int clusters = p.total_tiles < num_sms / 2 ? p.total_tiles : num_sms / 2;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(2 * clusters);
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, conv_halo_pair_kernel<EPI_PS2>, tmap_halo, L.tmap_w_half, p, nb, na);
 }
 
 cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,

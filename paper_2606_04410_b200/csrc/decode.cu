@@ -22,6 +22,9 @@ cudaError_t conv(ufnvc_handle *h, const ConvLayer &L, const ConvProblem &P, cons
                  cudaStream_t st, int *launches)
 {
     if (launches) ++*launches;
+    if (L.use_tc && L.taps == 9 && am.halo_ok && h->use_halo && !h->force_generic && h->use_pair_conv && L.has_half_map &&
+        E.mode == EPI_PS2 && P.W > 8)
+        return launch_conv_halo_pair(L, P, am.tm_halo, E, h->num_sms, st);
     if (L.use_tc && L.taps == 9 && am.halo_ok && h->use_halo && !h->force_generic)
         return launch_conv_halo(L, P, am.tm_halo, E, h->num_sms, st);
     if (L.use_tc && am.ok && !h->force_generic) return launch_conv_tc(L, P, am.tm, am.tile_h, am.tile_w, am.flat, E, h->num_sms, st);

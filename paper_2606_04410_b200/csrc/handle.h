@@ -14,6 +14,7 @@ struct ufnvc_handle {
     int max_chunks = 1;
     bool weights_loaded = false;
     int last_launches = 0;               // kernels enqueued by the last decode call (ufnvc_launches_per_call)
+    bool use_pair_conv = true;           // env UFNVC_PAIR_CONV=0: single-CTA halo conv for A8 (A/B test)
     bool use_pair_trunk = true;          // env UFNVC_PAIR_TRUNK=0: single-CTA fused MLP kernel (A/B test)
     bool use_fused_trunk = true;         // env UFNVC_FUSED_TRUNK=0: two 1x1 conv launches per block (A/B test)
     bool use_halo = true;                // env UFNVC_HALO=0: first-pass implicit-GEMM kernel for the 3x3 convs (A/B test)

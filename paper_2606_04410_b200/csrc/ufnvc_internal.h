@@ -49,6 +49,8 @@ struct ConvLayer {
     float *bias = nullptr;
     bool use_tc = false;     // tcgen05 path eligible (c_in % 64 == 0, n_pad % 16 == 0)
     CUtensorMap tmap_w;      // 3-D {c_in, n_pad, groups*taps}, box {64, block_n, 1}, 128B swizzle
+    CUtensorMap tmap_w_half; // same tensor, box {64, block_n / 2, 1}: one CTA's half of a weight tile (CTA-pair kernel)
+    bool has_half_map = false;
     int block_n = 0;
 };
 
@@ -109,6 +111,8 @@ cudaError_t launch_rans_decode(const RansParams &p, cudaStream_t st);
 // tcgen05 implicit-GEMM conv (conv_tc.cu)
 cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_in, int tile_h, int tile_w,
                            bool flat, const EpiParams &E, int num_sms, cudaStream_t st);
+cudaError_t launch_conv_halo_pair(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
+                                  cudaStream_t st);
 cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
                              cudaStream_t st);
 bool tc_make_halo_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, std::string &err);
