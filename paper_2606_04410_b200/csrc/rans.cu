@@ -23,7 +23,7 @@ __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
         const uint4 *src_l = reinterpret_cast<const uint4 *>(p.lut);
         uint4 *dc = reinterpret_cast<uint4 *>(s_cf), *dl = reinterpret_cast<uint4 *>(s_lut);
         for (int i = threadIdx.x; i < nb * 64; i += blockDim.x) dc[i] = src_c[i];
-        for (int i = threadIdx.x; i < nb * 32; i += blockDim.x) dl[i] = src_l[i];
+        for (int i = threadIdx.x; i < nb * (kLutBuckets / 8); i += blockDim.x) dl[i] = src_l[i];
     }
     __syncthreads();
 
@@ -83,7 +83,7 @@ __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
         const bool valid = j < n_steps && i < n;
         const uint32_t slot = x & 0xFFFFu;
         const uint32_t *c = s_cf + k * 256;
-        const uint32_t lh = s_lut[k * 256 + (slot >> 8)];
+        const uint32_t lh = s_lut[k * kLutBuckets + (slot >> kLutShift)];
         uint32_t lo = lh & 0xFFu, hi = lh >> 8;
         while (lo < hi) {                       // largest pos in [lo,hi] with c[pos] <= slot
             const uint32_t mid = (lo + hi + 1) >> 1;
@@ -133,7 +133,7 @@ __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
 cudaError_t launch_rans_decode(const RansParams &p, cudaStream_t st)
 {
     const int nb = p.n_buckets;
-    const size_t smem = (size_t)64 * 256 * (4 + 2);
+    const size_t smem = (size_t)64 * (256 * 4 + kLutBuckets * 2);
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(rans_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

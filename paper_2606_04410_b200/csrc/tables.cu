@@ -34,17 +34,17 @@ void build_cdf_tables(int nb, double smin, double smax, std::vector<uint32_t> &c
 // 256*b + 255.  The decode kernel then searches only [lo, hi] (usually one candidate).
 void build_search_lut(const std::vector<uint32_t> &cdf32, int nb, std::vector<uint16_t> &lut)
 {
-    lut.assign((size_t)nb * 256, 0);
+    lut.assign((size_t)nb * kLutBuckets, 0);
     for (int k = 0; k < nb; ++k) {
         const uint32_t *c = &cdf32[(size_t)k * 256];
         int p = 0;
-        for (int b = 0; b < 256; ++b) {
-            const uint32_t s0 = 256u * b, s1 = s0 + 255u;
+        for (int b = 0; b < kLutBuckets; ++b) {
+            const uint32_t s0 = uint32_t(b) << kLutShift, s1 = s0 + (1u << kLutShift) - 1u;
             while (p < 254 && c[p + 1] <= s0) ++p;
             const int lo = p;
             int q = p;
             while (q < 254 && c[q + 1] <= s1) ++q;
-            lut[(size_t)k * 256 + b] = uint16_t(lo | (q << 8));
+            lut[(size_t)k * kLutBuckets + b] = uint16_t(lo | (q << 8));
         }
     }
 }

@@ -99,7 +99,7 @@ struct RansParams {
     const uint8_t *idx;       // [n][h][w][c_y]
     const float *mu;
     const uint32_t *cf;       // [nb][256]: c[pos] | freq[pos] << 16
-    const uint16_t *lut;      // [nb][256]: lo | hi<<8 = first/last candidate position for slot>>8
+    const uint16_t *lut;      // [nb][kLutBuckets]: lo | hi<<8 = first/last candidate position for slot >> kLutShift
     int n_chunks, n_sub, h, w, c_y, rows_per_sub, W, n_buckets;
     bf16 *yhat;               // [n][h][w][c_y]
     int16_t *sym_tap;         // optional
@@ -131,6 +131,9 @@ struct TrunkMaps {
 bool trunk_make_maps(TrunkMaps &m, const bf16 *d_base, long long n_px, const ConvLayer &pw1, const ConvLayer &pw2, std::string &err);
 cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const ConvLayer &pw2, const bf16 *x, bf16 *out, long long n_px,
                              int num_sms, bool pair, cudaStream_t st);
+
+// rANS symbol search: a 64-slot LUT bucket holds 1.2 binary-search steps (warp maximum, measured law) against 2.4 for 256 slots
+constexpr int kLutShift = 6, kLutBuckets = 65536 >> kLutShift;
 
 // ---- host-side entropy tables + encoder fixture (tables.cpp part of api) ---------------------------------------
 void build_cdf_tables(int nb, double smin, double smax, std::vector<uint32_t> &cdf32);
