@@ -184,6 +184,12 @@ def run_ours(args):
         t_wall = time.perf_counter() - t_wall
         i1 = clocks.mark()
     total_ms = sum(step_ms)
+    # A6 / A7 split: a few extra steps AFTER the timed region (two more events per trunk block would cost launch gaps inside it)
+    detail_us = []
+    with torch.cuda.stream(stream):
+        for _ in range(5):
+            flush.zero_()
+            detail_us.append(dec.chunk_decode_profiled(z, bits, off, frames, stream=stream, detail=True))
     total_ms = replicas.max_over_ranks(total_ms, dev)
     frames_per_step = n * cfg.T
     value = world * frames_per_step * args.steps / (total_ms / 1e3)
@@ -239,12 +245,34 @@ def run_ours(args):
     achieved = 2.0 * macs_a8 / (a8_us * 1e-6) / 1e12
     peak = peaks["tensor_sustained"]
     stage_mean = {k: statistics.mean(s[k] for s in stage_us) for k in stage_us[0]}
+    stage_mean["A6"] = statistics.mean(s["A6"] for s in detail_us)
     prof = os.path.join(ROOT, "profiles", "traffic.json")
     traffic = json.load(open(prof)).get("a8_dram_bytes_per_launch") if os.path.exists(prof) else None
     roofline = dict(bound="tensor", achieved=achieved, peak=peak, unit="TFLOP/s", frac=achieved / peak, traffic=traffic,
                     kernel="A8 frame-decoder stages 1-3 (3 launches of the implicit-GEMM conv kernel)",
                     peak_source=f"{peaks['src']} bf16 sustained; burst {peaks['tensor_burst']}", stage_us=stage_mean,
                     flops_per_step=2.0 * macs_a8)
+    # ---- the other stages against the roofline that bounds each (algorithmic bytes / flops per chunk) ----
+    Ct, Ce, B, T = cfg.c_trunk, cfg.c_trunk * cfg.trunk_expand, cfg.n_trunk_blocks, cfg.T
+    act = n * T * P * Ct * 2                                                   # one trunk activation tensor, bf16
+    nsym = n * cfg.n_symbols
+    s3 = n * T * (P << 6) * cfg.dec_channels[3] * 2                            # A9 input, bf16
+    out_b = n * T * 3 * cfg.height * cfg.width * 4                             # fp32 frames
+    def hbm(name, nbytes, us):
+        a = nbytes / (us * 1e-6) / 1e9
+        return dict(stage=name, bound="hbm", achieved=a, peak=peaks["hbm"], unit="GB/s", frac=a / peaks["hbm"], bytes=nbytes, us=us)
+    def tens(name, flops, us):
+        a = flops / (us * 1e-6) / 1e12
+        return dict(stage=name, bound="tensor", achieved=a, peak=peak, unit="TFLOP/s", frac=a / peak, flops=flops, us=us)
+    a7_us = stage_mean["A6+A7"] - stage_mean["A6"]
+    stages = [hbm("A3+A4 rANS decode + dequant (serial-latency bound, reported against HBM as asked)", nsym * 7 + int(nsym * 0.35), stage_mean["A3+A4"]),
+              hbm("A5 cross-frame unfold", n * P * cfg.c_y * 2 + act, stage_mean["A5"])]
+    if B:
+        stages += [hbm("A6 depthwise 3x3 (all trunk blocks)", B * 2 * act, stage_mean["A6"]),
+                   tens("A7 fused trunk MLP (all trunk blocks)", B * 2.0 * n * T * P * 2 * Ct * Ce, a7_us)]
+    stages += [tens("A8 frame decoders, stages 1-3", 2.0 * macs_a8, a8_us),
+               hbm("A9 last stage + output", s3 + out_b, stage_mean["A9"])]
+    roofline["stages"] = stages
     fps_cpu, desc, cores, _ = cpu_oracle_time(cfg)
     line = dict(metric=METRIC, value=value, unit="frames/s", n_gpus=world, steps=args.steps, warmup=max(3, args.warmup),
                 ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16",

@@ -130,10 +130,12 @@ int ufnvc_launches_per_call(const ufnvc_handle *h, int n_chunks);
 
 /* Per-stage device time of the LAST ufnvc_chunk_decode_profiled call, in microseconds.
  * ufnvc_chunk_decode_profiled = ufnvc_chunk_decode with a cudaEvent after each stage A1+A2, A3+A4, A5, A6+A7
- * (all trunk blocks), A8 (stages 1-3), A9; it synchronises the stream at the end.  us_out_host[6]. */
+ * (all trunk blocks), A8 (stages 1-3), A9; it synchronises the stream at the end.  us_out_host[7]: the six stages, then
+ * [6] = A6 alone (sum of the depthwise launches; A7 = [3] - [6]) when detail != 0 (two more events per trunk block, which
+ * cost a few microseconds of launch gaps), else 0. */
 int ufnvc_chunk_decode_profiled(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, const uint8_t *bits_dev,
                                 size_t bits_bytes, const uint32_t *sub_off_dev, float *frames_dev,
-                                void *cuda_stream, float *us_out_host);
+                                void *cuda_stream, int detail, float *us_out_host);
 
 /* Debug counters of the last decode / entropy_params call (synchronises the device).  which = 0: number of latent
  * elements whose scale bucket was re-decided in fp64 by the hybrid head (R12); 0 when the head runs all-fp64. */

@@ -51,7 +51,7 @@ def _load():
         "ufnvc_get_status": (i, [vp, C.POINTER(C.c_uint32)]),
         "ufnvc_last_error": (C.c_char_p, [vp]),
         "ufnvc_launches_per_call": (i, [vp, i]),
-        "ufnvc_chunk_decode_profiled": (i, [vp, i, vp, vp, sz, vp, vp, vp, C.POINTER(C.c_float)]),
+        "ufnvc_chunk_decode_profiled": (i, [vp, i, vp, vp, sz, vp, vp, vp, i, C.POINTER(C.c_float)]),
         "ufnvc_debug_counter": (i, [vp, i, C.POINTER(C.c_uint64)]),
         "ufnvc_get_cdf": (i, [vp, vp]),
         "ufnvc_symbols_from_uniform": (i, [vp, vp, vp, sz, vp]),
@@ -227,11 +227,11 @@ class ChunkDecoder:
     def launches_per_call(self, n_chunks=1) -> int:
         return self._check(LIB.ufnvc_launches_per_call(self.handle, n_chunks), "ufnvc_launches_per_call")
 
-    def chunk_decode_profiled(self, z, bits, sub_off, frames, stream=None):
-        us = (C.c_float * 6)()
+    def chunk_decode_profiled(self, z, bits, sub_off, frames, stream=None, detail=False):
+        us = (C.c_float * 7)()
         self._check(LIB.ufnvc_chunk_decode_profiled(self.handle, z.shape[0], _ptr(z), _ptr(bits), bits.numel(), _ptr(sub_off),
-                                                    _ptr(frames), self._stream(stream), us), "ufnvc_chunk_decode_profiled")
-        return dict(zip(("A1+A2", "A3+A4", "A5", "A6+A7", "A8", "A9"), [float(x) for x in us]))
+                                                    _ptr(frames), self._stream(stream), int(detail), us), "ufnvc_chunk_decode_profiled")
+        return dict(zip(("A1+A2", "A3+A4", "A5", "A6+A7", "A8", "A9", "A6"), [float(x) for x in us]))
 
     # ---- encoder-side fixtures (host) ----
     def get_cdf(self) -> np.ndarray:

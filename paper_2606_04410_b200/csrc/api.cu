@@ -127,6 +127,7 @@ extern "C" int ufnvc_destroy(ufnvc_handle *h)
     cudaDeviceSynchronize();
     for (void *p : h->allocs) cudaFree(p);
     if (h->ev_made) for (auto &e : h->ev) cudaEventDestroy(e);
+    for (auto &e : h->ev_dw) cudaEventDestroy(e);
     delete h;
     return UFNVC_OK;
 }

@@ -31,7 +31,7 @@ cudaError_t conv(ufnvc_handle *h, const ConvLayer &L, const ConvProblem &P, cons
     return launch_conv_generic(L, P, E, st);
 }
 
-struct Stage { cudaEvent_t *ev; int i; };
+struct Stage { cudaEvent_t *ev; int i; cudaEvent_t *dw; };   // dw: one event after every depthwise launch (A6 / A7 split)
 inline void mark(Stage *s, cudaStream_t st) { if (s) cudaEventRecord(s->ev[s->i++], st); }
 
 int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bits_bytes, const uint32_t *sub_off, float *frames,
@@ -122,9 +122,11 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     const int Ce = Ct * c.trunk_expand;
     for (int k = 0; k < c.n_trunk_blocks; ++k) {
         const ufnvc_handle::TrunkBlock &tb = h->trunk[k];
+        if (sg && sg->dw) { cudaEventRecord(sg->dw[2 * k + 1], st); }
         if (h->dw_tma_ok) CU_TRY(launch_dwconv3x3_tma(h->tm_dw, h->fb, tb.dw_w, tb.dw_b, n * T, h->h, h->w, Ct, st));
         else CU_TRY(launch_dwconv3x3(h->fa, h->fb, tb.dw_w, tb.dw_b, n * T, h->h, h->w, Ct, st));
         if (launches) ++*launches;
+        if (sg && sg->dw) { cudaEventRecord(sg->dw[2 * k], st); }
         if (h->use_fused_trunk && tb.fused.ok && !h->force_generic) {
             CU_TRY(launch_trunk_mlp(tb.fused, tb.pw1, tb.pw2, h->fa, h->fa, (long long)n * T * P, h->num_sms, h->use_pair_trunk, st));
             if (launches) ++*launches;
@@ -286,7 +288,7 @@ extern "C" int ufnvc_launches_per_call(const ufnvc_handle *h, int n_chunks)
 
 extern "C" int ufnvc_chunk_decode_profiled(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, const uint8_t *bits_dev,
                                            size_t bits_bytes, const uint32_t *sub_off_dev, float *frames_dev, void *cuda_stream,
-                                           float *us_out_host)
+                                           int detail, float *us_out_host)
 {
     if (int rc = check_call(h, n_chunks, z_dev, bits_dev, sub_off_dev)) return rc;
     if (!frames_dev || !us_out_host) return fail(h, UFNVC_E_INVALID_ARG, "null frames_dev / us_out_host");
@@ -295,7 +297,12 @@ extern "C" int ufnvc_chunk_decode_profiled(ufnvc_handle *h, int n_chunks, const 
         for (auto &e : h->ev) CU_TRY(cudaEventCreate(&e));
         h->ev_made = true;
     }
-    Stage sg{h->ev, 0};
+    if (h->ev_dw.size() < size_t(2 * h->cfg.n_trunk_blocks)) {
+        const size_t old = h->ev_dw.size();
+        h->ev_dw.resize(size_t(2 * h->cfg.n_trunk_blocks));
+        for (size_t i = old; i < h->ev_dw.size(); ++i) CU_TRY(cudaEventCreate(&h->ev_dw[i]));
+    }
+    Stage sg{h->ev, 0, (detail && !h->ev_dw.empty()) ? h->ev_dw.data() : nullptr};
     if (int rc = run(h, n_chunks, z_dev, bits_dev, bits_bytes, sub_off_dev, frames_dev, st, nullptr, nullptr, nullptr, false, nullptr,
                      nullptr, nullptr, &sg, nullptr))
         return rc;
@@ -306,5 +313,13 @@ extern "C" int ufnvc_chunk_decode_profiled(ufnvc_handle *h, int n_chunks, const 
         CU_TRY(cudaEventElapsedTime(&ms, h->ev[i], h->ev[i + 1]));
         us_out_host[i] = ms * 1000.f;
     }
+    // us_out_host[6] = A6 alone: the sum over the trunk blocks of (event after the depthwise launch - event before it)
+    float dw_us = 0.f;
+    for (int k = 0; detail && k < h->cfg.n_trunk_blocks; ++k) {
+        float ms = 0.f;
+        CU_TRY(cudaEventElapsedTime(&ms, h->ev_dw[2 * k + 1], h->ev_dw[2 * k]));
+        dw_us += ms * 1000.f;
+    }
+    us_out_host[6] = dw_us;
     return UFNVC_OK;
 }

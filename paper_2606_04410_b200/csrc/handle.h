@@ -67,6 +67,7 @@ struct ufnvc_handle {
 
     std::vector<void *> allocs;          // everything cudaMalloc'ed, freed at destroy
     cudaEvent_t ev[8] = {};
+    std::vector<cudaEvent_t> ev_dw;      // profiled call: before / after every depthwise launch
     bool ev_made = false;
 };
 
