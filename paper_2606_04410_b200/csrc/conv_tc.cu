@@ -702,6 +702,15 @@ bool tc_encode_2d(CUtensorMap *tm, const void *base, unsigned long long dim0, un
     return encode(tm, base, 2, dims, strides, box, err);
 }
 
+bool tc_encode_3d(CUtensorMap *tm, const void *base, unsigned long long d0, unsigned long long d1, unsigned long long d2, unsigned b0,
+                  unsigned b1, unsigned b2, std::string &err)
+{
+    cuuint64_t dims[3] = {d0, d1, d2};
+    cuuint64_t strides[2] = {d0 * 2, d0 * d1 * 2};
+    cuuint32_t box[3] = {b0, b1, b2};
+    return encode(tm, base, 3, dims, strides, box, err);
+}
+
 bool tc_make_weight_tmap(ConvLayer &L, std::string &err)
 {
     L.use_tc = false;

@@ -160,9 +160,14 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
 
     // ---- A9: last stage (linear) + pixel-shuffle + clamp + crop + planar fp32 ----
     {
-        ConvProblem pr{x, n * T, sh, sw, T};
-        EpiParams E{EPI_FINAL, ACT_NONE, frames, nullptr, 0, 0, (long long)3 * c.height * c.width, 3, c.height, c.width};
-        CU_TRY(conv(h, h->dec[3], pr, *am, E, st, launches));
+        if (h->final_is.ok && !h->force_generic) {
+            CU_TRY(launch_final_is(h->final_is, h->dec[3], n * T, sh, sw, frames, c.height, c.width, h->num_sms, st));
+            ++*launches;
+        } else {
+            ConvProblem pr{x, n * T, sh, sw, T};
+            EpiParams E{EPI_FINAL, ACT_NONE, frames, nullptr, 0, 0, (long long)3 * c.height * c.width, 3, c.height, c.width};
+            CU_TRY(conv(h, h->dec[3], pr, *am, E, st, launches));
+        }
     }
     mark(sg, st);
     return UFNVC_OK;
@@ -243,6 +248,12 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
         if (ok && !trunk_make_maps(tb.fused, h->fb, (long long)n * T * h->h * h->w, tb.pw1, tb.pw2, h->err)) ok = false;
     for (int s = 0; ok && s < 3; ++s)
         ok = make_act_map(h, h->am_stage[s], h->stage[s], n * T, h->h << (s + 1), h->w << (s + 1), c.dec_channels[s + 1], false, T);
+    {
+        const char *fi = std::getenv("UFNVC_FINAL_IS");
+        h->final_is.ok = false;
+        if (ok && !(fi && fi[0] == '0') && c.dec_channels[3] % 64 == 0)
+            ok = final_make_maps(h->final_is, h->dec[3], h->stage[2], n * T, h->h << 3, h->w << 3, c.width, h->err);
+    }
     if (!ok) return fail(h, UFNVC_E_CUDA, h->err);
     h->weights_loaded = true;
     return UFNVC_OK;

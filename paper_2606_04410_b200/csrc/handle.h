@@ -61,6 +61,7 @@ struct ufnvc_handle {
         CUtensorMap tm_halo;             // 3x3 convs: box {64, 10, 18}: a 16 x 8 pixel tile plus halo (conv_halo_kernel)
         bool halo_ok = false;
     };
+    ufnvc::FinalMaps final_is;           // A9 input-stationary kernel (env UFNVC_FINAL_IS=0 disables)
     CUtensorMap tm_dw;                   // fa as the depthwise kernel reads it: box {64 ch, 10, 10}
     bool dw_tma_ok = false;
     ActMap am_xs, am_yhat, am_fa, am_fb, am_hidden, am_stage[3];

@@ -123,6 +123,18 @@ bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W
 bool tc_encode_2d(CUtensorMap *tm, const void *base, unsigned long long dim0, unsigned long long dim1, unsigned box0, unsigned box1,
                   std::string &err);   // 2-D bf16 map, dim0 contiguous, 128B swizzle, zero OOB fill
 
+bool tc_encode_3d(CUtensorMap *tm, const void *base, unsigned long long d0, unsigned long long d1, unsigned long long d2, unsigned b0,
+                  unsigned b1, unsigned b2, std::string &err);
+
+// A9, input-stationary (final_tc.cu): 9 taps folded into N, shifted sum of the partial planes in the epilogue
+struct FinalMaps {
+    CUtensorMap tm_in, tm_w;
+    bool ok = false;
+};
+bool final_make_maps(FinalMaps &m, const ConvLayer &L, const bf16 *in_base, int n_img, int H, int W, int out_w, std::string &err);
+cudaError_t launch_final_is(const FinalMaps &m, const ConvLayer &L, int n_img, int H, int W, float *out, int out_h, int out_w,
+                            int num_sms, cudaStream_t st);
+
 // fused trunk MLP (trunk_tc.cu): out = x + W2 GELU(W1 d + b1) + b2 in one kernel, hidden kept on chip
 struct TrunkMaps {
     CUtensorMap tm_d, tm_w1, tm_w2, tm_w1h, tm_w2h;   // *h: half tiles for the CTA-pair kernel
