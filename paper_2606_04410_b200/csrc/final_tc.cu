@@ -153,12 +153,15 @@ final_is_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant
                   "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
                 : "r"(taddr));
         };
-        int it = 0;
+        int it = 0, bias_grp = -1;
+        float bs[12];
         for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x, ++it) {
             const FTile t = f_tile(p, tile);
-            float bs[12];
+            if (t.grp != bias_grp) {                                       // (L1 is a few KB here: keep the bias out of the tile loop)
 #pragma unroll
-            for (int n = 0; n < 12; ++n) bs[n] = __ldg(p.bias + t.grp * 16 + n);
+                for (int n = 0; n < 12; ++n) bs[n] = __ldg(p.bias + t.grp * 16 + n);
+                bias_grp = t.grp;
+            }
             mbar_wait(bar(F_DFULL + g), it & 1);
             tc_fence_after();
             // Q[dy][n] = sum_dx P[(r, cx + dx - 1)][(dy, dx)][n]: the two side terms come from the neighbouring lanes
