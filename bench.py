@@ -246,7 +246,7 @@ def run_ours(args):
     peak = peaks["tensor_sustained"]
     stage_mean = {k: statistics.mean(s[k] for s in stage_us) for k in stage_us[0]}
     stage_mean["A6"] = statistics.mean(s["A6"] for s in detail_us)
-    prof = os.path.join(ROOT, "profiles", "traffic.json")
+    prof = os.path.join(ROOT, "profiles", "r01_traffic.json.txt")
     traffic = json.load(open(prof)).get("a8_dram_bytes_per_launch") if os.path.exists(prof) else None
     roofline = dict(bound="tensor", achieved=achieved, peak=peak, unit="TFLOP/s", frac=achieved / peak, traffic=traffic,
                     kernel="A8 frame-decoder stages 1-3 (3 launches of the implicit-GEMM conv kernel)",
