@@ -164,8 +164,11 @@ final_is_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant
             }
             mbar_wait(bar(F_DFULL + g), it & 1);
             tc_fence_after();
-            // Q[dy][n] = sum_dx P[(r, cx + dx - 1)][(dy, dx)][n]: the two side terms come from the neighbouring lanes
-            float Q[3][12];
+            // Q_dy[n] = sum_dx P[(r, cx + dx - 1)][(dy, dx)][n]: the two side terms come from the neighbouring lanes.  Q_0 and
+            // Q_2 are needed by rows r+1 / r-1, i.e. by other warps: they go straight to shared memory (6 float4 planes x 384
+            // pixels, double-buffered over tiles); only Q_1 stays in registers.
+            const uint32_t xq = base + kFOffXQ + uint32_t(it & 1) * kFXQ;
+            float Q1[12];
 #pragma unroll
             for (int dy = 0; dy < 3; ++dy) {
                 uint32_t v0[16], v1[16], v2[16];
@@ -173,24 +176,25 @@ final_is_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant
                 ld16(t_addr + uint32_t((dy * 3 + 1) * 16), v1);
                 ld16(t_addr + uint32_t((dy * 3 + 2) * 16), v2);
                 tmem_ld_wait();
+                float Qd[12];
 #pragma unroll
                 for (int n = 0; n < 12; ++n)
-                    Q[dy][n] = __shfl_up_sync(0xFFFFFFFFu, __uint_as_float(v0[n]), 1) + __uint_as_float(v1[n]) +
-                               __shfl_down_sync(0xFFFFFFFFu, __uint_as_float(v2[n]), 1);
+                    Qd[n] = __shfl_up_sync(0xFFFFFFFFu, __uint_as_float(v0[n]), 1) + __uint_as_float(v1[n]) +
+                            __shfl_down_sync(0xFFFFFFFFu, __uint_as_float(v2[n]), 1);
+                if (dy == 1) {
+#pragma unroll
+                    for (int n = 0; n < 12; ++n) Q1[n] = Qd[n];
+                } else {
+#pragma unroll
+                    for (int c4 = 0; c4 < 3; ++c4)
+                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};"
+                                     ::"r"(xq + uint32_t(3 * (dy >> 1) + c4) * (kFR * kFC * 16) + pix * 16u), "f"(Qd[4 * c4]), "f"(Qd[4 * c4 + 1]),
+                                       "f"(Qd[4 * c4 + 2]), "f"(Qd[4 * c4 + 3]) : "memory");
+                }
             }
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(F_DEMPTY + g));                  // accumulator g may be overwritten
-            // rows r-1 / r+1 belong to other warps: Q[0] and Q[2] go through shared memory (6 float4 planes x 384 pixels)
-            const uint32_t xq = base + kFOffXQ + uint32_t(it & 1) * kFXQ;
-#pragma unroll
-            for (int h = 0; h < 2; ++h)
-#pragma unroll
-                for (int c4 = 0; c4 < 3; ++c4) {
-                    const float *s = Q[2 * h] + 4 * c4;
-                    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(xq + uint32_t(3 * h + c4) * (kFR * kFC * 16) + pix * 16u),
-                                 "f"(s[0]), "f"(s[1]), "f"(s[2]), "f"(s[3]) : "memory");
-                }
             asm volatile("bar.sync 1, 384;" ::: "memory");                 // the 12 row warps
             const int y = t.y0 + r, x = t.x0 + cx;
             if (r >= 1 && r <= kFOutR && cx >= 1 && cx <= kFOutC && y < p.H && x < p.W) {
@@ -202,10 +206,10 @@ final_is_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant
                                  : "r"(xq + uint32_t(c4) * (kFR * kFC * 16) + (pix - kFC) * 16u));
                     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(dn.x), "=f"(dn.y), "=f"(dn.z), "=f"(dn.w)
                                  : "r"(xq + uint32_t(3 + c4) * (kFR * kFC * 16) + (pix + kFC) * 16u));
-                    o[4 * c4 + 0] = bs[4 * c4 + 0] + up.x + Q[1][4 * c4 + 0] + dn.x;
-                    o[4 * c4 + 1] = bs[4 * c4 + 1] + up.y + Q[1][4 * c4 + 1] + dn.y;
-                    o[4 * c4 + 2] = bs[4 * c4 + 2] + up.z + Q[1][4 * c4 + 2] + dn.z;
-                    o[4 * c4 + 3] = bs[4 * c4 + 3] + up.w + Q[1][4 * c4 + 3] + dn.w;
+                    o[4 * c4 + 0] = bs[4 * c4 + 0] + up.x + Q1[4 * c4 + 0] + dn.x;
+                    o[4 * c4 + 1] = bs[4 * c4 + 1] + up.y + Q1[4 * c4 + 1] + dn.y;
+                    o[4 * c4 + 2] = bs[4 * c4 + 2] + up.z + Q1[4 * c4 + 2] + dn.z;
+                    o[4 * c4 + 3] = bs[4 * c4 + 3] + up.w + Q1[4 * c4 + 3] + dn.w;
                 }
                 // packed column n = (2i + j) * 3 + c -> out[img][c][2y + i][2x + j] (R14), clamp (O9), crop
                 float *ob = p.out + (long long)t.img * 3 * p.out_h * p.out_w;
