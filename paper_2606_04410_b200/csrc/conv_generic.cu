@@ -2,6 +2,7 @@
 // The generic conv serves the shapes the tcgen05 kernel does not take (config 1's 48/32/16-channel layers) and is
 // the on-device cross-check of the tensor-core path.  Activations NHWC bf16, fp32 accumulate.
 //   out[pix][n] = bias[n] + sum_{tap, c} in[pix + tap][c] * w[group][tap][n][c]
+#include <cstdlib>
 #include "epilogue.cuh"
 #include "tc_ptx.cuh"
 #include "ufnvc_internal.h"
@@ -99,10 +100,13 @@ cudaError_t launch_conv_generic(const ConvLayer &L, const ConvProblem &P, const 
 // the side columns are L1 hits, loaded by the neighbouring warps of the block) and scattered into three rolling
 // accumulators (output rows r-1, r, r+1), so a row of outputs costs 3 vector loads and 1 store.  For C = 256 a warp is
 // exactly one pixel (512 contiguous bytes).
-// bf16x2 word -> packed (lo, hi) fp32 pair for the FFMA2 pipe: 2 integer ops
+// bf16x2 word -> packed (lo, hi) fp32 pair for the FFMA2 pipe: 2 integer ops.  The shift is written as a byte permute so
+// that it issues on the ALU pipe: the compiler turns "w << 16" into IMAD.U32, which competes with FFMA2 for the FMA pipe.
 __device__ __forceinline__ uint64_t dw_pair(uint32_t w)
 {
-    return f2_pack(__uint_as_float(w << 16), __uint_as_float(w & 0xFFFF0000u));
+    uint32_t lo;
+    asm("prmt.b32 %0, %1, 0, 0x1044;" : "=r"(lo) : "r"(w));
+    return f2_pack(__uint_as_float(lo), __uint_as_float(w & 0xFFFF0000u));
 }
 
 __global__ void __launch_bounds__(256, 2) dwconv3x3_kernel(const bf16 *__restrict__ in, bf16 *__restrict__ out,
@@ -183,94 +187,123 @@ __global__ void __launch_bounds__(256, 2) dwconv3x3_kernel(const bf16 *__restric
     }
 }
 
-// ---- A6, TMA-staged variant (C a multiple of 64).  One block = an 8 x 8 pixel tile of one image, all channels: one
-// TMA box {64 ch, 10, 10} per 64-channel slab brings the tile plus halo into shared memory (zero-filled outside the
-// image = the conv's zero padding), so ~50 KB per block x 4 blocks per SM are in flight without costing a register --
-// the register-only kernel above is latency-bound (16 warps/SM, 8 KB of unique loads in flight, 28 % of HBM peak).
+// ---- A6, TMA-staged variant (C a multiple of 64).  One tile = 8 x 8 pixels of one image, all channels: one TMA box
+// {64 ch, 10, 10} per 64-channel slab brings the tile plus halo into shared memory (zero-filled outside the image =
+// the conv's zero padding).  The kernel is persistent (two blocks per SM) and double-buffered: the load of a block's
+// next tile is in flight while it computes the current one, so ~100 KB per block are in flight without costing a
+// register -- the register-only kernel above is latency-bound (16 warps/SM, 8 KB of unique loads in flight).
 // Thread (x, c8) then walks down its column with the same rolling 3-row window, reading 3 conflict-free LDS.128 per row.
 constexpr int kDwT = 8;                                   // tile edge (pixels)
 constexpr int kDwHalo = kDwT + 2;
-constexpr uint32_t kDwSlab = ((kDwHalo * kDwHalo * 128 + 1023) / 1024) * 1024;     // 13312 B, 1024-aligned for the swizzle
+constexpr uint32_t kDwSlab = ((kDwHalo * kDwHalo * 128 + 1023) / 1024) * 1024;     // 13312 B per 64-channel slab (dense box, no swizzle)
 
-__global__ void __launch_bounds__(256, 2) dwconv3x3_tma_kernel(const __grid_constant__ CUtensorMap tm_in, bf16 *__restrict__ out,
+// V = channel PAIRS per thread: 4 (8 channels, LDS.128, C threads) is what is launched; 2 (4 channels, LDS.64, 2 C threads,
+// twice the warps at half the registers) measured 7 % slower on B200 (more address and loop overhead per output).
+template <int V>
+__global__ void __launch_bounds__(V == 4 ? 256 : 512, 2) dwconv3x3_tma_kernel(const __grid_constant__ CUtensorMap tm_in, bf16 *__restrict__ out,
                                                              const float *__restrict__ w9c, const float *__restrict__ bias,
-                                                             int H, int W, int C, int tiles_x, int tiles_y)
+                                                             int n_img, int H, int W, int C, int tiles_x, int tiles_y)
 {
     extern __shared__ __align__(1024) uint8_t dw_smem[];
     const uint32_t base = (smem_u32(dw_smem) + 1023u) & ~1023u;
     const int slabs = C >> 6;
-    const uint32_t bar = base + uint32_t(slabs) * kDwSlab;
-    int tile = blockIdx.x;
-    const int tx = tile % tiles_x; tile /= tiles_x;
-    const int ty = tile % tiles_y;
-    const int img = tile / tiles_y;
-    const int x0 = tx * kDwT, y0 = ty * kDwT;
+    const uint32_t buf_bytes = uint32_t(slabs) * kDwSlab;
+    const uint32_t bar = base + 2u * buf_bytes;                       // two full barriers, one per buffer
+    const int n_tiles = n_img * tiles_x * tiles_y;
+    auto issue = [&](int t, uint32_t b) {                              // thread 0: TMA the tile + halo into buffer b
+        const int tx = t % tiles_x, r = t / tiles_x;
+        const int ty = r % tiles_y, im = r / tiles_y;
+        mbar_expect_tx(bar + 8u * b, uint32_t(slabs) * (kDwHalo * kDwHalo * 128));
+        for (int s = 0; s < slabs; ++s)
+            tma_load_4d(base + b * buf_bytes + uint32_t(s) * kDwSlab, &tm_in, bar + 8u * b, s * 64, tx * kDwT - 1, ty * kDwT - 1, im);
+    };
     if (threadIdx.x == 0) {
         mbar_init(bar, 1);
+        mbar_init(bar + 8, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        mbar_expect_tx(bar, uint32_t(slabs) * (kDwHalo * kDwHalo * 128));
-        for (int s = 0; s < slabs; ++s) tma_load_4d(base + uint32_t(s) * kDwSlab, &tm_in, bar, s * 64, x0 - 1, y0 - 1, img);
+        if (int(blockIdx.x) < n_tiles) issue(blockIdx.x, 0);
+        if (int(blockIdx.x + gridDim.x) < n_tiles) issue(blockIdx.x + gridDim.x, 1);
     }
-    const int cv = C >> 3;
-    const int xl = threadIdx.x / cv, c8 = threadIdx.x % cv;           // column of the tile, 8-channel group
-    const int c0 = c8 * 8;
-    uint64_t wv[9][4], bv[4];
+    constexpr int CH = 2 * V;                                         // channels per thread
+    const int cv = C / CH;
+    const int xl = threadIdx.x / cv, cg = threadIdx.x % cv;           // column of the tile, channel group
+    const int c0 = cg * CH;
+    uint64_t wv[9][V];
 #pragma unroll
     for (int k = 0; k < 9; ++k) {
-        const float4 lo = __ldg(reinterpret_cast<const float4 *>(w9c + k * C + c0));
-        const float4 hi = __ldg(reinterpret_cast<const float4 *>(w9c + k * C + c0 + 4));
-        wv[k][0] = f2_pack(lo.x, lo.y); wv[k][1] = f2_pack(lo.z, lo.w);
-        wv[k][2] = f2_pack(hi.x, hi.y); wv[k][3] = f2_pack(hi.z, hi.w);
+#pragma unroll
+        for (int e = 0; e < V; e += 2) {
+            const float4 q = __ldg(reinterpret_cast<const float4 *>(w9c + k * C + c0 + 2 * e));
+            wv[k][e] = f2_pack(q.x, q.y); wv[k][e + 1] = f2_pack(q.z, q.w);
+        }
     }
-    {
-        const float4 lo = __ldg(reinterpret_cast<const float4 *>(bias + c0)), hi = __ldg(reinterpret_cast<const float4 *>(bias + c0 + 4));
-        bv[0] = f2_pack(lo.x, lo.y); bv[1] = f2_pack(lo.z, lo.w); bv[2] = f2_pack(hi.x, hi.y); bv[3] = f2_pack(hi.z, hi.w);
+    // the bias lives in shared memory and is added when a row is written out: that frees 8 registers, which the
+    // compiler otherwise pays for with local-memory spills inside the row loop
+    const uint32_t bias_s = bar + 16u + uint32_t(c0) * 4u;
+    if (xl == 0) {
+#pragma unroll
+        for (int e = 0; e < V; e += 2) {
+            const float4 q = __ldg(reinterpret_cast<const float4 *>(bias + c0 + 2 * e));
+            asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(bias_s + 8u * e), "f"(q.x), "f"(q.y), "f"(q.z), "f"(q.w) : "memory");
+        }
     }
-    __syncthreads();                                                  // barrier initialised before anyone polls it
-    mbar_wait(bar, 0);
+    __syncthreads();                                                  // barriers initialised before anyone polls them
 
-    const uint32_t slab_base = base + uint32_t(c8 >> 3) * kDwSlab;
-    const uint32_t chunk = uint32_t(c8 & 7);
-    auto lds = [&](int hy, int hx) {                                  // halo pixel -> this thread's 16 bytes (128B swizzle)
-        const uint32_t p = uint32_t(hy * kDwHalo + hx);
-        uint4 v;
-        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
-                     : "r"(slab_base + p * 128u + ((chunk ^ (p & 7u)) << 4)));
-        return v;
-    };
-    uint64_t accP[4], accC[4], accN[4];
+    uint32_t it = 0;
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const uint32_t b = it & 1u;
+        const int tx = tile % tiles_x, trow = tile / tiles_x;
+        const int ty = trow % tiles_y, img = trow / tiles_y;
+        const int x0 = tx * kDwT, y0 = ty * kDwT;
+        mbar_wait(bar + 8u * b, (it >> 1) & 1u);
+        const uint32_t slab_base = base + b * buf_bytes + uint32_t(c0 >> 6) * kDwSlab + uint32_t(c0 & 63) * 2u;
+        // no swizzle needed: 8 (16) consecutive lanes = the 8 (16) channel groups of one slab read one contiguous
+        // 128-byte pixel, which is exactly one conflict-free LDS.128 (LDS.64) phase
+        auto lds = [&](int hy, int hx, uint32_t *v) {                 // halo pixel -> this thread's 2V channels
+            const uint32_t a = slab_base + uint32_t(hy * kDwHalo + hx) * 128u;
+            if constexpr (V == 4) asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(a));
+            else asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=r"(v[0]), "=r"(v[1]) : "r"(a));
+        };
+        uint64_t accP[V], accC[V], accN[V];
 #pragma unroll
-    for (int e = 0; e < 4; ++e) { accP[e] = bv[e]; accC[e] = bv[e]; accN[e] = bv[e]; }
-    const int ox = x0 + xl;
-    bf16 *col_out = out + (((long long)img * H) * W + ox) * C + c0;
+        for (int e = 0; e < V; ++e) { accP[e] = 0ull; accC[e] = 0ull; accN[e] = 0ull; }
+        const int ox = x0 + xl;
+        bf16 *col_out = out + (((long long)img * H) * W + ox) * C + c0;
 #pragma unroll
-    for (int hy = 0; hy < kDwHalo; ++hy) {                            // halo row hy = image row y0 - 1 + hy
-        const uint4 vl = lds(hy, xl), vc = lds(hy, xl + 1), vr = lds(hy, xl + 2);
-        const uint32_t *pl = reinterpret_cast<const uint32_t *>(&vl), *pc = reinterpret_cast<const uint32_t *>(&vc),
-                       *pr = reinterpret_cast<const uint32_t *>(&vr);
+        for (int hy = 0; hy < kDwHalo; ++hy) {                        // halo row hy = image row y0 - 1 + hy
+            uint32_t pl[V], pc[V], pr[V];
+            lds(hy, xl, pl); lds(hy, xl + 1, pc); lds(hy, xl + 2, pr);
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const uint64_t fl = dw_pair(pl[e]), fc = dw_pair(pc[e]), fr = dw_pair(pr[e]);
-            accP[e] = f2_fma(wv[6][e], fl, f2_fma(wv[7][e], fc, f2_fma(wv[8][e], fr, accP[e])));
-            accC[e] = f2_fma(wv[3][e], fl, f2_fma(wv[4][e], fc, f2_fma(wv[5][e], fr, accC[e])));
-            accN[e] = f2_fma(wv[0][e], fl, f2_fma(wv[1][e], fc, f2_fma(wv[2][e], fr, accN[e])));
-        }
-        if (hy >= 2) {                                                // output row y0 + hy - 2 is complete
-            const int oy = y0 + hy - 2;
-            if (oy < H && ox < W) {
-                uint4 o;
-                __nv_bfloat162 *oe = reinterpret_cast<__nv_bfloat162 *>(&o);
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    float a, b;
-                    f2_unpack(accP[e], a, b);
-                    oe[e] = __floats2bfloat162_rn(a, b);
-                }
-                *reinterpret_cast<uint4 *>(col_out + (long long)oy * W * C) = o;
+            for (int e = 0; e < V; ++e) {
+                const uint64_t fl = dw_pair(pl[e]), fc = dw_pair(pc[e]), fr = dw_pair(pr[e]);
+                accP[e] = f2_fma(wv[6][e], fl, f2_fma(wv[7][e], fc, f2_fma(wv[8][e], fr, accP[e])));
+                accC[e] = f2_fma(wv[3][e], fl, f2_fma(wv[4][e], fc, f2_fma(wv[5][e], fr, accC[e])));
+                accN[e] = f2_fma(wv[0][e], fl, f2_fma(wv[1][e], fc, f2_mul(wv[2][e], fr)));
             }
-        }
+            if (hy >= 2) {                                            // output row y0 + hy - 2 is complete
+                const int oy = y0 + hy - 2;
+                if (oy < H && ox < W) {
+                    __nv_bfloat162 oe[V];
+                    uint64_t bq[V];
 #pragma unroll
-        for (int e = 0; e < 4; ++e) { accP[e] = accC[e]; accC[e] = accN[e]; accN[e] = bv[e]; }
+                    for (int e = 0; e < V; e += 2)
+                        asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(bq[e]), "=l"(bq[e + 1]) : "r"(bias_s + 8u * e));
+#pragma unroll
+                    for (int e = 0; e < V; ++e) {
+                        float a, b2;
+                        f2_unpack(f2_add(accP[e], bq[e]), a, b2);
+                        oe[e] = __floats2bfloat162_rn(a, b2);
+                    }
+                    bf16 *dst = col_out + (long long)oy * W * C;
+                    if constexpr (V == 4) *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(oe);
+                    else *reinterpret_cast<uint2 *>(dst) = *reinterpret_cast<const uint2 *>(oe);
+                }
+            }
+#pragma unroll
+            for (int e = 0; e < V; ++e) { accP[e] = accC[e]; accC[e] = accN[e]; }
+        }
+        __syncthreads();                                              // everyone is done reading buffer b
+        if (threadIdx.x == 0 && tile + 2 * int(gridDim.x) < n_tiles) issue(tile + 2 * int(gridDim.x), b);
     }
 }
 
@@ -278,14 +311,18 @@ cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const floa
                                  int C, cudaStream_t st)
 {
     const int tiles_x = (W + kDwT - 1) / kDwT, tiles_y = (H + kDwT - 1) / kDwT;
-    const size_t smem = 1024 + size_t(C >> 6) * kDwSlab + 16;
-    static thread_local bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(dwconv3x3_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    const size_t smem = 1024 + 2 * size_t(C >> 6) * kDwSlab + 16 + size_t(C) * 4;
+    static thread_local int n_sm = 0;
+    if (n_sm == 0) {
+        cudaError_t e = cudaFuncSetAttribute(dwconv3x3_tma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
-        configured = true;
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
     }
-    dwconv3x3_tma_kernel<<<n_img * tiles_x * tiles_y, C, smem, st>>>(tm_in, out, w9c, bias, H, W, C, tiles_x, tiles_y);
+    const int n_tiles = n_img * tiles_x * tiles_y;
+    const int grid = n_tiles < 2 * n_sm ? n_tiles : 2 * n_sm;          // persistent: two blocks per SM, double-buffered tiles
+    dwconv3x3_tma_kernel<4><<<grid, C, smem, st>>>(tm_in, out, w9c, bias, n_img, H, W, C, tiles_x, tiles_y);
     return cudaGetLastError();
 }
 

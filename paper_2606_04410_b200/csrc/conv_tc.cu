@@ -674,13 +674,13 @@ EncodeTiledFn encode_fn()
     return fn;
 }
 bool encode(CUtensorMap *tm, const void *base, int rank, const cuuint64_t *dims, const cuuint64_t *strides_bytes, const cuuint32_t *box,
-            std::string &err)
+            std::string &err, CUtensorMapSwizzle swz = CU_TENSOR_MAP_SWIZZLE_128B)
 {
     EncodeTiledFn fn = encode_fn();
     if (!fn) { err = "cuTensorMapEncodeTiled entry point not found"; return false; }
     cuuint32_t ones[5] = {1, 1, 1, 1, 1};
     CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, rank, const_cast<void *>(base), dims, strides_bytes, box, ones,
-                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, swz, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { err = "cuTensorMapEncodeTiled failed: " + std::to_string(int(r)); return false; }
     return true;
@@ -731,12 +731,13 @@ bool tc_make_weight_tmap(ConvLayer &L, std::string &err)
     return true;
 }
 
-bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, int tile_h, int tile_w, std::string &err)
+bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, int tile_h, int tile_w, std::string &err,
+                      bool swizzle)
 {
     cuuint64_t dims[4] = {cuuint64_t(C), cuuint64_t(W), cuuint64_t(H), cuuint64_t(n_img)};
     cuuint64_t strides[3] = {cuuint64_t(C) * 2, cuuint64_t(C) * 2 * W, cuuint64_t(C) * 2 * W * H};
     cuuint32_t box[4] = {cuuint32_t(kSlabK), cuuint32_t(tile_w), cuuint32_t(tile_h), 1};
-    return encode(tm, base, 4, dims, strides, box, err);
+    return encode(tm, base, 4, dims, strides, box, err, swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE);
 }
 
 bool tc_make_halo_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, std::string &err)

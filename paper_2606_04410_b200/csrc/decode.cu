@@ -240,7 +240,7 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
     {
         const char *dv = std::getenv("UFNVC_DW_TMA");
         if (ok && c.n_trunk_blocks > 0 && c.c_trunk % 64 == 0 && c.c_trunk <= 256 && !(dv && dv[0] == '0')) {
-            ok = tc_make_act_tmap(&h->tm_dw, h->fa, n * T, h->h, h->w, c.c_trunk, 10, 10, h->err);
+            ok = tc_make_act_tmap(&h->tm_dw, h->fa, n * T, h->h, h->w, c.c_trunk, 10, 10, h->err, /*swizzle=*/false);
             h->dw_tma_ok = ok;
         }
     }

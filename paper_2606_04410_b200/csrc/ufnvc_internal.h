@@ -118,7 +118,7 @@ cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUt
 bool tc_make_halo_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, std::string &err);
 bool tc_make_weight_tmap(ConvLayer &L, std::string &err);
 bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, int tile_h, int tile_w,
-                      std::string &err);
+                      std::string &err, bool swizzle = true);
 
 bool tc_encode_2d(CUtensorMap *tm, const void *base, unsigned long long dim0, unsigned long long dim1, unsigned box0, unsigned box1,
                   std::string &err);   // 2-D bf16 map, dim0 contiguous, 128B swizzle, zero OOB fill
