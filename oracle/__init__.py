@@ -196,6 +196,42 @@ def decode_symbols(orc: Oracle, cfg, cdf, idx, bits, sub_off):
     return sym, status
 
 
+def partition_index(c_y, h, w):
+    """NEXT-1, reading R17 (Fig. 4a, "a quadtree-like partition [36] for y_i is adopted"; PAPER.md:101
+    "the quantized latent y_i is divided into four partitions, where each partition's decoding depends on previously
+    decoded partitions").  The geometry is not in the text; R17 takes: channels in four equal groups g = floor(4c/C_y),
+    positions of a 2x2 cell numbered q = 2 (y mod 2) + (x mod 2), partition k = (q + g) mod 4.
+    Returns int [C_y][h][w] with values 0..3."""
+    assert c_y % 4 == 0
+    k = np.empty((c_y, h, w), np.int64)
+    for c in range(c_y):
+        g = (4 * c) // c_y
+        for y in range(h):
+            for x in range(w):
+                k[c, y, x] = (2 * (y % 2) + (x % 2) + g) % 4
+    return k
+
+
+def progressive_means(orc: Oracle, cfg, weights, mu0, sym):
+    """NEXT-1 (the network "predicts the mean mu^0 for the first partition and the scales for all four
+    partitions in a single forward pass"; "We retain the four-step progressive estimation for means
+    ... since mean estimation requires no bit-stream interaction, it executes entirely on GPU"; PAPER.md:125:
+    y = r + mu).  mu0, sym planar [C_y][h][w]; sym is the residual of EVERY partition, already decoded (O4).
+    Step 0: y = r + mu0 on partition 0.  Step k = 1..3 [R17]: mu^k = conv3x3_k([y decoded so far (0 elsewhere) ; mu0]),
+    y = r + mu^k on partition k.  Returns (yhat, mu) with mu[c,y,x] = the mean that element used."""
+    part = partition_index(cfg.c_y, mu0.shape[1], mu0.shape[2])
+    mu0 = orc.arr(mu0)
+    r = sym.astype(orc.dt)
+    mu = np.where(part == 0, mu0, 0.0).astype(orc.dt)
+    yhat = np.where(part == 0, r + mu0, 0.0).astype(orc.dt)
+    for k in (1, 2, 3):
+        s_in = np.concatenate([yhat, mu0], axis=0)
+        mu_k = orc.conv2d(s_in, weights[f"mu.{k}.w"], weights[f"mu.{k}.b"])
+        mu = np.where(part == k, mu_k, mu)
+        yhat = np.where(part == k, r + mu_k, yhat)
+    return yhat, mu
+
+
 def synthesis(orc: Oracle, cfg, weights, yhat, keep=False):
     """O6..O9: cross-frame unfold, shared trunk of DC blocks, T frame-specific
     decoders, clamp + crop.  yhat [C_y][h][w].  Returns frames [T][3][height][width] (+ taps)."""
@@ -234,7 +270,10 @@ def chunk_decode(orc: Oracle, cfg, weights, z, bits, sub_off, idx_override=None,
         mu = orc.arr(mu_override)
     cdf = orc.build_cdf(cfg.n_buckets, cfg.scale_min, cfg.scale_max)          # O3
     sym, status = decode_symbols(orc, cfg, cdf, idx, bits, sub_off)            # O4
-    yhat = sym.astype(orc.dt) + mu                                             # O5
+    if getattr(cfg, "mu_steps", 1) == 4:
+        yhat, mu = progressive_means(orc, cfg, weights, mu, sym)               # NEXT-1: mu becomes the per-element mean used
+    else:
+        yhat = sym.astype(orc.dt) + mu                                         # O5
     frames, taps = synthesis(orc, cfg, weights, yhat, keep=keep)
     return dict(mu=mu, u=u, idx=idx, sym=sym, status=status, yhat=yhat, frames=frames, taps=taps)
 

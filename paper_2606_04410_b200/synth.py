@@ -43,6 +43,7 @@ class ChunkConfig:
     weight_dtype: int = 1          # 0 = fp32, 1 = bf16
     mu_law: str = "normal"         # "normal": N(0,1); "uniform": U(-2,2)
     sigma_hi: float = 20.0         # ln sigma ~ U[ln scale_min, ln sigma_hi] (moment-matched, see make_weights)
+    mu_steps: int = 1              # 1: the head's mean serves every element; 4: progressive means (R17)
 
     # derived geometry (SURVEY.md section 8 notation)
     @property
@@ -82,6 +83,8 @@ class ChunkConfig:
         hz, wz, P = self.h_z, self.w_z, self.h * self.w
         m = hz * wz * 9 * (self.c_z * self.c_hyper + self.c_hyper * self.c_hyper
                            + self.c_hyper * 2 * self.c_y * 16)
+        if self.mu_steps == 4:
+            m += 3 * P * 9 * 2 * self.c_y * self.c_y
         m += P * self.c_y * self.T * self.c_trunk
         m += self.n_trunk_blocks * self.T * P * (9 * self.c_trunk
                                                  + 2 * self.c_trunk * self.c_trunk * self.trunk_expand)
@@ -104,6 +107,11 @@ CONFIGS = {
                    lanes_per_substream=384, n_chunks=4, sigma_hi=2.0),
     5: ChunkConfig("cfg5-4k", 4, 8, 2160, 3840, 128, 64, 128, 256, 8, 4, _DEC),
 }
+
+
+def progressive_config(cfg: ChunkConfig) -> ChunkConfig:
+    """Same workload with the four-step progressive means switched on (R17)."""
+    return dataclasses.replace(cfg, mu_steps=4, name=cfg.name + "-pmu")
 
 
 def crop_config(cfg: ChunkConfig, height: int, width: int, name: str | None = None) -> ChunkConfig:
@@ -178,6 +186,13 @@ def make_weights(cfg: ChunkConfig) -> dict:
     out[name + ".w"] = round_to_bf16(w) if cfg.weight_dtype == 1 else w
     out[name + ".b"] = b.astype(np.float32)
 
+    # progressive means (NEXT-1, R17): three 3x3 convs [yhat so far ; mu0] (2 C_y) -> C_y.  Gain so that a mean keeps
+    # the law of mu0: the input's second moment is ~ (E[yhat^2] * k/4 + E[mu0^2]) / 2 per channel at step k.
+    if cfg.mu_steps == 4:
+        var_mu = 1.0 if cfg.mu_law == "normal" else 4.0 / 3.0
+        for k in (1, 2, 3):
+            ex2_in = 0.5 * (_second_moment_yhat(cfg) * k / 4.0 + var_mu)
+            conv(f"mu.{k}", cfg.c_y, 2 * cfg.c_y, 3, var_mu / ex2_in)
     # cross-frame unfold (O6): gain so that E[F0^2] ~ 1.
     conv("xframe", cfg.T * cfg.c_trunk, cfg.c_y, 1, 1.0 / _second_moment_yhat(cfg))
     # trunk (O7): shared over t; W2 scaled by 1/B so the residual stream stays O(1).
