@@ -107,7 +107,7 @@ def run_reference(args):
     from paper_2606_04410_b200 import synth
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    cfg = synth.CONFIGS[args.config]
+    cfg = synth.CONFIGS[args.config] if args.mu_steps == 1 else synth.progressive_config(synth.CONFIGS[args.config])
     ts_fps = []
     for _ in range(args.warmup if args.warmup < 2 else 1):
         cpu_oracle_time(cfg)
@@ -133,7 +133,7 @@ def run_ours(args):
     dev = torch.device("cuda", local)
     peaks = load_peaks()
 
-    cfg = synth.CONFIGS[args.config]
+    cfg = synth.CONFIGS[args.config] if args.mu_steps == 1 else synth.progressive_config(synth.CONFIGS[args.config])
     n = cfg.n_chunks
     dec = binding.ChunkDecoder(cfg, device=local)
     dec.load_weights(synth.make_weights(cfg))
@@ -265,7 +265,10 @@ def run_ours(args):
         a = flops / (us * 1e-6) / 1e12
         return dict(stage=name, bound="tensor", achieved=a, peak=peak, unit="TFLOP/s", frac=a / peak, flops=flops, us=us)
     a7_us = stage_mean["A6+A7"] - stage_mean["A6"]
-    stages = [hbm("A3+A4 rANS decode + dequant (serial-latency bound, reported against HBM as asked)", nsym * 7 + int(nsym * 0.35), stage_mean["A3+A4"]),
+    a34 = "A3+A4 rANS decode + dequant (serial-latency bound, reported against HBM as asked)"
+    if cfg.mu_steps == 4:
+        a34 = "A3+A4 rANS decode + four-step progressive means (prep + 3 tensor-core convs, R21); bytes are the rANS stage's"
+    stages = [hbm(a34, nsym * 7 + int(nsym * 0.35), stage_mean["A3+A4"]),
               hbm("A5 cross-frame unfold", n * P * cfg.c_y * 2 + act, stage_mean["A5"])]
     if B:
         stages += [hbm("A6 depthwise 3x3 (all trunk blocks)", B * 2 * act, stage_mean["A6"]),
@@ -297,6 +300,8 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=3, help="SURVEY.md config number 1..5 (3 = 1080p headline)")
+    ap.add_argument("--mu-steps", type=int, default=1, choices=[1, 4],
+                    help="4: the same workload with the four-step progressive means switched on (SURVEY.md 8f NEXT-1, DESIGN.md R21)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     args = ap.parse_args()
     if args.impl == "reference":

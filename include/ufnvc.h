@@ -66,13 +66,16 @@ typedef struct ufnvc_config {
     int32_t lanes_per_substream; /* interleaved rANS lanes W per substream, multiple of 32 in [32,512] (default c_y) */
     int32_t max_chunks_per_call; /* independent chunks decoded by one call (1; 4 for config 4) */
     int32_t weight_dtype;        /* dtype of conv weights in the blob: 0 = fp32, 1 = bf16 */
+    int32_t mu_steps;            /* 1: the head's mean serves every element (A4); 4: four-step progressive means
+                                  * (R21) -- needs c_y % 32 == 0 and the mu.{1,2,3}
+                                  * tensors in the blob; three extra conv launches between A4 and A5 */
 } ufnvc_config;
 
 /* Optional device buffers that receive intermediates of ufnvc_chunk_decode_ex (parity/debug; any may be NULL).
  * Layouts are the library's own: channels-last. */
 typedef struct ufnvc_taps {
     uint32_t struct_size;
-    float *mu;          /* [n][h][w][c_y]  mean (O2) */
+    float *mu;          /* [n][h][w][c_y]  mean (O2); with mu_steps == 4 the mean each element used (R21) */
     float *lnscale;     /* [n][h][w][c_y]  clamped ln sigma (O2) */
     uint8_t *idx;       /* [n][h][w][c_y]  bucket index actually used for decoding */
     int16_t *sym;       /* [n][h][w][c_y]  decoded residual r (O4) */
@@ -94,7 +97,9 @@ int ufnvc_destroy(ufnvc_handle *h);
  *                 uint64 offset (from blob start, 16-byte aligned); uint64 nbytes };
  *   data.
  * Tensors (canonical [C_out][C_in][kh][kw], biases fp32 [C_out]): hyper.{0,1,2}.{w,b}, xframe.{w,b},
- * trunk.{k}.{dw,pw1,pw2}.{w,b}, dec.{t}.{s}.{w,b} (t < T, s < 4).  Missing / mis-shaped tensor: UFNVC_E_BAD_BLOB. */
+ * trunk.{k}.{dw,pw1,pw2}.{w,b}, dec.{t}.{s}.{w,b} (t < T, s < 4), and with mu_steps == 4 mu.{1,2,3}.{w,b}
+ * ([c_y][2 c_y][3][3]: input channels [0, c_y) = y decoded so far, [c_y, 2 c_y) = the head's mean).
+ * Missing / mis-shaped tensor: UFNVC_E_BAD_BLOB. */
 int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t bytes);
 
 /* The hot path, one call, everything enqueued on cuda_stream:

@@ -197,9 +197,9 @@ def decode_symbols(orc: Oracle, cfg, cdf, idx, bits, sub_off):
 
 
 def partition_index(c_y, h, w):
-    """NEXT-1, reading R17 (Fig. 4a, "a quadtree-like partition [36] for y_i is adopted"; PAPER.md:101
+    """NEXT-1, reading R21 (Fig. 4a, "a quadtree-like partition [36] for y_i is adopted"; PAPER.md:101
     "the quantized latent y_i is divided into four partitions, where each partition's decoding depends on previously
-    decoded partitions").  The geometry is not in the text; R17 takes: channels in four equal groups g = floor(4c/C_y),
+    decoded partitions").  The geometry is not in the text; R21 takes: channels in four equal groups g = floor(4c/C_y),
     positions of a 2x2 cell numbered q = 2 (y mod 2) + (x mod 2), partition k = (q + g) mod 4.
     Returns int [C_y][h][w] with values 0..3."""
     assert c_y % 4 == 0
@@ -217,7 +217,7 @@ def progressive_means(orc: Oracle, cfg, weights, mu0, sym):
     partitions in a single forward pass"; "We retain the four-step progressive estimation for means
     ... since mean estimation requires no bit-stream interaction, it executes entirely on GPU"; PAPER.md:125:
     y = r + mu).  mu0, sym planar [C_y][h][w]; sym is the residual of EVERY partition, already decoded (O4).
-    Step 0: y = r + mu0 on partition 0.  Step k = 1..3 [R17]: mu^k = conv3x3_k([y decoded so far (0 elsewhere) ; mu0]),
+    Step 0: y = r + mu0 on partition 0.  Step k = 1..3 [R21]: mu^k = conv3x3_k([y decoded so far (0 elsewhere) ; mu0]),
     y = r + mu^k on partition k.  Returns (yhat, mu) with mu[c,y,x] = the mean that element used."""
     part = partition_index(cfg.c_y, mu0.shape[1], mu0.shape[2])
     mu0 = orc.arr(mu0)

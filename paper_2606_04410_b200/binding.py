@@ -26,7 +26,7 @@ class ufnvc_config(C.Structure):
                 ("n_trunk_blocks", C.c_int32), ("trunk_expand", C.c_int32), ("dec_channels", C.c_int32 * 5),
                 ("n_buckets", C.c_int32), ("scale_min", C.c_double), ("scale_max", C.c_double),
                 ("rows_per_substream", C.c_int32), ("lanes_per_substream", C.c_int32),
-                ("max_chunks_per_call", C.c_int32), ("weight_dtype", C.c_int32)]
+                ("max_chunks_per_call", C.c_int32), ("weight_dtype", C.c_int32), ("mu_steps", C.c_int32)]
 
 
 class ufnvc_taps(C.Structure):
@@ -78,6 +78,7 @@ def make_config(cfg, max_chunks: int | None = None) -> ufnvc_config:
         setattr(c, f, getattr(cfg, f))
     c.dec_channels = (C.c_int32 * 5)(*cfg.dec_channels)
     c.max_chunks_per_call = max_chunks if max_chunks is not None else getattr(cfg, "n_chunks", 1)
+    c.mu_steps = getattr(cfg, "mu_steps", 1)
     return c
 
 

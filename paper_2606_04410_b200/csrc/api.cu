@@ -47,6 +47,8 @@ int validate(const ufnvc_config &c, std::string &why)
     BAD(c.lanes_per_substream < 32 || c.lanes_per_substream % 32 || c.lanes_per_substream > 512, "lanes_per_substream: multiple of 32 in [32,512]");
     BAD(c.max_chunks_per_call < 1 || c.max_chunks_per_call > 64, "max_chunks_per_call out of range");
     BAD(c.weight_dtype != 0 && c.weight_dtype != 1, "weight_dtype must be 0 or 1");
+    BAD(c.mu_steps != 1 && c.mu_steps != 4, "mu_steps must be 1 or 4");
+    BAD(c.mu_steps == 4 && c.c_y % 32, "mu_steps == 4 needs c_y % 32 == 0 (the mean convs run on tensor cores only)");
 #undef BAD
     return UFNVC_OK;
 }
@@ -108,6 +110,11 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
               dev_alloc(h, h->yhat, n * P * cfg->c_y) && dev_alloc(h, h->fa, n * T * P * cfg->c_trunk) &&
               dev_alloc(h, h->fb, n * T * P * cfg->c_trunk) &&
               dev_alloc(h, h->hidden, cfg->n_trunk_blocks ? n * T * P * cfg->c_trunk * cfg->trunk_expand : 1);
+    if (ok && cfg->mu_steps == 4) {
+        const size_t cs = (3 * size_t(cfg->c_y) + 63) / 64 * 64;       // [r | mu used | mu0 | zero pad], see weights.cu mu_net
+        ok = dev_alloc(h, h->ymu[0], n * P * cs) && dev_alloc(h, h->ymu[1], n * P * cs) && dev_alloc(h, h->sym, n * P * cfg->c_y) &&
+             cudaMemset(h->ymu[0], 0, n * P * cs * 2) == cudaSuccess && cudaMemset(h->ymu[1], 0, n * P * cs * 2) == cudaSuccess;
+    }
     for (int s = 0; ok && s < 3; ++s) ok = dev_alloc(h, h->stage[s], n * T * (P << (2 * (s + 1))) * cfg->dec_channels[s + 1]);
     if (ok) ok = cudaMemcpy(h->d_cf, cf.data(), cf.size() * 4, cudaMemcpyHostToDevice) == cudaSuccess &&
                  cudaMemcpy(h->d_lut, lut.data(), lut.size() * 2, cudaMemcpyHostToDevice) == cudaSuccess &&

@@ -216,7 +216,8 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
                 tmem_ld32(t_row + uint32_t(c0), v);
                 if (!inb) continue;
                 const int n = tc.nt * p.BN + c0;                  // 32 consecutive packed columns, one store run
-                const long long o = epi_offset(p.E, img, y, x, p.H, p.W, n);
+                const long long pix = ((long long)img * p.H + y) * p.W + x;
+                const long long o = MODE == EPI_MU ? pix * p.E.out_stride + n : epi_offset(p.E, img, y, x, p.H, p.W, n);
                 bf16 *dst = reinterpret_cast<bf16 *>(p.E.out) + o;
                 float f[32];
                 if (p.E.act == ACT_GELU) {
@@ -232,6 +233,47 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
                         const float4 b4 = __ldg(reinterpret_cast<const float4 *>(bias + c0 + j));
                         f[j] = __uint_as_float(v[j]) + b4.x; f[j + 1] = __uint_as_float(v[j + 1]) + b4.y;
                         f[j + 2] = __uint_as_float(v[j + 2]) + b4.z; f[j + 3] = __uint_as_float(v[j + 3]) + b4.w;
+                    }
+                }
+                if (MODE == EPI_MU) {
+                    // R21: f[j] is the candidate mean mu^k of channel n + j, used where the element belongs to partition
+                    // k (y = r + mu^k); elsewhere the mean used so far is carried over.  y travels as
+                    // the pair (r, mu): r is an integer, exact in bf16, so only mu is rounded between the steps.
+                    const EpiParams &E = p.E;
+                    const uint4 *rs = reinterpret_cast<const uint4 *>(E.sym + pix * E.c_y + n);
+                    const uint4 *ms = reinterpret_cast<const uint4 *>(E.y_in + pix * E.in_stride + E.c_y + n);
+                    const int q = 2 * (y & 1) + (x & 1);
+                    float rr[32];
+#pragma unroll
+                    for (int q4 = 0; q4 < 4; ++q4) {
+                        const uint4 r4 = rs[q4], m4 = ms[q4];
+                        const int16_t *re = reinterpret_cast<const int16_t *>(&r4);
+                        const bf16 *me = reinterpret_cast<const bf16 *>(&m4);
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            const int j = q4 * 8 + e;
+                            const int part = (q + (4 * (n + j)) / E.c_y) & 3;
+                            const float r = float(re[e]);
+                            if (part == E.mu_step) {
+                                if (E.mu_tap) E.mu_tap[pix * E.c_y + n + j] = f[j];
+                                if (E.yhat_tap) E.yhat_tap[pix * E.c_y + n + j] = r + f[j];
+                            } else {
+                                f[j] = __bfloat162float(me[e]);                   // 0 on partitions not decoded yet
+                            }
+                            rr[j] = part <= E.mu_step ? r : 0.0f;
+                            if (E.mu_last) f[j] += r;                             // last step: every partition is decoded
+                        }
+                    }
+                    if (!E.mu_last) {                                             // r block, then (below) the mu block
+#pragma unroll
+                        for (int q4 = 0; q4 < 4; ++q4) {
+                            uint4 o4;
+                            __nv_bfloat162 *oe = reinterpret_cast<__nv_bfloat162 *>(&o4);
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) oe[e] = __floats2bfloat162_rn(rr[q4 * 8 + 2 * e], rr[q4 * 8 + 2 * e + 1]);
+                            reinterpret_cast<uint4 *>(dst)[q4] = o4;
+                        }
+                        dst += E.c_y;
                     }
                 }
                 if (MODE == EPI_NHWC && p.E.residual) {
@@ -711,11 +753,11 @@ bool tc_encode_3d(CUtensorMap *tm, const void *base, unsigned long long d0, unsi
     return encode(tm, base, 3, dims, strides, box, err);
 }
 
-bool tc_make_weight_tmap(ConvLayer &L, std::string &err)
+bool tc_make_weight_tmap(ConvLayer &L, std::string &err, int block_n)
 {
     L.use_tc = false;
     if (L.c_in % kSlabK || L.n_pad % 16) return true;                  // not eligible: stays on the CUDA-core kernel
-    L.block_n = pick_block_n(L.n_pad);
+    L.block_n = (block_n > 0 && L.n_pad % block_n == 0) ? block_n : pick_block_n(L.n_pad);
     if (L.block_n != 16 && L.block_n % 32) return true;                // epilogue works on 32-column runs
     cuuint64_t dims[3] = {cuuint64_t(L.c_in), cuuint64_t(L.n_pad), cuuint64_t(L.groups) * L.taps};
     cuuint64_t strides[2] = {cuuint64_t(L.c_in) * 2, cuuint64_t(L.c_in) * 2 * L.n_pad};
@@ -836,6 +878,7 @@ cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUt
         case EPI_NHWC: return resident ? launch(conv_halo_kernel<EPI_NHWC, true>) : launch(conv_halo_kernel<EPI_NHWC, false>);
         case EPI_PS2: return resident ? launch(conv_halo_kernel<EPI_PS2, true>) : launch(conv_halo_kernel<EPI_PS2, false>);
         case EPI_HEAD: return resident ? cudaErrorInvalidValue : launch(conv_halo_kernel<EPI_HEAD, false>);
+        case EPI_MU: return resident ? launch(conv_halo_kernel<EPI_MU, true>) : launch(conv_halo_kernel<EPI_MU, false>);
         default: return resident ? launch(conv_halo_kernel<EPI_FINAL, true>) : launch(conv_halo_kernel<EPI_FINAL, false>);
     }
 }
@@ -883,6 +926,7 @@ cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUten
         case EPI_NHWC: return launch(conv_tc_kernel<EPI_NHWC>);
         case EPI_PS2: return launch(conv_tc_kernel<EPI_PS2>);
         case EPI_HEAD: return launch(conv_tc_kernel<EPI_HEAD>);
+        case EPI_MU: return launch(conv_tc_kernel<EPI_MU>);
         default: return launch(conv_tc_kernel<EPI_FINAL>);
     }
 }

@@ -100,10 +100,33 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     rp.cf = h->d_cf; rp.lut = h->d_lut;
     rp.n_chunks = n; rp.n_sub = h->n_sub; rp.h = h->h; rp.w = h->w; rp.c_y = c.c_y;
     rp.rows_per_sub = c.rows_per_substream; rp.W = c.lanes_per_substream; rp.n_buckets = c.n_buckets;
-    rp.yhat = h->yhat; rp.sym_tap = taps ? taps->sym : nullptr; rp.yhat_tap = taps ? taps->yhat : nullptr;
+    const bool progressive = c.mu_steps == 4;
+    rp.yhat = h->yhat; rp.sym_tap = progressive ? h->sym : (taps ? taps->sym : nullptr); rp.yhat_tap = taps ? taps->yhat : nullptr;
     rp.status = h->d_status;
     CU_TRY(launch_rans_decode(rp, st));
     *launches += 1;                            // rANS decode
+    if (progressive) {
+        // ---- NEXT-1 (R21): four-step progressive means, no bit-stream contact.  The rANS kernel has
+        // written r (h->sym) and r + mu0 (taps); step 0 keeps that on partition 0, steps 1..3 are 3x3 convs over
+        // [y decoded so far ; mu0] (y as the pair r, mu: mu_steps.cu) whose epilogue switches partition k on.  The last
+        // step writes the dense y that A5 reads.
+        if (taps && taps->sym) CU_TRY(cudaMemcpyAsync(taps->sym, h->sym, ne * 2, cudaMemcpyDeviceToDevice, st));
+        const int cs = h->mu_net[0].c_in;       // [r | mu used | mu0 | pad] channels per pixel
+        CU_TRY(launch_mu_prep(h->sym, mu, h->ymu[0], h->ymu[1], n, h->h, h->w, c.c_y, cs, st));
+        *launches += 1;
+        for (int k = 1; k <= 3; ++k) {
+            const int src = (k - 1) & 1;
+            ConvProblem pr{h->ymu[src], n, h->h, h->w, 1};
+            EpiParams E{};
+            E.mode = EPI_MU; E.act = ACT_NONE;
+            E.out = k < 3 ? static_cast<void *>(h->ymu[k & 1]) : static_cast<void *>(h->yhat);
+            E.out_stride = k < 3 ? cs : c.c_y;
+            E.y_in = h->ymu[src]; E.in_stride = cs;
+            E.sym = h->sym; E.c_y = c.c_y; E.mu_step = k; E.mu_last = k == 3;
+            E.mu_tap = taps ? taps->mu : nullptr; E.yhat_tap = taps ? taps->yhat : nullptr;
+            CU_TRY(conv(h, h->mu_net[k - 1], pr, h->am_ymu[src], E, st, launches));
+        }
+    }
     mark(sg, st);
     if (!frames) return UFNVC_OK;
 
@@ -229,6 +252,7 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
     if (h->hybrid_head) ok = ok && tc_make_weight_tmap(h->head_tc, err);
     for (auto &tb : h->trunk) ok = ok && tc_make_weight_tmap(tb.pw1, err) && tc_make_weight_tmap(tb.pw2, err);
     for (int s = 0; s < 4; ++s) ok = ok && tc_make_weight_tmap(h->dec[s], err);
+    for (int k = 0; k < 3 && c.mu_steps == 4; ++k) ok = ok && tc_make_weight_tmap(h->mu_net[k], err);
     if (!ok) return fail(h, UFNVC_E_CUDA, err);
     const int n = h->max_chunks, T = c.T;
     if (h->hybrid_head) ok = make_act_map(h, h->am_xs, h->xs, n, h->h_z, h->w_z, 2 * c.c_hyper, false, 1);
@@ -236,6 +260,11 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
          make_act_map(h, h->am_fb, h->fb, n * T, h->h, h->w, c.c_trunk, true, T) &&
          make_act_map(h, h->am_hidden, h->hidden, n * T, h->h, h->w, c.c_trunk * c.trunk_expand, true, T) &&
          make_act_map(h, h->am_fa, h->fa, n * T, h->h, h->w, c.c_trunk, false, T);
+    if (c.mu_steps == 4) {
+        for (int b = 0; ok && b < 2; ++b) ok = make_act_map(h, h->am_ymu[b], h->ymu[b], n, h->h, h->w, h->mu_net[0].c_in, false, 1);
+        if (ok && (!h->am_ymu[0].ok || !h->mu_net[0].use_tc || h->force_generic))
+            return fail(h, UFNVC_E_BAD_CONFIG, "mu_steps == 4 needs the tensor-core conv path (c_y % 32 == 0, UFNVC_FORCE_GENERIC unset)");
+    }
     h->dw_tma_ok = false;
     {
         const char *dv = std::getenv("UFNVC_DW_TMA");

@@ -37,6 +37,7 @@ struct ufnvc_handle {
     ufnvc::bf16 *xs = nullptr;           // [n][h_z][w_z][2*c_hyper]: bf16 hi | mid split of the fp64 hx2
     uint32_t *fix_list = nullptr, *fix_count = nullptr;
     ufnvc::ConvLayer xframe;
+    ufnvc::ConvLayer mu_net[3];          // mu_steps == 4: 3x3 convs [y so far ; mu0] -> mu^k, k = 1..3 (R21)
     struct TrunkBlock {
         float *dw_w = nullptr, *dw_b = nullptr;   // [9][C], [C] fp32
         ufnvc::ConvLayer pw1, pw2;
@@ -51,6 +52,8 @@ struct ufnvc_handle {
     uint8_t *idx = nullptr;
     ufnvc::bf16 *yhat = nullptr, *fa = nullptr, *fb = nullptr, *hidden = nullptr;
     ufnvc::bf16 *stage[3] = {nullptr, nullptr, nullptr};
+    ufnvc::bf16 *ymu[2] = {nullptr, nullptr};   // mu_steps == 4: [n][h][w][2 c_y] = y decoded so far | mu0, ping-pong
+    int16_t *sym = nullptr;                     // mu_steps == 4: decoded residual r, [n][h][w][c_y]
 
     // TMA descriptors of the activation tensors the tcgen05 convs read, built once at create (workspace is fixed)
     struct ActMap {
@@ -64,7 +67,7 @@ struct ufnvc_handle {
     ufnvc::FinalMaps final_is;           // A9 input-stationary kernel (env UFNVC_FINAL_IS=0 disables)
     CUtensorMap tm_dw;                   // fa as the depthwise kernel reads it: box {64 ch, 10, 10}
     bool dw_tma_ok = false;
-    ActMap am_xs, am_yhat, am_fa, am_fb, am_hidden, am_stage[3];
+    ActMap am_xs, am_yhat, am_fa, am_fb, am_hidden, am_stage[3], am_ymu[2];
 
     std::vector<void *> allocs;          // everything cudaMalloc'ed, freed at destroy
     cudaEvent_t ev[8] = {};

@@ -1,0 +1,58 @@
+// Progressive means, step 0 (R21).
+// the parameter network "predicts the mean mu^0 for the first partition and the scales for all four
+// partitions in a single forward pass"; "We retain the four-step progressive estimation for means ...
+// since mean estimation requires no bit-stream interaction, it executes entirely on GPU".
+// The residual r of EVERY partition is already decoded (A3).  y = r + mu travels as the PAIR (r, mu): r is an integer
+// in [-127, 127], exact in bf16, so only the small mean is rounded when the convs read it (a 2-term split of y that
+// costs c_y extra input channels and keeps the means ~10x closer to the fp64 oracle than bf16(y) would).
+// This kernel builds the input of the first mean conv,
+//   ymu0[pix] = [ partition 0 ? r : 0  |  partition 0 ? bf16(mu0) : 0  |  bf16(mu0)  |  zero pad ]   (channels-last),
+// and the mu0 block of the second ping-pong buffer.  Steps 1..3 are 3x3 tensor-core convs with the EPI_MU epilogue
+// (conv_tc.cu): on partition k the mean becomes mu^k and r is switched on; the last step writes y = r + mu for A5.
+#include "ufnvc_internal.h"
+
+namespace ufnvc {
+
+__global__ void __launch_bounds__(256) mu_prep_kernel(const int16_t *__restrict__ sym, const float *__restrict__ mu0,
+                                                      bf16 *__restrict__ ymu0, bf16 *__restrict__ ymu1, long long n_pix, int H, int W,
+                                                      int c_y, int stride)
+{
+    const int c8 = c_y >> 3;                                        // 8-channel groups per pixel
+    const long long total = n_pix * c8;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const long long pix = i / c8;
+        const int c0 = int(i - pix * c8) * 8;
+        const int x = int(pix % W), y = int((pix / W) % H);
+        const uint4 r4 = *reinterpret_cast<const uint4 *>(sym + pix * c_y + c0);
+        const float4 m0 = *reinterpret_cast<const float4 *>(mu0 + pix * c_y + c0);
+        const float4 m1 = *reinterpret_cast<const float4 *>(mu0 + pix * c_y + c0 + 4);
+        const int16_t *re = reinterpret_cast<const int16_t *>(&r4);
+        const float m[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+        uint4 rv, uv, mv;
+        bf16 *rq = reinterpret_cast<bf16 *>(&rv), *uq = reinterpret_cast<bf16 *>(&uv), *mq = reinterpret_cast<bf16 *>(&mv);
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+            const bool first = mu_partition(c0 + e, y, x, c_y) == 0;
+            rq[e] = __float2bfloat16_rn(first ? float(re[e]) : 0.0f);
+            uq[e] = __float2bfloat16_rn(first ? m[e] : 0.0f);
+            mq[e] = __float2bfloat16_rn(m[e]);
+        }
+        *reinterpret_cast<uint4 *>(ymu0 + pix * stride + c0) = rv;
+        *reinterpret_cast<uint4 *>(ymu0 + pix * stride + c_y + c0) = uv;
+        *reinterpret_cast<uint4 *>(ymu0 + pix * stride + 2 * c_y + c0) = mv;
+        *reinterpret_cast<uint4 *>(ymu1 + pix * stride + 2 * c_y + c0) = mv;
+    }
+}
+
+cudaError_t launch_mu_prep(const int16_t *sym, const float *mu0, bf16 *ymu0, bf16 *ymu1, int n_img, int H, int W, int c_y, int stride,
+                           cudaStream_t st)
+{
+    const long long n_pix = (long long)n_img * H * W;
+    const long long total = n_pix * (c_y >> 3);
+    long long blocks = (total + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    mu_prep_kernel<<<int(blocks), 256, 0, st>>>(sym, mu0, ymu0, ymu1, n_pix, H, W, c_y, stride);
+    return cudaGetLastError();
+}
+
+}  // namespace ufnvc

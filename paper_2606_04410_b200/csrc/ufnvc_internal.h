@@ -19,7 +19,8 @@ enum EpiMode : int {
     EPI_NHWC = 0,   // out[img][split][pix][n % n_split]  (bf16), optional residual with the same indexing
     EPI_PS2 = 1,    // pixel-shuffle x2 (R14): packed column n' = (2i+j)*C_o + c -> out[img][2y+i][2x+j][c] (bf16)
     EPI_FINAL = 2,  // EPI_PS2 + clamp [0,1] + crop + planar fp32 store out[img][c][Y][X]  (A9)
-    EPI_HEAD = 3    // hyper head (A2): pixel-shuffle x4 + crop; mu half -> fp32, scale half -> clamp, bucket, edge flag
+    EPI_HEAD = 3,   // hyper head (A2): pixel-shuffle x4 + crop; mu half -> fp32, scale half -> clamp, bucket, edge flag
+    EPI_MU = 4      // progressive means (R21): column n = latent channel; y = r + mu^k on partition k, old y elsewhere
 };
 enum Act : int { ACT_NONE = 0, ACT_GELU = 1 };
 
@@ -38,7 +39,17 @@ struct EpiParams {
     uint32_t *fix_list, *fix_count;   // elements whose tensor-core ln sigma is within flag_t of a bucket edge
     int c_y, lat_h, lat_w, n_buckets;
     float ln_lo, ln_hi, t_scale, flag_t;   // t = (u - ln_lo) * t_scale + 0.5; flag when |t - round(t)| < flag_t
+    // EPI_MU (uses c_y), mu^k = acc + bias.  The conv input is [r so far | mu used so far | mu0 | pad] (bf16, in_stride
+    // channels).  mu_last == 0: out has the same layout: r and mu blocks updated on partition mu_step.
+    // mu_last == 1: out = dense y = r + mu, [pix][out_stride] (what A5 reads).
+    const int16_t *sym;      // [pix][c_y] decoded residual r
+    const bf16 *y_in;        // the conv's own input
+    int in_stride, out_stride, mu_step, mu_last;
+    float *mu_tap, *yhat_tap;   // optional fp32 [pix][c_y], written on partition mu_step only
 };
+
+// R21: partition of latent element (channel c, row y, column x): four channel groups x the four positions of a 2x2 cell
+__host__ __device__ inline int mu_partition(int c, int y, int x, int c_y) { return (2 * (y & 1) + (x & 1) + (4 * c) / c_y) & 3; }
 
 // One conv layer as the kernels consume it.  Weights are K-major ("[n][k]", k = c_in contiguous) per tap and
 // per weight group: w[group][tap][n_pad][c_in] bf16; bias[group][n_pad] fp32.  For EPI_PS2/FINAL layers the
@@ -64,6 +75,10 @@ struct ConvProblem {
 cudaError_t launch_conv_generic(const ConvLayer &L, const ConvProblem &P, const EpiParams &E, cudaStream_t st);
 cudaError_t launch_dwconv3x3(const bf16 *in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
                              int C, cudaStream_t st);
+
+// progressive means, step 0 (R21): ymu0 = [partition 0 ? r : 0 | partition 0 ? mu0 : 0 | mu0 | pad], ymu1's mu0 block
+cudaError_t launch_mu_prep(const int16_t *sym, const float *mu0, bf16 *ymu0, bf16 *ymu1, int n_img, int H, int W, int c_y, int stride,
+                           cudaStream_t st);
 
 cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
                                  int C, cudaStream_t st);   // tm_in: NHWC map of `in` with box {64, 10, 10, 1}
@@ -116,7 +131,7 @@ cudaError_t launch_conv_halo_pair(const ConvLayer &L, const ConvProblem &P, cons
 cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
                              cudaStream_t st);
 bool tc_make_halo_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, std::string &err);
-bool tc_make_weight_tmap(ConvLayer &L, std::string &err);
+bool tc_make_weight_tmap(ConvLayer &L, std::string &err, int block_n = 0);   // block_n = 0: widest N tile that divides n_pad
 bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, int tile_h, int tile_w,
                       std::string &err, bool swizzle = true);
 

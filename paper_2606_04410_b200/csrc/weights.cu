@@ -83,6 +83,33 @@ struct Loader {
         return L.w && L.bias;
     }
 
+    // Progressive-mean conv k (R21): canonical [c_y][2 c_y][3][3] over [y so far ; mu0].  The kernel feeds y as TWO inputs,
+    // y = r + mu with r an integer (exact in bf16) and mu small (bf16 rounding error ~2^-9 |mu|), so the y block of
+    // the weights is used twice: device input channels = [r | mu used so far | mu0 | zero pad to a multiple of 64].
+    bool mu_net(ConvLayer &L, const std::string &name, int c_y)
+    {
+        const Tensor *tw = get(name + ".w", {uint32_t(c_y), uint32_t(2 * c_y), 3u, 3u});
+        const Tensor *tb = get(name + ".b", {uint32_t(c_y)});
+        if (!tw || !tb) return false;
+        const int c_in = (3 * c_y + 63) / 64 * 64;
+        L.c_in = c_in; L.n = c_y; L.n_pad = (c_y + 15) / 16 * 16; L.taps = 9; L.groups = 1;
+        std::vector<uint16_t> w(size_t(9) * L.n_pad * c_in, 0);
+        std::vector<float> b(L.n_pad, 0.f);
+        for (int o = 0; o < c_y; ++o) {
+            b[o] = tb->at(o);
+            for (int tap = 0; tap < 9; ++tap)
+                for (int c = 0; c < c_y; ++c) {
+                    const uint16_t wy = f32_to_bf16_rne(tw->at((size_t(o) * 2 * c_y + c) * 9 + tap));
+                    const uint16_t wm = f32_to_bf16_rne(tw->at((size_t(o) * 2 * c_y + c_y + c) * 9 + tap));
+                    uint16_t *row = &w[(size_t(tap) * L.n_pad + o) * c_in];
+                    row[c] = wy; row[c_y + c] = wy; row[2 * c_y + c] = wm;
+                }
+        }
+        L.w = reinterpret_cast<bf16 *>(upload(w));
+        L.bias = upload(b);
+        return L.w && L.bias;
+    }
+
     bool hyper(HyperLayer &L, const std::string &name, int c_in, int n)
     {
         const Tensor *tw = get(name + ".w", {uint32_t(n), uint32_t(c_in), 3u, 3u});
@@ -172,6 +199,7 @@ int load_weights_impl(ufnvc_handle *h, const void *blob, size_t bytes)
               ld.hyper(h->hyper[2], "hyper.2", c.c_hyper, 2 * c.c_y * 16);
     if (ok && h->hybrid_head) ok = ld.head_hybrid(h->head_tc, h->head_fix_w, h->head_fix_b, "hyper.2", c.c_hyper, c.c_y);
     ok = ok && ld.conv(h->xframe, {"xframe"}, c.c_y, c.T * c.c_trunk, 1, false);
+    for (int k = 1; ok && c.mu_steps == 4 && k <= 3; ++k) ok = ld.mu_net(h->mu_net[k - 1], "mu." + std::to_string(k), c.c_y);
     h->trunk.assign(c.n_trunk_blocks, ufnvc_handle::TrunkBlock());
     const int ce = c.c_trunk * c.trunk_expand;
     for (int k = 0; ok && k < c.n_trunk_blocks; ++k) {

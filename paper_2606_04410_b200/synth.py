@@ -43,7 +43,7 @@ class ChunkConfig:
     weight_dtype: int = 1          # 0 = fp32, 1 = bf16
     mu_law: str = "normal"         # "normal": N(0,1); "uniform": U(-2,2)
     sigma_hi: float = 20.0         # ln sigma ~ U[ln scale_min, ln sigma_hi] (moment-matched, see make_weights)
-    mu_steps: int = 1              # 1: the head's mean serves every element; 4: progressive means (R17)
+    mu_steps: int = 1              # 1: the head's mean serves every element; 4: progressive means (R21)
 
     # derived geometry (SURVEY.md section 8 notation)
     @property
@@ -110,7 +110,7 @@ CONFIGS = {
 
 
 def progressive_config(cfg: ChunkConfig) -> ChunkConfig:
-    """Same workload with the four-step progressive means switched on (R17)."""
+    """Same workload with the four-step progressive means switched on (R21)."""
     return dataclasses.replace(cfg, mu_steps=4, name=cfg.name + "-pmu")
 
 
@@ -186,7 +186,7 @@ def make_weights(cfg: ChunkConfig) -> dict:
     out[name + ".w"] = round_to_bf16(w) if cfg.weight_dtype == 1 else w
     out[name + ".b"] = b.astype(np.float32)
 
-    # progressive means (NEXT-1, R17): three 3x3 convs [yhat so far ; mu0] (2 C_y) -> C_y.  Gain so that a mean keeps
+    # progressive means (NEXT-1, R21): three 3x3 convs [yhat so far ; mu0] (2 C_y) -> C_y.  Gain so that a mean keeps
     # the law of mu0: the input's second moment is ~ (E[yhat^2] * k/4 + E[mu0^2]) / 2 per channel at step k.
     if cfg.mu_steps == 4:
         var_mu = 1.0 if cfg.mu_law == "normal" else 4.0 / 3.0

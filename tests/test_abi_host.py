@@ -1,5 +1,6 @@
 """CPU-only checks of the boundary: the library loads, exports what include/ufnvc.h declares, host logic works."""
 import ctypes as C
+import dataclasses
 import os
 import re
 import struct
@@ -30,7 +31,7 @@ def test_library_exports_every_declared_symbol():
 
 def test_config_struct_layout():
     c = binding.make_config(synth.CONFIGS[3])
-    assert c.struct_size == C.sizeof(binding.ufnvc_config) == 96
+    assert c.struct_size == C.sizeof(binding.ufnvc_config) == 104
     assert (c.T, c.height, c.width, c.c_y) == (8, 1080, 1920, 128)
     assert list(c.dec_channels) == [256, 192, 128, 64, 3] and c.max_chunks_per_call == 1
     assert binding.make_config(synth.CONFIGS[4]).max_chunks_per_call == 4
@@ -90,3 +91,30 @@ def test_no_gpu_fails_loudly():
     c.struct_size = 4
     assert binding.LIB.ufnvc_create(C.byref(c), C.byref(h)) == -2                       # validated before the device
     assert binding.LIB.ufnvc_last_error(None) == b"null handle"
+
+
+def test_mu_steps_is_validated_before_the_device():
+    """mu_steps (NEXT-1, R21): 1 or 4; 4 needs c_y % 32 == 0 (the mean convs exist on the tensor-core path only)."""
+    h = C.c_void_p()
+    for steps, c_y, want_bad in ((1, 32, False), (4, 32, False), (2, 32, True), (0, 32, True), (4, 24, True), (4, 128, False)):
+        c = binding.make_config(dataclasses.replace(synth.CONFIGS[1], mu_steps=steps, c_y=c_y))
+        rc = binding.LIB.ufnvc_create(C.byref(c), C.byref(h))
+        if want_bad:
+            assert rc == -2, (steps, c_y, rc)                                           # UFNVC_E_BAD_CONFIG
+        else:
+            assert rc != -2, (steps, c_y, rc)
+            if rc == 0:
+                binding.LIB.ufnvc_destroy(h)
+
+
+def test_progressive_weights_and_blob():
+    cfg = synth.progressive_config(synth.CONFIGS[2])
+    assert cfg.mu_steps == 4 and cfg.name.endswith("-pmu") and synth.CONFIGS[2].mu_steps == 1
+    w = synth.make_weights(synth.crop_config(cfg, 64, 64))
+    for k in (1, 2, 3):
+        assert w[f"mu.{k}.w"].shape == (cfg.c_y, 2 * cfg.c_y, 3, 3) and w[f"mu.{k}.b"].shape == (cfg.c_y,)
+        assert np.array_equal(synth.round_to_bf16(w[f"mu.{k}.w"]), w[f"mu.{k}.w"])      # bf16-representable
+    assert not any(k.startswith("mu.") for k in synth.make_weights(synth.crop_config(synth.CONFIGS[2], 64, 64)))
+    assert cfg.macs_per_chunk() - synth.CONFIGS[2].macs_per_chunk() == 3 * cfg.h * cfg.w * 9 * 2 * cfg.c_y * cfg.c_y
+    blob = binding.pack_weights_blob(w, cfg.weight_dtype)
+    assert b"mu.3.w" in blob

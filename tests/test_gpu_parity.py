@@ -23,6 +23,10 @@ CASES = {
     "cfg2-ragged": synth.crop_config(synth.CONFIGS[2], 150, 200),
     "cfg3-crop": synth.crop_config(synth.CONFIGS[3], 272, 480),
     "cfg2": synth.CONFIGS[2],
+    # four-step progressive means (NEXT-1, R21) on the same three small workloads
+    "cfg1-pmu": synth.progressive_config(synth.CONFIGS[1]),
+    "cfg2-ragged-pmu": synth.progressive_config(synth.crop_config(synth.CONFIGS[2], 150, 200)),
+    "cfg3-crop-pmu": synth.progressive_config(synth.crop_config(synth.CONFIGS[3], 272, 480)),
 }
 
 
@@ -47,7 +51,7 @@ def bf16_np(t):
     return t.float().cpu().numpy()
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg2-ragged", "cfg3-crop", "cfg2"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2-ragged", "cfg3-crop", "cfg2", "cfg1-pmu", "cfg2-ragged-pmu", "cfg3-crop-pmu"])
 def test_chunk_decode_matches_oracle(decoders, name):
     dec, case = decoders(name)
     cfg = case["cfg"]
@@ -72,7 +76,17 @@ def test_chunk_decode_matches_oracle(decoders, name):
         # A3 + A4: integer work is bit-exact
         assert np.array_equal(out["sym"][n].cpu().numpy(), nhwc(ref["sym"]))
         # yhat = r + mu: r is bit-exact, so yhat inherits mu's tolerance (R13); the tensor-core mean is good to ~3e-5
-        assert np.abs(out["yhat"][n].cpu().numpy() - nhwc(ref["yhat"])).max() <= 1e-4
+        d_y = np.abs(out["yhat"][n].cpu().numpy() - nhwc(ref["yhat"]))
+        if cfg.mu_steps == 4:
+            # progressive means come from bf16 tensor-core convs over [y so far ; mu0]: the north-star bound on mu
+            # applies (1e-2 relative, R13); partition 0 still carries the head's mean
+            assert (d_y <= 1e-2 * np.maximum(np.abs(mu_ref), 1.0)).all(), d_y.max()
+            import oracle
+            part0 = nhwc(oracle.partition_index(cfg.c_y, cfg.h, cfg.w)) == 0
+            assert d_y[part0].max() <= 1e-4
+            print(name, "progressive: max |d yhat| =", d_y.max(), " rms =", float(np.sqrt((d_y ** 2).mean())))
+        else:
+            assert d_y.max() <= 1e-4
         # A5 .. A8 intermediates: bf16 storage, loose stage-wise bounds relative to the tensor's scale
         taps = ref["taps"]
         for t in range(cfg.T):
@@ -285,4 +299,39 @@ def test_full_size_1080p_config3_matches_oracle():
     assert np.array_equal(out["sym"][0].cpu().numpy(), nhwc(ref["sym"]))          # 1,044,480 symbols bit-exact
     assert (out["idx"][0].cpu().numpy() != nhwc(ref["idx"])).mean() <= IDX_RATE
     assert res["max_abs"] <= PIX_TOL and res["psnr"] >= PSNR_MIN, res
+    dec.destroy()
+
+
+def test_full_size_progressive_means_match_oracle(orc):
+    """NEXT-1 at BASELINE.json configs[2]'s full latent size (128 x 68 x 120 = 1,044,480 elements), entropy stage only
+    (the oracle's O1-O5 plus the three mean convs take seconds; the synthesis is covered by the cropped -pmu cases):
+    symbols bit-exact, every mean and every y within the north-star bound."""
+    import oracle
+    from paper_2606_04410_b200 import binding
+    cfg = synth.progressive_config(synth.CONFIGS[3])
+    wts, z, u16 = synth.make_weights(cfg), synth.make_z(cfg), synth.make_uniform16(cfg)
+    st = oracle.make_stream(orc, cfg, wts, z[0], u16[0])
+    cdf = orc.build_cdf(cfg.n_buckets, cfg.scale_min, cfg.scale_max)
+    sym, status = oracle.decode_symbols(orc, cfg, cdf, st["idx"], st["bits"], st["sub_off"])
+    assert status == 0 and np.array_equal(sym, st["sym"])
+    yhat, mu = oracle.progressive_means(orc, cfg, wts, st["mu"], sym)
+    dec = binding.ChunkDecoder(cfg)
+    dec.load_weights(wts)
+    bits, off = binding.concat_streams([(st["bits"], st["sub_off"])])
+    dev = "cuda"
+    out = dec.chunk_decode_ex(torch.from_numpy(z).to(dev), torch.from_numpy(bits).to(dev),
+                              torch.from_numpy(off.astype(np.int64)).to(torch.int32).to(dev), taps=True, want_frames=False)
+    torch.cuda.synchronize()
+    assert dec.get_status() == 0
+    assert np.array_equal(out["sym"][0].cpu().numpy(), nhwc(sym))
+    mu_ref, y_ref = nhwc(mu), nhwc(yhat)
+    bound = 1e-2 * np.maximum(np.abs(mu_ref), 1.0)
+    d_mu = np.abs(out["mu"][0].cpu().numpy() - mu_ref)
+    d_y = np.abs(out["yhat"][0].cpu().numpy() - y_ref)
+    print("full-size progressive: max |d mu| =", d_mu.max(), " max |d y| =", d_y.max(), " rms =", float(np.sqrt((d_y ** 2).mean())))
+    assert (d_mu <= bound).all() and (d_y <= bound).all()
+    part = nhwc(oracle.partition_index(cfg.c_y, cfg.h, cfg.w))
+    for k in range(4):
+        assert (part == k).mean() == 0.25
+    assert d_mu[part == 0].max() <= 1e-4          # partition 0 keeps the head's mean
     dec.destroy()

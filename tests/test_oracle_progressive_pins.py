@@ -1,4 +1,4 @@
-"""Pins for the oracle's four-step progressive means (R17).
+"""Pins for the oracle's four-step progressive means (R21).
 
 The paper fixes the STRUCTURE (four partitions; the mean of partition k is estimated from the partitions decoded
 before it; the residual of every partition is already there; y = r + mu), not the geometry or the net, so the pins
@@ -33,7 +33,7 @@ def random_case(cfg, seed):
 
 
 def test_partition_table_by_hand():
-    """R17 for C_y = 4, one 2x2 cell: channel c is its own group, k = (2y + x + c) mod 4."""
+    """R21 for C_y = 4, one 2x2 cell: channel c is its own group, k = (2y + x + c) mod 4."""
     by_hand = np.array([[[0, 1], [2, 3]],      # c = 0
                         [[1, 2], [3, 0]],      # c = 1
                         [[2, 3], [0, 1]],      # c = 2
