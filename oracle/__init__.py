@@ -196,6 +196,76 @@ def decode_symbols(orc: Oracle, cfg, cdf, idx, bits, sub_off):
     return sym, status
 
 
+# ---------------------------------------------------------------------------------------------
+# NEXT-3: the hyper-latent's own entropy coding, so that a chunk is bytes only.  Reading R22.
+# ---------------------------------------------------------------------------------------------
+def z_geometry(cfg):
+    g = geometry(cfg)
+    return dict(h_z=g["h_z"], w_z=g["w_z"], n_sub_z=-(-g["h_z"] // cfg.rows_per_substream))
+
+
+def z_prior_index(orc: Oracle, cfg, weights):
+    """R22: z has a factorised prior (PAPER.md:125 names z only as "hyper-prior"; the prior's form is not in the
+    text): zero-mean Gaussian per channel with one learned ln sigma per channel (`zprior.lnscale` [C_z]), quantised
+    with the SAME bucket rule and the SAME tables as y (O2, O3).  Returns uint8 [C_z]."""
+    idx, _ = orc.bucket_index(np.asarray(weights["zprior.lnscale"], np.float64), cfg.n_buckets, cfg.scale_min, cfg.scale_max)
+    return idx
+
+
+def _z_stream_idx(cfg, idx_c, r0, r1, w_z):
+    return np.ascontiguousarray(np.broadcast_to(idx_c[None, None, :], (r1 - r0, w_z, idx_c.size))).ravel()
+
+
+def encode_z(orc: Oracle, cfg, cdf, weights, z):
+    """Fixture ENCODER for z [C_z][h_z][w_z] (mirror of decode_z): substreams of rows_per_substream rows of the
+    hyper-latent, stream order (row, col, channel) as for y [R9].  Returns (bytes, sub_off[n_sub_z + 1])."""
+    zg = z_geometry(cfg)
+    idx_c = z_prior_index(orc, cfg, weights)
+    parts, off = [], [0]
+    for s in range(zg["n_sub_z"]):
+        r0, r1 = s * cfg.rows_per_substream, min((s + 1) * cfg.rows_per_substream, zg["h_z"])
+        b = orc.rans_encode_substream(cdf, _z_stream_idx(cfg, idx_c, r0, r1, zg["w_z"]),
+                                      _stream_order(np.asarray(z, np.int16), r0, r1), cfg.lanes_per_substream)
+        parts.append(b)
+        off.append(off[-1] + b.size)
+    return np.concatenate(parts), np.asarray(off, np.uint32)
+
+
+def decode_z(orc: Oracle, cfg, cdf, weights, bits, sub_off):
+    """NEXT-3 / R22: the same arithmetic decoder as O4, the table of every symbol chosen by its CHANNEL alone.
+    Returns (z int16 [C_z][h_z][w_z], status)."""
+    zg = z_geometry(cfg)
+    idx_c = z_prior_index(orc, cfg, weights)
+    z = np.zeros((cfg.c_z, zg["h_z"], zg["w_z"]), np.int16)
+    status = 0
+    for s in range(zg["n_sub_z"]):
+        r0, r1 = s * cfg.rows_per_substream, min((s + 1) * cfg.rows_per_substream, zg["h_z"])
+        ss, st = orc.rans_decode_substream(cdf, _z_stream_idx(cfg, idx_c, r0, r1, zg["w_z"]), cfg.lanes_per_substream,
+                                           bits[int(sub_off[s]):int(sub_off[s + 1])])
+        z[:, r0:r1, :] = np.transpose(ss.reshape(r1 - r0, zg["w_z"], cfg.c_z), (2, 0, 1))
+        status = status or st
+    return z, status
+
+
+def pack_chunk_bytes(z_bits, z_off, y_bits, y_off):
+    """Container of one chunk for the bytes-only call: the z substreams, then the y substreams, one offset table."""
+    off = np.concatenate([np.asarray(z_off, np.int64), np.asarray(y_off, np.int64)[1:] + int(z_off[-1])])
+    return np.concatenate([z_bits, y_bits]), off.astype(np.uint32)
+
+
+def chunk_decode_bytes(orc: Oracle, cfg, weights, bits, sub_off, keep=False):
+    """One chunk from bytes only: decode z (NEXT-3), then O1..O9 on the rest of the container."""
+    zg = z_geometry(cfg)
+    cdf = orc.build_cdf(cfg.n_buckets, cfg.scale_min, cfg.scale_max)
+    nz = zg["n_sub_z"]
+    z, st_z = decode_z(orc, cfg, cdf, weights, bits, sub_off[:nz + 1])
+    y0 = int(sub_off[nz])
+    out = chunk_decode(orc, cfg, weights, z, bits[y0:], np.asarray(sub_off[nz:], np.int64) - y0, keep=keep)
+    out["z"] = z
+    out["status"] = out["status"] or st_z
+    return out
+
+
 def partition_index(c_y, h, w):
     """NEXT-1, reading R21 (Fig. 4a, "a quadtree-like partition [36] for y_i is adopted"; PAPER.md:101
     "the quantized latent y_i is divided into four partitions, where each partition's decoding depends on previously

@@ -186,6 +186,9 @@ def make_weights(cfg: ChunkConfig) -> dict:
     out[name + ".w"] = round_to_bf16(w) if cfg.weight_dtype == 1 else w
     out[name + ".b"] = b.astype(np.float32)
 
+    # factorised prior of the hyper-latent (NEXT-3, R22): one ln sigma per channel, around the law make_z draws from
+    rng = _rng(cfg, "zprior")
+    out["zprior.lnscale"] = (math.log(2.0) + rng.uniform(-0.3, 0.3, size=(cfg.c_z,))).astype(np.float32)
     # progressive means (NEXT-1, R21): three 3x3 convs [yhat so far ; mu0] (2 C_y) -> C_y.  Gain so that a mean keeps
     # the law of mu0: the input's second moment is ~ (E[yhat^2] * k/4 + E[mu0^2]) / 2 per channel at step k.
     if cfg.mu_steps == 4:
