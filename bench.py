@@ -190,6 +190,27 @@ def run_ours(args):
         for _ in range(5):
             flush.zero_()
             detail_us.append(dec.chunk_decode_profiled(z, bits, off, frames, stream=stream, detail=True))
+    # ---- NEXT-3 (R22): the same chunks from BYTES ONLY (z entropy-decoded on the device first), 10 extra steps ----
+    zparts = [dec.encode_z(z_host[c]) for c in range(n)]
+    all_bits, all_off = binding.concat_streams([binding.pack_chunk_bytes(zb, zo, pb, po) for (zb, zo), (pb, po) in zip(zparts, parts)])
+    ab, ao = torch.from_numpy(all_bits).to(dev), torch.from_numpy(all_off.astype(np.int64).astype(np.int32)).to(dev)
+    bytes_ms = []
+    with torch.cuda.stream(stream):
+        dec.chunk_decode_bytes(ab, ao, n_chunks=n, frames=frames, stream=stream)
+        stream.synchronize()
+        assert dec.get_status() == 0, "bit-stream status (bytes-only call)"
+        bytes_launches = dec.launches_per_call(n)
+        for _ in range(10):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            dec.chunk_decode_bytes(ab, ao, n_chunks=n, frames=frames, stream=stream)
+            e1.record(stream)
+            e1.synchronize()
+            bytes_ms.append(e0.elapsed_time(e1))
+    bytes_in = dict(value=n * cfg.T / (statistics.mean(bytes_ms) / 1e3), unit="frames/s (this rank)", ms_per_step=statistics.mean(bytes_ms),
+                    steps=10, z_stream_bytes=int(sum(int(zo[-1]) for _, zo in zparts)), y_stream_bytes=int(sum(int(po[-1]) for _, po in parts)),
+                    launches_per_call=bytes_launches, call="ufnvc_chunk_decode_bytes")
     total_ms = replicas.max_over_ranks(total_ms, dev)
     frames_per_step = n * cfg.T
     value = world * frames_per_step * args.steps / (total_ms / 1e3)
@@ -286,7 +307,7 @@ def run_ours(args):
                 clocks=clocks.summary(i0, i1), gpu_launches=dec.launches_per_call(n) * args.steps,
                 e2e=dict(value=e2e_val, unit="frames/s", h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, steps=e2e_steps,
                          overlap="D2H of step i on a copy stream overlaps the decode of step i+1 (two buffer sets)"),
-                roofline=roofline,
+                roofline=roofline, bytes_in=bytes_in,
                 cpu_baseline=dict(value=fps_cpu, unit="frames/s", cores=cores, kind="oracle", sample=desc),
                 wall_s_timed_region=t_wall)
     print(json.dumps(line))

@@ -98,7 +98,8 @@ int ufnvc_destroy(ufnvc_handle *h);
  *   data.
  * Tensors (canonical [C_out][C_in][kh][kw], biases fp32 [C_out]): hyper.{0,1,2}.{w,b}, xframe.{w,b},
  * trunk.{k}.{dw,pw1,pw2}.{w,b}, dec.{t}.{s}.{w,b} (t < T, s < 4), and with mu_steps == 4 mu.{1,2,3}.{w,b}
- * ([c_y][2 c_y][3][3]: input channels [0, c_y) = y decoded so far, [c_y, 2 c_y) = the head's mean).
+ * ([c_y][2 c_y][3][3]: input channels [0, c_y) = y decoded so far, [c_y, 2 c_y) = the head's mean); optional
+ * zprior.lnscale (fp32 [c_z], see the bytes-only entry points).
  * Missing / mis-shaped tensor: UFNVC_E_BAD_BLOB. */
 int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t bytes);
 
@@ -110,6 +111,22 @@ int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t bytes);
  * Bit-stream corruption never faults: reads are clamped and a status word is set (ufnvc_get_status). */
 int ufnvc_chunk_decode(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, const uint8_t *bits_dev,
                        size_t bits_bytes, const uint32_t *sub_off_dev, float *frames_dev, void *cuda_stream);
+
+/* ---- bytes-only entry points (R22).  The hyper-latent z has a factorised prior: a
+ * zero-mean Gaussian per channel with ln sigma = zprior.lnscale[c] (fp32 [c_z], optional blob tensor), bucketed by the
+ * rule of O2 onto the SAME tables as y; it is rANS-coded like y: n_sub_z = ceil(h_z / rows_per_substream) substreams
+ * of rows_per_substream rows, stream order (row, col, channel), lanes_per_substream lanes.
+ * Without zprior.lnscale in the blob these calls return UFNVC_E_NO_WEIGHTS. ---- */
+
+/* z only: sub_off_dev uint32 [n_chunks * n_sub_z + 1]; z_dev int16 [n_chunks][c_z][h_z][w_z] (output). */
+int ufnvc_decode_z(ufnvc_handle *h, int n_chunks, const uint8_t *bits_dev, size_t bits_bytes, const uint32_t *sub_off_dev,
+                   int16_t *z_dev, void *cuda_stream);
+
+/* One call from bytes to frames: per chunk the container holds the n_sub_z substreams of z, then the n_sub substreams
+ * of r; sub_off_dev uint32 [n_chunks * (n_sub_z + n_sub) + 1].  Two more launches than ufnvc_chunk_decode (the z rANS
+ * decode and a layout change); the status word ORs both decodes. */
+int ufnvc_chunk_decode_bytes(ufnvc_handle *h, int n_chunks, const uint8_t *bits_dev, size_t bits_bytes,
+                             const uint32_t *sub_off_dev, float *frames_dev, void *cuda_stream);
 
 /* Same, with parity hooks: idx_override_dev / mu_override_dev ([n][h][w][c_y], may be NULL) replace the
  * hyper-decoder's indices / means ("teacher forcing", R12; the entropy-only mode of DESIGN.md);
@@ -162,6 +179,13 @@ int ufnvc_symbols_from_uniform(const ufnvc_handle *h, const uint8_t *idx_host, c
  * Returns the byte count (> 0) or a negative status (UFNVC_E_INVALID_ARG if cap is too small). */
 long ufnvc_encode_chunk(const ufnvc_handle *h, const uint8_t *idx_host, const int16_t *sym_host, uint8_t *bits_host,
                         size_t cap, uint32_t *sub_off_host);
+
+/* Bucket index of every channel's z prior, uint8 [c_z] (R22). */
+int ufnvc_get_z_prior_index(const ufnvc_handle *h, uint8_t *idx_host);
+
+/* rANS-encode the hyper-latent of one chunk (mirror of ufnvc_decode_z).  z_host int16 [c_z][h_z][w_z]; writes the
+ * substreams to bits_host and n_sub_z + 1 offsets to sub_off_host; returns the byte count or a negative status. */
+long ufnvc_encode_z(const ufnvc_handle *h, const int16_t *z_host, uint8_t *bits_host, size_t cap, uint32_t *sub_off_host);
 
 #ifdef __cplusplus
 }

@@ -56,6 +56,10 @@ def _load():
         "ufnvc_get_cdf": (i, [vp, vp]),
         "ufnvc_symbols_from_uniform": (i, [vp, vp, vp, sz, vp]),
         "ufnvc_encode_chunk": (C.c_long, [vp, vp, vp, vp, sz, vp]),
+        "ufnvc_decode_z": (i, [vp, i, vp, sz, vp, vp, vp]),
+        "ufnvc_chunk_decode_bytes": (i, [vp, i, vp, sz, vp, vp, vp]),
+        "ufnvc_get_z_prior_index": (i, [vp, vp]),
+        "ufnvc_encode_z": (C.c_long, [vp, vp, vp, sz, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -66,7 +70,8 @@ def _load():
 LIB = _load()
 EXPORTS = ("ufnvc_create", "ufnvc_destroy", "ufnvc_load_weights", "ufnvc_chunk_decode", "ufnvc_chunk_decode_ex",
            "ufnvc_entropy_params", "ufnvc_get_status", "ufnvc_last_error", "ufnvc_launches_per_call",
-           "ufnvc_chunk_decode_profiled", "ufnvc_debug_counter", "ufnvc_get_cdf", "ufnvc_symbols_from_uniform", "ufnvc_encode_chunk")
+           "ufnvc_chunk_decode_profiled", "ufnvc_debug_counter", "ufnvc_get_cdf", "ufnvc_symbols_from_uniform", "ufnvc_encode_chunk",
+           "ufnvc_decode_z", "ufnvc_chunk_decode_bytes", "ufnvc_get_z_prior_index", "ufnvc_encode_z")
 
 
 def make_config(cfg, max_chunks: int | None = None) -> ufnvc_config:
@@ -133,6 +138,7 @@ class ChunkDecoder:
         self.h, self.w = self.H // 16, self.W // 16
         self.h_z, self.w_z = -(-self.h // 4), -(-self.w // 4)
         self.n_sub = -(-self.h // cfg.rows_per_substream)
+        self.n_sub_z = -(-self.h_z // cfg.rows_per_substream)
         hp = C.c_void_p()
         rc = LIB.ufnvc_create(C.byref(self.c), C.byref(hp))
         if rc != 0:
@@ -205,6 +211,34 @@ class ChunkDecoder:
         out["frames"] = frames
         return out
 
+    # ---- bytes-only entry points (NEXT-3, R22) ----
+    def decode_z(self, bits, sub_off, n_chunks=1, stream=None):
+        z = torch.empty((n_chunks, self.cfg.c_z, self.h_z, self.w_z), dtype=torch.int16, device=self.device)
+        self._check(LIB.ufnvc_decode_z(self.handle, n_chunks, _ptr(bits), bits.numel(), _ptr(sub_off), _ptr(z), self._stream(stream)),
+                    "ufnvc_decode_z")
+        return z
+
+    def chunk_decode_bytes(self, bits, sub_off, n_chunks=1, frames=None, stream=None):
+        frames = frames if frames is not None else self.new_frames(n_chunks)
+        self._check(LIB.ufnvc_chunk_decode_bytes(self.handle, n_chunks, _ptr(bits), bits.numel(), _ptr(sub_off), _ptr(frames),
+                                                 self._stream(stream)), "ufnvc_chunk_decode_bytes")
+        return frames
+
+    def get_z_prior_index(self) -> np.ndarray:
+        idx = np.empty(self.cfg.c_z, np.uint8)
+        self._check(LIB.ufnvc_get_z_prior_index(self.handle, _ptr(idx)), "ufnvc_get_z_prior_index")
+        return idx
+
+    def encode_z(self, z: np.ndarray):
+        """z: int16 [c_z][h_z][w_z] host array of ONE chunk -> (bytes uint8, sub_off uint32 [n_sub_z+1])."""
+        z = np.ascontiguousarray(z, np.int16)
+        G = self.cfg.lanes_per_substream // 32
+        cap = 2 * z.size + self.n_sub_z * (G * 140 + 16) + 64
+        bits = np.zeros(cap, np.uint8)
+        off = np.zeros(self.n_sub_z + 1, np.uint32)
+        n = self._check(LIB.ufnvc_encode_z(self.handle, _ptr(z), _ptr(bits), cap, _ptr(off)), "ufnvc_encode_z")
+        return bits[:n].copy(), off
+
     def entropy_params(self, z, stream=None):
         n = z.shape[0]
         e = (n, self.h, self.w, self.cfg.c_y)
@@ -258,6 +292,12 @@ class ChunkDecoder:
         off = np.zeros(self.n_sub + 1, np.uint32)
         n = self._check(LIB.ufnvc_encode_chunk(self.handle, _ptr(idx), _ptr(sym), _ptr(bits), cap, _ptr(off)), "ufnvc_encode_chunk")
         return bits[:n].copy(), off
+
+
+def pack_chunk_bytes(z_bits, z_off, y_bits, y_off):
+    """One chunk's container for ufnvc_chunk_decode_bytes: z substreams, then y substreams, one offset table."""
+    off = np.concatenate([np.asarray(z_off, np.int64), np.asarray(y_off, np.int64)[1:] + int(z_off[-1])])
+    return np.concatenate([z_bits, y_bits]), off.astype(np.uint32)
 
 
 def concat_streams(parts):

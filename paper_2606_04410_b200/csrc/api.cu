@@ -75,6 +75,7 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     h->h_z = (h->h + 3) / 4;
     h->w_z = (h->w + 3) / 4;
     h->n_sub = (h->h + cfg->rows_per_substream - 1) / cfg->rows_per_substream;
+    h->n_sub_z = (h->h_z + cfg->rows_per_substream - 1) / cfg->rows_per_substream;
     h->max_chunks = cfg->max_chunks_per_call;
     const char *fg = std::getenv("UFNVC_FORCE_GENERIC");
     h->force_generic = fg && fg[0] == '1';
@@ -115,6 +116,9 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
         ok = dev_alloc(h, h->ymu[0], n * P * cs) && dev_alloc(h, h->ymu[1], n * P * cs) && dev_alloc(h, h->sym, n * P * cfg->c_y) &&
              cudaMemset(h->ymu[0], 0, n * P * cs * 2) == cudaSuccess && cudaMemset(h->ymu[1], 0, n * P * cs * 2) == cudaSuccess;
     }
+    ok = ok && dev_alloc(h, h->z_idx, n * Pz * cfg->c_z) && dev_alloc(h, h->z_zero_mu, n * Pz * cfg->c_z) &&
+         dev_alloc(h, h->z_scratch, n * Pz * cfg->c_z) && dev_alloc(h, h->z_hwc, n * Pz * cfg->c_z) &&
+         dev_alloc(h, h->z_planar, n * Pz * cfg->c_z) && cudaMemset(h->z_zero_mu, 0, n * Pz * cfg->c_z * 4) == cudaSuccess;
     for (int s = 0; ok && s < 3; ++s) ok = dev_alloc(h, h->stage[s], n * T * (P << (2 * (s + 1))) * cfg->dec_channels[s + 1]);
     if (ok) ok = cudaMemcpy(h->d_cf, cf.data(), cf.size() * 4, cudaMemcpyHostToDevice) == cudaSuccess &&
                  cudaMemcpy(h->d_lut, lut.data(), lut.size() * 2, cudaMemcpyHostToDevice) == cudaSuccess &&
@@ -182,6 +186,41 @@ extern "C" int ufnvc_symbols_from_uniform(const ufnvc_handle *h, const uint8_t *
         sym_host[i] = int16_t(lo - 127);
     }
     return UFNVC_OK;
+}
+
+extern "C" int ufnvc_get_z_prior_index(const ufnvc_handle *h, uint8_t *idx_host)
+{
+    if (!h || !idx_host) return UFNVC_E_INVALID_ARG;
+    if (!h->z_prior_loaded) return UFNVC_E_NO_WEIGHTS;
+    std::memcpy(idx_host, h->z_idx_c.data(), h->z_idx_c.size());
+    return UFNVC_OK;
+}
+
+extern "C" long ufnvc_encode_z(const ufnvc_handle *h, const int16_t *z_host, uint8_t *bits_host, size_t cap, uint32_t *sub_off_host)
+{
+    if (!h || !z_host || !bits_host || !sub_off_host) return UFNVC_E_INVALID_ARG;
+    if (!h->z_prior_loaded) return UFNVC_E_NO_WEIGHTS;
+    const int cz = h->cfg.c_z, pz = h->h_z * h->w_z;
+    std::vector<uint8_t> idx(size_t(pz) * cz);
+    std::vector<int16_t> sym(size_t(pz) * cz);
+    for (int p = 0; p < pz; ++p)
+        for (int c = 0; c < cz; ++c) {                    // planar [c_z][pz] -> stream order (row, col, channel)
+            idx[size_t(p) * cz + c] = h->z_idx_c[c];
+            sym[size_t(p) * cz + c] = z_host[size_t(c) * pz + p];
+        }
+    size_t pos = 0;
+    sub_off_host[0] = 0;
+    for (int s = 0; s < h->n_sub_z; ++s) {
+        const int r0 = s * h->cfg.rows_per_substream;
+        const int rows = std::min(h->cfg.rows_per_substream, h->h_z - r0);
+        const size_t e0 = size_t(r0) * h->w_z * cz, cnt = size_t(rows) * h->w_z * cz;
+        const long nb = encode_substream(h->cdf32.data(), idx.data() + e0, sym.data() + e0, cnt, h->cfg.lanes_per_substream,
+                                         bits_host + pos, cap - pos);
+        if (nb < 0) return nb;
+        pos += size_t(nb);
+        sub_off_host[s + 1] = uint32_t(pos);
+    }
+    return long(pos);
 }
 
 extern "C" long ufnvc_encode_chunk(const ufnvc_handle *h, const uint8_t *idx_host, const int16_t *sym_host, uint8_t *bits_host,

@@ -94,9 +94,10 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     mark(sg, st);
 
     // ---- A3 + A4: rANS decode + dequantisation ----
-    CU_TRY(cudaMemsetAsync(h->d_status, 0, 4, st));
+    if (!h->keep_status) CU_TRY(cudaMemsetAsync(h->d_status, 0, 4, st));
     RansParams rp{};
     rp.bits = bits; rp.bits_bytes = bits_bytes; rp.sub_off = sub_off; rp.idx = idx; rp.mu = mu;
+    rp.sub_stride = h->y_sub_stride > 0 ? h->y_sub_stride : h->n_sub; rp.sub_first = h->y_sub_stride > 0 ? h->n_sub_z : 0;
     rp.cf = h->d_cf; rp.lut = h->d_lut;
     rp.n_chunks = n; rp.n_sub = h->n_sub; rp.h = h->h; rp.w = h->w; rp.c_y = c.c_y;
     rp.rows_per_sub = c.rows_per_substream; rp.W = c.lanes_per_substream; rp.n_buckets = c.n_buckets;
@@ -305,6 +306,63 @@ extern "C" int ufnvc_chunk_decode(ufnvc_handle *h, int n_chunks, const int16_t *
     if (!frames_dev) return fail(h, UFNVC_E_INVALID_ARG, "frames_dev is null");
     return run(h, n_chunks, z_dev, bits_dev, bits_bytes, sub_off_dev, frames_dev, static_cast<cudaStream_t>(cuda_stream), nullptr,
                nullptr, nullptr, false, nullptr, nullptr, nullptr, nullptr, nullptr);
+}
+
+// ---- NEXT-3 (R22): the hyper-latent from bytes ------------------------------------------------------------------
+namespace {
+int decode_z_impl(ufnvc_handle *h, int n, const uint8_t *bits, size_t bits_bytes, const uint32_t *sub_off, int sub_stride,
+                  int16_t *z_planar_out, cudaStream_t st, int *launches)
+{
+    const ufnvc_config &c = h->cfg;
+    if (!h->z_prior_loaded) return fail(h, UFNVC_E_NO_WEIGHTS, "the weights blob holds no zprior.lnscale tensor");
+    CU_TRY(cudaMemsetAsync(h->d_status, 0, 4, st));
+    RansParams rp{};
+    rp.bits = bits; rp.bits_bytes = bits_bytes; rp.sub_off = sub_off; rp.sub_stride = sub_stride; rp.sub_first = 0;
+    rp.idx = h->z_idx; rp.mu = h->z_zero_mu; rp.cf = h->d_cf; rp.lut = h->d_lut;
+    rp.n_chunks = n; rp.n_sub = h->n_sub_z; rp.h = h->h_z; rp.w = h->w_z; rp.c_y = c.c_z;
+    rp.rows_per_sub = c.rows_per_substream; rp.W = c.lanes_per_substream; rp.n_buckets = c.n_buckets;
+    rp.yhat = h->z_scratch; rp.sym_tap = h->z_hwc; rp.yhat_tap = nullptr; rp.status = h->d_status;
+    CU_TRY(launch_rans_decode(rp, st));
+    CU_TRY(launch_z_hwc_to_planar(h->z_hwc, z_planar_out, n, c.c_z, h->h_z * h->w_z, st));
+    if (launches) *launches += 2;
+    return UFNVC_OK;
+}
+}  // namespace
+
+extern "C" int ufnvc_decode_z(ufnvc_handle *h, int n_chunks, const uint8_t *bits_dev, size_t bits_bytes, const uint32_t *sub_off_dev,
+                              int16_t *z_dev, void *cuda_stream)
+{
+    if (!h) return UFNVC_E_INVALID_ARG;
+    if (!h->weights_loaded) return fail(h, UFNVC_E_NO_WEIGHTS, "ufnvc_load_weights has not succeeded on this handle");
+    if (n_chunks < 1 || n_chunks > h->max_chunks) return fail(h, UFNVC_E_INVALID_ARG, "n_chunks outside [1, max_chunks_per_call]");
+    if (!bits_dev || !sub_off_dev || !z_dev) return fail(h, UFNVC_E_INVALID_ARG, "null device pointer");
+    if (reinterpret_cast<uintptr_t>(bits_dev) & 3) return fail(h, UFNVC_E_INVALID_ARG, "bits_dev must be 4-byte aligned");
+    int launches = 0;
+    const int rc = decode_z_impl(h, n_chunks, bits_dev, bits_bytes, sub_off_dev, h->n_sub_z, z_dev, static_cast<cudaStream_t>(cuda_stream),
+                                 &launches);
+    h->last_launches = launches;
+    return rc;
+}
+
+extern "C" int ufnvc_chunk_decode_bytes(ufnvc_handle *h, int n_chunks, const uint8_t *bits_dev, size_t bits_bytes,
+                                        const uint32_t *sub_off_dev, float *frames_dev, void *cuda_stream)
+{
+    if (!h) return UFNVC_E_INVALID_ARG;
+    if (!h->weights_loaded) return fail(h, UFNVC_E_NO_WEIGHTS, "ufnvc_load_weights has not succeeded on this handle");
+    if (n_chunks < 1 || n_chunks > h->max_chunks) return fail(h, UFNVC_E_INVALID_ARG, "n_chunks outside [1, max_chunks_per_call]");
+    if (!bits_dev || !sub_off_dev || !frames_dev) return fail(h, UFNVC_E_INVALID_ARG, "null device pointer");
+    if (reinterpret_cast<uintptr_t>(bits_dev) & 3) return fail(h, UFNVC_E_INVALID_ARG, "bits_dev must be 4-byte aligned");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int launches = 0;
+    if (int rc = decode_z_impl(h, n_chunks, bits_dev, bits_bytes, sub_off_dev, h->n_sub_z + h->n_sub, h->z_planar, st, &launches)) return rc;
+    // the y decode ORs into the same status word: keep the z stage's bits by skipping run()'s reset
+    h->y_sub_stride = h->n_sub_z + h->n_sub;
+    h->keep_status = true;
+    const int rc = run(h, n_chunks, h->z_planar, bits_dev, bits_bytes, sub_off_dev, frames_dev, st, nullptr, nullptr, nullptr, false,
+                       nullptr, nullptr, nullptr, nullptr, &launches);
+    h->y_sub_stride = 0;
+    h->keep_status = false;
+    return rc;
 }
 
 extern "C" int ufnvc_entropy_params(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, float *mu_dev, float *lnscale_dev,

@@ -54,6 +54,16 @@ struct ufnvc_handle {
     ufnvc::bf16 *stage[3] = {nullptr, nullptr, nullptr};
     ufnvc::bf16 *ymu[2] = {nullptr, nullptr};   // mu_steps == 4: [n][h][w][2 c_y] = y decoded so far | mu0, ping-pong
     int16_t *sym = nullptr;                     // mu_steps == 4: decoded residual r, [n][h][w][c_y]
+    // NEXT-3 (R22): the hyper-latent's own entropy decode (bytes-only entry points)
+    int n_sub_z = 0;
+    int y_sub_stride = 0;                       // > 0 while a bytes-only call runs: offset-table entries per chunk
+    bool keep_status = false;                   // bytes-only call: the y decode must not clear the z decode's status bits
+    bool z_prior_loaded = false;
+    std::vector<uint8_t> z_idx_c;               // [c_z] bucket index of each channel's prior (host copy)
+    uint8_t *z_idx = nullptr;                   // [n][h_z][w_z][c_z]: z_idx_c broadcast, what the rANS kernel reads
+    float *z_zero_mu = nullptr;                 // [n][h_z][w_z][c_z] zeros (the prior is zero-mean)
+    ufnvc::bf16 *z_scratch = nullptr;           // the kernel's bf16 "y" output, unused for z
+    int16_t *z_hwc = nullptr, *z_planar = nullptr;
 
     // TMA descriptors of the activation tensors the tcgen05 convs read, built once at create (workspace is fixed)
     struct ActMap {

@@ -38,7 +38,8 @@ __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
     const int n_steps = (n + p.W - 1) / p.W;
 
     // ---- container parsing, every read clamped to the substream ----
-    const uint32_t so = p.sub_off[sub], se = p.sub_off[sub + 1];
+    const int so_i = chunk * p.sub_stride + p.sub_first + s;
+    const uint32_t so = p.sub_off[so_i], se = p.sub_off[so_i + 1];
     uint32_t st = 0;
     uint32_t sub_bytes = 0;
     if (se < so || (size_t)se > p.bits_bytes || (so & 3)) st |= UFNVC_STREAM_BAD_HEADER; else sub_bytes = se - so;
@@ -128,6 +129,26 @@ __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
     if (__any_sync(0xFFFFFFFFu, x != (1u << 16))) st |= UFNVC_STREAM_BAD_END_STATE;
     if (q != nw) st |= UFNVC_STREAM_BAD_WORD_COUNT;
     if (st && lane == 0) atomicOr(p.status, st);
+}
+
+__global__ void z_hwc_to_planar_kernel(const int16_t *__restrict__ in, int16_t *__restrict__ out, int n_chunks, int c_z, int pz)
+{
+    const long long total = (long long)n_chunks * c_z * pz;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const int p = int(i % pz);                                   // out index: ((n * c_z) + c) * pz + p
+        const long long r = i / pz;
+        const int c = int(r % c_z);
+        const int n = int(r / c_z);
+        out[i] = in[((long long)n * pz + p) * c_z + c];
+    }
+}
+
+cudaError_t launch_z_hwc_to_planar(const int16_t *z_hwc, int16_t *z_planar, int n_chunks, int c_z, int pz, cudaStream_t st)
+{
+    const long long total = (long long)n_chunks * c_z * pz;
+    const int blocks = int((total + 255) / 256 < 1184 ? (total + 255) / 256 : 1184);
+    z_hwc_to_planar_kernel<<<blocks, 256, 0, st>>>(z_hwc, z_planar, n_chunks, c_z, pz);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_rans_decode(const RansParams &p, cudaStream_t st)

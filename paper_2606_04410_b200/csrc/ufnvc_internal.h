@@ -110,7 +110,8 @@ cudaError_t launch_hyper_head(const HyperLayer &L, const double *in, int n_img, 
 struct RansParams {
     const uint8_t *bits;
     size_t bits_bytes;
-    const uint32_t *sub_off;  // [n_chunks*n_sub + 1]
+    const uint32_t *sub_off;  // substream s of chunk c: entries [c * sub_stride + sub_first + s] and the next one
+    int sub_stride, sub_first;   // (n_sub, 0) for the y-only container; (n_sub_z + n_sub, 0 | n_sub_z) for the bytes-only one
     const uint8_t *idx;       // [n][h][w][c_y]
     const float *mu;
     const uint32_t *cf;       // [nb][256]: c[pos] | freq[pos] << 16
@@ -122,6 +123,8 @@ struct RansParams {
     uint32_t *status;         // device word, OR-ed
 };
 cudaError_t launch_rans_decode(const RansParams &p, cudaStream_t st);
+// NEXT-3 (R22): decoded hyper-latent, channels-last int16 [n][pz][c_z] -> the planar [n][c_z][pz] layout of z_dev
+cudaError_t launch_z_hwc_to_planar(const int16_t *z_hwc, int16_t *z_planar, int n_chunks, int c_z, int pz, cudaStream_t st);
 
 // tcgen05 implicit-GEMM conv (conv_tc.cu)
 cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_in, int tile_h, int tile_w,

@@ -1,4 +1,5 @@
 // ufnvc_load_weights: parse the blob (include/ufnvc.h), convert / permute / pad, upload.
+#include <cmath>
 #include <cstring>
 
 #include "handle.h"
@@ -213,6 +214,26 @@ int load_weights_impl(ufnvc_handle *h, const void *blob, size_t bytes)
         ok = ld.conv(h->dec[s], names, c.dec_channels[s], 4 * c.dec_channels[s + 1], 3, true);
     }
     if (!ok) return fail(h, ld.err.find("cuda") == 0 ? UFNVC_E_CUDA : UFNVC_E_BAD_BLOB, ld.err);
+    // NEXT-3 (R22), optional: the factorised prior of z -- one ln sigma per channel, bucketed in double by the rule of
+    // O2 (hyper.cu), then broadcast to the [n][h_z][w_z][c_z] index map the rANS kernel reads.
+    h->z_prior_loaded = false;
+    if (ld.t.count("zprior.lnscale")) {
+        const Tensor *tz = ld.get("zprior.lnscale", {uint32_t(c.c_z)});
+        if (!tz || tz->dtype != 0) return fail(h, UFNVC_E_BAD_BLOB, "zprior.lnscale must be fp32 [c_z]");
+        const double lo = std::log(c.scale_min), hi = std::log(c.scale_max);
+        h->z_idx_c.resize(c.c_z);
+        for (int ch = 0; ch < c.c_z; ++ch) {
+            double u = double(tz->at(ch));
+            u = u < lo ? lo : (u > hi ? hi : u);
+            const int k = int(std::floor(double(c.n_buckets - 1) * (u - lo) / (hi - lo) + 0.5));
+            h->z_idx_c[ch] = uint8_t(k < 0 ? 0 : (k > c.n_buckets - 1 ? c.n_buckets - 1 : k));
+        }
+        const size_t cnt = size_t(h->max_chunks) * h->h_z * h->w_z * c.c_z;
+        std::vector<uint8_t> full(cnt);
+        for (size_t i = 0; i < cnt; ++i) full[i] = h->z_idx_c[i % c.c_z];
+        if (cudaMemcpy(h->z_idx, full.data(), cnt, cudaMemcpyHostToDevice) != cudaSuccess) return fail(h, UFNVC_E_CUDA, "cudaMemcpy(z_idx) failed");
+        h->z_prior_loaded = true;
+    }
     return UFNVC_OK;
 }
 

@@ -335,3 +335,73 @@ def test_full_size_progressive_means_match_oracle(orc):
         assert (part == k).mean() == 0.25
     assert d_mu[part == 0].max() <= 1e-4          # partition 0 keeps the head's mean
     dec.destroy()
+
+
+# ---- NEXT-3 (R22): the hyper-latent from bytes, and the bytes-only call ----------------------------------
+@pytest.mark.parametrize("name", ["cfg1", "cfg2-ragged", "cfg3-crop"])
+def test_decode_z_and_bytes_only_call(decoders, orc, name):
+    import oracle
+    from paper_2606_04410_b200 import binding
+    dec, case = decoders(name)
+    cfg, wts = case["cfg"], case["weights"]
+    cdf = orc.build_cdf(cfg.n_buckets, cfg.scale_min, cfg.scale_max)
+    assert np.array_equal(dec.get_z_prior_index(), oracle.z_prior_index(orc, cfg, wts))
+    parts_z, parts_all = [], []
+    for n, ch in enumerate(case["chunks"]):
+        zb, zo = oracle.encode_z(orc, cfg, cdf, wts, case["z"][n])
+        zb2, zo2 = dec.encode_z(case["z"][n])                         # the library's own fixture encoder: same bytes
+        assert np.array_equal(zb, zb2) and np.array_equal(zo, zo2)
+        parts_z.append((zb, zo))
+        parts_all.append(oracle.pack_chunk_bytes(zb, zo, ch["stream"]["bits"], ch["stream"]["sub_off"]))
+    dev = "cuda"
+
+    def up(a, dt=None):
+        t = torch.from_numpy(a.astype(np.int64) if dt is not None else a)
+        return (t.to(dt) if dt is not None else t).to(dev)
+    bits, off = binding.concat_streams(parts_z)
+    z = dec.decode_z(up(bits), up(off, torch.int32), n_chunks=cfg.n_chunks)
+    torch.cuda.synchronize()
+    assert dec.get_status() == 0
+    assert np.array_equal(z.cpu().numpy(), case["z"])                 # integer work: bit-exact
+    # bytes in, frames out == the z-in call on the same inputs, bit for bit
+    bits, off = binding.concat_streams(parts_all)
+    f_bytes = dec.chunk_decode_bytes(up(bits), up(off, torch.int32), n_chunks=cfg.n_chunks)
+    torch.cuda.synchronize()
+    assert dec.get_status() == 0
+    zi, bi, oi = gpu_inputs(case)
+    f_z = dec.chunk_decode(zi, bi, oi)
+    torch.cuda.synchronize()
+    assert torch.equal(f_bytes, f_z)
+    ref = case["chunks"][0]["out"]["frames"]
+    assert np.abs(f_bytes[0].cpu().numpy() - ref).max() <= PIX_TOL
+    # a flipped byte inside the z part, or inside the y part, is reported and never faults
+    for where in (int(off[1]) // 2, int(off[dec.n_sub_z]) + 200):
+        bad = bits.copy()
+        bad[where] ^= 0x77
+        dec.chunk_decode_bytes(up(bad), up(off, torch.int32), n_chunks=cfg.n_chunks)
+        torch.cuda.synchronize()
+        assert dec.get_status() != 0
+
+
+def test_decode_z_full_size_and_without_prior(orc):
+    """Config 3's hyper-latent at full size (64 x 17 x 30, 5 substreams, ragged last one); a blob without zprior.lnscale
+    keeps every other entry point working and makes the bytes-only ones fail loudly."""
+    import oracle
+    from paper_2606_04410_b200 import binding
+    cfg = synth.CONFIGS[3]
+    wts, z = synth.make_weights(cfg), synth.make_z(cfg)
+    cdf = orc.build_cdf(cfg.n_buckets, cfg.scale_min, cfg.scale_max)
+    zb, zo = oracle.encode_z(orc, cfg, cdf, wts, z[0])
+    dec = binding.ChunkDecoder(cfg)
+    dec.load_weights(wts)
+    assert dec.n_sub_z == 5 and zo.size == 6
+    got = dec.decode_z(torch.from_numpy(zb).cuda(), torch.from_numpy(zo.astype(np.int64)).to(torch.int32).cuda())
+    torch.cuda.synchronize()
+    assert dec.get_status() == 0 and np.array_equal(got.cpu().numpy(), z)
+    dec.load_weights({k: v for k, v in wts.items() if not k.startswith("zprior.")})
+    with pytest.raises(binding.UfnvcError):
+        dec.decode_z(torch.from_numpy(zb).cuda(), torch.from_numpy(zo.astype(np.int64)).to(torch.int32).cuda())
+    mu, ls, idx = dec.entropy_params(torch.from_numpy(z).cuda())       # the z-in path is untouched
+    torch.cuda.synchronize()
+    assert idx.shape == (1, cfg.h, cfg.w, cfg.c_y)
+    dec.destroy()
