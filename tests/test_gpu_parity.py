@@ -405,3 +405,51 @@ def test_decode_z_full_size_and_without_prior(orc):
     torch.cuda.synchronize()
     assert idx.shape == (1, cfg.h, cfg.w, cfg.c_y)
     dec.destroy()
+
+
+def test_multi_chunk_progressive_bytes_only_and_graph():
+    """The two widened paths together, on a two-chunk call (config 4's layer plan: C_y = 192, T = 16, 384 lanes, cropped):
+    mu_steps = 4 with the chunks handed over as bytes only; per-chunk parity against the oracle; the whole call captured
+    in a CUDA graph replays bit-identically."""
+    import dataclasses
+    import oracle
+    from paper_2606_04410_b200 import binding
+    cfg = synth.progressive_config(dataclasses.replace(synth.crop_config(synth.CONFIGS[4], 96, 160), n_chunks=2))
+    case = oracle_case(cfg)
+    orc = oracle.Oracle()
+    cdf = orc.build_cdf(cfg.n_buckets, cfg.scale_min, cfg.scale_max)
+    parts = []
+    for n, ch in enumerate(case["chunks"]):
+        zb, zo = oracle.encode_z(orc, cfg, cdf, case["weights"], case["z"][n])
+        parts.append(oracle.pack_chunk_bytes(zb, zo, ch["stream"]["bits"], ch["stream"]["sub_off"]))
+    bits_h, off_h = binding.concat_streams(parts)
+    bits = torch.from_numpy(bits_h).cuda()
+    off = torch.from_numpy(off_h.astype(np.int64)).to(torch.int32).cuda()
+    dec = binding.ChunkDecoder(cfg)
+    dec.load_weights(case["weights"])
+    ref = dec.chunk_decode_bytes(bits, off, n_chunks=2).clone()
+    torch.cuda.synchronize()
+    assert dec.get_status() == 0
+    for n, ch in enumerate(case["chunks"]):
+        f = ref[n].cpu().numpy()
+        assert np.abs(f - ch["out"]["frames"]).max() <= PIX_TOL and psnr(f, ch["out"]["frames"]) >= PSNR_MIN
+    zi, bi, oi = gpu_inputs(case)
+    out = dec.chunk_decode_ex(zi, bi, oi, taps=True)
+    torch.cuda.synchronize()
+    assert torch.equal(out["frames"], ref)
+    for n, ch in enumerate(case["chunks"]):
+        assert np.array_equal(out["sym"][n].cpu().numpy(), nhwc(ch["out"]["sym"]))
+        mu_ref = nhwc(ch["out"]["mu"])
+        assert (np.abs(out["mu"][n].cpu().numpy() - mu_ref) <= 1e-2 * np.maximum(np.abs(mu_ref), 1.0)).all()
+    frames = dec.new_frames(2)
+    s = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        g.capture_begin()
+        dec.chunk_decode_bytes(bits, off, n_chunks=2, frames=frames, stream=s)
+        g.capture_end()
+    frames.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert dec.get_status() == 0 and torch.equal(frames, ref)
+    dec.destroy()
