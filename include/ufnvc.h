@@ -180,6 +180,17 @@ int ufnvc_symbols_from_uniform(const ufnvc_handle *h, const uint8_t *idx_host, c
 long ufnvc_encode_chunk(const ufnvc_handle *h, const uint8_t *idx_host, const int16_t *sym_host, uint8_t *bits_host,
                         size_t cap, uint32_t *sub_off_host);
 
+/* GPU rANS ENCODE of r (the entropy-coding half of a chunk encoder; "the result r_i
+ * is arithmetically encoded using scale sigma_i").  Exact mirror of the decoder and byte-identical to
+ * ufnvc_encode_chunk / the oracle's encoder.  idx_dev uint8, sym_dev int16: [n_chunks][h][w][c_y] on the device;
+ * bits_dev (4-byte aligned, capacity cap bytes) receives the substreams of all chunks back to back and sub_off_dev
+ * uint32 [n_chunks * n_sub + 1] their byte offsets -- exactly what ufnvc_chunk_decode takes.  A symbol outside
+ * [-127, 127] or an index >= n_buckets sets UFNVC_STREAM_BAD_HEADER in the status word; cap too small sets
+ * UFNVC_STREAM_BAD_WORD_COUNT and writes offsets only (sub_off_dev[last] = bytes needed).  Asynchronous on cuda_stream;
+ * the first call allocates scratch. */
+int ufnvc_encode_chunk_dev(ufnvc_handle *h, int n_chunks, const uint8_t *idx_dev, const int16_t *sym_dev, uint8_t *bits_dev,
+                           size_t cap, uint32_t *sub_off_dev, void *cuda_stream);
+
 /* Bucket index of every channel's z prior, uint8 [c_z] (R22). */
 int ufnvc_get_z_prior_index(const ufnvc_handle *h, uint8_t *idx_host);
 

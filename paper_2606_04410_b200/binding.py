@@ -60,6 +60,7 @@ def _load():
         "ufnvc_chunk_decode_bytes": (i, [vp, i, vp, sz, vp, vp, vp]),
         "ufnvc_get_z_prior_index": (i, [vp, vp]),
         "ufnvc_encode_z": (C.c_long, [vp, vp, vp, sz, vp]),
+        "ufnvc_encode_chunk_dev": (i, [vp, i, vp, vp, vp, sz, vp, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -71,7 +72,7 @@ LIB = _load()
 EXPORTS = ("ufnvc_create", "ufnvc_destroy", "ufnvc_load_weights", "ufnvc_chunk_decode", "ufnvc_chunk_decode_ex",
            "ufnvc_entropy_params", "ufnvc_get_status", "ufnvc_last_error", "ufnvc_launches_per_call",
            "ufnvc_chunk_decode_profiled", "ufnvc_debug_counter", "ufnvc_get_cdf", "ufnvc_symbols_from_uniform", "ufnvc_encode_chunk",
-           "ufnvc_decode_z", "ufnvc_chunk_decode_bytes", "ufnvc_get_z_prior_index", "ufnvc_encode_z")
+           "ufnvc_decode_z", "ufnvc_chunk_decode_bytes", "ufnvc_get_z_prior_index", "ufnvc_encode_z", "ufnvc_encode_chunk_dev")
 
 
 def make_config(cfg, max_chunks: int | None = None) -> ufnvc_config:
@@ -238,6 +239,17 @@ class ChunkDecoder:
         off = np.zeros(self.n_sub_z + 1, np.uint32)
         n = self._check(LIB.ufnvc_encode_z(self.handle, _ptr(z), _ptr(bits), cap, _ptr(off)), "ufnvc_encode_z")
         return bits[:n].copy(), off
+
+    def encode_chunk_dev(self, idx, sym, cap=None, stream=None):
+        """GPU rANS encode (NEXT-4): idx uint8, sym int16 device tensors [n][h][w][c_y] -> (bits uint8 [cap], sub_off int32)."""
+        n = idx.shape[0]
+        G = self.cfg.lanes_per_substream // 32
+        cap = cap if cap is not None else n * (2 * idx[0].numel() + self.n_sub * (G * 140 + 16) + 64)
+        bits = torch.zeros(cap, dtype=torch.uint8, device=self.device)
+        off = torch.zeros(n * self.n_sub + 1, dtype=torch.int32, device=self.device)
+        self._check(LIB.ufnvc_encode_chunk_dev(self.handle, n, _ptr(idx), _ptr(sym), _ptr(bits), cap, _ptr(off), self._stream(stream)),
+                    "ufnvc_encode_chunk_dev")
+        return bits, off
 
     def entropy_params(self, z, stream=None):
         n = z.shape[0]

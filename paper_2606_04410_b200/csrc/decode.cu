@@ -365,6 +365,45 @@ extern "C" int ufnvc_chunk_decode_bytes(ufnvc_handle *h, int n_chunks, const uin
     return rc;
 }
 
+// ---- NEXT-4 (part): GPU rANS encode of r, the mirror of A3 ---------------------------------------------------------
+extern "C" int ufnvc_encode_chunk_dev(ufnvc_handle *h, int n_chunks, const uint8_t *idx_dev, const int16_t *sym_dev, uint8_t *bits_dev,
+                                      size_t cap, uint32_t *sub_off_dev, void *cuda_stream)
+{
+    if (!h) return UFNVC_E_INVALID_ARG;
+    if (n_chunks < 1 || n_chunks > h->max_chunks) return fail(h, UFNVC_E_INVALID_ARG, "n_chunks outside [1, max_chunks_per_call]");
+    if (!idx_dev || !sym_dev || !bits_dev || !sub_off_dev) return fail(h, UFNVC_E_INVALID_ARG, "null device pointer");
+    if (reinterpret_cast<uintptr_t>(bits_dev) & 3) return fail(h, UFNVC_E_INVALID_ARG, "bits_dev must be 4-byte aligned");
+    const ufnvc_config &c = h->cfg;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int G = c.lanes_per_substream / 32;
+    if (!h->enc_tmp) {
+        const size_t n_sym = size_t(c.rows_per_substream) * h->w * c.c_y;
+        const size_t steps = (n_sym + c.lanes_per_substream - 1) / c.lanes_per_substream;
+        h->enc_tmp_stride = steps * 32;
+        h->enc_stage_stride = (size_t(8) * G + size_t(G) * 132 + 2 * steps * c.lanes_per_substream + 31) / 16 * 16;
+        const size_t subs = size_t(h->max_chunks) * h->n_sub;
+        void *a = nullptr, *b = nullptr, *d = nullptr;
+        if (cudaMalloc(&a, subs * G * h->enc_tmp_stride * 2) != cudaSuccess || cudaMalloc(&b, subs * h->enc_stage_stride) != cudaSuccess ||
+            cudaMalloc(&d, subs * 4) != cudaSuccess) {
+            cudaFree(a); cudaFree(b); cudaFree(d);
+            cudaGetLastError();
+            return fail(h, UFNVC_E_OOM, "cudaMalloc failed (encoder scratch)");
+        }
+        h->allocs.push_back(a); h->allocs.push_back(b); h->allocs.push_back(d);
+        h->enc_tmp = static_cast<uint16_t *>(a); h->enc_stage = static_cast<uint8_t *>(b); h->enc_sizes = static_cast<uint32_t *>(d);
+    }
+    CU_TRY(cudaMemsetAsync(h->d_status, 0, 4, st));
+    RansEncParams p{};
+    p.idx = idx_dev; p.sym = sym_dev; p.cf = h->d_cf;
+    p.n_chunks = n_chunks; p.n_sub = h->n_sub; p.h = h->h; p.w = h->w; p.c_y = c.c_y;
+    p.rows_per_sub = c.rows_per_substream; p.W = c.lanes_per_substream; p.n_buckets = c.n_buckets;
+    p.tmp_words = h->enc_tmp; p.tmp_stride = h->enc_tmp_stride; p.stage = h->enc_stage; p.stage_stride = h->enc_stage_stride;
+    p.sizes = h->enc_sizes; p.bits_out = bits_dev; p.cap = cap; p.sub_off = sub_off_dev; p.status = h->d_status;
+    CU_TRY(launch_rans_encode(p, st));
+    h->last_launches = 2;
+    return UFNVC_OK;
+}
+
 extern "C" int ufnvc_entropy_params(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, float *mu_dev, float *lnscale_dev,
                                     uint8_t *idx_dev, void *cuda_stream)
 {

@@ -79,6 +79,12 @@ struct ufnvc_handle {
     bool dw_tma_ok = false;
     ActMap am_xs, am_yhat, am_fa, am_fb, am_hidden, am_stage[3], am_ymu[2];
 
+    // GPU rANS encoder scratch (NEXT-4), allocated by the first ufnvc_encode_chunk_dev call
+    uint16_t *enc_tmp = nullptr;
+    uint8_t *enc_stage = nullptr;
+    uint32_t *enc_sizes = nullptr;
+    size_t enc_tmp_stride = 0, enc_stage_stride = 0;
+
     std::vector<void *> allocs;          // everything cudaMalloc'ed, freed at destroy
     cudaEvent_t ev[8] = {};
     std::vector<cudaEvent_t> ev_dw;      // profiled call: before / after every depthwise launch

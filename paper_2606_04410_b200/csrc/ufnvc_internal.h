@@ -123,6 +123,24 @@ struct RansParams {
     uint32_t *status;         // device word, OR-ed
 };
 cudaError_t launch_rans_decode(const RansParams &p, cudaStream_t st);
+
+// GPU rANS encode (rans_encode.cu), mirror of the decoder: same geometry fields
+struct RansEncParams {
+    const uint8_t *idx;       // [n][h][w][c_y]
+    const int16_t *sym;       // [n][h][w][c_y]
+    const uint32_t *cf;       // [nb][256]: c[pos] | freq[pos] << 16
+    int n_chunks, n_sub, h, w, c_y, rows_per_sub, W, n_buckets;
+    uint16_t *tmp_words;      // scratch: [n*n_sub][W/32][tmp_stride] words in emission order
+    size_t tmp_stride;
+    uint8_t *stage;           // scratch: [n*n_sub][stage_stride] one finished substream each
+    size_t stage_stride;
+    uint32_t *sizes;          // [n*n_sub] bytes of each substream
+    uint8_t *bits_out;        // packed substreams (4-byte aligned), capacity cap
+    size_t cap;
+    uint32_t *sub_off;        // [n*n_sub + 1] byte offsets into bits_out
+    uint32_t *status;
+};
+cudaError_t launch_rans_encode(const RansEncParams &p, cudaStream_t st);
 // NEXT-3 (R22): decoded hyper-latent, channels-last int16 [n][pz][c_z] -> the planar [n][c_z][pz] layout of z_dev
 cudaError_t launch_z_hwc_to_planar(const int16_t *z_hwc, int16_t *z_planar, int n_chunks, int c_z, int pz, cudaStream_t st);
 

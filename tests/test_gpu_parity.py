@@ -453,3 +453,64 @@ def test_multi_chunk_progressive_bytes_only_and_graph():
     torch.cuda.synchronize()
     assert dec.get_status() == 0 and torch.equal(frames, ref)
     dec.destroy()
+
+
+# ---- NEXT-4 (part): GPU rANS encode, byte-identical to the oracle's encoder ----------------------------------------
+@pytest.mark.parametrize("name", ["cfg1", "cfg2-ragged", "cfg3-crop", "cfg2"])
+def test_gpu_rans_encode_is_byte_identical_to_oracle(decoders, name):
+    from paper_2606_04410_b200 import binding
+    dec, case = decoders(name)
+    cfg = case["cfg"]
+    idx = torch.from_numpy(np.stack([nhwc(ch["stream"]["idx"]) for ch in case["chunks"]])).cuda()
+    sym = torch.from_numpy(np.stack([nhwc(ch["stream"]["sym"]) for ch in case["chunks"]])).cuda()
+    bits, off = dec.encode_chunk_dev(idx, sym)
+    torch.cuda.synchronize()
+    assert dec.get_status() == 0
+    want_bits, want_off = binding.concat_streams([(c["stream"]["bits"], c["stream"]["sub_off"]) for c in case["chunks"]])
+    got_off = off.cpu().numpy().astype(np.uint32)
+    assert np.array_equal(got_off, want_off)
+    assert np.array_equal(bits.cpu().numpy()[:int(got_off[-1])], want_bits)
+    # and the library decodes its own stream back (device to device, no host in between)
+    zi, _, _ = gpu_inputs(case)
+    out = dec.chunk_decode_ex(zi, bits[:int(got_off[-1])], off, taps=True, want_frames=False)
+    torch.cuda.synchronize()
+    assert dec.get_status() == 0 and torch.equal(out["sym"], sym)
+    # error paths: a symbol outside the alphabet, and an output buffer that is too small
+    bad = sym.clone()
+    bad.view(-1)[5] = 200
+    dec.encode_chunk_dev(idx, bad)
+    torch.cuda.synchronize()
+    assert dec.get_status() != 0
+    _, off2 = dec.encode_chunk_dev(idx, sym, cap=64)
+    torch.cuda.synchronize()
+    assert dec.get_status() != 0 and int(off2[-1]) == int(got_off[-1])
+
+
+def test_gpu_rans_encode_full_size_1080p(orc):
+    """All 1,044,480 symbols of config 3 (17 substreams, 512 lanes): byte-identical to the oracle's encoder, exact-law
+    (mu, sigma) maps as in the entropy-only mode; timing printed."""
+    import oracle
+    from paper_2606_04410_b200 import binding
+    cfg = synth.CONFIGS[3]
+    _, u = synth.make_exact_law_params(cfg)
+    idx_chw, _ = orc.bucket_index(np.moveaxis(u[0], -1, 0), cfg.n_buckets, cfg.scale_min, cfg.scale_max)
+    cdf = orc.build_cdf(cfg.n_buckets, cfg.scale_min, cfg.scale_max)
+    u16 = synth.make_uniform16(cfg)[0]
+    sym_chw = orc.symbols_from_uniform(cdf, idx_chw, np.transpose(u16, (2, 0, 1)))
+    want_bits, want_off = oracle.encode_chunk(orc, cfg, cdf, idx_chw, sym_chw)
+    dec = binding.ChunkDecoder(cfg)
+    idx = torch.from_numpy(nhwc(idx_chw)[None]).cuda()
+    sym = torch.from_numpy(nhwc(sym_chw)[None]).cuda()
+    bits, off = dec.encode_chunk_dev(idx, sym)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(10):
+        bits, off = dec.encode_chunk_dev(idx, sym)
+    e1.record()
+    e1.synchronize()
+    assert dec.get_status() == 0
+    got_off = off.cpu().numpy().astype(np.uint32)
+    assert np.array_equal(got_off, want_off) and np.array_equal(bits.cpu().numpy()[:int(got_off[-1])], want_bits)
+    print("GPU rANS encode, 1080p chunk:", e0.elapsed_time(e1) / 10 * 1e3, "us incl. output allocation;", int(got_off[-1]), "bytes")
+    dec.destroy()
