@@ -124,6 +124,12 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
         }
         const int grp = group_of(p, img);
         const float *bias = p.bias + (long long)grp * p.n_pad + tc.nt * p.BN;
+        float bias_lane[4] = {0.f, 0.f, 0.f, 0.f};                   // EPI_HEAD: bias of column c0 + lane for this warp's chunks
+        if (MODE == EPI_HEAD) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (half * 32 + q * 64 < p.BN) bias_lane[q] = __ldg(bias + half * 32 + q * 64 + lane);
+        }
         mbar_wait(tfull0 + 8u * acc, acc_phase);
         tc_fence_after();
         const uint32_t t_row = tmem_base + (uint32_t(quad * 32) << 16) + uint32_t(acc * p.BN);
@@ -162,29 +168,43 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
             }
         } else if (MODE == EPI_HEAD) {
             // A2: pixel-shuffle x4 + crop + split.  A 32-column chunk is 32 consecutive latent channels of one sub-pixel.
+            // The map is tiny (one tile per CTA), so nothing overlaps this epilogue and its serial latencies are the
+            // cost: the biases are read BEFORE the accumulator is waited for (one per lane and chunk, handed round by
+            // shuffles), and the list-slot atomic of a chunk is consumed one chunk later.
+            const EpiParams &E = p.E;
+            uint32_t pend_fm = 0, pend_off = 0, pend_base = 0, pend_total = 0;
+            long long pend_e0 = 0;
+            auto flush_pending = [&]() {
+                if (pend_total) {                                               // warp-uniform
+                    uint32_t w = __shfl_sync(0xFFFFFFFFu, pend_base, 31) + pend_off;
+                    while (pend_fm) {
+                        const int j = __ffs(pend_fm) - 1;
+                        pend_fm &= pend_fm - 1;
+                        E.fix_list[w++] = uint32_t(pend_e0 + j);
+                    }
+                }
+                pend_total = 0;
+            };
             for (int c0 = half * 32; c0 < p.BN; c0 += 64) {
                 uint32_t v[32];
                 tmem_ld32(t_row + uint32_t(c0), v);
-                if (!inb) continue;
-                const EpiParams &E = p.E;
+                const float bl = bias_lane[c0 >> 6];
                 const int n = tc.nt * p.BN + c0;
                 const int sij = n / E.c_y, c2 = n - sij * E.c_y;
                 const int ly = 4 * y + ((sij >> 2) & 3), lx = 4 * x + (sij & 3);
-                if (ly >= E.lat_h || lx >= E.lat_w) continue;                      // crop [R2]
+                const bool live = inb && ly < E.lat_h && lx < E.lat_w;             // crop [R2]; dead lanes still join the scans
                 const long long e0 = (((long long)img * E.lat_h + ly) * E.lat_w + lx) * E.c_y + c2;
                 float f[32];
 #pragma unroll
-                for (int j = 0; j < 32; j += 4) {
-                    const float4 b4 = __ldg(reinterpret_cast<const float4 *>(bias + c0 + j));
-                    f[j] = __uint_as_float(v[j]) + b4.x; f[j + 1] = __uint_as_float(v[j + 1]) + b4.y;
-                    f[j + 2] = __uint_as_float(v[j + 2]) + b4.z; f[j + 3] = __uint_as_float(v[j + 3]) + b4.w;
-                }
-                if ((sij >> 4) == 0) {                                             // mean
-                    float4 *dst = reinterpret_cast<float4 *>(E.mu + e0);
+                for (int j = 0; j < 32; ++j) f[j] = __uint_as_float(v[j]) + __shfl_sync(0xFFFFFFFFu, bl, j);
+                if ((sij >> 4) == 0) {                                             // mean (n is warp-uniform)
+                    if (live) {
 #pragma unroll
-                    for (int q = 0; q < 8; ++q) dst[q] = make_float4(f[4 * q], f[4 * q + 1], f[4 * q + 2], f[4 * q + 3]);
+                        for (int q = 0; q < 4; ++q) st_global_256(E.mu + e0 + 8 * q, f + 8 * q);
+                    }
                 } else {                                                           // ln sigma -> bucket, edge flag
                     uint32_t packed[8];
+                    uint32_t fm = 0;                                               // bit j: element j is decided by hyper_fix_kernel
 #pragma unroll
                     for (int j = 0; j < 32; ++j) {
                         const float u = fminf(fmaxf(f[j], E.ln_lo), E.ln_hi);
@@ -194,22 +214,35 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
                         int k = int(tf);
                         k = k < 0 ? 0 : (k > E.n_buckets - 1 ? E.n_buckets - 1 : k);
                         const float fr = t - tf;
-                        if (fminf(fr, 1.0f - fr) < E.flag_t) {                     // decided exactly by hyper_fix_kernel
-                            const uint32_t pos = atomicAdd(E.fix_count, 1u);
-                            E.fix_list[pos] = uint32_t(e0 + j);
-                        }
+                        if (fminf(fr, 1.0f - fr) < E.flag_t) fm |= 1u << j;
                         if ((j & 3) == 0) packed[j >> 2] = uint32_t(k); else packed[j >> 2] |= uint32_t(k) << (8 * (j & 3));
                     }
-                    uint4 *di = reinterpret_cast<uint4 *>(E.idx + e0);
-                    di[0] = make_uint4(packed[0], packed[1], packed[2], packed[3]);
-                    di[1] = make_uint4(packed[4], packed[5], packed[6], packed[7]);
-                    if (E.lnscale) {
-                        float4 *dl = reinterpret_cast<float4 *>(E.lnscale + e0);
+                    if (!live) fm = 0;
+                    // one atomic per warp and chunk instead of one per flagged element: 1.2 % of a million elements on a
+                    // single address serialised in L2 and stretched this epilogue to 6-28 us
+                    const uint32_t cnt = __popc(fm);
+                    uint32_t incl = cnt;
 #pragma unroll
-                        for (int q = 0; q < 8; ++q) dl[q] = make_float4(f[4 * q], f[4 * q + 1], f[4 * q + 2], f[4 * q + 3]);
+                    for (int d = 1; d < 32; d <<= 1) {
+                        const uint32_t o = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+                        if (lane >= d) incl += o;
+                    }
+                    const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+                    flush_pending();                                               // the previous chunk's slots have arrived by now
+                    if (total) {
+                        if (lane == 31) pend_base = atomicAdd(E.fix_count, total);
+                        pend_fm = fm; pend_off = incl - cnt; pend_e0 = e0; pend_total = total;
+                    }
+                    if (live) {
+                        st_global_256(E.idx + e0, packed);
+                        if (E.lnscale) {
+#pragma unroll
+                            for (int q = 0; q < 4; ++q) st_global_256(E.lnscale + e0 + 8 * q, f + 8 * q);
+                        }
                     }
                 }
             }
+            flush_pending();
         } else {
             for (int c0 = half * 32; c0 < p.BN; c0 += 64) {
                 uint32_t v[32];
@@ -301,6 +334,7 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
         if (lane == 0) { if (pair_rank < 0) mbar_arrive(tempty0 + 8u * acc); else mbar_arrive_cluster(tempty0 + 8u * acc); }
     }
 }
+
 
 template <int MODE>
 __global__ void __launch_bounds__(kThreads, 1)

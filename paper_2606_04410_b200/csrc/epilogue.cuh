@@ -83,6 +83,19 @@ __device__ __forceinline__ void gelu_bias2(float acc0, float acc1, float b0, flo
 __device__ __forceinline__ float apply_act(float v, int act) { return act == ACT_GELU ? gelu_erf(v) : v; }
 
 // Destination element offset of packed output column n of input pixel (img, y, x); EPI_NHWC / EPI_PS2 only.
+// 256-bit global store (sm_100: STG.E.256): one thread writes a whole 32-byte sector, so a row that a thread owns never
+// reaches L2 as half-sector partial writes (which cost a read-modify-write each).  p must be 32-byte aligned.
+__device__ __forceinline__ void st_global_256(void *p, const float *f)
+{
+    asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(f[0]), "f"(f[1]), "f"(f[2]), "f"(f[3]), "f"(f[4]),
+                 "f"(f[5]), "f"(f[6]), "f"(f[7]) : "memory");
+}
+__device__ __forceinline__ void st_global_256(void *p, const uint32_t *u)
+{
+    asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(u[0]), "r"(u[1]), "r"(u[2]), "r"(u[3]), "r"(u[4]),
+                 "r"(u[5]), "r"(u[6]), "r"(u[7]) : "memory");
+}
+
 __device__ __forceinline__ long long epi_offset(const EpiParams &E, int img, int y, int x, int H, int W, int n)
 {
     if (E.mode == EPI_NHWC) {
