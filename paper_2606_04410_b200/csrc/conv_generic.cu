@@ -307,14 +307,130 @@ __global__ void __launch_bounds__(V == 4 ? 256 : 512, 2) dwconv3x3_tma_kernel(co
     }
 }
 
+// ---- A6, column-blocked variant (what is launched).  Same tiles, TMA boxes and double buffering as above, but a thread owns
+// ONE channel pair of NC adjacent columns instead of four pairs of one column: a warp is the 32 pairs of one 64-channel slab,
+// so a halo pixel is one conflict-free LDS.32 wavefront (128 contiguous bytes), a halo row of NC + 2 pixels serves NC
+// outputs (NC + 2 bf16x2 -> f32x2 conversions instead of 3 NC), the 9 weights take 18 registers instead of 72 and the bias
+// stays in registers.  ncu on the 8-channel kernel showed why this matters: nothing saturated (issue 44 %, FMA 21 %, ALU
+// 30 %), 4 warps per scheduler at 128 registers, 0.83 eligible.  Bottom-edge tiles stop at the last image row and are
+// ordered last, so the blocks that get one tile more than the others get the cheap ones.
+#ifndef UFNVC_DW_NC
+#define UFNVC_DW_NC 4
+#endif
+constexpr int kDwNC = UFNVC_DW_NC;                     // columns per thread
+template <int NC>
+__global__ void __launch_bounds__(NC == 4 ? 256 : 512, 2) dwconv3x3_cols_kernel(const __grid_constant__ CUtensorMap tm_in, bf16 *__restrict__ out,
+                                                             const float *__restrict__ w9c, const float *__restrict__ bias,
+                                                             int n_img, int H, int W, int C, int tiles_x, int tiles_y)
+{
+    extern __shared__ __align__(1024) uint8_t dw_smem[];
+    const uint32_t base = (smem_u32(dw_smem) + 1023u) & ~1023u;
+    const int slabs = C >> 6;
+    const uint32_t buf_bytes = uint32_t(slabs) * kDwSlab;
+    const uint32_t bar = base + 2u * buf_bytes;                       // two full barriers, one per buffer
+    const int n_tiles = n_img * tiles_x * tiles_y;
+    const int n_full = n_img * tiles_x * (tiles_y - 1);               // tiles above the bottom tile row come first
+    auto coord = [&](int t, int &tx, int &ty, int &im) {
+        if (t < n_full) {
+            tx = t % tiles_x;
+            const int r = t / tiles_x;
+            ty = r % (tiles_y - 1); im = r / (tiles_y - 1);
+        } else {
+            const int u = t - n_full;
+            tx = u % tiles_x; im = u / tiles_x; ty = tiles_y - 1;
+        }
+    };
+    auto issue = [&](int t, uint32_t b) {                              // thread 0: TMA the tile + halo into buffer b
+        int tx, ty, im;
+        coord(t, tx, ty, im);
+        mbar_expect_tx(bar + 8u * b, uint32_t(slabs) * (kDwHalo * kDwHalo * 128));
+        for (int s = 0; s < slabs; ++s)
+            tma_load_4d(base + b * buf_bytes + uint32_t(s) * kDwSlab, &tm_in, bar + 8u * b, s * 64, tx * kDwT - 1, ty * kDwT - 1, im);
+    };
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        mbar_init(bar + 8, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        if (int(blockIdx.x) < n_tiles) issue(blockIdx.x, 0);
+        if (int(blockIdx.x + gridDim.x) < n_tiles) issue(blockIdx.x + gridDim.x, 1);
+    }
+    const int cp = C >> 1;                                            // channel pairs; a multiple of 32
+    const int g = threadIdx.x / cp, p = threadIdx.x % cp;             // column group of the tile, channel pair
+    const int c0 = 2 * p;
+    uint64_t wv[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        const float2 q = __ldg(reinterpret_cast<const float2 *>(w9c + k * C + c0));
+        wv[k] = f2_pack(q.x, q.y);
+    }
+    uint64_t bv;
+    {
+        const float2 q = __ldg(reinterpret_cast<const float2 *>(bias + c0));
+        bv = f2_pack(q.x, q.y);
+    }
+    __syncthreads();                                                  // barriers initialised before anyone polls them
+
+    const long long row_stride = (long long)W * C;
+    uint32_t it = 0;
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const uint32_t b = it & 1u;
+        int tx, ty, img;
+        coord(tile, tx, ty, img);
+        const int x0 = tx * kDwT + g * NC, y0 = ty * kDwT;
+        mbar_wait(bar + 8u * b, (it >> 1) & 1u);
+        // halo pixel (hy, g * NC + j), this thread's pair: lanes of a warp read 128 contiguous bytes
+        const uint32_t tb = base + b * buf_bytes + uint32_t(p >> 5) * kDwSlab + uint32_t(p & 31) * 4u + uint32_t(g * NC) * 128u;
+        uint64_t accP[NC], accC[NC], accN[NC];
+#pragma unroll
+        for (int j = 0; j < NC; ++j) { accP[j] = 0ull; accC[j] = 0ull; accN[j] = 0ull; }
+        bf16 *dst = out + (((long long)img * H + y0) * W + x0) * C + c0;
+#pragma unroll
+        for (int hy = 0; hy < kDwHalo; ++hy) {                        // halo row hy = image row y0 - 1 + hy
+            if (hy >= 3 && y0 + hy - 2 >= H) break;                   // block-uniform: no output row needs this halo row
+            uint64_t f[NC + 2];
+#pragma unroll
+            for (int j = 0; j < NC + 2; ++j) {
+                uint32_t w;
+                asm volatile("ld.shared.b32 %0, [%1];" : "=r"(w) : "r"(tb + uint32_t(hy * kDwHalo + j) * 128u));
+                f[j] = dw_pair(w);
+            }
+#pragma unroll
+            for (int j = 0; j < NC; ++j) {
+                accP[j] = f2_fma(wv[6], f[j], f2_fma(wv[7], f[j + 1], f2_fma(wv[8], f[j + 2], accP[j])));
+                accC[j] = f2_fma(wv[3], f[j], f2_fma(wv[4], f[j + 1], f2_fma(wv[5], f[j + 2], accC[j])));
+                accN[j] = f2_fma(wv[0], f[j], f2_fma(wv[1], f[j + 1], f2_mul(wv[2], f[j + 2])));
+            }
+            if (hy >= 2) {                                            // output row y0 + hy - 2 is complete
+#pragma unroll
+                for (int j = 0; j < NC; ++j) {
+                    if (x0 + j < W) {
+                        float a, b2;
+                        f2_unpack(f2_add(accP[j], bv), a, b2);
+                        *reinterpret_cast<__nv_bfloat162 *>(dst + j * C) = __floats2bfloat162_rn(a, b2);
+                    }
+                }
+                dst += row_stride;
+            }
+#pragma unroll
+            for (int j = 0; j < NC; ++j) { accP[j] = accC[j]; accC[j] = accN[j]; }
+        }
+        __syncthreads();                                              // everyone is done reading buffer b
+        if (threadIdx.x == 0 && tile + 2 * int(gridDim.x) < n_tiles) issue(tile + 2 * int(gridDim.x), b);
+    }
+}
+
 cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
                                  int C, cudaStream_t st)
 {
     const int tiles_x = (W + kDwT - 1) / kDwT, tiles_y = (H + kDwT - 1) / kDwT;
-    const size_t smem = 1024 + 2 * size_t(C >> 6) * kDwSlab + 16 + size_t(C) * 4;
-    static thread_local int n_sm = 0;
+    const size_t smem = 1024 + 2 * size_t(C >> 6) * kDwSlab + 16;
+    static thread_local int n_sm = 0, variant = 0;
     if (n_sm == 0) {
+        const char *v = std::getenv("UFNVC_DW_VARIANT");              // tuning knob: 0 = 8 channels x 1 column, 2 / 4 = 1 pair x NC columns
+        variant = v ? std::atoi(v) : kDwNC;
         cudaError_t e = cudaFuncSetAttribute(dwconv3x3_tma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(dwconv3x3_cols_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(dwconv3x3_cols_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
         int dev = 0;
         cudaGetDevice(&dev);
@@ -322,7 +438,9 @@ cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const floa
     }
     const int n_tiles = n_img * tiles_x * tiles_y;
     const int grid = n_tiles < 2 * n_sm ? n_tiles : 2 * n_sm;          // persistent: two blocks per SM, double-buffered tiles
-    dwconv3x3_tma_kernel<4><<<grid, C, smem, st>>>(tm_in, out, w9c, bias, n_img, H, W, C, tiles_x, tiles_y);
+    if (variant == 2) dwconv3x3_cols_kernel<2><<<grid, (C / 2) * (kDwT / 2), smem, st>>>(tm_in, out, w9c, bias, n_img, H, W, C, tiles_x, tiles_y);
+    else if (variant == 4) dwconv3x3_cols_kernel<4><<<grid, (C / 2) * (kDwT / 4), smem, st>>>(tm_in, out, w9c, bias, n_img, H, W, C, tiles_x, tiles_y);
+    else dwconv3x3_tma_kernel<4><<<grid, C, smem + size_t(C) * 4, st>>>(tm_in, out, w9c, bias, n_img, H, W, C, tiles_x, tiles_y);
     return cudaGetLastError();
 }
 
