@@ -314,19 +314,16 @@ __global__ void __launch_bounds__(V == 4 ? 256 : 512, 2) dwconv3x3_tma_kernel(co
 // stays in registers.  ncu on the 8-channel kernel showed why this matters: nothing saturated (issue 44 %, FMA 21 %, ALU
 // 30 %), 4 warps per scheduler at 128 registers, 0.83 eligible.  Bottom-edge tiles stop at the last image row and are
 // ordered last, so the blocks that get one tile more than the others get the cheap ones.
-#ifndef UFNVC_DW_NC
-#define UFNVC_DW_NC 4
-#endif
-constexpr int kDwNC = UFNVC_DW_NC;                     // columns per thread
-template <int NC>
-__global__ void __launch_bounds__(NC == 4 ? 256 : 512, 2) dwconv3x3_cols_kernel(const __grid_constant__ CUtensorMap tm_in, bf16 *__restrict__ out,
-                                                             const float *__restrict__ w9c, const float *__restrict__ bias,
-                                                             int n_img, int H, int W, int C, int tiles_x, int tiles_y)
+constexpr int kDwNC = 4;                                 // columns per thread
+template <int CC>                                         // CC = channel count (64, 128, 192 or 256), compile-time so that the
+__global__ void __launch_bounds__(CC, 2) dwconv3x3_cols_kernel(const __grid_constant__ CUtensorMap tm_in, bf16 *__restrict__ out,  // column
+                                                             const float *__restrict__ w9c, const float *__restrict__ bias,     // stores are
+                                                             int n_img, int H, int W, int tiles_x, int tiles_y)                 // immediates
 {
+    constexpr int NC = kDwNC, C = CC, slabs = CC >> 6;
     extern __shared__ __align__(1024) uint8_t dw_smem[];
     const uint32_t base = (smem_u32(dw_smem) + 1023u) & ~1023u;
-    const int slabs = C >> 6;
-    const uint32_t buf_bytes = uint32_t(slabs) * kDwSlab;
+    constexpr uint32_t buf_bytes = uint32_t(slabs) * kDwSlab;
     const uint32_t bar = base + 2u * buf_bytes;                       // two full barriers, one per buffer
     const int n_tiles = n_img * tiles_x * tiles_y;
     const int n_full = n_img * tiles_x * (tiles_y - 1);               // tiles above the bottom tile row come first
@@ -340,21 +337,26 @@ __global__ void __launch_bounds__(NC == 4 ? 256 : 512, 2) dwconv3x3_cols_kernel(
             tx = u % tiles_x; im = u / tiles_x; ty = tiles_y - 1;
         }
     };
-    auto issue = [&](int t, uint32_t b) {                              // thread 0: TMA the tile + halo into buffer b
+    auto issue = [&](int t, uint32_t b) {                              // one elected lane: TMA the tile + halo into buffer b
         int tx, ty, im;
         coord(t, tx, ty, im);
         mbar_expect_tx(bar + 8u * b, uint32_t(slabs) * (kDwHalo * kDwHalo * 128));
+#pragma unroll
         for (int s = 0; s < slabs; ++s)
             tma_load_4d(base + b * buf_bytes + uint32_t(s) * kDwSlab, &tm_in, bar + 8u * b, s * 64, tx * kDwT - 1, ty * kDwT - 1, im);
     };
+    const bool producer_warp = threadIdx.x < 32;
     if (threadIdx.x == 0) {
         mbar_init(bar, 1);
         mbar_init(bar + 8, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+    if (producer_warp && elect_one()) {
         if (int(blockIdx.x) < n_tiles) issue(blockIdx.x, 0);
         if (int(blockIdx.x + gridDim.x) < n_tiles) issue(blockIdx.x + gridDim.x, 1);
     }
-    const int cp = C >> 1;                                            // channel pairs; a multiple of 32
+    constexpr int cp = C >> 1;                                        // channel pairs; a multiple of 32
     const int g = threadIdx.x / cp, p = threadIdx.x % cp;             // column group of the tile, channel pair
     const int c0 = 2 * p;
     uint64_t wv[9];
@@ -377,6 +379,7 @@ __global__ void __launch_bounds__(NC == 4 ? 256 : 512, 2) dwconv3x3_cols_kernel(
         int tx, ty, img;
         coord(tile, tx, ty, img);
         const int x0 = tx * kDwT + g * NC, y0 = ty * kDwT;
+        const int n_cols = W - x0;                                    // columns j < n_cols are inside the image
         mbar_wait(bar + 8u * b, (it >> 1) & 1u);
         // halo pixel (hy, g * NC + j), this thread's pair: lanes of a warp read 128 contiguous bytes
         const uint32_t tb = base + b * buf_bytes + uint32_t(p >> 5) * kDwSlab + uint32_t(p & 31) * 4u + uint32_t(g * NC) * 128u;
@@ -401,22 +404,38 @@ __global__ void __launch_bounds__(NC == 4 ? 256 : 512, 2) dwconv3x3_cols_kernel(
                 accN[j] = f2_fma(wv[0], f[j], f2_fma(wv[1], f[j + 1], f2_mul(wv[2], f[j + 2])));
             }
             if (hy >= 2) {                                            // output row y0 + hy - 2 is complete
+                __nv_bfloat162 o[NC];
 #pragma unroll
                 for (int j = 0; j < NC; ++j) {
-                    if (x0 + j < W) {
-                        float a, b2;
-                        f2_unpack(f2_add(accP[j], bv), a, b2);
-                        *reinterpret_cast<__nv_bfloat162 *>(dst + j * C) = __floats2bfloat162_rn(a, b2);
-                    }
+                    float a, b2;
+                    f2_unpack(f2_add(accP[j], bv), a, b2);
+                    o[j] = __floats2bfloat162_rn(a, b2);
                 }
+#pragma unroll
+                for (int j = 0; j < NC; ++j)                          // predicated stores at immediate offsets j * C
+                    if (j < n_cols) *reinterpret_cast<__nv_bfloat162 *>(dst + j * C) = o[j];
                 dst += row_stride;
             }
 #pragma unroll
             for (int j = 0; j < NC; ++j) { accP[j] = accC[j]; accC[j] = accN[j]; }
         }
         __syncthreads();                                              // everyone is done reading buffer b
-        if (threadIdx.x == 0 && tile + 2 * int(gridDim.x) < n_tiles) issue(tile + 2 * int(gridDim.x), b);
+        if (producer_warp && tile + 2 * int(gridDim.x) < n_tiles && elect_one()) issue(tile + 2 * int(gridDim.x), b);
     }
+}
+
+template <int CC>
+static cudaError_t launch_dw_cols(const CUtensorMap &tm_in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
+                                  int tiles_x, int tiles_y, int grid, size_t smem, cudaStream_t st)
+{
+    static thread_local bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(dwconv3x3_cols_kernel<CC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dwconv3x3_cols_kernel<CC><<<grid, CC, smem, st>>>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
@@ -426,11 +445,9 @@ cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const floa
     const size_t smem = 1024 + 2 * size_t(C >> 6) * kDwSlab + 16;
     static thread_local int n_sm = 0, variant = 0;
     if (n_sm == 0) {
-        const char *v = std::getenv("UFNVC_DW_VARIANT");              // tuning knob: 0 = 8 channels x 1 column, 2 / 4 = 1 pair x NC columns
+        const char *v = std::getenv("UFNVC_DW_VARIANT");              // tuning knob: 0 = 8 channels x 1 column, else 1 pair x 4 columns
         variant = v ? std::atoi(v) : kDwNC;
         cudaError_t e = cudaFuncSetAttribute(dwconv3x3_tma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(dwconv3x3_cols_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(dwconv3x3_cols_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
         int dev = 0;
         cudaGetDevice(&dev);
@@ -438,9 +455,16 @@ cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const floa
     }
     const int n_tiles = n_img * tiles_x * tiles_y;
     const int grid = n_tiles < 2 * n_sm ? n_tiles : 2 * n_sm;          // persistent: two blocks per SM, double-buffered tiles
-    if (variant == 2) dwconv3x3_cols_kernel<2><<<grid, (C / 2) * (kDwT / 2), smem, st>>>(tm_in, out, w9c, bias, n_img, H, W, C, tiles_x, tiles_y);
-    else if (variant == 4) dwconv3x3_cols_kernel<4><<<grid, (C / 2) * (kDwT / 4), smem, st>>>(tm_in, out, w9c, bias, n_img, H, W, C, tiles_x, tiles_y);
-    else dwconv3x3_tma_kernel<4><<<grid, C, smem + size_t(C) * 4, st>>>(tm_in, out, w9c, bias, n_img, H, W, C, tiles_x, tiles_y);
+    if (variant != 0) {
+        switch (C) {
+            case 64: return launch_dw_cols<64>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st);
+            case 128: return launch_dw_cols<128>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st);
+            case 192: return launch_dw_cols<192>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st);
+            case 256: return launch_dw_cols<256>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st);
+            default: break;
+        }
+    }
+    dwconv3x3_tma_kernel<4><<<grid, C, smem + size_t(C) * 4, st>>>(tm_in, out, w9c, bias, n_img, H, W, C, tiles_x, tiles_y);
     return cudaGetLastError();
 }
 
