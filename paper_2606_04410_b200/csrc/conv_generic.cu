@@ -351,11 +351,6 @@ __global__ void __launch_bounds__(CC, 2) dwconv3x3_cols_kernel(const __grid_cons
         mbar_init(bar + 8, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    __syncwarp();
-    if (producer_warp && elect_one()) {
-        if (int(blockIdx.x) < n_tiles) issue(blockIdx.x, 0);
-        if (int(blockIdx.x + gridDim.x) < n_tiles) issue(blockIdx.x + gridDim.x, 1);
-    }
     constexpr int cp = C >> 1;                                        // channel pairs; a multiple of 32
     const int g = threadIdx.x / cp, p = threadIdx.x % cp;             // column group of the tile, channel pair
     const int c0 = 2 * p;
@@ -369,6 +364,12 @@ __global__ void __launch_bounds__(CC, 2) dwconv3x3_cols_kernel(const __grid_cons
     {
         const float2 q = __ldg(reinterpret_cast<const float2 *>(bias + c0));
         bv = f2_pack(q.x, q.y);
+    }
+    pdl_grid_sync();                                                  // weights and bias are static; the input is the predecessor's output
+    __syncwarp();                                                     // the elected lane need not be the one that initialised the barriers
+    if (producer_warp && elect_one()) {
+        if (int(blockIdx.x) < n_tiles) issue(blockIdx.x, 0);
+        if (int(blockIdx.x + gridDim.x) < n_tiles) issue(blockIdx.x + gridDim.x, 1);
     }
     __syncthreads();                                                  // barriers initialised before anyone polls them
 
@@ -434,8 +435,7 @@ static cudaError_t launch_dw_cols(const CUtensorMap &tm_in, bf16 *out, const flo
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    dwconv3x3_cols_kernel<CC><<<grid, CC, smem, st>>>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y);
-    return cudaGetLastError();
+    return launch_pdl(dwconv3x3_cols_kernel<CC>, grid, CC, smem, st, 1, tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y);
 }
 
 cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,

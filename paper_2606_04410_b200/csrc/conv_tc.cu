@@ -373,6 +373,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
+    pdl_grid_sync();                                                 // the predecessor kernel's output is complete and visible from here on
 
     if (warp == 0) {
         // ===================== TMA producer =====================
@@ -496,6 +497,7 @@ conv_halo_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_consta
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
+    pdl_grid_sync();                                                 // the predecessor kernel's output is complete and visible from here on
 
     // weight-set key of a tile: resident weights are reloaded only when it changes
     auto tile_key = [&](const TileCoord &tc) { return group_of(p, tc.img) * p.n_tiles + tc.nt; };
@@ -656,6 +658,7 @@ conv_halo_pair_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_c
     cluster_sync_all();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
+    pdl_grid_sync();                                                 // the predecessor kernel's output is complete and visible from here on
 
     if (warp == 0) {
         // ===================== TMA producer (both CTAs): own halo tile, own half of every weight tile =====================
@@ -853,16 +856,7 @@ cudaError_t launch_conv_halo_pair(const ConvLayer &L, const ConvProblem &P, cons
         configured = true;
     }
     const int clusters = p.total_tiles < num_sms / 2 ? p.total_tiles : num_sms / 2;
-    cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(2 * clusters);
-    cfg.blockDim = dim3(kThreads);
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, conv_halo_pair_kernel<EPI_PS2>, tmap_halo, L.tmap_w_half, p, nb, na);
+    return launch_pdl(conv_halo_pair_kernel<EPI_PS2>, 2 * clusters, kThreads, smem, st, 2, tmap_halo, L.tmap_w_half, p, nb, na);
 }
 
 cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
@@ -905,8 +899,7 @@ cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUt
             if (e != cudaSuccess) return e;
             for (auto &c : configured) if (!c) { c = (const void *)kern; break; }
         }
-        kern<<<grid, kThreads, smem, st>>>(tmap_halo, L.tmap_w, p, nb, na);
-        return cudaGetLastError();
+        return launch_pdl(kern, grid, kThreads, smem, st, 1, tmap_halo, L.tmap_w, p, nb, na);
     };
     switch (E.mode) {
         case EPI_NHWC: return resident ? launch(conv_halo_kernel<EPI_NHWC, true>) : launch(conv_halo_kernel<EPI_NHWC, false>);
@@ -953,8 +946,7 @@ cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUten
             if (e != cudaSuccess) return e;
             for (auto &c : configured) if (!c) { c = (const void *)kern; break; }
         }
-        kern<<<grid, kThreads, smem, st>>>(tmap_in, L.tmap_w, p);
-        return cudaGetLastError();
+        return launch_pdl(kern, grid, kThreads, smem, st, 1, tmap_in, L.tmap_w, p);
     };
     switch (E.mode) {
         case EPI_NHWC: return launch(conv_tc_kernel<EPI_NHWC>);

@@ -88,6 +88,7 @@ final_is_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
+    pdl_grid_sync();                                                 // the predecessor kernel's output is complete and visible from here on
 
     if (warp == 0) {
         // ===================== TMA producer =====================
@@ -275,8 +276,7 @@ cudaError_t launch_final_is(const FinalMaps &m, const ConvLayer &L, int n_img, i
         configured = true;
     }
     const int grid = p.total_tiles < num_sms ? p.total_tiles : num_sms;
-    final_is_kernel<<<grid, kFThreads, kFSmem, st>>>(m.tm_in, m.tm_w, p);
-    return cudaGetLastError();
+    return launch_pdl(final_is_kernel, grid, kFThreads, kFSmem, st, 1, m.tm_in, m.tm_w, p);
 }
 
 }  // namespace ufnvc

@@ -100,6 +100,17 @@ __device__ __forceinline__ void umma_commit(uint32_t bar)
 // One elected lane of a converged warp.  Unlike `lane == 0`, the compiler knows exactly one thread is active inside the
 // branch, so tcgen05.mma / TMA operands live in uniform registers without a per-instruction "waterfall" loop (with
 // `lane == 0` every UTCHMMA cost ~25 SASS instructions of ELECT / BRA.U.ANY: the A9 kernel was bound by MMA issue).
+// Programmatic dependent launch (PDL).  A kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may become
+// resident while its predecessor in the stream is still draining: everything above this call (barrier init, TMEM allocation,
+// tensor-map prefetch, loads of weights that no kernel of the decode writes) overlaps the predecessor's tail.  The wait returns
+// once the predecessor grid has completed and its writes are visible; only then are the dependents allowed to launch, so at most
+// one successor is ever resident early.  Without the launch attribute both instructions are no-ops.
+__device__ __forceinline__ void pdl_grid_sync()
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
 __device__ __forceinline__ bool elect_one()
 {
     uint32_t pred;

@@ -96,6 +96,7 @@ trunk_mlp_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
+    pdl_grid_sync();                                                 // the predecessor kernel's output is complete and visible from here on
 
     if (warp == 0) {
         // ===================== TMA producer: d tile, then W1 / W2 chunks in MMA consumption order =====================
@@ -370,6 +371,7 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
     cluster_sync_all();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
+    pdl_grid_sync();                                                 // the predecessor kernel's output is complete and visible from here on
 
     if (warp == 0) {
         // ===================== TMA producer (both CTAs): own d tile, own half of every weight tile =====================
@@ -646,22 +648,12 @@ cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const Con
         }
         const int n_ptiles = (p.n_tiles + 1) / 2;
         const int clusters = n_ptiles < num_sms / 2 ? n_ptiles : num_sms / 2;
-        cudaLaunchConfig_t cfg{};
-        cfg.gridDim = dim3(2 * clusters);
-        cfg.blockDim = dim3(kTrunkThreads);
-        cfg.dynamicSmemBytes = kTrunkSmem;
-        cfg.stream = st;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-        cfg.attrs = attr; cfg.numAttrs = 1;
         static const bool tmh = [] { const char *e = std::getenv("UFNVC_TRUNK_TMEM_HIDDEN"); return !(e && e[0] == '0'); }();
-        return tmh ? cudaLaunchKernelEx(&cfg, trunk_mlp_pair_kernel<true>, m.tm_d, m.tm_w1h, m.tm_w2h, p)
-                   : cudaLaunchKernelEx(&cfg, trunk_mlp_pair_kernel<false>, m.tm_d, m.tm_w1h, m.tm_w2h, p);
+        return tmh ? launch_pdl(trunk_mlp_pair_kernel<true>, 2 * clusters, kTrunkThreads, kTrunkSmem, st, 2, m.tm_d, m.tm_w1h, m.tm_w2h, p)
+                   : launch_pdl(trunk_mlp_pair_kernel<false>, 2 * clusters, kTrunkThreads, kTrunkSmem, st, 2, m.tm_d, m.tm_w1h, m.tm_w2h, p);
     }
     const int grid = p.n_tiles < num_sms ? p.n_tiles : num_sms;
-    trunk_mlp_kernel<<<grid, kTrunkThreads, kTrunkSmem, st>>>(m.tm_d, m.tm_w1, m.tm_w2, p);
-    return cudaGetLastError();
+    return launch_pdl(trunk_mlp_kernel, grid, kTrunkThreads, kTrunkSmem, st, 1, m.tm_d, m.tm_w1, m.tm_w2, p);
 }
 
 }  // namespace ufnvc

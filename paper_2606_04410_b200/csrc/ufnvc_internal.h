@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <cstdlib>
 #include <string>
 #include <vector>
 
@@ -72,6 +73,34 @@ struct ConvProblem {
 };
 
 // ---- kernels (each .cu exposes host launchers; all enqueue on `st` and return cudaGetLastError()) -------------
+// Launch with programmatic stream serialization (PDL, see pdl_grid_sync in tc_ptx.cuh) and an optional cluster of cluster_x CTAs.
+// UFNVC_PDL=0 turns the attribute off (plain stream order) for A/B timing.
+inline bool pdl_enabled()
+{
+    static const bool on = [] { const char *e = std::getenv("UFNVC_PDL"); return !(e && e[0] == '0'); }();
+    return on;
+}
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t st, int cluster_x, Args &&...args)
+{
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[2];
+    unsigned n = 0;
+    if (cluster_x > 1) {
+        attr[n].id = cudaLaunchAttributeClusterDimension;
+        attr[n].val.clusterDim.x = unsigned(cluster_x); attr[n].val.clusterDim.y = 1; attr[n].val.clusterDim.z = 1;
+        ++n;
+    }
+    if (pdl_enabled()) {
+        attr[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[n].val.programmaticStreamSerializationAllowed = 1;
+        ++n;
+    }
+    cfg.attrs = attr; cfg.numAttrs = n;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 cudaError_t launch_conv_generic(const ConvLayer &L, const ConvProblem &P, const EpiParams &E, cudaStream_t st);
 cudaError_t launch_dwconv3x3(const bf16 *in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
                              int C, cudaStream_t st);
