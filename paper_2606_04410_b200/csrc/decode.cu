@@ -45,6 +45,9 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     const int P = h->h * h->w, Pz = h->h_z * h->w_z;
     const size_t ne = size_t(n) * P * c.c_y;
 
+    // the status word is cleared up front (nothing before the rANS kernel touches it) so that no memset node sits between
+    // the hyper head's last kernel and the rANS kernel, which is launched with programmatic stream serialization
+    if (!entropy_params_only && !h->keep_status) CU_TRY(cudaMemsetAsync(h->d_status, 0, 4, st));
     // ---- A1 + A2: hyper-decoder in fp64 -> mu, ln sigma, bucket index ----
     const bool need_hyper = entropy_params_only || !idx_ovr || !mu_ovr || (taps && (taps->mu || taps->lnscale));
     mark(sg, st);
@@ -94,7 +97,6 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     mark(sg, st);
 
     // ---- A3 + A4: rANS decode + dequantisation ----
-    if (!h->keep_status) CU_TRY(cudaMemsetAsync(h->d_status, 0, 4, st));
     RansParams rp{};
     rp.bits = bits; rp.bits_bytes = bits_bytes; rp.sub_off = sub_off; rp.idx = idx; rp.mu = mu;
     rp.sub_stride = h->y_sub_stride > 0 ? h->y_sub_stride : h->n_sub; rp.sub_first = h->y_sub_stride > 0 ? h->n_sub_z : 0;

@@ -265,6 +265,8 @@ __global__ void __launch_bounds__(256) hyper_fix_kernel(const uint32_t *__restri
                                                         const double *__restrict__ fix_b, int c_h, int hz, int wz, HeadParams hp)
 {
     const int lane = threadIdx.x & 31;
+    asm volatile("griddepcontrol.wait;" ::: "memory");              // PDL: the head conv has written the list and its count
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); // the rANS blocks may start loading their tables
     const unsigned n = *count;
     const unsigned warps = (gridDim.x * blockDim.x) >> 5;
     for (unsigned i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; i < n; i += warps) {
@@ -342,8 +344,7 @@ cudaError_t launch_hyper_reduce_split(const double *part, const double *bias, do
 cudaError_t launch_hyper_fix(const uint32_t *list, const uint32_t *count, const double *x2, const double *fix_w, const double *fix_b,
                              int c_h, int hz, int wz, const HeadParams &hp, int num_sms, cudaStream_t st)
 {
-    hyper_fix_kernel<<<num_sms * 4, 256, 0, st>>>(list, count, x2, fix_w, fix_b, c_h, hz, wz, hp);
-    return cudaGetLastError();
+    return launch_pdl(hyper_fix_kernel, unsigned(num_sms * 4), 256u, 0, st, 1, list, count, x2, fix_w, fix_b, c_h, hz, wz, hp);
 }
 
 cudaError_t launch_hyper_head(const HyperLayer &L, const double *in, int n_img, int hz, int wz, const HeadParams &hp,

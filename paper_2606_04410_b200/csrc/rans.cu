@@ -25,6 +25,10 @@ __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
         for (int i = threadIdx.x; i < nb * 64; i += blockDim.x) dc[i] = src_c[i];
         for (int i = threadIdx.x; i < nb * (kLutBuckets / 8); i += blockDim.x) dl[i] = src_l[i];
     }
+    // PDL: the 192 KB of static tables above load while the predecessor (the hyper head's fix-up kernel) is still running;
+    // idx, mu and the status word are only touched after the predecessor grid has completed.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     __syncthreads();
 
     const int sub = blockIdx.x;                 // chunk * n_sub + s
@@ -161,8 +165,7 @@ cudaError_t launch_rans_decode(const RansParams &p, cudaStream_t st)
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    rans_decode_kernel<<<p.n_chunks * p.n_sub, p.W, smem, st>>>(p, nb);
-    return cudaGetLastError();
+    return launch_pdl(rans_decode_kernel, unsigned(p.n_chunks * p.n_sub), unsigned(p.W), smem, st, 1, p, nb);
 }
 
 }  // namespace ufnvc
