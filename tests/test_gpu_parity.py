@@ -4,6 +4,7 @@ Tolerances (BASELINE.json north_star): symbols and CDF indices bit-exact when fe
 rate <= 1e-5, only at bucket boundaries; mu within 1e-2 relative (|d mu| <= 1e-2 max(|mu|,1), R13), ln sigma within
 1e-2; pixels <= 2e-2 max abs on [0,1] and PSNR >= 45 dB against the oracle's frames.
 """
+import dataclasses
 import math
 
 import numpy as np
@@ -28,6 +29,11 @@ CASES = {
     "cfg2-ragged-pmu": synth.progressive_config(synth.crop_config(synth.CONFIGS[2], 150, 200)),
     "cfg3-crop-pmu": synth.progressive_config(synth.crop_config(synth.CONFIGS[3], 272, 480)),
 }
+# narrower trunks: the depthwise kernel is compiled per channel count (64 / 128 / 192 / 256); w = 13 leaves a last column group
+# with one valid column, h = 10 a bottom tile with two valid rows
+for _ct in (64, 128, 192):
+    CASES[f"trunk{_ct}"] = dataclasses.replace(synth.crop_config(synth.CONFIGS[2], 150, 200), T=2, c_trunk=_ct, n_trunk_blocks=2,
+                                               dec_channels=(_ct, 64, 64, 32, 3), name=f"cfg2-ragged-trunk{_ct}")
 
 
 @pytest.fixture(scope="module")
@@ -51,7 +57,8 @@ def bf16_np(t):
     return t.float().cpu().numpy()
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg2-ragged", "cfg3-crop", "cfg2", "cfg1-pmu", "cfg2-ragged-pmu", "cfg3-crop-pmu"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2-ragged", "cfg3-crop", "cfg2", "cfg1-pmu", "cfg2-ragged-pmu", "cfg3-crop-pmu",
+                                  "trunk64", "trunk128", "trunk192"])
 def test_chunk_decode_matches_oracle(decoders, name):
     dec, case = decoders(name)
     cfg = case["cfg"]
