@@ -110,6 +110,7 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
               dev_alloc(h, h->lnscale, n * P * cfg->c_y) && dev_alloc(h, h->idx, n * P * cfg->c_y) &&
               dev_alloc(h, h->yhat, n * P * cfg->c_y) && dev_alloc(h, h->fa, n * T * P * cfg->c_trunk) &&
               dev_alloc(h, h->fb, n * T * P * cfg->c_trunk) &&
+              dev_alloc(h, h->trunk_sync, size_t(cfg->n_trunk_blocks > 0 ? cfg->n_trunk_blocks : 1) * ((n * T * P + 127) / 128 + 4)) &&
               dev_alloc(h, h->hidden, cfg->n_trunk_blocks ? n * T * P * cfg->c_trunk * cfg->trunk_expand : 1);
     if (ok && cfg->mu_steps == 4) {
         const size_t cs = (3 * size_t(cfg->c_y) + 63) / 64 * 64;       // [r | mu used | mu0 | zero pad], see weights.cu mu_net

@@ -315,16 +315,21 @@ __global__ void __launch_bounds__(V == 4 ? 256 : 512, 2) dwconv3x3_tma_kernel(co
 // 30 %), 4 warps per scheduler at 128 registers, 0.83 eligible.  Bottom-edge tiles stop at the last image row and are
 // ordered last, so the blocks that get one tile more than the others get the cheap ones.
 constexpr int kDwNC = 4;                                 // columns per thread
+// Warp roles: CC / 32 compute warps and one producer warp.  The producer claims tiles (a per-launch counter if given, else
+// static striding), waits for their inputs, and issues their TMA as soon as the buffer is free; compute warps only ever wait on
+// the full barrier of their buffer and release it with one arrive per warp -- no block-wide barrier per tile.
 template <int CC>                                         // CC = channel count (64, 128, 192 or 256), compile-time so that the
-__global__ void __launch_bounds__(CC, 2) dwconv3x3_cols_kernel(const __grid_constant__ CUtensorMap tm_in, bf16 *__restrict__ out,  // column
+__global__ void __launch_bounds__(CC + 32, 2) dwconv3x3_cols_kernel(const __grid_constant__ CUtensorMap tm_in, bf16 *__restrict__ out,  // column
                                                              const float *__restrict__ w9c, const float *__restrict__ bias,     // stores are
-                                                             int n_img, int H, int W, int tiles_x, int tiles_y)                 // immediates
+                                                             int n_img, int H, int W, int tiles_x, int tiles_y,                 // immediates
+                                                             uint32_t *__restrict__ sched, const uint32_t *dep_flags, uint32_t dep_need)
 {
     constexpr int NC = kDwNC, C = CC, slabs = CC >> 6;
     extern __shared__ __align__(1024) uint8_t dw_smem[];
     const uint32_t base = (smem_u32(dw_smem) + 1023u) & ~1023u;
     constexpr uint32_t buf_bytes = uint32_t(slabs) * kDwSlab;
-    const uint32_t bar = base + 2u * buf_bytes;                       // two full barriers, one per buffer
+    const uint32_t bar = base + 2u * buf_bytes;                       // full[0], full[1], empty[0], empty[1]
+    volatile int *s_tile = reinterpret_cast<volatile int *>(dw_smem + (bar + 32u - smem_u32(dw_smem)));   // tile held by each buffer, -1 = none
     const int n_tiles = n_img * tiles_x * tiles_y;
     const int n_full = n_img * tiles_x * (tiles_y - 1);               // tiles above the bottom tile row come first
     auto coord = [&](int t, int &tx, int &ty, int &im) {
@@ -337,26 +342,79 @@ __global__ void __launch_bounds__(CC, 2) dwconv3x3_cols_kernel(const __grid_cons
             tx = u % tiles_x; im = u / tiles_x; ty = tiles_y - 1;
         }
     };
-    auto issue = [&](int t, uint32_t b) {                              // one elected lane: TMA the tile + halo into buffer b
-        int tx, ty, im;
-        coord(t, tx, ty, im);
-        mbar_expect_tx(bar + 8u * b, uint32_t(slabs) * (kDwHalo * kDwHalo * 128));
-#pragma unroll
-        for (int s = 0; s < slabs; ++s)
-            tma_load_4d(base + b * buf_bytes + uint32_t(s) * kDwSlab, &tm_in, bar + 8u * b, s * 64, tx * kDwT - 1, ty * kDwT - 1, im);
-    };
-    const bool producer_warp = threadIdx.x < 32;
     if (threadIdx.x == 0) {
         mbar_init(bar, 1);
         mbar_init(bar + 8, 1);
+        mbar_init(bar + 16, CC / 32);
+        mbar_init(bar + 24, CC / 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    const int lane = threadIdx.x & 31;
+    __syncthreads();                                                  // barriers initialised before anyone touches them
+
+    if (threadIdx.x >= CC) {
+        // ===================== producer warp =====================
+        // The input is the predecessor's output.  Without dep_flags the whole predecessor grid is waited for (PDL).  With
+        // dep_flags (tail filling) the predecessor is the trunk MLP kernel of the previous block, which counts its finished
+        // 128-pixel tiles: a tile of this kernel then only waits for the MLP tiles that cover its halo box, so the blocks of
+        // this grid that become resident while the MLP kernel runs its last, partly filled round start working.  Those MLP
+        // tiles have also finished READING the rows of `out` this tile overwrites (an MLP tile reads its rows of `out`, this
+        // kernel's output buffer, before it writes and counts), and every older kernel completed before the MLP kernel passed
+        // its own griddepcontrol.wait, which precedes the launch of this grid.
+        if (!dep_flags) asm volatile("griddepcontrol.wait;" ::: "memory");
+        asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t b = it & 1u;
+            int t = int(blockIdx.x + it * gridDim.x);
+            if (sched) {
+                if (lane == 0) t = int(atomicAdd(sched, 1u));
+                t = __shfl_sync(0xFFFFFFFFu, t, 0);
+            }
+            if (t >= n_tiles) t = -1;
+            int tx = 0, ty = 0, im = 0;
+            if (t >= 0) coord(t, tx, ty, im);
+            if (t >= 0 && dep_flags) {
+                const int ya = max(ty * kDwT - 1, 0), yb = min(ty * kDwT + kDwT, H - 1);
+                const int xa = max(tx * kDwT - 1, 0), xb = min(tx * kDwT + kDwT, W - 1);
+                const int f_lo = int((((long long)im * H + ya) * W + xa) >> 7), f_hi = int((((long long)im * H + yb) * W + xb) >> 7);
+                for (int f = f_lo + lane; f <= f_hi; f += 32) {
+                    uint32_t v, spins = 0;
+                    for (;;) {
+                        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(dep_flags + f) : "memory");
+                        if (v >= dep_need) break;
+                        __nanosleep(64);
+                        if (++spins > (1u << 22)) __trap();            // seconds: the producer kernel is gone; fail loudly, never hang
+                    }
+                }
+                asm volatile("fence.acq_rel.gpu;" ::: "memory");
+                __syncwarp();
+            }
+            if (it >= 2) mbar_wait(bar + 16u + 8u * b, ((it >> 1) - 1u) & 1u);    // every compute warp has released buffer b
+            if (elect_one()) {
+                s_tile[b] = t;
+                if (t < 0) {
+                    mbar_arrive(bar + 8u * b);                        // completes the phase: the compute warps read -1 and leave
+                } else {
+                    if (dep_flags) asm volatile("fence.proxy.async;" ::: "memory");   // the MLP kernel's generic-proxy writes -> this TMA read
+                    mbar_expect_tx(bar + 8u * b, uint32_t(slabs) * (kDwHalo * kDwHalo * 128));
+#pragma unroll
+                    for (int s = 0; s < slabs; ++s)
+                        tma_load_4d(base + b * buf_bytes + uint32_t(s) * kDwSlab, &tm_in, bar + 8u * b, s * 64, tx * kDwT - 1, ty * kDwT - 1, im);
+                }
+            }
+            __syncwarp();
+            if (t < 0) break;
+        }
+        return;
+    }
+
+    // ===================== compute warps =====================
     constexpr int cp = C >> 1;                                        // channel pairs; a multiple of 32
     const int g = threadIdx.x / cp, p = threadIdx.x % cp;             // column group of the tile, channel pair
     const int c0 = 2 * p;
     uint64_t wv[9];
 #pragma unroll
-    for (int k = 0; k < 9; ++k) {
+    for (int k = 0; k < 9; ++k) {                                     // weights and bias are static: no wait needed
         const float2 q = __ldg(reinterpret_cast<const float2 *>(w9c + k * C + c0));
         wv[k] = f2_pack(q.x, q.y);
     }
@@ -365,23 +423,16 @@ __global__ void __launch_bounds__(CC, 2) dwconv3x3_cols_kernel(const __grid_cons
         const float2 q = __ldg(reinterpret_cast<const float2 *>(bias + c0));
         bv = f2_pack(q.x, q.y);
     }
-    pdl_grid_sync();                                                  // weights and bias are static; the input is the predecessor's output
-    __syncwarp();                                                     // the elected lane need not be the one that initialised the barriers
-    if (producer_warp && elect_one()) {
-        if (int(blockIdx.x) < n_tiles) issue(blockIdx.x, 0);
-        if (int(blockIdx.x + gridDim.x) < n_tiles) issue(blockIdx.x + gridDim.x, 1);
-    }
-    __syncthreads();                                                  // barriers initialised before anyone polls them
-
     const long long row_stride = (long long)W * C;
-    uint32_t it = 0;
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+    for (uint32_t it = 0;; ++it) {
         const uint32_t b = it & 1u;
+        mbar_wait(bar + 8u * b, (it >> 1) & 1u);
+        const int tile = s_tile[b];                                   // written by the producer before its arrive on full[b]
+        if (tile < 0) break;
         int tx, ty, img;
         coord(tile, tx, ty, img);
         const int x0 = tx * kDwT + g * NC, y0 = ty * kDwT;
         const int n_cols = W - x0;                                    // columns j < n_cols are inside the image
-        mbar_wait(bar + 8u * b, (it >> 1) & 1u);
         // halo pixel (hy, g * NC + j), this thread's pair: lanes of a warp read 128 contiguous bytes
         const uint32_t tb = base + b * buf_bytes + uint32_t(p >> 5) * kDwSlab + uint32_t(p & 31) * 4u + uint32_t(g * NC) * 128u;
         uint64_t accP[NC], accC[NC], accN[NC];
@@ -420,14 +471,14 @@ __global__ void __launch_bounds__(CC, 2) dwconv3x3_cols_kernel(const __grid_cons
 #pragma unroll
             for (int j = 0; j < NC; ++j) { accP[j] = accC[j]; accC[j] = accN[j]; }
         }
-        __syncthreads();                                              // everyone is done reading buffer b
-        if (producer_warp && tile + 2 * int(gridDim.x) < n_tiles && elect_one()) issue(tile + 2 * int(gridDim.x), b);
+        __syncwarp();                                                 // every lane of this warp is done reading buffer b
+        if (lane == 0) mbar_arrive(bar + 16u + 8u * b);
     }
 }
 
 template <int CC>
 static cudaError_t launch_dw_cols(const CUtensorMap &tm_in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
-                                  int tiles_x, int tiles_y, int grid, size_t smem, cudaStream_t st)
+                                  int tiles_x, int tiles_y, int grid, size_t smem, cudaStream_t st, uint32_t *sched, const uint32_t *dep)
 {
     static thread_local bool configured = false;
     if (!configured) {
@@ -435,14 +486,14 @@ static cudaError_t launch_dw_cols(const CUtensorMap &tm_in, bf16 *out, const flo
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    return launch_pdl(dwconv3x3_cols_kernel<CC>, grid, CC, smem, st, 1, tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y);
+    return launch_pdl(dwconv3x3_cols_kernel<CC>, grid, CC + 32, smem, st, 1, tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, sched, dep, 8u);
 }
 
 cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
-                                 int C, cudaStream_t st)
+                                 int C, cudaStream_t st, uint32_t *sched, const uint32_t *dep_flags)
 {
     const int tiles_x = (W + kDwT - 1) / kDwT, tiles_y = (H + kDwT - 1) / kDwT;
-    const size_t smem = 1024 + 2 * size_t(C >> 6) * kDwSlab + 16;
+    const size_t smem = 1024 + 2 * size_t(C >> 6) * kDwSlab + 48;     // + four barriers + the two tile slots of the cols kernel
     static thread_local int n_sm = 0, variant = 0;
     if (n_sm == 0) {
         const char *v = std::getenv("UFNVC_DW_VARIANT");              // tuning knob: 0 = 8 channels x 1 column, else 1 pair x 4 columns
@@ -457,14 +508,14 @@ cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const floa
     const int grid = n_tiles < 2 * n_sm ? n_tiles : 2 * n_sm;          // persistent: two blocks per SM, double-buffered tiles
     if (variant != 0) {
         switch (C) {
-            case 64: return launch_dw_cols<64>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st);
-            case 128: return launch_dw_cols<128>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st);
-            case 192: return launch_dw_cols<192>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st);
-            case 256: return launch_dw_cols<256>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st);
+            case 64: return launch_dw_cols<64>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st, sched, dep_flags);
+            case 128: return launch_dw_cols<128>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st, sched, dep_flags);
+            case 192: return launch_dw_cols<192>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st, sched, dep_flags);
+            case 256: return launch_dw_cols<256>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st, sched, dep_flags);
             default: break;
         }
     }
-    dwconv3x3_tma_kernel<4><<<grid, C, smem + size_t(C) * 4, st>>>(tm_in, out, w9c, bias, n_img, H, W, C, tiles_x, tiles_y);
+    dwconv3x3_tma_kernel<4><<<grid, C, smem - 32 + size_t(C) * 4, st>>>(tm_in, out, w9c, bias, n_img, H, W, C, tiles_x, tiles_y);
     return cudaGetLastError();
 }
 

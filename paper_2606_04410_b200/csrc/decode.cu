@@ -48,6 +48,8 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     // the status word is cleared up front (nothing before the rANS kernel touches it) so that no memset node sits between
     // the hyper head's last kernel and the rANS kernel, which is launched with programmatic stream serialization
     if (!entropy_params_only && !h->keep_status) CU_TRY(cudaMemsetAsync(h->d_status, 0, 4, st));
+    if (!entropy_params_only && frames && c.n_trunk_blocks > 0 && h->tail_fill)
+        CU_TRY(cudaMemsetAsync(h->trunk_sync, 0, size_t(c.n_trunk_blocks) * h->trunk_sync_stride * 4, st));
     // ---- A1 + A2: hyper-decoder in fp64 -> mu, ln sigma, bucket index ----
     const bool need_hyper = entropy_params_only || !idx_ovr || !mu_ovr || (taps && (taps->mu || taps->lnscale));
     mark(sg, st);
@@ -148,13 +150,22 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     const int Ce = Ct * c.trunk_expand;
     for (int k = 0; k < c.n_trunk_blocks; ++k) {
         const ufnvc_handle::TrunkBlock &tb = h->trunk[k];
+        // every block must be fused for the counters to be produced where the next depthwise kernel expects them
+        bool fused_ok = h->use_fused_trunk && !h->force_generic;
+        for (const auto &t2 : h->trunk) fused_ok = fused_ok && t2.fused.ok;
         if (sg && sg->dw) { cudaEventRecord(sg->dw[2 * k + 1], st); }
-        if (h->dw_tma_ok) CU_TRY(launch_dwconv3x3_tma(h->tm_dw, h->fb, tb.dw_w, tb.dw_b, n * T, h->h, h->w, Ct, st));
+        // tail filling: block k's depthwise tiles wait for the MLP tiles of block k - 1 that cover their halo
+        // box instead of for the whole MLP grid, and are handed out by a per-block counter
+        uint32_t *sync_k = h->trunk_sync + size_t(k) * h->trunk_sync_stride;
+        const bool mlp_counts = fused_ok && trunk_counts_tiles((long long)n * T * P, h->use_pair_trunk) && h->tail_fill;
+        if (h->dw_tma_ok) CU_TRY(launch_dwconv3x3_tma(h->tm_dw, h->fb, tb.dw_w, tb.dw_b, n * T, h->h, h->w, Ct, st, h->tail_fill ? sync_k : nullptr,
+                                                      (k > 0 && mlp_counts) ? sync_k - h->trunk_sync_stride + 1 : nullptr));
         else CU_TRY(launch_dwconv3x3(h->fa, h->fb, tb.dw_w, tb.dw_b, n * T, h->h, h->w, Ct, st));
         if (launches) ++*launches;
         if (sg && sg->dw) { cudaEventRecord(sg->dw[2 * k], st); }
-        if (h->use_fused_trunk && tb.fused.ok && !h->force_generic) {
-            CU_TRY(launch_trunk_mlp(tb.fused, tb.pw1, tb.pw2, h->fa, h->fa, (long long)n * T * P, h->num_sms, h->use_pair_trunk, st));
+        if (fused_ok) {
+            CU_TRY(launch_trunk_mlp(tb.fused, tb.pw1, tb.pw2, h->fa, h->fa, (long long)n * T * P, h->num_sms, h->use_pair_trunk, st,
+                                    mlp_counts ? sync_k + 1 : nullptr));
             if (launches) ++*launches;
             continue;
         }
@@ -267,6 +278,11 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
         for (int b = 0; ok && b < 2; ++b) ok = make_act_map(h, h->am_ymu[b], h->ymu[b], n, h->h, h->w, h->mu_net[0].c_in, false, 1);
         if (ok && (!h->am_ymu[0].ok || !h->mu_net[0].use_tc || h->force_generic))
             return fail(h, UFNVC_E_BAD_CONFIG, "mu_steps == 4 needs the tensor-core conv path (c_y % 32 == 0, UFNVC_FORCE_GENERIC unset)");
+    }
+    h->trunk_sync_stride = size_t(((long long)n * T * h->h * h->w + 127) / 128 + 4);
+    {
+        const char *tf = std::getenv("UFNVC_TAIL_FILL");              // 0: whole-grid waits and static tile striding
+        h->tail_fill = !(tf && tf[0] == '0');
     }
     h->dw_tma_ok = false;
     {

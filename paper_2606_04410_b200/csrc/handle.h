@@ -77,6 +77,11 @@ struct ufnvc_handle {
     ufnvc::FinalMaps final_is;           // A9 input-stationary kernel (env UFNVC_FINAL_IS=0 disables)
     CUtensorMap tm_dw;                   // fa as the depthwise kernel reads it: box {64 ch, 10, 10}
     bool dw_tma_ok = false;
+    // per trunk block: [0] = the depthwise kernel's dynamic tile counter, [1 ..] = one completion counter per 128-pixel tile of
+    // the trunk MLP kernel (8 epilogue warps each); zeroed at the start of every call (tail filling)
+    uint32_t *trunk_sync = nullptr;
+    size_t trunk_sync_stride = 0;
+    bool tail_fill = true;
     ActMap am_xs, am_yhat, am_fa, am_fb, am_hidden, am_stage[3], am_ymu[2];
 
     // GPU rANS encoder scratch (NEXT-4), allocated by the first ufnvc_encode_chunk_dev call

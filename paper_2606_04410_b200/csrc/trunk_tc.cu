@@ -41,6 +41,7 @@ struct TrunkParams {
     const float *b1, *b2;                // [hidden], [256]
     const bf16 *x;                       // residual input  [n_px][256]
     bf16 *out;                           // [n_px][256] (may alias x: a tile reads its own rows before writing them)
+    uint32_t *tile_done;                 // optional: [n_tiles] counters, +1 per epilogue warp (8 per tile) once its rows are written
 };
 
 // barrier slots (8 bytes each) from kOffBar
@@ -587,6 +588,9 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(oempty_l);
+            // tail filling: the depthwise kernel of the next trunk block polls these counters instead of waiting for the whole
+            // grid (the __syncwarp above orders every lane's stores before lane 0's release)
+            if (p.tile_done && lane == 0) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p.tile_done + tile) : "memory");
         }
     }
 
@@ -623,10 +627,13 @@ bool trunk_make_maps(TrunkMaps &m, const bf16 *d_base, long long n_px, const Con
     return true;
 }
 
+bool trunk_counts_tiles(long long n_px, bool pair) { return pair && (n_px + kTM - 1) / kTM >= 2; }
+
 cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const ConvLayer &pw2, const bf16 *x, bf16 *out, long long n_px,
-                             int num_sms, bool pair, cudaStream_t st)
+                             int num_sms, bool pair, cudaStream_t st, uint32_t *tile_done)
 {
     TrunkParams p{};
+    p.tile_done = tile_done;
     p.n_px = int(n_px);
     p.n_tiles = int((n_px + kTM - 1) / kTM);
     p.n_chunks = pw1.n / kHC;

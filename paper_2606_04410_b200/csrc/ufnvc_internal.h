@@ -110,7 +110,7 @@ cudaError_t launch_mu_prep(const int16_t *sym, const float *mu0, bf16 *ymu0, bf1
                            cudaStream_t st);
 
 cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
-                                 int C, cudaStream_t st);   // tm_in: NHWC map of `in` with box {64, 10, 10, 1}
+                                 int C, cudaStream_t st, uint32_t *sched = nullptr, const uint32_t *dep_flags = nullptr);   // tm_in: NHWC map of `in` with box {64, 10, 10, 1}
 
 // fp64 hyper-decoder (A1 + A2), R12: the scale decision is taken in double on both sides.
 struct HyperLayer {
@@ -207,7 +207,9 @@ struct TrunkMaps {
 };
 bool trunk_make_maps(TrunkMaps &m, const bf16 *d_base, long long n_px, const ConvLayer &pw1, const ConvLayer &pw2, std::string &err);
 cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const ConvLayer &pw2, const bf16 *x, bf16 *out, long long n_px,
-                             int num_sms, bool pair, cudaStream_t st);
+                             int num_sms, bool pair, cudaStream_t st, uint32_t *tile_done = nullptr);
+// true if launch_trunk_mlp(..., pair, ...) runs the CTA-pair kernel, the one that counts finished tiles in tile_done
+bool trunk_counts_tiles(long long n_px, bool pair);
 
 // rANS symbol search: a 64-slot LUT bucket holds 1.2 binary-search steps (warp maximum, measured law) against 2.4 for 256 slots
 constexpr int kLutShift = 6, kLutBuckets = 65536 >> kLutShift;
