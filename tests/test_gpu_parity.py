@@ -125,6 +125,28 @@ def test_plain_entry_point_equals_ex_and_is_deterministic(decoders):
     assert torch.equal(a, d)
 
 
+def test_tail_filling_off_gives_bit_identical_frames(decoders, monkeypatch):
+    """The trunk's per-tile waits (depthwise tiles start on the MLP kernel's tile counters, dynamic tile claims) only change
+    WHEN a tile runs: frames must equal those of whole-grid waits with static striding bit for bit, call after call."""
+    from paper_2606_04410_b200 import binding
+    dec, case = decoders("cfg3-crop")
+    z, bits, off = gpu_inputs(case)
+    ref = dec.chunk_decode(z, bits, off).clone()
+    monkeypatch.setenv("UFNVC_TAIL_FILL", "0")          # read when the handle is created
+    plain = binding.ChunkDecoder(case["cfg"])
+    monkeypatch.delenv("UFNVC_TAIL_FILL")
+    try:
+        plain.load_weights(case["weights"])
+        a = plain.chunk_decode(z, bits, off).clone()
+        torch.cuda.synchronize()
+        assert plain.get_status() == 0
+        assert torch.equal(a, ref)
+        for _ in range(5):                              # tile claims differ from call to call; results must not
+            assert torch.equal(dec.chunk_decode(z, bits, off), ref)
+    finally:
+        plain.destroy()
+
+
 def test_whole_call_is_cuda_graph_capturable(decoders):
     """ufnvc_chunk_decode only enqueues (no sync, no allocation): the 25-kernel sequence can be captured once in a CUDA
     graph and replayed; the replay's frames equal the direct call's bit for bit."""
