@@ -103,15 +103,20 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
         if ((i & 255) != 255) cf[i] = h->cdf32[i] | ((h->cdf32[i + 1] - h->cdf32[i]) << 16);
 
     const size_t n = size_t(h->max_chunks), P = size_t(h->h) * h->w, Pz = size_t(h->h_z) * h->w_z, T = size_t(cfg->T);
-    bool ok = dev_alloc(h, h->d_cf, cf.size()) && dev_alloc(h, h->d_lut, lut.size()) && dev_alloc(h, h->d_status, 1) &&
+    bool ok = dev_alloc(h, h->d_cf, cf.size()) && dev_alloc(h, h->d_lut, lut.size()) &&
               dev_alloc(h, h->hx0, n * Pz * cfg->c_z) && dev_alloc(h, h->hx1, n * Pz * cfg->c_hyper) &&
               dev_alloc(h, h->hx2, n * Pz * cfg->c_hyper) && dev_alloc(h, h->xs, n * Pz * 2 * cfg->c_hyper) &&
-              dev_alloc(h, h->fix_list, n * P * cfg->c_y) && dev_alloc(h, h->fix_count, 1) && dev_alloc(h, h->hpart, 9 * n * Pz * cfg->c_hyper) && dev_alloc(h, h->mu, n * P * cfg->c_y) &&
+              dev_alloc(h, h->fix_list, n * P * cfg->c_y) && dev_alloc(h, h->hpart, 9 * n * Pz * cfg->c_hyper) && dev_alloc(h, h->mu, n * P * cfg->c_y) &&
               dev_alloc(h, h->lnscale, n * P * cfg->c_y) && dev_alloc(h, h->idx, n * P * cfg->c_y) &&
               dev_alloc(h, h->yhat, n * P * cfg->c_y) && dev_alloc(h, h->fa, n * T * P * cfg->c_trunk) &&
               dev_alloc(h, h->fb, n * T * P * cfg->c_trunk) &&
-              dev_alloc(h, h->trunk_sync, size_t(cfg->n_trunk_blocks > 0 ? cfg->n_trunk_blocks : 1) * ((n * T * P + 127) / 128 + 4)) &&
+              dev_alloc(h, h->zero_block, 4 + size_t(cfg->n_trunk_blocks > 0 ? cfg->n_trunk_blocks : 1) * ((n * T * P + 127) / 128 + 4)) &&
               dev_alloc(h, h->hidden, cfg->n_trunk_blocks ? n * T * P * cfg->c_trunk * cfg->trunk_expand : 1);
+    if (ok) {      // everything a call clears up front sits in one block so that ONE memset node does it (decode.cu run())
+        h->zero_words = 4 + size_t(cfg->n_trunk_blocks > 0 ? cfg->n_trunk_blocks : 1) * ((n * T * P + 127) / 128 + 4);
+        h->d_status = h->zero_block; h->fix_count = h->zero_block + 1; h->trunk_sync = h->zero_block + 4;
+        ok = cudaMemset(h->zero_block, 0, h->zero_words * 4) == cudaSuccess;
+    }
     if (ok && cfg->mu_steps == 4) {
         const size_t cs = (3 * size_t(cfg->c_y) + 63) / 64 * 64;       // [r | mu used | mu0 | zero pad], see weights.cu mu_net
         ok = dev_alloc(h, h->ymu[0], n * P * cs) && dev_alloc(h, h->ymu[1], n * P * cs) && dev_alloc(h, h->sym, n * P * cfg->c_y) &&

@@ -45,11 +45,16 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     const int P = h->h * h->w, Pz = h->h_z * h->w_z;
     const size_t ne = size_t(n) * P * c.c_y;
 
-    // the status word is cleared up front (nothing before the rANS kernel touches it) so that no memset node sits between
-    // the hyper head's last kernel and the rANS kernel, which is launched with programmatic stream serialization
-    if (!entropy_params_only && !h->keep_status) CU_TRY(cudaMemsetAsync(h->d_status, 0, 4, st));
-    if (!entropy_params_only && frames && c.n_trunk_blocks > 0 && h->tail_fill)
-        CU_TRY(cudaMemsetAsync(h->trunk_sync, 0, size_t(c.n_trunk_blocks) * h->trunk_sync_stride * 4, st));
+    // everything the call clears (status word, the head's fix-up count, the trunk's tile counters) is cleared up front by ONE
+    // memset, so that no memset node sits between kernels launched with programmatic stream serialization
+    {
+        // [status | fix_count | pad | trunk counters]: the status word is skipped when an earlier call's status is kept, the
+        // trunk counters when this call does not reach the trunk
+        const bool keep = entropy_params_only || h->keep_status;
+        const bool trunk = !entropy_params_only && frames && c.n_trunk_blocks > 0 && h->tail_fill;
+        const size_t words = trunk ? 4 + size_t(c.n_trunk_blocks) * h->trunk_sync_stride : 4;
+        CU_TRY(cudaMemsetAsync(h->zero_block + (keep ? 1 : 0), 0, (words - (keep ? 1 : 0)) * 4, st));
+    }
     // ---- A1 + A2: hyper-decoder in fp64 -> mu, ln sigma, bucket index ----
     const bool need_hyper = entropy_params_only || !idx_ovr || !mu_ovr || (taps && (taps->mu || taps->lnscale));
     mark(sg, st);
@@ -61,7 +66,6 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
             // layer 1 also emits the bf16 hi|mid split; the head runs on tensor cores; elements whose ln sigma lands within
             // flag_u of a bucket edge are re-decided in fp64 (identical decisions to the all-fp64 path, R12)
             CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, h->hpart, n, h->h_z, h->w_z, st, h->xs));
-            CU_TRY(cudaMemsetAsync(h->fix_count, 0, 4, st));
             const double step = (hp.ln_hi - hp.ln_lo) / double(c.n_buckets - 1 > 0 ? c.n_buckets - 1 : 1);
             EpiParams E{};
             E.mode = EPI_HEAD; E.act = ACT_NONE;

@@ -80,6 +80,8 @@ struct ufnvc_handle {
     // per trunk block: [0] = the depthwise kernel's dynamic tile counter, [1 ..] = one completion counter per 128-pixel tile of
     // the trunk MLP kernel (8 epilogue warps each); zeroed at the start of every call (tail filling)
     uint32_t *trunk_sync = nullptr;
+    uint32_t *zero_block = nullptr;      // [0] = status word, [1] = fix_count, [4 ..] = trunk_sync: cleared by one memset per call
+    size_t zero_words = 0;
     size_t trunk_sync_stride = 0;
     bool tail_fill = true;
     ActMap am_xs, am_yhat, am_fa, am_fb, am_hidden, am_stage[3], am_ymu[2];

@@ -12,6 +12,8 @@ namespace ufnvc {
 
 __global__ void z_to_f64_kernel(const int16_t *__restrict__ z, double *__restrict__ out, int n_chunks, int c_z, int pz)
 {
+    asm volatile("griddepcontrol.wait;" ::: "memory");              // PDL: launched early, the predecessor's output is complete from here on
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     // z planar [n][c][pz] -> out NHWC [n][pz][c]
     const long long total = (long long)n_chunks * c_z * pz;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
@@ -138,6 +140,8 @@ __global__ void __launch_bounds__(256) hyper_conv_fast_kernel(const double *__re
 {
     __shared__ __align__(16) double As[2][FK][FM + FPAD];
     __shared__ __align__(16) double Bs[2][FK][FN];
+    asm volatile("griddepcontrol.wait;" ::: "memory");              // PDL: launched early, the predecessor's output is complete from here on
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     const int pz = hz * wz;
     const int M = n_img * pz;
     const int m0 = blockIdx.x * FM, n0 = blockIdx.y * FN;
@@ -221,6 +225,8 @@ __global__ void __launch_bounds__(256) hyper_conv_fast_kernel(const double *__re
 __global__ void hyper_reduce_kernel(const double *__restrict__ part, const double *__restrict__ bias, double *__restrict__ out,
                                     long long MN, int n_out)
 {
+    asm volatile("griddepcontrol.wait;" ::: "memory");              // PDL: launched early, the predecessor's output is complete from here on
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < MN; i += (long long)gridDim.x * blockDim.x) {
         double v = part[i];
 #pragma unroll
@@ -234,7 +240,7 @@ cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z
 {
     const long long total = (long long)n_chunks * c_z * pz;
     const int blocks = int((total + 255) / 256 < 1184 ? (total + 255) / 256 : 1184);
-    z_to_f64_kernel<<<blocks, 256, 0, st>>>(z, out, n_chunks, c_z, pz);
+    return launch_pdl(z_to_f64_kernel, unsigned(blocks), 256u, 0, st, 1, z, out, n_chunks, c_z, pz);
     return cudaGetLastError();
 }
 
@@ -242,6 +248,8 @@ cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z
 __global__ void hyper_reduce_split_kernel(const double *__restrict__ part, const double *__restrict__ bias, double *__restrict__ out,
                                           bf16 *__restrict__ xs, long long MN, int n_out)
 {
+    asm volatile("griddepcontrol.wait;" ::: "memory");              // PDL: launched early, the predecessor's output is complete from here on
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < MN; i += (long long)gridDim.x * blockDim.x) {
         double v = part[i];
 #pragma unroll
@@ -320,11 +328,11 @@ cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out
     const int M = n_img * hz * wz;
     if (fast_ok(L) && part) {                   // split over the 9 taps, then a deterministic reduce + bias + ReLU
         dim3 grid((M + FM - 1) / FM, (L.n + FN - 1) / FN, 9);
-        hyper_conv_fast_kernel<true><<<grid, 256, 0, st>>>(in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e, part);
+        if (cudaError_t le = launch_pdl_grid(hyper_conv_fast_kernel<true>, grid, 256u, st, in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e, part)) return le;
         const long long MN = (long long)M * L.n;
         const int blocks = int((MN + 255) / 256 < 1184 ? (MN + 255) / 256 : 1184);
-        if (xs) hyper_reduce_split_kernel<<<blocks, 256, 0, st>>>(part, L.bias, out, xs, MN, L.n);
-        else hyper_reduce_kernel<<<blocks, 256, 0, st>>>(part, L.bias, out, MN, L.n);
+        if (xs) { if (cudaError_t le = launch_pdl(hyper_reduce_split_kernel, unsigned(blocks), 256u, 0, st, 1, part, L.bias, out, xs, MN, L.n)) return le; }
+        else if (cudaError_t le = launch_pdl(hyper_reduce_kernel, unsigned(blocks), 256u, 0, st, 1, part, L.bias, out, MN, L.n)) return le;
         return cudaGetLastError();
     }
     dim3 grid((M + HM - 1) / HM, (L.n + HN - 1) / HN);
@@ -357,7 +365,7 @@ cudaError_t launch_hyper_head(const HyperLayer &L, const double *in, int n_img, 
     const int M = n_img * hz * wz;
     if (fast_ok(L)) {
         dim3 grid((M + FM - 1) / FM, (L.n + FN - 1) / FN);
-        hyper_conv_fast_kernel<false><<<grid, 256, 0, st>>>(in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e, nullptr);
+        if (cudaError_t le = launch_pdl_grid(hyper_conv_fast_kernel<false>, grid, 256u, st, in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e, (double *)nullptr)) return le;
         return cudaGetLastError();
     }
     dim3 grid((M + HM - 1) / HM, (L.n + HN - 1) / HN);
