@@ -266,8 +266,17 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
     // tcgen05 path: weight descriptors + descriptors of the (fixed) workspace activations
     const ufnvc_config &c = h->cfg;
     std::string err;
-    bool ok = tc_make_weight_tmap(h->xframe, err);
-    if (h->hybrid_head) ok = ok && tc_make_weight_tmap(h->head_tc, err);
+    const char *xbn = std::getenv("UFNVC_XFRAME_BN");               // tuning knob: N tile of the A5 cross-frame conv (0 = widest)
+    bool ok = tc_make_weight_tmap(h->xframe, err, xbn ? std::atoi(xbn) : 0);
+    if (h->hybrid_head) {
+        // N tile of the hyper head conv: the z map is tiny (510 pixels at 1080p = 4-6 M tiles), so with the widest N tile
+        // (256) fewer tiles than SMs exist and each CTA runs one long tile with its epilogue exposed; 128 doubles the tile
+        // count (measured at 1080p: A1+A2 98 -> 93 us; 64 and 32 are slower again).  UFNVC_HEAD_BN overrides.
+        const char *bn = std::getenv("UFNVC_HEAD_BN");
+        const long long m_tiles = ((long long)h->max_chunks * h->h_z * h->w_z + 127) / 128;
+        const int auto_bn = (h->head_tc.n_pad % 128 == 0 && m_tiles * (h->head_tc.n_pad / 256) < h->num_sms) ? 128 : 0;
+        ok = ok && tc_make_weight_tmap(h->head_tc, err, bn ? std::atoi(bn) : auto_bn);
+    }
     for (auto &tb : h->trunk) ok = ok && tc_make_weight_tmap(tb.pw1, err) && tc_make_weight_tmap(tb.pw2, err);
     for (int s = 0; s < 4; ++s) ok = ok && tc_make_weight_tmap(h->dec[s], err);
     for (int k = 0; k < 3 && c.mu_steps == 4; ++k) ok = ok && tc_make_weight_tmap(h->mu_net[k], err);
