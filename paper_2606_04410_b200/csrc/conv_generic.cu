@@ -486,7 +486,7 @@ static cudaError_t launch_dw_cols(const CUtensorMap &tm_in, bf16 *out, const flo
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    return launch_pdl(dwconv3x3_cols_kernel<CC>, grid, CC + 32, smem, st, 1, tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, sched, dep, 8u);
+    return launch_pdl(dwconv3x3_cols_kernel<CC>, grid, CC + 32, smem, st, 1, tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, sched, dep, kTrunkTileSignals);
 }
 
 cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,

@@ -30,6 +30,7 @@ constexpr int kC = 256;                  // trunk width: K of GEMM1, N of GEMM2
 constexpr int kHC = 128;                 // hidden columns per chunk
 constexpr int kTM = 128;                 // pixels per tile
 constexpr int kTrunkThreads = 320;
+static_assert(kTrunkThreads / 32 - 2 == int(kTrunkTileSignals), "one tile_done increment per epilogue warp (warps 2..9)");
 constexpr int kWStages = 3;
 constexpr uint32_t kSlab = 16384;        // 128 rows x 128 B
 constexpr uint32_t kWStage = 32768;
