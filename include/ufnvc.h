@@ -12,7 +12,8 @@
  *
  * Conventions
  *   - plain pointers and sizes only; "_dev" = device pointer (cudaMalloc / torch CUDA tensor), "_host" = host.
- *   - every function returns 0 (UFNVC_OK) or a negative ufnvc_status; no exceptions cross the ABI; no globals.
+ *   - every function returns 0 (UFNVC_OK) or a negative ufnvc_status; no exceptions cross the ABI; no globals, no
+ *     environment variables: everything that selects a code path is a field of ufnvc_config.
  *   - a handle is used from one host thread and one CUDA stream at a time; it owns weights, CDF tables,
  *     TMA descriptors and a workspace sized at create for max_chunks_per_call.
  *   - ufnvc_chunk_decode only ENQUEUES work on `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy
@@ -69,7 +70,20 @@ typedef struct ufnvc_config {
     int32_t mu_steps;            /* 1: the head's mean serves every element (A4); 4: four-step progressive means
                                   * (R21) -- needs c_y % 32 == 0 and the mu.{1,2,3}
                                   * tensors in the blob; three extra conv launches between A4 and A5 */
+    uint32_t debug_flags;        /* 0 = the default (fastest) kernels.  OR of UFNVC_DBG_*: each bit swaps one GPU kernel or
+                                  * launch mechanism for its slower cross-check variant (never a CPU path).  Per handle;
+                                  * the library reads no environment variable and keeps no process-wide state. */
 } ufnvc_config;
+
+/* ufnvc_config.debug_flags: A/B and cross-check switches (tests/test_gpu_parity.py runs every one against the oracle) */
+#define UFNVC_DBG_FORCE_GENERIC 0x01u   /* every dense conv on the CUDA-core kernel (no tcgen05), all-fp64 hyper head, unfused trunk */
+#define UFNVC_DBG_NO_PDL 0x02u          /* plain stream order instead of programmatic dependent launch */
+#define UFNVC_DBG_NO_TAIL_FILL 0x04u    /* trunk: whole-grid waits and static tile striding instead of per-tile counters */
+#define UFNVC_DBG_FP64_HEAD 0x08u       /* hyper head (A1 layer 3 + A2) entirely on the FP64 pipe instead of tensor cores + fix-up */
+#define UFNVC_DBG_NO_CTA_PAIRS 0x10u    /* single-CTA tcgen05 kernels (cta_group::1) for A7 and A8 instead of CTA pairs */
+#define UFNVC_DBG_UNFUSED_TRUNK 0x20u   /* A7 as two 1x1 conv launches with the hidden tensor in HBM */
+#define UFNVC_DBG_GENERIC_FINAL 0x40u   /* A9 on the output-stationary halo conv kernel instead of the input-stationary one */
+#define UFNVC_DBG_PLAIN_DEPTHWISE 0x80u /* A6 on the register-only kernel (no TMA staging, no tile counters) */
 
 /* Optional device buffers that receive intermediates of ufnvc_chunk_decode_ex (parity/debug; any may be NULL).
  * Layouts are the library's own: channels-last. */

@@ -302,24 +302,26 @@ def progressive_means(orc: Oracle, cfg, weights, mu0, sym):
     return yhat, mu
 
 
-def synthesis(orc: Oracle, cfg, weights, yhat, keep=False):
+def synthesis(orc: Oracle, cfg, weights, yhat, keep=False, only_frames=None):
     """O6..O9: cross-frame unfold, shared trunk of DC blocks, T frame-specific
-    decoders, clamp + crop.  yhat [C_y][h][w].  Returns frames [T][3][height][width] (+ taps)."""
+    decoders, clamp + crop.  yhat [C_y][h][w].  Returns frames [T][3][height][width] (+ taps).
+    only_frames: frame indices to compute (the T frames are independent after O6, PAPER.md:85 "operating in parallel");
+    the others are left as NaN -- used by the full-size parity tests of configs 4 and 5 to bound the oracle's time."""
     taps = {}
     f0 = orc.conv2d(yhat, weights["xframe.w"], weights["xframe.b"])            # O6: [T*C_t][h][w]
-    frames = np.empty((cfg.T, 3, cfg.height, cfg.width), orc.dt)
+    frames = np.full((cfg.T, 3, cfg.height, cfg.width), np.nan, orc.dt)
     if keep:
         taps["F0"] = f0.reshape(cfg.T, cfg.c_trunk, *f0.shape[1:]).copy()
         taps["trunk"] = []
         taps["stage"] = [[] for _ in range(cfg.T)]
-    for t in range(cfg.T):
+    for t in (range(cfg.T) if only_frames is None else only_frames):
         x = np.ascontiguousarray(f0[t * cfg.c_trunk:(t + 1) * cfg.c_trunk])
         for k in range(cfg.n_trunk_blocks):                                    # O7, same weights for every t [R15]
             d = orc.dwconv3x3(x, weights[f"trunk.{k}.dw.w"], weights[f"trunk.{k}.dw.b"])
             e = orc.gelu(orc.conv2d(d, weights[f"trunk.{k}.pw1.w"], weights[f"trunk.{k}.pw1.b"]))
             x = x + orc.conv2d(e, weights[f"trunk.{k}.pw2.w"], weights[f"trunk.{k}.pw2.b"])
         if keep:
-            taps["trunk"].append(x.copy())
+            taps["trunk"].append(x.copy())           # (indexed by position in only_frames when that is given)
         for s in range(4):                                                     # O8 [R10]
             a = orc.conv2d(x, weights[f"dec.{t}.{s}.w"], weights[f"dec.{t}.{s}.b"])
             if s < 3:

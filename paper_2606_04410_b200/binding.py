@@ -26,7 +26,8 @@ class ufnvc_config(C.Structure):
                 ("n_trunk_blocks", C.c_int32), ("trunk_expand", C.c_int32), ("dec_channels", C.c_int32 * 5),
                 ("n_buckets", C.c_int32), ("scale_min", C.c_double), ("scale_max", C.c_double),
                 ("rows_per_substream", C.c_int32), ("lanes_per_substream", C.c_int32),
-                ("max_chunks_per_call", C.c_int32), ("weight_dtype", C.c_int32), ("mu_steps", C.c_int32)]
+                ("max_chunks_per_call", C.c_int32), ("weight_dtype", C.c_int32), ("mu_steps", C.c_int32),
+                ("debug_flags", C.c_uint32)]
 
 
 class ufnvc_taps(C.Structure):
@@ -75,7 +76,12 @@ EXPORTS = ("ufnvc_create", "ufnvc_destroy", "ufnvc_load_weights", "ufnvc_chunk_d
            "ufnvc_decode_z", "ufnvc_chunk_decode_bytes", "ufnvc_get_z_prior_index", "ufnvc_encode_z", "ufnvc_encode_chunk_dev")
 
 
-def make_config(cfg, max_chunks: int | None = None) -> ufnvc_config:
+# ufnvc_config.debug_flags (include/ufnvc.h)
+DBG = dict(force_generic=0x01, no_pdl=0x02, no_tail_fill=0x04, fp64_head=0x08, no_cta_pairs=0x10, unfused_trunk=0x20,
+           generic_final=0x40, plain_depthwise=0x80)
+
+
+def make_config(cfg, max_chunks: int | None = None, debug_flags: int = 0) -> ufnvc_config:
     """cfg: any object with the ufnvc_config field names (e.g. synth.ChunkConfig)."""
     c = ufnvc_config()
     c.struct_size = C.sizeof(ufnvc_config)
@@ -85,6 +91,7 @@ def make_config(cfg, max_chunks: int | None = None) -> ufnvc_config:
     c.dec_channels = (C.c_int32 * 5)(*cfg.dec_channels)
     c.max_chunks_per_call = max_chunks if max_chunks is not None else getattr(cfg, "n_chunks", 1)
     c.mu_steps = getattr(cfg, "mu_steps", 1)
+    c.debug_flags = debug_flags
     return c
 
 
@@ -127,13 +134,13 @@ def _ptr(t):
 class ChunkDecoder:
     """One ufnvc_handle.  Methods carry the names of the C entry points they call."""
 
-    def __init__(self, cfg, max_chunks: int | None = None, device: int = 0):
+    def __init__(self, cfg, max_chunks: int | None = None, device: int = 0, debug_flags: int = 0):
         if not torch.cuda.is_available():
             raise UfnvcError("ufnvc needs a CUDA device (sm_100); there is no CPU fallback")
         torch.cuda.set_device(device)
         self.device = torch.device("cuda", device)
         self.cfg = cfg
-        self.c = make_config(cfg, max_chunks)
+        self.c = make_config(cfg, max_chunks, debug_flags)
         self.H = -(-cfg.height // 32) * 32
         self.W = -(-cfg.width // 32) * 32
         self.h, self.w = self.H // 16, self.W // 16

@@ -49,6 +49,18 @@ int validate(const ufnvc_config &c, std::string &why)
     BAD(c.weight_dtype != 0 && c.weight_dtype != 1, "weight_dtype must be 0 or 1");
     BAD(c.mu_steps != 1 && c.mu_steps != 4, "mu_steps must be 1 or 4");
     BAD(c.mu_steps == 4 && c.c_y % 32, "mu_steps == 4 needs c_y % 32 == 0 (the mean convs run on tensor cores only)");
+    BAD(c.debug_flags & ~0xFFu, "unknown debug_flags bit");
+    BAD(c.mu_steps == 4 && (c.debug_flags & UFNVC_DBG_FORCE_GENERIC), "mu_steps == 4 has no CUDA-core variant");
+    // every kernel indexes latent elements and activation pixels with 32-bit integers (byte offsets are 64-bit)
+    {
+        const long long Hp = (c.height + 31) / 32 * 32, Wp = (c.width + 31) / 32 * 32, P = (Hp / 16) * (Wp / 16);
+        const long long n = c.max_chunks_per_call;
+        long long cmax = c.c_trunk * (long long)c.trunk_expand;
+        BAD(n * P * c.c_y >= (1ll << 31), "max_chunks_per_call * h * w * c_y must stay below 2^31");
+        BAD(n * c.T * P * cmax >= (1ll << 31), "max_chunks_per_call * T * h * w * c_trunk * trunk_expand must stay below 2^31");
+        for (int s = 1; s <= 3; ++s) BAD(n * c.T * (P << (2 * s)) * c.dec_channels[s] >= (1ll << 31), "a decoder stage tensor must stay below 2^31 elements");
+        BAD(n * c.T * 3 * (long long)c.height * c.width >= (1ll << 31), "the frame tensor must stay below 2^31 elements");
+    }
 #undef BAD
     return UFNVC_OK;
 }
@@ -77,22 +89,28 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     h->n_sub = (h->h + cfg->rows_per_substream - 1) / cfg->rows_per_substream;
     h->n_sub_z = (h->h_z + cfg->rows_per_substream - 1) / cfg->rows_per_substream;
     h->max_chunks = cfg->max_chunks_per_call;
-    const char *fg = std::getenv("UFNVC_FORCE_GENERIC");
-    h->force_generic = fg && fg[0] == '1';
-    const char *hl = std::getenv("UFNVC_HALO");
-    h->use_halo = !(hl && hl[0] == '0');
-    const char *ft = std::getenv("UFNVC_FUSED_TRUNK");
-    h->use_fused_trunk = !(ft && ft[0] == '0');
-    const char *pc = std::getenv("UFNVC_PAIR_CONV");
-    h->use_pair_conv = !(pc && pc[0] == '0');
-    const char *pt = std::getenv("UFNVC_PAIR_TRUNK");
-    h->use_pair_trunk = !(pt && pt[0] == '0');
-
-    const char *hy = std::getenv("UFNVC_HYBRID_HEAD");
-    h->hybrid_head = !(hy && hy[0] == '0') && cfg->weight_dtype == 1 && cfg->c_y % 32 == 0 && cfg->c_hyper % 32 == 0 &&
+    const uint32_t dbg = cfg->debug_flags;
+    h->force_generic = dbg & UFNVC_DBG_FORCE_GENERIC;
+    h->use_fused_trunk = !(dbg & UFNVC_DBG_UNFUSED_TRUNK);
+    h->use_pair_conv = h->use_pair_trunk = !(dbg & UFNVC_DBG_NO_CTA_PAIRS);
+    h->pdl = !(dbg & UFNVC_DBG_NO_PDL);
+    h->tail_fill = !(dbg & UFNVC_DBG_NO_TAIL_FILL);
+    h->use_final_is = !(dbg & UFNVC_DBG_GENERIC_FINAL);
+    h->use_dw_tma = !(dbg & UFNVC_DBG_PLAIN_DEPTHWISE);
+    h->hybrid_head = !(dbg & UFNVC_DBG_FP64_HEAD) && cfg->weight_dtype == 1 && cfg->c_y % 32 == 0 && cfg->c_hyper % 32 == 0 &&
                      !h->force_generic;
-
-    if (const char *fu = std::getenv("UFNVC_HEAD_FLAG_U")) h->head_flag_u = std::atof(fu);
+    // Error model of the tensor-core head (R12): ln sigma = sum of K = 9 * 2 c_hyper exact bf16 x bf16 products
+    // accumulated in fp32.  (i) the 2-term split drops |x - hi - mid| <= 2^-18 |x| (two round-to-nearest steps of 8
+    // bits); (ii) K fp32 additions: probabilistic rounding bound lambda sqrt(K) 2^-24 sum|terms| with lambda = 3.
+    // sum |w||x| <= |w|_2 |x|_2 (Cauchy-Schwarz), so |error| <= kappa |w row|_2 |x patch|_2.
+    h->head_kappa = std::ldexp(1.0, -18) + 3.0 * std::sqrt(18.0 * cfg->c_hyper) * std::ldexp(1.0, -24);
+    // function attributes are per device: configure every kernel for the device this handle lives on
+    if (configure_rans_kernels() != cudaSuccess || configure_depthwise_kernels() != cudaSuccess || configure_conv_tc_kernels() != cudaSuccess ||
+        configure_trunk_kernels() != cudaSuccess || configure_final_kernels() != cudaSuccess) {
+        cudaGetLastError();
+        delete h;
+        return UFNVC_E_CUDA;
+    }
 
     // O3 tables + search accelerator
     build_cdf_tables(cfg->n_buckets, cfg->scale_min, cfg->scale_max, h->cdf32);
@@ -105,7 +123,7 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     const size_t n = size_t(h->max_chunks), P = size_t(h->h) * h->w, Pz = size_t(h->h_z) * h->w_z, T = size_t(cfg->T);
     bool ok = dev_alloc(h, h->d_cf, cf.size()) && dev_alloc(h, h->d_lut, lut.size()) &&
               dev_alloc(h, h->hx0, n * Pz * cfg->c_z) && dev_alloc(h, h->hx1, n * Pz * cfg->c_hyper) &&
-              dev_alloc(h, h->hx2, n * Pz * cfg->c_hyper) && dev_alloc(h, h->xs, n * Pz * 2 * cfg->c_hyper) &&
+              dev_alloc(h, h->hx2, n * Pz * cfg->c_hyper) && dev_alloc(h, h->xs, n * Pz * 2 * cfg->c_hyper) && dev_alloc(h, h->xnorm2, n * Pz) &&
               dev_alloc(h, h->fix_list, n * P * cfg->c_y) && dev_alloc(h, h->hpart, 9 * n * Pz * cfg->c_hyper) && dev_alloc(h, h->mu, n * P * cfg->c_y) &&
               dev_alloc(h, h->lnscale, n * P * cfg->c_y) && dev_alloc(h, h->idx, n * P * cfg->c_y) &&
               dev_alloc(h, h->yhat, n * P * cfg->c_y) && dev_alloc(h, h->fa, n * T * P * cfg->c_trunk) &&
@@ -143,6 +161,7 @@ extern "C" int ufnvc_destroy(ufnvc_handle *h)
     if (!h) return UFNVC_E_INVALID_ARG;
     cudaDeviceSynchronize();
     for (void *p : h->allocs) cudaFree(p);
+    for (void *p : h->weight_allocs) cudaFree(p);
     if (h->ev_made) for (auto &e : h->ev) cudaEventDestroy(e);
     for (auto &e : h->ev_dw) cudaEventDestroy(e);
     delete h;
@@ -233,6 +252,8 @@ extern "C" long ufnvc_encode_chunk(const ufnvc_handle *h, const uint8_t *idx_hos
                                    size_t cap, uint32_t *sub_off_host)
 {
     if (!h || !idx_host || !sym_host || !bits_host || !sub_off_host) return UFNVC_E_INVALID_ARG;
+    for (size_t i = 0, e = size_t(h->h) * h->w * h->cfg.c_y; i < e; ++i)
+        if (idx_host[i] >= h->cfg.n_buckets) return UFNVC_E_INVALID_ARG;       // the tables hold n_buckets rows
     size_t pos = 0;
     sub_off_host[0] = 0;
     for (int s = 0; s < h->n_sub; ++s) {

@@ -2,7 +2,6 @@
 // The generic conv serves the shapes the tcgen05 kernel does not take (config 1's 48/32/16-channel layers) and is
 // the on-device cross-check of the tensor-core path.  Activations NHWC bf16, fp32 accumulate.
 //   out[pix][n] = bias[n] + sum_{tap, c} in[pix + tap][c] * w[group][tap][n][c]
-#include <cstdlib>
 #include "epilogue.cuh"
 #include "tc_ptx.cuh"
 #include "ufnvc_internal.h"
@@ -88,7 +87,7 @@ __global__ void __launch_bounds__(256) conv_generic_kernel(const bf16 *__restric
     }
 }
 
-cudaError_t launch_conv_generic(const ConvLayer &L, const ConvProblem &P, const EpiParams &E, cudaStream_t st)
+cudaError_t launch_conv_generic(const ConvLayer &L, const ConvProblem &P, const EpiParams &E, LaunchStream st)
 {
     dim3 grid((P.H * P.W + GM - 1) / GM, (L.n + GN - 1) / GN, P.n_img);
     conv_generic_kernel<<<grid, 256, 0, st>>>(P.in, L.w, L.bias, P.n_img, P.H, P.W, L.c_in, L.n, L.n_pad, L.taps, L.groups, E);
@@ -187,128 +186,16 @@ __global__ void __launch_bounds__(256, 2) dwconv3x3_kernel(const bf16 *__restric
     }
 }
 
-// ---- A6, TMA-staged variant (C a multiple of 64).  One tile = 8 x 8 pixels of one image, all channels: one TMA box
+// ---- A6, TMA-staged kernel (C a multiple of 64).  One tile = 8 x 8 pixels of one image, all channels: one TMA box
 // {64 ch, 10, 10} per 64-channel slab brings the tile plus halo into shared memory (zero-filled outside the image =
 // the conv's zero padding).  The kernel is persistent (two blocks per SM) and double-buffered: the load of a block's
 // next tile is in flight while it computes the current one, so ~100 KB per block are in flight without costing a
 // register -- the register-only kernel above is latency-bound (16 warps/SM, 8 KB of unique loads in flight).
-// Thread (x, c8) then walks down its column with the same rolling 3-row window, reading 3 conflict-free LDS.128 per row.
 constexpr int kDwT = 8;                                   // tile edge (pixels)
 constexpr int kDwHalo = kDwT + 2;
 constexpr uint32_t kDwSlab = ((kDwHalo * kDwHalo * 128 + 1023) / 1024) * 1024;     // 13312 B per 64-channel slab (dense box, no swizzle)
 
-// V = channel PAIRS per thread: 4 (8 channels, LDS.128, C threads) is what is launched; 2 (4 channels, LDS.64, 2 C threads,
-// twice the warps at half the registers) measured 7 % slower on B200 (more address and loop overhead per output).
-template <int V>
-__global__ void __launch_bounds__(V == 4 ? 256 : 512, 2) dwconv3x3_tma_kernel(const __grid_constant__ CUtensorMap tm_in, bf16 *__restrict__ out,
-                                                             const float *__restrict__ w9c, const float *__restrict__ bias,
-                                                             int n_img, int H, int W, int C, int tiles_x, int tiles_y)
-{
-    extern __shared__ __align__(1024) uint8_t dw_smem[];
-    const uint32_t base = (smem_u32(dw_smem) + 1023u) & ~1023u;
-    const int slabs = C >> 6;
-    const uint32_t buf_bytes = uint32_t(slabs) * kDwSlab;
-    const uint32_t bar = base + 2u * buf_bytes;                       // two full barriers, one per buffer
-    const int n_tiles = n_img * tiles_x * tiles_y;
-    auto issue = [&](int t, uint32_t b) {                              // thread 0: TMA the tile + halo into buffer b
-        const int tx = t % tiles_x, r = t / tiles_x;
-        const int ty = r % tiles_y, im = r / tiles_y;
-        mbar_expect_tx(bar + 8u * b, uint32_t(slabs) * (kDwHalo * kDwHalo * 128));
-        for (int s = 0; s < slabs; ++s)
-            tma_load_4d(base + b * buf_bytes + uint32_t(s) * kDwSlab, &tm_in, bar + 8u * b, s * 64, tx * kDwT - 1, ty * kDwT - 1, im);
-    };
-    if (threadIdx.x == 0) {
-        mbar_init(bar, 1);
-        mbar_init(bar + 8, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        if (int(blockIdx.x) < n_tiles) issue(blockIdx.x, 0);
-        if (int(blockIdx.x + gridDim.x) < n_tiles) issue(blockIdx.x + gridDim.x, 1);
-    }
-    constexpr int CH = 2 * V;                                         // channels per thread
-    const int cv = C / CH;
-    const int xl = threadIdx.x / cv, cg = threadIdx.x % cv;           // column of the tile, channel group
-    const int c0 = cg * CH;
-    uint64_t wv[9][V];
-#pragma unroll
-    for (int k = 0; k < 9; ++k) {
-#pragma unroll
-        for (int e = 0; e < V; e += 2) {
-            const float4 q = __ldg(reinterpret_cast<const float4 *>(w9c + k * C + c0 + 2 * e));
-            wv[k][e] = f2_pack(q.x, q.y); wv[k][e + 1] = f2_pack(q.z, q.w);
-        }
-    }
-    // the bias lives in shared memory and is added when a row is written out: that frees 8 registers, which the
-    // compiler otherwise pays for with local-memory spills inside the row loop
-    const uint32_t bias_s = bar + 16u + uint32_t(c0) * 4u;
-    if (xl == 0) {
-#pragma unroll
-        for (int e = 0; e < V; e += 2) {
-            const float4 q = __ldg(reinterpret_cast<const float4 *>(bias + c0 + 2 * e));
-            asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(bias_s + 8u * e), "f"(q.x), "f"(q.y), "f"(q.z), "f"(q.w) : "memory");
-        }
-    }
-    __syncthreads();                                                  // barriers initialised before anyone polls them
-
-    uint32_t it = 0;
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
-        const uint32_t b = it & 1u;
-        const int tx = tile % tiles_x, trow = tile / tiles_x;
-        const int ty = trow % tiles_y, img = trow / tiles_y;
-        const int x0 = tx * kDwT, y0 = ty * kDwT;
-        mbar_wait(bar + 8u * b, (it >> 1) & 1u);
-        const uint32_t slab_base = base + b * buf_bytes + uint32_t(c0 >> 6) * kDwSlab + uint32_t(c0 & 63) * 2u;
-        // no swizzle needed: 8 (16) consecutive lanes = the 8 (16) channel groups of one slab read one contiguous
-        // 128-byte pixel, which is exactly one conflict-free LDS.128 (LDS.64) phase
-        auto lds = [&](int hy, int hx, uint32_t *v) {                 // halo pixel -> this thread's 2V channels
-            const uint32_t a = slab_base + uint32_t(hy * kDwHalo + hx) * 128u;
-            if constexpr (V == 4) asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(a));
-            else asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=r"(v[0]), "=r"(v[1]) : "r"(a));
-        };
-        uint64_t accP[V], accC[V], accN[V];
-#pragma unroll
-        for (int e = 0; e < V; ++e) { accP[e] = 0ull; accC[e] = 0ull; accN[e] = 0ull; }
-        const int ox = x0 + xl;
-        bf16 *col_out = out + (((long long)img * H) * W + ox) * C + c0;
-#pragma unroll
-        for (int hy = 0; hy < kDwHalo; ++hy) {                        // halo row hy = image row y0 - 1 + hy
-            uint32_t pl[V], pc[V], pr[V];
-            lds(hy, xl, pl); lds(hy, xl + 1, pc); lds(hy, xl + 2, pr);
-#pragma unroll
-            for (int e = 0; e < V; ++e) {
-                const uint64_t fl = dw_pair(pl[e]), fc = dw_pair(pc[e]), fr = dw_pair(pr[e]);
-                accP[e] = f2_fma(wv[6][e], fl, f2_fma(wv[7][e], fc, f2_fma(wv[8][e], fr, accP[e])));
-                accC[e] = f2_fma(wv[3][e], fl, f2_fma(wv[4][e], fc, f2_fma(wv[5][e], fr, accC[e])));
-                accN[e] = f2_fma(wv[0][e], fl, f2_fma(wv[1][e], fc, f2_mul(wv[2][e], fr)));
-            }
-            if (hy >= 2) {                                            // output row y0 + hy - 2 is complete
-                const int oy = y0 + hy - 2;
-                if (oy < H && ox < W) {
-                    __nv_bfloat162 oe[V];
-                    uint64_t bq[V];
-#pragma unroll
-                    for (int e = 0; e < V; e += 2)
-                        asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(bq[e]), "=l"(bq[e + 1]) : "r"(bias_s + 8u * e));
-#pragma unroll
-                    for (int e = 0; e < V; ++e) {
-                        float a, b2;
-                        f2_unpack(f2_add(accP[e], bq[e]), a, b2);
-                        oe[e] = __floats2bfloat162_rn(a, b2);
-                    }
-                    bf16 *dst = col_out + (long long)oy * W * C;
-                    if constexpr (V == 4) *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(oe);
-                    else *reinterpret_cast<uint2 *>(dst) = *reinterpret_cast<const uint2 *>(oe);
-                }
-            }
-#pragma unroll
-            for (int e = 0; e < V; ++e) { accP[e] = accC[e]; accC[e] = accN[e]; }
-        }
-        __syncthreads();                                              // everyone is done reading buffer b
-        if (threadIdx.x == 0 && tile + 2 * int(gridDim.x) < n_tiles) issue(tile + 2 * int(gridDim.x), b);
-    }
-}
-
-// ---- A6, column-blocked variant (what is launched).  Same tiles, TMA boxes and double buffering as above, but a thread owns
-// ONE channel pair of NC adjacent columns instead of four pairs of one column: a warp is the 32 pairs of one 64-channel slab,
+// Column-blocked: a thread owns ONE channel pair of NC adjacent columns (a first version gave it four pairs of one column): a warp is the 32 pairs of one 64-channel slab,
 // so a halo pixel is one conflict-free LDS.32 wavefront (128 contiguous bytes), a halo row of NC + 2 pixels serves NC
 // outputs (NC + 2 bf16x2 -> f32x2 conversions instead of 3 NC), the 9 weights take 18 registers instead of 72 and the bias
 // stays in registers.  ncu on the 8-channel kernel showed why this matters: nothing saturated (issue 44 %, FMA 21 %, ALU
@@ -478,49 +365,38 @@ __global__ void __launch_bounds__(CC + 32, 2) dwconv3x3_cols_kernel(const __grid
 
 template <int CC>
 static cudaError_t launch_dw_cols(const CUtensorMap &tm_in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
-                                  int tiles_x, int tiles_y, int grid, size_t smem, cudaStream_t st, uint32_t *sched, const uint32_t *dep)
+                                  int tiles_x, int tiles_y, int grid, size_t smem, LaunchStream st, uint32_t *sched, const uint32_t *dep)
 {
-    static thread_local bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(dwconv3x3_cols_kernel<CC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
     return launch_pdl(dwconv3x3_cols_kernel<CC>, grid, CC + 32, smem, st, 1, tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, sched, dep, kTrunkTileSignals);
 }
 
+cudaError_t configure_depthwise_kernels()
+{
+    cudaError_t e = cudaFuncSetAttribute(dwconv3x3_cols_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(dwconv3x3_cols_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(dwconv3x3_cols_kernel<192>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(dwconv3x3_cols_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    return e;
+}
+
 cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
-                                 int C, cudaStream_t st, uint32_t *sched, const uint32_t *dep_flags)
+                                 int C, int num_sms, LaunchStream st, uint32_t *sched, const uint32_t *dep_flags)
 {
     const int tiles_x = (W + kDwT - 1) / kDwT, tiles_y = (H + kDwT - 1) / kDwT;
-    const size_t smem = 1024 + 2 * size_t(C >> 6) * kDwSlab + 48;     // + four barriers + the two tile slots of the cols kernel
-    static thread_local int n_sm = 0, variant = 0;
-    if (n_sm == 0) {
-        const char *v = std::getenv("UFNVC_DW_VARIANT");              // tuning knob: 0 = 8 channels x 1 column, else 1 pair x 4 columns
-        variant = v ? std::atoi(v) : kDwNC;
-        cudaError_t e = cudaFuncSetAttribute(dwconv3x3_tma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        if (e != cudaSuccess) return e;
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-    }
+    const size_t smem = 1024 + 2 * size_t(C >> 6) * kDwSlab + 48;     // + four barriers + the two tile slots
     const int n_tiles = n_img * tiles_x * tiles_y;
-    const int grid = n_tiles < 2 * n_sm ? n_tiles : 2 * n_sm;          // persistent: two blocks per SM, double-buffered tiles
-    if (variant != 0) {
-        switch (C) {
-            case 64: return launch_dw_cols<64>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st, sched, dep_flags);
-            case 128: return launch_dw_cols<128>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st, sched, dep_flags);
-            case 192: return launch_dw_cols<192>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st, sched, dep_flags);
-            case 256: return launch_dw_cols<256>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st, sched, dep_flags);
-            default: break;
-        }
+    const int grid = n_tiles < 2 * num_sms ? n_tiles : 2 * num_sms;    // persistent: two blocks per SM, double-buffered tiles
+    switch (C) {
+        case 64: return launch_dw_cols<64>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st, sched, dep_flags);
+        case 128: return launch_dw_cols<128>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st, sched, dep_flags);
+        case 192: return launch_dw_cols<192>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st, sched, dep_flags);
+        case 256: return launch_dw_cols<256>(tm_in, out, w9c, bias, n_img, H, W, tiles_x, tiles_y, grid, smem, st, sched, dep_flags);
+        default: return cudaErrorInvalidValue;
     }
-    dwconv3x3_tma_kernel<4><<<grid, C, smem - 32 + size_t(C) * 4, st>>>(tm_in, out, w9c, bias, n_img, H, W, C, tiles_x, tiles_y);
-    return cudaGetLastError();
 }
 
 cudaError_t launch_dwconv3x3(const bf16 *in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
-                             int C, cudaStream_t st)
+                             int C, LaunchStream st)
 {
     // segment length: the shortest of {H, 16, 8} rows that still gives >= ~32 warps per SM (148 SMs)
     int rows = H;

@@ -125,10 +125,24 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
         const int grp = group_of(p, img);
         const float *bias = p.bias + (long long)grp * p.n_pad + tc.nt * p.BN;
         float bias_lane[4] = {0.f, 0.f, 0.f, 0.f};                   // EPI_HEAD: bias of column c0 + lane for this warp's chunks
+        float wn_lane[4] = {0.f, 0.f, 0.f, 0.f};                     // EPI_HEAD: kappa_t * |w row|_2 of the same columns
+        float xpatch = 0.f;                                          // EPI_HEAD: |x|_2 over the 3x3 neighbourhood of this z-pixel
         if (MODE == EPI_HEAD) {
 #pragma unroll
             for (int q = 0; q < 4; ++q)
-                if (half * 32 + q * 64 < p.BN) bias_lane[q] = __ldg(bias + half * 32 + q * 64 + lane);
+                if (half * 32 + q * 64 < p.BN) {
+                    bias_lane[q] = __ldg(bias + half * 32 + q * 64 + lane);
+                    wn_lane[q] = p.E.kappa_t * __ldg(p.E.wnorm + tc.nt * p.BN + half * 32 + q * 64 + lane);
+                }
+            if (inb) {
+                float s2 = 0.f;
+#pragma unroll
+                for (int t = 0; t < 9; ++t) {
+                    const int yy = y + t / 3 - 1, xx = x + t % 3 - 1;
+                    if (yy >= 0 && yy < p.H && xx >= 0 && xx < p.W) s2 += __ldg(p.E.xnorm2 + ((long long)img * p.H + yy) * p.W + xx);
+                }
+                xpatch = sqrtf(s2);
+            }
         }
         mbar_wait(tfull0 + 8u * acc, acc_phase);
         tc_fence_after();
@@ -188,7 +202,7 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
             for (int c0 = half * 32; c0 < p.BN; c0 += 64) {
                 uint32_t v[32];
                 tmem_ld32(t_row + uint32_t(c0), v);
-                const float bl = bias_lane[c0 >> 6];
+                const float bl = bias_lane[c0 >> 6], wl = wn_lane[c0 >> 6];
                 const int n = tc.nt * p.BN + c0;
                 const int sij = n / E.c_y, c2 = n - sij * E.c_y;
                 const int ly = 4 * y + ((sij >> 2) & 3), lx = 4 * x + (sij & 3);
@@ -214,7 +228,7 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
                         int k = int(tf);
                         k = k < 0 ? 0 : (k > E.n_buckets - 1 ? E.n_buckets - 1 : k);
                         const float fr = t - tf;
-                        if (fminf(fr, 1.0f - fr) < E.flag_t) fm |= 1u << j;
+                        if (fminf(fr, 1.0f - fr) < xpatch * __shfl_sync(0xFFFFFFFFu, wl, j)) fm |= 1u << j;
                         if ((j & 3) == 0) packed[j >> 2] = uint32_t(k); else packed[j >> 2] |= uint32_t(k) << (8 * (j & 3));
                     }
                     if (!live) fm = 0;
@@ -824,8 +838,23 @@ bool tc_make_halo_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int 
     return tc_make_act_tmap(tm, base, n_img, H, W, C, kHaloTH + 2, kHaloTW + 2, err);
 }
 
+cudaError_t configure_conv_tc_kernels()
+{
+    cudaError_t e = cudaSuccess;
+    auto set = [&](auto kern) { if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); };
+    set(conv_halo_pair_kernel<EPI_PS2>);
+    set(conv_halo_kernel<EPI_NHWC, true>); set(conv_halo_kernel<EPI_NHWC, false>);
+    set(conv_halo_kernel<EPI_PS2, true>); set(conv_halo_kernel<EPI_PS2, false>);
+    set(conv_halo_kernel<EPI_HEAD, false>);
+    set(conv_halo_kernel<EPI_MU, true>); set(conv_halo_kernel<EPI_MU, false>);
+    set(conv_halo_kernel<EPI_FINAL, true>); set(conv_halo_kernel<EPI_FINAL, false>);
+    set(conv_tc_kernel<EPI_NHWC>); set(conv_tc_kernel<EPI_PS2>); set(conv_tc_kernel<EPI_HEAD>); set(conv_tc_kernel<EPI_MU>);
+    set(conv_tc_kernel<EPI_FINAL>);
+    return e;
+}
+
 cudaError_t launch_conv_halo_pair(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
-                                  cudaStream_t st)
+                                  LaunchStream st)
 {
     if (L.taps != 9 || !L.has_half_map || E.mode != EPI_PS2) return cudaErrorInvalidValue;
     TcParams p{};
@@ -849,18 +878,12 @@ cudaError_t launch_conv_halo_pair(const ConvLayer &L, const ConvProblem &P, cons
     if (nb > 12) nb = 12;
     if (nb < 2) return cudaErrorInvalidValue;
     const size_t smem = 1024 + size_t(na) * kHaloStage + size_t(nb) * bh_bytes + 256 + 16 * size_t(nb) + 16 * size_t(na);
-    static thread_local bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(conv_halo_pair_kernel<EPI_PS2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
     const int clusters = p.total_tiles < num_sms / 2 ? p.total_tiles : num_sms / 2;
     return launch_pdl(conv_halo_pair_kernel<EPI_PS2>, 2 * clusters, kThreads, smem, st, 2, tmap_halo, L.tmap_w_half, p, nb, na);
 }
 
 cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
-                             cudaStream_t st)
+                             LaunchStream st)
 {
     if (L.taps != 9) return cudaErrorInvalidValue;
     TcParams p{};
@@ -890,17 +913,7 @@ cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUt
     while (na < 8 && 1024 + size_t(na + 1) * kHaloStage + size_t(nb) * b_bytes + 2048 <= 227 * 1024) ++na;
     const size_t smem = 1024 + size_t(na) * kHaloStage + size_t(nb) * b_bytes + 256 + 16 * size_t(nb) + 16 * size_t(na);
     const int grid = p.total_tiles < num_sms ? p.total_tiles : num_sms;
-    auto launch = [&](auto kern) -> cudaError_t {
-        static thread_local const void *configured[16] = {};
-        bool done = false;
-        for (const void *c : configured) done |= (c == (const void *)kern);
-        if (!done) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-            if (e != cudaSuccess) return e;
-            for (auto &c : configured) if (!c) { c = (const void *)kern; break; }
-        }
-        return launch_pdl(kern, grid, kThreads, smem, st, 1, tmap_halo, L.tmap_w, p, nb, na);
-    };
+    auto launch = [&](auto kern) -> cudaError_t { return launch_pdl(kern, grid, kThreads, smem, st, 1, tmap_halo, L.tmap_w, p, nb, na); };
     switch (E.mode) {
         case EPI_NHWC: return resident ? launch(conv_halo_kernel<EPI_NHWC, true>) : launch(conv_halo_kernel<EPI_NHWC, false>);
         case EPI_PS2: return resident ? launch(conv_halo_kernel<EPI_PS2, true>) : launch(conv_halo_kernel<EPI_PS2, false>);
@@ -911,7 +924,7 @@ cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUt
 }
 
 cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_in, int tile_h, int tile_w, bool flat,
-                           const EpiParams &E, int num_sms, cudaStream_t st)
+                           const EpiParams &E, int num_sms, LaunchStream st)
 {
     TcParams p{};
     p.H = P.H; p.W = P.W;
@@ -937,17 +950,7 @@ cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUten
     p.E = E;
     const size_t smem = size_t(kStages) * (kABytes + size_t(L.block_n) * 128) + 1024 + 256;
     const int grid = p.total_tiles < num_sms ? p.total_tiles : num_sms;
-    auto launch = [&](auto kern) -> cudaError_t {
-        static thread_local const void *configured[16] = {};
-        bool done = false;
-        for (const void *c : configured) done |= (c == (const void *)kern);
-        if (!done) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-            if (e != cudaSuccess) return e;
-            for (auto &c : configured) if (!c) { c = (const void *)kern; break; }
-        }
-        return launch_pdl(kern, grid, kThreads, smem, st, 1, tmap_in, L.tmap_w, p);
-    };
+    auto launch = [&](auto kern) -> cudaError_t { return launch_pdl(kern, grid, kThreads, smem, st, 1, tmap_in, L.tmap_w, p); };
     switch (E.mode) {
         case EPI_NHWC: return launch(conv_tc_kernel<EPI_NHWC>);
         case EPI_PS2: return launch(conv_tc_kernel<EPI_PS2>);

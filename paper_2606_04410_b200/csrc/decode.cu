@@ -2,7 +2,6 @@
 // One host call, zero host synchronisations, everything on the caller's stream.
 #include <algorithm>
 #include <cmath>
-#include <cstdlib>
 #include <cstring>
 
 #include "handle.h"
@@ -19,13 +18,13 @@ namespace {
 
 // conv dispatch: tcgen05 implicit GEMM when the layer and the activation map qualify, CUDA-core kernel otherwise.
 cudaError_t conv(ufnvc_handle *h, const ConvLayer &L, const ConvProblem &P, const ufnvc_handle::ActMap &am, const EpiParams &E,
-                 cudaStream_t st, int *launches)
+                 LaunchStream st, int *launches)
 {
     if (launches) ++*launches;
-    if (L.use_tc && L.taps == 9 && am.halo_ok && h->use_halo && !h->force_generic && h->use_pair_conv && L.has_half_map &&
+    if (L.use_tc && L.taps == 9 && am.halo_ok && !h->force_generic && h->use_pair_conv && L.has_half_map &&
         E.mode == EPI_PS2 && P.W > 8)
         return launch_conv_halo_pair(L, P, am.tm_halo, E, h->num_sms, st);
-    if (L.use_tc && L.taps == 9 && am.halo_ok && h->use_halo && !h->force_generic)
+    if (L.use_tc && L.taps == 9 && am.halo_ok && !h->force_generic)
         return launch_conv_halo(L, P, am.tm_halo, E, h->num_sms, st);
     if (L.use_tc && am.ok && !h->force_generic) return launch_conv_tc(L, P, am.tm, am.tile_h, am.tile_w, am.flat, E, h->num_sms, st);
     return launch_conv_generic(L, P, E, st);
@@ -35,10 +34,11 @@ struct Stage { cudaEvent_t *ev; int i; cudaEvent_t *dw; };   // dw: one event af
 inline void mark(Stage *s, cudaStream_t st) { if (s) cudaEventRecord(s->ev[s->i++], st); }
 
 int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bits_bytes, const uint32_t *sub_off, float *frames,
-        cudaStream_t st, const uint8_t *idx_ovr, const float *mu_ovr, const ufnvc_taps *taps, bool entropy_params_only,
+        cudaStream_t stream, const uint8_t *idx_ovr, const float *mu_ovr, const ufnvc_taps *taps, bool entropy_params_only,
         float *mu_out, float *ls_out, uint8_t *idx_out, Stage *sg, int *launches)
 {
     const ufnvc_config &c = h->cfg;
+    const LaunchStream st{stream, h->pdl};
     int local_launches = 0;                    // kernels of this library enqueued by this call (memsets / copies not counted)
     if (!launches) launches = &local_launches;
     struct Publish { ufnvc_handle *h; int *n; ~Publish() { h->last_launches = *n; } } publish{h, launches};
@@ -65,14 +65,14 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
         if (h->hybrid_head && h->am_xs.ok && h->head_tc.use_tc) {
             // layer 1 also emits the bf16 hi|mid split; the head runs on tensor cores; elements whose ln sigma lands within
             // flag_u of a bucket edge are re-decided in fp64 (identical decisions to the all-fp64 path, R12)
-            CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, h->hpart, n, h->h_z, h->w_z, st, h->xs));
+            CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, h->hpart, n, h->h_z, h->w_z, st, h->xs, h->xnorm2));
             const double step = (hp.ln_hi - hp.ln_lo) / double(c.n_buckets - 1 > 0 ? c.n_buckets - 1 : 1);
             EpiParams E{};
             E.mode = EPI_HEAD; E.act = ACT_NONE;
             E.mu = h->mu; E.lnscale = h->lnscale; E.idx = h->idx; E.fix_list = h->fix_list; E.fix_count = h->fix_count;
             E.c_y = c.c_y; E.lat_h = h->h; E.lat_w = h->w; E.n_buckets = c.n_buckets;
             E.ln_lo = float(hp.ln_lo); E.ln_hi = float(hp.ln_hi); E.t_scale = float(1.0 / step);
-            E.flag_t = float(h->head_flag_u / step);
+            E.wnorm = h->head_wnorm; E.xnorm2 = h->xnorm2; E.kappa_t = float(h->head_kappa / step);
             ConvProblem pr{h->xs, n, h->h_z, h->w_z, 1};
             // z maps are tiny (17 x 30 at 1080p): the shifted-TMA-box kernel tiles them with the least padding
             CU_TRY(launch_conv_tc(h->head_tc, pr, h->am_xs.tm, h->am_xs.tile_h, h->am_xs.tile_w, false, E, h->num_sms, st));
@@ -162,7 +162,7 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
         // box instead of for the whole MLP grid, and are handed out by a per-block counter
         uint32_t *sync_k = h->trunk_sync + size_t(k) * h->trunk_sync_stride;
         const bool mlp_counts = fused_ok && trunk_counts_tiles((long long)n * T * P, h->use_pair_trunk) && h->tail_fill;
-        if (h->dw_tma_ok) CU_TRY(launch_dwconv3x3_tma(h->tm_dw, h->fb, tb.dw_w, tb.dw_b, n * T, h->h, h->w, Ct, st, h->tail_fill ? sync_k : nullptr,
+        if (h->dw_tma_ok) CU_TRY(launch_dwconv3x3_tma(h->tm_dw, h->fb, tb.dw_w, tb.dw_b, n * T, h->h, h->w, Ct, h->num_sms, st, h->tail_fill ? sync_k : nullptr,
                                                       (k > 0 && mlp_counts) ? sync_k - h->trunk_sync_stride + 1 : nullptr));
         else CU_TRY(launch_dwconv3x3(h->fa, h->fb, tb.dw_w, tb.dw_b, n * T, h->h, h->w, Ct, st));
         if (launches) ++*launches;
@@ -266,16 +266,14 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
     // tcgen05 path: weight descriptors + descriptors of the (fixed) workspace activations
     const ufnvc_config &c = h->cfg;
     std::string err;
-    const char *xbn = std::getenv("UFNVC_XFRAME_BN");               // tuning knob: N tile of the A5 cross-frame conv (0 = widest)
-    bool ok = tc_make_weight_tmap(h->xframe, err, xbn ? std::atoi(xbn) : 0);
+    bool ok = tc_make_weight_tmap(h->xframe, err, 0);
     if (h->hybrid_head) {
         // N tile of the hyper head conv: the z map is tiny (510 pixels at 1080p = 4-6 M tiles), so with the widest N tile
         // (256) fewer tiles than SMs exist and each CTA runs one long tile with its epilogue exposed; 128 doubles the tile
-        // count (measured at 1080p: A1+A2 98 -> 93 us; 64 and 32 are slower again).  UFNVC_HEAD_BN overrides.
-        const char *bn = std::getenv("UFNVC_HEAD_BN");
+        // count (measured at 1080p: A1+A2 98 -> 93 us; 64 and 32 are slower again).
         const long long m_tiles = ((long long)h->max_chunks * h->h_z * h->w_z + 127) / 128;
         const int auto_bn = (h->head_tc.n_pad % 128 == 0 && m_tiles * (h->head_tc.n_pad / 256) < h->num_sms) ? 128 : 0;
-        ok = ok && tc_make_weight_tmap(h->head_tc, err, bn ? std::atoi(bn) : auto_bn);
+        ok = ok && tc_make_weight_tmap(h->head_tc, err, auto_bn);
     }
     for (auto &tb : h->trunk) ok = ok && tc_make_weight_tmap(tb.pw1, err) && tc_make_weight_tmap(tb.pw2, err);
     for (int s = 0; s < 4; ++s) ok = ok && tc_make_weight_tmap(h->dec[s], err);
@@ -290,31 +288,21 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
     if (c.mu_steps == 4) {
         for (int b = 0; ok && b < 2; ++b) ok = make_act_map(h, h->am_ymu[b], h->ymu[b], n, h->h, h->w, h->mu_net[0].c_in, false, 1);
         if (ok && (!h->am_ymu[0].ok || !h->mu_net[0].use_tc || h->force_generic))
-            return fail(h, UFNVC_E_BAD_CONFIG, "mu_steps == 4 needs the tensor-core conv path (c_y % 32 == 0, UFNVC_FORCE_GENERIC unset)");
+            return fail(h, UFNVC_E_BAD_CONFIG, "mu_steps == 4 needs the tensor-core conv path (c_y % 32 == 0, no UFNVC_DBG_FORCE_GENERIC)");
     }
     h->trunk_sync_stride = size_t(((long long)n * T * h->h * h->w + 127) / 128 + 4);
-    {
-        const char *tf = std::getenv("UFNVC_TAIL_FILL");              // 0: whole-grid waits and static tile striding
-        h->tail_fill = !(tf && tf[0] == '0');
-    }
     h->dw_tma_ok = false;
-    {
-        const char *dv = std::getenv("UFNVC_DW_TMA");
-        if (ok && c.n_trunk_blocks > 0 && c.c_trunk % 64 == 0 && c.c_trunk <= 256 && !(dv && dv[0] == '0')) {
-            ok = tc_make_act_tmap(&h->tm_dw, h->fa, n * T, h->h, h->w, c.c_trunk, 10, 10, h->err, /*swizzle=*/false);
-            h->dw_tma_ok = ok;
-        }
+    if (ok && c.n_trunk_blocks > 0 && c.c_trunk % 64 == 0 && c.c_trunk <= 256 && h->use_dw_tma) {
+        ok = tc_make_act_tmap(&h->tm_dw, h->fa, n * T, h->h, h->w, c.c_trunk, 10, 10, h->err, /*swizzle=*/false);
+        h->dw_tma_ok = ok;
     }
     for (auto &tb : h->trunk)
         if (ok && !trunk_make_maps(tb.fused, h->fb, (long long)n * T * h->h * h->w, tb.pw1, tb.pw2, h->err)) ok = false;
     for (int s = 0; ok && s < 3; ++s)
         ok = make_act_map(h, h->am_stage[s], h->stage[s], n * T, h->h << (s + 1), h->w << (s + 1), c.dec_channels[s + 1], false, T);
-    {
-        const char *fi = std::getenv("UFNVC_FINAL_IS");
-        h->final_is.ok = false;
-        if (ok && !(fi && fi[0] == '0') && c.dec_channels[3] % 64 == 0)
-            ok = final_make_maps(h->final_is, h->dec[3], h->stage[2], n * T, h->h << 3, h->w << 3, c.width, h->err);
-    }
+    h->final_is.ok = false;
+    if (ok && h->use_final_is && c.dec_channels[3] % 64 == 0)
+        ok = final_make_maps(h->final_is, h->dec[3], h->stage[2], n * T, h->h << 3, h->w << 3, c.width, h->err);
     if (!ok) return fail(h, UFNVC_E_CUDA, h->err);
     h->weights_loaded = true;
     return UFNVC_OK;
@@ -342,9 +330,10 @@ extern "C" int ufnvc_chunk_decode(ufnvc_handle *h, int n_chunks, const int16_t *
 // ---- NEXT-3 (R22): the hyper-latent from bytes ------------------------------------------------------------------
 namespace {
 int decode_z_impl(ufnvc_handle *h, int n, const uint8_t *bits, size_t bits_bytes, const uint32_t *sub_off, int sub_stride,
-                  int16_t *z_planar_out, cudaStream_t st, int *launches)
+                  int16_t *z_planar_out, cudaStream_t stream, int *launches)
 {
     const ufnvc_config &c = h->cfg;
+    const LaunchStream st{stream, h->pdl};
     if (!h->z_prior_loaded) return fail(h, UFNVC_E_NO_WEIGHTS, "the weights blob holds no zprior.lnscale tensor");
     CU_TRY(cudaMemsetAsync(h->d_status, 0, 4, st));
     RansParams rp{};
@@ -405,7 +394,7 @@ extern "C" int ufnvc_encode_chunk_dev(ufnvc_handle *h, int n_chunks, const uint8
     if (!idx_dev || !sym_dev || !bits_dev || !sub_off_dev) return fail(h, UFNVC_E_INVALID_ARG, "null device pointer");
     if (reinterpret_cast<uintptr_t>(bits_dev) & 3) return fail(h, UFNVC_E_INVALID_ARG, "bits_dev must be 4-byte aligned");
     const ufnvc_config &c = h->cfg;
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const LaunchStream st{static_cast<cudaStream_t>(cuda_stream), h->pdl};
     const int G = c.lanes_per_substream / 32;
     if (!h->enc_tmp) {
         const size_t n_sym = size_t(c.rows_per_substream) * h->w * c.c_y;

@@ -258,8 +258,13 @@ bool final_make_maps(FinalMaps &m, const ConvLayer &L, const bf16 *in_base, int 
     return true;
 }
 
+cudaError_t configure_final_kernels()
+{
+    return cudaFuncSetAttribute(final_is_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kFSmem));
+}
+
 cudaError_t launch_final_is(const FinalMaps &m, const ConvLayer &L, int n_img, int H, int W, float *out, int out_h, int out_w,
-                            int num_sms, cudaStream_t st)
+                            int num_sms, LaunchStream st)
 {
     FinalParams p{};
     p.n_img = n_img; p.H = H; p.W = W;
@@ -269,12 +274,6 @@ cudaError_t launch_final_is(const FinalMaps &m, const ConvLayer &L, int n_img, i
     p.groups = L.groups;
     p.bias = L.bias;
     p.out = out; p.out_h = out_h; p.out_w = out_w;
-    static thread_local bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(final_is_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kFSmem));
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
     const int grid = p.total_tiles < num_sms ? p.total_tiles : num_sms;
     return launch_pdl(final_is_kernel, grid, kFThreads, kFSmem, st, 1, m.tm_in, m.tm_w, p);
 }

@@ -14,11 +14,14 @@ struct ufnvc_handle {
     int max_chunks = 1;
     bool weights_loaded = false;
     int last_launches = 0;               // kernels enqueued by the last decode call (ufnvc_launches_per_call)
-    bool use_pair_conv = true;           // env UFNVC_PAIR_CONV=0: single-CTA halo conv for A8 (A/B test)
-    bool use_pair_trunk = true;          // env UFNVC_PAIR_TRUNK=0: single-CTA fused MLP kernel (A/B test)
-    bool use_fused_trunk = true;         // env UFNVC_FUSED_TRUNK=0: two 1x1 conv launches per block (A/B test)
-    bool use_halo = true;                // env UFNVC_HALO=0: first-pass implicit-GEMM kernel for the 3x3 convs (A/B test)
-    bool force_generic = false;          // env UFNVC_FORCE_GENERIC=1: CUDA-core convs everywhere (cross-check)
+    // code-path switches, all derived from ufnvc_config.debug_flags at create (include/ufnvc.h UFNVC_DBG_*; 0 = defaults)
+    bool use_pair_conv = true;           // CTA-pair halo conv for A8 (else single-CTA)
+    bool use_pair_trunk = true;          // CTA-pair fused MLP kernel (else single-CTA)
+    bool use_fused_trunk = true;         // fused MLP kernel (else two 1x1 conv launches per block)
+    bool force_generic = false;          // CUDA-core convs everywhere (cross-check)
+    bool pdl = true;                     // programmatic dependent launch along the kernel chain
+    bool use_final_is = true;            // A9 input-stationary kernel
+    bool use_dw_tma = true;              // A6 TMA-staged kernel
     std::string err;
 
     // entropy tables (O3)
@@ -31,7 +34,11 @@ struct ufnvc_handle {
     ufnvc::HyperLayer hyper[3];
     // hybrid head (R12): tensor-core evaluation of the last hyper conv + exact fp64 re-evaluation near bucket edges
     bool hybrid_head = false;
-    double head_flag_u = 5e-4;           // |ln sigma - bucket edge| below which the fp64 re-evaluation decides (env UFNVC_HEAD_FLAG_U)
+    // a-priori bound on |tensor-core ln sigma - fp64 ln sigma| = head_kappa * |w row|_2 * |x patch|_2 (decode.cu); elements
+    // closer than that to a bucket edge are re-decided in fp64
+    double head_kappa = 0.0;
+    float *head_wnorm = nullptr;         // [2 c_y 16] |w row|_2 per packed head column
+    float *xnorm2 = nullptr;             // [n][h_z][w_z] sum over channels of hx2^2
     ufnvc::ConvLayer head_tc;
     double *head_fix_w = nullptr, *head_fix_b = nullptr;   // [c_y*16][9][c_hyper], [c_y*16] (scale half)
     ufnvc::bf16 *xs = nullptr;           // [n][h_z][w_z][2*c_hyper]: bf16 hi | mid split of the fp64 hx2
@@ -74,7 +81,7 @@ struct ufnvc_handle {
         CUtensorMap tm_halo;             // 3x3 convs: box {64, 10, 18}: a 16 x 8 pixel tile plus halo (conv_halo_kernel)
         bool halo_ok = false;
     };
-    ufnvc::FinalMaps final_is;           // A9 input-stationary kernel (env UFNVC_FINAL_IS=0 disables)
+    ufnvc::FinalMaps final_is;           // A9 input-stationary kernel
     CUtensorMap tm_dw;                   // fa as the depthwise kernel reads it: box {64 ch, 10, 10}
     bool dw_tma_ok = false;
     // per trunk block: [0] = the depthwise kernel's dynamic tile counter, [1 ..] = one completion counter per 128-pixel tile of
@@ -92,7 +99,8 @@ struct ufnvc_handle {
     uint32_t *enc_sizes = nullptr;
     size_t enc_tmp_stride = 0, enc_stage_stride = 0;
 
-    std::vector<void *> allocs;          // everything cudaMalloc'ed, freed at destroy
+    std::vector<void *> allocs;          // workspace and tables, freed at destroy
+    std::vector<void *> weight_allocs;   // what ufnvc_load_weights uploaded; freed by the next load and at destroy
     cudaEvent_t ev[8] = {};
     std::vector<cudaEvent_t> ev_dw;      // profiled call: before / after every depthwise launch
     bool ev_made = false;

@@ -236,7 +236,7 @@ __global__ void hyper_reduce_kernel(const double *__restrict__ part, const doubl
     }
 }
 
-cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z, int pz, cudaStream_t st)
+cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z, int pz, LaunchStream st)
 {
     const long long total = (long long)n_chunks * c_z * pz;
     const int blocks = int((total + 255) / 256 < 1184 ? (total + 255) / 256 : 1184);
@@ -244,25 +244,36 @@ cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z
     return cudaGetLastError();
 }
 
-// same reduce, also emitting the 2-term bf16 split of the fp64 result: xs[m][o] = hi = bf16(v), xs[m][n_out + o] = bf16(v - hi)
+// same reduce, also emitting the 2-term bf16 split of the fp64 result: xs[m][o] = hi = bf16(v), xs[m][n_out + o] = bf16(v - hi),
+// and xnorm2[m] = sum_o v^2 (fp32), the input of the head's a-priori error bound (decode.cu, R12).  One warp per
+// z-pixel m, lanes stride the channels, fixed-order tree reduction: run-to-run deterministic.
 __global__ void hyper_reduce_split_kernel(const double *__restrict__ part, const double *__restrict__ bias, double *__restrict__ out,
-                                          bf16 *__restrict__ xs, long long MN, int n_out)
+                                          bf16 *__restrict__ xs, float *__restrict__ xnorm2, long long M, int n_out)
 {
     asm volatile("griddepcontrol.wait;" ::: "memory");              // PDL: launched early, the predecessor's output is complete from here on
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < MN; i += (long long)gridDim.x * blockDim.x) {
-        double v = part[i];
+    const int lane = threadIdx.x & 31;
+    const long long warps = ((long long)gridDim.x * blockDim.x) >> 5;
+    const long long MN = M * n_out;
+    for (long long m = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5; m < M; m += warps) {
+        double ss = 0.0;
+        for (int o = lane; o < n_out; o += 32) {
+            const long long i = m * n_out + o;
+            double v = part[i];
 #pragma unroll
-        for (int t = 1; t < 9; ++t) v += part[t * MN + i];
-        const int o = int(i % n_out);
-        const long long m = i / n_out;
-        v += bias[o];
-        v = v > 0.0 ? v : 0.0;
-        out[i] = v;
-        const bf16 hi = __double2bfloat16(v);
-        const bf16 mid = __double2bfloat16(v - double(__bfloat162float(hi)));
-        xs[m * 2 * n_out + o] = hi;
-        xs[m * 2 * n_out + n_out + o] = mid;
+            for (int t = 1; t < 9; ++t) v += part[t * MN + i];               // fixed tap order
+            v += bias[o];
+            v = v > 0.0 ? v : 0.0;
+            out[i] = v;
+            const bf16 hi = __double2bfloat16(v);
+            const bf16 mid = __double2bfloat16(v - double(__bfloat162float(hi)));
+            xs[m * 2 * n_out + o] = hi;
+            xs[m * 2 * n_out + n_out + o] = mid;
+            ss = fma(v, v, ss);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xFFFFFFFFu, ss, o);
+        if (lane == 0) xnorm2[m] = float(ss);
     }
 }
 
@@ -320,7 +331,7 @@ __global__ void __launch_bounds__(256) hyper_fix_kernel(const uint32_t *__restri
 static bool fast_ok(const HyperLayer &L) { return L.c_in % FK == 0 && L.n % 4 == 0; }
 
 cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out, double *part, int n_img, int hz, int wz,
-                              cudaStream_t st, bf16 *xs)
+                              LaunchStream st, bf16 *xs, float *xnorm2)
 {
     HyperEpi e{};
     e.mode = 0;
@@ -331,7 +342,10 @@ cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out
         if (cudaError_t le = launch_pdl_grid(hyper_conv_fast_kernel<true>, grid, 256u, st, in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e, part)) return le;
         const long long MN = (long long)M * L.n;
         const int blocks = int((MN + 255) / 256 < 1184 ? (MN + 255) / 256 : 1184);
-        if (xs) { if (cudaError_t le = launch_pdl(hyper_reduce_split_kernel, unsigned(blocks), 256u, 0, st, 1, part, L.bias, out, xs, MN, L.n)) return le; }
+        if (xs) {
+            const int wblocks = int(((long long)M * 32 + 255) / 256 < 1184 ? ((long long)M * 32 + 255) / 256 : 1184);
+            if (cudaError_t le = launch_pdl(hyper_reduce_split_kernel, unsigned(wblocks), 256u, 0, st, 1, part, L.bias, out, xs, xnorm2, (long long)M, L.n)) return le;
+        }
         else if (cudaError_t le = launch_pdl(hyper_reduce_kernel, unsigned(blocks), 256u, 0, st, 1, part, L.bias, out, MN, L.n)) return le;
         return cudaGetLastError();
     }
@@ -340,23 +354,14 @@ cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out
     return cudaGetLastError();
 }
 
-cudaError_t launch_hyper_reduce_split(const double *part, const double *bias, double *out, bf16 *xs, long long M, int n_out,
-                                      cudaStream_t st)
-{
-    const long long MN = M * n_out;
-    const int blocks = int((MN + 255) / 256 < 1184 ? (MN + 255) / 256 : 1184);
-    hyper_reduce_split_kernel<<<blocks, 256, 0, st>>>(part, bias, out, xs, MN, n_out);
-    return cudaGetLastError();
-}
-
 cudaError_t launch_hyper_fix(const uint32_t *list, const uint32_t *count, const double *x2, const double *fix_w, const double *fix_b,
-                             int c_h, int hz, int wz, const HeadParams &hp, int num_sms, cudaStream_t st)
+                             int c_h, int hz, int wz, const HeadParams &hp, int num_sms, LaunchStream st)
 {
     return launch_pdl(hyper_fix_kernel, unsigned(num_sms * 4), 256u, 0, st, 1, list, count, x2, fix_w, fix_b, c_h, hz, wz, hp);
 }
 
 cudaError_t launch_hyper_head(const HyperLayer &L, const double *in, int n_img, int hz, int wz, const HeadParams &hp,
-                              cudaStream_t st)
+                              LaunchStream st)
 {
     HyperEpi e{};
     e.mode = 1;

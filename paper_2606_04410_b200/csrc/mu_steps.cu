@@ -45,7 +45,7 @@ __global__ void __launch_bounds__(256) mu_prep_kernel(const int16_t *__restrict_
 }
 
 cudaError_t launch_mu_prep(const int16_t *sym, const float *mu0, bf16 *ymu0, bf16 *ymu1, int n_img, int H, int W, int c_y, int stride,
-                           cudaStream_t st)
+                           LaunchStream st)
 {
     const long long n_pix = (long long)n_img * H * W;
     const long long total = n_pix * (c_y >> 3);

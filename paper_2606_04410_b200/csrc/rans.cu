@@ -80,7 +80,12 @@ __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
         for (int s = 0; s < kPre; ++s) {
             const int ii = i0 + (j0 + s) * p.W;
             kk[s] = 0; mm[s] = 0.f;
-            if (j0 + s < n_steps && ii < n) { kk[s] = p.idx[ebase + ii]; mm[s] = p.mu[ebase + ii]; }
+            if (j0 + s < n_steps && ii < n) {
+                kk[s] = p.idx[ebase + ii]; mm[s] = p.mu[ebase + ii];
+                // an index past the tables (possible only through idx_override_dev) must not read shared memory out of
+                // bounds: clamp and report, like every other malformed input (off the serial chain: this is the prefetch)
+                if (kk[s] >= uint32_t(nb)) { kk[s] = uint32_t(nb - 1); st |= UFNVC_STREAM_BAD_HEADER; }
+            }
         }
     };
     auto step = [&](uint32_t k, float mu, int j) {
@@ -147,7 +152,7 @@ __global__ void z_hwc_to_planar_kernel(const int16_t *__restrict__ in, int16_t *
     }
 }
 
-cudaError_t launch_z_hwc_to_planar(const int16_t *z_hwc, int16_t *z_planar, int n_chunks, int c_z, int pz, cudaStream_t st)
+cudaError_t launch_z_hwc_to_planar(const int16_t *z_hwc, int16_t *z_planar, int n_chunks, int c_z, int pz, LaunchStream st)
 {
     const long long total = (long long)n_chunks * c_z * pz;
     const int blocks = int((total + 255) / 256 < 1184 ? (total + 255) / 256 : 1184);
@@ -155,16 +160,17 @@ cudaError_t launch_z_hwc_to_planar(const int16_t *z_hwc, int16_t *z_planar, int 
     return cudaGetLastError();
 }
 
-cudaError_t launch_rans_decode(const RansParams &p, cudaStream_t st)
+constexpr size_t kRansSmem = (size_t)64 * (256 * 4 + kLutBuckets * 2);
+
+cudaError_t configure_rans_kernels()
+{
+    return cudaFuncSetAttribute(rans_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRansSmem);
+}
+
+cudaError_t launch_rans_decode(const RansParams &p, LaunchStream st)
 {
     const int nb = p.n_buckets;
-    const size_t smem = (size_t)64 * (256 * 4 + kLutBuckets * 2);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(rans_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    const size_t smem = kRansSmem;
     return launch_pdl(rans_decode_kernel, unsigned(p.n_chunks * p.n_sub), unsigned(p.W), smem, st, 1, p, nb);
 }
 

@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(1024) rans_pack_kernel(RansEncParams p, int n_
     }
 }
 
-cudaError_t launch_rans_encode(const RansEncParams &p, cudaStream_t st)
+cudaError_t launch_rans_encode(const RansEncParams &p, LaunchStream st)
 {
     const int n_total = p.n_chunks * p.n_sub;
     rans_encode_kernel<<<n_total, p.W, 0, st>>>(p);

@@ -16,8 +16,6 @@
 // warp 0 = TMA producer, warp 1 = MMA issuer + TMEM allocator, warps 2..9 = epilogue.  Persistent, grid = #SMs.
 #include <cuda.h>
 
-#include <cstdlib>
-
 #include "epilogue.cuh"
 #include "tc_ptx.cuh"
 #include "ufnvc_internal.h"
@@ -330,7 +328,7 @@ namespace {
 // TMH = true: the GELU'd hidden chunk goes back into TMEM (bf16, over the fp32 columns it came from) and GEMM2 reads its
 // A operand from there: no 64 KB Hs buffer (the weight ring grows from 3 to 5 stages), and per tile 256 KB of st.shared
 // plus 256 KB of A-operand reads leave the shared-memory port, which TMA writes + MMA operand reads had saturated.
-template <bool TMH>
+constexpr bool TMH = true;     // (the shared-memory-hidden variant, TMH = false, lost the A/B and is no longer instantiated)
 __global__ void __launch_bounds__(kTrunkThreads, 1)
 trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant__ CUtensorMap tm_w1h,
                       const __grid_constant__ CUtensorMap tm_w2h, const TrunkParams p)
@@ -630,8 +628,15 @@ bool trunk_make_maps(TrunkMaps &m, const bf16 *d_base, long long n_px, const Con
 
 bool trunk_counts_tiles(long long n_px, bool pair) { return pair && (n_px + kTM - 1) / kTM >= 2; }
 
+cudaError_t configure_trunk_kernels()
+{
+    cudaError_t e = cudaFuncSetAttribute(trunk_mlp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kTrunkSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(trunk_mlp_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kTrunkSmem));
+    return e;
+}
+
 cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const ConvLayer &pw2, const bf16 *x, bf16 *out, long long n_px,
-                             int num_sms, bool pair, cudaStream_t st, uint32_t *tile_done)
+                             int num_sms, bool pair, LaunchStream st, uint32_t *tile_done)
 {
     TrunkParams p{};
     p.tile_done = tile_done;
@@ -640,25 +645,10 @@ cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const Con
     p.n_chunks = pw1.n / kHC;
     p.b1 = pw1.bias; p.b2 = pw2.bias;
     p.x = x; p.out = out;
-    static thread_local bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(trunk_mlp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kTrunkSmem));
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
     if (pair && p.n_tiles >= 2) {
-        static thread_local bool configured2 = false;
-        if (!configured2) {
-            cudaError_t e = cudaFuncSetAttribute(trunk_mlp_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kTrunkSmem));
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(trunk_mlp_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kTrunkSmem));
-            if (e != cudaSuccess) return e;
-            configured2 = true;
-        }
         const int n_ptiles = (p.n_tiles + 1) / 2;
         const int clusters = n_ptiles < num_sms / 2 ? n_ptiles : num_sms / 2;
-        static const bool tmh = [] { const char *e = std::getenv("UFNVC_TRUNK_TMEM_HIDDEN"); return !(e && e[0] == '0'); }();
-        return tmh ? launch_pdl(trunk_mlp_pair_kernel<true>, 2 * clusters, kTrunkThreads, kTrunkSmem, st, 2, m.tm_d, m.tm_w1h, m.tm_w2h, p)
-                   : launch_pdl(trunk_mlp_pair_kernel<false>, 2 * clusters, kTrunkThreads, kTrunkSmem, st, 2, m.tm_d, m.tm_w1h, m.tm_w2h, p);
+        return launch_pdl(trunk_mlp_pair_kernel, 2 * clusters, kTrunkThreads, kTrunkSmem, st, 2, m.tm_d, m.tm_w1h, m.tm_w2h, p);
     }
     const int grid = p.n_tiles < num_sms ? p.n_tiles : num_sms;
     return launch_pdl(trunk_mlp_kernel, grid, kTrunkThreads, kTrunkSmem, st, 1, m.tm_d, m.tm_w1, m.tm_w2, p);

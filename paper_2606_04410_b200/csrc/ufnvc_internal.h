@@ -37,9 +37,14 @@ struct EpiParams {
     // EPI_HEAD: packed column n' = (s*16 + 4i+j)*c_y + c2 of z-pixel (zy, zx) -> latent (4zy+i, 4zx+j), channel c2
     float *mu, *lnscale;     // [n][lat_h][lat_w][c_y]
     uint8_t *idx;
-    uint32_t *fix_list, *fix_count;   // elements whose tensor-core ln sigma is within flag_t of a bucket edge
+    uint32_t *fix_list, *fix_count;   // elements whose tensor-core ln sigma may be on the wrong side of a bucket edge
     int c_y, lat_h, lat_w, n_buckets;
-    float ln_lo, ln_hi, t_scale, flag_t;   // t = (u - ln_lo) * t_scale + 0.5; flag when |t - round(t)| < flag_t
+    float ln_lo, ln_hi, t_scale;      // t = (u - ln_lo) * t_scale + 0.5
+    // element (z-pixel m, packed column n') is flagged when |t - round(t)| < kappa_t * wnorm[n'] * sqrt(sum of xnorm2 over the
+    // 3x3 neighbourhood of m): the a-priori bound on the tensor-core value's error, in bucket units (decode.cu)
+    const float *wnorm;               // [n_pad]: L2 norm of packed weight row n' over its 9 * c_hyper taps
+    const float *xnorm2;              // [n][h_z][w_z]: sum over channels of the squared layer-2 activation
+    float kappa_t;
     // EPI_MU (uses c_y), mu^k = acc + bias.  The conv input is [r so far | mu used so far | mu0 | pad] (bf16, in_stride
     // channels).  mu_last == 0: out has the same layout: r and mu blocks updated on partition mu_step.
     // mu_last == 1: out = dense y = r + mu, [pix][out_stride] (what A5 reads).
@@ -73,18 +78,19 @@ struct ConvProblem {
 };
 
 // ---- kernels (each .cu exposes host launchers; all enqueue on `st` and return cudaGetLastError()) -------------
-// Launch with programmatic stream serialization (PDL, see pdl_grid_sync in tc_ptx.cuh) and an optional cluster of cluster_x CTAs.
-// UFNVC_PDL=0 turns the attribute off (plain stream order) for A/B timing.
-inline bool pdl_enabled()
-{
-    static const bool on = [] { const char *e = std::getenv("UFNVC_PDL"); return !(e && e[0] == '0'); }();
-    return on;
-}
+// The stream a launcher enqueues on plus the per-handle launch mode.  pdl: launch with programmatic stream serialization
+// (see pdl_grid_sync in tc_ptx.cuh); off = plain stream order (ufnvc_config.debug_flags & UFNVC_DBG_NO_PDL, for A/B timing).
+struct LaunchStream {
+    cudaStream_t s;
+    bool pdl;
+    operator cudaStream_t() const { return s; }
+};
+// Launch with an optional cluster of cluster_x CTAs and, when st.pdl, programmatic stream serialization.
 template <typename... KArgs, typename... Args>
-inline cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t st, int cluster_x, Args &&...args)
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, LaunchStream st, int cluster_x, Args &&...args)
 {
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = st.s;
     cudaLaunchAttribute attr[2];
     unsigned n = 0;
     if (cluster_x > 1) {
@@ -92,7 +98,7 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned bl
         attr[n].val.clusterDim.x = unsigned(cluster_x); attr[n].val.clusterDim.y = 1; attr[n].val.clusterDim.z = 1;
         ++n;
     }
-    if (pdl_enabled()) {
+    if (st.pdl) {
         attr[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         attr[n].val.programmaticStreamSerializationAllowed = 1;
         ++n;
@@ -102,27 +108,36 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned bl
 }
 
 template <typename... KArgs, typename... Args>
-inline cudaError_t launch_pdl_grid(void (*kern)(KArgs...), dim3 grid, unsigned block, cudaStream_t st, Args &&...args)   // 3-D grid, no dynamic smem
+inline cudaError_t launch_pdl_grid(void (*kern)(KArgs...), dim3 grid, unsigned block, LaunchStream st, Args &&...args)   // 3-D grid, no dynamic smem
 {
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = grid; cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cfg.gridDim = grid; cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = 0; cfg.stream = st.s;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr; cfg.numAttrs = pdl_enabled() ? 1u : 0u;
+    cfg.attrs = attr; cfg.numAttrs = st.pdl ? 1u : 0u;
     return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
-cudaError_t launch_conv_generic(const ConvLayer &L, const ConvProblem &P, const EpiParams &E, cudaStream_t st);
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) for every kernel of a translation unit that needs more than 48 KB, on the
+// CURRENT device.  Function attributes are per device: ufnvc_create calls all of these for the device the handle lives on, so
+// the launchers hold no "already configured" state (a second handle on another GPU of the same process configures that GPU).
+cudaError_t configure_rans_kernels();
+cudaError_t configure_depthwise_kernels();
+cudaError_t configure_conv_tc_kernels();
+cudaError_t configure_trunk_kernels();
+cudaError_t configure_final_kernels();
+
+cudaError_t launch_conv_generic(const ConvLayer &L, const ConvProblem &P, const EpiParams &E, LaunchStream st);
 cudaError_t launch_dwconv3x3(const bf16 *in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
-                             int C, cudaStream_t st);
+                             int C, LaunchStream st);
 
 // progressive means, step 0 (R21): ymu0 = [partition 0 ? r : 0 | partition 0 ? mu0 : 0 | mu0 | pad], ymu1's mu0 block
 cudaError_t launch_mu_prep(const int16_t *sym, const float *mu0, bf16 *ymu0, bf16 *ymu1, int n_img, int H, int W, int c_y, int stride,
-                           cudaStream_t st);
+                           LaunchStream st);
 
 cudaError_t launch_dwconv3x3_tma(const CUtensorMap &tm_in, bf16 *out, const float *w9c, const float *bias, int n_img, int H, int W,
-                                 int C, cudaStream_t st, uint32_t *sched = nullptr, const uint32_t *dep_flags = nullptr);   // tm_in: NHWC map of `in` with box {64, 10, 10, 1}
+                                 int C, int num_sms, LaunchStream st, uint32_t *sched = nullptr, const uint32_t *dep_flags = nullptr);   // tm_in: NHWC map of `in` with box {64, 10, 10, 1}
 
 // fp64 hyper-decoder (A1 + A2), R12: the scale decision is taken in double on both sides.
 struct HyperLayer {
@@ -130,9 +145,9 @@ struct HyperLayer {
     double *w = nullptr;     // [9][c_in][n]
     double *bias = nullptr;  // [n]
 };
-cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z, int pz, cudaStream_t st);
+cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z, int pz, LaunchStream st);
 cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out, double *part, int n_img, int hz, int wz,
-                              cudaStream_t st, bf16 *xs = nullptr);   // part: [9][M][n] scratch for the split-tap fast path (may be null)
+                              LaunchStream st, bf16 *xs = nullptr, float *xnorm2 = nullptr);   // part: [9][M][n] scratch for the split-tap fast path (may be null)
 struct HeadParams {
     int c_y, h, w, n_buckets;
     double ln_lo, ln_hi;
@@ -140,12 +155,10 @@ struct HeadParams {
     uint8_t *idx;
 };
 // hybrid head helpers (hyper.cu)
-cudaError_t launch_hyper_reduce_split(const double *part, const double *bias, double *out, bf16 *xs, long long M, int n_out,
-                                      cudaStream_t st);
 cudaError_t launch_hyper_fix(const uint32_t *list, const uint32_t *count, const double *x2, const double *fix_w, const double *fix_b,
-                             int c_h, int hz, int wz, const HeadParams &hp, int num_sms, cudaStream_t st);
+                             int c_h, int hz, int wz, const HeadParams &hp, int num_sms, LaunchStream st);
 cudaError_t launch_hyper_head(const HyperLayer &L, const double *in, int n_img, int hz, int wz, const HeadParams &hp,
-                              cudaStream_t st);
+                              LaunchStream st);
 
 // rANS decode + dequantisation (A3 + A4)
 struct RansParams {
@@ -163,7 +176,7 @@ struct RansParams {
     float *yhat_tap;          // optional
     uint32_t *status;         // device word, OR-ed
 };
-cudaError_t launch_rans_decode(const RansParams &p, cudaStream_t st);
+cudaError_t launch_rans_decode(const RansParams &p, LaunchStream st);
 
 // GPU rANS encode (rans_encode.cu), mirror of the decoder: same geometry fields
 struct RansEncParams {
@@ -181,17 +194,17 @@ struct RansEncParams {
     uint32_t *sub_off;        // [n*n_sub + 1] byte offsets into bits_out
     uint32_t *status;
 };
-cudaError_t launch_rans_encode(const RansEncParams &p, cudaStream_t st);
+cudaError_t launch_rans_encode(const RansEncParams &p, LaunchStream st);
 // NEXT-3 (R22): decoded hyper-latent, channels-last int16 [n][pz][c_z] -> the planar [n][c_z][pz] layout of z_dev
-cudaError_t launch_z_hwc_to_planar(const int16_t *z_hwc, int16_t *z_planar, int n_chunks, int c_z, int pz, cudaStream_t st);
+cudaError_t launch_z_hwc_to_planar(const int16_t *z_hwc, int16_t *z_planar, int n_chunks, int c_z, int pz, LaunchStream st);
 
 // tcgen05 implicit-GEMM conv (conv_tc.cu)
 cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_in, int tile_h, int tile_w,
-                           bool flat, const EpiParams &E, int num_sms, cudaStream_t st);
+                           bool flat, const EpiParams &E, int num_sms, LaunchStream st);
 cudaError_t launch_conv_halo_pair(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
-                                  cudaStream_t st);
+                                  LaunchStream st);
 cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
-                             cudaStream_t st);
+                             LaunchStream st);
 bool tc_make_halo_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, std::string &err);
 bool tc_make_weight_tmap(ConvLayer &L, std::string &err, int block_n = 0);   // block_n = 0: widest N tile that divides n_pad
 bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, int tile_h, int tile_w,
@@ -210,7 +223,7 @@ struct FinalMaps {
 };
 bool final_make_maps(FinalMaps &m, const ConvLayer &L, const bf16 *in_base, int n_img, int H, int W, int out_w, std::string &err);
 cudaError_t launch_final_is(const FinalMaps &m, const ConvLayer &L, int n_img, int H, int W, float *out, int out_h, int out_w,
-                            int num_sms, cudaStream_t st);
+                            int num_sms, LaunchStream st);
 
 // fused trunk MLP (trunk_tc.cu): out = x + W2 GELU(W1 d + b1) + b2 in one kernel, hidden kept on chip
 struct TrunkMaps {
@@ -219,7 +232,7 @@ struct TrunkMaps {
 };
 bool trunk_make_maps(TrunkMaps &m, const bf16 *d_base, long long n_px, const ConvLayer &pw1, const ConvLayer &pw2, std::string &err);
 cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const ConvLayer &pw2, const bf16 *x, bf16 *out, long long n_px,
-                             int num_sms, bool pair, cudaStream_t st, uint32_t *tile_done = nullptr);
+                             int num_sms, bool pair, LaunchStream st, uint32_t *tile_done = nullptr);
 // the CTA-pair trunk kernel adds 1 to tile_done[tile] per epilogue warp of the CTA that owns the 128-pixel tile: a tile is
 // complete (written, and its input rows no longer read) when its counter reaches kTrunkTileSignals
 constexpr uint32_t kTrunkTileSignals = 8;

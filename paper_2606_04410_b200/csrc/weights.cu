@@ -54,7 +54,7 @@ struct Loader {
     {
         T *d = nullptr;
         if (cudaMalloc(&d, v.size() * sizeof(T)) != cudaSuccess) { err = "cudaMalloc failed (weights)"; return nullptr; }
-        h->allocs.push_back(d);
+        h->weight_allocs.push_back(d);
         if (cudaMemcpy(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess) { err = "cudaMemcpy failed (weights)"; return nullptr; }
         return d;
     }
@@ -131,7 +131,7 @@ struct Loader {
     // (channels [0,c_h) = hi, [c_h,2c_h) = mid, weights duplicated), plus the fp64 weights of the scale half laid out
     // per output row for the exact re-evaluation of elements that land near a bucket edge.
     // packed row n' = (s*16 + 4i+j) * c_y + c2   <-   canonical o = (s*c_y + c2)*16 + 4i+j   (s = 0: mu, 1: ln sigma)
-    bool head_hybrid(ConvLayer &L, double *&fix_w, double *&fix_b, const std::string &name, int c_h, int c_y)
+    bool head_hybrid(ConvLayer &L, double *&fix_w, double *&fix_b, float *&wnorm, const std::string &name, int c_h, int c_y)
     {
         const int n = 2 * c_y * 16;
         const Tensor *tw = get(name + ".w", {uint32_t(n), uint32_t(c_h), 3u, 3u});
@@ -141,10 +141,14 @@ struct Loader {
         std::vector<uint16_t> w(size_t(9) * n * L.c_in);
         std::vector<float> b(n);
         std::vector<double> fw(size_t(c_y) * 16 * 9 * c_h), fb(size_t(c_y) * 16);
+        std::vector<float> wn(n);                                  // |w row|_2, rounded up: input of the head's error bound
         for (int np = 0; np < n; ++np) {
             const int sij = np / c_y, c2 = np % c_y, sft = sij / 16, ij = sij % 16;
             const int o = (sft * c_y + c2) * 16 + ij;
             b[np] = tb->at(o);
+            double ss = 0.0;
+            for (size_t i = 0; i < size_t(9) * c_h; ++i) { const double v = double(tw->at(size_t(o) * 9 * c_h + i)); ss += v * v; }
+            wn[np] = std::nextafter(float(std::sqrt(ss)), INFINITY);
             for (int tap = 0; tap < 9; ++tap)
                 for (int c = 0; c < c_h; ++c) {
                     const float v = tw->at((size_t(o) * c_h + c) * 9 + tap);
@@ -157,8 +161,8 @@ struct Loader {
         }
         L.w = reinterpret_cast<bf16 *>(upload(w));
         L.bias = upload(b);
-        fix_w = upload(fw); fix_b = upload(fb);
-        return L.w && L.bias && fix_w && fix_b;
+        fix_w = upload(fw); fix_b = upload(fb); wnorm = upload(wn);
+        return L.w && L.bias && fix_w && fix_b && wnorm;
     }
 
     bool depthwise(float *&dw, float *&db, const std::string &name, int C)
@@ -185,6 +189,11 @@ int load_weights_impl(ufnvc_handle *h, const void *blob, size_t bytes)
     uint32_t n_t; std::memcpy(&n_t, p + 8, 4);
     if (n_t > 100000 || 16 + size_t(n_t) * sizeof(DirEntry) > bytes) return fail(h, UFNVC_E_BAD_BLOB, "directory exceeds blob");
     Loader ld; ld.h = h;
+    if (!h->weight_allocs.empty()) {                        // a reload replaces the previous weights: nothing may still read them
+        cudaDeviceSynchronize();
+        for (void *q : h->weight_allocs) cudaFree(q);
+        h->weight_allocs.clear();
+    }
     for (uint32_t i = 0; i < n_t; ++i) {
         DirEntry e; std::memcpy(&e, p + 16 + size_t(i) * sizeof(DirEntry), sizeof(DirEntry));
         e.name[39] = 0;
@@ -198,7 +207,7 @@ int load_weights_impl(ufnvc_handle *h, const void *blob, size_t bytes)
     const ufnvc_config &c = h->cfg;
     bool ok = ld.hyper(h->hyper[0], "hyper.0", c.c_z, c.c_hyper) && ld.hyper(h->hyper[1], "hyper.1", c.c_hyper, c.c_hyper) &&
               ld.hyper(h->hyper[2], "hyper.2", c.c_hyper, 2 * c.c_y * 16);
-    if (ok && h->hybrid_head) ok = ld.head_hybrid(h->head_tc, h->head_fix_w, h->head_fix_b, "hyper.2", c.c_hyper, c.c_y);
+    if (ok && h->hybrid_head) ok = ld.head_hybrid(h->head_tc, h->head_fix_w, h->head_fix_b, h->head_wnorm, "hyper.2", c.c_hyper, c.c_y);
     ok = ok && ld.conv(h->xframe, {"xframe"}, c.c_y, c.T * c.c_trunk, 1, false);
     for (int k = 1; ok && c.mu_steps == 4 && k <= 3; ++k) ok = ld.mu_net(h->mu_net[k - 1], "mu." + std::to_string(k), c.c_y);
     h->trunk.assign(c.n_trunk_blocks, ufnvc_handle::TrunkBlock());
@@ -224,6 +233,7 @@ int load_weights_impl(ufnvc_handle *h, const void *blob, size_t bytes)
         h->z_idx_c.resize(c.c_z);
         for (int ch = 0; ch < c.c_z; ++ch) {
             double u = double(tz->at(ch));
+            if (!std::isfinite(u)) return fail(h, UFNVC_E_BAD_BLOB, "zprior.lnscale holds a non-finite value");
             u = u < lo ? lo : (u > hi ? hi : u);
             const int k = int(std::floor(double(c.n_buckets - 1) * (u - lo) / (hi - lo) + 0.5));
             h->z_idx_c[ch] = uint8_t(k < 0 ? 0 : (k > c.n_buckets - 1 ? c.n_buckets - 1 : k));

@@ -155,3 +155,91 @@ def test_rans_lanes_are_independent_streams(orc, cdf):
     assert h0[1] == h1[1]
     n0 = 128 + 2 * int(h0[1])
     assert np.array_equal(d0[h0[0]:h0[0] + n0], d1[h1[0]:h1[0] + n0])
+
+
+def _scalar_lane_decode(cdf, idx, n, W, data):
+    """Textbook scalar rANS decoder (x -> (s, x') with x' = f (x >> 16) + slot - c, renormalise by one 16-bit word while
+    x < 2^16), written here with Python ints.  It walks the container warp-stream by warp-stream through ITS OWN header
+    entry (byte offset, word count) and inside a warp-stream step by step, lanes in ascending order.  Returns the
+    symbols, and per warp-stream (words consumed, words present, all lanes back at 2^16)."""
+    G = W // 32
+    hdr = np.frombuffer(data[:8 * G].tobytes(), np.uint32).reshape(G, 2)
+    steps = -(-n // W)
+    sym = np.zeros(n, np.int64)
+    info = []
+    for g in range(G):
+        off, nw = int(hdr[g, 0]), int(hdr[g, 1])
+        x = [int(v) for v in np.frombuffer(data[off:off + 128].tobytes(), np.uint32)]
+        words = np.frombuffer(data[off + 128:off + 128 + 2 * nw].tobytes(), np.uint16)
+        q = 0
+        for j in range(steps):
+            lanes = [l for l in range(32) if j * W + 32 * g + l < n]
+            for l in lanes:
+                i = j * W + 32 * g + l
+                c = cdf[idx[i]]
+                slot = x[l] & 0xFFFF
+                p = int(np.searchsorted(c, slot, side="right")) - 1
+                sym[i] = p - 127
+                x[l] = int(c[p + 1] - c[p]) * (x[l] >> 16) + slot - int(c[p])
+            for l in lanes:                      # renormalisation reads the words in ascending lane order
+                if x[l] < 1 << 16:
+                    x[l] = (x[l] << 16) | int(words[q])
+                    q += 1
+        info.append((q, nw, all(v == 1 << 16 for v in x)))
+    return sym, info
+
+
+@pytest.mark.parametrize("W,n", [(64, 64 * 37 + 5), (512, 512 * 9 + 300), (384, 384 * 7 + 33)])
+def test_rans_multi_warp_stream_container_against_scalar_decoder(orc, cdf, W, n):
+    """G > 1 warp-streams: every warp-stream owns header entry g, 32 start states and its own word run.  A per-warp-stream
+    offset / count mistake that the encoder mirrors would pass a round trip; it cannot pass a decoder written
+    separately that reads each header entry itself, nor the non-overlap and coverage checks on the byte ranges."""
+    rng = np.random.default_rng(W + n)
+    idx, sym = _random_case(orc, cdf, n, rng)
+    data = orc.rans_encode_substream(cdf, idx, sym, W)
+    got, info = _scalar_lane_decode(cdf, idx, n, W, data)
+    assert np.array_equal(got, sym)
+    assert all(q == nw and ended for q, nw, ended in info)
+    G = W // 32
+    hdr = data[:8 * G].view(np.uint32).reshape(G, 2)
+    spans = sorted((int(o), int(o) + 128 + 2 * int(c)) for o, c in hdr)
+    assert spans[0][0] == 8 * G and spans[-1][1] <= data.size <= spans[-1][1] + 3      # header, then the runs, then pad
+    for (a0, a1), (b0, b1) in zip(spans, spans[1:]):
+        assert a1 <= b0 <= a1 + 3 and b0 % 4 == 0                                     # disjoint, 4-byte aligned, no holes
+    # the oracle's own decoder agrees (status 0) and so does a decode after shuffling the ORDER of the warp-stream
+    # runs inside the container (header entries re-pointed): only the header ties a run to its lanes
+    out, st = orc.rans_decode_substream(cdf, idx, W, data)
+    assert st == 0 and np.array_equal(out, sym)
+    perm = rng.permutation(G)
+    parts, new_hdr, pos = [], np.zeros((G, 2), np.uint32), 8 * G
+    for g in perm:
+        o, c = int(hdr[g, 0]), int(hdr[g, 1])
+        run = data[o:o + 128 + 2 * c]
+        run = np.concatenate([run, np.zeros((-run.size) % 4, np.uint8)])
+        new_hdr[g] = (pos, c)
+        parts.append(run)
+        pos += run.size
+    moved = np.concatenate([new_hdr.view(np.uint8).ravel()] + parts)
+    out, st = orc.rans_decode_substream(cdf, idx, W, moved)
+    assert st == 0 and np.array_equal(out, sym)
+
+
+def test_rans_other_warp_streams_bytes_change_only_their_own_run(orc, cdf):
+    """Replace the symbols of warp-stream 1 (lanes 32..63) by a DIFFERENT random draw: warp-stream 0's states and words are
+    unchanged byte for byte, warp-stream 1's differ, and both decode back."""
+    rng = np.random.default_rng(12)
+    W, n = 64, 64 * 50
+    idx, sym = _random_case(orc, cdf, n, rng, 20, 64)
+    d0 = orc.rans_encode_substream(cdf, idx, sym, W)
+    sym2 = sym.copy().reshape(-1, W)
+    sym2[:, 32:] = orc.symbols_from_uniform(cdf, idx.reshape(-1, W)[:, 32:], rng.integers(0, 1 << 16, (n // W, 32)).astype(np.uint16))
+    assert (sym2 != sym.reshape(-1, W)).any()
+    d1 = orc.rans_encode_substream(cdf, idx, sym2.ravel(), W)
+    h0, h1 = d0[:16].view(np.uint32).reshape(2, 2), d1[:16].view(np.uint32).reshape(2, 2)
+    assert h0[0, 1] == h1[0, 1]
+    n0 = 128 + 2 * int(h0[0, 1])
+    assert np.array_equal(d0[h0[0, 0]:h0[0, 0] + n0], d1[h1[0, 0]:h1[0, 0] + n0])
+    r0, r1 = d0[h0[1, 0]:h0[1, 0] + 128 + 2 * int(h0[1, 1])], d1[h1[1, 0]:h1[1, 0] + 128 + 2 * int(h1[1, 1])]
+    assert r0.size != r1.size or not np.array_equal(r0, r1)
+    out, st = orc.rans_decode_substream(cdf, idx, W, d1)
+    assert st == 0 and np.array_equal(out, sym2.ravel())

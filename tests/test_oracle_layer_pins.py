@@ -115,6 +115,37 @@ def test_head_split_and_shuffle_by_hand(orc):
         assert u[c, i, j] == min(max(raw, math.log(cfg.scale_min)), math.log(cfg.scale_max))
 
 
+def test_head_crop_when_latent_is_not_a_multiple_of_4(orc):
+    """R2: h_z = ceil(h/4), w_z = ceil(w/4); the head is shuffled x4 to [4 h_z, 4 w_z] and cropped TOP-LEFT to [h, w].
+    160x224 padded frame: h = 10, w = 14, h_z = 3, w_z = 4 (shuffled map 12 x 16, two rows and two columns dropped).
+    z carries a position code through pass-through convs, the head adds its own channel number, so every element of
+    mu / u has a value known by hand: code(zy, zx) + (c 16 + 4 i + j) / 1024 at latent (4 zy + i, 4 zx + j)."""
+    cfg = synth.crop_config(synth.CONFIGS[1], 150, 200)
+    g = oracle.geometry(cfg)
+    assert (g["h"], g["w"], g["h_z"], g["w_z"]) == (10, 14, 3, 4)
+    w = {k: np.zeros_like(v) for k, v in synth.make_weights(cfg).items()}
+    for name in ("hyper.0.w", "hyper.1.w"):
+        w[name][0, 0, 1, 1] = 1.0                                # centre tap, channel 0 -> channel 0
+    w["hyper.2.w"][:, 0, 1, 1] = 1.0
+    n_head = 2 * cfg.c_y * 16
+    w["hyper.2.b"] = np.arange(n_head) / 1024.0
+    z = np.zeros((cfg.c_z, 3, 4), np.int16)
+    z[0] = np.arange(12).reshape(3, 4)                           # non-negative: ReLU passes it
+    mu, u, idx = oracle.entropy_params(orc, cfg, w, z)
+    assert mu.shape == (cfg.c_y, 10, 14) and u.shape == mu.shape and idx.shape == mu.shape
+    lo, hi = math.log(cfg.scale_min), math.log(cfg.scale_max)
+    for c in (0, 7, cfg.c_y - 1):
+        for ly in range(10):
+            for lx in range(14):
+                code = (ly // 4) * 4 + lx // 4
+                sub = 4 * (ly % 4) + lx % 4
+                assert mu[c, ly, lx] == code + (c * 16 + sub) / 1024.0
+                raw = code + ((cfg.c_y + c) * 16 + sub) / 1024.0
+                assert u[c, ly, lx] == min(max(raw, lo), hi)
+    # the dropped rows / columns are the BOTTOM / RIGHT ones: the last kept row is latent row 9 = (zy 2, i 1)
+    assert mu[0, 9, 13] == (2 * 4 + 3) + (4 * 1 + 1) / 1024.0
+
+
 def test_trunk_block_identity_when_w2_zero(orc):
     cfg = synth.crop_config(synth.CONFIGS[2], 32, 48)
     wts = synth.make_weights(cfg)
@@ -167,3 +198,21 @@ def test_end_to_end_tiny_round_trip_and_fp32_vs_fp64(orc, orc32):
     assert np.array_equal(o32["sym"], st["sym"])
     assert np.abs(o32["frames"] - f).max() <= 1e-4                     # bounds the fp32 variant's own error
     assert np.abs(o32["mu"] - st["mu"]).max() <= 1e-4
+
+
+def test_fp32_oracle_vs_fp64_on_a_config2_crop_with_trunk(orc, orc32):
+    """SURVEY.md 8c "fp32 oracle vs an fp64 run of the same loops <= 1e-4 on configs 1-2": the plain-fp32 build that
+    BASELINE.json names, against the fp64 build the parity tests use as truth (R12/R24), on config 2's layer
+    plan (bf16 weights, 4 trunk blocks, 256 -> 3 decoders) at a 96 x 64 crop.  Indices are teacher-forced (the bucket
+    decision is taken in fp64 by definition, R12), so the comparison is about the arithmetic of O5..O9 only."""
+    cfg = synth.crop_config(synth.CONFIGS[2], 64, 96)
+    wts, z, u16 = synth.make_weights(cfg), synth.make_z(cfg), synth.make_uniform16(cfg)
+    st = oracle.make_stream(orc, cfg, wts, z[0], u16[0])
+    a = oracle.chunk_decode(orc, cfg, wts, z[0], st["bits"], st["sub_off"], keep=True)
+    b = oracle.chunk_decode(orc32, cfg, wts, z[0], st["bits"], st["sub_off"], idx_override=st["idx"], keep=True)
+    assert a["status"] == 0 and b["status"] == 0 and np.array_equal(a["sym"], b["sym"])
+    assert np.abs(b["mu"] - a["mu"]).max() <= 1e-4
+    assert (b["idx"] == a["idx"]).all()
+    for t in range(cfg.T):
+        assert np.abs(b["taps"]["trunk"][t] - a["taps"]["trunk"][t]).max() <= 1e-4 * max(1.0, np.abs(a["taps"]["trunk"][t]).max())
+    assert np.abs(b["frames"] - a["frames"]).max() <= 1e-4
