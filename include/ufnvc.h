@@ -73,6 +73,10 @@ typedef struct ufnvc_config {
     uint32_t debug_flags;        /* 0 = the default (fastest) kernels.  OR of UFNVC_DBG_*: each bit swaps one GPU kernel or
                                   * launch mechanism for its slower cross-check variant (never a CPU path).  Per handle;
                                   * the library reads no environment variable and keeps no process-wide state. */
+    int32_t n_ctx_blocks;        /* 0: no temporal context (BASELINE.json's layer plans).  > 0: temporal chunk context (PAPER.md:
+                                  * 79-81, 125, 356; R23) with that many DC blocks in the cross-chunk context generation
+                                  * (11 / 12 / 9 for the paper's HT-S / HT-L / LD): the handle carries the state C_i from call to
+                                  * call (ufnvc_reset_context starts a new video).  Needs c_trunk == 256 and the ctx.* tensors. */
 } ufnvc_config;
 
 /* ufnvc_config.debug_flags: A/B and cross-check switches (tests/test_gpu_parity.py runs every one against the oracle) */
@@ -111,7 +115,10 @@ int ufnvc_destroy(ufnvc_handle *h);
  *                 uint64 offset (from blob start, 16-byte aligned); uint64 nbytes };
  *   data.
  * Tensors (canonical [C_out][C_in][kh][kw], biases fp32 [C_out]): hyper.{0,1,2}.{w,b}, xframe.{w,b},
- * trunk.{k}.{dw,pw1,pw2}.{w,b}, dec.{t}.{s}.{w,b} (t < T, s < 4), and with mu_steps == 4 mu.{1,2,3}.{w,b}
+ * trunk.{k}.{dw,pw1,pw2}.{w,b}, dec.{t}.{s}.{w,b} (t < T, s < 4); with n_ctx_blocks > 0 xframe.w is
+ * [T c_trunk][c_y + c_trunk][1][1] (input = [y ; C_i]) and ctx.fold.{w,b} [c_trunk][T c_trunk][1][1],
+ * ctx.{k}.{dw,pw1,pw2}.{w,b} (k < n_ctx_blocks, shapes of a trunk block), ctx.out.{w,b} [c_trunk][c_trunk][1][1],
+ * ctx.prior.{w,b} [c_hyper][c_trunk][1][1] are required (R23); with mu_steps == 4 mu.{1,2,3}.{w,b}
  * ([c_y][2 c_y][3][3]: input channels [0, c_y) = y decoded so far, [c_y, 2 c_y) = the head's mean); optional
  * zprior.lnscale (fp32 [c_z], see the bytes-only entry points).
  * Missing / mis-shaped tensor: UFNVC_E_BAD_BLOB. */
@@ -142,6 +149,20 @@ int ufnvc_decode_z(ufnvc_handle *h, int n_chunks, const uint8_t *bits_dev, size_
 int ufnvc_chunk_decode_bytes(ufnvc_handle *h, int n_chunks, const uint8_t *bits_dev, size_t bits_bytes,
                              const uint32_t *sub_off_dev, float *frames_dev, void *cuda_stream);
 
+/* ---- temporal chunk context (SURVEY.md 8f NEXT-2a, R23; only with n_ctx_blocks > 0, else UFNVC_E_BAD_CONFIG).
+ * the chunk decoder's feature F_i "is also propagated to the next chunk to form the next temporal context";
+ * the chunk decoder and the prior are conditioned on C_i.  State per chunk slot of a call (slot k of
+ * successive calls = successive chunks of video k): C_i, a bf16 tensor [c_trunk] per latent pixel.  ufnvc_chunk_decode
+ * (and _ex / _bytes / _profiled with frames) decodes under the current state and replaces it by C_{i+1}; a call that stops
+ * after the entropy stage (frames_dev NULL) and ufnvc_entropy_params read the state and leave it alone.  A fresh handle
+ * holds the zero context. ---- */
+
+/* C = 0 for the first n_chunks slots (start of a new video).  Asynchronous on cuda_stream. */
+int ufnvc_reset_context(ufnvc_handle *h, int n_chunks, void *cuda_stream);
+/* Copy the state out / in: ctx_dev bf16 [n_chunks][h][w][c_trunk] (parity hooks: teacher-forced context). */
+int ufnvc_get_context(ufnvc_handle *h, int n_chunks, uint16_t *ctx_dev, void *cuda_stream);
+int ufnvc_set_context(ufnvc_handle *h, int n_chunks, const uint16_t *ctx_dev, void *cuda_stream);
+
 /* Same, with parity hooks: idx_override_dev / mu_override_dev ([n][h][w][c_y], may be NULL) replace the
  * hyper-decoder's indices / means ("teacher forcing", R12; the entropy-only mode of DESIGN.md);
  * taps (may be NULL) receives intermediates.  frames_dev may be NULL to stop after the entropy stage. */
@@ -166,9 +187,10 @@ int ufnvc_launches_per_call(const ufnvc_handle *h, int n_chunks);
 
 /* Per-stage device time of the LAST ufnvc_chunk_decode_profiled call, in microseconds.
  * ufnvc_chunk_decode_profiled = ufnvc_chunk_decode with a cudaEvent after each stage A1+A2, A3+A4, A5, A6+A7
- * (all trunk blocks), A8 (stages 1-3), A9; it synchronises the stream at the end.  us_out_host[7]: the six stages, then
- * [6] = A6 alone (sum of the depthwise launches; A7 = [3] - [6]) when detail != 0 (two more events per trunk block, which
- * cost a few microseconds of launch gaps), else 0. */
+ * (all trunk blocks), A8 (stages 1-3), A9, context generation; it synchronises the stream at the end.  us_out_host[8]: the
+ * six stages, then [6] = A6 alone (sum of the depthwise launches, serialised by their own events) when detail != 0 (two
+ * more events per trunk block, which cost a few microseconds of launch gaps), else 0; [7] = context generation (R23; 0
+ * without a temporal context). */
 int ufnvc_chunk_decode_profiled(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, const uint8_t *bits_dev,
                                 size_t bits_bytes, const uint32_t *sub_off_dev, float *frames_dev,
                                 void *cuda_stream, int detail, float *us_out_host);

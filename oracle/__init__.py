@@ -150,13 +150,46 @@ def geometry(cfg):
 # ---------------------------------------------------------------------------------------------
 # the path, in the paper's order
 # ---------------------------------------------------------------------------------------------
-def entropy_params(orc: Oracle, cfg, weights, z):
+def round_bf16(a):
+    """Nearest-even rounding to bfloat16 (8 significant bits), returned in the input's float type.  The temporal context
+    state is DEFINED as a bf16 tensor (R19/R23): this is the one place the oracle applies a storage rounding."""
+    u = np.ascontiguousarray(a, dtype=np.float32).view(np.uint32)
+    r = ((u >> 16) & 1) + np.uint32(0x7FFF)
+    return ((u + r) & np.uint32(0xFFFF0000)).view(np.float32).astype(np.asarray(a).dtype)
+
+
+def has_context(cfg):
+    return getattr(cfg, "n_ctx_blocks", 0) > 0
+
+
+def zero_context(cfg):
+    g = geometry(cfg)
+    return np.zeros((cfg.c_trunk, g["h"], g["w"]), np.float64)
+
+
+def context_prior(orc: Oracle, cfg, weights, ctx):
+    """NEXT-2a, reading R23 (the prior input s_i is "derived from hyper-prior z_i and temporal context
+    C_i"; how is not in the text).  R23: the context enters the hyper-decoder at the hyper-latent's resolution as
+    q = ReLU(W_p pool4(C_i) + b_p), pool4 = mean over the 4 x 4 block of latent pixels under a z-pixel (zeros past the
+    latent's edge, always divided by 16), W_p a 1x1 conv C_c -> C_h; s = x2 + q feeds the head conv.
+    ctx [C_c][h][w].  Returns q [C_h][h_z][w_z]."""
+    g = geometry(cfg)
+    c = np.zeros((ctx.shape[0], 4 * g["h_z"], 4 * g["w_z"]), orc.dt)
+    c[:, :g["h"], :g["w"]] = ctx
+    pool = c.reshape(ctx.shape[0], g["h_z"], 4, g["w_z"], 4).sum(axis=(2, 4)) / 16.0
+    return orc.relu(orc.conv2d(pool, weights["ctx.prior.w"], weights["ctx.prior.b"]))
+
+
+def entropy_params(orc: Oracle, cfg, weights, z, ctx=None):
     """O1 + O2 (one forward pass gives the scale of every element and the mean).
-    z: int [C_z][h_z][w_z].  Returns mu, u = clamped ln sigma, idx, each [C_y][h][w]."""
+    z: int [C_z][h_z][w_z]; ctx: the temporal chunk context C_i [C_c][h][w] when the config has one (R23).
+    Returns mu, u = clamped ln sigma, idx, each [C_y][h][w]."""
     g = geometry(cfg)
     x0 = orc.arr(z)
     x1 = orc.relu(orc.conv2d(x0, weights["hyper.0.w"], weights["hyper.0.b"]))
     x2 = orc.relu(orc.conv2d(x1, weights["hyper.1.w"], weights["hyper.1.b"]))
+    if has_context(cfg):
+        x2 = x2 + context_prior(orc, cfg, weights, zero_context(cfg) if ctx is None else ctx)     # s_i (R23)
     x3 = orc.conv2d(x2, weights["hyper.2.w"], weights["hyper.2.b"])
     ps = orc.pixel_shuffle(x3, 4)[:, :g["h"], :g["w"]]
     mu = np.ascontiguousarray(ps[:cfg.c_y])
@@ -302,12 +335,18 @@ def progressive_means(orc: Oracle, cfg, weights, mu0, sym):
     return yhat, mu
 
 
-def synthesis(orc: Oracle, cfg, weights, yhat, keep=False, only_frames=None):
+def synthesis(orc: Oracle, cfg, weights, yhat, keep=False, only_frames=None, ctx=None, want_features=False):
     """O6..O9: cross-frame unfold, shared trunk of DC blocks, T frame-specific
     decoders, clamp + crop.  yhat [C_y][h][w].  Returns frames [T][3][height][width] (+ taps).
     only_frames: frame indices to compute (the T frames are independent after O6, PAPER.md:85 "operating in parallel");
     the others are left as NaN -- used by the full-size parity tests of configs 4 and 5 to bound the oracle's time."""
     taps = {}
+    if has_context(cfg):
+        # R23 (PAPER.md:79 "conditioned on the temporal chunk context C_i"): the chunk decoder's first layer sees the
+        # concatenation [y ; C_i]; xframe.w is [T*C_t][C_y + C_c][1][1]
+        yhat = np.concatenate([orc.arr(yhat), orc.arr(zero_context(cfg) if ctx is None else ctx)], axis=0)
+    if want_features:
+        taps["features"] = [None] * cfg.T                                      # F_i, the trunk's output per frame
     f0 = orc.conv2d(yhat, weights["xframe.w"], weights["xframe.b"])            # O6: [T*C_t][h][w]
     frames = np.full((cfg.T, 3, cfg.height, cfg.width), np.nan, orc.dt)
     if keep:
@@ -322,6 +361,8 @@ def synthesis(orc: Oracle, cfg, weights, yhat, keep=False, only_frames=None):
             x = x + orc.conv2d(e, weights[f"trunk.{k}.pw2.w"], weights[f"trunk.{k}.pw2.b"])
         if keep:
             taps["trunk"].append(x.copy())           # (indexed by position in only_frames when that is given)
+        if want_features:
+            taps["features"][t] = x.copy()
         for s in range(4):                                                     # O8 [R10]
             a = orc.conv2d(x, weights[f"dec.{t}.{s}.w"], weights[f"dec.{t}.{s}.b"])
             if s < 3:
@@ -333,9 +374,26 @@ def synthesis(orc: Oracle, cfg, weights, yhat, keep=False, only_frames=None):
     return frames, taps
 
 
-def chunk_decode(orc: Oracle, cfg, weights, z, bits, sub_off, idx_override=None, mu_override=None, keep=False):
-    """One chunk, O1..O9.  z [C_z][h_z][w_z]; bits uint8; sub_off [n_sub+1] byte offsets into bits."""
-    mu, u, idx = entropy_params(orc, cfg, weights, z)
+def context_generation(orc: Oracle, cfg, weights, features):
+    """NEXT-2a, reading R23.  PAPER.md:81: the feature F_i "is also propagated to the next chunk to form the next temporal
+    context"; PAPER.md:356 (Supp. B): the cross-chunk context generation module is a stack of DC blocks (11 for HT-S).
+    R23: C_{i+1} = bf16( conv1x1_out( DCblock^{B_c}( conv1x1_fold( [F_i[0]; ...; F_i[T-1]] ) ) ) ), the fold mixing the T
+    per-frame features (T*C_t channels) into one C_c-channel map at latent resolution -- the mirror of the cross-frame
+    unfold O6 -- and the DC block being O7's (depthwise 3x3, 1x1 x4, GELU, 1x1, residual).
+    features: list of T arrays [C_t][h][w].  Returns C_{i+1} [C_c][h][w], bf16-representable values."""
+    x = orc.conv2d(np.concatenate([orc.arr(f) for f in features], axis=0), weights["ctx.fold.w"], weights["ctx.fold.b"])
+    for k in range(cfg.n_ctx_blocks):
+        d = orc.dwconv3x3(x, weights[f"ctx.{k}.dw.w"], weights[f"ctx.{k}.dw.b"])
+        e = orc.gelu(orc.conv2d(d, weights[f"ctx.{k}.pw1.w"], weights[f"ctx.{k}.pw1.b"]))
+        x = x + orc.conv2d(e, weights[f"ctx.{k}.pw2.w"], weights[f"ctx.{k}.pw2.b"])
+    return round_bf16(orc.conv2d(x, weights["ctx.out.w"], weights["ctx.out.b"]))
+
+
+def chunk_decode(orc: Oracle, cfg, weights, z, bits, sub_off, idx_override=None, mu_override=None, keep=False, ctx=None):
+    """One chunk, O1..O9.  z [C_z][h_z][w_z]; bits uint8; sub_off [n_sub+1] byte offsets into bits.  With a temporal
+    context in the config (R23): ctx = C_i (None = the zero context of a sequence's first chunk); the result then
+    also carries "ctx_next" = C_{i+1}."""
+    mu, u, idx = entropy_params(orc, cfg, weights, z, ctx=ctx)
     if idx_override is not None:
         idx = np.ascontiguousarray(idx_override, np.uint8)
     if mu_override is not None:
@@ -346,14 +404,31 @@ def chunk_decode(orc: Oracle, cfg, weights, z, bits, sub_off, idx_override=None,
         yhat, mu = progressive_means(orc, cfg, weights, mu, sym)               # NEXT-1: mu becomes the per-element mean used
     else:
         yhat = sym.astype(orc.dt) + mu                                         # O5
-    frames, taps = synthesis(orc, cfg, weights, yhat, keep=keep)
-    return dict(mu=mu, u=u, idx=idx, sym=sym, status=status, yhat=yhat, frames=frames, taps=taps)
+    frames, taps = synthesis(orc, cfg, weights, yhat, keep=keep, ctx=ctx, want_features=has_context(cfg))
+    out = dict(mu=mu, u=u, idx=idx, sym=sym, status=status, yhat=yhat, frames=frames, taps=taps)
+    if has_context(cfg):
+        out["ctx_next"] = context_generation(orc, cfg, weights, taps["features"])
+    return out
 
 
-def make_stream(orc: Oracle, cfg, weights, z, u16_hwc, idx_override=None):
-    """Fixture: what an encoder would have produced for this z -- run the prior net (O1, O2), draw r from the
-    quantised tables by inverse CDF with the given 16-bit uniforms [h][w][C_y] (R7), encode (mirror of O4)."""
-    mu, u, idx = entropy_params(orc, cfg, weights, z)
+def chunk_decode_sequence(orc: Oracle, cfg, weights, zs, streams, keep=False):
+    """Successive chunks of ONE video ("a sequential chunk-by-chunk coding process"): C_0 = 0, chunk i is
+    decoded under C_i and hands C_{i+1} on.  streams[i] = (bits, sub_off).  Returns the list of per-chunk results, each
+    with the context it was decoded under ("ctx")."""
+    ctx, outs = zero_context(cfg), []
+    for z, (bits, sub_off) in zip(zs, streams):
+        out = chunk_decode(orc, cfg, weights, z, bits, sub_off, keep=keep, ctx=ctx)
+        out["ctx"] = ctx
+        outs.append(out)
+        ctx = out["ctx_next"]
+    return outs
+
+
+def make_stream(orc: Oracle, cfg, weights, z, u16_hwc, idx_override=None, ctx=None):
+    """Fixture: what an encoder would have produced for this z -- run the prior net (O1, O2; under the context C_i when
+    the config has one), draw r from the quantised tables by inverse CDF with the given 16-bit uniforms [h][w][C_y]
+    (R7), encode (mirror of O4)."""
+    mu, u, idx = entropy_params(orc, cfg, weights, z, ctx=ctx)
     if idx_override is not None:
         idx = np.ascontiguousarray(idx_override, np.uint8)
     cdf = orc.build_cdf(cfg.n_buckets, cfg.scale_min, cfg.scale_max)

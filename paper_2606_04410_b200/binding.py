@@ -27,7 +27,7 @@ class ufnvc_config(C.Structure):
                 ("n_buckets", C.c_int32), ("scale_min", C.c_double), ("scale_max", C.c_double),
                 ("rows_per_substream", C.c_int32), ("lanes_per_substream", C.c_int32),
                 ("max_chunks_per_call", C.c_int32), ("weight_dtype", C.c_int32), ("mu_steps", C.c_int32),
-                ("debug_flags", C.c_uint32)]
+                ("debug_flags", C.c_uint32), ("n_ctx_blocks", C.c_int32)]
 
 
 class ufnvc_taps(C.Structure):
@@ -62,6 +62,9 @@ def _load():
         "ufnvc_get_z_prior_index": (i, [vp, vp]),
         "ufnvc_encode_z": (C.c_long, [vp, vp, vp, sz, vp]),
         "ufnvc_encode_chunk_dev": (i, [vp, i, vp, vp, vp, sz, vp, vp]),
+        "ufnvc_reset_context": (i, [vp, i, vp]),
+        "ufnvc_get_context": (i, [vp, i, vp, vp]),
+        "ufnvc_set_context": (i, [vp, i, vp, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -73,7 +76,8 @@ LIB = _load()
 EXPORTS = ("ufnvc_create", "ufnvc_destroy", "ufnvc_load_weights", "ufnvc_chunk_decode", "ufnvc_chunk_decode_ex",
            "ufnvc_entropy_params", "ufnvc_get_status", "ufnvc_last_error", "ufnvc_launches_per_call",
            "ufnvc_chunk_decode_profiled", "ufnvc_debug_counter", "ufnvc_get_cdf", "ufnvc_symbols_from_uniform", "ufnvc_encode_chunk",
-           "ufnvc_decode_z", "ufnvc_chunk_decode_bytes", "ufnvc_get_z_prior_index", "ufnvc_encode_z", "ufnvc_encode_chunk_dev")
+           "ufnvc_decode_z", "ufnvc_chunk_decode_bytes", "ufnvc_get_z_prior_index", "ufnvc_encode_z", "ufnvc_encode_chunk_dev",
+           "ufnvc_reset_context", "ufnvc_get_context", "ufnvc_set_context")
 
 
 # ufnvc_config.debug_flags (include/ufnvc.h)
@@ -92,6 +96,7 @@ def make_config(cfg, max_chunks: int | None = None, debug_flags: int = 0) -> ufn
     c.max_chunks_per_call = max_chunks if max_chunks is not None else getattr(cfg, "n_chunks", 1)
     c.mu_steps = getattr(cfg, "mu_steps", 1)
     c.debug_flags = debug_flags
+    c.n_ctx_blocks = getattr(cfg, "n_ctx_blocks", 0)
     return c
 
 
@@ -219,6 +224,19 @@ class ChunkDecoder:
         out["frames"] = frames
         return out
 
+    # ---- temporal chunk context (NEXT-2a, R23) ----
+    def reset_context(self, n_chunks=1, stream=None):
+        self._check(LIB.ufnvc_reset_context(self.handle, n_chunks, self._stream(stream)), "ufnvc_reset_context")
+
+    def get_context(self, n_chunks=1, stream=None):
+        ctx = torch.empty((n_chunks, self.h, self.w, self.cfg.c_trunk), dtype=torch.bfloat16, device=self.device)
+        self._check(LIB.ufnvc_get_context(self.handle, n_chunks, _ptr(ctx), self._stream(stream)), "ufnvc_get_context")
+        return ctx
+
+    def set_context(self, ctx, stream=None):
+        assert ctx.dtype == torch.bfloat16 and ctx.shape[1:] == (self.h, self.w, self.cfg.c_trunk)
+        self._check(LIB.ufnvc_set_context(self.handle, ctx.shape[0], _ptr(ctx), self._stream(stream)), "ufnvc_set_context")
+
     # ---- bytes-only entry points (NEXT-3, R22) ----
     def decode_z(self, bits, sub_off, n_chunks=1, stream=None):
         z = torch.empty((n_chunks, self.cfg.c_z, self.h_z, self.w_z), dtype=torch.int16, device=self.device)
@@ -282,10 +300,10 @@ class ChunkDecoder:
         return self._check(LIB.ufnvc_launches_per_call(self.handle, n_chunks), "ufnvc_launches_per_call")
 
     def chunk_decode_profiled(self, z, bits, sub_off, frames, stream=None, detail=False):
-        us = (C.c_float * 7)()
+        us = (C.c_float * 8)()
         self._check(LIB.ufnvc_chunk_decode_profiled(self.handle, z.shape[0], _ptr(z), _ptr(bits), bits.numel(), _ptr(sub_off),
                                                     _ptr(frames), self._stream(stream), int(detail), us), "ufnvc_chunk_decode_profiled")
-        return dict(zip(("A1+A2", "A3+A4", "A5", "A6+A7", "A8", "A9", "A6"), [float(x) for x in us]))
+        return dict(zip(("A1+A2", "A3+A4", "A5", "A6+A7", "A8", "A9", "A6", "ctx"), [float(x) for x in us]))
 
     # ---- encoder-side fixtures (host) ----
     def get_cdf(self) -> np.ndarray:

@@ -50,6 +50,12 @@ int validate(const ufnvc_config &c, std::string &why)
     BAD(c.mu_steps != 1 && c.mu_steps != 4, "mu_steps must be 1 or 4");
     BAD(c.mu_steps == 4 && c.c_y % 32, "mu_steps == 4 needs c_y % 32 == 0 (the mean convs run on tensor cores only)");
     BAD(c.debug_flags & ~0xFFu, "unknown debug_flags bit");
+    BAD(c.n_ctx_blocks < 0 || c.n_ctx_blocks > 64, "n_ctx_blocks out of range");
+    BAD(c.n_ctx_blocks > 0 && (c.c_trunk != 256 || (c.c_trunk * c.trunk_expand) % 128 || c.c_y % 64 || c.weight_dtype != 1 ||
+                               c.c_hyper % 16 || c.c_z % 16),
+        "a temporal context needs c_trunk == 256, c_y % 64 == 0, bf16 weights (the context generation runs on the fused tensor-core kernels)");
+    BAD(c.n_ctx_blocks > 0 && (c.debug_flags & (UFNVC_DBG_FORCE_GENERIC | UFNVC_DBG_UNFUSED_TRUNK | UFNVC_DBG_PLAIN_DEPTHWISE)),
+        "the context generation has no CUDA-core / unfused / plain-depthwise variant");
     BAD(c.mu_steps == 4 && (c.debug_flags & UFNVC_DBG_FORCE_GENERIC), "mu_steps == 4 has no CUDA-core variant");
     // every kernel indexes latent elements and activation pixels with 32-bit integers (byte offsets are 64-bit)
     {
@@ -89,6 +95,8 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     h->n_sub = (h->h + cfg->rows_per_substream - 1) / cfg->rows_per_substream;
     h->n_sub_z = (h->h_z + cfg->rows_per_substream - 1) / cfg->rows_per_substream;
     h->max_chunks = cfg->max_chunks_per_call;
+    h->has_ctx = cfg->n_ctx_blocks > 0;
+    h->c_cat = cfg->c_y + (h->has_ctx ? cfg->c_trunk : 0);
     const uint32_t dbg = cfg->debug_flags;
     h->force_generic = dbg & UFNVC_DBG_FORCE_GENERIC;
     h->use_fused_trunk = !(dbg & UFNVC_DBG_UNFUSED_TRUNK);
@@ -100,10 +108,10 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     h->hybrid_head = !(dbg & UFNVC_DBG_FP64_HEAD) && cfg->weight_dtype == 1 && cfg->c_y % 32 == 0 && cfg->c_hyper % 32 == 0 &&
                      !h->force_generic;
     // Error model of the tensor-core head (R12): ln sigma = sum of K = 9 * 2 c_hyper exact bf16 x bf16 products
-    // accumulated in fp32.  (i) the 2-term split drops |x - hi - mid| <= 2^-18 |x| (two round-to-nearest steps of 8
-    // bits); (ii) K fp32 additions: probabilistic rounding bound lambda sqrt(K) 2^-24 sum|terms| with lambda = 3.
+    // accumulated in fp32.  (i) the 2-term split drops |x - hi - mid| <= 2^-16 |x| (two round-to-nearest steps to 8
+    // significant bits, unit roundoff 2^-8 each); (ii) K fp32 additions: probabilistic rounding bound lambda sqrt(K) 2^-24 sum|terms| with lambda = 3.
     // sum |w||x| <= |w|_2 |x|_2 (Cauchy-Schwarz), so |error| <= kappa |w row|_2 |x patch|_2.
-    h->head_kappa = std::ldexp(1.0, -18) + 3.0 * std::sqrt(18.0 * cfg->c_hyper) * std::ldexp(1.0, -24);
+    h->head_kappa = std::ldexp(1.0, -16) + 3.0 * std::sqrt(18.0 * cfg->c_hyper) * std::ldexp(1.0, -24);
     // function attributes are per device: configure every kernel for the device this handle lives on
     if (configure_rans_kernels() != cudaSuccess || configure_depthwise_kernels() != cudaSuccess || configure_conv_tc_kernels() != cudaSuccess ||
         configure_trunk_kernels() != cudaSuccess || configure_final_kernels() != cudaSuccess) {
@@ -114,7 +122,7 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
 
     // O3 tables + search accelerator
     build_cdf_tables(cfg->n_buckets, cfg->scale_min, cfg->scale_max, h->cdf32);
-    std::vector<uint16_t> lut;
+    std::vector<uint32_t> lut;
     std::vector<uint32_t> cf(h->cdf32.size(), 0u);
     build_search_lut(h->cdf32, cfg->n_buckets, lut);
     for (size_t i = 0; i < cf.size(); ++i)                                          // pos 255 is never a symbol
@@ -126,12 +134,12 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
               dev_alloc(h, h->hx2, n * Pz * cfg->c_hyper) && dev_alloc(h, h->xs, n * Pz * 2 * cfg->c_hyper) && dev_alloc(h, h->xnorm2, n * Pz) &&
               dev_alloc(h, h->fix_list, n * P * cfg->c_y) && dev_alloc(h, h->hpart, 9 * n * Pz * cfg->c_hyper) && dev_alloc(h, h->mu, n * P * cfg->c_y) &&
               dev_alloc(h, h->lnscale, n * P * cfg->c_y) && dev_alloc(h, h->idx, n * P * cfg->c_y) &&
-              dev_alloc(h, h->yhat, n * P * cfg->c_y) && dev_alloc(h, h->fa, n * T * P * cfg->c_trunk) &&
+              dev_alloc(h, h->yhat, n * P * size_t(h->c_cat)) && dev_alloc(h, h->fa, n * T * P * cfg->c_trunk) &&
               dev_alloc(h, h->fb, n * T * P * cfg->c_trunk) &&
-              dev_alloc(h, h->zero_block, 4 + size_t(cfg->n_trunk_blocks > 0 ? cfg->n_trunk_blocks : 1) * ((n * T * P + 127) / 128 + 4)) &&
+              dev_alloc(h, h->zero_block, 4 + size_t(cfg->n_trunk_blocks + cfg->n_ctx_blocks + 1) * ((n * T * P + 127) / 128 + 4)) &&
               dev_alloc(h, h->hidden, cfg->n_trunk_blocks ? n * T * P * cfg->c_trunk * cfg->trunk_expand : 1);
     if (ok) {      // everything a call clears up front sits in one block so that ONE memset node does it (decode.cu run())
-        h->zero_words = 4 + size_t(cfg->n_trunk_blocks > 0 ? cfg->n_trunk_blocks : 1) * ((n * T * P + 127) / 128 + 4);
+        h->zero_words = 4 + size_t(cfg->n_trunk_blocks + cfg->n_ctx_blocks + 1) * ((n * T * P + 127) / 128 + 4);
         h->d_status = h->zero_block; h->fix_count = h->zero_block + 1; h->trunk_sync = h->zero_block + 4;
         ok = cudaMemset(h->zero_block, 0, h->zero_words * 4) == cudaSuccess;
     }
@@ -143,9 +151,12 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     ok = ok && dev_alloc(h, h->z_idx, n * Pz * cfg->c_z) && dev_alloc(h, h->z_zero_mu, n * Pz * cfg->c_z) &&
          dev_alloc(h, h->z_scratch, n * Pz * cfg->c_z) && dev_alloc(h, h->z_hwc, n * Pz * cfg->c_z) &&
          dev_alloc(h, h->z_planar, n * Pz * cfg->c_z) && cudaMemset(h->z_zero_mu, 0, n * Pz * cfg->c_z * 4) == cudaSuccess;
+    if (ok && h->has_ctx)
+        ok = dev_alloc(h, h->ca, n * P * cfg->c_trunk) && dev_alloc(h, h->cb, n * P * cfg->c_trunk) && dev_alloc(h, h->ctx_q, n * Pz * cfg->c_hyper) &&
+             cudaMemset(h->yhat, 0, n * P * size_t(h->c_cat) * 2) == cudaSuccess && cudaMemset(h->ctx_q, 0, n * Pz * cfg->c_hyper * 8) == cudaSuccess;
     for (int s = 0; ok && s < 3; ++s) ok = dev_alloc(h, h->stage[s], n * T * (P << (2 * (s + 1))) * cfg->dec_channels[s + 1]);
     if (ok) ok = cudaMemcpy(h->d_cf, cf.data(), cf.size() * 4, cudaMemcpyHostToDevice) == cudaSuccess &&
-                 cudaMemcpy(h->d_lut, lut.data(), lut.size() * 2, cudaMemcpyHostToDevice) == cudaSuccess &&
+                 cudaMemcpy(h->d_lut, lut.data(), lut.size() * 4, cudaMemcpyHostToDevice) == cudaSuccess &&
                  cudaMemset(h->d_status, 0, 4) == cudaSuccess;
     if (!ok) {
         cudaGetLastError();

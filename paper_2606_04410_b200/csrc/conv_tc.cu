@@ -56,6 +56,7 @@ struct TcParams {
     int tiles_y, tiles_x, TH, TW;
     int H, W;                     // real image dims: global pixel -> (img, y, x) for the epilogue
     int taps, slabs;              // k-blocks per tile = taps * slabs
+    int tap_img;                  // 1: tap t is image img * taps + t of the activation map (fold over stacked images), no spatial shift
     int n_tiles, BN, n_real, n_pad;
     int groups;
     int total_tiles;
@@ -402,7 +403,7 @@ conv_tc_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant
                     mbar_wait(empty_bar(stage), phase ^ 1);
                     const uint32_t a_dst = smem_base + stage * stage_bytes, b_dst = a_dst + kABytes;
                     mbar_expect_tx(full_bar(stage), stage_bytes);
-                    tma_load_4d(a_dst, &tmap_a, full_bar(stage), slab * kSlabK, tc.x0 + dx, tc.y0 + dy, tc.img);
+                    tma_load_4d(a_dst, &tmap_a, full_bar(stage), slab * kSlabK, tc.x0 + dx, tc.y0 + dy, p.tap_img ? tc.img * p.taps + tap : tc.img);
                     tma_load_3d(b_dst, &tmap_b, full_bar(stage), slab * kSlabK, tc.nt * p.BN, grp * p.taps + tap);
                     if (++stage == kStages) { stage = 0; phase ^= 1; }
                 }
@@ -941,6 +942,8 @@ cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUten
     p.tiles_y = (p.Hm + tile_h - 1) / tile_h;
     p.tiles_x = (p.Wm + tile_w - 1) / tile_w;
     p.taps = L.taps; p.slabs = L.c_in / kSlabK;
+    p.tap_img = P.taps_are_images ? 1 : 0;
+    if (p.tap_img && flat) return cudaErrorInvalidValue;
     p.BN = L.block_n; p.n_tiles = L.n_pad / L.block_n; p.n_real = L.n; p.n_pad = L.n_pad;
     p.groups = L.groups;
     p.total_tiles = p.n_img_m * p.tiles_y * p.tiles_x * p.n_tiles;

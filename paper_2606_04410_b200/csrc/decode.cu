@@ -52,7 +52,8 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
         // trunk counters when this call does not reach the trunk
         const bool keep = entropy_params_only || h->keep_status;
         const bool trunk = !entropy_params_only && frames && c.n_trunk_blocks > 0 && h->tail_fill;
-        const size_t words = trunk ? 4 + size_t(c.n_trunk_blocks) * h->trunk_sync_stride : 4;
+        const bool trunk_or_ctx = !entropy_params_only && frames && (c.n_trunk_blocks > 0 || h->has_ctx) && h->tail_fill;
+        const size_t words = (trunk || trunk_or_ctx) ? 4 + size_t(c.n_trunk_blocks + c.n_ctx_blocks) * h->trunk_sync_stride : 4;
         CU_TRY(cudaMemsetAsync(h->zero_block + (keep ? 1 : 0), 0, (words - (keep ? 1 : 0)) * 4, st));
     }
     // ---- A1 + A2: hyper-decoder in fp64 -> mu, ln sigma, bucket index ----
@@ -65,7 +66,7 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
         if (h->hybrid_head && h->am_xs.ok && h->head_tc.use_tc) {
             // layer 1 also emits the bf16 hi|mid split; the head runs on tensor cores; elements whose ln sigma lands within
             // flag_u of a bucket edge are re-decided in fp64 (identical decisions to the all-fp64 path, R12)
-            CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, h->hpart, n, h->h_z, h->w_z, st, h->xs, h->xnorm2));
+            CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, h->hpart, n, h->h_z, h->w_z, st, h->xs, h->xnorm2, h->has_ctx ? h->ctx_q : nullptr));
             const double step = (hp.ln_hi - hp.ln_lo) / double(c.n_buckets - 1 > 0 ? c.n_buckets - 1 : 1);
             EpiParams E{};
             E.mode = EPI_HEAD; E.act = ACT_NONE;
@@ -80,7 +81,7 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
                                     h->num_sms, st));
             *launches += 2;                    // head conv + fp64 fix
         } else {
-            CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, h->hpart, n, h->h_z, h->w_z, st));
+            CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, h->hpart, n, h->h_z, h->w_z, st, nullptr, nullptr, h->has_ctx ? h->ctx_q : nullptr));
             CU_TRY(launch_hyper_head(h->hyper[2], h->hx2, n, h->h_z, h->w_z, hp, st));
         }
         auto hyper_kernels = [](const HyperLayer &L) { return (L.c_in % 16 == 0 && L.n % 4 == 0) ? 2 : 1; };   // split-tap + reduce
@@ -109,6 +110,7 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     rp.cf = h->d_cf; rp.lut = h->d_lut;
     rp.n_chunks = n; rp.n_sub = h->n_sub; rp.h = h->h; rp.w = h->w; rp.c_y = c.c_y;
     rp.rows_per_sub = c.rows_per_substream; rp.W = c.lanes_per_substream; rp.n_buckets = c.n_buckets;
+    rp.y_stride = h->c_cat;
     const bool progressive = c.mu_steps == 4;
     rp.yhat = h->yhat; rp.sym_tap = progressive ? h->sym : (taps ? taps->sym : nullptr); rp.yhat_tap = taps ? taps->yhat : nullptr;
     rp.status = h->d_status;
@@ -129,7 +131,7 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
             EpiParams E{};
             E.mode = EPI_MU; E.act = ACT_NONE;
             E.out = k < 3 ? static_cast<void *>(h->ymu[k & 1]) : static_cast<void *>(h->yhat);
-            E.out_stride = k < 3 ? cs : c.c_y;
+            E.out_stride = k < 3 ? cs : h->c_cat;
             E.y_in = h->ymu[src]; E.in_stride = cs;
             E.sym = h->sym; E.c_y = c.c_y; E.mu_step = k; E.mu_last = k == 3;
             E.mu_tap = taps ? taps->mu : nullptr; E.yhat_tap = taps ? taps->yhat : nullptr;
@@ -211,6 +213,36 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
         }
     }
     mark(sg, st);
+
+    // ---- NEXT-2a (R23): context generation, C_{i+1} = bf16(conv_out(DCblock^{B_c}(conv_fold([F_i[0]; ..; F_i[T-1]])))), then its
+    // prior branch q.  F_i is the trunk's output, still in fa.  The new state overwrites the context block of the [y ; C]
+    // buffer, which nothing of this call reads any more (A5 consumed it; every kernel of the chain waits for its predecessor).
+    if (h->has_ctx) {
+        {
+            ConvProblem pr{h->fa, n, h->h, h->w, 1, true};
+            EpiParams E{EPI_NHWC, ACT_NONE, h->ca, nullptr, Ct, 0, (long long)P * Ct, 0, 0, 0};
+            CU_TRY(conv(h, h->ctx_fold, pr, h->am_fa, E, st, launches));
+        }
+        for (int k = 0; k < c.n_ctx_blocks; ++k) {
+            const ufnvc_handle::TrunkBlock &tb = h->ctx_blocks[k];
+            uint32_t *sync_k = h->trunk_sync + size_t(c.n_trunk_blocks + k) * h->trunk_sync_stride;
+            const bool mlp_counts = trunk_counts_tiles((long long)n * P, h->use_pair_trunk) && h->tail_fill;
+            CU_TRY(launch_dwconv3x3_tma(h->tm_dw_ctx, h->cb, tb.dw_w, tb.dw_b, n, h->h, h->w, Ct, h->num_sms, st, h->tail_fill ? sync_k : nullptr,
+                                        (k > 0 && mlp_counts) ? sync_k - h->trunk_sync_stride + 1 : nullptr));
+            CU_TRY(launch_trunk_mlp(tb.fused, tb.pw1, tb.pw2, h->ca, h->ca, (long long)n * P, h->num_sms, h->use_pair_trunk, st,
+                                    mlp_counts ? sync_k + 1 : nullptr));
+            *launches += 2;
+        }
+        {
+            ConvProblem pr{h->ca, n, h->h, h->w, 1};
+            EpiParams E{EPI_NHWC, ACT_NONE, h->yhat + c.c_y, nullptr, Ct, 0, (long long)P * h->c_cat, 0, 0, 0};
+            E.pix_stride = h->c_cat;
+            CU_TRY(conv(h, h->ctx_out, pr, h->am_ca, E, st, launches));
+        }
+        CU_TRY(launch_ctx_prior(h->yhat + c.c_y, h->c_cat, Ct, h->ctx_prior_w, h->ctx_prior_b, h->ctx_q, n, h->h, h->w, h->h_z, h->w_z, c.c_hyper, st));
+        ++*launches;
+    }
+    mark(sg, st);
     return UFNVC_OK;
 }
 
@@ -277,11 +309,15 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
     }
     for (auto &tb : h->trunk) ok = ok && tc_make_weight_tmap(tb.pw1, err) && tc_make_weight_tmap(tb.pw2, err);
     for (int s = 0; s < 4; ++s) ok = ok && tc_make_weight_tmap(h->dec[s], err);
+    if (h->has_ctx) {
+        ok = ok && tc_make_weight_tmap(h->ctx_fold, err) && tc_make_weight_tmap(h->ctx_out, err);
+        for (auto &tb : h->ctx_blocks) ok = ok && tc_make_weight_tmap(tb.pw1, err) && tc_make_weight_tmap(tb.pw2, err);
+    }
     for (int k = 0; k < 3 && c.mu_steps == 4; ++k) ok = ok && tc_make_weight_tmap(h->mu_net[k], err);
     if (!ok) return fail(h, UFNVC_E_CUDA, err);
     const int n = h->max_chunks, T = c.T;
     if (h->hybrid_head) ok = make_act_map(h, h->am_xs, h->xs, n, h->h_z, h->w_z, 2 * c.c_hyper, false, 1);
-    ok = ok && make_act_map(h, h->am_yhat, h->yhat, n, h->h, h->w, c.c_y, true, 1) &&
+    ok = ok && make_act_map(h, h->am_yhat, h->yhat, n, h->h, h->w, h->c_cat, true, 1) &&
          make_act_map(h, h->am_fb, h->fb, n * T, h->h, h->w, c.c_trunk, true, T) &&
          make_act_map(h, h->am_hidden, h->hidden, n * T, h->h, h->w, c.c_trunk * c.trunk_expand, true, T) &&
          make_act_map(h, h->am_fa, h->fa, n * T, h->h, h->w, c.c_trunk, false, T);
@@ -298,6 +334,13 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
     }
     for (auto &tb : h->trunk)
         if (ok && !trunk_make_maps(tb.fused, h->fb, (long long)n * T * h->h * h->w, tb.pw1, tb.pw2, h->err)) ok = false;
+    if (ok && h->has_ctx) {
+        ok = make_act_map(h, h->am_ca, h->ca, n, h->h, h->w, c.c_trunk, false, 1) &&
+             tc_make_act_tmap(&h->tm_dw_ctx, h->ca, n, h->h, h->w, c.c_trunk, 10, 10, h->err, /*swizzle=*/false);
+        for (auto &tb : h->ctx_blocks)
+            if (ok && (!trunk_make_maps(tb.fused, h->cb, (long long)n * h->h * h->w, tb.pw1, tb.pw2, h->err) || !tb.fused.ok)) ok = false;
+        if (ok && (!h->am_fa.ok || !h->ctx_fold.use_tc || !h->ctx_out.use_tc || !h->am_ca.ok)) { ok = false; h->err = "context generation needs the tensor-core conv path"; }
+    }
     for (int s = 0; ok && s < 3; ++s)
         ok = make_act_map(h, h->am_stage[s], h->stage[s], n * T, h->h << (s + 1), h->w << (s + 1), c.dec_channels[s + 1], false, T);
     h->final_is.ok = false;
@@ -341,6 +384,7 @@ int decode_z_impl(ufnvc_handle *h, int n, const uint8_t *bits, size_t bits_bytes
     rp.idx = h->z_idx; rp.mu = h->z_zero_mu; rp.cf = h->d_cf; rp.lut = h->d_lut;
     rp.n_chunks = n; rp.n_sub = h->n_sub_z; rp.h = h->h_z; rp.w = h->w_z; rp.c_y = c.c_z;
     rp.rows_per_sub = c.rows_per_substream; rp.W = c.lanes_per_substream; rp.n_buckets = c.n_buckets;
+    rp.y_stride = c.c_z;
     rp.yhat = h->z_scratch; rp.sym_tap = h->z_hwc; rp.yhat_tap = nullptr; rp.status = h->d_status;
     CU_TRY(launch_rans_decode(rp, st));
     CU_TRY(launch_z_hwc_to_planar(h->z_hwc, z_planar_out, n, c.c_z, h->h_z * h->w_z, st));
@@ -464,7 +508,12 @@ extern "C" int ufnvc_chunk_decode_profiled(ufnvc_handle *h, int n_chunks, const 
                      nullptr, nullptr, &sg, nullptr))
         return rc;
     CU_TRY(cudaStreamSynchronize(st));
-    // events: 0 start, 1 after A1+A2, 2 after A3+A4, 3 after A5, 4 after trunk, 5 after A8, 6 after A9
+    // events: 0 start, 1 after A1+A2, 2 after A3+A4, 3 after A5, 4 after trunk, 5 after A8, 6 after A9, 7 after the context generation
+    {
+        float ms = 0.f;
+        CU_TRY(cudaEventElapsedTime(&ms, h->ev[6], h->ev[7]));
+        us_out_host[7] = ms * 1000.f;
+    }
     for (int i = 0; i < 6; ++i) {
         float ms = 0.f;
         CU_TRY(cudaEventElapsedTime(&ms, h->ev[i], h->ev[i + 1]));
@@ -479,4 +528,57 @@ extern "C" int ufnvc_chunk_decode_profiled(ufnvc_handle *h, int n_chunks, const 
     }
     us_out_host[6] = dw_us;
     return UFNVC_OK;
+}
+
+// ---- NEXT-2a (R23): the temporal context state ------------------------------------------------------------------------
+namespace {
+int ctx_call_ok(ufnvc_handle *h, int n_chunks)
+{
+    if (!h) return UFNVC_E_INVALID_ARG;
+    if (!h->has_ctx) return fail(h, UFNVC_E_BAD_CONFIG, "this handle has no temporal context (n_ctx_blocks == 0)");
+    if (!h->weights_loaded) return fail(h, UFNVC_E_NO_WEIGHTS, "ufnvc_load_weights has not succeeded on this handle");
+    if (n_chunks < 1 || n_chunks > h->max_chunks) return fail(h, UFNVC_E_INVALID_ARG, "n_chunks outside [1, max_chunks_per_call]");
+    return UFNVC_OK;
+}
+int ctx_refresh_prior(ufnvc_handle *h, int n, cudaStream_t stream)
+{
+    const ufnvc_config &c = h->cfg;
+    const LaunchStream st{stream, false};          // follows a copy / memset node: plain stream order
+    CU_TRY(launch_ctx_prior(h->yhat + c.c_y, h->c_cat, c.c_trunk, h->ctx_prior_w, h->ctx_prior_b, h->ctx_q, n, h->h, h->w, h->h_z, h->w_z,
+                            c.c_hyper, st));
+    return UFNVC_OK;
+}
+}  // namespace
+
+extern "C" int ufnvc_reset_context(ufnvc_handle *h, int n_chunks, void *cuda_stream)
+{
+    if (int rc = ctx_call_ok(h, n_chunks)) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const ufnvc_config &c = h->cfg;
+    const size_t rows = size_t(n_chunks) * h->h * h->w;
+    CU_TRY(cudaMemset2DAsync(h->yhat + c.c_y, size_t(h->c_cat) * 2, 0, size_t(c.c_trunk) * 2, rows, st));
+    return ctx_refresh_prior(h, n_chunks, st);      // q of the zero context is ReLU(b_p), not zero
+}
+
+extern "C" int ufnvc_get_context(ufnvc_handle *h, int n_chunks, uint16_t *ctx_dev, void *cuda_stream)
+{
+    if (int rc = ctx_call_ok(h, n_chunks)) return rc;
+    if (!ctx_dev) return fail(h, UFNVC_E_INVALID_ARG, "null ctx_dev");
+    const ufnvc_config &c = h->cfg;
+    const size_t rows = size_t(n_chunks) * h->h * h->w;
+    CU_TRY(cudaMemcpy2DAsync(ctx_dev, size_t(c.c_trunk) * 2, h->yhat + c.c_y, size_t(h->c_cat) * 2, size_t(c.c_trunk) * 2, rows,
+                             cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(cuda_stream)));
+    return UFNVC_OK;
+}
+
+extern "C" int ufnvc_set_context(ufnvc_handle *h, int n_chunks, const uint16_t *ctx_dev, void *cuda_stream)
+{
+    if (int rc = ctx_call_ok(h, n_chunks)) return rc;
+    if (!ctx_dev) return fail(h, UFNVC_E_INVALID_ARG, "null ctx_dev");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const ufnvc_config &c = h->cfg;
+    const size_t rows = size_t(n_chunks) * h->h * h->w;
+    CU_TRY(cudaMemcpy2DAsync(h->yhat + c.c_y, size_t(h->c_cat) * 2, ctx_dev, size_t(c.c_trunk) * 2, size_t(c.c_trunk) * 2, rows,
+                             cudaMemcpyDeviceToDevice, st));
+    return ctx_refresh_prior(h, n_chunks, st);
 }

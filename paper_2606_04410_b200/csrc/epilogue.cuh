@@ -100,7 +100,7 @@ __device__ __forceinline__ long long epi_offset(const EpiParams &E, int img, int
 {
     if (E.mode == EPI_NHWC) {
         const int grp = n / E.n_split, c = n - grp * E.n_split;
-        return (long long)img * E.img_stride + (long long)grp * E.split_stride + ((long long)y * W + x) * E.n_split + c;
+        return (long long)img * E.img_stride + (long long)grp * E.split_stride + ((long long)y * W + x) * (E.pix_stride ? E.pix_stride : E.n_split) + c;
     }
     const int ij = n / E.c_o, c = n - ij * E.c_o;
     const int oy = 2 * y + (ij >> 1), ox = 2 * x + (ij & 1);

@@ -27,7 +27,7 @@ struct ufnvc_handle {
     // entropy tables (O3)
     std::vector<uint32_t> cdf32;         // [nb][256], host copy
     uint32_t *d_cf = nullptr;             // [nb][256]: c[pos] | freq[pos] << 16
-    uint16_t *d_lut = nullptr;
+    uint32_t *d_lut = nullptr;
     uint32_t *d_status = nullptr;
 
     // layers
@@ -52,6 +52,18 @@ struct ufnvc_handle {
     };
     std::vector<TrunkBlock> trunk;
     ufnvc::ConvLayer dec[4];             // groups = T
+    // temporal chunk context (NEXT-2a, R23).  The state C_i lives in the context block of the [y ; C] buffer
+    // (`yhat`, c_cat = c_y + c_trunk channels per pixel) that the cross-frame unfold reads; ctx_q is its prior branch
+    // q = ReLU(W_p pool4(C_i) + b_p) in fp64, recomputed whenever the state changes.
+    bool has_ctx = false;
+    int c_cat = 0;                       // channels per pixel of `yhat`: c_y, or c_y + c_trunk with a context
+    ufnvc::ConvLayer ctx_fold, ctx_out;  // 1x1: T c_trunk -> c_trunk (taps = T images), c_trunk -> c_trunk
+    std::vector<TrunkBlock> ctx_blocks;
+    double *ctx_prior_w = nullptr, *ctx_prior_b = nullptr;   // [c_trunk][c_hyper] (k-major), [c_hyper]
+    double *ctx_q = nullptr;             // [n][h_z][w_z][c_hyper]
+    ufnvc::bf16 *ca = nullptr, *cb = nullptr;   // [n][h][w][c_trunk] ping-pong of the context generation
+    CUtensorMap tm_dw_ctx;               // ca as the depthwise kernel reads it
+    bool dw_ctx_ok = false;
 
     // workspace (sized for max_chunks)
     double *hx0 = nullptr, *hx1 = nullptr, *hx2 = nullptr, *hpart = nullptr;
@@ -91,7 +103,7 @@ struct ufnvc_handle {
     size_t zero_words = 0;
     size_t trunk_sync_stride = 0;
     bool tail_fill = true;
-    ActMap am_xs, am_yhat, am_fa, am_fb, am_hidden, am_stage[3], am_ymu[2];
+    ActMap am_xs, am_yhat, am_fa, am_fb, am_hidden, am_stage[3], am_ymu[2], am_ca;
 
     // GPU rANS encoder scratch (NEXT-4), allocated by the first ufnvc_encode_chunk_dev call
     uint16_t *enc_tmp = nullptr;
@@ -101,7 +113,7 @@ struct ufnvc_handle {
 
     std::vector<void *> allocs;          // workspace and tables, freed at destroy
     std::vector<void *> weight_allocs;   // what ufnvc_load_weights uploaded; freed by the next load and at destroy
-    cudaEvent_t ev[8] = {};
+    cudaEvent_t ev[9] = {};
     std::vector<cudaEvent_t> ev_dw;      // profiled call: before / after every depthwise launch
     bool ev_made = false;
 };

@@ -223,7 +223,7 @@ __global__ void __launch_bounds__(256) hyper_conv_fast_kernel(const double *__re
 }
 
 __global__ void hyper_reduce_kernel(const double *__restrict__ part, const double *__restrict__ bias, double *__restrict__ out,
-                                    long long MN, int n_out)
+                                    long long MN, int n_out, const double *__restrict__ addend)
 {
     asm volatile("griddepcontrol.wait;" ::: "memory");              // PDL: launched early, the predecessor's output is complete from here on
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -232,7 +232,9 @@ __global__ void hyper_reduce_kernel(const double *__restrict__ part, const doubl
 #pragma unroll
         for (int t = 1; t < 9; ++t) v += part[t * MN + i];                   // fixed tap order: run-to-run deterministic
         v += bias[i % n_out];
-        out[i] = v > 0.0 ? v : 0.0;
+        v = v > 0.0 ? v : 0.0;
+        if (addend) v += addend[i];                                          // s = x2 + q (R23)
+        out[i] = v;
     }
 }
 
@@ -248,7 +250,8 @@ cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z
 // and xnorm2[m] = sum_o v^2 (fp32), the input of the head's a-priori error bound (decode.cu, R12).  One warp per
 // z-pixel m, lanes stride the channels, fixed-order tree reduction: run-to-run deterministic.
 __global__ void hyper_reduce_split_kernel(const double *__restrict__ part, const double *__restrict__ bias, double *__restrict__ out,
-                                          bf16 *__restrict__ xs, float *__restrict__ xnorm2, long long M, int n_out)
+                                          bf16 *__restrict__ xs, float *__restrict__ xnorm2, long long M, int n_out,
+                                          const double *__restrict__ addend)
 {
     asm volatile("griddepcontrol.wait;" ::: "memory");              // PDL: launched early, the predecessor's output is complete from here on
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -264,6 +267,7 @@ __global__ void hyper_reduce_split_kernel(const double *__restrict__ part, const
             for (int t = 1; t < 9; ++t) v += part[t * MN + i];               // fixed tap order
             v += bias[o];
             v = v > 0.0 ? v : 0.0;
+            if (addend) v += addend[i];                                      // s = x2 + q (R23)
             out[i] = v;
             const bf16 hi = __double2bfloat16(v);
             const bf16 mid = __double2bfloat16(v - double(__bfloat162float(hi)));
@@ -331,7 +335,7 @@ __global__ void __launch_bounds__(256) hyper_fix_kernel(const uint32_t *__restri
 static bool fast_ok(const HyperLayer &L) { return L.c_in % FK == 0 && L.n % 4 == 0; }
 
 cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out, double *part, int n_img, int hz, int wz,
-                              LaunchStream st, bf16 *xs, float *xnorm2)
+                              LaunchStream st, bf16 *xs, float *xnorm2, const double *addend)
 {
     HyperEpi e{};
     e.mode = 0;
@@ -344,14 +348,60 @@ cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out
         const int blocks = int((MN + 255) / 256 < 1184 ? (MN + 255) / 256 : 1184);
         if (xs) {
             const int wblocks = int(((long long)M * 32 + 255) / 256 < 1184 ? ((long long)M * 32 + 255) / 256 : 1184);
-            if (cudaError_t le = launch_pdl(hyper_reduce_split_kernel, unsigned(wblocks), 256u, 0, st, 1, part, L.bias, out, xs, xnorm2, (long long)M, L.n)) return le;
+            if (cudaError_t le = launch_pdl(hyper_reduce_split_kernel, unsigned(wblocks), 256u, 0, st, 1, part, L.bias, out, xs, xnorm2, (long long)M, L.n, addend)) return le;
         }
-        else if (cudaError_t le = launch_pdl(hyper_reduce_kernel, unsigned(blocks), 256u, 0, st, 1, part, L.bias, out, MN, L.n)) return le;
+        else if (cudaError_t le = launch_pdl(hyper_reduce_kernel, unsigned(blocks), 256u, 0, st, 1, part, L.bias, out, MN, L.n, addend)) return le;
         return cudaGetLastError();
     }
+    if (addend || xs) return cudaErrorInvalidValue;       // the slow-shape kernel has no context branch (api.cu validates the shapes)
     dim3 grid((M + HM - 1) / HM, (L.n + HN - 1) / HN);
     hyper_conv_kernel<<<grid, 256, 0, st>>>(in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e);
     return cudaGetLastError();
+}
+
+// ---- R23: q = ReLU(W_p pool4(C) + b_p), the context branch of the prior input, in fp64.  The context is a bf16 tensor (its
+// values are exact in fp64 and so are the 16-term sums), so both sides of the parity test evaluate the same real numbers up
+// to the order of a 256-term fp64 sum.  One block per z-pixel: pool into shared memory, then thread o = output channel.
+__global__ void __launch_bounds__(128) ctx_prior_kernel(const bf16 *__restrict__ ctx, int stride, int c_ctx, const double *__restrict__ w_p,
+                                                        const double *__restrict__ b_p, double *__restrict__ q, int h, int w, int hz, int wz,
+                                                        int c_h)
+{
+    extern __shared__ double pool[];                                 // [c_ctx]
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    const int m = blockIdx.x, pz = hz * wz;
+    const int img = m / pz, r = m % pz, zy = r / wz, zx = r % wz;
+    for (int k = threadIdx.x; k < c_ctx; k += blockDim.x) {
+        double s = 0.0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int y = 4 * zy + i, x = 4 * zx + j;
+                if (y < h && x < w) s += double(__bfloat162float(ctx[(((long long)img * h + y) * w + x) * stride + k]));
+            }
+        pool[k] = s / 16.0;
+    }
+    __syncthreads();
+    for (int o = threadIdx.x; o < c_h; o += blockDim.x) {
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;               // fixed summation order: deterministic
+        int k = 0;
+        for (; k + 3 < c_ctx; k += 4) {
+            a0 = fma(w_p[(long long)k * c_h + o], pool[k], a0);
+            a1 = fma(w_p[(long long)(k + 1) * c_h + o], pool[k + 1], a1);
+            a2 = fma(w_p[(long long)(k + 2) * c_h + o], pool[k + 2], a2);
+            a3 = fma(w_p[(long long)(k + 3) * c_h + o], pool[k + 3], a3);
+        }
+        for (; k < c_ctx; ++k) a0 = fma(w_p[(long long)k * c_h + o], pool[k], a0);
+        const double v = (a0 + a1) + (a2 + a3) + b_p[o];
+        q[(long long)m * c_h + o] = v > 0.0 ? v : 0.0;
+    }
+}
+
+cudaError_t launch_ctx_prior(const bf16 *ctx, int stride, int c_ctx, const double *w_p, const double *b_p, double *q, int n_img, int h, int w,
+                             int hz, int wz, int c_h, LaunchStream st)
+{
+    return launch_pdl(ctx_prior_kernel, unsigned(n_img * hz * wz), 128u, size_t(c_ctx) * 8, st, 1, ctx, stride, c_ctx, w_p, b_p, q, h, w, hz, wz, c_h);
 }
 
 cudaError_t launch_hyper_fix(const uint32_t *list, const uint32_t *count, const double *x2, const double *fix_w, const double *fix_b,

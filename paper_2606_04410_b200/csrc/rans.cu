@@ -12,18 +12,29 @@
 
 namespace ufnvc {
 
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+
+// TAPS: the optional fp32 / int16 outputs exist (parity taps, or the residual the progressive means need).
+// STRIDED: y is a channel block of a wider tensor (y_stride != c_y, R23).
+template <bool TAPS, bool STRIDED>
 __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    // s_cf[k][pos] = c[pos] | freq[pos] << 16 (one 32-bit read gives both; freq <= 65282 fits 16 bits), then the search LUT
-    uint32_t *s_cf = reinterpret_cast<uint32_t *>(smem_raw);
-    uint16_t *s_lut = reinterpret_cast<uint16_t *>(s_cf + nb * 256);
+    // tables in shared memory, addressed as 32-bit shared addresses (one LDS per access, no generic-address arithmetic in
+    // the serial chain): cf[k][pos] = c[pos] | freq[pos] << 16 (freq <= 65282 fits 16 bits), then the search entries
+    const uint32_t s_cf = uint32_t(__cvta_generic_to_shared(smem_raw));
+    const uint32_t s_lut = s_cf + uint32_t(nb) * 1024u;
     {
         const uint4 *src_c = reinterpret_cast<const uint4 *>(p.cf);
         const uint4 *src_l = reinterpret_cast<const uint4 *>(p.lut);
-        uint4 *dc = reinterpret_cast<uint4 *>(s_cf), *dl = reinterpret_cast<uint4 *>(s_lut);
+        uint4 *dc = reinterpret_cast<uint4 *>(smem_raw), *dl = reinterpret_cast<uint4 *>(smem_raw + size_t(nb) * 1024);
         for (int i = threadIdx.x; i < nb * 64; i += blockDim.x) dc[i] = src_c[i];
-        for (int i = threadIdx.x; i < nb * (kLutBuckets / 8); i += blockDim.x) dl[i] = src_l[i];
+        for (int i = threadIdx.x; i < nb * (kLutBuckets / 4); i += blockDim.x) dl[i] = src_l[i];
     }
     // PDL: the 192 KB of static tables above load while the predecessor (the hyper head's fix-up kernel) is still running;
     // idx, mu and the status word are only touched after the predecessor grid has completed.
@@ -68,43 +79,51 @@ __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
     uint32_t w0 = (lane < nw) ? words[lane] : 0u;
     uint32_t w1 = (32u + lane < nw) ? words[32 + lane] : 0u;
     uint32_t w2 = (64u + lane < nw) ? words[64 + lane] : 0u;
+    const uint32_t below = (1u << lane) - 1u;
 
     // idx / mu do not depend on the decoder state: they are fetched kPre steps ahead into two register banks, so the
-    // serial chain of a step holds no global-memory latency (with a 1-deep prefetch every step waited ~800 cycles).
+    // serial chain of a step holds no global-memory latency.  What is kept of the index is the byte offset of its cf table.
     constexpr int kPre = 8;
     const int i0 = g * 32 + lane;
     uint32_t kA[kPre], kB[kPre];
     float mA[kPre], mB[kPre];
     auto fetch = [&](uint32_t (&kk)[kPre], float (&mm)[kPre], int j0) {
 #pragma unroll
-        for (int s = 0; s < kPre; ++s) {
-            const int ii = i0 + (j0 + s) * p.W;
-            kk[s] = 0; mm[s] = 0.f;
-            if (j0 + s < n_steps && ii < n) {
-                kk[s] = p.idx[ebase + ii]; mm[s] = p.mu[ebase + ii];
+        for (int t = 0; t < kPre; ++t) {
+            const int ii = i0 + (j0 + t) * p.W;
+            kk[t] = 0; mm[t] = 0.f;
+            if (ii < n) {                                  // (false for every step past the last one, too)
+                uint32_t k = p.idx[ebase + ii];
+                mm[t] = p.mu[ebase + ii];
                 // an index past the tables (possible only through idx_override_dev) must not read shared memory out of
                 // bounds: clamp and report, like every other malformed input (off the serial chain: this is the prefetch)
-                if (kk[s] >= uint32_t(nb)) { kk[s] = uint32_t(nb - 1); st |= UFNVC_STREAM_BAD_HEADER; }
+                if (k >= uint32_t(nb)) { k = uint32_t(nb - 1); st |= UFNVC_STREAM_BAD_HEADER; }
+                kk[t] = k << 10;
             }
         }
     };
-    auto step = [&](uint32_t k, float mu, int j) {
+    // one symbol per lane.  The serial chain: LDS (search entry) -> ~8 integer ops -> LDS (c | freq) -> multiply-add ->
+    // compare -> ballot -> popc -> shuffle -> merge.  Everything else (dequantisation, stores) hangs off it.
+    auto step = [&](const uint32_t kofs, const float mu, const int j, const bool check) {
         const int i = i0 + j * p.W;
-        const bool valid = j < n_steps && i < n;
+        const bool valid = !check || i < n;
         const uint32_t slot = x & 0xFFFFu;
-        const uint32_t *c = s_cf + k * 256;
-        const uint32_t lh = s_lut[k * kLutBuckets + (slot >> kLutShift)];
-        uint32_t lo = lh & 0xFFu, hi = lh >> 8;
-        while (lo < hi) {                       // largest pos in [lo,hi] with c[pos] <= slot
-            const uint32_t mid = (lo + hi + 1) >> 1;
-            if ((c[mid] & 0xFFFFu) <= slot) lo = mid; else hi = mid - 1;
+        const uint32_t ent = lds_u32(s_lut + (kofs << 1) + ((slot >> kLutShift) << 2));
+        const uint32_t off = slot & ((1u << kLutShift) - 1u);
+        uint32_t pos = (ent & 0xFFu) + uint32_t(off >= ((ent >> 8) & 0xFFu)) + uint32_t(off >= ((ent >> 16) & 0xFFu)) + uint32_t(off >= (ent >> 24));
+        if ((ent & 0xFF00u) == 0xFF00u) {       // > 3 symbols start inside this 128-slot bin (the packed tails): bisect
+            uint32_t lo = ent & 0xFFu, hi = lo + ((ent >> 16) & 0xFFu);
+            while (lo < hi) {                   // largest pos in [lo,hi] with c[pos] <= slot
+                const uint32_t mid = (lo + hi + 1) >> 1;
+                if ((lds_u32(s_cf + kofs + (mid << 2)) & 0xFFFFu) <= slot) lo = mid; else hi = mid - 1;
+            }
+            pos = lo;
         }
-        const uint32_t cf = c[lo];
-        const uint32_t cp = cf & 0xFFFFu, f = cf >> 16;
-        uint32_t xn = f * (x >> 16) + slot - cp;
+        const uint32_t cf = lds_u32(s_cf + kofs + (pos << 2));
+        uint32_t xn = (cf >> 16) * (x >> 16) + slot - (cf & 0xFFFFu);
         const bool need = valid && xn < (1u << 16);
         const uint32_t m = __ballot_sync(0xFFFFFFFFu, need);
-        const uint32_t r = q - qb + __popc(m & ((1u << lane) - 1u));     // index into the window, < 64
+        const uint32_t r = q - qb + __popc(m & below);                   // index into the window, < 64
         const uint32_t wa = __shfl_sync(0xFFFFFFFFu, w0, r & 31);
         const uint32_t wb = __shfl_sync(0xFFFFFFFFu, w1, r & 31);
         if (need) xn = (xn << 16) | (r < 32 ? wa : wb);
@@ -117,26 +136,46 @@ __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
             w2 = (a < nw) ? words[a] : 0u;
         }
         if (valid) {
-            const int sym = int(lo) - 127;
+            const int sym = int(pos) - 127;
             const float y = float(sym) + mu;                             // O5
-            p.yhat[ebase + i] = __float2bfloat16_rn(y);
-            if (p.sym_tap) p.sym_tap[ebase + i] = int16_t(sym);
-            if (p.yhat_tap) p.yhat_tap[ebase + i] = y;
+            const long long e = ebase + i;
+            if (!STRIDED) {
+                p.yhat[e] = __float2bfloat16_rn(y);
+            } else {                                                     // y is the first channel block of a wider tensor (R23)
+                const long long pix = e / p.c_y;
+                p.yhat[pix * p.y_stride + (e - pix * p.c_y)] = __float2bfloat16_rn(y);
+            }
+            if (TAPS) {
+                if (p.sym_tap) p.sym_tap[e] = int16_t(sym);
+                if (p.yhat_tap) p.yhat_tap[e] = y;
+            }
         }
     };
 
+    const int n_full = n / p.W;                 // steps in which every lane has a symbol
     fetch(kA, mA, 0);
     for (int j0 = 0; j0 < n_steps; j0 += 2 * kPre) {
         fetch(kB, mB, j0 + kPre);
+        if (j0 + kPre <= n_full) {
 #pragma unroll
-        for (int s = 0; s < kPre; ++s) step(kA[s], mA[s], j0 + s);
+            for (int t = 0; t < kPre; ++t) step(kA[t], mA[t], j0 + t, false);
+        } else {
+#pragma unroll
+            for (int t = 0; t < kPre; ++t) if (j0 + t < n_steps) step(kA[t], mA[t], j0 + t, true);
+        }
         fetch(kA, mA, j0 + 2 * kPre);
+        if (j0 + 2 * kPre <= n_full) {
 #pragma unroll
-        for (int s = 0; s < kPre; ++s) step(kB[s], mB[s], j0 + kPre + s);
+            for (int t = 0; t < kPre; ++t) step(kB[t], mB[t], j0 + kPre + t, false);
+        } else {
+#pragma unroll
+            for (int t = 0; t < kPre; ++t) if (j0 + kPre + t < n_steps) step(kB[t], mB[t], j0 + kPre + t, true);
+        }
     }
     // end-state invariant (O4): every lane back at 2^16 and every word consumed
     if (__any_sync(0xFFFFFFFFu, x != (1u << 16))) st |= UFNVC_STREAM_BAD_END_STATE;
     if (q != nw) st |= UFNVC_STREAM_BAD_WORD_COUNT;
+    st = __reduce_or_sync(0xFFFFFFFFu, st);     // (a clamped index was seen by one lane only)
     if (st && lane == 0) atomicOr(p.status, st);
 }
 
@@ -160,18 +199,26 @@ cudaError_t launch_z_hwc_to_planar(const int16_t *z_hwc, int16_t *z_planar, int 
     return cudaGetLastError();
 }
 
-constexpr size_t kRansSmem = (size_t)64 * (256 * 4 + kLutBuckets * 2);
+constexpr size_t kRansSmem = (size_t)64 * (256 * 4 + kLutBuckets * 4);
 
 cudaError_t configure_rans_kernels()
 {
-    return cudaFuncSetAttribute(rans_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRansSmem);
+    cudaError_t e = cudaFuncSetAttribute(rans_decode_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRansSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(rans_decode_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRansSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(rans_decode_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRansSmem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(rans_decode_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRansSmem);
+    return e;
 }
 
 cudaError_t launch_rans_decode(const RansParams &p, LaunchStream st)
 {
     const int nb = p.n_buckets;
-    const size_t smem = kRansSmem;
-    return launch_pdl(rans_decode_kernel, unsigned(p.n_chunks * p.n_sub), unsigned(p.W), smem, st, 1, p, nb);
+    const bool taps = p.sym_tap || p.yhat_tap, strided = p.y_stride != p.c_y;
+    const unsigned grid = unsigned(p.n_chunks * p.n_sub), block = unsigned(p.W);
+    if (taps) return strided ? launch_pdl(rans_decode_kernel<true, true>, grid, block, kRansSmem, st, 1, p, nb)
+                             : launch_pdl(rans_decode_kernel<true, false>, grid, block, kRansSmem, st, 1, p, nb);
+    return strided ? launch_pdl(rans_decode_kernel<false, true>, grid, block, kRansSmem, st, 1, p, nb)
+                   : launch_pdl(rans_decode_kernel<false, false>, grid, block, kRansSmem, st, 1, p, nb);
 }
 
 }  // namespace ufnvc

@@ -1,6 +1,6 @@
 // Host-side entropy-model tables and the encoder-side fixture of libufnvc.
 //   * quantised discretised-Gaussian CDF tables, one per scale bucket (readings R7/R8)
-//   * the search accelerator the rANS decode kernel uses (slot>>8 -> candidate position range)
+//   * the search accelerator the rANS decode kernel uses (slot >> 7 -> position, see build_search_lut)
 //   * the rANS ENCODER (mirror of O4), used by callers that need a valid bit-stream (bench.py, tests)
 // r = round(y - mu) "is arithmetically encoded using scale sigma".
 #include <algorithm>
@@ -30,11 +30,16 @@ void build_cdf_tables(int nb, double smin, double smax, std::vector<uint32_t> &c
     }
 }
 
-// For every bucket and every 256-slot bin b: lo = position holding slot 256*b, hi = position holding slot
-// 256*b + 255.  The decode kernel then searches only [lo, hi] (usually one candidate).
-void build_search_lut(const std::vector<uint32_t> &cdf32, int nb, std::vector<uint16_t> &lut)
+// Search accelerator of the decode kernel.  For every table and every bin b of 2^kLutShift = 128 slots, one 32-bit entry:
+//   byte 0      lo = the position holding slot 128 b (largest p with c[p] <= 128 b)
+//   bytes 1..3  d_i = c[lo + i] - 128 b for the (at most three) further positions that START inside the bin, 0x80 when
+//               there is none: the position of slot 128 b + off is  lo + (off >= d_1) + (off >= d_2) + (off >= d_3)
+//               -- no second table access and no loop.
+//   more than three starts inside the bin (only where the tails' 1-slot symbols are packed: < 0.5 % of the mass):
+//               byte 1 = 0xFF, byte 2 = their count m; the kernel then bisects [lo, lo + m].
+void build_search_lut(const std::vector<uint32_t> &cdf32, int nb, std::vector<uint32_t> &lut)
 {
-    lut.assign((size_t)nb * kLutBuckets, 0);
+    lut.assign((size_t)nb * kLutBuckets, 0u);
     for (int k = 0; k < nb; ++k) {
         const uint32_t *c = &cdf32[(size_t)k * 256];
         int p = 0;
@@ -44,7 +49,14 @@ void build_search_lut(const std::vector<uint32_t> &cdf32, int nb, std::vector<ui
             const int lo = p;
             int q = p;
             while (q < 254 && c[q + 1] <= s1) ++q;
-            lut[(size_t)k * kLutBuckets + b] = uint16_t(lo | (q << 8));
+            const int m = q - lo;
+            uint32_t e = uint32_t(lo);
+            if (m <= 3) {
+                for (int i = 1; i <= 3; ++i) e |= (i <= m ? c[lo + i] - s0 : 0x80u) << (8 * i);
+            } else {
+                e |= 0xFFu << 8 | uint32_t(m) << 16 | 0x80u << 24;
+            }
+            lut[(size_t)k * kLutBuckets + b] = e;
         }
     }
 }

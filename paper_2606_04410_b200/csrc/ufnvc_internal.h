@@ -52,6 +52,8 @@ struct EpiParams {
     const bf16 *y_in;        // the conv's own input
     int in_stride, out_stride, mu_step, mu_last;
     float *mu_tap, *yhat_tap;   // optional fp32 [pix][c_y], written on partition mu_step only
+    int pix_stride;          // EPI_NHWC: elements between pixels of a group; 0 = n_split (dense).  > n_split: the conv writes a
+                             // channel block of a wider tensor (context generation -> [y ; C] buffer, R23)
 };
 
 // R21: partition of latent element (channel c, row y, column x): four channel groups x the four positions of a 2x2 cell
@@ -75,6 +77,7 @@ struct ConvProblem {
     const bf16 *in;          // [n_img][H][W][c_in] bf16 NHWC
     int n_img, H, W;
     int imgs_per_group_cycle; // weight group of image i = (groups == 1) ? 0 : i % groups
+    bool taps_are_images = false;   // 1x1 "fold" over T stacked images (R23): tap t reads image img * taps + t of `in` (n_img output images)
 };
 
 // ---- kernels (each .cu exposes host launchers; all enqueue on `st` and return cudaGetLastError()) -------------
@@ -146,8 +149,13 @@ struct HyperLayer {
     double *bias = nullptr;  // [n]
 };
 cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z, int pz, LaunchStream st);
+// addend (optional, [M][n]): added AFTER the ReLU -- the context branch q of the prior input s = x2 + q (R23)
 cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out, double *part, int n_img, int hz, int wz,
-                              LaunchStream st, bf16 *xs = nullptr, float *xnorm2 = nullptr);   // part: [9][M][n] scratch for the split-tap fast path (may be null)
+                              LaunchStream st, bf16 *xs = nullptr, float *xnorm2 = nullptr, const double *addend = nullptr);
+// q = ReLU(W_p pool4(C) + b_p) in fp64 from the bf16 context block of the [y ; C] buffer (R23): ctx [n][h][w][stride] (channel
+// block already offset), w_p [c_ctx][c_h] (k-major), q [n][h_z][w_z][c_h]
+cudaError_t launch_ctx_prior(const bf16 *ctx, int stride, int c_ctx, const double *w_p, const double *b_p, double *q, int n_img, int h, int w,
+                             int hz, int wz, int c_h, LaunchStream st);   // part: [9][M][n] scratch for the split-tap fast path (may be null)
 struct HeadParams {
     int c_y, h, w, n_buckets;
     double ln_lo, ln_hi;
@@ -169,9 +177,10 @@ struct RansParams {
     const uint8_t *idx;       // [n][h][w][c_y]
     const float *mu;
     const uint32_t *cf;       // [nb][256]: c[pos] | freq[pos] << 16
-    const uint16_t *lut;      // [nb][kLutBuckets]: lo | hi<<8 = first/last candidate position for slot >> kLutShift
+    const uint32_t *lut;      // [nb][kLutBuckets]: search accelerator entry of bin slot >> kLutShift (tables.cu)
     int n_chunks, n_sub, h, w, c_y, rows_per_sub, W, n_buckets;
-    bf16 *yhat;               // [n][h][w][c_y]
+    int y_stride;             // elements between pixels of yhat (c_y = dense; c_y + C_c when y shares a buffer with the context, R23)
+    bf16 *yhat;               // [n][h][w][y_stride], channels [0, c_y)
     int16_t *sym_tap;         // optional
     float *yhat_tap;          // optional
     uint32_t *status;         // device word, OR-ed
@@ -239,12 +248,12 @@ constexpr uint32_t kTrunkTileSignals = 8;
 // true if launch_trunk_mlp(..., pair, ...) runs the CTA-pair kernel, the one that counts finished tiles in tile_done
 bool trunk_counts_tiles(long long n_px, bool pair);
 
-// rANS symbol search: a 64-slot LUT bucket holds 1.2 binary-search steps (warp maximum, measured law) against 2.4 for 256 slots
-constexpr int kLutShift = 6, kLutBuckets = 65536 >> kLutShift;
+// rANS symbol search: 128-slot bins, one 32-bit entry each (tables.cu build_search_lut)
+constexpr int kLutShift = 7, kLutBuckets = 65536 >> kLutShift;
 
 // ---- host-side entropy tables + encoder fixture (tables.cpp part of api) ---------------------------------------
 void build_cdf_tables(int nb, double smin, double smax, std::vector<uint32_t> &cdf32);
-void build_search_lut(const std::vector<uint32_t> &cdf32, int nb, std::vector<uint16_t> &lut);
+void build_search_lut(const std::vector<uint32_t> &cdf32, int nb, std::vector<uint32_t> &lut);
 long encode_substream(const uint32_t *cdf32, const uint8_t *idx, const int16_t *sym, size_t n, int W, uint8_t *out,
                       size_t cap);
 

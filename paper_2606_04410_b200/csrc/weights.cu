@@ -165,6 +165,40 @@ struct Loader {
         return L.w && L.bias && fix_w && fix_b && wnorm;
     }
 
+    // R23 fold: canonical [n][T c_t][1][1] -> a conv with T "taps" of c_t channels each (tap t = frame t's feature map)
+    bool fold(ConvLayer &L, const std::string &name, int n, int T, int c_t)
+    {
+        const Tensor *tw = get(name + ".w", {uint32_t(n), uint32_t(T * c_t), 1u, 1u});
+        const Tensor *tb = get(name + ".b", {uint32_t(n)});
+        if (!tw || !tb) return false;
+        L.c_in = c_t; L.n = n; L.n_pad = (n + 15) / 16 * 16; L.taps = T; L.groups = 1;
+        std::vector<uint16_t> w(size_t(T) * L.n_pad * c_t, 0);
+        std::vector<float> b(L.n_pad, 0.f);
+        for (int o = 0; o < n; ++o) {
+            b[o] = tb->at(o);
+            for (int t = 0; t < T; ++t)
+                for (int c = 0; c < c_t; ++c) w[(size_t(t) * L.n_pad + o) * c_t + c] = f32_to_bf16_rne(tw->at(size_t(o) * T * c_t + size_t(t) * c_t + c));
+        }
+        L.w = reinterpret_cast<bf16 *>(upload(w));
+        L.bias = upload(b);
+        return L.w && L.bias;
+    }
+
+    // R23 prior branch: canonical [c_h][c_ctx][1][1] -> fp64 [c_ctx][c_h] (k-major) + bias
+    bool prior(double *&w_p, double *&b_p, const std::string &name, int c_ctx, int c_h)
+    {
+        const Tensor *tw = get(name + ".w", {uint32_t(c_h), uint32_t(c_ctx), 1u, 1u});
+        const Tensor *tb = get(name + ".b", {uint32_t(c_h)});
+        if (!tw || !tb) return false;
+        std::vector<double> w(size_t(c_ctx) * c_h), b(c_h);
+        for (int o = 0; o < c_h; ++o) {
+            b[o] = double(tb->at(o));
+            for (int k = 0; k < c_ctx; ++k) w[size_t(k) * c_h + o] = double(tw->at(size_t(o) * c_ctx + k));
+        }
+        w_p = upload(w); b_p = upload(b);
+        return w_p && b_p;
+    }
+
     bool depthwise(float *&dw, float *&db, const std::string &name, int C)
     {
         const Tensor *tw = get(name + ".w", {uint32_t(C), 1u, 3u, 3u});
@@ -208,7 +242,7 @@ int load_weights_impl(ufnvc_handle *h, const void *blob, size_t bytes)
     bool ok = ld.hyper(h->hyper[0], "hyper.0", c.c_z, c.c_hyper) && ld.hyper(h->hyper[1], "hyper.1", c.c_hyper, c.c_hyper) &&
               ld.hyper(h->hyper[2], "hyper.2", c.c_hyper, 2 * c.c_y * 16);
     if (ok && h->hybrid_head) ok = ld.head_hybrid(h->head_tc, h->head_fix_w, h->head_fix_b, h->head_wnorm, "hyper.2", c.c_hyper, c.c_y);
-    ok = ok && ld.conv(h->xframe, {"xframe"}, c.c_y, c.T * c.c_trunk, 1, false);
+    ok = ok && ld.conv(h->xframe, {"xframe"}, h->c_cat, c.T * c.c_trunk, 1, false);          // [y ; C_i] with a context (R23)
     for (int k = 1; ok && c.mu_steps == 4 && k <= 3; ++k) ok = ld.mu_net(h->mu_net[k - 1], "mu." + std::to_string(k), c.c_y);
     h->trunk.assign(c.n_trunk_blocks, ufnvc_handle::TrunkBlock());
     const int ce = c.c_trunk * c.trunk_expand;
@@ -216,6 +250,16 @@ int load_weights_impl(ufnvc_handle *h, const void *blob, size_t bytes)
         const std::string b = "trunk." + std::to_string(k);
         ok = ld.depthwise(h->trunk[k].dw_w, h->trunk[k].dw_b, b + ".dw", c.c_trunk) &&
              ld.conv(h->trunk[k].pw1, {b + ".pw1"}, c.c_trunk, ce, 1, false) && ld.conv(h->trunk[k].pw2, {b + ".pw2"}, ce, c.c_trunk, 1, false);
+    }
+    h->ctx_blocks.assign(c.n_ctx_blocks, ufnvc_handle::TrunkBlock());
+    if (ok && h->has_ctx) {
+        ok = ld.fold(h->ctx_fold, "ctx.fold", c.c_trunk, c.T, c.c_trunk) && ld.conv(h->ctx_out, {"ctx.out"}, c.c_trunk, c.c_trunk, 1, false) &&
+             ld.prior(h->ctx_prior_w, h->ctx_prior_b, "ctx.prior", c.c_trunk, c.c_hyper);
+        for (int k = 0; ok && k < c.n_ctx_blocks; ++k) {
+            const std::string b = "ctx." + std::to_string(k);
+            ok = ld.depthwise(h->ctx_blocks[k].dw_w, h->ctx_blocks[k].dw_b, b + ".dw", c.c_trunk) &&
+                 ld.conv(h->ctx_blocks[k].pw1, {b + ".pw1"}, c.c_trunk, ce, 1, false) && ld.conv(h->ctx_blocks[k].pw2, {b + ".pw2"}, ce, c.c_trunk, 1, false);
+        }
     }
     for (int s = 0; ok && s < 4; ++s) {
         std::vector<std::string> names;

@@ -44,6 +44,7 @@ class ChunkConfig:
     mu_law: str = "normal"         # "normal": N(0,1); "uniform": U(-2,2)
     sigma_hi: float = 20.0         # ln sigma ~ U[ln scale_min, ln sigma_hi] (moment-matched, see make_weights)
     mu_steps: int = 1              # 1: the head's mean serves every element; 4: progressive means (R21)
+    n_ctx_blocks: int = 0          # > 0: temporal chunk context (R23) with that many DC blocks in the context generation
 
     # derived geometry (SURVEY.md section 8 notation)
     @property
@@ -85,7 +86,10 @@ class ChunkConfig:
                            + self.c_hyper * 2 * self.c_y * 16)
         if self.mu_steps == 4:
             m += 3 * P * 9 * 2 * self.c_y * self.c_y
-        m += P * self.c_y * self.T * self.c_trunk
+        m += P * (self.c_y + (self.c_trunk if self.n_ctx_blocks else 0)) * self.T * self.c_trunk
+        if self.n_ctx_blocks:      # prior branch, fold, DC blocks, output conv (R23)
+            m += hz * wz * self.c_trunk * self.c_hyper + P * self.T * self.c_trunk * self.c_trunk + P * self.c_trunk * self.c_trunk
+            m += self.n_ctx_blocks * P * (9 * self.c_trunk + 2 * self.c_trunk * self.c_trunk * self.trunk_expand)
         m += self.n_trunk_blocks * self.T * P * (9 * self.c_trunk
                                                  + 2 * self.c_trunk * self.c_trunk * self.trunk_expand)
         pix = P
@@ -112,6 +116,12 @@ CONFIGS = {
 def progressive_config(cfg: ChunkConfig) -> ChunkConfig:
     """Same workload with the four-step progressive means switched on (R21)."""
     return dataclasses.replace(cfg, mu_steps=4, name=cfg.name + "-pmu")
+
+
+def context_config(cfg: ChunkConfig, n_ctx_blocks: int = 11) -> ChunkConfig:
+    """Same workload with the temporal chunk context switched on (R23); 11 DC blocks in
+    the cross-chunk context generation is the paper's HT-S count."""
+    return dataclasses.replace(cfg, n_ctx_blocks=n_ctx_blocks, name=cfg.name + f"-ctx{n_ctx_blocks}")
 
 
 def crop_config(cfg: ChunkConfig, height: int, width: int, name: str | None = None) -> ChunkConfig:
@@ -198,6 +208,22 @@ def make_weights(cfg: ChunkConfig) -> dict:
             conv(f"mu.{k}", cfg.c_y, 2 * cfg.c_y, 3, var_mu / ex2_in)
     # cross-frame unfold (O6): gain so that E[F0^2] ~ 1.
     conv("xframe", cfg.T * cfg.c_trunk, cfg.c_y, 1, 1.0 / _second_moment_yhat(cfg))
+    if cfg.n_ctx_blocks > 0:
+        # temporal chunk context (NEXT-2a, R23).  The unfold sees [y ; C_i]: the context columns get their own gain (C has
+        # second moment ~2, y ~60) so that each half contributes a comparable share of F0
+        cc = cfg.c_trunk
+        conv("xframe.ctx", cfg.T * cfg.c_trunk, cc, 1, 0.5 / 2.0)
+        out["xframe.w"] = np.concatenate([out["xframe.w"] * np.float32(math.sqrt(0.5)), out.pop("xframe.ctx.w")], axis=1)
+        if cfg.weight_dtype == 1:
+            out["xframe.w"] = round_to_bf16(out["xframe.w"])
+        out.pop("xframe.ctx.b")
+        conv("ctx.fold", cc, cfg.T * cfg.c_trunk, 1, 1.0 / 1.5)
+        for k in range(cfg.n_ctx_blocks):
+            conv(f"ctx.{k}.dw", cc, 1, 3, 1.0)
+            conv(f"ctx.{k}.pw1", cc * cfg.trunk_expand, cc, 1, 2.0)
+            conv(f"ctx.{k}.pw2", cc, cc * cfg.trunk_expand, 1, 1.0 / cfg.n_ctx_blocks)
+        conv("ctx.out", cc, cc, 1, 1.0 / 2.0)
+        conv("ctx.prior", cfg.c_hyper, cc, 1, 2.0 * 1.0 / 0.5)       # q = ReLU(W_p pool4(C) + b_p) with E[q^2] ~ 1
     # trunk (O7): shared over t; W2 scaled by 1/B so the residual stream stays O(1).
     ce = cfg.c_trunk * cfg.trunk_expand
     for k in range(cfg.n_trunk_blocks):

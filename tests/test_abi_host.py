@@ -31,7 +31,7 @@ def test_library_exports_every_declared_symbol():
 
 def test_config_struct_layout():
     c = binding.make_config(synth.CONFIGS[3])
-    assert c.struct_size == C.sizeof(binding.ufnvc_config) == 104
+    assert c.struct_size == C.sizeof(binding.ufnvc_config) == 112
     assert (c.T, c.height, c.width, c.c_y) == (8, 1080, 1920, 128)
     assert list(c.dec_channels) == [256, 192, 128, 64, 3] and c.max_chunks_per_call == 1
     assert binding.make_config(synth.CONFIGS[4]).max_chunks_per_call == 4

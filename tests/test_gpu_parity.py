@@ -40,15 +40,15 @@ CASES["cfg3-crop-T1"] = dataclasses.replace(synth.crop_config(synth.CONFIGS[3], 
 
 
 def bf16_bound(want, n_roundings):
-    """Bound on the error of a bf16-stored activation tensor ("Tolerances"): every bf16 store rounds to 8
-    significant bits, relative error uniform in +-2^-9, i.e. rms 2^-9 / sqrt 3 of the element; the layer gains are ~1
-    (R11), so after L roundings on the path the error has rms <= sqrt(L) 2^-9 rms(x) (a factor sqrt 3 above the
-    expectation), and its maximum over <= 1e8 elements stays under 6 sigma of the element-wise worst case
-    sqrt(L) 2^-9 / sqrt 3 * max|x|.  Returns (rms bound, max bound)."""
+    """Bound on the error of a bf16-stored activation tensor ("Tolerances"): a bf16 store keeps 8 significant
+    bits, so its relative error is uniform in +-2^-8 (2^e / |x|) <= +-2^-8, rms <= 2^-8 / sqrt 3 of the element; the
+    layer gains are ~1 (R11), so after L roundings on the path the error has rms <= sqrt(L) 2^-8 / sqrt 3 * rms(x), and its
+    maximum over <= 1e8 elements stays under 6 sigma of the element-wise worst case, sqrt(L) 2^-8 / sqrt 3 * max|x|.
+    Returns (rms bound, max bound)."""
     rms = float(np.sqrt(np.mean(np.square(want, dtype=np.float64))))
     amp = float(np.abs(want).max())
-    r = math.sqrt(n_roundings) * 2.0 ** -9
-    return r * max(rms, 1e-3), 6.0 * r / math.sqrt(3.0) * max(amp, 1.0)
+    r = math.sqrt(n_roundings) * 2.0 ** -8 / math.sqrt(3.0)
+    return r * max(rms, 1e-3), 6.0 * r * max(amp, 1.0)
 
 
 @pytest.fixture(scope="module")
