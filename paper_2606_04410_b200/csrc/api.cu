@@ -36,7 +36,8 @@ int validate(const ufnvc_config &c, std::string &why)
     BAD(c.struct_size != sizeof(ufnvc_config), "struct_size mismatch");
     BAD(c.T < 1 || c.T > 64, "T out of range");
     BAD(c.height < 1 || c.width < 1 || c.height > 16384 || c.width > 16384, "frame size out of range");
-    BAD(c.c_y < 8 || c.c_y % 8 || c.c_z < 1 || c.c_hyper < 1, "c_y must be a multiple of 8; c_z, c_hyper >= 1");
+    BAD(c.c_y < 8 || c.c_y % 8 || c.c_z < 16 || c.c_z % 16 || c.c_hyper < 16 || c.c_hyper % 16,
+        "c_y must be a multiple of 8; c_z and c_hyper multiples of 16");
     BAD(c.c_trunk < 8 || c.c_trunk % 8, "c_trunk must be a multiple of 8");
     BAD(c.n_trunk_blocks < 0 || c.n_trunk_blocks > 64 || c.trunk_expand < 1, "bad trunk");
     BAD(c.dec_channels[0] != c.c_trunk || c.dec_channels[4] != 3, "dec_channels[0] must equal c_trunk and [4] must be 3");
@@ -113,7 +114,7 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     // sum |w||x| <= |w|_2 |x|_2 (Cauchy-Schwarz), so |error| <= kappa |w row|_2 |x patch|_2.
     h->head_kappa = std::ldexp(1.0, -16) + 3.0 * std::sqrt(18.0 * cfg->c_hyper) * std::ldexp(1.0, -24);
     // function attributes are per device: configure every kernel for the device this handle lives on
-    if (configure_rans_kernels() != cudaSuccess || configure_depthwise_kernels() != cudaSuccess || configure_conv_tc_kernels() != cudaSuccess ||
+    if (configure_rans_kernels() != cudaSuccess || configure_hyper_kernels() != cudaSuccess || configure_depthwise_kernels() != cudaSuccess || configure_conv_tc_kernels() != cudaSuccess ||
         configure_trunk_kernels() != cudaSuccess || configure_final_kernels() != cudaSuccess) {
         cudaGetLastError();
         delete h;
@@ -130,9 +131,9 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
 
     const size_t n = size_t(h->max_chunks), P = size_t(h->h) * h->w, Pz = size_t(h->h_z) * h->w_z, T = size_t(cfg->T);
     bool ok = dev_alloc(h, h->d_cf, cf.size()) && dev_alloc(h, h->d_lut, lut.size()) &&
-              dev_alloc(h, h->hx0, n * Pz * cfg->c_z) && dev_alloc(h, h->hx1, n * Pz * cfg->c_hyper) &&
-              dev_alloc(h, h->hx2, n * Pz * cfg->c_hyper) && dev_alloc(h, h->xs, n * Pz * 2 * cfg->c_hyper) && dev_alloc(h, h->xnorm2, n * Pz) &&
-              dev_alloc(h, h->fix_list, n * P * cfg->c_y) && dev_alloc(h, h->hpart, 9 * n * Pz * cfg->c_hyper) && dev_alloc(h, h->mu, n * P * cfg->c_y) &&
+              dev_alloc(h, h->hx1, n * Pz * cfg->c_hyper) &&
+              dev_alloc(h, h->hx2, n * Pz * cfg->c_hyper) && dev_alloc(h, h->xs, n * Pz * 2 * cfg->c_hyper) && dev_alloc(h, h->xnorm2, n * Pz * size_t((cfg->c_hyper + 31) / 32)) &&
+              dev_alloc(h, h->fix_list, n * P * cfg->c_y) && dev_alloc(h, h->mu, n * P * cfg->c_y) &&
               dev_alloc(h, h->lnscale, n * P * cfg->c_y) && dev_alloc(h, h->idx, n * P * cfg->c_y) &&
               dev_alloc(h, h->yhat, n * P * size_t(h->c_cat)) && dev_alloc(h, h->fa, n * T * P * cfg->c_trunk) &&
               dev_alloc(h, h->fb, n * T * P * cfg->c_trunk) &&

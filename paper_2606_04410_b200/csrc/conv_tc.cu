@@ -140,7 +140,10 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
 #pragma unroll
                 for (int t = 0; t < 9; ++t) {
                     const int yy = y + t / 3 - 1, xx = x + t % 3 - 1;
-                    if (yy >= 0 && yy < p.H && xx >= 0 && xx < p.W) s2 += __ldg(p.E.xnorm2 + ((long long)img * p.H + yy) * p.W + xx);
+                    if (yy >= 0 && yy < p.H && xx >= 0 && xx < p.W) {
+                        const float *xp = p.E.xnorm2 + (((long long)img * p.H + yy) * p.W + xx) * p.E.xnorm_parts;
+                        for (int q = 0; q < p.E.xnorm_parts; ++q) s2 += __ldg(xp + q);
+                    }
                 }
                 xpatch = sqrtf(s2);
             }
@@ -843,7 +846,7 @@ cudaError_t configure_conv_tc_kernels()
 {
     cudaError_t e = cudaSuccess;
     auto set = [&](auto kern) { if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); };
-    set(conv_halo_pair_kernel<EPI_PS2>);
+    set(conv_halo_pair_kernel<EPI_PS2>); set(conv_halo_pair_kernel<EPI_HEAD>);
     set(conv_halo_kernel<EPI_NHWC, true>); set(conv_halo_kernel<EPI_NHWC, false>);
     set(conv_halo_kernel<EPI_PS2, true>); set(conv_halo_kernel<EPI_PS2, false>);
     set(conv_halo_kernel<EPI_HEAD, false>);
@@ -857,7 +860,7 @@ cudaError_t configure_conv_tc_kernels()
 cudaError_t launch_conv_halo_pair(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
                                   LaunchStream st)
 {
-    if (L.taps != 9 || !L.has_half_map || E.mode != EPI_PS2) return cudaErrorInvalidValue;
+    if (L.taps != 9 || !L.has_half_map || (E.mode != EPI_PS2 && E.mode != EPI_HEAD)) return cudaErrorInvalidValue;
     TcParams p{};
     p.H = P.H; p.W = P.W;
     p.n_img_m = P.n_img; p.Hm = P.H; p.Wm = P.W;
@@ -880,6 +883,7 @@ cudaError_t launch_conv_halo_pair(const ConvLayer &L, const ConvProblem &P, cons
     if (nb < 2) return cudaErrorInvalidValue;
     const size_t smem = 1024 + size_t(na) * kHaloStage + size_t(nb) * bh_bytes + 256 + 16 * size_t(nb) + 16 * size_t(na);
     const int clusters = p.total_tiles < num_sms / 2 ? p.total_tiles : num_sms / 2;
+    if (E.mode == EPI_HEAD) return launch_pdl(conv_halo_pair_kernel<EPI_HEAD>, 2 * clusters, kThreads, smem, st, 2, tmap_halo, L.tmap_w_half, p, nb, na);
     return launch_pdl(conv_halo_pair_kernel<EPI_PS2>, 2 * clusters, kThreads, smem, st, 2, tmap_halo, L.tmap_w_half, p, nb, na);
 }
 

@@ -60,33 +60,37 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     const bool need_hyper = entropy_params_only || !idx_ovr || !mu_ovr || (taps && (taps->mu || taps->lnscale));
     mark(sg, st);
     if (need_hyper) {
-        CU_TRY(launch_z_to_f64(z, h->hx0, n, c.c_z, Pz, st));
-        CU_TRY(launch_hyper_conv(h->hyper[0], h->hx0, h->hx1, h->hpart, n, h->h_z, h->w_z, st));
+        // layer 0 reads the int16 hyper-latent directly; layers 0 and 1 are one fp64 launch each (hyper.cu)
+        CU_TRY(launch_hyper_conv(h->hyper[0], z, true, h->hx1, n, h->h_z, h->w_z, st));
         HeadParams hp{c.c_y, h->h, h->w, c.n_buckets, std::log(c.scale_min), std::log(c.scale_max), h->mu, h->lnscale, h->idx};
+        const double *q = h->has_ctx ? h->ctx_q : nullptr;
         if (h->hybrid_head && h->am_xs.ok && h->head_tc.use_tc) {
-            // layer 1 also emits the bf16 hi|mid split; the head runs on tensor cores; elements whose ln sigma lands within
-            // flag_u of a bucket edge are re-decided in fp64 (identical decisions to the all-fp64 path, R12)
-            CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, h->hpart, n, h->h_z, h->w_z, st, h->xs, h->xnorm2, h->has_ctx ? h->ctx_q : nullptr));
+            // layer 1 also emits the bf16 hi|mid split; the head runs on tensor cores; elements whose ln sigma may land on the
+            // wrong side of a bucket edge are re-decided in fp64 (identical decisions to the all-fp64 path, R12)
+            CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, false, h->hx2, n, h->h_z, h->w_z, st, h->xs, h->xnorm2, q));
             const double step = (hp.ln_hi - hp.ln_lo) / double(c.n_buckets - 1 > 0 ? c.n_buckets - 1 : 1);
             EpiParams E{};
             E.mode = EPI_HEAD; E.act = ACT_NONE;
             E.mu = h->mu; E.lnscale = h->lnscale; E.idx = h->idx; E.fix_list = h->fix_list; E.fix_count = h->fix_count;
             E.c_y = c.c_y; E.lat_h = h->h; E.lat_w = h->w; E.n_buckets = c.n_buckets;
             E.ln_lo = float(hp.ln_lo); E.ln_hi = float(hp.ln_hi); E.t_scale = float(1.0 / step);
-            E.wnorm = h->head_wnorm; E.xnorm2 = h->xnorm2; E.kappa_t = float(h->head_kappa / step);
+            E.wnorm = h->head_wnorm; E.xnorm2 = h->xnorm2; E.xnorm_parts = hyper_xnorm_parts(h->hyper[1]); E.kappa_t = float(h->head_kappa / step);
             ConvProblem pr{h->xs, n, h->h_z, h->w_z, 1};
-            // z maps are tiny (17 x 30 at 1080p): the shifted-TMA-box kernel tiles them with the least padding
-            CU_TRY(launch_conv_tc(h->head_tc, pr, h->am_xs.tm, h->am_xs.tile_h, h->am_xs.tile_w, false, E, h->num_sms, st));
+            // The head is bound by L2 -> SM weight traffic (18.9 MB of weights, re-read once per M tile): the CTA-pair halo
+            // kernel shares every weight tile between two 16 x 8 pixel tiles (M = 256) and loads the activations once per
+            // slab instead of once per tap.  Fallback: the shifted-TMA-box kernel (narrow maps, debug flag).
+            if (h->use_pair_conv && h->head_tc.has_half_map && h->am_xs.halo_ok && h->w_z > 8)
+                CU_TRY(launch_conv_halo_pair(h->head_tc, pr, h->am_xs.tm_halo, E, h->num_sms, st));
+            else
+                CU_TRY(launch_conv_tc(h->head_tc, pr, h->am_xs.tm, h->am_xs.tile_h, h->am_xs.tile_w, false, E, h->num_sms, st));
             CU_TRY(launch_hyper_fix(h->fix_list, h->fix_count, h->hx2, h->head_fix_w, h->head_fix_b, c.c_hyper, h->h_z, h->w_z, hp,
                                     h->num_sms, st));
-            *launches += 2;                    // head conv + fp64 fix
+            *launches += 4;                    // two fp64 layers + head conv + fp64 fix
         } else {
-            CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, h->hx2, h->hpart, n, h->h_z, h->w_z, st, nullptr, nullptr, h->has_ctx ? h->ctx_q : nullptr));
+            CU_TRY(launch_hyper_conv(h->hyper[1], h->hx1, false, h->hx2, n, h->h_z, h->w_z, st, nullptr, nullptr, q));
             CU_TRY(launch_hyper_head(h->hyper[2], h->hx2, n, h->h_z, h->w_z, hp, st));
+            *launches += 3;
         }
-        auto hyper_kernels = [](const HyperLayer &L) { return (L.c_in % 16 == 0 && L.n % 4 == 0) ? 2 : 1; };   // split-tap + reduce
-        *launches += 1 + hyper_kernels(h->hyper[0]) + hyper_kernels(h->hyper[1]);
-        if (!(h->hybrid_head && h->am_xs.ok && h->head_tc.use_tc)) *launches += 1;
     }
     if (entropy_params_only) {
         if (mu_out) CU_TRY(cudaMemcpyAsync(mu_out, h->mu, ne * 4, cudaMemcpyDeviceToDevice, st));
@@ -482,9 +486,9 @@ extern "C" int ufnvc_launches_per_call(const ufnvc_handle *h, int n_chunks)
 {
     if (!h || n_chunks < 1) return UFNVC_E_INVALID_ARG;
     // kernels counted by the last decode on this handle (the count does not depend on n_chunks); before any decode, the
-    // count of the default path: 7 hyper (hybrid head) + rANS + A5 + (depthwise + fused MLP) per trunk block + 4 stages
+    // count of the default path: 4 hyper (hybrid head) + rANS + A5 + (depthwise + fused MLP) per trunk block + 4 stages
     if (h->last_launches > 0) return h->last_launches;
-    return 7 + 1 + 1 + 2 * h->cfg.n_trunk_blocks + 4;
+    return 4 + 1 + 1 + 2 * h->cfg.n_trunk_blocks + 4;
 }
 
 extern "C" int ufnvc_chunk_decode_profiled(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, const uint8_t *bits_dev,

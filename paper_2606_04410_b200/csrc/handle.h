@@ -66,7 +66,7 @@ struct ufnvc_handle {
     bool dw_ctx_ok = false;
 
     // workspace (sized for max_chunks)
-    double *hx0 = nullptr, *hx1 = nullptr, *hx2 = nullptr, *hpart = nullptr;
+    double *hx1 = nullptr, *hx2 = nullptr;
     float *mu = nullptr, *lnscale = nullptr;
     uint8_t *idx = nullptr;
     ufnvc::bf16 *yhat = nullptr, *fa = nullptr, *fb = nullptr, *hidden = nullptr;

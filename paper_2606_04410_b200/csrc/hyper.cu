@@ -10,21 +10,6 @@
 
 namespace ufnvc {
 
-__global__ void z_to_f64_kernel(const int16_t *__restrict__ z, double *__restrict__ out, int n_chunks, int c_z, int pz)
-{
-    asm volatile("griddepcontrol.wait;" ::: "memory");              // PDL: launched early, the predecessor's output is complete from here on
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    // z planar [n][c][pz] -> out NHWC [n][pz][c]
-    const long long total = (long long)n_chunks * c_z * pz;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
-        const int c = int(i % c_z);
-        const long long r = i / c_z;
-        const int p = int(r % pz);
-        const int n = int(r / pz);
-        out[i] = double(z[((long long)n * c_z + c) * pz + p]);
-    }
-}
-
 constexpr int HM = 32, HN = 64, HK = 16;
 
 struct HyperEpi {
@@ -128,15 +113,13 @@ __global__ void __launch_bounds__(256) hyper_conv_kernel(const double *__restric
 
 // ---- fast path: 64 x 64 tile, 256 threads, 4 x 4 doubles per thread, K step 16, register-prefetch double buffering.
 // Requires c_in % 16 == 0 (a K step never straddles a tap) and n_out % 4 == 0.  DFMA-pipe bound by design: per warp
-// and k, 2 broadcast A vectors + 512 B of conflict-free B feed 512 DFMAs.  SPLIT = true: blockIdx.z = tap, raw partial
-// sums go to part[tap][M][n_out] and hyper_reduce_kernel adds them in tap order (deterministic), for the two small
-// layers that would otherwise occupy 16 CTAs.
+// and k, 2 broadcast A vectors + 512 B of conflict-free B feed 512 DFMAs.  Used by the all-fp64 head (N = 4096 gives it
+// enough blocks); layers 0 and 1 run on hyper_conv_direct_kernel below.
 constexpr int FM = 64, FN = 64, FK = 16, FPAD = 2;
 
-template <bool SPLIT>
 __global__ void __launch_bounds__(256) hyper_conv_fast_kernel(const double *__restrict__ in, const double *__restrict__ wt,
                                                               const double *__restrict__ bias, int n_img, int hz, int wz,
-                                                              int c_in, int n_out, HyperEpi epi, double *__restrict__ part)
+                                                              int c_in, int n_out, HyperEpi epi)
 {
     __shared__ __align__(16) double As[2][FK][FM + FPAD];
     __shared__ __align__(16) double Bs[2][FK][FN];
@@ -155,7 +138,7 @@ __global__ void __launch_bounds__(256) hyper_conv_fast_kernel(const double *__re
     const int b_k = tid >> 4, b_n = (tid & 15) * 4;
     const bool b_ok = n0 + b_n < n_out;
 
-    const int tap_lo = SPLIT ? blockIdx.z : 0, tap_hi = SPLIT ? blockIdx.z + 1 : 9;
+    const int tap_lo = 0, tap_hi = 9;
     const int ksteps_per_tap = c_in / FK;
     const int total_steps = (tap_hi - tap_lo) * ksteps_per_tap;
 
@@ -213,71 +196,141 @@ __global__ void __launch_bounds__(256) hyper_conv_fast_kernel(const double *__re
         for (int j = 0; j < 4; ++j) {
             const int o = n0 + (j < 2 ? tx * 2 + j : 32 + tx * 2 + (j - 2));
             if (o >= n_out) continue;
-            if (SPLIT) {
-                part[((long long)blockIdx.z * M + m) * n_out + o] = acc[i][j];
+            hyper_epilogue(epi, acc[i][j] + bias[o], m, o, pz, wz, n_out);
+        }
+    }
+}
+
+// ---- layers 0 and 1 (O1): direct implicit GEMM in fp64, ONE launch per layer.  B200's plain DFMA rate is 16 per clock and SM
+// (measured: 75 MFMA of layer 1 never ran under 16 us), so the two layers cost >= 25 us whatever the kernel; the job here is to
+// keep every SM's FP64 pipe busy without extra launches.  The z map is tiny (510 pixels at 1080p), so the output tile is small
+// -- 16 pixels x 32 channels, 32 x 4 tiles for 510 x 128 -- and K (9 taps x C_in) is split FOUR ways inside the block: 512
+// threads = 4 groups of 128, each group runs a quarter of the K steps on its own double-buffered shared-memory stage (named
+// barriers, no block-wide sync in the loop) with 2 x 2 outputs per thread; the groups' partial sums are added in fixed order
+// at the end (deterministic).  (The first build split the 9 taps over blockIdx.z and added the partials in a second launch:
+// 5 launches for the two layers where there are 2 now.)
+// ZIN: the input is the int16 hyper-latent itself, planar [n][c_z][pz] (layer 0), converted on load.
+// Epilogue: + bias, ReLU; layer 1 also adds the context branch q (R23), writes the 2-term bf16 split hi | mid the tensor-core
+// head reads, and this block's share of sum_c v^2 per pixel (xnorm2[m][n-tile]; the head adds the shares in order).
+constexpr int DM = 16, DN = 32, DK = 16, DG = 4;
+constexpr size_t kDirectSmem = size_t(DG) * 2 * DK * (DM + 2 + DN) * sizeof(double);      // 51.2 KB: dynamic
+
+template <bool ZIN>
+__global__ void __launch_bounds__(128 * DG) hyper_conv_direct_kernel(const void *__restrict__ in_raw, const double *__restrict__ wt,
+                                                                     const double *__restrict__ bias, int n_img, int hz, int wz, int c_in,
+                                                                     int n_out, double *__restrict__ out, const double *__restrict__ addend,
+                                                                     bf16 *__restrict__ xs, float *__restrict__ xnorm2)
+{
+    extern __shared__ __align__(16) double direct_smem[];
+    double (*As)[2][DK][DM + 2] = reinterpret_cast<double (*)[2][DK][DM + 2]>(direct_smem);
+    double (*Bs)[2][DK][DN] = reinterpret_cast<double (*)[2][DK][DN]>(direct_smem + size_t(DG) * 2 * DK * (DM + 2));
+    asm volatile("griddepcontrol.wait;" ::: "memory");              // PDL: launched early, the predecessor's output is complete from here on
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    const int pz = hz * wz;
+    const int M = n_img * pz;
+    const int m0 = blockIdx.x * DM, n0 = blockIdx.y * DN;
+    const int grp = threadIdx.x >> 7, tid = threadIdx.x & 127;
+    const int ty = tid >> 4, tx = tid & 15;                         // pixels 2 ty, 2 ty + 1; channels 2 tx, 2 tx + 1
+    // loaders (per group): A 16 px x 16 k (2 consecutive k per thread), B 16 k x 32 n (4 consecutive n per thread)
+    const int a_pix = tid >> 3, a_k = (tid & 7) * 2;
+    const int gm = m0 + a_pix;
+    const int a_img = gm < M ? gm / pz : 0, a_p = gm < M ? gm % pz : 0;
+    const int a_y = a_p / wz, a_x = a_p % wz;
+    const int b_k = tid >> 3, b_n = (tid & 7) * 4;
+    const bool b_ok = n0 + b_n < n_out;                             // n_out % 4 == 0
+    const int ksteps_per_tap = c_in / DK;
+    const int total_steps = 9 * ksteps_per_tap;
+    const int s_lo = total_steps * grp / DG, s_hi = total_steps * (grp + 1) / DG;     // this group's K steps
+    const double *in = static_cast<const double *>(in_raw);
+    const int16_t *zin = static_cast<const int16_t *>(in_raw);
+
+    double ra[2];
+    double2 rb[2];
+    auto gload = [&](int step) {
+        const int tap = step / ksteps_per_tap, k0 = (step % ksteps_per_tap) * DK;
+        const int yy = a_y + tap / 3 - 1, xx = a_x + tap % 3 - 1;
+        ra[0] = ra[1] = 0.0;
+        if (gm < M && yy >= 0 && yy < hz && xx >= 0 && xx < wz) {
+            if (ZIN) {
+                const long long o = ((long long)a_img * c_in + k0 + a_k) * pz + (long long)yy * wz + xx;
+                ra[0] = double(zin[o]); ra[1] = double(zin[o + pz]);
             } else {
-                hyper_epilogue(epi, acc[i][j] + bias[o], m, o, pz, wz, n_out);
+                const double2 v = *reinterpret_cast<const double2 *>(in + ((long long)a_img * pz + (long long)yy * wz + xx) * c_in + k0 + a_k);
+                ra[0] = v.x; ra[1] = v.y;
             }
         }
-    }
-}
-
-__global__ void hyper_reduce_kernel(const double *__restrict__ part, const double *__restrict__ bias, double *__restrict__ out,
-                                    long long MN, int n_out, const double *__restrict__ addend)
-{
-    asm volatile("griddepcontrol.wait;" ::: "memory");              // PDL: launched early, the predecessor's output is complete from here on
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < MN; i += (long long)gridDim.x * blockDim.x) {
-        double v = part[i];
-#pragma unroll
-        for (int t = 1; t < 9; ++t) v += part[t * MN + i];                   // fixed tap order: run-to-run deterministic
-        v += bias[i % n_out];
-        v = v > 0.0 ? v : 0.0;
-        if (addend) v += addend[i];                                          // s = x2 + q (R23)
-        out[i] = v;
-    }
-}
-
-cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z, int pz, LaunchStream st)
-{
-    const long long total = (long long)n_chunks * c_z * pz;
-    const int blocks = int((total + 255) / 256 < 1184 ? (total + 255) / 256 : 1184);
-    return launch_pdl(z_to_f64_kernel, unsigned(blocks), 256u, 0, st, 1, z, out, n_chunks, c_z, pz);
-    return cudaGetLastError();
-}
-
-// same reduce, also emitting the 2-term bf16 split of the fp64 result: xs[m][o] = hi = bf16(v), xs[m][n_out + o] = bf16(v - hi),
-// and xnorm2[m] = sum_o v^2 (fp32), the input of the head's a-priori error bound (decode.cu, R12).  One warp per
-// z-pixel m, lanes stride the channels, fixed-order tree reduction: run-to-run deterministic.
-__global__ void hyper_reduce_split_kernel(const double *__restrict__ part, const double *__restrict__ bias, double *__restrict__ out,
-                                          bf16 *__restrict__ xs, float *__restrict__ xnorm2, long long M, int n_out,
-                                          const double *__restrict__ addend)
-{
-    asm volatile("griddepcontrol.wait;" ::: "memory");              // PDL: launched early, the predecessor's output is complete from here on
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    const int lane = threadIdx.x & 31;
-    const long long warps = ((long long)gridDim.x * blockDim.x) >> 5;
-    const long long MN = M * n_out;
-    for (long long m = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5; m < M; m += warps) {
-        double ss = 0.0;
-        for (int o = lane; o < n_out; o += 32) {
-            const long long i = m * n_out + o;
-            double v = part[i];
-#pragma unroll
-            for (int t = 1; t < 9; ++t) v += part[t * MN + i];               // fixed tap order
-            v += bias[o];
-            v = v > 0.0 ? v : 0.0;
-            if (addend) v += addend[i];                                      // s = x2 + q (R23)
-            out[i] = v;
-            const bf16 hi = __double2bfloat16(v);
-            const bf16 mid = __double2bfloat16(v - double(__bfloat162float(hi)));
-            xs[m * 2 * n_out + o] = hi;
-            xs[m * 2 * n_out + n_out + o] = mid;
-            ss = fma(v, v, ss);
+        rb[0] = rb[1] = make_double2(0.0, 0.0);
+        if (b_ok) {
+            const double2 *src = reinterpret_cast<const double2 *>(wt + ((long long)tap * c_in + k0 + b_k) * n_out + n0 + b_n);
+            rb[0] = src[0]; rb[1] = src[1];
         }
+    };
+    auto sstore = [&](int buf) {
+        As[grp][buf][a_k][a_pix] = ra[0]; As[grp][buf][a_k + 1][a_pix] = ra[1];
+        *reinterpret_cast<double2 *>(&Bs[grp][buf][b_k][b_n]) = rb[0];
+        *reinterpret_cast<double2 *>(&Bs[grp][buf][b_k][b_n + 2]) = rb[1];
+    };
+    auto group_sync = [&]() { asm volatile("bar.sync %0, 128;" ::"r"(grp + 1) : "memory"); };
+
+    double acc[2][2] = {};
+    if (s_lo < s_hi) {
+        gload(s_lo);
+        sstore(0);
+    }
+    group_sync();
+    for (int step = s_lo; step < s_hi; ++step) {
+        const int buf = (step - s_lo) & 1;
+        if (step + 1 < s_hi) gload(step + 1);
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xFFFFFFFFu, ss, o);
-        if (lane == 0) xnorm2[m] = float(ss);
+        for (int k = 0; k < DK; ++k) {
+            const double2 a = *reinterpret_cast<const double2 *>(&As[grp][buf][k][ty * 2]);
+            const double2 b = *reinterpret_cast<const double2 *>(&Bs[grp][buf][k][tx * 2]);
+            acc[0][0] = fma(a.x, b.x, acc[0][0]); acc[0][1] = fma(a.x, b.y, acc[0][1]);
+            acc[1][0] = fma(a.y, b.x, acc[1][0]); acc[1][1] = fma(a.y, b.y, acc[1][1]);
+        }
+        if (step + 1 < s_hi) sstore(buf ^ 1);
+        group_sync();
+    }
+    // fixed-order reduction over the K groups: groups 1.. park their partial sums in their own (now idle) B stage
+    double *red = &Bs[grp][0][0][0];
+    if (grp > 0) {
+        red[tid] = acc[0][0]; red[128 + tid] = acc[0][1];           // 512 of the group's 2 x 16 x 32 doubles
+        red[256 + tid] = acc[1][0]; red[384 + tid] = acc[1][1];
+    }
+    __syncthreads();
+    if (grp > 0) return;
+#pragma unroll
+    for (int g2 = 1; g2 < DG; ++g2) {
+        const double *r2 = &Bs[g2][0][0][0];
+        acc[0][0] += r2[tid]; acc[0][1] += r2[128 + tid]; acc[1][0] += r2[256 + tid]; acc[1][1] += r2[384 + tid];
+    }
+
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const int m = m0 + ty * 2 + i;                              // uniform per half-warp; every lane joins the shuffles
+        double ss = 0.0;
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int o = n0 + tx * 2 + j;
+            if (m < M && o < n_out) {
+                double v = acc[i][j] + bias[o];
+                v = v > 0.0 ? v : 0.0;
+                const long long e = (long long)m * n_out + o;
+                if (addend) v += addend[e];                         // s = x2 + q (R23)
+                out[e] = v;
+                if (xs) {
+                    const bf16 hi = __double2bfloat16(v);
+                    xs[(long long)m * 2 * n_out + o] = hi;
+                    xs[(long long)m * 2 * n_out + n_out + o] = __double2bfloat16(v - double(__bfloat162float(hi)));
+                }
+                ss = fma(v, v, ss);
+            }
+        }
+        if (xnorm2) {                                               // the 16 lanes tx = 0..15 of this half-warp hold pixel m's 32 channels
+#pragma unroll
+            for (int o = 8; o > 0; o >>= 1) ss += __shfl_xor_sync(0xFFFFFFFFu, ss, o);
+            if (tx == 0 && m < M) xnorm2[(long long)m * gridDim.y + blockIdx.y] = float(ss);
+        }
     }
 }
 
@@ -301,21 +354,47 @@ __global__ void __launch_bounds__(256) hyper_fix_kernel(const uint32_t *__restri
         const int img = int(r / unsigned(hp.h));
         const int zy = ly >> 2, zx = lx >> 2, ij = ((ly & 3) << 2) | (lx & 3);
         const double *wrow = fix_w + (size_t(c2) * 16 + ij) * 9 * c_h;
-        // lanes stride the channels; 4 independent accumulators (channel blocks) keep the fp64 pipe and the loads busy.
-        // Fixed summation order per element -> run-to-run deterministic.
+        // lanes stride the channels.  The kernel is bound by the latency of its loads (x patch and weight row come from L2),
+        // not by the 1152 DFMAs of an element: all loads of THREE taps are issued before their FMAs (24 in flight per lane
+        // for c_h = 128; one tap at a time measured 1.4x slower).  Four accumulators, fixed summation order per element ->
+        // run-to-run deterministic.
         double a4[4] = {0.0, 0.0, 0.0, 0.0};
+        if (c_h == 128) {
 #pragma unroll
-        for (int tap = 0; tap < 9; ++tap) {
-            const int yy = zy + tap / 3 - 1, xx = zx + tap % 3 - 1;
-            if (yy < 0 || yy >= hz || xx < 0 || xx >= wz) continue;
-            const double *xr = x2 + ((size_t(img) * hz + yy) * wz + xx) * c_h;
-            const double *wr = wrow + tap * c_h;
-            int c = lane;
-            for (; c + 96 < c_h; c += 128) {
+            for (int t3 = 0; t3 < 9; t3 += 3) {
+                double xv[3][4], wv[3][4];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) a4[u] = fma(xr[c + 32 * u], wr[c + 32 * u], a4[u]);
+                for (int t = 0; t < 3; ++t) {
+                    const int tap = t3 + t;
+                    const int yy = zy + tap / 3 - 1, xx = zx + tap % 3 - 1;
+                    const bool ok = yy >= 0 && yy < hz && xx >= 0 && xx < wz;
+                    const double *xr = x2 + ((size_t(img) * hz + (ok ? yy : zy)) * wz + (ok ? xx : zx)) * c_h;
+                    const double *wr = wrow + tap * c_h;
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        xv[t][u] = ok ? xr[lane + 32 * u] : 0.0;
+                        wv[t][u] = wr[lane + 32 * u];
+                    }
+                }
+#pragma unroll
+                for (int t = 0; t < 3; ++t)
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) a4[u] = fma(xv[t][u], wv[t][u], a4[u]);
             }
-            for (; c < c_h; c += 32) a4[0] = fma(xr[c], wr[c], a4[0]);
+        } else {
+#pragma unroll
+            for (int tap = 0; tap < 9; ++tap) {
+                const int yy = zy + tap / 3 - 1, xx = zx + tap % 3 - 1;
+                if (yy < 0 || yy >= hz || xx < 0 || xx >= wz) continue;
+                const double *xr = x2 + ((size_t(img) * hz + yy) * wz + xx) * c_h;
+                const double *wr = wrow + tap * c_h;
+                int c = lane;
+                for (; c + 96 < c_h; c += 128) {
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) a4[u] = fma(xr[c + 32 * u], wr[c + 32 * u], a4[u]);
+                }
+                for (; c < c_h; c += 32) a4[0] = fma(xr[c], wr[c], a4[0]);
+            }
         }
         double acc = (a4[0] + a4[1]) + (a4[2] + a4[3]);
 #pragma unroll
@@ -334,29 +413,38 @@ __global__ void __launch_bounds__(256) hyper_fix_kernel(const uint32_t *__restri
 
 static bool fast_ok(const HyperLayer &L) { return L.c_in % FK == 0 && L.n % 4 == 0; }
 
-cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out, double *part, int n_img, int hz, int wz,
-                              LaunchStream st, bf16 *xs, float *xnorm2, const double *addend)
+cudaError_t configure_hyper_kernels()
 {
-    HyperEpi e{};
-    e.mode = 0;
-    e.out = out;
+    cudaError_t e = cudaFuncSetAttribute(hyper_conv_direct_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kDirectSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(hyper_conv_direct_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kDirectSmem));
+    return e;
+}
+
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_direct(void (*kern)(KArgs...), dim3 grid, LaunchStream st, Args &&...args)      // 2-D grid + dynamic smem + PDL
+{
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = dim3(128 * DG); cfg.dynamicSmemBytes = kDirectSmem; cfg.stream = st.s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = st.pdl ? 1u : 0u;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
+int hyper_xnorm_parts(const HyperLayer &L) { return (L.n + DN - 1) / DN; }
+
+cudaError_t launch_hyper_conv(const HyperLayer &L, const void *in, bool in_is_z, double *out, int n_img, int hz, int wz, LaunchStream st,
+                              bf16 *xs, float *xnorm2, const double *addend)
+{
     const int M = n_img * hz * wz;
-    if (fast_ok(L) && part) {                   // split over the 9 taps, then a deterministic reduce + bias + ReLU
-        dim3 grid((M + FM - 1) / FM, (L.n + FN - 1) / FN, 9);
-        if (cudaError_t le = launch_pdl_grid(hyper_conv_fast_kernel<true>, grid, 256u, st, in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e, part)) return le;
-        const long long MN = (long long)M * L.n;
-        const int blocks = int((MN + 255) / 256 < 1184 ? (MN + 255) / 256 : 1184);
-        if (xs) {
-            const int wblocks = int(((long long)M * 32 + 255) / 256 < 1184 ? ((long long)M * 32 + 255) / 256 : 1184);
-            if (cudaError_t le = launch_pdl(hyper_reduce_split_kernel, unsigned(wblocks), 256u, 0, st, 1, part, L.bias, out, xs, xnorm2, (long long)M, L.n, addend)) return le;
-        }
-        else if (cudaError_t le = launch_pdl(hyper_reduce_kernel, unsigned(blocks), 256u, 0, st, 1, part, L.bias, out, MN, L.n, addend)) return le;
-        return cudaGetLastError();
+    if (L.c_in % DK == 0 && L.n % 4 == 0) {
+        dim3 grid((M + DM - 1) / DM, (L.n + DN - 1) / DN);
+        if (in_is_z)
+            return launch_direct(hyper_conv_direct_kernel<true>, grid, st, in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, out, addend, xs, xnorm2);
+        return launch_direct(hyper_conv_direct_kernel<false>, grid, st, in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, out, addend, xs, xnorm2);
     }
-    if (addend || xs) return cudaErrorInvalidValue;       // the slow-shape kernel has no context branch (api.cu validates the shapes)
-    dim3 grid((M + HM - 1) / HM, (L.n + HN - 1) / HN);
-    hyper_conv_kernel<<<grid, 256, 0, st>>>(in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e);
-    return cudaGetLastError();
+    return cudaErrorInvalidValue;         // api.cu validates c_z % 16 == 0, c_hyper % 16 == 0
 }
 
 // ---- R23: q = ReLU(W_p pool4(C) + b_p), the context branch of the prior input, in fp64.  The context is a bf16 tensor (its
@@ -420,7 +508,7 @@ cudaError_t launch_hyper_head(const HyperLayer &L, const double *in, int n_img, 
     const int M = n_img * hz * wz;
     if (fast_ok(L)) {
         dim3 grid((M + FM - 1) / FM, (L.n + FN - 1) / FN);
-        if (cudaError_t le = launch_pdl_grid(hyper_conv_fast_kernel<false>, grid, 256u, st, in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e, (double *)nullptr)) return le;
+        if (cudaError_t le = launch_pdl_grid(hyper_conv_fast_kernel, grid, 256u, st, in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, e)) return le;
         return cudaGetLastError();
     }
     dim3 grid((M + HM - 1) / HM, (L.n + HN - 1) / HN);

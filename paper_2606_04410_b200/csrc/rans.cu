@@ -18,33 +18,62 @@ __device__ __forceinline__ uint32_t lds_u32(uint32_t addr)
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
     return v;
 }
+// prefetch loads as volatile asm: the compiler keeps them where they are written (a whole register bank ahead of their use)
+// instead of sinking them next to the consumer, where every step would wait for an L2 round trip
+__device__ __forceinline__ uint32_t ldg_u8(const uint8_t *p)
+{
+    uint32_t v;
+    asm volatile("ld.global.nc.u8 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float ldg_f32(const float *p)
+{
+    float v;
+    asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
+
+constexpr int kRansWarps = 4;        // warp-streams per block: one per SM sub-partition, so a step's ~90 instructions never queue
+                                     // behind another warp's (16 warps per block measured 0.33 us per step, issue-slot bound)
 
 // TAPS: the optional fp32 / int16 outputs exist (parity taps, or the residual the progressive means need).
 // STRIDED: y is a channel block of a wider tensor (y_stride != c_y, R23).
+// Grid: (substream, group of blockDim.x / 32 warp-streams).
 template <bool TAPS, bool STRIDED>
-__global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
+__global__ void __launch_bounds__(32 * kRansWarps) rans_decode_kernel(RansParams p, int nb, int groups_per_sub)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     // tables in shared memory, addressed as 32-bit shared addresses (one LDS per access, no generic-address arithmetic in
     // the serial chain): cf[k][pos] = c[pos] | freq[pos] << 16 (freq <= 65282 fits 16 bits), then the search entries
     const uint32_t s_cf = uint32_t(__cvta_generic_to_shared(smem_raw));
     const uint32_t s_lut = s_cf + uint32_t(nb) * 1024u;
-    {
-        const uint4 *src_c = reinterpret_cast<const uint4 *>(p.cf);
-        const uint4 *src_l = reinterpret_cast<const uint4 *>(p.lut);
-        uint4 *dc = reinterpret_cast<uint4 *>(smem_raw), *dl = reinterpret_cast<uint4 *>(smem_raw + size_t(nb) * 1024);
-        for (int i = threadIdx.x; i < nb * 64; i += blockDim.x) dc[i] = src_c[i];
-        for (int i = threadIdx.x; i < nb * (kLutBuckets / 4); i += blockDim.x) dl[i] = src_l[i];
+    const uint32_t s_bar = s_lut + uint32_t(nb) * uint32_t(kLutBuckets) * 4u;
+    if (threadIdx.x == 0) {
+        // the 192 KB of static tables arrive by bulk async copies (one thread, 32 KB pieces) while the predecessor kernel is
+        // still running (PDL): nothing here depends on it
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(s_bar) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        const uint32_t cf_bytes = uint32_t(nb) * 1024u, lut_bytes = uint32_t(nb) * uint32_t(kLutBuckets) * 4u;
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(s_bar), "r"(cf_bytes + lut_bytes) : "memory");
+        for (uint32_t o = 0; o < cf_bytes; o += 32768u) {
+            const uint32_t nbytes = cf_bytes - o < 32768u ? cf_bytes - o : 32768u;
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(s_cf + o),
+                         "l"(reinterpret_cast<const unsigned char *>(p.cf) + o), "r"(nbytes), "r"(s_bar) : "memory");
+        }
+        for (uint32_t o = 0; o < lut_bytes; o += 32768u) {
+            const uint32_t nbytes = lut_bytes - o < 32768u ? lut_bytes - o : 32768u;
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(s_lut + o),
+                         "l"(reinterpret_cast<const unsigned char *>(p.lut) + o), "r"(nbytes), "r"(s_bar) : "memory");
+        }
     }
-    // PDL: the 192 KB of static tables above load while the predecessor (the hyper head's fix-up kernel) is still running;
-    // idx, mu and the status word are only touched after the predecessor grid has completed.
+    // idx, mu, the bit-stream and the status word are only touched after the predecessor grid has completed
     asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    __syncthreads();
+    __syncthreads();                            // the barrier is initialised
 
-    const int sub = blockIdx.x;                 // chunk * n_sub + s
+    const int sub = blockIdx.x / groups_per_sub;                        // chunk * n_sub + s
     const int chunk = sub / p.n_sub, s = sub % p.n_sub;
-    const int g = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = (blockIdx.x % groups_per_sub) * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     const int G = p.W >> 5;
     const int row0 = s * p.rows_per_sub;
     const int rows = min(p.rows_per_sub, p.h - row0);
@@ -82,42 +111,48 @@ __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
     const uint32_t below = (1u << lane) - 1u;
 
     // idx / mu do not depend on the decoder state: they are fetched kPre steps ahead into two register banks, so the
-    // serial chain of a step holds no global-memory latency.  What is kept of the index is the byte offset of its cf table.
+    // serial chain of a step holds no global-memory latency.  Raw values: nothing consumes them before their step.
     constexpr int kPre = 8;
     const int i0 = g * 32 + lane;
+    const uint8_t *idx_p = p.idx + ebase + i0;
+    const float *mu_p = p.mu + ebase + i0;
     uint32_t kA[kPre], kB[kPre];
     float mA[kPre], mB[kPre];
     auto fetch = [&](uint32_t (&kk)[kPre], float (&mm)[kPre], int j0) {
 #pragma unroll
         for (int t = 0; t < kPre; ++t) {
-            const int ii = i0 + (j0 + t) * p.W;
+            const long long o = (long long)(j0 + t) * p.W;
             kk[t] = 0; mm[t] = 0.f;
-            if (ii < n) {                                  // (false for every step past the last one, too)
-                uint32_t k = p.idx[ebase + ii];
-                mm[t] = p.mu[ebase + ii];
-                // an index past the tables (possible only through idx_override_dev) must not read shared memory out of
-                // bounds: clamp and report, like every other malformed input (off the serial chain: this is the prefetch)
-                if (k >= uint32_t(nb)) { k = uint32_t(nb - 1); st |= UFNVC_STREAM_BAD_HEADER; }
-                kk[t] = k << 10;
-            }
+            if (i0 + o < n) { kk[t] = ldg_u8(idx_p + o); mm[t] = ldg_f32(mu_p + o); }     // (false for every step past the last one, too)
         }
     };
+    // running output pointers (element offset of this lane's symbol of the current step)
+    long long e_run = ebase + i0;
     // one symbol per lane.  The serial chain: LDS (search entry) -> ~8 integer ops -> LDS (c | freq) -> multiply-add ->
     // compare -> ballot -> popc -> shuffle -> merge.  Everything else (dequantisation, stores) hangs off it.
-    auto step = [&](const uint32_t kofs, const float mu, const int j, const bool check) {
-        const int i = i0 + j * p.W;
-        const bool valid = !check || i < n;
+    auto step = [&](uint32_t k, const float mu, const int j, const bool check) {
+        const bool valid = !check || i0 + j * p.W < n;
+        // an index past the tables (possible only through idx_override_dev) must not read shared memory out of bounds:
+        // clamp and report, like every other malformed input
+        if (k >= uint32_t(nb)) { k = uint32_t(nb - 1); st |= UFNVC_STREAM_BAD_HEADER; }
+        const uint32_t kofs = k << 10;
         const uint32_t slot = x & 0xFFFFu;
         const uint32_t ent = lds_u32(s_lut + (kofs << 1) + ((slot >> kLutShift) << 2));
         const uint32_t off = slot & ((1u << kLutShift) - 1u);
-        uint32_t pos = (ent & 0xFFu) + uint32_t(off >= ((ent >> 8) & 0xFFu)) + uint32_t(off >= ((ent >> 16) & 0xFFu)) + uint32_t(off >= (ent >> 24));
-        if ((ent & 0xFF00u) == 0xFF00u) {       // > 3 symbols start inside this 128-slot bin (the packed tails): bisect
-            uint32_t lo = ent & 0xFFu, hi = lo + ((ent >> 16) & 0xFFu);
-            while (lo < hi) {                   // largest pos in [lo,hi] with c[pos] <= slot
-                const uint32_t mid = (lo + hi + 1) >> 1;
-                if ((lds_u32(s_cf + kofs + (mid << 2)) & 0xFFFFu) <= slot) lo = mid; else hi = mid - 1;
+        const uint32_t lo = ent & 0xFFu, b1 = __byte_perm(ent, 0, 0x4441), b2 = __byte_perm(ent, 0, 0x4442), b3 = ent >> 24;
+        uint32_t pos = lo + uint32_t(off >= b1) + uint32_t(off >= b2) + uint32_t(off >= b3);
+        if (b1 >= 0xFEu) {                      // > 3 symbols start inside this 128-slot bin (the packed tails)
+            if (b1 == 0xFEu) {                  // a run of 1-slot symbols starting at offset b2, b3 of them
+                const int t = int(off) - int(b2) + 1;
+                pos = lo + uint32_t(min(int(b3), max(t, 0)));
+            } else {                            // bisect: largest pos in [lo, lo + b2] with c[pos] <= slot
+                uint32_t l = lo, hi = lo + b2;
+                while (l < hi) {
+                    const uint32_t mid = (l + hi + 1) >> 1;
+                    if ((lds_u32(s_cf + kofs + (mid << 2)) & 0xFFFFu) <= slot) l = mid; else hi = mid - 1;
+                }
+                pos = l;
             }
-            pos = lo;
         }
         const uint32_t cf = lds_u32(s_cf + kofs + (pos << 2));
         uint32_t xn = (cf >> 16) * (x >> 16) + slot - (cf & 0xFFFFu);
@@ -138,22 +173,27 @@ __global__ void __launch_bounds__(512) rans_decode_kernel(RansParams p, int nb)
         if (valid) {
             const int sym = int(pos) - 127;
             const float y = float(sym) + mu;                             // O5
-            const long long e = ebase + i;
             if (!STRIDED) {
-                p.yhat[e] = __float2bfloat16_rn(y);
+                p.yhat[e_run] = __float2bfloat16_rn(y);
             } else {                                                     // y is the first channel block of a wider tensor (R23)
-                const long long pix = e / p.c_y;
-                p.yhat[pix * p.y_stride + (e - pix * p.c_y)] = __float2bfloat16_rn(y);
+                const long long pix = e_run / p.c_y;
+                p.yhat[pix * p.y_stride + (e_run - pix * p.c_y)] = __float2bfloat16_rn(y);
             }
             if (TAPS) {
-                if (p.sym_tap) p.sym_tap[e] = int16_t(sym);
-                if (p.yhat_tap) p.yhat_tap[e] = y;
+                if (p.sym_tap) p.sym_tap[e_run] = int16_t(sym);
+                if (p.yhat_tap) p.yhat_tap[e_run] = y;
             }
         }
+        e_run += p.W;
     };
 
     const int n_full = n / p.W;                 // steps in which every lane has a symbol
     fetch(kA, mA, 0);
+    {                                           // the tables have landed
+        uint32_t done = 0;
+        while (!done)
+            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(s_bar) : "memory");
+    }
     for (int j0 = 0; j0 < n_steps; j0 += 2 * kPre) {
         fetch(kB, mB, j0 + kPre);
         if (j0 + kPre <= n_full) {
@@ -199,7 +239,7 @@ cudaError_t launch_z_hwc_to_planar(const int16_t *z_hwc, int16_t *z_planar, int 
     return cudaGetLastError();
 }
 
-constexpr size_t kRansSmem = (size_t)64 * (256 * 4 + kLutBuckets * 4);
+constexpr size_t kRansSmem = (size_t)64 * (256 * 4 + kLutBuckets * 4) + 16;      // tables + the arrival barrier
 
 cudaError_t configure_rans_kernels()
 {
@@ -214,11 +254,14 @@ cudaError_t launch_rans_decode(const RansParams &p, LaunchStream st)
 {
     const int nb = p.n_buckets;
     const bool taps = p.sym_tap || p.yhat_tap, strided = p.y_stride != p.c_y;
-    const unsigned grid = unsigned(p.n_chunks * p.n_sub), block = unsigned(p.W);
-    if (taps) return strided ? launch_pdl(rans_decode_kernel<true, true>, grid, block, kRansSmem, st, 1, p, nb)
-                             : launch_pdl(rans_decode_kernel<true, false>, grid, block, kRansSmem, st, 1, p, nb);
-    return strided ? launch_pdl(rans_decode_kernel<false, true>, grid, block, kRansSmem, st, 1, p, nb)
-                   : launch_pdl(rans_decode_kernel<false, false>, grid, block, kRansSmem, st, 1, p, nb);
+    const int G = p.W / 32;
+    const int wpb = G % kRansWarps == 0 ? kRansWarps : (G % 2 == 0 ? 2 : 1);      // warp-streams per block
+    const int groups = G / wpb;
+    const unsigned grid = unsigned(p.n_chunks * p.n_sub * groups), block = unsigned(32 * wpb);
+    if (taps) return strided ? launch_pdl(rans_decode_kernel<true, true>, grid, block, kRansSmem, st, 1, p, nb, groups)
+                             : launch_pdl(rans_decode_kernel<true, false>, grid, block, kRansSmem, st, 1, p, nb, groups);
+    return strided ? launch_pdl(rans_decode_kernel<false, true>, grid, block, kRansSmem, st, 1, p, nb, groups)
+                   : launch_pdl(rans_decode_kernel<false, false>, grid, block, kRansSmem, st, 1, p, nb, groups);
 }
 
 }  // namespace ufnvc

@@ -36,7 +36,9 @@ void build_cdf_tables(int nb, double smin, double smax, std::vector<uint32_t> &c
 //               there is none: the position of slot 128 b + off is  lo + (off >= d_1) + (off >= d_2) + (off >= d_3)
 //               -- no second table access and no loop.
 //   more than three starts inside the bin (only where the tails' 1-slot symbols are packed: < 0.5 % of the mass):
-//               byte 1 = 0xFF, byte 2 = their count m; the kernel then bisects [lo, lo + m].
+//     - the starts are CONSECUTIVE slots d, d + 1, .., d + m - 1 (a run of 1-slot symbols, the far tails of every table):
+//               byte 1 = 0xFE, byte 2 = d, byte 3 = m:   position = lo + min(m, max(0, off - d + 1))
+//     - otherwise byte 1 = 0xFF, byte 2 = m; the kernel then bisects [lo, lo + m].
 void build_search_lut(const std::vector<uint32_t> &cdf32, int nb, std::vector<uint32_t> &lut)
 {
     lut.assign((size_t)nb * kLutBuckets, 0u);
@@ -54,7 +56,10 @@ void build_search_lut(const std::vector<uint32_t> &cdf32, int nb, std::vector<ui
             if (m <= 3) {
                 for (int i = 1; i <= 3; ++i) e |= (i <= m ? c[lo + i] - s0 : 0x80u) << (8 * i);
             } else {
-                e |= 0xFFu << 8 | uint32_t(m) << 16 | 0x80u << 24;
+                bool run = m <= 255;
+                for (int i = 2; run && i <= m; ++i) run = c[lo + i] == c[lo + 1] + uint32_t(i - 1);
+                if (run) e |= 0xFEu << 8 | (c[lo + 1] - s0) << 16 | uint32_t(m) << 24;
+                else e |= 0xFFu << 8 | uint32_t(m) << 16 | 0x80u << 24;
             }
             lut[(size_t)k * kLutBuckets + b] = e;
         }

@@ -43,7 +43,8 @@ struct EpiParams {
     // element (z-pixel m, packed column n') is flagged when |t - round(t)| < kappa_t * wnorm[n'] * sqrt(sum of xnorm2 over the
     // 3x3 neighbourhood of m): the a-priori bound on the tensor-core value's error, in bucket units (decode.cu)
     const float *wnorm;               // [n_pad]: L2 norm of packed weight row n' over its 9 * c_hyper taps
-    const float *xnorm2;              // [n][h_z][w_z]: sum over channels of the squared layer-2 activation
+    const float *xnorm2;              // [n][h_z][w_z][xnorm_parts]: shares of the sum over channels of the squared layer-2 activation
+    int xnorm_parts;
     float kappa_t;
     // EPI_MU (uses c_y), mu^k = acc + bias.  The conv input is [r so far | mu used so far | mu0 | pad] (bf16, in_stride
     // channels).  mu_last == 0: out has the same layout: r and mu blocks updated on partition mu_step.
@@ -126,6 +127,7 @@ inline cudaError_t launch_pdl_grid(void (*kern)(KArgs...), dim3 grid, unsigned b
 // CURRENT device.  Function attributes are per device: ufnvc_create calls all of these for the device the handle lives on, so
 // the launchers hold no "already configured" state (a second handle on another GPU of the same process configures that GPU).
 cudaError_t configure_rans_kernels();
+cudaError_t configure_hyper_kernels();
 cudaError_t configure_depthwise_kernels();
 cudaError_t configure_conv_tc_kernels();
 cudaError_t configure_trunk_kernels();
@@ -148,14 +150,17 @@ struct HyperLayer {
     double *w = nullptr;     // [9][c_in][n]
     double *bias = nullptr;  // [n]
 };
-cudaError_t launch_z_to_f64(const int16_t *z, double *out, int n_chunks, int c_z, int pz, LaunchStream st);
-// addend (optional, [M][n]): added AFTER the ReLU -- the context branch q of the prior input s = x2 + q (R23)
-cudaError_t launch_hyper_conv(const HyperLayer &L, const double *in, double *out, double *part, int n_img, int hz, int wz,
-                              LaunchStream st, bf16 *xs = nullptr, float *xnorm2 = nullptr, const double *addend = nullptr);
+// layers 0 / 1 of the hyper-decoder (O1) in fp64, one launch each.  in: the int16 hyper-latent, planar [n][c_z][pz]
+// (in_is_z), or the previous layer's NHWC fp64 output.  Optional (layer 1): addend [M][n] added AFTER the ReLU -- the context
+// branch q of the prior input s = x2 + q (R23); xs = 2-term bf16 split hi | mid of the result; xnorm2[M][hyper_xnorm_parts]
+// = per-pixel shares of sum_c v^2.
+cudaError_t launch_hyper_conv(const HyperLayer &L, const void *in, bool in_is_z, double *out, int n_img, int hz, int wz, LaunchStream st,
+                              bf16 *xs = nullptr, float *xnorm2 = nullptr, const double *addend = nullptr);
+int hyper_xnorm_parts(const HyperLayer &L);
 // q = ReLU(W_p pool4(C) + b_p) in fp64 from the bf16 context block of the [y ; C] buffer (R23): ctx [n][h][w][stride] (channel
 // block already offset), w_p [c_ctx][c_h] (k-major), q [n][h_z][w_z][c_h]
 cudaError_t launch_ctx_prior(const bf16 *ctx, int stride, int c_ctx, const double *w_p, const double *b_p, double *q, int n_img, int h, int w,
-                             int hz, int wz, int c_h, LaunchStream st);   // part: [9][M][n] scratch for the split-tap fast path (may be null)
+                             int hz, int wz, int c_h, LaunchStream st);
 struct HeadParams {
     int c_y, h, w, n_buckets;
     double ln_lo, ln_hi;
