@@ -16,6 +16,9 @@
 // warp 0 = TMA producer, warp 1 = MMA issuer + TMEM allocator, warps 2..9 = epilogue.  Persistent, grid = #SMs.
 #include <cuda.h>
 
+#include <algorithm>
+#include <cstring>
+
 #include "epilogue.cuh"
 #include "tc_ptx.cuh"
 #include "ufnvc_internal.h"
@@ -27,17 +30,21 @@ namespace {
 constexpr int kC = 256;                  // trunk width: K of GEMM1, N of GEMM2
 constexpr int kHC = 128;                 // hidden columns per chunk
 constexpr int kTM = 128;                 // pixels per tile
-constexpr int kTrunkThreads = 320;
-static_assert(kTrunkThreads / 32 - 2 == int(kTrunkTileSignals), "one tile_done increment per epilogue warp (warps 2..9)");
+constexpr int kTrunkThreads = 320;       // single-CTA kernel: TMA warp, MMA warp, 8 epilogue warps
+constexpr int kPairThreads = 576;        // CTA-pair kernel: TMA warp, MMA warp, 16 epilogue warps
+static_assert(kPairThreads / 32 - 2 == int(kTrunkTileSignals), "one tile_done increment per epilogue warp (warps 2..17)");
 constexpr int kWStages = 3;
 constexpr uint32_t kSlab = 16384;        // 128 rows x 128 B
 constexpr uint32_t kWStage = 32768;
 constexpr uint32_t kOffA = 0, kOffHs = 4 * kSlab, kOffW = kOffHs + 4 * kSlab, kOffBar = kOffW + kWStages * kWStage;
 constexpr uint32_t kTrunkSmem = kOffBar + 256 + 1024;        // + alignment slack
 
+constexpr int kMaxHidden = 1024;         // biases travel in the kernel parameters (constant bank): warp-uniform reads
 struct TrunkParams {
     int n_tiles, n_chunks, n_px;
-    const float *b1, *b2;                // [hidden], [256]
+    const float *b1, *b2;                // [hidden], [256] (device copies: the single-CTA kernel reads these)
+    float hb1v[kMaxHidden];              // b1 / 2 by value (CTA-pair kernel: constant bank, warp-uniform reads)
+    float b2v[kC];                       // b2 by value
     const bf16 *x;                       // residual input  [n_px][256]
     bf16 *out;                           // [n_px][256] (may alias x: a tile reads its own rows before writing them)
     uint32_t *tile_done;                 // optional: [n_tiles] counters, +1 per epilogue warp (8 per tile) once its rows are written
@@ -328,10 +335,37 @@ namespace {
 // TMH = true: the GELU'd hidden chunk goes back into TMEM (bf16, over the fp32 columns it came from) and GEMM2 reads its
 // A operand from there: no 64 KB Hs buffer (the weight ring grows from 3 to 5 stages), and per tile 256 KB of st.shared
 // plus 256 KB of A-operand reads leave the shared-memory port, which TMA writes + MMA operand reads had saturated.
+// (acc0, acc1) + bias -> GELU of each, returned as one bf16x2 word (low half = element 0): the form GEMM2 reads from TMEM.
+// hb = (b0 / 2, b1 / 2).  With w = v / 2:  GELU(v) = w + w tanh(w (2a + 8b w^2)),  (a, b) = (0.80015708, 0.03470089) fitted to
+// the erf form (max |error| 2.7e-4, rms 1.3e-4 -- a quarter of the bf16 rounding of the stored result; the three-coefficient fit
+// of epilogue.cuh is 10x closer but needs a clamp and two more operations).  Five packed-fp32 operations, two MUFU.TANH and
+// one pack per PAIR.  Why this form: at the tensor pipe's full rate a scheduler has 16 issue slots per 32 hidden elements, and
+// clock64 around the phases of the epilogue warps showed the previous GELU (7 packed operations, 2 FMNMX, 2 MUFU, 2 bias
+// shuffles, 1 pack = 14 slots per pair and 14 FMA-pipe cycles) taking 1650 of a chunk's 2048 tensor cycles on every scheduler;
+// with the output drain on the same warps the hidden chunk came back too late for GEMM2 and the tensor pipe idled 45 % of
+// the time.  An f16x2 version was no better (B200 issues fma.f16x2 at the same 2 cycles as fma.f32x2, and tanh.approx.f16x2
+// is two MUFU operations); the floor that remains is the MUFU pipe: 4 lanes per clock = 1024 cycles per chunk.
+__device__ __forceinline__ uint32_t gelu_bias2_pk(float acc0, float acc1, float hb0, float hb1)
+{
+    const uint64_t w = f2_fma(f2_pack(acc0, acc1), f2_pack(0.5f, 0.5f), f2_pack(hb0, hb1));
+    const uint64_t pl = f2_fma(f2_pack(8.0f * 0.03470089f, 8.0f * 0.03470089f), f2_mul(w, w), f2_pack(2.0f * 0.80015708f, 2.0f * 0.80015708f));
+    float u0, u1, t0, t1, g0, g1;
+    f2_unpack(f2_mul(w, pl), u0, u1);
+    asm("tanh.approx.f32 %0, %1;" : "=f"(t0) : "f"(u0));
+    asm("tanh.approx.f32 %0, %1;" : "=f"(t1) : "f"(u1));
+    f2_unpack(f2_fma(w, f2_pack(t0, t1), w), g0, g1);
+    return pack_bf16x2(g0, g1);
+}
+__device__ __forceinline__ void ld_global_256(const void *p, uint32_t (&u)[8])
+{
+    asm volatile("ld.global.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];" : "=r"(u[0]), "=r"(u[1]), "=r"(u[2]), "=r"(u[3]), "=r"(u[4]), "=r"(u[5]),
+                 "=r"(u[6]), "=r"(u[7]) : "l"(p));
+}
+
 constexpr bool TMH = true;     // (the shared-memory-hidden variant, TMH = false, lost the A/B and is no longer instantiated)
-__global__ void __launch_bounds__(kTrunkThreads, 1)
+__global__ void __launch_bounds__(kPairThreads, 1)
 trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant__ CUtensorMap tm_w1h,
-                      const __grid_constant__ CUtensorMap tm_w2h, const TrunkParams p)
+                      const __grid_constant__ CUtensorMap tm_w2h, const __grid_constant__ TrunkParams p)
 {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -356,10 +390,10 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
         mbar_init(bar(B_AFULL), 1); mbar_init(bar(B_AEMPTY), 1);
         for (int s = 0; s < NS; ++s) { mbar_init(bar(B_WFULL + s), 1); mbar_init(bar(B_WEMPTY + s), 1); }
         for (int b = 0; b < 2; ++b) {
-            mbar_init(bar(B_HACC_FULL + b), 1); mbar_init(bar(B_HACC_EMPTY + b), 16);     // 8 epilogue warps x 2 CTAs
-            mbar_init(bar(B_HS_FULL + b), 16);  mbar_init(bar(B_HS_EMPTY + b), 1);
+            mbar_init(bar(B_HACC_FULL + b), 1); mbar_init(bar(B_HACC_EMPTY + b), 32);     // 16 epilogue warps x 2 CTAs
+            mbar_init(bar(B_HS_FULL + b), 32);  mbar_init(bar(B_HS_EMPTY + b), 1);
         }
-        mbar_init(bar(B_OFULL), 1); mbar_init(bar(B_OEMPTY), 16);
+        mbar_init(bar(B_OFULL), 1); mbar_init(bar(B_OEMPTY), 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     cluster_sync_all();                                              // peer barriers are initialised before anyone signals
@@ -468,9 +502,10 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
                     for (int j = 0; j < 2; ++j)
 #pragma unroll
                         for (int k = 0; k < 4; ++k) {
-                            if (TMH)     // hidden 64 j + 16 k .. +15 = 8 packed columns at Hacc[b] + 64 j + 8 k (see the GELU warps)
-                                umma2_bf16_ts(o_acc, h_acc + uint32_t(b) * kHC + uint32_t(64 * j + 8 * k), w + uint32_t(j) * (kSlab >> 4) + 2 * k, hi,
-                                              idesc2, uint32_t(c | j | k));
+                            if (TMH)     // hidden 64 j + 16 k .. +15 = 8 packed columns at Hacc[b] + 64 j + 32 (k / 2) + 8 (k % 2): every GELU
+                                         // warp packs its 32 hidden columns into the first 16 of the fp32 columns it read
+                                umma2_bf16_ts(o_acc, h_acc + uint32_t(b) * kHC + uint32_t(64 * j + 32 * (k >> 1) + 8 * (k & 1)),
+                                              w + uint32_t(j) * (kSlab >> 4) + 2 * k, hi, idesc2, uint32_t(c | j | k));
                             else
                                 umma2_bf16_lh(o_acc, hs_lo + uint32_t(2 * b + j) * (kSlab >> 4) + 2 * k, hi, w + uint32_t(j) * (kSlab >> 4) + 2 * k,
                                               hi, idesc2, uint32_t(c | j | k));
@@ -482,111 +517,88 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
             }
         }
     } else {
-        // ===================== epilogue warps (both CTAs) =====================
-        const int quad = warp & 3, half = (warp - 2) >> 2;
+        // ===================== epilogue warps (both CTAs): 16 = 4 TMEM lane quadrants x 4 column parts =====================
+        // Four warps per scheduler: the GELU of a chunk costs every scheduler >= 1024 MUFU-pipe cycles (one MUFU.TANH per
+        // element at 4 lanes per clock) beside ~900 FMA-pipe cycles, against 2048 tensor cycles per chunk; with two warps per
+        // scheduler the two pipes overlapped badly (1650-1700 cycles per chunk, measured), the hidden chunk came back too
+        // late for GEMM2 and the tensor pipe idled half the time.
+        const int quad = warp & 3, part = (warp - 2) >> 2;               // part: hidden columns [32 part, +32) of a chunk
         const int r = quad * 32 + lane;
         const uint32_t t_lane = tmem_base + (uint32_t(quad * 32) << 16);
-        const uint32_t hacc_empty_l = mapa_rank(bar(B_HACC_EMPTY), 0), hs_full_l = mapa_rank(bar(B_HS_FULL), 0),
-                       oempty_l = mapa_rank(bar(B_OEMPTY), 0);
+        const uint32_t hs_full_l = mapa_rank(bar(B_HS_FULL), 0), oempty_l = mapa_rank(bar(B_OEMPTY), 0);
         uint32_t ph_use = 0;
-        float2 bnext = __ldg(reinterpret_cast<const float2 *>(p.b1 + half * 64) + lane);          // chunk 0
-        float b2r[4];                                                     // b2[half*128 + 32 i + lane]
-#pragma unroll
-        for (int i = 0; i < 4; ++i) b2r[i] = __ldg(p.b2 + half * 128 + 32 * i + lane);
         int it = 0;
         for (int pt = pair0; pt < n_ptiles; pt += n_pairs, ++it) {
             const int tile = 2 * pt + int(rank);
             for (int c = 0; c < NC; ++c) {
                 const int b = c & 1;
                 mbar_wait(bar(B_HACC_FULL + b), (ph_use >> b) & 1);
-                if (!TMH) mbar_wait(bar(B_HS_EMPTY + b), ((ph_use >> b) & 1) ^ 1);
                 ph_use ^= 1u << b;
                 tc_fence_after();
-                // this chunk's 64 biases live 2 per lane (fetched one chunk ahead: with ~225 KB of shared memory the L1 is a few
-                // KB, so a bias load in the dependent chain costs an L2 round trip); the next chunk's are requested now
-                const float2 bcur = bnext;
-                {
-                    const int cn = c + 1 < NC ? c + 1 : 0;
-                    bnext = __ldg(reinterpret_cast<const float2 *>(p.b1 + cn * kHC + half * 64) + lane);
+                uint32_t v[32], pk[16];
+                tmem_ld32(t_lane + kC + uint32_t(b) * kHC + uint32_t(part * 32), v);
+#pragma unroll
+                for (int j = 0; j < 32; j += 2) {                         // half biases from the constant bank: warp-uniform address
+                    const float *hb = p.hb1v + c * kHC + part * 32 + j;
+                    pk[j / 2] = gelu_bias2_pk(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), hb[0], hb[1]);
                 }
-                const uint32_t hs_row = base + kOffHs + uint32_t(2 * b + half) * kSlab + uint32_t(r) * 128u;
-                // both 32-column loads are in flight before the single wait: a TMEM load costs ~400 cycles while the tensor
-                // core is accumulating, and it sits on the GEMM1 -> GELU -> GEMM2 critical chain
-                uint32_t vv[2][32], hid[32];
-                tmem_ld32_nowait(t_lane + kC + uint32_t(b) * kHC + uint32_t(half * 64), vv[0]);
-                tmem_ld32_nowait(t_lane + kC + uint32_t(b) * kHC + uint32_t(half * 64 + 32), vv[1]);
-                tmem_ld_wait();
+                // the 32 hidden columns of this warp go, packed, over the first 16 of the 32 fp32 columns it has just read (no other
+                // warp touches those): hidden column h of the chunk = packed column 32 (h / 32) + (h % 32) / 2 of Hacc[b]
+                tmem_st16(t_lane + kC + uint32_t(b) * kHC + uint32_t(part * 32), pk);
+                tmem_st_wait();
                 tc_fence_before();
-                __syncwarp();
-                if (!TMH && lane == 0) mbar_arrive_cluster(hacc_empty_l + 8u * b);
-#pragma unroll
-                for (int q = 0; q < 2; ++q) {
-                    uint32_t (&v)[32] = vv[q];
-                    uint32_t pk[16];
-#pragma unroll
-                    for (int j = 0; j < 32; j += 2) {                     // columns q*32 + j, j+1 <- lane (q*32 + j) / 2
-                        const float bx = __shfl_sync(0xFFFFFFFFu, bcur.x, q * 16 + j / 2);
-                        const float by = __shfl_sync(0xFFFFFFFFu, bcur.y, q * 16 + j / 2);
-                        float f0, f1;
-                        gelu_bias2(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), bx, by, f0, f1);
-                        pk[j / 2] = pack_bf16x2(f0, f1);
-                    }
-                    if (TMH) {
-#pragma unroll
-                        for (int jj = 0; jj < 16; ++jj) hid[q * 16 + jj] = pk[jj];
-                    } else {
-#pragma unroll
-                        for (int jj = 0; jj < 4; ++jj) {
-                            const uint32_t chunk = uint32_t(q * 4 + jj) ^ uint32_t(r & 7);
-                            st_shared_v4(hs_row + (chunk << 4), pk[4 * jj], pk[4 * jj + 1], pk[4 * jj + 2], pk[4 * jj + 3]);
-                        }
-                    }
-                }
-                if (TMH) {      // this warp read fp32 columns [64 half, 64 half + 64) of Hacc[b]; its 64 bf16 go over the first 32 of them
-                    tmem_st32(t_lane + kC + uint32_t(b) * kHC + uint32_t(half * 64), hid);
-                    tmem_st_wait();
-                }
-                tc_fence_before();
-                if (!TMH) fence_proxy_async();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(hs_full_l + 8u * b);
             }
             const long long row = (long long)tile * kTM + r;
             const bool inb = row < p.n_px;
-            uint4 res[16];
+            // residual row segment (64 columns = 4 x 32 B), fetched BEFORE the wait for the last GEMM2s.  A thread is a pixel row
+            // (TMEM lane), so every lane touches its own 32-byte sector: 256-bit accesses halve the L1 wavefronts of this drain,
+            // which -- with the bias shuffles it used to have -- kept the epilogue warps busy for ~7.7 k of a tile's 16.4 k
+            // tensor cycles (measured with clock64 around the phases) while the next tile's first GELUs waited for them.
+            uint32_t res[4][8];
             {
-                const uint4 *rs = reinterpret_cast<const uint4 *>(p.x + row * kC + half * 128);
+                const bf16 *rs = p.x + row * kC + part * 64;
 #pragma unroll
-                for (int g = 0; g < 16; ++g) res[g] = inb ? rs[g] : make_uint4(0, 0, 0, 0);
+                for (int g = 0; g < 4; ++g) {
+                    if (inb) ld_global_256(rs + 16 * g, res[g]);
+                    else {
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) res[g][e] = 0u;
+                    }
+                }
             }
             mbar_wait(bar(B_OFULL), it & 1);
             tc_fence_after();
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                uint32_t v[32];
-                const int c0 = half * 128 + q * 32;
-                tmem_ld32(t_lane + uint32_t(c0), v);
-                uint4 *dst = reinterpret_cast<uint4 *>(p.out + row * kC + c0);
-#pragma unroll
-                for (int g = 0; g < 4; ++g) {
-                    const __nv_bfloat162 *re = reinterpret_cast<const __nv_bfloat162 *>(&res[q * 4 + g]);
-                    float bs[8];
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) bs[e] = __shfl_sync(0xFFFFFFFFu, b2r[q], g * 8 + e);
-                    uint4 o4;
-                    uint32_t *oe = reinterpret_cast<uint32_t *>(&o4);
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        const float2 xr = __bfloat1622float2(re[e]);
-                        oe[e] = pack_bf16x2(__uint_as_float(v[g * 8 + 2 * e]) + bs[2 * e] + xr.x,
-                                            __uint_as_float(v[g * 8 + 2 * e + 1]) + bs[2 * e + 1] + xr.y);
-                    }
-                    if (inb) dst[g] = o4;                                 // (shuffles above need every lane)
-                }
-            }
+            // Oacc is single-buffered: the next tile's first GEMM2 waits until it is drained.  Both 32-column loads of this
+            // warp are issued together and the accumulator is RELEASED as soon as they have landed in registers; the adds,
+            // the packing and the stores follow.
+            uint32_t va[32], vb[32];
+            tmem_ld32_nowait(t_lane + uint32_t(part * 64), va);
+            tmem_ld32_nowait(t_lane + uint32_t(part * 64 + 32), vb);
+            tmem_ld_wait();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(oempty_l);
+            if (lane == 0) mbar_arrive_cluster(oempty_l);                 // Oacc is in registers: the next tile may accumulate
+            auto emit = [&](const uint32_t (&vq)[32], int q) {
+                const int c0 = part * 64 + q * 32;
+                bf16 *dst = p.out + row * kC + c0;
+#pragma unroll
+                for (int g = 0; g < 2; ++g) {                             // 16 columns = one 32-byte sector
+                    uint32_t o8[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const uint32_t xr = res[q * 2 + g][e];            // bf16 pair -> fp32: low half << 16, high half masked
+                        const float *bc = p.b2v + c0 + g * 16 + 2 * e;    // (warp-uniform address, constant bank)
+                        o8[e] = pack_bf16x2(__uint_as_float(vq[g * 16 + 2 * e]) + bc[0] + __uint_as_float(xr << 16),
+                                            __uint_as_float(vq[g * 16 + 2 * e + 1]) + bc[1] + __uint_as_float(xr & 0xFFFF0000u));
+                    }
+                    if (inb) st_global_256(dst + 16 * g, o8);
+                }
+            };
+            emit(va, 0);
+            emit(vb, 1);
+            __syncwarp();
             // tail filling: the depthwise kernel of the next trunk block polls these counters instead of waiting for the whole
             // grid (the __syncwarp above orders every lane's stores before lane 0's release)
             if (p.tile_done && lane == 0) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p.tile_done + tile) : "memory");
@@ -606,7 +618,7 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
 // ---------------------------------------------------------------- host side ----------------------------------
 bool trunk_fusable(const ConvLayer &pw1, const ConvLayer &pw2)
 {
-    return pw1.c_in == kC && pw2.n == kC && pw2.n_pad == kC && pw1.n == pw2.c_in && pw1.n_pad == pw1.n && pw1.n % kHC == 0 &&
+    return pw1.c_in == kC && pw2.n == kC && pw2.n_pad == kC && pw1.n == pw2.c_in && pw1.n_pad == pw1.n && pw1.n % kHC == 0 && pw1.n <= kMaxHidden &&
            pw1.taps == 1 && pw2.taps == 1 && pw1.groups == 1 && pw2.groups == 1;
 }
 
@@ -644,11 +656,17 @@ cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const Con
     p.n_tiles = int((n_px + kTM - 1) / kTM);
     p.n_chunks = pw1.n / kHC;
     p.b1 = pw1.bias; p.b2 = pw2.bias;
+    if (pw1.bias_host.size() >= size_t(pw1.n) && pw2.bias_host.size() >= size_t(kC) && pw1.n <= kMaxHidden) {
+        for (int i = 0; i < pw1.n; ++i) p.hb1v[i] = 0.5f * pw1.bias_host[i];
+        std::copy(pw2.bias_host.begin(), pw2.bias_host.begin() + kC, p.b2v);
+    } else if (pair) {
+        return cudaErrorInvalidValue;
+    }
     p.x = x; p.out = out;
     if (pair && p.n_tiles >= 2) {
         const int n_ptiles = (p.n_tiles + 1) / 2;
         const int clusters = n_ptiles < num_sms / 2 ? n_ptiles : num_sms / 2;
-        return launch_pdl(trunk_mlp_pair_kernel, 2 * clusters, kTrunkThreads, kTrunkSmem, st, 2, m.tm_d, m.tm_w1h, m.tm_w2h, p);
+        return launch_pdl(trunk_mlp_pair_kernel, 2 * clusters, kPairThreads, kTrunkSmem, st, 2, m.tm_d, m.tm_w1h, m.tm_w2h, p);
     }
     const int grid = p.n_tiles < num_sms ? p.n_tiles : num_sms;
     return launch_pdl(trunk_mlp_kernel, grid, kTrunkThreads, kTrunkSmem, st, 1, m.tm_d, m.tm_w1, m.tm_w2, p);

@@ -67,6 +67,7 @@ struct ConvLayer {
     int c_in = 0, n = 0, n_pad = 0, taps = 1, groups = 1;
     bf16 *w = nullptr;
     float *bias = nullptr;
+    std::vector<float> bias_host;   // host copy of bias (group 0 .. groups-1, n_pad each): kernels that take biases by value
     bool use_tc = false;     // tcgen05 path eligible (c_in % 64 == 0, n_pad % 16 == 0)
     CUtensorMap tmap_w;      // 3-D {c_in, n_pad, groups*taps}, box {64, block_n, 1}, 128B swizzle
     CUtensorMap tmap_w_half; // same tensor, box {64, block_n / 2, 1}: one CTA's half of a weight tile (CTA-pair kernel)
@@ -247,9 +248,9 @@ struct TrunkMaps {
 bool trunk_make_maps(TrunkMaps &m, const bf16 *d_base, long long n_px, const ConvLayer &pw1, const ConvLayer &pw2, std::string &err);
 cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const ConvLayer &pw2, const bf16 *x, bf16 *out, long long n_px,
                              int num_sms, bool pair, LaunchStream st, uint32_t *tile_done = nullptr);
-// the CTA-pair trunk kernel adds 1 to tile_done[tile] per epilogue warp of the CTA that owns the 128-pixel tile: a tile is
+// the CTA-pair trunk kernel adds 1 to tile_done[tile] per epilogue warp (16) of the CTA that owns the 128-pixel tile: a tile is
 // complete (written, and its input rows no longer read) when its counter reaches kTrunkTileSignals
-constexpr uint32_t kTrunkTileSignals = 8;
+constexpr uint32_t kTrunkTileSignals = 16;
 // true if launch_trunk_mlp(..., pair, ...) runs the CTA-pair kernel, the one that counts finished tiles in tile_done
 bool trunk_counts_tiles(long long n_px, bool pair);
 

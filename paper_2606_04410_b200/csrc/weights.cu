@@ -81,6 +81,7 @@ struct Loader {
         }
         L.w = reinterpret_cast<bf16 *>(upload(w));
         L.bias = upload(b);
+        L.bias_host = b;
         return L.w && L.bias;
     }
 
