@@ -77,6 +77,9 @@ typedef struct ufnvc_config {
                                   * 79-81, 125, 356; R23) with that many DC blocks in the cross-chunk context generation
                                   * (11 / 12 / 9 for the paper's HT-S / HT-L / LD): the handle carries the state C_i from call to
                                   * call (ufnvc_reset_context starts a new video).  Needs c_trunk == 256 and the ctx.* tensors. */
+    int32_t n_enc_blocks;        /* 0: decoder only.  > 0: the handle also carries the chunk ENCODER (DESIGN.md
+                                  * R24) with that many DC blocks (6 / 7 / 3 for the paper's HT-S / HT-L / LD) and ufnvc_chunk_encode
+                                  * works.  Needs c_trunk == 256, mu_steps == 1 and the enc.* / henc.* tensors. */
 } ufnvc_config;
 
 /* ufnvc_config.debug_flags: A/B and cross-check switches (tests/test_gpu_parity.py runs every one against the oracle) */
@@ -118,7 +121,10 @@ int ufnvc_destroy(ufnvc_handle *h);
  * trunk.{k}.{dw,pw1,pw2}.{w,b}, dec.{t}.{s}.{w,b} (t < T, s < 4); with n_ctx_blocks > 0 xframe.w is
  * [T c_trunk][c_y + c_trunk][1][1] (input = [y ; C_i]) and ctx.fold.{w,b} [c_trunk][T c_trunk][1][1],
  * ctx.{k}.{dw,pw1,pw2}.{w,b} (k < n_ctx_blocks, shapes of a trunk block), ctx.out.{w,b} [c_trunk][c_trunk][1][1],
- * ctx.prior.{w,b} [c_hyper][c_trunk][1][1] are required (R23); with mu_steps == 4 mu.{1,2,3}.{w,b}
+ * ctx.prior.{w,b} [c_hyper][c_trunk][1][1] are required (R23); with n_enc_blocks > 0 enc.patch.{w,b} [c_trunk][192][1][1],
+ * enc.fold.{w,b} [c_trunk][T 4 c_trunk][1][1], enc.{k}.{dw,pw1,pw2}.{w,b} (k < n_enc_blocks), enc.y.{w,b} [c_y][c_trunk][1][1],
+ * henc.0.{w,b} [c_hyper][16 c_y][1][1], henc.1.{w,b} [c_z][c_hyper][3][3] and, with a context, enc.ctx.{w,b}
+ * [c_trunk][c_trunk][1][1] (R24); with mu_steps == 4 mu.{1,2,3}.{w,b}
  * ([c_y][2 c_y][3][3]: input channels [0, c_y) = y decoded so far, [c_y, 2 c_y) = the head's mean); optional
  * zprior.lnscale (fp32 [c_z], see the bytes-only entry points).
  * Missing / mis-shaped tensor: UFNVC_E_BAD_BLOB. */
@@ -226,6 +232,34 @@ long ufnvc_encode_chunk(const ufnvc_handle *h, const uint8_t *idx_host, const in
  * the first call allocates scratch. */
 int ufnvc_encode_chunk_dev(ufnvc_handle *h, int n_chunks, const uint8_t *idx_dev, const int16_t *sym_dev, uint8_t *bits_dev,
                            size_t cap, uint32_t *sub_off_dev, void *cuda_stream);
+
+/* ---- chunk ENCODE (R24; only with n_enc_blocks > 0, else UFNVC_E_BAD_CONFIG).  PAPER.md:79:
+ * the chunk is patch-embedded to 1/8 resolution, conditioned on C_i and distilled by the chunk encoder into one latent y;
+ * r = round(y - mu) is coded with sigma, mu and sigma coming from the DECODER's prior net run on the
+ * hyper-latent.  One call, everything on cuda_stream:
+ *   frames_dev   float [n_chunks][T][3][height][width] in [0,1]                       (input)
+ *   bits_dev     the rANS bit-stream ufnvc_chunk_decode takes, capacity cap bytes     (output, 4-byte aligned)
+ *   sub_off_dev  uint32 [n_chunks * n_sub + 1]                                        (output)
+ *   z_dev        int16 [n_chunks][c_z][h_z][w_z], the hyper-latent                    (output; what ufnvc_chunk_decode takes)
+ *   taps         optional intermediates for parity (any pointer may be NULL)
+ * Status bits as for ufnvc_encode_chunk_dev.  With a temporal context the call reads the handle's state C_i and leaves it alone:
+ * decoding the produced bytes (as an encoder does to stay in step with its decoder) advances it. */
+typedef struct ufnvc_enc_taps {
+    uint32_t struct_size;
+    float *y;      /* [n][h][w][c_y]      unquantised latent (E5) */
+    float *zf;     /* [n][c_z][h_z][w_z]  hyper-encoder output before rounding (E6) */
+    int16_t *sym;  /* [n][h][w][c_y]      r = round(y - mu) */
+    float *mu;     /* [n][h][w][c_y]      the prior net's mean for the coded z */
+    uint8_t *idx;  /* [n][h][w][c_y]      its scale bucket */
+} ufnvc_enc_taps;
+int ufnvc_chunk_encode(ufnvc_handle *h, int n_chunks, const float *frames_dev, uint8_t *bits_dev, size_t cap, uint32_t *sub_off_dev,
+                       int16_t *z_dev, const ufnvc_enc_taps *taps, void *cuda_stream);
+
+/* Colour interface (PAPER.md:384 Supp. C: "a unified YUV444 colorspace that serves as a universal interface"; BT.709 for the RGB
+ * tests): full-range BT.709 on [0,1] floats, planar [n_img][3][height][width] in and out (in_dev == out_dev allowed).
+ * to_yuv != 0: RGB -> YUV444, else YUV444 -> RGB.  Not part of ufnvc_chunk_decode / _encode: the codec's tensors are whatever
+ * three-plane signal the caller feeds it. */
+int ufnvc_convert_colour(const float *in_dev, float *out_dev, int n_img, int height, int width, int to_yuv, void *cuda_stream);
 
 /* Bucket index of every channel's z prior, uint8 [c_z] (R22). */
 int ufnvc_get_z_prior_index(const ufnvc_handle *h, uint8_t *idx_host);

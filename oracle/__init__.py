@@ -435,3 +435,97 @@ def make_stream(orc: Oracle, cfg, weights, z, u16_hwc, idx_override=None, ctx=No
     sym = orc.symbols_from_uniform(cdf, idx, np.transpose(u16_hwc, (2, 0, 1)))
     bits, sub_off = encode_chunk(orc, cfg, cdf, idx, sym)
     return dict(mu=mu, u=u, idx=idx, sym=sym, bits=bits, sub_off=sub_off, cdf=cdf)
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-4: chunk ENCODE, reading R24, and the colour interface of Supp. C.
+# ---------------------------------------------------------------------------------------------
+def rgb_to_yuv444(rgb):
+    """PAPER.md:384 (Supp. C): "a unified YUV444 colorspace that serves as a universal interface ... For both YUV420 and RGB
+    videos, they will be converted into YUV444"; the RGB tests use BT.709.  Full-range BT.709 on [0,1] floats:
+    Y = 0.2126 R + 0.7152 G + 0.0722 B, Cb = (B - Y) / 1.8556 + 1/2, Cr = (R - Y) / 1.5748 + 1/2.  rgb [..., 3, H, W]."""
+    rgb = np.asarray(rgb, np.float64)
+    r, g, b = rgb[..., 0, :, :], rgb[..., 1, :, :], rgb[..., 2, :, :]
+    y = 0.2126 * r + 0.7152 * g + 0.0722 * b
+    return np.stack([y, (b - y) / 1.8556 + 0.5, (r - y) / 1.5748 + 0.5], axis=-3)
+
+
+def yuv444_to_rgb(yuv):
+    """Inverse of rgb_to_yuv444: R = Y + 1.5748 (Cr - 1/2), B = Y + 1.8556 (Cb - 1/2), G = (Y - 0.2126 R - 0.0722 B) / 0.7152."""
+    yuv = np.asarray(yuv, np.float64)
+    y, cb, cr = yuv[..., 0, :, :], yuv[..., 1, :, :] - 0.5, yuv[..., 2, :, :] - 0.5
+    r = y + 1.5748 * cr
+    b = y + 1.8556 * cb
+    g = (y - 0.2126 * r - 0.0722 * b) / 0.7152
+    return np.stack([r, g, b], axis=-3)
+
+
+def space_to_depth(x, r):
+    """[C][H r][W r] -> [r r C][H][W] with channel (r i + j) C + c = x[c, r y + i, r x + j] (the inverse of a pixel shuffle,
+    position-major: all channels of sub-position (i, j) are contiguous)."""
+    c, hh, ww = x.shape
+    assert hh % r == 0 and ww % r == 0
+    h, w = hh // r, ww // r
+    return np.ascontiguousarray(x.reshape(c, h, r, w, r).transpose(2, 4, 0, 1, 3).reshape(r * r * c, h, w))
+
+
+def encoder_features(orc: Oracle, cfg, weights, frames, ctx=None):
+    """R24, E1..E5 ("transforming it to 1/8 resolution via patch embedding ... conditioned on the temporal chunk
+    context C_i, and fed into a chunk encoder ... distill the spatial-temporal information of the entire chunk into a compact
+    latent representation y_i"; the chunk encoder is a stack of DC blocks).  The layer plan is the mirror of the
+    decode configs: E1 patch embedding = space-to-depth x8 of every frame (zero-padded to the codec's H x W) + 1x1 conv
+    192 -> C_t, weights shared over t; E2 = space-to-depth x2 (to the latent's 1/16 resolution) and a 1x1 fold over the T
+    frames (T 4 C_t -> C_t); E3 = + 1x1 conv of the context C_i (when the config has one); E4 = B_e DC blocks (O7's block);
+    E5 = 1x1 conv C_t -> C_y.  frames [T][3][height][width] in [0,1].  Returns y [C_y][h][w] (unquantised)."""
+    g = geometry(cfg)
+    x = np.zeros((cfg.T, 3, g["H"], g["W"]), orc.dt)
+    x[:, :, :cfg.height, :cfg.width] = frames
+    s2 = []
+    for t in range(cfg.T):
+        p8 = space_to_depth(x[t], 8)                                            # [192][H/8][W/8], channel (8 i + j) 3 + c
+        f1 = orc.conv2d(p8, weights["enc.patch.w"], weights["enc.patch.b"])     # E1
+        s2.append(space_to_depth(f1, 2))                                        # [4 C_t][h][w]
+    feat = orc.conv2d(np.concatenate(s2, axis=0), weights["enc.fold.w"], weights["enc.fold.b"])      # E2
+    if has_context(cfg):
+        feat = feat + orc.conv2d(orc.arr(zero_context(cfg) if ctx is None else ctx), weights["enc.ctx.w"], weights["enc.ctx.b"])   # E3
+    for k in range(cfg.n_enc_blocks):                                           # E4
+        d = orc.dwconv3x3(feat, weights[f"enc.{k}.dw.w"], weights[f"enc.{k}.dw.b"])
+        e = orc.gelu(orc.conv2d(d, weights[f"enc.{k}.pw1.w"], weights[f"enc.{k}.pw1.b"]))
+        feat = feat + orc.conv2d(e, weights[f"enc.{k}.pw2.w"], weights[f"enc.{k}.pw2.b"])
+    return orc.conv2d(feat, weights["enc.y.w"], weights["enc.y.b"])             # E5
+
+
+def hyper_encoder(orc: Oracle, cfg, weights, y):
+    """R24, E6: the hyper-latent.  y zero-padded to [4 h_z][4 w_z], space-to-depth x4 -> [16 C_y][h_z][w_z]; ReLU(1x1 conv
+    16 C_y -> C_h); 3x3 conv C_h -> C_z; z = clip(rint(.), -127, 127) (the coder's alphabet, R7).  Returns (z int16, zf)."""
+    g = geometry(cfg)
+    yp = np.zeros((cfg.c_y, 4 * g["h_z"], 4 * g["w_z"]), orc.dt)
+    yp[:, :g["h"], :g["w"]] = y
+    a = orc.relu(orc.conv2d(space_to_depth(yp, 4), weights["henc.0.w"], weights["henc.0.b"]))
+    zf = orc.conv2d(a, weights["henc.1.w"], weights["henc.1.b"])
+    return np.clip(np.rint(zf), -127, 127).astype(np.int16), zf
+
+
+def quantise(y, mu):
+    """"After quantization via r_i = round(y_i - mu_i), the result r_i is arithmetically encoded using scale
+    sigma_i".  Round half to even, in fp32 -- the precision both sides take this integer decision in -- clipped to the
+    coder's alphabet [-127, 127] (R7).  Returns int16."""
+    d = np.asarray(y, np.float32) - np.asarray(mu, np.float32)
+    return np.clip(np.rint(d), -127, 127).astype(np.int16)
+
+
+def chunk_encode(orc: Oracle, cfg, weights, frames, ctx=None, z_override=None, y_override=None):
+    """One chunk, frames -> bytes (R24): E1..E6, the decoder's own prior net on z, quantisation, the mirror
+    of O4.  Only the single-pass mean (mu_steps == 1).  z_override / y_override: teacher forcing for the parity tests (the
+    integer decisions z and r depend on floats that differ between implementations at rounding edges).
+    Returns dict(y, z, zf, mu, u, idx, sym, bits, sub_off)."""
+    assert getattr(cfg, "mu_steps", 1) == 1
+    y = encoder_features(orc, cfg, weights, frames, ctx=ctx) if y_override is None else orc.arr(y_override)
+    z, zf = hyper_encoder(orc, cfg, weights, y)
+    if z_override is not None:
+        z = np.asarray(z_override, np.int16)
+    mu, u, idx = entropy_params(orc, cfg, weights, z, ctx=ctx)
+    sym = quantise(y, mu)
+    cdf = orc.build_cdf(cfg.n_buckets, cfg.scale_min, cfg.scale_max)
+    bits, sub_off = encode_chunk(orc, cfg, cdf, idx, sym)
+    return dict(y=y, z=z, zf=zf, mu=mu, u=u, idx=idx, sym=sym, bits=bits, sub_off=sub_off)

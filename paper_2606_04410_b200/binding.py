@@ -27,13 +27,18 @@ class ufnvc_config(C.Structure):
                 ("n_buckets", C.c_int32), ("scale_min", C.c_double), ("scale_max", C.c_double),
                 ("rows_per_substream", C.c_int32), ("lanes_per_substream", C.c_int32),
                 ("max_chunks_per_call", C.c_int32), ("weight_dtype", C.c_int32), ("mu_steps", C.c_int32),
-                ("debug_flags", C.c_uint32), ("n_ctx_blocks", C.c_int32)]
+                ("debug_flags", C.c_uint32), ("n_ctx_blocks", C.c_int32), ("n_enc_blocks", C.c_int32)]
 
 
 class ufnvc_taps(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("mu", C.c_void_p), ("lnscale", C.c_void_p), ("idx", C.c_void_p),
                 ("sym", C.c_void_p), ("yhat", C.c_void_p), ("f0", C.c_void_p), ("trunk", C.c_void_p),
                 ("stage", C.c_void_p * 3)]
+
+
+class ufnvc_enc_taps(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("y", C.c_void_p), ("zf", C.c_void_p), ("sym", C.c_void_p), ("mu", C.c_void_p),
+                ("idx", C.c_void_p)]
 
 
 def _load():
@@ -62,6 +67,8 @@ def _load():
         "ufnvc_get_z_prior_index": (i, [vp, vp]),
         "ufnvc_encode_z": (C.c_long, [vp, vp, vp, sz, vp]),
         "ufnvc_encode_chunk_dev": (i, [vp, i, vp, vp, vp, sz, vp, vp]),
+        "ufnvc_chunk_encode": (i, [vp, i, vp, vp, sz, vp, vp, C.POINTER(ufnvc_enc_taps), vp]),
+        "ufnvc_convert_colour": (i, [vp, vp, i, i, i, i, vp]),
         "ufnvc_reset_context": (i, [vp, i, vp]),
         "ufnvc_get_context": (i, [vp, i, vp, vp]),
         "ufnvc_set_context": (i, [vp, i, vp, vp]),
@@ -77,7 +84,7 @@ EXPORTS = ("ufnvc_create", "ufnvc_destroy", "ufnvc_load_weights", "ufnvc_chunk_d
            "ufnvc_entropy_params", "ufnvc_get_status", "ufnvc_last_error", "ufnvc_launches_per_call",
            "ufnvc_chunk_decode_profiled", "ufnvc_debug_counter", "ufnvc_get_cdf", "ufnvc_symbols_from_uniform", "ufnvc_encode_chunk",
            "ufnvc_decode_z", "ufnvc_chunk_decode_bytes", "ufnvc_get_z_prior_index", "ufnvc_encode_z", "ufnvc_encode_chunk_dev",
-           "ufnvc_reset_context", "ufnvc_get_context", "ufnvc_set_context")
+           "ufnvc_reset_context", "ufnvc_get_context", "ufnvc_set_context", "ufnvc_chunk_encode", "ufnvc_convert_colour")
 
 
 # ufnvc_config.debug_flags (include/ufnvc.h)
@@ -97,6 +104,7 @@ def make_config(cfg, max_chunks: int | None = None, debug_flags: int = 0) -> ufn
     c.mu_steps = getattr(cfg, "mu_steps", 1)
     c.debug_flags = debug_flags
     c.n_ctx_blocks = getattr(cfg, "n_ctx_blocks", 0)
+    c.n_enc_blocks = getattr(cfg, "n_enc_blocks", 0)
     return c
 
 
@@ -224,6 +232,29 @@ class ChunkDecoder:
         out["frames"] = frames
         return out
 
+    # ---- chunk encode (NEXT-4, R24) ----
+    def chunk_encode(self, frames, cap=None, taps=False, stream=None):
+        """frames: float32 device tensor [n][T][3][height][width] -> dict(bits uint8 [cap], sub_off int32, z int16, + taps)."""
+        n, cfg, dev = frames.shape[0], self.cfg, self.device
+        G = cfg.lanes_per_substream // 32
+        ne = self.h * self.w * cfg.c_y
+        cap = cap if cap is not None else n * (2 * ne + self.n_sub * (G * 140 + 16) + 64)
+        out = dict(bits=torch.zeros(cap, dtype=torch.uint8, device=dev), sub_off=torch.zeros(n * self.n_sub + 1, dtype=torch.int32, device=dev),
+                   z=torch.empty((n, cfg.c_z, self.h_z, self.w_z), dtype=torch.int16, device=dev))
+        tp = None
+        if taps:
+            e = (n, self.h, self.w, cfg.c_y)
+            out.update(y=torch.empty(e, dtype=torch.float32, device=dev), zf=torch.empty((n, cfg.c_z, self.h_z, self.w_z), dtype=torch.float32, device=dev),
+                       sym=torch.empty(e, dtype=torch.int16, device=dev), mu=torch.empty(e, dtype=torch.float32, device=dev),
+                       idx=torch.empty(e, dtype=torch.uint8, device=dev))
+            tp = ufnvc_enc_taps()
+            tp.struct_size = C.sizeof(ufnvc_enc_taps)
+            for k in ("y", "zf", "sym", "mu", "idx"):
+                setattr(tp, k, out[k].data_ptr())
+        self._check(LIB.ufnvc_chunk_encode(self.handle, n, _ptr(frames), _ptr(out["bits"]), cap, _ptr(out["sub_off"]), _ptr(out["z"]),
+                                           C.byref(tp) if tp is not None else None, self._stream(stream)), "ufnvc_chunk_encode")
+        return out
+
     # ---- temporal chunk context (NEXT-2a, DESIGN.md R23) ----
     def reset_context(self, n_chunks=1, stream=None):
         self._check(LIB.ufnvc_reset_context(self.handle, n_chunks, self._stream(stream)), "ufnvc_reset_context")
@@ -329,6 +360,18 @@ class ChunkDecoder:
         off = np.zeros(self.n_sub + 1, np.uint32)
         n = self._check(LIB.ufnvc_encode_chunk(self.handle, _ptr(idx), _ptr(sym), _ptr(bits), cap, _ptr(off)), "ufnvc_encode_chunk")
         return bits[:n].copy(), off
+
+
+def convert_colour(x, to_yuv: bool, stream=None):
+    """BT.709 full-range RGB <-> YUV444 on a float32 device tensor [..., 3, H, W] (ufnvc_convert_colour); returns a new tensor."""
+    assert x.dtype == torch.float32 and x.is_cuda and x.shape[-3] == 3 and x.is_contiguous()
+    out = torch.empty_like(x)
+    n_img = x.numel() // (3 * x.shape[-2] * x.shape[-1])
+    s = stream if stream is not None else torch.cuda.current_stream()
+    rc = LIB.ufnvc_convert_colour(_ptr(x), _ptr(out), n_img, x.shape[-2], x.shape[-1], int(to_yuv), C.c_void_p(s.cuda_stream))
+    if rc != 0:
+        raise UfnvcError(f"ufnvc_convert_colour failed ({rc})")
+    return out
 
 
 def pack_chunk_bytes(z_bits, z_off, y_bits, y_off):

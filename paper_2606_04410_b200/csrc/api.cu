@@ -57,6 +57,12 @@ int validate(const ufnvc_config &c, std::string &why)
         "a temporal context needs c_trunk == 256, c_y % 64 == 0, bf16 weights (the context generation runs on the fused tensor-core kernels)");
     BAD(c.n_ctx_blocks > 0 && (c.debug_flags & (UFNVC_DBG_FORCE_GENERIC | UFNVC_DBG_UNFUSED_TRUNK | UFNVC_DBG_PLAIN_DEPTHWISE)),
         "the context generation has no CUDA-core / unfused / plain-depthwise variant");
+    BAD(c.n_enc_blocks < 0 || c.n_enc_blocks > 64, "n_enc_blocks out of range");
+    BAD(c.n_enc_blocks > 0 && (c.c_trunk != 256 || (c.c_trunk * c.trunk_expand) % 128 || c.c_y % 32 || c.weight_dtype != 1 || c.mu_steps != 1 ||
+                               c.c_y > 400),
+        "the encoder needs c_trunk == 256, c_y % 32 == 0 (<= 400), bf16 weights and mu_steps == 1");
+    BAD(c.n_enc_blocks > 0 && (c.debug_flags & (UFNVC_DBG_FORCE_GENERIC | UFNVC_DBG_UNFUSED_TRUNK | UFNVC_DBG_PLAIN_DEPTHWISE)),
+        "the encoder has no CUDA-core / unfused / plain-depthwise variant");
     BAD(c.mu_steps == 4 && (c.debug_flags & UFNVC_DBG_FORCE_GENERIC), "mu_steps == 4 has no CUDA-core variant");
     // every kernel indexes latent elements and activation pixels with 32-bit integers (byte offsets are 64-bit)
     {
@@ -97,6 +103,7 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     h->n_sub_z = (h->h_z + cfg->rows_per_substream - 1) / cfg->rows_per_substream;
     h->max_chunks = cfg->max_chunks_per_call;
     h->has_ctx = cfg->n_ctx_blocks > 0;
+    h->has_enc = cfg->n_enc_blocks > 0;
     h->c_cat = cfg->c_y + (h->has_ctx ? cfg->c_trunk : 0);
     const uint32_t dbg = cfg->debug_flags;
     h->force_generic = dbg & UFNVC_DBG_FORCE_GENERIC;
@@ -137,10 +144,10 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
               dev_alloc(h, h->lnscale, n * P * cfg->c_y) && dev_alloc(h, h->idx, n * P * cfg->c_y) &&
               dev_alloc(h, h->yhat, n * P * size_t(h->c_cat)) && dev_alloc(h, h->fa, n * T * P * cfg->c_trunk) &&
               dev_alloc(h, h->fb, n * T * P * cfg->c_trunk) &&
-              dev_alloc(h, h->zero_block, 4 + size_t(cfg->n_trunk_blocks + cfg->n_ctx_blocks + 1) * ((n * T * P + 127) / 128 + 4)) &&
+              dev_alloc(h, h->zero_block, 4 + size_t(cfg->n_trunk_blocks + std::max(cfg->n_ctx_blocks, cfg->n_enc_blocks) + 1) * ((n * T * P + 127) / 128 + 4)) &&
               dev_alloc(h, h->hidden, cfg->n_trunk_blocks ? n * T * P * cfg->c_trunk * cfg->trunk_expand : 1);
     if (ok) {      // everything a call clears up front sits in one block so that ONE memset node does it (decode.cu run())
-        h->zero_words = 4 + size_t(cfg->n_trunk_blocks + cfg->n_ctx_blocks + 1) * ((n * T * P + 127) / 128 + 4);
+        h->zero_words = 4 + size_t(cfg->n_trunk_blocks + std::max(cfg->n_ctx_blocks, cfg->n_enc_blocks) + 1) * ((n * T * P + 127) / 128 + 4);
         h->d_status = h->zero_block; h->fix_count = h->zero_block + 1; h->trunk_sync = h->zero_block + 4;
         ok = cudaMemset(h->zero_block, 0, h->zero_words * 4) == cudaSuccess;
     }
@@ -152,9 +159,13 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     ok = ok && dev_alloc(h, h->z_idx, n * Pz * cfg->c_z) && dev_alloc(h, h->z_zero_mu, n * Pz * cfg->c_z) &&
          dev_alloc(h, h->z_scratch, n * Pz * cfg->c_z) && dev_alloc(h, h->z_hwc, n * Pz * cfg->c_z) &&
          dev_alloc(h, h->z_planar, n * Pz * cfg->c_z) && cudaMemset(h->z_zero_mu, 0, n * Pz * cfg->c_z * 4) == cudaSuccess;
+    if (ok && (h->has_ctx || h->has_enc)) ok = dev_alloc(h, h->ca, n * P * cfg->c_trunk) && dev_alloc(h, h->cb, n * P * cfg->c_trunk);
     if (ok && h->has_ctx)
-        ok = dev_alloc(h, h->ca, n * P * cfg->c_trunk) && dev_alloc(h, h->cb, n * P * cfg->c_trunk) && dev_alloc(h, h->ctx_q, n * Pz * cfg->c_hyper) &&
+        ok = dev_alloc(h, h->ctx_q, n * Pz * cfg->c_hyper) &&
              cudaMemset(h->yhat, 0, n * P * size_t(h->c_cat) * 2) == cudaSuccess && cudaMemset(h->ctx_q, 0, n * Pz * cfg->c_hyper * 8) == cudaSuccess;
+    if (ok && h->has_enc)
+        ok = dev_alloc(h, h->p8, n * T * (P * 4) * 192) && dev_alloc(h, h->s2, n * T * P * 4 * cfg->c_trunk) && dev_alloc(h, h->ey, n * P * cfg->c_y) &&
+             dev_alloc(h, h->henc_a, n * Pz * cfg->c_hyper) && dev_alloc(h, h->esym, n * P * cfg->c_y) && dev_alloc(h, h->ez, n * Pz * cfg->c_z);
     for (int s = 0; ok && s < 3; ++s) ok = dev_alloc(h, h->stage[s], n * T * (P << (2 * (s + 1))) * cfg->dec_channels[s + 1]);
     if (ok) ok = cudaMemcpy(h->d_cf, cf.data(), cf.size() * 4, cudaMemcpyHostToDevice) == cudaSuccess &&
                  cudaMemcpy(h->d_lut, lut.data(), lut.size() * 4, cudaMemcpyHostToDevice) == cudaSuccess &&
@@ -223,6 +234,13 @@ extern "C" int ufnvc_symbols_from_uniform(const ufnvc_handle *h, const uint8_t *
         sym_host[i] = int16_t(lo - 127);
     }
     return UFNVC_OK;
+}
+
+extern "C" int ufnvc_convert_colour(const float *in_dev, float *out_dev, int n_img, int height, int width, int to_yuv, void *cuda_stream)
+{
+    if (!in_dev || !out_dev || n_img < 1 || height < 1 || width < 1) return UFNVC_E_INVALID_ARG;
+    return launch_colour(in_dev, out_dev, (long long)height * width, n_img, to_yuv != 0, static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess
+               ? UFNVC_OK : UFNVC_E_CUDA;
 }
 
 extern "C" int ufnvc_get_z_prior_index(const ufnvc_handle *h, uint8_t *idx_host)

@@ -327,6 +327,12 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
                         dst += E.c_y;
                     }
                 }
+                if (MODE == EPI_NHWC && p.E.out_f32) {                   // fp32 output (the encoder's unquantised latent)
+                    float *df = reinterpret_cast<float *>(p.E.out) + o;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) st_global_256(df + 8 * q, f + 8 * q);
+                    continue;
+                }
                 if (MODE == EPI_NHWC && p.E.residual) {
                     const uint4 *rs = reinterpret_cast<const uint4 *>(p.E.residual + o);
 #pragma unroll
@@ -829,10 +835,11 @@ bool tc_make_weight_tmap(ConvLayer &L, std::string &err, int block_n)
 }
 
 bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, int tile_h, int tile_w, std::string &err,
-                      bool swizzle)
+                      bool swizzle, int pix_stride)
 {
+    const cuuint64_t ps = cuuint64_t(pix_stride > 0 ? pix_stride : C) * 2;      // bytes between pixels
     cuuint64_t dims[4] = {cuuint64_t(C), cuuint64_t(W), cuuint64_t(H), cuuint64_t(n_img)};
-    cuuint64_t strides[3] = {cuuint64_t(C) * 2, cuuint64_t(C) * 2 * W, cuuint64_t(C) * 2 * W * H};
+    cuuint64_t strides[3] = {ps, ps * W, ps * W * H};
     cuuint32_t box[4] = {cuuint32_t(kSlabK), cuuint32_t(tile_w), cuuint32_t(tile_h), 1};
     return encode(tm, base, 4, dims, strides, box, err, swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE);
 }

@@ -338,9 +338,32 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
     }
     for (auto &tb : h->trunk)
         if (ok && !trunk_make_maps(tb.fused, h->fb, (long long)n * T * h->h * h->w, tb.pw1, tb.pw2, h->err)) ok = false;
-    if (ok && h->has_ctx) {
+    if (ok && (h->has_ctx || h->has_enc))
         ok = make_act_map(h, h->am_ca, h->ca, n, h->h, h->w, c.c_trunk, false, 1) &&
              tc_make_act_tmap(&h->tm_dw_ctx, h->ca, n, h->h, h->w, c.c_trunk, 10, 10, h->err, /*swizzle=*/false);
+    if (ok && h->has_enc) {
+        // encoder (R24): patches [n T][H/8][W/8][192], embedded + space-to-depth x2 [n T][h][w][4 c_trunk]
+        ok = tc_make_weight_tmap(h->enc_patch, err) && tc_make_weight_tmap(h->enc_fold, err) && tc_make_weight_tmap(h->enc_y, err);
+        for (auto &tb : h->enc_blocks) ok = ok && tc_make_weight_tmap(tb.pw1, err) && tc_make_weight_tmap(tb.pw2, err);
+        if (!ok) return fail(h, UFNVC_E_CUDA, err);
+        ok = make_act_map(h, h->am_p8, h->p8, n * T, 2 * h->h, 2 * h->w, 192, false, T) &&
+             make_act_map(h, h->am_s2, h->s2, n * T, h->h, h->w, 4 * c.c_trunk, false, T);
+        for (auto &tb : h->enc_blocks)
+            if (ok && (!trunk_make_maps(tb.fused, h->cb, (long long)n * h->h * h->w, tb.pw1, tb.pw2, h->err) || !tb.fused.ok)) ok = false;
+        if (ok && h->has_ctx) {
+            // E3 reads the context block of the [y ; C] buffer in place: a tensor map with the buffer's pixel stride
+            ok = tc_make_weight_tmap(h->enc_ctx, err);
+            if (!ok) return fail(h, UFNVC_E_CUDA, err);
+            pick_tile(h->h, h->w, h->am_cin.tile_h, h->am_cin.tile_w);
+            h->am_cin.flat = false;
+            ok = tc_make_act_tmap(&h->am_cin.tm, h->yhat + c.c_y, n, h->h, h->w, c.c_trunk, h->am_cin.tile_h, h->am_cin.tile_w, h->err, true, h->c_cat);
+            h->am_cin.ok = ok;
+        }
+        if (ok && (!h->am_p8.ok || !h->am_s2.ok || !h->am_ca.ok || !h->enc_patch.use_tc || !h->enc_fold.use_tc || !h->enc_y.use_tc)) {
+            ok = false; h->err = "the encoder needs the tensor-core conv path";
+        }
+    }
+    if (ok && h->has_ctx) {
         for (auto &tb : h->ctx_blocks)
             if (ok && (!trunk_make_maps(tb.fused, h->cb, (long long)n * h->h * h->w, tb.pw1, tb.pw2, h->err) || !tb.fused.ok)) ok = false;
         if (ok && (!h->am_fa.ok || !h->ctx_fold.use_tc || !h->ctx_out.use_tc || !h->am_ca.ok)) { ok = false; h->err = "context generation needs the tensor-core conv path"; }
@@ -434,15 +457,13 @@ extern "C" int ufnvc_chunk_decode_bytes(ufnvc_handle *h, int n_chunks, const uin
 }
 
 // ---- NEXT-4 (part): GPU rANS encode of r, the mirror of A3 ---------------------------------------------------------
-extern "C" int ufnvc_encode_chunk_dev(ufnvc_handle *h, int n_chunks, const uint8_t *idx_dev, const int16_t *sym_dev, uint8_t *bits_dev,
-                                      size_t cap, uint32_t *sub_off_dev, void *cuda_stream)
+namespace {
+// idx + r on the device -> the bit-stream ufnvc_chunk_decode takes (rans_encode.cu); allocates its scratch on first use
+int encode_dev_impl(ufnvc_handle *h, int n_chunks, const uint8_t *idx_dev, const int16_t *sym_dev, uint8_t *bits_dev, size_t cap,
+                    uint32_t *sub_off_dev, cudaStream_t stream, bool clear_status)
 {
-    if (!h) return UFNVC_E_INVALID_ARG;
-    if (n_chunks < 1 || n_chunks > h->max_chunks) return fail(h, UFNVC_E_INVALID_ARG, "n_chunks outside [1, max_chunks_per_call]");
-    if (!idx_dev || !sym_dev || !bits_dev || !sub_off_dev) return fail(h, UFNVC_E_INVALID_ARG, "null device pointer");
-    if (reinterpret_cast<uintptr_t>(bits_dev) & 3) return fail(h, UFNVC_E_INVALID_ARG, "bits_dev must be 4-byte aligned");
     const ufnvc_config &c = h->cfg;
-    const LaunchStream st{static_cast<cudaStream_t>(cuda_stream), h->pdl};
+    const LaunchStream st{stream, h->pdl};
     const int G = c.lanes_per_substream / 32;
     if (!h->enc_tmp) {
         const size_t n_sym = size_t(c.rows_per_substream) * h->w * c.c_y;
@@ -460,7 +481,7 @@ extern "C" int ufnvc_encode_chunk_dev(ufnvc_handle *h, int n_chunks, const uint8
         h->allocs.push_back(a); h->allocs.push_back(b); h->allocs.push_back(d);
         h->enc_tmp = static_cast<uint16_t *>(a); h->enc_stage = static_cast<uint8_t *>(b); h->enc_sizes = static_cast<uint32_t *>(d);
     }
-    CU_TRY(cudaMemsetAsync(h->d_status, 0, 4, st));
+    if (clear_status) CU_TRY(cudaMemsetAsync(h->d_status, 0, 4, stream));
     RansEncParams p{};
     p.idx = idx_dev; p.sym = sym_dev; p.cf = h->d_cf;
     p.n_chunks = n_chunks; p.n_sub = h->n_sub; p.h = h->h; p.w = h->w; p.c_y = c.c_y;
@@ -468,8 +489,20 @@ extern "C" int ufnvc_encode_chunk_dev(ufnvc_handle *h, int n_chunks, const uint8
     p.tmp_words = h->enc_tmp; p.tmp_stride = h->enc_tmp_stride; p.stage = h->enc_stage; p.stage_stride = h->enc_stage_stride;
     p.sizes = h->enc_sizes; p.bits_out = bits_dev; p.cap = cap; p.sub_off = sub_off_dev; p.status = h->d_status;
     CU_TRY(launch_rans_encode(p, st));
-    h->last_launches = 2;
     return UFNVC_OK;
+}
+}  // namespace
+
+extern "C" int ufnvc_encode_chunk_dev(ufnvc_handle *h, int n_chunks, const uint8_t *idx_dev, const int16_t *sym_dev, uint8_t *bits_dev,
+                                      size_t cap, uint32_t *sub_off_dev, void *cuda_stream)
+{
+    if (!h) return UFNVC_E_INVALID_ARG;
+    if (n_chunks < 1 || n_chunks > h->max_chunks) return fail(h, UFNVC_E_INVALID_ARG, "n_chunks outside [1, max_chunks_per_call]");
+    if (!idx_dev || !sym_dev || !bits_dev || !sub_off_dev) return fail(h, UFNVC_E_INVALID_ARG, "null device pointer");
+    if (reinterpret_cast<uintptr_t>(bits_dev) & 3) return fail(h, UFNVC_E_INVALID_ARG, "bits_dev must be 4-byte aligned");
+    const int rc = encode_dev_impl(h, n_chunks, idx_dev, sym_dev, bits_dev, cap, sub_off_dev, static_cast<cudaStream_t>(cuda_stream), true);
+    h->last_launches = 2;
+    return rc;
 }
 
 extern "C" int ufnvc_entropy_params(ufnvc_handle *h, int n_chunks, const int16_t *z_dev, float *mu_dev, float *lnscale_dev,
@@ -585,4 +618,93 @@ extern "C" int ufnvc_set_context(ufnvc_handle *h, int n_chunks, const uint16_t *
     CU_TRY(cudaMemcpy2DAsync(h->yhat + c.c_y, size_t(h->c_cat) * 2, ctx_dev, size_t(c.c_trunk) * 2, size_t(c.c_trunk) * 2, rows,
                              cudaMemcpyDeviceToDevice, st));
     return ctx_refresh_prior(h, n_chunks, st);
+}
+
+// ---- NEXT-4 (R24): chunk ENCODE, frames -> bytes --------------------------------------------------------------------------
+// E1 patch gather + 1x1 embedding (space-to-depth x2 store) -> E2 fold over the T frames -> E3 + context -> E4 DC blocks ->
+// E5 latent head (fp32) -> E6 hyper-encoder (z) -> the decoder's prior net on z (A1 + A2) -> E8 quantiser -> GPU rANS encoder.
+extern "C" int ufnvc_chunk_encode(ufnvc_handle *h, int n_chunks, const float *frames_dev, uint8_t *bits_dev, size_t cap,
+                                  uint32_t *sub_off_dev, int16_t *z_dev, const ufnvc_enc_taps *taps, void *cuda_stream)
+{
+    if (!h) return UFNVC_E_INVALID_ARG;
+    if (!h->has_enc) return fail(h, UFNVC_E_BAD_CONFIG, "this handle has no encoder (n_enc_blocks == 0)");
+    if (!h->weights_loaded) return fail(h, UFNVC_E_NO_WEIGHTS, "ufnvc_load_weights has not succeeded on this handle");
+    if (n_chunks < 1 || n_chunks > h->max_chunks) return fail(h, UFNVC_E_INVALID_ARG, "n_chunks outside [1, max_chunks_per_call]");
+    if (!frames_dev || !bits_dev || !sub_off_dev || !z_dev) return fail(h, UFNVC_E_INVALID_ARG, "null device pointer");
+    if (reinterpret_cast<uintptr_t>(bits_dev) & 3) return fail(h, UFNVC_E_INVALID_ARG, "bits_dev must be 4-byte aligned");
+    if (taps && taps->struct_size != sizeof(ufnvc_enc_taps)) return fail(h, UFNVC_E_INVALID_ARG, "ufnvc_enc_taps.struct_size mismatch");
+    const ufnvc_config &c = h->cfg;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const LaunchStream st{stream, h->pdl};
+    const int n = n_chunks, T = c.T, Ct = c.c_trunk, P = h->h * h->w, Pz = h->h_z * h->w_z;
+    int launches = 0;
+    // one memset for the status word and the encoder blocks' tile counters (same block of words the decode call clears)
+    {
+        const size_t words = h->tail_fill ? 4 + size_t(c.n_trunk_blocks + c.n_enc_blocks) * h->trunk_sync_stride : 4;
+        CU_TRY(cudaMemsetAsync(h->zero_block, 0, words * 4, stream));
+    }
+    // E1: 8x8 patches of every frame, then the 1x1 embedding whose epilogue stores space-to-depth x2 (ready for the fold)
+    CU_TRY(launch_enc_patchify(frames_dev, h->p8, n * T, c.height, c.width, 2 * h->h, 2 * h->w, st));
+    ++launches;
+    {
+        ConvProblem pr{h->p8, n * T, 2 * h->h, 2 * h->w, 1};
+        EpiParams E{EPI_NHWC, ACT_NONE, h->s2, nullptr, Ct, 0, (long long)P * 4 * Ct, 0, 0, 0};
+        E.unps2 = 1;
+        CU_TRY(conv(h, h->enc_patch, pr, h->am_p8, E, st, &launches));
+    }
+    // E2: fold over the T frames (tap t = frame t of the chunk), 4 c_trunk channels each
+    {
+        ConvProblem pr{h->s2, n, h->h, h->w, 1, true};
+        EpiParams E{EPI_NHWC, ACT_NONE, h->ca, nullptr, Ct, 0, (long long)P * Ct, 0, 0, 0};
+        CU_TRY(conv(h, h->enc_fold, pr, h->am_s2, E, st, &launches));
+    }
+    // E3: + 1x1 conv of the temporal context C_i, read in place from the [y ; C] buffer
+    if (h->has_ctx) {
+        ConvProblem pr{h->yhat + c.c_y, n, h->h, h->w, 1};
+        EpiParams E{EPI_NHWC, ACT_NONE, h->ca, h->ca, Ct, 0, (long long)P * Ct, 0, 0, 0};
+        CU_TRY(conv(h, h->enc_ctx, pr, h->am_cin, E, st, &launches));
+    }
+    // E4: the chunk encoder's DC blocks, on the depthwise + fused MLP kernels of the trunk (one image per chunk)
+    for (int k = 0; k < c.n_enc_blocks; ++k) {
+        const ufnvc_handle::TrunkBlock &tb = h->enc_blocks[k];
+        uint32_t *sync_k = h->trunk_sync + size_t(c.n_trunk_blocks + k) * h->trunk_sync_stride;
+        const bool mlp_counts = trunk_counts_tiles((long long)n * P, h->use_pair_trunk) && h->tail_fill;
+        CU_TRY(launch_dwconv3x3_tma(h->tm_dw_ctx, h->cb, tb.dw_w, tb.dw_b, n, h->h, h->w, Ct, h->num_sms, st, h->tail_fill ? sync_k : nullptr,
+                                    (k > 0 && mlp_counts) ? sync_k - h->trunk_sync_stride + 1 : nullptr));
+        CU_TRY(launch_trunk_mlp(tb.fused, tb.pw1, tb.pw2, h->ca, h->ca, (long long)n * P, h->num_sms, h->use_pair_trunk, st,
+                                mlp_counts ? sync_k + 1 : nullptr));
+        launches += 2;
+    }
+    // E5: latent head, fp32 out
+    {
+        ConvProblem pr{h->ca, n, h->h, h->w, 1};
+        EpiParams E{EPI_NHWC, ACT_NONE, h->ey, nullptr, c.c_y, 0, (long long)P * c.c_y, 0, 0, 0};
+        E.out_f32 = 1;
+        CU_TRY(conv(h, h->enc_y, pr, h->am_ca, E, st, &launches));
+    }
+    // E6: hyper-encoder -> z (int16, planar: what A1 reads), then the decoder's own prior net on it
+    CU_TRY(launch_hyper_encoder(h->ey, h->henc_w0, h->henc_b0, h->henc_w1, h->henc_b1, h->henc_a, h->ez, taps ? taps->zf : nullptr, n, h->h, h->w,
+                                h->h_z, h->w_z, c.c_y, c.c_hyper, c.c_z, st));
+    launches += 2;
+    CU_TRY(cudaMemcpyAsync(z_dev, h->ez, size_t(n) * Pz * c.c_z * 2, cudaMemcpyDeviceToDevice, stream));
+    {
+        h->keep_status = true;                 // run() must not clear what this call's memset cleared (it would also re-clear counters)
+        const int rc = run(h, n, h->ez, nullptr, 0, nullptr, nullptr, stream, nullptr, nullptr, nullptr, true, nullptr, nullptr, nullptr, nullptr,
+                           &launches);
+        h->keep_status = false;
+        if (rc) return rc;
+    }
+    // E8: r = round(y - mu), then the mirror of A3
+    const size_t ne = size_t(n) * P * c.c_y;
+    CU_TRY(launch_enc_quantise(h->ey, h->mu, h->esym, (long long)ne, st));
+    ++launches;
+    if (taps) {
+        if (taps->y) CU_TRY(cudaMemcpyAsync(taps->y, h->ey, ne * 4, cudaMemcpyDeviceToDevice, stream));
+        if (taps->sym) CU_TRY(cudaMemcpyAsync(taps->sym, h->esym, ne * 2, cudaMemcpyDeviceToDevice, stream));
+        if (taps->mu) CU_TRY(cudaMemcpyAsync(taps->mu, h->mu, ne * 4, cudaMemcpyDeviceToDevice, stream));
+        if (taps->idx) CU_TRY(cudaMemcpyAsync(taps->idx, h->idx, ne, cudaMemcpyDeviceToDevice, stream));
+    }
+    if (int rc = encode_dev_impl(h, n, h->idx, h->esym, bits_dev, cap, sub_off_dev, stream, false)) return rc;
+    h->last_launches = launches + 2;
+    return UFNVC_OK;
 }

@@ -99,6 +99,8 @@ __device__ __forceinline__ void st_global_256(void *p, const uint32_t *u)
 __device__ __forceinline__ long long epi_offset(const EpiParams &E, int img, int y, int x, int H, int W, int n)
 {
     if (E.mode == EPI_NHWC) {
+        if (E.unps2)
+            return (long long)img * E.img_stride + (((long long)(y >> 1) * (W >> 1) + (x >> 1)) * 4 + ((y & 1) * 2 + (x & 1))) * E.n_split + n;
         const int grp = n / E.n_split, c = n - grp * E.n_split;
         return (long long)img * E.img_stride + (long long)grp * E.split_stride + ((long long)y * W + x) * (E.pix_stride ? E.pix_stride : E.n_split) + c;
     }

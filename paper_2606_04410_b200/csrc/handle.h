@@ -64,6 +64,15 @@ struct ufnvc_handle {
     ufnvc::bf16 *ca = nullptr, *cb = nullptr;   // [n][h][w][c_trunk] ping-pong of the context generation
     CUtensorMap tm_dw_ctx;               // ca as the depthwise kernel reads it
     bool dw_ctx_ok = false;
+    // chunk encoder (NEXT-4, R24): E1 patch embedding, E2 fold over frames, E3 context, E4 DC blocks (on ca / cb),
+    // E5 latent head, E6 hyper-encoder, E8 quantiser; then the GPU rANS encoder
+    bool has_enc = false;
+    ufnvc::ConvLayer enc_patch, enc_fold, enc_ctx, enc_y;
+    std::vector<TrunkBlock> enc_blocks;
+    float *henc_w0 = nullptr, *henc_b0 = nullptr, *henc_w1 = nullptr, *henc_b1 = nullptr;   // fp32 [16 c_y][c_h], [c_h], [9][c_h][c_z], [c_z]
+    ufnvc::bf16 *p8 = nullptr, *s2 = nullptr;   // [n T][H/8][W/8][192] patches; [n T][h][w][4 c_trunk] embedded + space-to-depth x2
+    float *ey = nullptr, *henc_a = nullptr;     // [n][h][w][c_y] unquantised latent; [n][h_z][w_z][c_hyper]
+    int16_t *esym = nullptr, *ez = nullptr;     // [n][h][w][c_y] residual; [n][c_z][h_z][w_z] hyper-latent
 
     // workspace (sized for max_chunks)
     double *hx1 = nullptr, *hx2 = nullptr;
@@ -104,6 +113,7 @@ struct ufnvc_handle {
     size_t trunk_sync_stride = 0;
     bool tail_fill = true;
     ActMap am_xs, am_yhat, am_fa, am_fb, am_hidden, am_stage[3], am_ymu[2], am_ca;
+    ActMap am_p8, am_s2, am_cin;         // encoder (R24); am_cin: the context block of the [y ; C] buffer as a conv input
 
     // GPU rANS encoder scratch (NEXT-4), allocated by the first ufnvc_encode_chunk_dev call
     uint16_t *enc_tmp = nullptr;

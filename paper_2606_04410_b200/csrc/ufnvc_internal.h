@@ -53,6 +53,9 @@ struct EpiParams {
     const bf16 *y_in;        // the conv's own input
     int in_stride, out_stride, mu_step, mu_last;
     float *mu_tap, *yhat_tap;   // optional fp32 [pix][c_y], written on partition mu_step only
+    int unps2;               // EPI_NHWC: 1 = space-to-depth x2 store (R24 E1 -> E2): pixel (y, x), column n ->
+                             // out[img][y / 2][x / 2][(2 (y % 2) + x % 2) n_split + n]
+    int out_f32;             // EPI_NHWC: 1 = `out` is fp32 (the unquantised latent y, R24 E5)
     int pix_stride;          // EPI_NHWC: elements between pixels of a group; 0 = n_split (dense).  > n_split: the conv writes a
                              // channel block of a wider tensor (context generation -> [y ; C] buffer, R23)
 };
@@ -213,6 +216,13 @@ cudaError_t launch_rans_encode(const RansEncParams &p, LaunchStream st);
 // NEXT-3 (R22): decoded hyper-latent, channels-last int16 [n][pz][c_z] -> the planar [n][c_z][pz] layout of z_dev
 cudaError_t launch_z_hwc_to_planar(const int16_t *z_hwc, int16_t *z_planar, int n_chunks, int c_z, int pz, LaunchStream st);
 
+// encoder-side kernels (encode.cu, R24)
+cudaError_t launch_enc_patchify(const float *frames, bf16 *out, int n_img, int height, int width, int H8, int W8, LaunchStream st);
+cudaError_t launch_hyper_encoder(const float *y, const float *w0, const float *b0, const float *w1, const float *b1, float *a, int16_t *z,
+                                 float *zf_tap, int n_img, int h, int w, int hz, int wz, int c_y, int c_h, int c_z, LaunchStream st);
+cudaError_t launch_enc_quantise(const float *y, const float *mu, int16_t *sym, long long n, LaunchStream st);
+cudaError_t launch_colour(const float *in, float *out, long long plane, long long n_img, bool to_yuv, cudaStream_t st);
+
 // tcgen05 implicit-GEMM conv (conv_tc.cu)
 cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_in, int tile_h, int tile_w,
                            bool flat, const EpiParams &E, int num_sms, LaunchStream st);
@@ -223,7 +233,7 @@ cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUt
 bool tc_make_halo_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, std::string &err);
 bool tc_make_weight_tmap(ConvLayer &L, std::string &err, int block_n = 0);   // block_n = 0: widest N tile that divides n_pad
 bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, int tile_h, int tile_w,
-                      std::string &err, bool swizzle = true);
+                      std::string &err, bool swizzle = true, int pix_stride = 0);   // pix_stride: elements between pixels (0 = C)
 
 bool tc_encode_2d(CUtensorMap *tm, const void *base, unsigned long long dim0, unsigned long long dim1, unsigned box0, unsigned box1,
                   std::string &err);   // 2-D bf16 map, dim0 contiguous, 128B swizzle, zero OOB fill

@@ -200,6 +200,22 @@ struct Loader {
         return w_p && b_p;
     }
 
+    // R24 hyper-encoder: canonical [n][c_in][k][k] -> fp32 [tap][c_in][n] (k-major: a thread per output reads coalesced) + bias
+    bool plain(float *&w_d, float *&b_d, const std::string &name, int c_in, int n, int k)
+    {
+        const Tensor *tw = get(name + ".w", {uint32_t(n), uint32_t(c_in), uint32_t(k), uint32_t(k)});
+        const Tensor *tb = get(name + ".b", {uint32_t(n)});
+        if (!tw || !tb) return false;
+        std::vector<float> w(size_t(k) * k * c_in * n), b(n);
+        for (int o = 0; o < n; ++o) {
+            b[o] = tb->at(o);
+            for (int c = 0; c < c_in; ++c)
+                for (int tap = 0; tap < k * k; ++tap) w[(size_t(tap) * c_in + c) * n + o] = tw->at((size_t(o) * c_in + c) * k * k + tap);
+        }
+        w_d = upload(w); b_d = upload(b);
+        return w_d && b_d;
+    }
+
     bool depthwise(float *&dw, float *&db, const std::string &name, int C)
     {
         const Tensor *tw = get(name + ".w", {uint32_t(C), 1u, 3u, 3u});
@@ -260,6 +276,18 @@ int load_weights_impl(ufnvc_handle *h, const void *blob, size_t bytes)
             const std::string b = "ctx." + std::to_string(k);
             ok = ld.depthwise(h->ctx_blocks[k].dw_w, h->ctx_blocks[k].dw_b, b + ".dw", c.c_trunk) &&
                  ld.conv(h->ctx_blocks[k].pw1, {b + ".pw1"}, c.c_trunk, ce, 1, false) && ld.conv(h->ctx_blocks[k].pw2, {b + ".pw2"}, ce, c.c_trunk, 1, false);
+        }
+    }
+    h->enc_blocks.assign(c.n_enc_blocks, ufnvc_handle::TrunkBlock());
+    if (ok && h->has_enc) {
+        ok = ld.conv(h->enc_patch, {"enc.patch"}, 192, c.c_trunk, 1, false) && ld.fold(h->enc_fold, "enc.fold", c.c_trunk, c.T, 4 * c.c_trunk) &&
+             ld.conv(h->enc_y, {"enc.y"}, c.c_trunk, c.c_y, 1, false) &&
+             ld.plain(h->henc_w0, h->henc_b0, "henc.0", 16 * c.c_y, c.c_hyper, 1) && ld.plain(h->henc_w1, h->henc_b1, "henc.1", c.c_hyper, c.c_z, 3);
+        if (ok && h->has_ctx) ok = ld.conv(h->enc_ctx, {"enc.ctx"}, c.c_trunk, c.c_trunk, 1, false);
+        for (int k = 0; ok && k < c.n_enc_blocks; ++k) {
+            const std::string b = "enc." + std::to_string(k);
+            ok = ld.depthwise(h->enc_blocks[k].dw_w, h->enc_blocks[k].dw_b, b + ".dw", c.c_trunk) &&
+                 ld.conv(h->enc_blocks[k].pw1, {b + ".pw1"}, c.c_trunk, ce, 1, false) && ld.conv(h->enc_blocks[k].pw2, {b + ".pw2"}, ce, c.c_trunk, 1, false);
         }
     }
     for (int s = 0; ok && s < 4; ++s) {

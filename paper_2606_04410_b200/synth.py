@@ -45,6 +45,7 @@ class ChunkConfig:
     sigma_hi: float = 20.0         # ln sigma ~ U[ln scale_min, ln sigma_hi] (moment-matched, see make_weights)
     mu_steps: int = 1              # 1: the head's mean serves every element; 4: progressive means (R21)
     n_ctx_blocks: int = 0          # > 0: temporal chunk context (R23) with that many DC blocks in the context generation
+    n_enc_blocks: int = 0          # > 0: the blob also carries a chunk ENCODER (R24) with that many DC blocks
 
     # derived geometry (SURVEY.md section 8 notation)
     @property
@@ -122,6 +123,31 @@ def context_config(cfg: ChunkConfig, n_ctx_blocks: int = 11) -> ChunkConfig:
     """Same workload with the temporal chunk context switched on (R23); 11 DC blocks in
     the cross-chunk context generation is the paper's HT-S count."""
     return dataclasses.replace(cfg, n_ctx_blocks=n_ctx_blocks, name=cfg.name + f"-ctx{n_ctx_blocks}")
+
+
+def encoder_config(cfg: ChunkConfig, n_enc_blocks: int = 6) -> ChunkConfig:
+    """Same workload with the chunk encoder's weights in the blob (R24); 6 DC blocks in the
+    chunk encoder is the paper's HT-S count."""
+    return dataclasses.replace(cfg, n_enc_blocks=n_enc_blocks, name=cfg.name + f"-enc{n_enc_blocks}")
+
+
+def make_frames(cfg: ChunkConfig) -> np.ndarray:
+    """Synthetic input frames for the encoder, [n_chunks][T][3][height][width] fp32 in [0,1]: smooth low-frequency fields plus a
+    little noise, drifting over t (stands in for natural video; only the value range and the smoothness matter here)."""
+    rng = _rng(cfg, "frames")
+    n, T, H, W = cfg.n_chunks, cfg.T, cfg.height, cfg.width
+    gy, gx = np.meshgrid(np.linspace(0, 1, H, dtype=np.float32), np.linspace(0, 1, W, dtype=np.float32), indexing="ij")
+    out = np.empty((n, T, 3, H, W), np.float32)
+    for i in range(n):
+        ph = rng.uniform(0, 2 * np.pi, size=(3, 4)).astype(np.float32)
+        fr = rng.uniform(1.0, 6.0, size=(3, 4)).astype(np.float32)
+        for t in range(T):
+            for c in range(3):
+                f = 0.5 + 0.18 * np.sin(2 * np.pi * fr[c, 0] * gx + ph[c, 0] + 0.15 * t) * np.cos(2 * np.pi * fr[c, 1] * gy + ph[c, 1])
+                f += 0.12 * np.sin(2 * np.pi * (fr[c, 2] * gx + fr[c, 3] * gy) + ph[c, 2] + 0.1 * t)
+                out[i, t, c] = f
+        out[i] += rng.normal(0.0, 0.02, size=(T, 3, H, W)).astype(np.float32)
+    return np.clip(out, 0.0, 1.0)
 
 
 def crop_config(cfg: ChunkConfig, height: int, width: int, name: str | None = None) -> ChunkConfig:
@@ -230,6 +256,21 @@ def make_weights(cfg: ChunkConfig) -> dict:
         conv(f"trunk.{k}.dw", cfg.c_trunk, 1, 3, 1.0)
         conv(f"trunk.{k}.pw1", ce, cfg.c_trunk, 1, 2.0)
         conv(f"trunk.{k}.pw2", cfg.c_trunk, ce, 1, 1.0 / max(1, cfg.n_trunk_blocks))
+    # chunk encoder (NEXT-4, R24): patch embedding, fold over frames, DC blocks, latent head, hyper-encoder.  Gains so that y has
+    # the second moment the decoder's cross-frame layer was scaled for and z ~ N(0, 2^2) like make_z.
+    if cfg.n_enc_blocks > 0:
+        ct = cfg.c_trunk
+        conv("enc.patch", ct, 192, 1, 1.0 / 0.3)                    # frames in [0,1]: E[x^2] ~ 0.3
+        conv("enc.fold", ct, cfg.T * 4 * ct, 1, 1.0)
+        if cfg.n_ctx_blocks > 0:
+            conv("enc.ctx", ct, ct, 1, 0.5)
+        for k in range(cfg.n_enc_blocks):
+            conv(f"enc.{k}.dw", ct, 1, 3, 1.0)
+            conv(f"enc.{k}.pw1", ct * cfg.trunk_expand, ct, 1, 2.0)
+            conv(f"enc.{k}.pw2", ct, ct * cfg.trunk_expand, 1, 1.0 / cfg.n_enc_blocks)
+        conv("enc.y", cfg.c_y, ct, 1, _second_moment_yhat(cfg) / 2.0)
+        conv("henc.0", cfg.c_hyper, 16 * cfg.c_y, 1, 2.0 / _second_moment_yhat(cfg))
+        conv("henc.1", cfg.c_z, cfg.c_hyper, 3, 4.0)
     # frame-specific decoders (O8): distinct weights per frame index t.
     for t in range(cfg.T):
         for s in range(4):
