@@ -249,6 +249,57 @@ def run_ours(args):
     bytes_in = dict(value=n * cfg.T / (statistics.mean(bytes_ms) / 1e3), unit="frames/s (this rank)", ms_per_step=statistics.mean(bytes_ms),
                     steps=10, z_stream_bytes=int(sum(int(zo[-1]) for _, zo in zparts)), y_stream_bytes=int(sum(int(po[-1]) for _, po in parts)),
                     launches_per_call=bytes_launches, call="ufnvc_chunk_decode_bytes")
+    # ---- widened rows of SURVEY.md 8f, 10 extra steps each on handles of their own (rank 0's figures are printed):
+    # NEXT-2a temporal context with the paper's HT-S count of 11 context DC blocks (R23), NEXT-4 chunk encode with 6 (R24) ----
+    def timed(fn, reps=10, before=None):
+        ms = []
+        with torch.cuda.stream(stream):
+            for _ in range(reps + 2):
+                if before:
+                    before()
+                flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                fn()
+                e1.record(stream)
+                e1.synchronize()
+                ms.append(e0.elapsed_time(e1))
+        return statistics.mean(ms[2:])
+    extra = {}
+    if args.config in (2, 3) and args.mu_steps == 1:
+        ccfg = synth.context_config(cfg, 11)
+        cdec = binding.ChunkDecoder(ccfg, device=local)
+        cdec.load_weights(synth.make_weights(ccfg))
+        cdec.reset_context(n, stream=stream)
+        _, _, cidx = cdec.entropy_params(z, stream=stream)
+        stream.synchronize()
+        cparts = [cdec.encode_chunk(cidx[c].cpu().numpy(), cdec.symbols_from_uniform(cidx[c].cpu().numpy(), u16[c])) for c in range(n)]
+        cb, co = binding.concat_streams(cparts)
+        cb, co = torch.from_numpy(cb).to(dev), torch.from_numpy(co.astype(np.int64).astype(np.int32)).to(dev)
+        ms = timed(lambda: cdec.chunk_decode(z, cb, co, frames=frames, stream=stream), before=lambda: cdec.reset_context(n, stream=stream))
+        assert cdec.get_status() == 0, "bit-stream status (context leg)"
+        prof = cdec.chunk_decode_profiled(z, cb, co, frames, stream=stream)
+        extra["context"] = dict(value=n * cfg.T / (ms / 1e3), unit="frames/s (this rank)", ms_per_step=ms, n_ctx_blocks=11,
+                                context_generation_us=prof["ctx"], launches_per_call=cdec.launches_per_call(n), workload=ccfg.name,
+                                call="ufnvc_chunk_decode on a handle with n_ctx_blocks = 11 (state reset, untimed, before every step)")
+        cdec.destroy()
+        ecfg = synth.encoder_config(cfg, 6)
+        edec = binding.ChunkDecoder(ecfg, device=local)
+        edec.load_weights(synth.make_weights(ecfg))
+        fr_in = torch.from_numpy(synth.make_frames(ecfg)).to(dev)
+        res = {}
+        ms = timed(lambda: res.update(edec.chunk_encode(fr_in, stream=stream)))
+        assert edec.get_status() == 0, "status (encode leg)"
+        nbytes = int(res["sub_off"][-1].item())
+        back = edec.chunk_decode(res["z"], res["bits"][:nbytes], res["sub_off"], frames=frames, stream=stream)
+        stream.synchronize()
+        assert edec.get_status() == 0, "the decoder rejects the encoder's stream"
+        mse = float(((back - fr_in) ** 2).mean())
+        extra["encode"] = dict(value=n * cfg.T / (ms / 1e3), unit="encoded frames/s (this rank)", ms_per_step=ms, n_enc_blocks=6,
+                               stream_bytes=nbytes, launches_per_call=edec.launches_per_call(n), workload=ecfg.name,
+                               call="ufnvc_chunk_encode (frames resident on the device -> bytes on the device)",
+                               note="random-init weights: the round trip decodes cleanly (status 0) but reconstructs noise, mse %.3f" % mse)
+        edec.destroy()
     frames_per_step = n * cfg.T
     value = replicas.job_throughput(frames_per_step, args.steps, total_ms, dev)       # all ranks' frames / max-over-ranks time
     total_ms = replicas.max_over_ranks(total_ms, dev)
@@ -365,7 +416,7 @@ def run_ours(args):
                 e2e=dict(value=e2e_val, unit="frames/s", h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, steps=e2e_steps,
                          overlap="D2H of step i on a copy stream overlaps the decode of step i+1 (two buffer sets)",
                          bound="PCIe: the boundary's output is fp32 planar frames (199 MB per 1080p chunk)"),
-                roofline=roofline, bytes_in=bytes_in,
+                roofline=roofline, bytes_in=bytes_in, **extra,
                 cpu_baseline=dict(value=fps_cpu, unit="frames/s", cores=cores, kind="oracle", sample=desc, seconds=sec_cpu,
                                   fp32_oracle=dict(value=fps32, seconds=sec32, sample=desc32)),
                 wall_s_timed_region=t_wall)

@@ -31,8 +31,8 @@ constexpr int kC = 256;                  // trunk width: K of GEMM1, N of GEMM2
 constexpr int kHC = 128;                 // hidden columns per chunk
 constexpr int kTM = 128;                 // pixels per tile
 constexpr int kTrunkThreads = 320;       // single-CTA kernel: TMA warp, MMA warp, 8 epilogue warps
-constexpr int kPairThreads = 576;        // CTA-pair kernel: TMA warp, MMA warp, 16 epilogue warps
-static_assert(kPairThreads / 32 - 2 == int(kTrunkTileSignals), "one tile_done increment per epilogue warp (warps 2..17)");
+constexpr int kPairThreads = 448;        // CTA-pair kernel: TMA warp, MMA warp, 4 GELU warps, 8 drain warps
+static_assert(kPairThreads / 32 - 6 == int(kTrunkTileSignals), "one tile_done increment per drain warp (warps 6..13)");
 constexpr int kWStages = 3;
 constexpr uint32_t kSlab = 16384;        // 128 rows x 128 B
 constexpr uint32_t kWStage = 32768;
@@ -371,9 +371,9 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
     const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     constexpr int NS = TMH ? 5 : 3;                            // weight-ring stages
     constexpr uint32_t offW = TMH ? kOffHs : kOffW, offBar = offW + NS * kWStage;
-    constexpr uint32_t B_WFULL = 2, B_WEMPTY = B_WFULL + NS, B_HACC_FULL = B_WEMPTY + NS, B_HACC_EMPTY = B_HACC_FULL + 2,
-                       B_HS_FULL = B_HACC_EMPTY + 2, B_HS_EMPTY = B_HS_FULL + 2, B_OFULL = B_HS_EMPTY + 2, B_OEMPTY = B_OFULL + 1,
-                       B_TMEM_SLOT = B_OEMPTY + 1;                     // (shadow the file-scope slots: 3-stage layout)
+    // HS_FULL: one barrier per Hacc buffer and 32-column sub-step of a chunk (2 x 4)
+    constexpr uint32_t B_WFULL = 2, B_WEMPTY = B_WFULL + NS, B_HACC_FULL = B_WEMPTY + NS, B_HS_FULL = B_HACC_FULL + 2,
+                       B_OFULL = B_HS_FULL + 8, B_OEMPTY = B_OFULL + 1, B_TMEM_SLOT = B_OEMPTY + 1;   // (shadow the file-scope slots)
     auto bar = [&](uint32_t slot) { return base + offBar + 8u * slot; };
     volatile uint32_t *tmem_slot_ptr =
         reinterpret_cast<volatile uint32_t *>(smem_raw + (bar(B_TMEM_SLOT) - smem_u32(smem_raw)));
@@ -390,10 +390,10 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
         mbar_init(bar(B_AFULL), 1); mbar_init(bar(B_AEMPTY), 1);
         for (int s = 0; s < NS; ++s) { mbar_init(bar(B_WFULL + s), 1); mbar_init(bar(B_WEMPTY + s), 1); }
         for (int b = 0; b < 2; ++b) {
-            mbar_init(bar(B_HACC_FULL + b), 1); mbar_init(bar(B_HACC_EMPTY + b), 32);     // 16 epilogue warps x 2 CTAs
-            mbar_init(bar(B_HS_FULL + b), 32);  mbar_init(bar(B_HS_EMPTY + b), 1);
+            mbar_init(bar(B_HACC_FULL + b), 1);
+            for (int q = 0; q < 4; ++q) mbar_init(bar(B_HS_FULL + 4 * b + q), 8);         // 4 GELU warps x 2 CTAs per sub-step
         }
-        mbar_init(bar(B_OFULL), 1); mbar_init(bar(B_OEMPTY), 32);
+        mbar_init(bar(B_OFULL), 1); mbar_init(bar(B_OEMPTY), 16);                         // 8 drain warps x 2 CTAs
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     cluster_sync_all();                                              // peer barriers are initialised before anyone signals
@@ -454,7 +454,7 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
             const uint32_t a_lo = lo(base + kOffA), hs_lo = lo(base + kOffHs), w_lo = lo(base + offW);
             const uint32_t o_acc = tmem_base, h_acc = tmem_base + kC;
             int ws = 0; uint32_t wp = 0;
-            uint32_t ph_hacc = 0, ph_hs = 0;
+            uint32_t ph_hs = 0;
             auto w_wait = [&]() {
                 mbar_wait_cluster(bar(B_WFULL + ws), wp);
                 tc_fence_after();
@@ -463,11 +463,7 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
             auto w_release = [&]() { umma2_commit_both(bar(B_WEMPTY + ws)); if (++ws == NS) { ws = 0; wp ^= 1; } };
             auto gemm1 = [&](int c) {
                 const int b = c & 1;
-                if (!TMH) {                                            // TMH: Hacc[b] is released by GEMM2(c-2), in issue order
-                    mbar_wait_cluster(bar(B_HACC_EMPTY + b), ((ph_hacc >> b) & 1) ^ 1);
-                    ph_hacc ^= 1u << b;
-                    tc_fence_after();
-                }
+                // Hacc[b] is released by GEMM2(c-2), in issue order (the tensor pipe executes in order)
                 const uint32_t d = h_acc + uint32_t(b) * kHC;
                 const uint32_t w = w_wait();
 #pragma unroll
@@ -493,115 +489,138 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
                         if (c + LA + 1 == NC) umma2_commit_both(bar(B_AEMPTY));
                     }
                     const int b = c & 1;
-                    mbar_wait_cluster(bar(B_HS_FULL + b), (ph_hs >> b) & 1);
+                    const uint32_t hs_par = (ph_hs >> b) & 1;
                     ph_hs ^= 1u << b;
-                    if (c == 0) mbar_wait_cluster(bar(B_OEMPTY), (it & 1) ^ 1);
-                    tc_fence_after();
-                    const uint32_t w = w_wait();
+                    uint32_t w = 0;
+                    // GEMM2(c) in four steps of K = 32: step q is issued as soon as the GELU warps have stored hidden columns
+                    // [32 q, 32 q + 32) -- the first MMAs run while the rest of the chunk is still in the GELU
 #pragma unroll
-                    for (int j = 0; j < 2; ++j)
-#pragma unroll
-                        for (int k = 0; k < 4; ++k) {
-                            if (TMH)     // hidden 64 j + 16 k .. +15 = 8 packed columns at Hacc[b] + 64 j + 32 (k / 2) + 8 (k % 2): every GELU
-                                         // warp packs its 32 hidden columns into the first 16 of the fp32 columns it read
-                                umma2_bf16_ts(o_acc, h_acc + uint32_t(b) * kHC + uint32_t(64 * j + 32 * (k >> 1) + 8 * (k & 1)),
-                                              w + uint32_t(j) * (kSlab >> 4) + 2 * k, hi, idesc2, uint32_t(c | j | k));
-                            else
-                                umma2_bf16_lh(o_acc, hs_lo + uint32_t(2 * b + j) * (kSlab >> 4) + 2 * k, hi, w + uint32_t(j) * (kSlab >> 4) + 2 * k,
-                                              hi, idesc2, uint32_t(c | j | k));
+                    for (int q = 0; q < 4; ++q) {
+                        mbar_wait_cluster(bar(B_HS_FULL + 4 * b + q), hs_par);
+                        if (q == 0) {
+                            if (c == 0) mbar_wait_cluster(bar(B_OEMPTY), (it & 1) ^ 1);
+                            w = w_wait();
                         }
+                        tc_fence_after();
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const int kk = 2 * q + e, j = kk >> 2, k = kk & 3;     // K slice kk = hidden columns [16 kk, +16)
+                            // hidden 32 q + 16 e .. +15 = 8 packed columns at Hacc[b] + 32 q + 8 e: a GELU warp packs the 32 hidden
+                            // columns of a sub-step into the first 16 of the fp32 columns it read
+                            umma2_bf16_ts(o_acc, h_acc + uint32_t(b) * kHC + uint32_t(32 * q + 8 * e), w + uint32_t(j) * (kSlab >> 4) + 2 * k, hi,
+                                          idesc2, uint32_t(c | kk));
+                        }
+                    }
                     w_release();
-                    if (!TMH) umma2_commit_both(bar(B_HS_EMPTY + b));
                 }
                 umma2_commit_both(bar(B_OFULL));
             }
         }
     } else {
-        // ===================== epilogue warps (both CTAs): 16 = 4 TMEM lane quadrants x 4 column parts =====================
-        // Four warps per scheduler: the GELU of a chunk costs every scheduler >= 1024 MUFU-pipe cycles (one MUFU.TANH per
-        // element at 4 lanes per clock) beside ~900 FMA-pipe cycles, against 2048 tensor cycles per chunk; with two warps per
-        // scheduler the two pipes overlapped badly (1650-1700 cycles per chunk, measured), the hidden chunk came back too
-        // late for GEMM2 and the tensor pipe idled half the time.
-        const int quad = warp & 3, part = (warp - 2) >> 2;               // part: hidden columns [32 part, +32) of a chunk
+        // ===================== epilogue warps (both CTAs) =====================
+        // Warps 2..5: GELU, one per TMEM lane quadrant = one per scheduler.  Warps 6..13: output drain, two per quadrant.
+        // Why two kinds: clock64 around the phases showed the epilogue as ONE serial resource per scheduler -- the GELU of
+        // the next tile's first chunks waited for the previous tile's drain, and GEMM2(c) for the slowest of 32 warps.
+        // Now the GELU warp of a scheduler walks a chunk in four 32-column sub-steps and signals each (GEMM2's first MMAs are
+        // issued a quarter of the way through), the MUFU pipe -- the floor of this phase: one MUFU.TANH per element at 4
+        // lanes per clock = 1024 cycles per chunk -- is fed by one instruction stream, and the drain runs beside it.
+        const int quad = warp & 3;
         const int r = quad * 32 + lane;
         const uint32_t t_lane = tmem_base + (uint32_t(quad * 32) << 16);
-        const uint32_t hs_full_l = mapa_rank(bar(B_HS_FULL), 0), oempty_l = mapa_rank(bar(B_OEMPTY), 0);
-        uint32_t ph_use = 0;
-        int it = 0;
-        for (int pt = pair0; pt < n_ptiles; pt += n_pairs, ++it) {
-            const int tile = 2 * pt + int(rank);
-            for (int c = 0; c < NC; ++c) {
-                const int b = c & 1;
-                mbar_wait(bar(B_HACC_FULL + b), (ph_use >> b) & 1);
-                ph_use ^= 1u << b;
-                tc_fence_after();
-                uint32_t v[32], pk[16];
-                tmem_ld32(t_lane + kC + uint32_t(b) * kHC + uint32_t(part * 32), v);
+        if (warp < 6) {
+            const uint32_t hs_full_l = mapa_rank(bar(B_HS_FULL), 0);
+            uint32_t ph_use = 0;
+            for (int pt = pair0; pt < n_ptiles; pt += n_pairs) {
+                for (int c = 0; c < NC; ++c) {
+                    const int b = c & 1;
+                    mbar_wait(bar(B_HACC_FULL + b), (ph_use >> b) & 1);
+                    ph_use ^= 1u << b;
+                    tc_fence_after();
+                    const uint32_t hbase = t_lane + kC + uint32_t(b) * kHC;
+                    uint32_t va[32], vb[32];
+                    tmem_ld32_nowait(hbase, va);
+                    auto sub = [&](const uint32_t (&v)[32], int q) {
+                        uint32_t pk[16];
 #pragma unroll
-                for (int j = 0; j < 32; j += 2) {                         // half biases from the constant bank: warp-uniform address
-                    const float *hb = p.hb1v + c * kHC + part * 32 + j;
-                    pk[j / 2] = gelu_bias2_pk(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), hb[0], hb[1]);
+                        for (int j = 0; j < 32; j += 2) {                 // half biases from the constant bank: warp-uniform address
+                            const float *hb = p.hb1v + c * kHC + q * 32 + j;
+                            pk[j / 2] = gelu_bias2_pk(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), hb[0], hb[1]);
+                        }
+                        // the 32 hidden columns of the sub-step go, packed, over the first 16 of the fp32 columns just read
+                        tmem_st16(hbase + uint32_t(q * 32), pk);
+                        tmem_st_wait();
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive_cluster(hs_full_l + 8u * uint32_t(4 * b + q));
+                    };
+                    // the load of sub-step q + 1 is in flight while sub-step q is computed
+                    tmem_ld_wait(); tmem_ld32_nowait(hbase + 32, vb); sub(va, 0);
+                    tmem_ld_wait(); tmem_ld32_nowait(hbase + 64, va); sub(vb, 1);
+                    tmem_ld_wait(); tmem_ld32_nowait(hbase + 96, vb); sub(va, 2);
+                    tmem_ld_wait(); sub(vb, 3);
                 }
-                // the 32 hidden columns of this warp go, packed, over the first 16 of the 32 fp32 columns it has just read (no other
-                // warp touches those): hidden column h of the chunk = packed column 32 (h / 32) + (h % 32) / 2 of Hacc[b]
-                tmem_st16(t_lane + kC + uint32_t(b) * kHC + uint32_t(part * 32), pk);
-                tmem_st_wait();
+            }
+        } else {
+            const int half = (warp - 6) >> 2;                            // output columns [128 half, +128)
+            const uint32_t oempty_l = mapa_rank(bar(B_OEMPTY), 0);
+            int it = 0;
+            for (int pt = pair0; pt < n_ptiles; pt += n_pairs, ++it) {
+                const int tile = 2 * pt + int(rank);
+                const long long row = (long long)tile * kTM + r;
+                const bool inb = row < p.n_px;
+                // residual row segment (128 columns = 8 x 32 B), fetched BEFORE the wait for the last GEMM2s.  A thread is a
+                // pixel row (TMEM lane), so every lane touches its own 32-byte sector: 256-bit accesses halve the L1 wavefronts.
+                uint32_t res[8][8];
+                {
+                    const bf16 *rs = p.x + row * kC + half * 128;
+#pragma unroll
+                    for (int g = 0; g < 8; ++g) {
+                        if (inb) ld_global_256(rs + 16 * g, res[g]);
+                        else {
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) res[g][e] = 0u;
+                        }
+                    }
+                }
+                mbar_wait(bar(B_OFULL), it & 1);
+                tc_fence_after();
+                // Oacc is single-buffered: the next tile's first GEMM2 waits until it is in registers.  Two loads in flight at
+                // a time; the accumulator is RELEASED as soon as the last load has landed.
+                uint32_t va[32], vb[32];
+                auto emit = [&](const uint32_t (&vq)[32], int q) {
+                    const int c0 = half * 128 + q * 32;
+                    bf16 *dst = p.out + row * kC + c0;
+#pragma unroll
+                    for (int g = 0; g < 2; ++g) {                         // 16 columns = one 32-byte sector
+                        uint32_t o8[8];
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            const uint32_t xr = res[q * 2 + g][e];        // bf16 pair -> fp32: low half << 16, high half masked
+                            const float *bc = p.b2v + c0 + g * 16 + 2 * e;      // (warp-uniform address, constant bank)
+                            o8[e] = pack_bf16x2(__uint_as_float(vq[g * 16 + 2 * e]) + bc[0] + __uint_as_float(xr << 16),
+                                                __uint_as_float(vq[g * 16 + 2 * e + 1]) + bc[1] + __uint_as_float(xr & 0xFFFF0000u));
+                        }
+                        if (inb) st_global_256(dst + 16 * g, o8);
+                    }
+                };
+                tmem_ld32_nowait(t_lane + uint32_t(half * 128), va);
+                tmem_ld32_nowait(t_lane + uint32_t(half * 128 + 32), vb);
+                tmem_ld_wait();
+                emit(va, 0);
+                tmem_ld32_nowait(t_lane + uint32_t(half * 128 + 64), va);
+                emit(vb, 1);
+                tmem_ld32_nowait(t_lane + uint32_t(half * 128 + 96), vb);
+                tmem_ld_wait();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(hs_full_l + 8u * b);
+                if (lane == 0) mbar_arrive_cluster(oempty_l);             // Oacc is in registers: the next tile may accumulate
+                emit(va, 2);
+                emit(vb, 3);
+                __syncwarp();
+                // tail filling: the depthwise kernel of the next trunk block polls these counters instead of waiting for the
+                // whole grid (the __syncwarp above orders every lane's stores before lane 0's release)
+                if (p.tile_done && lane == 0) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p.tile_done + tile) : "memory");
             }
-            const long long row = (long long)tile * kTM + r;
-            const bool inb = row < p.n_px;
-            // residual row segment (64 columns = 4 x 32 B), fetched BEFORE the wait for the last GEMM2s.  A thread is a pixel row
-            // (TMEM lane), so every lane touches its own 32-byte sector: 256-bit accesses halve the L1 wavefronts of this drain,
-            // which -- with the bias shuffles it used to have -- kept the epilogue warps busy for ~7.7 k of a tile's 16.4 k
-            // tensor cycles (measured with clock64 around the phases) while the next tile's first GELUs waited for them.
-            uint32_t res[4][8];
-            {
-                const bf16 *rs = p.x + row * kC + part * 64;
-#pragma unroll
-                for (int g = 0; g < 4; ++g) {
-                    if (inb) ld_global_256(rs + 16 * g, res[g]);
-                    else {
-#pragma unroll
-                        for (int e = 0; e < 8; ++e) res[g][e] = 0u;
-                    }
-                }
-            }
-            mbar_wait(bar(B_OFULL), it & 1);
-            tc_fence_after();
-            // Oacc is single-buffered: the next tile's first GEMM2 waits until it is drained.  Both 32-column loads of this
-            // warp are issued together and the accumulator is RELEASED as soon as they have landed in registers; the adds,
-            // the packing and the stores follow.
-            uint32_t va[32], vb[32];
-            tmem_ld32_nowait(t_lane + uint32_t(part * 64), va);
-            tmem_ld32_nowait(t_lane + uint32_t(part * 64 + 32), vb);
-            tmem_ld_wait();
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(oempty_l);                 // Oacc is in registers: the next tile may accumulate
-            auto emit = [&](const uint32_t (&vq)[32], int q) {
-                const int c0 = part * 64 + q * 32;
-                bf16 *dst = p.out + row * kC + c0;
-#pragma unroll
-                for (int g = 0; g < 2; ++g) {                             // 16 columns = one 32-byte sector
-                    uint32_t o8[8];
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) {
-                        const uint32_t xr = res[q * 2 + g][e];            // bf16 pair -> fp32: low half << 16, high half masked
-                        const float *bc = p.b2v + c0 + g * 16 + 2 * e;    // (warp-uniform address, constant bank)
-                        o8[e] = pack_bf16x2(__uint_as_float(vq[g * 16 + 2 * e]) + bc[0] + __uint_as_float(xr << 16),
-                                            __uint_as_float(vq[g * 16 + 2 * e + 1]) + bc[1] + __uint_as_float(xr & 0xFFFF0000u));
-                    }
-                    if (inb) st_global_256(dst + 16 * g, o8);
-                }
-            };
-            emit(va, 0);
-            emit(vb, 1);
-            __syncwarp();
-            // tail filling: the depthwise kernel of the next trunk block polls these counters instead of waiting for the whole
-            // grid (the __syncwarp above orders every lane's stores before lane 0's release)
-            if (p.tile_done && lane == 0) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p.tile_done + tile) : "memory");
         }
     }
 
