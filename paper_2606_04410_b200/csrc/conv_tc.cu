@@ -54,6 +54,10 @@ struct TcParams {
     int n_img_m, Hm, Wm;          // activation as the TMA map sees it (flattened for 1x1 convs)
     int flat, tw_shift;           // flat: rows of 128 consecutive pixels; tw_shift = log2(TW)
     int tiles_y, tiles_x, TH, TW;
+    int xpose;                    // CTA-pair halo kernel: the map's dimension 1 is the image's y and dimension 2 its x (Hm = W, Wm = H)
+    int tiles_img;                // CTA-pair halo kernel: tiles per image; the schedule runs over PAIRS of consecutive tiles
+    int reverse;                  // CTA-pair halo kernel: schedule unit u stands for unit total_tiles - 1 - u
+    FastDiv fd_pairs;             // pairs per image = ceil(tiles_img / 2)
     int H, W;                     // real image dims: global pixel -> (img, y, x) for the epilogue
     int taps, slabs;              // k-blocks per tile = taps * slabs
     int tap_img;                  // 1: tap t is image img * taps + t of the activation map (fold over stacked images), no spatial shift
@@ -91,6 +95,26 @@ __device__ __forceinline__ TileCoord tile_coord(const TcParams &p, int tile)
     return c;
 }
 
+// CTA-pair halo kernel: schedule unit -> this CTA's tile.  A unit is (image, pair of consecutive tiles of that image in row-major
+// tile order, n tile); the two tiles of a pair need not be neighbours (each CTA loads its own halo box, the pair shares only the
+// weights), so an odd tile count per row costs nothing and only an odd count per IMAGE leaves one half-empty pair.  A tile past
+// the image's last gets an origin outside the map: TMA fills zeros and the epilogue's bounds test masks it.
+__device__ __forceinline__ TileCoord tile_coord_pair(const TcParams &p, int unit, int rank)
+{
+    TileCoord c;
+    uint32_t r, nt, pi, img, ty, tx;
+    if (p.reverse) unit = p.total_tiles - 1 - unit;
+    p.fd_ntiles.divmod(uint32_t(unit), r, nt);
+    p.fd_pairs.divmod(r, img, pi);
+    const uint32_t id = 2 * pi + uint32_t(rank);
+    p.fd_tx.divmod(id, ty, tx);
+    c.nt = int(nt);
+    c.img = int(img);
+    c.y0 = int(id) < p.tiles_img ? int(ty) * p.TH : p.Hm + p.TH;
+    c.x0 = int(tx) * p.TW;
+    return c;
+}
+
 // 8 epilogue warps: warp w reads TMEM lanes 32*(w%4) .. +31 (a hardware rule), and the two warps of a lane quadrant
 // split the 32-column chunks between them (even / odd), so every SM sub-partition holds two epilogue warps and the
 // tcgen05.ld / MUFU latencies of one hide behind the other.  tcgen05.ld -> bias -> act -> store, per tile of the
@@ -109,13 +133,13 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
     int it = 0;
     const int tile0 = pair_rank < 0 ? int(blockIdx.x) : int(blockIdx.x >> 1), tstride = pair_rank < 0 ? int(gridDim.x) : int(gridDim.x >> 1);
     for (int tile = tile0; tile < p.total_tiles; tile += tstride, ++it) {
-        TileCoord tc = tile_coord(p, tile);
-        if (pair_rank >= 0) tc.x0 = 2 * tc.x0 + pair_rank * p.TW;
+        const TileCoord tc = pair_rank >= 0 ? tile_coord_pair(p, tile, pair_rank) : tile_coord(p, tile);
         const int acc = it & 1;
         const uint32_t acc_phase = (it >> 1) & 1;
         const int ym = tc.y0 + my, xm = tc.x0 + mx;
         const bool inb = ym < p.Hm && xm < p.Wm;
         int img = tc.img, y = ym, x = xm;
+        if (p.xpose) { y = xm; x = ym; }                          // transposed tile map: map dimension 1 is the image's y
         if (p.flat) {                                             // map-space row of 128 pixels -> real (img, y, x)
             const unsigned gp = unsigned(ym) * 128u + unsigned(xm);
             img = int(gp / P);
@@ -689,8 +713,7 @@ conv_halo_pair_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_c
         if (elect_one()) {
             int sa = 0, sb = 0; uint32_t pa = 0, pb = 0;
             for (int tile = pair0; tile < p.total_tiles; tile += n_pairs) {
-                TileCoord tc = tile_coord(p, tile);
-                tc.x0 = 2 * tc.x0 + int(rank) * p.TW;                              // may lie past the image: an all-zero tile
+                const TileCoord tc = tile_coord_pair(p, tile, int(rank));          // may lie past the image: an all-zero tile
                 const int grp = group_of(p, tc.img);
                 for (int slab = 0; slab < p.slabs; ++slab) {
                     mbar_wait(aempty(sa), pa ^ 1);
@@ -700,8 +723,10 @@ conv_halo_pair_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_c
                     for (int tap = 0; tap < 9; ++tap) {
                         mbar_wait(bempty(sb), pb ^ 1);
                         if (rank == 0) mbar_expect_tx(bfull(sb), 2 * bh_bytes);
+                        // transposed map: the k-block the MMA thread pairs with view (tap / 3, tap % 3) holds image tap (tap % 3, tap / 3)
+                        const int wtap = p.xpose ? (tap % 3) * 3 + tap / 3 : tap;
                         tma_load_3d_pair(b_base + uint32_t(sb) * bh_bytes, &tmap_bh, mapa_rank(bfull(sb), 0), slab * kSlabK,
-                                         tc.nt * p.BN + int(rank) * (p.BN >> 1), grp * 9 + tap);
+                                         tc.nt * p.BN + int(rank) * (p.BN >> 1), grp * 9 + wtap);
                         if (++sb == nb_stages) { sb = 0; pb ^= 1; }
                     }
                 }
@@ -849,6 +874,25 @@ bool tc_make_halo_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int 
     return tc_make_act_tmap(tm, base, n_img, H, W, C, kHaloTH + 2, kHaloTW + 2, err);
 }
 
+// The halo tile is 16 map rows x 8 map columns.  With the image's y as the map's dimension 1 the same tile covers 8 image rows x
+// 16 image columns; whichever orientation pads the image to fewer tiles is used (A8 stage 1 at 68 x 120: 75 tiles against 72).
+bool halo_prefers_transposed(int H, int W)
+{
+    const long normal = long((H + kHaloTH - 1) / kHaloTH) * ((W + kHaloTW - 1) / kHaloTW);
+    const long xposed = long((W + kHaloTH - 1) / kHaloTH) * ((H + kHaloTW - 1) / kHaloTW);
+    return xposed < normal;
+}
+
+// Same activation, dimensions 1 and 2 exchanged: {C, H, W, n_img} with strides {row, pixel, image}; box {64, 10 rows, 18 columns}.
+bool tc_make_halo_tmap_transposed(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, std::string &err)
+{
+    const cuuint64_t ps = cuuint64_t(C) * 2;
+    cuuint64_t dims[4] = {cuuint64_t(C), cuuint64_t(H), cuuint64_t(W), cuuint64_t(n_img)};
+    cuuint64_t strides[3] = {ps * W, ps, ps * W * H};
+    cuuint32_t box[4] = {cuuint32_t(kSlabK), cuuint32_t(kHaloTW + 2), cuuint32_t(kHaloTH + 2), 1};
+    return encode(tm, base, 4, dims, strides, box, err);
+}
+
 cudaError_t configure_conv_tc_kernels()
 {
     cudaError_t e = cudaSuccess;
@@ -865,21 +909,26 @@ cudaError_t configure_conv_tc_kernels()
 }
 
 cudaError_t launch_conv_halo_pair(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
-                                  LaunchStream st)
+                                  LaunchStream st, bool transposed)
 {
     if (L.taps != 9 || !L.has_half_map || (E.mode != EPI_PS2 && E.mode != EPI_HEAD)) return cudaErrorInvalidValue;
     TcParams p{};
     p.H = P.H; p.W = P.W;
-    p.n_img_m = P.n_img; p.Hm = P.H; p.Wm = P.W;
+    p.xpose = transposed ? 1 : 0;
+    p.reverse = P.reverse ? 1 : 0;
+    p.n_img_m = P.n_img; p.Hm = transposed ? P.W : P.H; p.Wm = transposed ? P.H : P.W;
     p.TH = kHaloTH; p.TW = kHaloTW;
     p.flat = 0; p.tw_shift = 3;
-    p.tiles_y = (P.H + kHaloTH - 1) / kHaloTH;
-    p.tiles_x = ((P.W + kHaloTW - 1) / kHaloTW + 1) / 2;          // tile PAIRS along x; rank r owns x tile 2 txp + r
+    p.tiles_y = (p.Hm + kHaloTH - 1) / kHaloTH;
+    p.tiles_x = (p.Wm + kHaloTW - 1) / kHaloTW;
+    p.tiles_img = p.tiles_y * p.tiles_x;
+    const int pairs = (p.tiles_img + 1) / 2;                       // schedule unit = (image, pair of consecutive tiles, n tile)
     p.taps = 9; p.slabs = L.c_in / kSlabK;
     p.BN = L.block_n; p.n_tiles = L.n_pad / L.block_n; p.n_real = L.n; p.n_pad = L.n_pad;
     p.groups = L.groups;
-    p.total_tiles = p.n_img_m * p.tiles_y * p.tiles_x * p.n_tiles;
+    p.total_tiles = p.n_img_m * pairs * p.n_tiles;
     p.fd_ntiles = make_fastdiv(p.n_tiles); p.fd_tx = make_fastdiv(p.tiles_x); p.fd_ty = make_fastdiv(p.tiles_y);
+    p.fd_pairs = make_fastdiv(pairs);
     p.fd_groups = make_fastdiv(p.groups);
     p.bias = L.bias;
     p.E = E;

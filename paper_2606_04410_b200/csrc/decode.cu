@@ -23,7 +23,7 @@ cudaError_t conv(ufnvc_handle *h, const ConvLayer &L, const ConvProblem &P, cons
     if (launches) ++*launches;
     if (L.use_tc && L.taps == 9 && am.halo_ok && !h->force_generic && h->use_pair_conv && L.has_half_map &&
         E.mode == EPI_PS2 && P.W > 8)
-        return launch_conv_halo_pair(L, P, am.tm_halo, E, h->num_sms, st);
+        return launch_conv_halo_pair(L, P, am.halo_t ? am.tm_halo_t : am.tm_halo, E, h->num_sms, st, am.halo_t);
     if (L.use_tc && L.taps == 9 && am.halo_ok && !h->force_generic)
         return launch_conv_halo(L, P, am.tm_halo, E, h->num_sms, st);
     if (L.use_tc && am.ok && !h->force_generic) return launch_conv_tc(L, P, am.tm, am.tile_h, am.tile_w, am.flat, E, h->num_sms, st);
@@ -80,7 +80,7 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
             // kernel shares every weight tile between two 16 x 8 pixel tiles (M = 256) and loads the activations once per
             // slab instead of once per tap.  Fallback: the shifted-TMA-box kernel (narrow maps, debug flag).
             if (h->use_pair_conv && h->head_tc.has_half_map && h->am_xs.halo_ok && h->w_z > 8)
-                CU_TRY(launch_conv_halo_pair(h->head_tc, pr, h->am_xs.tm_halo, E, h->num_sms, st));
+                CU_TRY(launch_conv_halo_pair(h->head_tc, pr, h->am_xs.halo_t ? h->am_xs.tm_halo_t : h->am_xs.tm_halo, E, h->num_sms, st, h->am_xs.halo_t));
             else
                 CU_TRY(launch_conv_tc(h->head_tc, pr, h->am_xs.tm, h->am_xs.tile_h, h->am_xs.tile_w, false, E, h->num_sms, st));
             CU_TRY(launch_hyper_fix(h->fix_list, h->fix_count, h->hx2, h->head_fix_w, h->head_fix_b, c.c_hyper, h->h_z, h->w_z, hp,
@@ -196,6 +196,8 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
     for (int s = 0; s < 3; ++s) {
         const int co = c.dec_channels[s + 1];
         ConvProblem pr{x, n * T, sh, sw, T};
+        pr.reverse = (s & 1) == 0;         // trunk forwards, stage 1 backwards, 2 forwards, 3 backwards, A9 forwards: each kernel
+                                           // starts on the data its predecessor wrote last, which is still in L2
         EpiParams E{EPI_PS2, ACT_GELU, h->stage[s], nullptr, 0, 0, (long long)sh * sw * 4 * co, co, 0, 0};
         CU_TRY(conv(h, h->dec[s], pr, *am, E, st, launches));
         sh *= 2; sw *= 2;
@@ -289,6 +291,11 @@ static bool make_act_map(ufnvc_handle *h, ufnvc_handle::ActMap &am, const bf16 *
         if (!tc_make_act_tmap(&am.tm, base, n_img, H, W, C, am.tile_h, am.tile_w, err)) { h->err = err; return false; }
         if (!tc_make_halo_tmap(&am.tm_halo, base, n_img, H, W, C, err)) { h->err = err; return false; }
         am.halo_ok = true;
+        am.halo_t = false;
+        if (halo_prefers_transposed(H, W) && h->use_transposed_tiles) {
+            if (!tc_make_halo_tmap_transposed(&am.tm_halo_t, base, n_img, H, W, C, err)) { h->err = err; return false; }
+            am.halo_t = true;
+        }
     }
     am.ok = true;
     return true;

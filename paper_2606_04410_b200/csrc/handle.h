@@ -22,6 +22,7 @@ struct ufnvc_handle {
     bool pdl = true;                     // programmatic dependent launch along the kernel chain
     bool use_final_is = true;            // A9 input-stationary kernel
     bool use_dw_tma = true;              // A6 TMA-staged kernel
+    bool use_transposed_tiles = true;    // CTA-pair halo conv: 8 x 16 tiles where they pad the image less
     std::string err;
 
     // entropy tables (O3)
@@ -101,6 +102,8 @@ struct ufnvc_handle {
         bool ok = false;
         CUtensorMap tm_halo;             // 3x3 convs: box {64, 10, 18}: a 16 x 8 pixel tile plus halo (conv_halo_kernel)
         bool halo_ok = false;
+        CUtensorMap tm_halo_t;           // the same with the image's y as map dimension 1 (CTA-pair kernel), when that pads to fewer tiles
+        bool halo_t = false;
     };
     ufnvc::FinalMaps final_is;           // A9 input-stationary kernel
     CUtensorMap tm_dw;                   // fa as the depthwise kernel reads it: box {64 ch, 10, 10}

@@ -83,6 +83,8 @@ struct ConvProblem {
     int n_img, H, W;
     int imgs_per_group_cycle; // weight group of image i = (groups == 1) ? 0 : i % groups
     bool taps_are_images = false;   // 1x1 "fold" over T stacked images (R23): tap t reads image img * taps + t of `in` (n_img output images)
+    bool reverse = false;           // CTA-pair halo kernel: walk the schedule backwards -- the tiles the producer kernel wrote last
+                                    // (still in L2) are read first
 };
 
 // ---- kernels (each .cu exposes host launchers; all enqueue on `st` and return cudaGetLastError()) -------------
@@ -227,10 +229,12 @@ cudaError_t launch_colour(const float *in, float *out, long long plane, long lon
 cudaError_t launch_conv_tc(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_in, int tile_h, int tile_w,
                            bool flat, const EpiParams &E, int num_sms, LaunchStream st);
 cudaError_t launch_conv_halo_pair(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
-                                  LaunchStream st);
+                                  LaunchStream st, bool transposed);   // transposed: tmap_halo from tc_make_halo_tmap_transposed
 cudaError_t launch_conv_halo(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
                              LaunchStream st);
 bool tc_make_halo_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, std::string &err);
+bool tc_make_halo_tmap_transposed(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, std::string &err);
+bool halo_prefers_transposed(int H, int W);   // the 16 x 8 halo tile pads the image to fewer tiles as 8 rows x 16 columns
 bool tc_make_weight_tmap(ConvLayer &L, std::string &err, int block_n = 0);   // block_n = 0: widest N tile that divides n_pad
 bool tc_make_act_tmap(CUtensorMap *tm, const bf16 *base, int n_img, int H, int W, int C, int tile_h, int tile_w,
                       std::string &err, bool swizzle = true, int pix_stride = 0);   // pix_stride: elements between pixels (0 = C)
