@@ -367,13 +367,22 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
                         for (int e = 0; e < 8; ++e) f[q * 8 + e] += __bfloat162float(re[e]);
                     }
                 }
+                // A thread owns a pixel row, so every lane of a store touches its own cache line: 256-bit stores (two per 32-column
+                // run instead of four of 128 bits) halve the L1 wavefronts -- the 1x1 unfold conv (A5: 2 k-blocks per 64 KB of output)
+                // is bound by exactly these stores.
+                uint32_t o16[16];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    uint4 o4;
-                    __nv_bfloat162 *oe = reinterpret_cast<__nv_bfloat162 *>(&o4);
+                for (int e = 0; e < 16; ++e) {
+                    const __nv_bfloat162 h2 = __floats2bfloat162_rn(f[2 * e], f[2 * e + 1]);
+                    o16[e] = *reinterpret_cast<const uint32_t *>(&h2);
+                }
+                if ((reinterpret_cast<uintptr_t>(dst) & 31u) == 0) {
+                    st_global_256(dst, o16);
+                    st_global_256(dst + 16, o16 + 8);
+                } else {
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) oe[e] = __floats2bfloat162_rn(f[q * 8 + 2 * e], f[q * 8 + 2 * e + 1]);
-                    reinterpret_cast<uint4 *>(dst)[q] = o4;
+                    for (int q = 0; q < 4; ++q)
+                        reinterpret_cast<uint4 *>(dst)[q] = make_uint4(o16[4 * q], o16[4 * q + 1], o16[4 * q + 2], o16[4 * q + 3]);
                 }
             }
         }
@@ -880,7 +889,7 @@ bool halo_prefers_transposed(int H, int W)
 {
     const long normal = long((H + kHaloTH - 1) / kHaloTH) * ((W + kHaloTW - 1) / kHaloTW);
     const long xposed = long((W + kHaloTH - 1) / kHaloTH) * ((H + kHaloTW - 1) / kHaloTW);
-    return xposed < normal;
+    return xposed < normal && H > kHaloTW;             // (the pair kernel wants more than one tile width along map dimension 1)
 }
 
 // Same activation, dimensions 1 and 2 exchanged: {C, H, W, n_img} with strides {row, pixel, image}; box {64, 10 rows, 18 columns}.
