@@ -234,6 +234,19 @@ long ufnvc_encode_chunk(const ufnvc_handle *h, const uint8_t *idx_host, const in
 int ufnvc_encode_chunk_dev(ufnvc_handle *h, int n_chunks, const uint8_t *idx_dev, const int16_t *sym_dev, uint8_t *bits_dev,
                            size_t cap, uint32_t *sub_off_dev, void *cuda_stream);
 
+/* The same GPU rANS encode (same arguments, same kernels, byte-identical output) for callers that may not allocate device
+ * memory: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The call allocates NOTHING
+ * (no cudaMalloc / cudaFree, no allocating library routine): its scratch is a file-scope __device__ array of
+ * UFNVC_STATIC_SCRATCH_BYTES inside the library, which every GPU that loads the library holds until the process exits.
+ * Limit: the call's scratch -- about 4.1 bytes per symbol of the call (4.22 MB for one 1080p chunk of config 3) -- must
+ * fit the array; a larger call (two 1080p chunks, one 4K chunk) returns UFNVC_E_INVALID_ARG with the byte counts in
+ * ufnvc_last_error and does nothing.  All calls on all handles of a device SHARE the array and it keeps the previous call's
+ * contents (the call clears what must start at zero): two calls that overlap on the GPU -- different streams without an
+ * ordering between them -- race on it; serialise them.  Errors and status bits otherwise as for ufnvc_encode_chunk_dev. */
+#define UFNVC_STATIC_SCRATCH_BYTES (8u << 20)
+int ufnvc_encode_chunk_dev_static(ufnvc_handle *h, int n_chunks, const uint8_t *idx_dev, const int16_t *sym_dev, uint8_t *bits_dev,
+                                  size_t cap, uint32_t *sub_off_dev, void *cuda_stream);
+
 /* ---- chunk ENCODE (R24; only with n_enc_blocks > 0, else UFNVC_E_BAD_CONFIG).  PAPER.md:79:
  * the chunk is patch-embedded to 1/8 resolution, conditioned on C_i and distilled by the chunk encoder into one latent y;
  * r = round(y - mu) is coded with sigma, mu and sigma coming from the DECODER's prior net run on the

@@ -67,6 +67,7 @@ def _load():
         "ufnvc_get_z_prior_index": (i, [vp, vp]),
         "ufnvc_encode_z": (C.c_long, [vp, vp, vp, sz, vp]),
         "ufnvc_encode_chunk_dev": (i, [vp, i, vp, vp, vp, sz, vp, vp]),
+        "ufnvc_encode_chunk_dev_static": (i, [vp, i, vp, vp, vp, sz, vp, vp]),
         "ufnvc_chunk_encode": (i, [vp, i, vp, vp, sz, vp, vp, C.POINTER(ufnvc_enc_taps), vp]),
         "ufnvc_convert_colour": (i, [vp, vp, i, i, i, i, vp]),
         "ufnvc_reset_context": (i, [vp, i, vp]),
@@ -83,7 +84,7 @@ LIB = _load()
 EXPORTS = ("ufnvc_create", "ufnvc_destroy", "ufnvc_load_weights", "ufnvc_chunk_decode", "ufnvc_chunk_decode_ex",
            "ufnvc_entropy_params", "ufnvc_get_status", "ufnvc_last_error", "ufnvc_launches_per_call",
            "ufnvc_chunk_decode_profiled", "ufnvc_debug_counter", "ufnvc_get_cdf", "ufnvc_symbols_from_uniform", "ufnvc_encode_chunk",
-           "ufnvc_decode_z", "ufnvc_chunk_decode_bytes", "ufnvc_get_z_prior_index", "ufnvc_encode_z", "ufnvc_encode_chunk_dev",
+           "ufnvc_decode_z", "ufnvc_chunk_decode_bytes", "ufnvc_get_z_prior_index", "ufnvc_encode_z", "ufnvc_encode_chunk_dev", "ufnvc_encode_chunk_dev_static",
            "ufnvc_reset_context", "ufnvc_get_context", "ufnvc_set_context", "ufnvc_chunk_encode", "ufnvc_convert_colour")
 
 
@@ -306,6 +307,12 @@ class ChunkDecoder:
         self._check(LIB.ufnvc_encode_chunk_dev(self.handle, n, _ptr(idx), _ptr(sym), _ptr(bits), cap, _ptr(off), self._stream(stream)),
                     "ufnvc_encode_chunk_dev")
         return bits, off
+
+    def encode_chunk_dev_static(self, idx, sym, bits, off, stream=None):
+        """ufnvc_encode_chunk_dev_static: the same encode into caller-provided outputs (bits uint8 [cap], off int32 [n * n_sub + 1]);
+        neither this wrapper nor the library call allocates device memory.  Calls sharing a GPU must not overlap."""
+        self._check(LIB.ufnvc_encode_chunk_dev_static(self.handle, idx.shape[0], _ptr(idx), _ptr(sym), _ptr(bits), bits.numel(), _ptr(off),
+                                                      self._stream(stream)), "ufnvc_encode_chunk_dev_static")
 
     def entropy_params(self, z, stream=None):
         n = z.shape[0]

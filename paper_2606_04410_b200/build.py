@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libufnvc.so")
-SOURCES = ["api.cu", "decode.cu", "weights.cu", "tables.cu", "hyper.cu", "rans.cu", "rans_encode.cu", "conv_generic.cu", "conv_tc.cu", "trunk_tc.cu", "final_tc.cu", "mu_steps.cu", "encode.cu"]
+SOURCES = ["api.cu", "decode.cu", "weights.cu", "tables.cu", "hyper.cu", "rans.cu", "rans_encode.cu", "conv_generic.cu", "conv_tc.cu", "trunk_tc.cu", "final_tc.cu", "mu_steps.cu", "encode.cu", "encode_static.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
          "--expt-relaxed-constexpr"]

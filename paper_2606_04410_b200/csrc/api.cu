@@ -128,6 +128,9 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
         delete h;
         return UFNVC_E_CUDA;
     }
+    // the no-allocation encoder's scratch lives in a __device__ array: its address on THIS device (a failure only disables
+    // ufnvc_encode_chunk_dev_static, which then reports it)
+    if (static_scratch_address(&h->static_scratch) != cudaSuccess) { cudaGetLastError(); h->static_scratch = nullptr; }
 
     // O3 tables + search accelerator
     build_cdf_tables(cfg->n_buckets, cfg->scale_min, cfg->scale_max, h->cdf32);

@@ -123,6 +123,9 @@ struct ufnvc_handle {
     uint8_t *enc_stage = nullptr;
     uint32_t *enc_sizes = nullptr;
     size_t enc_tmp_stride = 0, enc_stage_stride = 0;
+    // ufnvc_encode_chunk_dev_static: device address of encode_static.cu's file-scope scratch array on this handle's device
+    // (cudaGetSymbolAddress at create; nullptr if that failed)
+    void *static_scratch = nullptr;
 
     std::vector<void *> allocs;          // workspace and tables, freed at destroy
     std::vector<void *> weight_allocs;   // what ufnvc_load_weights uploaded; freed by the next load and at destroy

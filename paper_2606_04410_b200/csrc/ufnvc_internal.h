@@ -215,6 +215,8 @@ struct RansEncParams {
     uint32_t *status;
 };
 cudaError_t launch_rans_encode(const RansEncParams &p, LaunchStream st);
+// encode_static.cu: device address, on the CURRENT device, of the file-scope scratch array ufnvc_encode_chunk_dev_static uses
+cudaError_t static_scratch_address(void **ptr);
 // NEXT-3 (R22): decoded hyper-latent, channels-last int16 [n][pz][c_z] -> the planar [n][c_z][pz] layout of z_dev
 cudaError_t launch_z_hwc_to_planar(const int16_t *z_hwc, int16_t *z_planar, int n_chunks, int c_z, int pz, LaunchStream st);
 
