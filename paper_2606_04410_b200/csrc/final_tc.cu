@@ -1,19 +1,25 @@
 // A9, input-stationary: the last decoder stage (3x3 conv 64 -> 12, pixel-shuffle x2, clamp, crop, planar fp32) with the
-// nine taps folded into the N dimension of ONE GEMM per input pixel.
+// three COLUMNS of the 3x3 stencil folded into the N dimension of the GEMM and its three ROWS taken by the tensor core from
+// shifted views of the same input tile.
 //
-//   P[p][tap*16 + n] = sum_k X[p][k] * W[tap][n][k]           (tcgen05: M = 128 input pixels, N = 144, K = 64)
-//   conv[n][y][x]    = b[n] + sum_{dy,dx} P[(y+dy-1, x+dx-1)][(3 dy + dx)*16 + n]
+//   R[p][dx*16 + n] = sum_dy sum_k X[p + 32 (dy - 1)][k] * W[dy][dx][n][k]   (tcgen05: M = 128 input pixels, N = 48, K = 3 x 64)
+//   conv[n][y][x]   = b[n] + R[(y, x-1)][n] + R[(y, x)][16 + n] + R[(y, x+1)][32 + n]
 //
-// The output-stationary kernel (conv_halo_kernel<EPI_FINAL>) issues 36 MMAs of N = 16 per 128 pixels and every one of
-// them fetches a 4 KB A operand: it sits at ~80 % of the shared-memory port ("A9 floor").  Here
-// 128 input pixels cost 4 MMAs (9x fewer operand bytes); the price is a shifted sum of the nine partial planes, which
-// lives in different TMEM lanes (= pixels): dx by warp shuffles (a warp is one row of 32 pixels), dy through a small
-// shared-memory exchange between the 12 row-warps of a tile.
+// The output-stationary kernel (conv_halo_kernel<EPI_FINAL>) issues 36 MMAs of N = 16 per 128 pixels and sits at ~80 % of
+// the shared-memory port ("A9 floor").  A first input-stationary version folded all nine taps into N
+// (4 MMAs of N = 144 per 128 pixels), summed the column shifts with 72 warp shuffles per warp and the row shifts through a
+// shared-memory exchange with a barrier between the 12 row warps; clock64 traces showed those warps, then (rows through
+// shifted views, columns through the exchange) the shared-memory port the bound: MMA operand reads, TMA writes, exchange
+// traffic and shuffles all cross it (about 320 KB per tile at 128 B per clock = the 2700-cycle tile period measured).
+// Here a tile row is 32 consecutive pixels of 128 B, so "the pixel one row up / down" is the same buffer viewed from 4 KB
+// earlier / later -- the row shift costs no data movement at all -- and what is left to the warps is the column shift
+// between neighbouring lanes of ONE warp: 24 shuffles, no shared-memory exchange, no barrier, no coupling between warps.
 //
 // Tile = 12 rows x 32 columns of INPUT pixels (window origin one pixel up-left of the 10 x 30 output pixels it yields);
 // one TMA box {64 ch, 32, 12} (zero-filled outside the image = the conv's zero padding) = three 128-row A operands.
 // warp 0 = TMA producer, warp 1 = MMA issuer + TMEM allocator, warps 2..13 = one per tile row (group g = row / 4 reads
-// accumulator g; warp % 4 = TMEM lane quadrant).  Weights of the current frame (18 KB) stay resident in shared memory.
+// accumulator g; warp % 4 = TMEM lane quadrant).  Accumulators are double-buffered over tiles (2 x 3 x 48 columns), the
+// weights of the current frame (18 KB) stay resident in shared memory.
 #include <cuda.h>
 
 #include "tc_ptx.cuh"
@@ -25,25 +31,47 @@ namespace {
 
 constexpr int kFR = 12, kFC = 32;                       // input rows / columns per tile
 constexpr int kFOutR = kFR - 2, kFOutC = kFC - 2;       // output pixels per tile: 10 x 30
-constexpr int kFN = 144;                                // 9 taps x 16 packed output columns
+constexpr int kFN = 48;                                 // 3 stencil columns x 16 packed output columns
+constexpr int kFAccStride = 64;                         // TMEM columns between accumulators (6 of them: 2 buffers x 3 row groups)
 constexpr int kFThreads = 14 * 32;
 constexpr uint32_t kFABytes = kFR * kFC * 128;          // 49152: one input tile, 64 channels
-constexpr uint32_t kFWBytes = kFN * 128;                // 18432: one frame's weights
-constexpr int kFAStages = 2;
-constexpr uint32_t kFXQ = kFR * kFC * 16 * 6;           // exchange buffer: 6 float4 planes x 384 pixels = 36864 B
-constexpr uint32_t kFOffW = kFAStages * kFABytes, kFOffXQ = kFOffW + 2 * 18432, kFOffBar = kFOffXQ + 2 * kFXQ;
+constexpr uint32_t kFWBytes = 9 * 16 * 128;             // 18432: one frame's weights
+constexpr uint32_t kFWdy = 3 * 16 * 128;                // 6144: the 48 rows [dx][n] of one stencil row
+constexpr int kFAStages = 3;
+// The weights sit BEFORE the input stages and 4 KB of padding after them: the views shifted by one tile row (-4 KB / +4 KB) of the
+// first / last row group then read mapped shared memory (values that only reach the tile's halo rows, which produce no output).
+constexpr uint32_t kFOffW = 0, kFOffA = kFWBytes, kFOffBar = kFOffA + kFAStages * kFABytes + 4096;
 constexpr uint32_t kFSmem = kFOffBar + 256 + 1024;
+
+struct FDiv {                                            // division by a runtime constant (tile index -> coordinates)
+    uint32_t d, mul, shr;
+    __device__ __forceinline__ uint32_t div(uint32_t n) const { return (__umulhi(n, mul) + n) >> shr; }
+};
+FDiv make_fdiv(uint32_t d)
+{
+    FDiv f;
+    f.d = d;
+    uint32_t l = 0;
+    while ((1ull << l) < d) ++l;
+    f.mul = uint32_t(((1ull << 32) * ((1ull << l) - d)) / d + 1);
+    f.shr = l;
+    return f;
+}
 
 struct FinalParams {
     int n_img, H, W;             // input images (NHWC bf16, 64 channels)
     int tiles_y, tiles_x, total_tiles;
+    FDiv fd_tx, fd_ty, fd_groups;
     int groups;                  // weight sets (frame index = img % groups)
     const float *bias;           // [groups][16]
     float *out;                  // [n_img][3][out_h][out_w]
     int out_h, out_w;
 };
 
-enum : uint32_t { F_AFULL = 0, F_AEMPTY = 2, F_WFULL = 4, F_WFREE = 5, F_DFULL = 6, F_DEMPTY = 9, F_TMEM = 12 };
+enum : uint32_t {
+    F_AFULL = 0, F_AEMPTY = F_AFULL + kFAStages, F_WFULL = F_AEMPTY + kFAStages, F_WFREE = F_WFULL + 1, F_DFULL = F_WFREE + 1,
+    F_DEMPTY = F_DFULL + 6, F_TMEM = F_DEMPTY + 6
+};
 
 }  // namespace
 
@@ -53,13 +81,12 @@ struct FTile { int img, y0, x0, grp; };     // (y0, x0) = input-window origin = 
 __device__ __forceinline__ FTile f_tile(const FinalParams &p, int tile)
 {
     FTile t;
-    const int tx = tile % p.tiles_x;
-    const int r = tile / p.tiles_x;
-    const int ty = r % p.tiles_y;
-    t.img = r / p.tiles_y;
-    t.y0 = ty * kFOutR - 1;
-    t.x0 = tx * kFOutC - 1;
-    t.grp = p.groups == 1 ? 0 : t.img % p.groups;
+    const uint32_t r = p.fd_tx.div(uint32_t(tile)), tx = uint32_t(tile) - r * p.fd_tx.d;
+    const uint32_t img = p.fd_ty.div(r), ty = r - img * p.fd_ty.d;
+    t.img = int(img);
+    t.y0 = int(ty) * kFOutR - 1;
+    t.x0 = int(tx) * kFOutC - 1;
+    t.grp = p.groups == 1 ? 0 : int(img - p.fd_groups.div(img) * p.fd_groups.d);
     return t;
 }
 
@@ -77,7 +104,7 @@ final_is_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_w) : "memory");
         for (int s = 0; s < kFAStages; ++s) { mbar_init(bar(F_AFULL + s), 1); mbar_init(bar(F_AEMPTY + s), 1); }
         mbar_init(bar(F_WFULL), 1); mbar_init(bar(F_WFREE), 1);
-        for (int g = 0; g < 3; ++g) { mbar_init(bar(F_DFULL + g), 1); mbar_init(bar(F_DEMPTY + g), 4); }
+        for (int a = 0; a < 6; ++a) { mbar_init(bar(F_DFULL + a), 1); mbar_init(bar(F_DEMPTY + a), 4); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) {
@@ -97,7 +124,8 @@ final_is_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant
             int prev_grp = -1;
             for (int tile = blockIdx.x; tile < p.total_tiles; tile += gridDim.x) {
                 const FTile t = f_tile(p, tile);
-                if (t.grp != prev_grp) {                                  // this frame's weights: [144 rows][64 k], resident
+                if (t.grp != prev_grp) {
+                    // this frame's weights, resident: [dy][dx][16 n][64 k] -- the 48 rows (dx, n) of one stencil row dy are one B operand
                     if (prev_grp >= 0) { mbar_wait(bar(F_WFREE), pfree); pfree ^= 1; }
                     mbar_expect_tx(bar(F_WFULL), kFWBytes);
                     tma_load_3d(base + kFOffW, &tm_w, bar(F_WFULL), 0, 0, t.grp);
@@ -105,16 +133,16 @@ final_is_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant
                 }
                 mbar_wait(bar(F_AEMPTY + sa), pa ^ 1);
                 mbar_expect_tx(bar(F_AFULL + sa), kFABytes);
-                tma_load_4d(base + uint32_t(sa) * kFABytes, &tm_in, bar(F_AFULL + sa), 0, t.x0, t.y0, t.img);
+                tma_load_4d(base + kFOffA + uint32_t(sa) * kFABytes, &tm_in, bar(F_AFULL + sa), 0, t.x0, t.y0, t.img);
                 if (++sa == kFAStages) { sa = 0; pa ^= 1; }
             }
         }
     } else if (warp == 1) {
-        // ===================== MMA issuer: 3 accumulators (row groups) x 4 k-steps of N = 144 =====================
+        // ===================== MMA issuer: per tile 3 row groups x (3 row shifts x 4 k-steps) of N = 48 =====================
         if (elect_one()) {
             const uint32_t idesc = umma_idesc_bf16(128, kFN);
             const uint32_t hi = uint32_t(1024 >> 4) | (1u << 14) | (2u << 29);
-            const uint32_t a_lo0 = ((base & 0x3FFFFu) >> 4) | (1u << 16);
+            const uint32_t a_lo0 = (((base + kFOffA) & 0x3FFFFu) >> 4) | (1u << 16);
             const uint32_t w_lo = (((base + kFOffW) & 0x3FFFFu) >> 4) | (1u << 16);
             int sa = 0; uint32_t pa = 0, pw = 0;
             int prev_grp = -1, it = 0;
@@ -124,15 +152,19 @@ final_is_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant
                 mbar_wait(bar(F_AFULL + sa), pa);
                 tc_fence_after();
                 const uint32_t a_lo = a_lo0 + uint32_t(sa) * (kFABytes >> 4);
+                const int buf = it & 1;
 #pragma unroll
                 for (int g = 0; g < 3; ++g) {
-                    mbar_wait(bar(F_DEMPTY + g), (it & 1) ^ 1);           // the row warps of group g have drained accumulator g
+                    mbar_wait(bar(F_DEMPTY + 3 * buf + g), ((it >> 1) & 1) ^ 1);   // the row warps of group g have drained this accumulator
                     tc_fence_after();
 #pragma unroll
-                    for (int k = 0; k < 4; ++k)
-                        umma_bf16_lh(tmem_base + uint32_t(g * kFN), a_lo + uint32_t(g) * (16384 >> 4) + 2 * k, hi, w_lo + 2 * k, hi, idesc,
-                                     uint32_t(k));
-                    umma_commit(bar(F_DFULL + g));
+                    for (int dy = 0; dy < 3; ++dy)
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)                               // view shifted by dy - 1 tile rows = (dy - 1) * 4096 B = 256 units
+                            umma_bf16_lh(tmem_base + uint32_t((3 * buf + g) * kFAccStride),
+                                         a_lo + uint32_t(g) * (16384 >> 4) + uint32_t(256 * dy) - 256u + 2 * k, hi,
+                                         w_lo + uint32_t(dy) * (kFWdy >> 4) + 2 * k, hi, idesc, uint32_t(dy | k));
+                    umma_commit(bar(F_DFULL + 3 * buf + g));
                 }
                 umma_commit(bar(F_AEMPTY + sa));
                 if (++sa == kFAStages) { sa = 0; pa ^= 1; }
@@ -144,8 +176,7 @@ final_is_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant
         // ===================== row warps 2..13: one tile row each =====================
         const int q = warp & 3, g = (warp - 2) >> 2;                       // TMEM lane quadrant (a hardware rule), row group
         const int r = 4 * g + q, cx = lane;
-        const uint32_t t_addr = tmem_base + (uint32_t(q * 32) << 16) + uint32_t(g * kFN);
-        const uint32_t pix = uint32_t(r * kFC + cx);
+        const uint32_t t_row = tmem_base + (uint32_t(q * 32) << 16);
         auto ld16 = [](uint32_t taddr, uint32_t (&v)[16]) {
             asm volatile(
                 "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
@@ -163,55 +194,27 @@ final_is_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant
                 for (int n = 0; n < 12; ++n) bs[n] = __ldg(p.bias + t.grp * 16 + n);
                 bias_grp = t.grp;
             }
-            mbar_wait(bar(F_DFULL + g), it & 1);
+            const int buf = it & 1;
+            mbar_wait(bar(F_DFULL + 3 * buf + g), (it >> 1) & 1);
             tc_fence_after();
-            // Q_dy[n] = sum_dx P[(r, cx + dx - 1)][(dy, dx)][n]: the two side terms come from the neighbouring lanes.  Q_0 and
-            // Q_2 are needed by rows r+1 / r-1, i.e. by other warps: they go straight to shared memory (6 float4 planes x 384
-            // pixels, double-buffered over tiles); only Q_1 stays in registers.
-            const uint32_t xq = base + kFOffXQ + uint32_t(it & 1) * kFXQ;
-            float Q1[12];
-#pragma unroll
-            for (int dy = 0; dy < 3; ++dy) {
-                uint32_t v0[16], v1[16], v2[16];
-                ld16(t_addr + uint32_t((dy * 3 + 0) * 16), v0);
-                ld16(t_addr + uint32_t((dy * 3 + 1) * 16), v1);
-                ld16(t_addr + uint32_t((dy * 3 + 2) * 16), v2);
-                tmem_ld_wait();
-                float Qd[12];
-#pragma unroll
-                for (int n = 0; n < 12; ++n)
-                    Qd[n] = __shfl_up_sync(0xFFFFFFFFu, __uint_as_float(v0[n]), 1) + __uint_as_float(v1[n]) +
-                            __shfl_down_sync(0xFFFFFFFFu, __uint_as_float(v2[n]), 1);
-                if (dy == 1) {
-#pragma unroll
-                    for (int n = 0; n < 12; ++n) Q1[n] = Qd[n];
-                } else {
-#pragma unroll
-                    for (int c4 = 0; c4 < 3; ++c4)
-                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};"
-                                     ::"r"(xq + uint32_t(3 * (dy >> 1) + c4) * (kFR * kFC * 16) + pix * 16u), "f"(Qd[4 * c4]), "f"(Qd[4 * c4 + 1]),
-                                       "f"(Qd[4 * c4 + 2]), "f"(Qd[4 * c4 + 3]) : "memory");
-                }
-            }
+            // R_dx of this pixel: columns [16 dx, 16 dx + 12) of the accumulator.  The output pixel (y, x) takes R_0 from the pixel to
+            // its left and R_2 from the pixel to its right: the neighbouring lanes of this warp.
+            uint32_t r0[16], r1[16], r2[16];
+            const uint32_t t_acc = t_row + uint32_t((3 * buf + g) * kFAccStride);
+            ld16(t_acc, r0);
+            ld16(t_acc + 16, r1);
+            ld16(t_acc + 32, r2);
+            tmem_ld_wait();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar(F_DEMPTY + g));                  // accumulator g may be overwritten
-            asm volatile("bar.sync 1, 384;" ::: "memory");                 // the 12 row warps
+            if (lane == 0) mbar_arrive(bar(F_DEMPTY + 3 * buf + g));        // the accumulator may be overwritten (by tile it + 2)
+            float o[12];
+#pragma unroll
+            for (int n = 0; n < 12; ++n)
+                o[n] = bs[n] + __shfl_up_sync(0xFFFFFFFFu, __uint_as_float(r0[n]), 1) + __uint_as_float(r1[n]) +
+                       __shfl_down_sync(0xFFFFFFFFu, __uint_as_float(r2[n]), 1);
             const int y = t.y0 + r, x = t.x0 + cx;
             if (r >= 1 && r <= kFOutR && cx >= 1 && cx <= kFOutC && y < p.H && x < p.W) {
-                float o[12];
-#pragma unroll
-                for (int c4 = 0; c4 < 3; ++c4) {
-                    float4 up, dn;                                         // Q[0] of row r-1, Q[2] of row r+1
-                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(up.x), "=f"(up.y), "=f"(up.z), "=f"(up.w)
-                                 : "r"(xq + uint32_t(c4) * (kFR * kFC * 16) + (pix - kFC) * 16u));
-                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(dn.x), "=f"(dn.y), "=f"(dn.z), "=f"(dn.w)
-                                 : "r"(xq + uint32_t(3 + c4) * (kFR * kFC * 16) + (pix + kFC) * 16u));
-                    o[4 * c4 + 0] = bs[4 * c4 + 0] + up.x + Q1[4 * c4 + 0] + dn.x;
-                    o[4 * c4 + 1] = bs[4 * c4 + 1] + up.y + Q1[4 * c4 + 1] + dn.y;
-                    o[4 * c4 + 2] = bs[4 * c4 + 2] + up.z + Q1[4 * c4 + 2] + dn.z;
-                    o[4 * c4 + 3] = bs[4 * c4 + 3] + up.w + Q1[4 * c4 + 3] + dn.w;
-                }
                 // packed column n = (2i + j) * 3 + c -> out[img][c][2y + i][2x + j] (R14), clamp (O9), crop
                 float *ob = p.out + (long long)t.img * 3 * p.out_h * p.out_w;
                 const int ox = 2 * x;
@@ -253,7 +256,7 @@ bool final_make_maps(FinalMaps &m, const ConvLayer &L, const bf16 *in_base, int 
     if (!final_is_eligible(L, out_w)) return true;
     if (!tc_make_act_tmap(&m.tm_in, in_base, n_img, H, W, 64, kFR, kFC, err)) return false;
     // weights [group][tap][16][64] bf16 are [group][144][64]: one box = one frame's whole weight set
-    if (!tc_encode_3d(&m.tm_w, L.w, 64, kFN, (unsigned long long)L.groups, 64, kFN, 1, err)) return false;
+    if (!tc_encode_3d(&m.tm_w, L.w, 64, 144, (unsigned long long)L.groups, 64, 144, 1, err)) return false;
     m.ok = true;
     return true;
 }
@@ -271,6 +274,7 @@ cudaError_t launch_final_is(const FinalMaps &m, const ConvLayer &L, int n_img, i
     p.tiles_y = (H + kFOutR - 1) / kFOutR;
     p.tiles_x = (W + kFOutC - 1) / kFOutC;
     p.total_tiles = n_img * p.tiles_y * p.tiles_x;
+    p.fd_tx = make_fdiv(uint32_t(p.tiles_x)); p.fd_ty = make_fdiv(uint32_t(p.tiles_y)); p.fd_groups = make_fdiv(uint32_t(L.groups));
     p.groups = L.groups;
     p.bias = L.bias;
     p.out = out; p.out_h = out_h; p.out_w = out_w;

@@ -250,6 +250,7 @@ bool tc_encode_3d(CUtensorMap *tm, const void *base, unsigned long long d0, unsi
 // A9, input-stationary (final_tc.cu): 9 taps folded into N, shifted sum of the partial planes in the epilogue
 struct FinalMaps {
     CUtensorMap tm_in, tm_w;
+    const bf16 *in_base = nullptr;
     bool ok = false;
 };
 bool final_make_maps(FinalMaps &m, const ConvLayer &L, const bf16 *in_base, int n_img, int H, int W, int out_w, std::string &err);
