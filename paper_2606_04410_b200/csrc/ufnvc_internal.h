@@ -129,6 +129,18 @@ inline cudaError_t launch_pdl_grid(void (*kern)(KArgs...), dim3 grid, unsigned b
     return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl_grid_smem(void (*kern)(KArgs...), dim3 grid, unsigned block, size_t smem, LaunchStream st, Args &&...args)   // 3-D grid + dynamic smem
+{
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = st.s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = st.pdl ? 1u : 0u;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 // cudaFuncSetAttribute(MaxDynamicSharedMemorySize) for every kernel of a translation unit that needs more than 48 KB, on the
 // CURRENT device.  Function attributes are per device: ufnvc_create calls all of these for the device the handle lives on, so
 // the launchers hold no "already configured" state (a second handle on another GPU of the same process configures that GPU).
