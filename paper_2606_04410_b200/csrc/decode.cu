@@ -321,7 +321,10 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
     for (auto &tb : h->trunk) ok = ok && tc_make_weight_tmap(tb.pw1, err) && tc_make_weight_tmap(tb.pw2, err);
     for (int s = 0; s < 4; ++s) ok = ok && tc_make_weight_tmap(h->dec[s], err);
     if (h->has_ctx) {
-        ok = ok && tc_make_weight_tmap(h->ctx_fold, err) && tc_make_weight_tmap(h->ctx_out, err);
+        // the fold over T has K = T c_trunk on only h w / 128 pixel tiles per chunk: halve the n tile when that leaves SMs without
+        // work (each CTA then streams half the weight bytes of its long K loop)
+        const int fold_bn = (long long)h->max_chunks * h->h * h->w / 128 * (c.c_trunk / 256) <= h->num_sms / 2 ? 128 : 0;
+        ok = ok && tc_make_weight_tmap(h->ctx_fold, err, fold_bn) && tc_make_weight_tmap(h->ctx_out, err);
         for (auto &tb : h->ctx_blocks) ok = ok && tc_make_weight_tmap(tb.pw1, err) && tc_make_weight_tmap(tb.pw2, err);
     }
     for (int k = 0; k < 3 && c.mu_steps == 4; ++k) ok = ok && tc_make_weight_tmap(h->mu_net[k], err);
@@ -350,7 +353,8 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
              tc_make_act_tmap(&h->tm_dw_ctx, h->ca, n, h->h, h->w, c.c_trunk, 10, 10, h->err, /*swizzle=*/false);
     if (ok && h->has_enc) {
         // encoder (R24): patches [n T][H/8][W/8][192], embedded + space-to-depth x2 [n T][h][w][4 c_trunk]
-        ok = tc_make_weight_tmap(h->enc_patch, err) && tc_make_weight_tmap(h->enc_fold, err) && tc_make_weight_tmap(h->enc_y, err);
+        const int fold_bn = (long long)h->max_chunks * h->h * h->w / 128 * (c.c_trunk / 256) <= h->num_sms / 2 ? 128 : 0;
+        ok = tc_make_weight_tmap(h->enc_patch, err) && tc_make_weight_tmap(h->enc_fold, err, fold_bn) && tc_make_weight_tmap(h->enc_y, err);
         for (auto &tb : h->enc_blocks) ok = ok && tc_make_weight_tmap(tb.pw1, err) && tc_make_weight_tmap(tb.pw2, err);
         if (!ok) return fail(h, UFNVC_E_CUDA, err);
         ok = make_act_map(h, h->am_p8, h->p8, n * T, 2 * h->h, 2 * h->w, 192, false, T) &&
