@@ -92,6 +92,7 @@ typedef struct ufnvc_config {
 #define UFNVC_DBG_GENERIC_FINAL 0x40u   /* A9 on the output-stationary halo conv kernel instead of the input-stationary one */
 #define UFNVC_DBG_PLAIN_DEPTHWISE 0x80u /* A6 on the register-only kernel (no TMA staging, no tile counters) */
 #define UFNVC_DBG_NO_TRANSPOSED_TILES 0x100u /* A8 / head: 16 x 8 pixel tiles only (never the 8 x 16 transposed tile map) */
+#define UFNVC_DBG_NO_QUAD_CLUSTERS 0x200u /* A7: every cluster one CTA pair (no weight multicast between two pairs) */
 
 /* Optional device buffers that receive intermediates of ufnvc_chunk_decode_ex (parity/debug; any may be NULL).
  * Layouts are the library's own: channels-last. */

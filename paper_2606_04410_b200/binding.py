@@ -90,7 +90,7 @@ EXPORTS = ("ufnvc_create", "ufnvc_destroy", "ufnvc_load_weights", "ufnvc_chunk_d
 
 # ufnvc_config.debug_flags (include/ufnvc.h)
 DBG = dict(force_generic=0x01, no_pdl=0x02, no_tail_fill=0x04, fp64_head=0x08, no_cta_pairs=0x10, unfused_trunk=0x20,
-           generic_final=0x40, plain_depthwise=0x80, no_transposed_tiles=0x100)
+           generic_final=0x40, plain_depthwise=0x80, no_transposed_tiles=0x100, no_quad_clusters=0x200)
 
 
 def make_config(cfg, max_chunks: int | None = None, debug_flags: int = 0) -> ufnvc_config:

@@ -50,7 +50,7 @@ int validate(const ufnvc_config &c, std::string &why)
     BAD(c.weight_dtype != 0 && c.weight_dtype != 1, "weight_dtype must be 0 or 1");
     BAD(c.mu_steps != 1 && c.mu_steps != 4, "mu_steps must be 1 or 4");
     BAD(c.mu_steps == 4 && c.c_y % 32, "mu_steps == 4 needs c_y % 32 == 0 (the mean convs run on tensor cores only)");
-    BAD(c.debug_flags & ~0x1FFu, "unknown debug_flags bit");
+    BAD(c.debug_flags & ~0x3FFu, "unknown debug_flags bit");
     BAD(c.n_ctx_blocks < 0 || c.n_ctx_blocks > 64, "n_ctx_blocks out of range");
     BAD(c.n_ctx_blocks > 0 && (c.c_trunk != 256 || (c.c_trunk * c.trunk_expand) % 128 || c.c_y % 64 || c.weight_dtype != 1 ||
                                c.c_hyper % 16 || c.c_z % 16),
@@ -114,6 +114,7 @@ extern "C" int ufnvc_create(const ufnvc_config *cfg, ufnvc_handle **out)
     h->use_final_is = !(dbg & UFNVC_DBG_GENERIC_FINAL);
     h->use_dw_tma = !(dbg & UFNVC_DBG_PLAIN_DEPTHWISE);
     h->use_transposed_tiles = !(dbg & UFNVC_DBG_NO_TRANSPOSED_TILES);
+    h->use_quad_clusters = !(dbg & UFNVC_DBG_NO_QUAD_CLUSTERS);
     h->hybrid_head = !(dbg & UFNVC_DBG_FP64_HEAD) && cfg->weight_dtype == 1 && cfg->c_y % 32 == 0 && cfg->c_hyper % 32 == 0 &&
                      !h->force_generic;
     // Error model of the tensor-core head (R12): ln sigma = sum of K = 9 * 2 c_hyper exact bf16 x bf16 products

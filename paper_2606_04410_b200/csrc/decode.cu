@@ -175,7 +175,7 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
         if (sg && sg->dw) { cudaEventRecord(sg->dw[2 * k], st); }
         if (fused_ok) {
             CU_TRY(launch_trunk_mlp(tb.fused, tb.pw1, tb.pw2, h->fa, h->fa, (long long)n * T * P, h->num_sms, h->use_pair_trunk, st,
-                                    mlp_counts ? sync_k + 1 : nullptr));
+                                    mlp_counts ? sync_k + 1 : nullptr, h->use_quad_clusters));
             if (launches) ++*launches;
             continue;
         }
@@ -236,7 +236,7 @@ int run(ufnvc_handle *h, int n, const int16_t *z, const uint8_t *bits, size_t bi
             CU_TRY(launch_dwconv3x3_tma(h->tm_dw_ctx, h->cb, tb.dw_w, tb.dw_b, n, h->h, h->w, Ct, h->num_sms, st, h->tail_fill ? sync_k : nullptr,
                                         (k > 0 && mlp_counts) ? sync_k - h->trunk_sync_stride + 1 : nullptr));
             CU_TRY(launch_trunk_mlp(tb.fused, tb.pw1, tb.pw2, h->ca, h->ca, (long long)n * P, h->num_sms, h->use_pair_trunk, st,
-                                    mlp_counts ? sync_k + 1 : nullptr));
+                                    mlp_counts ? sync_k + 1 : nullptr, h->use_quad_clusters));
             *launches += 2;
         }
         {
@@ -683,7 +683,7 @@ extern "C" int ufnvc_chunk_encode(ufnvc_handle *h, int n_chunks, const float *fr
         CU_TRY(launch_dwconv3x3_tma(h->tm_dw_ctx, h->cb, tb.dw_w, tb.dw_b, n, h->h, h->w, Ct, h->num_sms, st, h->tail_fill ? sync_k : nullptr,
                                     (k > 0 && mlp_counts) ? sync_k - h->trunk_sync_stride + 1 : nullptr));
         CU_TRY(launch_trunk_mlp(tb.fused, tb.pw1, tb.pw2, h->ca, h->ca, (long long)n * P, h->num_sms, h->use_pair_trunk, st,
-                                mlp_counts ? sync_k + 1 : nullptr));
+                                mlp_counts ? sync_k + 1 : nullptr, h->use_quad_clusters));
         launches += 2;
     }
     // E5: latent head, fp32 out

@@ -23,6 +23,7 @@ struct ufnvc_handle {
     bool use_final_is = true;            // A9 input-stationary kernel
     bool use_dw_tma = true;              // A6 TMA-staged kernel
     bool use_transposed_tiles = true;    // CTA-pair halo conv: 8 x 16 tiles where they pad the image less
+    bool use_quad_clusters = true;       // fused MLP kernel: clusters of two CTA pairs sharing the weight tiles by multicast
     std::string err;
 
     // entropy tables (O3)

@@ -264,6 +264,31 @@ __device__ __forceinline__ void umma2_commit_both(uint32_t bar)
                  ::"r"(bar), "h"((unsigned short)3) : "memory");
 }
 
+// the same with an explicit CTA mask (clusters of two pairs: bits 2p, 2p + 1 = pair p; all four = every CTA of the cluster)
+__device__ __forceinline__ void umma2_commit_mask(uint32_t bar, uint32_t mask)
+{
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(bar), "h"((unsigned short)mask) : "memory");
+}
+// TMA load multicast to the CTAs of `mask`: data and completion bytes land at the SAME CTA-relative offsets (dst, bar) in each
+__device__ __forceinline__ void tma_load_2d_mcast(uint32_t dst, const CUtensorMap *tm, uint32_t bar, int c0, int c1, uint32_t mask)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1, {%3, %4}], [%2], %5;"
+        ::"r"(dst), "l"(tm), "r"(bar), "r"(c0), "r"(c1), "h"((unsigned short)mask)
+        : "memory");
+}
+__device__ __forceinline__ uint32_t cluster_nctarank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void mbar_arrive_cluster_release(uint32_t cluster_addr)
+{
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+
 }  // namespace
 }  // namespace ufnvc
 

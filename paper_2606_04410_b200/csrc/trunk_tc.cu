@@ -31,8 +31,8 @@ constexpr int kC = 256;                  // trunk width: K of GEMM1, N of GEMM2
 constexpr int kHC = 128;                 // hidden columns per chunk
 constexpr int kTM = 128;                 // pixels per tile
 constexpr int kTrunkThreads = 320;       // single-CTA kernel: TMA warp, MMA warp, 8 epilogue warps
-constexpr int kPairThreads = 448;        // CTA-pair kernel: TMA warp, MMA warp, 4 GELU warps, 8 drain warps
-static_assert(kPairThreads / 32 - 6 == int(kTrunkTileSignals), "one tile_done increment per drain warp (warps 6..13)");
+constexpr int kPairThreads = 512;        // CTA-pair kernel: weight TMA warp, MMA warp, 4 GELU warps, 8 drain warps, relay warp, input-tile TMA warp
+static_assert(kPairThreads / 32 - 8 == int(kTrunkTileSignals), "one tile_done increment per drain warp (warps 6..13)");
 constexpr int kWStages = 3;
 constexpr uint32_t kSlab = 16384;        // 128 rows x 128 B
 constexpr uint32_t kWStage = 32768;
@@ -373,22 +373,32 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
     constexpr uint32_t offW = TMH ? kOffHs : kOffW, offBar = offW + NS * kWStage;
     // HS_FULL: one barrier per Hacc buffer and 32-column sub-step of a chunk (2 x 4)
     constexpr uint32_t B_WFULL = 2, B_WEMPTY = B_WFULL + NS, B_HACC_FULL = B_WEMPTY + NS, B_HS_FULL = B_HACC_FULL + 2,
-                       B_OFULL = B_HS_FULL + 8, B_OEMPTY = B_OFULL + 1, B_TMEM_SLOT = B_OEMPTY + 1;   // (shadow the file-scope slots)
+                       B_OFULL = B_HS_FULL + 8, B_OEMPTY = B_OFULL + 1, B_PFULL = B_OEMPTY + 1, B_TMEM_SLOT = B_PFULL + NS;   // (shadow the file-scope slots)
     auto bar = [&](uint32_t slot) { return base + offBar + 8u * slot; };
     volatile uint32_t *tmem_slot_ptr =
         reinterpret_cast<volatile uint32_t *>(smem_raw + (bar(B_TMEM_SLOT) - smem_u32(smem_raw)));
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t rank = cluster_ctarank();
+    // Cluster = one CTA pair, or (preferred cluster dimension, where the GPC has room) TWO pairs that share every weight tile: each
+    // of the four CTAs then fetches a quarter of it and multicasts it to its counterpart in the other pair, which halves the
+    // L2 -> SM weight traffic -- the kernel moves 704 KB per CTA and tile pair, and at the tensor pipe's rate that is the whole
+    // chip's L2 output bandwidth.  The pairs of a cluster walk the weight ring in lockstep; a pair that has run out
+    // of tiles computes a padding tile (rows past n_px: zero-filled loads, masked stores).
+    const uint32_t rank = cluster_ctarank(), nranks = cluster_nctarank();
+    const uint32_t hb = rank & 1u, leader = rank & ~1u, pc = rank >> 1;      // half of the pair, the pair's MMA-issuing CTA, pair in cluster
+    const bool quad = nranks == 4;
+    const uint32_t pair_mask = 3u << (2 * pc), all_mask = quad ? 0xFu : 0x3u;
     const int NC = p.n_chunks;
     const int n_pairs = gridDim.x >> 1, pair0 = blockIdx.x >> 1;
     const int n_ptiles = (p.n_tiles + 1) >> 1;                       // tile pairs; a missing odd tile is all padding
+    const int first_pair = pair0 - int(pc);                          // the cluster's first pair has the most tiles: its count is everyone's
+    const int rounds = first_pair < n_ptiles ? (n_ptiles - first_pair + n_pairs - 1) / n_pairs : 0;
 
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_d) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_w1h) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_w2h) : "memory");
         mbar_init(bar(B_AFULL), 1); mbar_init(bar(B_AEMPTY), 1);
-        for (int s = 0; s < NS; ++s) { mbar_init(bar(B_WFULL + s), 1); mbar_init(bar(B_WEMPTY + s), 1); }
+        for (int s = 0; s < NS; ++s) { mbar_init(bar(B_WFULL + s), 1); mbar_init(bar(B_WEMPTY + s), quad ? 2 : 1); mbar_init(bar(B_PFULL + s), 2); }
         for (int b = 0; b < 2; ++b) {
             mbar_init(bar(B_HACC_FULL + b), 1);
             for (int q = 0; q < 4; ++q) mbar_init(bar(B_HS_FULL + 4 * b + q), 8);         // 4 GELU warps x 2 CTAs per sub-step
@@ -408,35 +418,41 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
     pdl_grid_sync();                                                 // the predecessor kernel's output is complete and visible from here on
 
     if (warp == 0) {
-        // ===================== TMA producer (both CTAs): own d tile, own half of every weight tile =====================
+        // ===================== weight producer (both CTAs): own half of every weight tile (a quarter, multicast, in two-pair clusters) ====
         if (elect_one()) {
-            const uint32_t afull_l = mapa_rank(bar(B_AFULL), 0);     // the leader's barriers, as cluster addresses
-            int ws = 0; uint32_t wp = 0, ap = 0;
+            const uint32_t mc_mask = (1u << rank) | (1u << (rank ^ 2u));   // this CTA and its counterpart in the other pair
+            int ws = 0; uint32_t wp = 0;
             auto w_slot = [&](uint32_t &full_l) {
-                mbar_wait(bar(B_WEMPTY + ws), wp ^ 1);                // local: multicast commit of the MMAs that read it
-                if (rank == 0) mbar_expect_tx(bar(B_WFULL + ws), 2 * kWStage);
-                full_l = mapa_rank(bar(B_WFULL + ws), 0);
+                mbar_wait_cluster(bar(B_WEMPTY + ws), wp ^ 1);        // local: multicast commit of the MMAs (of every pair) that read it
+                if (quad) {                                           // own quarter + the counterpart's quarter land here
+                    mbar_expect_tx(bar(B_WFULL + ws), kWStage);
+                    full_l = bar(B_WFULL + ws);
+                } else {
+                    if (hb == 0) mbar_expect_tx(bar(B_WFULL + ws), 2 * kWStage);
+                    full_l = mapa_rank(bar(B_WFULL + ws), leader);
+                }
                 return base + offW + uint32_t(ws) * kWStage;
             };
             auto w_next = [&]() { if (++ws == NS) { ws = 0; wp ^= 1; } };
             auto load_w1 = [&](int c) {                               // rows c*128 + rank*64 .. +63 of W1, 4 k slabs of 8 KB
                 uint32_t full_l;
                 const uint32_t dst = w_slot(full_l);
-                for (int s = 0; s < 4; ++s) tma_load_2d_pair(dst + uint32_t(s) * (kSlab / 2), &tm_w1h, full_l, s * 64, c * kHC + int(rank) * 64);
+                if (quad) {                                           // k slabs 2 pc, 2 pc + 1 of this half, to both pairs
+                    for (int s = 2 * int(pc); s < 2 * int(pc) + 2; ++s)
+                        tma_load_2d_mcast(dst + uint32_t(s) * (kSlab / 2), &tm_w1h, full_l, s * 64, c * kHC + int(hb) * 64, mc_mask);
+                } else {
+                    for (int s = 0; s < 4; ++s) tma_load_2d_pair(dst + uint32_t(s) * (kSlab / 2), &tm_w1h, full_l, s * 64, c * kHC + int(hb) * 64);
+                }
                 w_next();
             };
             auto load_w2 = [&](int c) {                               // rows rank*128 .. +127 of W2, k slabs c*128 + {0, 64}
                 uint32_t full_l;
                 const uint32_t dst = w_slot(full_l);
-                for (int j = 0; j < 2; ++j) tma_load_2d_pair(dst + uint32_t(j) * kSlab, &tm_w2h, full_l, c * kHC + j * 64, int(rank) * 128);
+                if (quad) tma_load_2d_mcast(dst + pc * kSlab, &tm_w2h, full_l, c * kHC + int(pc) * 64, int(hb) * 128, mc_mask);
+                else for (int j = 0; j < 2; ++j) tma_load_2d_pair(dst + uint32_t(j) * kSlab, &tm_w2h, full_l, c * kHC + j * 64, int(hb) * 128);
                 w_next();
             };
-            for (int pt = pair0; pt < n_ptiles; pt += n_pairs) {
-                const int tile = 2 * pt + int(rank);
-                mbar_wait(bar(B_AEMPTY), ap ^ 1);
-                if (rank == 0) mbar_expect_tx(bar(B_AFULL), 2 * 4 * kSlab);
-                for (int s = 0; s < 4; ++s) tma_load_2d_pair(base + kOffA + s * kSlab, &tm_d, afull_l, s * 64, tile * kTM);
-                ap ^= 1;
+            for (int j = 0; j < rounds; ++j) {
                 load_w1(0);
                 if (!TMH && NC > 1) load_w1(1);
                 for (int c = 0; c < NC; ++c) {                     // the order the MMA warp consumes them in
@@ -447,7 +463,7 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
         }
     } else if (warp == 1) {
         // ===================== MMA issuer: leader CTA only =====================
-        if (rank == 0 && elect_one()) {
+        if (hb == 0 && elect_one()) {
             const uint32_t idesc1 = umma_idesc_bf16(2 * kTM, kHC), idesc2 = umma_idesc_bf16(2 * kTM, kC);
             const uint32_t hi = uint32_t(1024 >> 4) | (1u << 14) | (2u << 29);
             auto lo = [](uint32_t addr) { return ((addr & 0x3FFFFu) >> 4) | (1u << 16); };
@@ -455,12 +471,12 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
             const uint32_t o_acc = tmem_base, h_acc = tmem_base + kC;
             int ws = 0; uint32_t wp = 0;
             uint32_t ph_hs = 0;
-            auto w_wait = [&]() {
-                mbar_wait_cluster(bar(B_WFULL + ws), wp);
+            auto w_wait = [&]() {                                     // (two pairs: both CTAs' relay warps have seen their halves land)
+                mbar_wait_cluster(bar((quad ? B_PFULL : B_WFULL) + ws), wp);
                 tc_fence_after();
                 return w_lo + uint32_t(ws) * (kWStage >> 4);
             };
-            auto w_release = [&]() { umma2_commit_both(bar(B_WEMPTY + ws)); if (++ws == NS) { ws = 0; wp ^= 1; } };
+            auto w_release = [&]() { umma2_commit_mask(bar(B_WEMPTY + ws), all_mask); if (++ws == NS) { ws = 0; wp ^= 1; } };
             auto gemm1 = [&](int c) {
                 const int b = c & 1;
                 // Hacc[b] is released by GEMM2(c-2), in issue order (the tensor pipe executes in order)
@@ -473,20 +489,20 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
                         umma2_bf16_lh(d, a_lo + uint32_t(s) * (kSlab >> 4) + 2 * k, hi, w + uint32_t(s) * (kSlab >> 5) + 2 * k, hi, idesc1,
                                       uint32_t(s | k));
                 w_release();
-                umma2_commit_both(bar(B_HACC_FULL + b));
+                umma2_commit_mask(bar(B_HACC_FULL + b), pair_mask);
             };
             int it = 0;
-            for (int pt = pair0; pt < n_ptiles; pt += n_pairs, ++it) {
+            for (; it < rounds; ++it) {
                 mbar_wait_cluster(bar(B_AFULL), it & 1);
                 tc_fence_after();
                 constexpr int LA = TMH ? 1 : 2;                           // GEMM1 lookahead (chunks)
                 gemm1(0);
                 if (LA == 2 && NC > 1) gemm1(1);
-                if (NC <= LA) umma2_commit_both(bar(B_AEMPTY));
+                if (NC <= LA) umma2_commit_mask(bar(B_AEMPTY), pair_mask);
                 for (int c = 0; c < NC; ++c) {
                     if (c + LA < NC) {
                         gemm1(c + LA);
-                        if (c + LA + 1 == NC) umma2_commit_both(bar(B_AEMPTY));
+                        if (c + LA + 1 == NC) umma2_commit_mask(bar(B_AEMPTY), pair_mask);
                     }
                     const int b = c & 1;
                     const uint32_t hs_par = (ph_hs >> b) & 1;
@@ -513,7 +529,34 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
                     }
                     w_release();
                 }
-                umma2_commit_both(bar(B_OFULL));
+                umma2_commit_mask(bar(B_OFULL), pair_mask);
+            }
+        }
+    } else if (warp == 15) {
+        // ===================== input-tile producer (both CTAs): own d tile.  A thread of its own: behind the weight loads in one
+        // program order, a pair waiting for its A buffer would hold back the weight quarters the OTHER pair of the cluster needs.
+        if (elect_one()) {
+            const uint32_t afull_l = mapa_rank(bar(B_AFULL), leader);     // the leader's barrier, as a cluster address
+            uint32_t ap = 0;
+            for (int j = 0; j < rounds; ++j) {
+                const int tile = 2 * (pair0 + j * n_pairs) + int(hb);  // past n_tiles: an all-padding tile (zero-filled by TMA)
+                mbar_wait(bar(B_AEMPTY), ap ^ 1);
+                if (hb == 0) mbar_expect_tx(bar(B_AFULL), 2 * 4 * kSlab);
+                for (int s = 0; s < 4; ++s) tma_load_2d_pair(base + kOffA + s * kSlab, &tm_d, afull_l, s * 64, tile * kTM);
+                ap ^= 1;
+            }
+        }
+    } else if (warp == 14) {
+        // ===================== relay (clusters of two pairs): this CTA's half of a weight stage has landed -> tell the pair's leader ====
+        // A multicast TMA signals the barrier at the same offset in each destination CTA, so the leader cannot be told directly.
+        if (quad && lane == 0) {
+            const uint32_t pfull_l = mapa_rank(bar(B_PFULL), leader);
+            int ws = 0; uint32_t wp = 0;
+            const int uses = rounds * 2 * NC;
+            for (int u = 0; u < uses; ++u) {
+                mbar_wait_cluster(bar(B_WFULL + ws), wp);
+                mbar_arrive_cluster(pfull_l + 8u * uint32_t(ws));          // (relaxed: the bytes are in shared memory before the barrier flips)
+                if (++ws == NS) { ws = 0; wp ^= 1; }
             }
         }
     } else {
@@ -528,9 +571,9 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
         const int r = quad * 32 + lane;
         const uint32_t t_lane = tmem_base + (uint32_t(quad * 32) << 16);
         if (warp < 6) {
-            const uint32_t hs_full_l = mapa_rank(bar(B_HS_FULL), 0);
+            const uint32_t hs_full_l = mapa_rank(bar(B_HS_FULL), leader);
             uint32_t ph_use = 0;
-            for (int pt = pair0; pt < n_ptiles; pt += n_pairs) {
+            for (int j = 0; j < rounds; ++j) {
                 for (int c = 0; c < NC; ++c) {
                     const int b = c & 1;
                     mbar_wait(bar(B_HACC_FULL + b), (ph_use >> b) & 1);
@@ -562,10 +605,9 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
             }
         } else {
             const int half = (warp - 6) >> 2;                            // output columns [128 half, +128)
-            const uint32_t oempty_l = mapa_rank(bar(B_OEMPTY), 0);
-            int it = 0;
-            for (int pt = pair0; pt < n_ptiles; pt += n_pairs, ++it) {
-                const int tile = 2 * pt + int(rank);
+            const uint32_t oempty_l = mapa_rank(bar(B_OEMPTY), leader);
+            for (int it = 0; it < rounds; ++it) {
+                const int tile = 2 * (pair0 + it * n_pairs) + int(hb);
                 const long long row = (long long)tile * kTM + r;
                 const bool inb = row < p.n_px;
                 // residual row segment (128 columns = 8 x 32 B), fetched BEFORE the wait for the last GEMM2s.  A thread is a
@@ -619,7 +661,7 @@ trunk_mlp_pair_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_con
                 __syncwarp();
                 // tail filling: the depthwise kernel of the next trunk block polls these counters instead of waiting for the
                 // whole grid (the __syncwarp above orders every lane's stores before lane 0's release)
-                if (p.tile_done && lane == 0) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p.tile_done + tile) : "memory");
+                if (p.tile_done && lane == 0 && tile < p.n_tiles) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p.tile_done + tile) : "memory");
             }
         }
     }
@@ -667,7 +709,7 @@ cudaError_t configure_trunk_kernels()
 }
 
 cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const ConvLayer &pw2, const bf16 *x, bf16 *out, long long n_px,
-                             int num_sms, bool pair, LaunchStream st, uint32_t *tile_done)
+                             int num_sms, bool pair, LaunchStream st, uint32_t *tile_done, bool quad_clusters)
 {
     TrunkParams p{};
     p.tile_done = tile_done;
@@ -685,7 +727,25 @@ cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const Con
     if (pair && p.n_tiles >= 2) {
         const int n_ptiles = (p.n_tiles + 1) / 2;
         const int clusters = n_ptiles < num_sms / 2 ? n_ptiles : num_sms / 2;
-        return launch_pdl(trunk_mlp_pair_kernel, 2 * clusters, kPairThreads, kTrunkSmem, st, 2, m.tm_d, m.tm_w1h, m.tm_w2h, p);
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(unsigned(2 * clusters)); cfg.blockDim = dim3(kPairThreads); cfg.dynamicSmemBytes = kTrunkSmem; cfg.stream = st.s;
+        cudaLaunchAttribute attr[3];
+        unsigned na = 0;
+        attr[na].id = cudaLaunchAttributeClusterDimension;
+        attr[na].val.clusterDim.x = 2; attr[na].val.clusterDim.y = 1; attr[na].val.clusterDim.z = 1;
+        ++na;
+        if (quad_clusters && clusters % 2 == 0) {                   // two pairs per cluster where the GPC has room, one pair elsewhere
+            attr[na].id = cudaLaunchAttributePreferredClusterDimension;
+            attr[na].val.preferredClusterDim.x = 4; attr[na].val.preferredClusterDim.y = 1; attr[na].val.preferredClusterDim.z = 1;
+            ++na;
+        }
+        if (st.pdl) {
+            attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            attr[na].val.programmaticStreamSerializationAllowed = 1;
+            ++na;
+        }
+        cfg.attrs = attr; cfg.numAttrs = na;
+        return cudaLaunchKernelEx(&cfg, trunk_mlp_pair_kernel, m.tm_d, m.tm_w1h, m.tm_w2h, p);
     }
     const int grid = p.n_tiles < num_sms ? p.n_tiles : num_sms;
     return launch_pdl(trunk_mlp_kernel, grid, kTrunkThreads, kTrunkSmem, st, 1, m.tm_d, m.tm_w1, m.tm_w2, p);

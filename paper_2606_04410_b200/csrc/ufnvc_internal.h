@@ -276,7 +276,7 @@ struct TrunkMaps {
 };
 bool trunk_make_maps(TrunkMaps &m, const bf16 *d_base, long long n_px, const ConvLayer &pw1, const ConvLayer &pw2, std::string &err);
 cudaError_t launch_trunk_mlp(const TrunkMaps &m, const ConvLayer &pw1, const ConvLayer &pw2, const bf16 *x, bf16 *out, long long n_px,
-                             int num_sms, bool pair, LaunchStream st, uint32_t *tile_done = nullptr);
+                             int num_sms, bool pair, LaunchStream st, uint32_t *tile_done = nullptr, bool quad_clusters = true);
 // the CTA-pair trunk kernel adds 1 to tile_done[tile] per drain warp (8) of the CTA that owns the 128-pixel tile: a tile is
 // complete (written, and its input rows no longer read) when its counter reaches kTrunkTileSignals
 constexpr uint32_t kTrunkTileSignals = 8;

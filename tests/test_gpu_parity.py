@@ -191,7 +191,7 @@ def test_whole_call_is_cuda_graph_capturable(decoders):
 
 
 @pytest.mark.parametrize("flag", ["force_generic", "no_pdl", "no_tail_fill", "fp64_head", "no_cta_pairs", "unfused_trunk",
-                                  "generic_final", "plain_depthwise", "no_transposed_tiles"])
+                                  "generic_final", "plain_depthwise", "no_transposed_tiles", "no_quad_clusters"])
 def test_every_debug_variant_matches_oracle(decoders, flag):
     """ufnvc_config.debug_flags swaps one kernel (or launch mechanism) for its kept cross-check variant; every kept variant
     is held to the same parity bar as the default path, on the crop of the headline layer plan that reaches every kernel."""
@@ -221,7 +221,7 @@ def test_every_debug_variant_matches_oracle(decoders, flag):
 def test_unknown_debug_flag_is_rejected():
     from paper_2606_04410_b200 import binding
     with pytest.raises(binding.UfnvcError, match="-2"):
-        binding.ChunkDecoder(synth.CONFIGS[1], debug_flags=0x200)
+        binding.ChunkDecoder(synth.CONFIGS[1], debug_flags=0x400)
 
 
 @pytest.mark.parametrize("scale", [10.0, 100.0])
