@@ -15,11 +15,12 @@
 // earlier / later -- the row shift costs no data movement at all -- and what is left to the warps is the column shift
 // between neighbouring lanes of ONE warp: 24 shuffles, no shared-memory exchange, no barrier, no coupling between warps.
 //
-// Tile = 12 rows x 32 columns of INPUT pixels (window origin one pixel up-left of the 10 x 30 output pixels it yields);
-// one TMA box {64 ch, 32, 12} (zero-filled outside the image = the conv's zero padding) = three 128-row A operands.
-// warp 0 = TMA producer, warp 1 = MMA issuer + TMEM allocator, warps 2..13 = one per tile row (group g = row / 4 reads
-// accumulator g; warp % 4 = TMEM lane quadrant).  Accumulators are double-buffered over tiles (2 x 3 x 48 columns), the
-// weights of the current frame (18 KB) stay resident in shared memory.
+// Tile = 16 rows x 32 columns of INPUT pixels (window origin one pixel up-left of the 14 x 30 output pixels it yields; 12 rows
+// measured 173 us, 16 rows 159 us: one halo row in eight instead of one in six);
+// one TMA box {64 ch, 32, 16} (zero-filled outside the image = the conv's zero padding) = four 128-row A operands.
+// warp 0 = TMA producer, warp 1 = MMA issuer + TMEM allocator, warps 2..17 = one per tile row (group g = row / 4 reads
+// accumulator g; warp % 4 = TMEM lane quadrant).  Accumulators are double-buffered over tiles (2 x 4 x 48 of 64 columns: all of
+// TMEM), the weights of the current frame (18 KB) stay resident in shared memory.
 #include <cuda.h>
 
 #include "tc_ptx.cuh"
@@ -29,12 +30,13 @@ namespace ufnvc {
 
 namespace {
 
-constexpr int kFR = 12, kFC = 32;                       // input rows / columns per tile
-constexpr int kFOutR = kFR - 2, kFOutC = kFC - 2;       // output pixels per tile: 10 x 30
+constexpr int kFG = 4;                                  // row groups (128-pixel MMA operands) per tile
+constexpr int kFR = 4 * kFG, kFC = 32;                  // input rows / columns per tile
+constexpr int kFOutR = kFR - 2, kFOutC = kFC - 2;       // output pixels per tile: 14 x 30
 constexpr int kFN = 48;                                 // 3 stencil columns x 16 packed output columns
-constexpr int kFAccStride = 64;                         // TMEM columns between accumulators (6 of them: 2 buffers x 3 row groups)
-constexpr int kFThreads = 14 * 32;
-constexpr uint32_t kFABytes = kFR * kFC * 128;          // 49152: one input tile, 64 channels
+constexpr int kFAccStride = 64;                         // TMEM columns between accumulators (2 buffers x kFG row groups = 512 columns)
+constexpr int kFThreads = (2 + kFR) * 32;
+constexpr uint32_t kFABytes = kFR * kFC * 128;          // 65536: one input tile, 64 channels
 constexpr uint32_t kFWBytes = 9 * 16 * 128;             // 18432: one frame's weights
 constexpr uint32_t kFWdy = 3 * 16 * 128;                // 6144: the 48 rows [dx][n] of one stencil row
 constexpr int kFAStages = 3;
@@ -42,6 +44,7 @@ constexpr int kFAStages = 3;
 // first / last row group then read mapped shared memory (values that only reach the tile's halo rows, which produce no output).
 constexpr uint32_t kFOffW = 0, kFOffA = kFWBytes, kFOffBar = kFOffA + kFAStages * kFABytes + 4096;
 constexpr uint32_t kFSmem = kFOffBar + 256 + 1024;
+static_assert(2 * kFG * kFAccStride <= 512 && kFSmem <= 227 * 1024, "accumulators fit TMEM, the stages fit shared memory");
 
 struct FDiv {                                            // division by a runtime constant (tile index -> coordinates)
     uint32_t d, mul, shr;
@@ -70,7 +73,7 @@ struct FinalParams {
 
 enum : uint32_t {
     F_AFULL = 0, F_AEMPTY = F_AFULL + kFAStages, F_WFULL = F_AEMPTY + kFAStages, F_WFREE = F_WFULL + 1, F_DFULL = F_WFREE + 1,
-    F_DEMPTY = F_DFULL + 6, F_TMEM = F_DEMPTY + 6
+    F_DEMPTY = F_DFULL + 2 * kFG, F_TMEM = F_DEMPTY + 2 * kFG
 };
 
 }  // namespace
@@ -104,7 +107,7 @@ final_is_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_w) : "memory");
         for (int s = 0; s < kFAStages; ++s) { mbar_init(bar(F_AFULL + s), 1); mbar_init(bar(F_AEMPTY + s), 1); }
         mbar_init(bar(F_WFULL), 1); mbar_init(bar(F_WFREE), 1);
-        for (int a = 0; a < 6; ++a) { mbar_init(bar(F_DFULL + a), 1); mbar_init(bar(F_DEMPTY + a), 4); }
+        for (int a = 0; a < 2 * kFG; ++a) { mbar_init(bar(F_DFULL + a), 1); mbar_init(bar(F_DEMPTY + a), 4); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) {
@@ -154,17 +157,17 @@ final_is_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant
                 const uint32_t a_lo = a_lo0 + uint32_t(sa) * (kFABytes >> 4);
                 const int buf = it & 1;
 #pragma unroll
-                for (int g = 0; g < 3; ++g) {
-                    mbar_wait(bar(F_DEMPTY + 3 * buf + g), ((it >> 1) & 1) ^ 1);   // the row warps of group g have drained this accumulator
+                for (int g = 0; g < kFG; ++g) {
+                    mbar_wait(bar(F_DEMPTY + kFG * buf + g), ((it >> 1) & 1) ^ 1);   // the row warps of group g have drained this accumulator
                     tc_fence_after();
 #pragma unroll
                     for (int dy = 0; dy < 3; ++dy)
 #pragma unroll
                         for (int k = 0; k < 4; ++k)                               // view shifted by dy - 1 tile rows = (dy - 1) * 4096 B = 256 units
-                            umma_bf16_lh(tmem_base + uint32_t((3 * buf + g) * kFAccStride),
+                            umma_bf16_lh(tmem_base + uint32_t((kFG * buf + g) * kFAccStride),
                                          a_lo + uint32_t(g) * (16384 >> 4) + uint32_t(256 * dy) - 256u + 2 * k, hi,
                                          w_lo + uint32_t(dy) * (kFWdy >> 4) + 2 * k, hi, idesc, uint32_t(dy | k));
-                    umma_commit(bar(F_DFULL + 3 * buf + g));
+                    umma_commit(bar(F_DFULL + kFG * buf + g));
                 }
                 umma_commit(bar(F_AEMPTY + sa));
                 if (++sa == kFAStages) { sa = 0; pa ^= 1; }
@@ -195,19 +198,19 @@ final_is_kernel(const __grid_constant__ CUtensorMap tm_in, const __grid_constant
                 bias_grp = t.grp;
             }
             const int buf = it & 1;
-            mbar_wait(bar(F_DFULL + 3 * buf + g), (it >> 1) & 1);
+            mbar_wait(bar(F_DFULL + kFG * buf + g), (it >> 1) & 1);
             tc_fence_after();
             // R_dx of this pixel: columns [16 dx, 16 dx + 12) of the accumulator.  The output pixel (y, x) takes R_0 from the pixel to
             // its left and R_2 from the pixel to its right: the neighbouring lanes of this warp.
             uint32_t r0[16], r1[16], r2[16];
-            const uint32_t t_acc = t_row + uint32_t((3 * buf + g) * kFAccStride);
+            const uint32_t t_acc = t_row + uint32_t((kFG * buf + g) * kFAccStride);
             ld16(t_acc, r0);
             ld16(t_acc + 16, r1);
             ld16(t_acc + 32, r2);
             tmem_ld_wait();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar(F_DEMPTY + 3 * buf + g));        // the accumulator may be overwritten (by tile it + 2)
+            if (lane == 0) mbar_arrive(bar(F_DEMPTY + kFG * buf + g));        // the accumulator may be overwritten (by tile it + 2)
             float o[12];
 #pragma unroll
             for (int n = 0; n < 12; ++n)
