@@ -287,6 +287,11 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
             flush_pending();
         } else {
             for (int c0 = half * 32; c0 < p.BN; c0 += 64) {
+                // the chunk's 32 biases are requested BEFORE the accumulator load is waited for: with ~225 KB of shared memory the L1
+                // is a few KB, a bias load is an L2 round trip, and behind the TMEM wait it was a second one in a row per chunk
+                float4 bb[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) bb[j] = __ldg(reinterpret_cast<const float4 *>(bias + c0) + j);
                 uint32_t v[32];
                 tmem_ld32(t_row + uint32_t(c0), v);
                 if (!inb) continue;
@@ -298,14 +303,14 @@ __device__ __forceinline__ void epilogue_warps(const TcParams &p, uint32_t tmem_
                 if (p.E.act == ACT_GELU) {
 #pragma unroll
                     for (int j = 0; j < 32; j += 4) {
-                        const float4 b4 = __ldg(reinterpret_cast<const float4 *>(bias + c0 + j));
+                        const float4 b4 = bb[j >> 2];
                         gelu_bias2(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), b4.x, b4.y, f[j], f[j + 1]);
                         gelu_bias2(__uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]), b4.z, b4.w, f[j + 2], f[j + 3]);
                     }
                 } else {
 #pragma unroll
                     for (int j = 0; j < 32; j += 4) {
-                        const float4 b4 = __ldg(reinterpret_cast<const float4 *>(bias + c0 + j));
+                        const float4 b4 = bb[j >> 2];
                         f[j] = __uint_as_float(v[j]) + b4.x; f[j + 1] = __uint_as_float(v[j + 1]) + b4.y;
                         f[j + 2] = __uint_as_float(v[j + 2]) + b4.z; f[j + 3] = __uint_as_float(v[j + 3]) + b4.w;
                     }
