@@ -201,136 +201,147 @@ __global__ void __launch_bounds__(256) hyper_conv_fast_kernel(const double *__re
     }
 }
 
-// ---- layers 0 and 1 (O1): direct implicit GEMM in fp64, ONE launch per layer.  B200's plain DFMA rate is 16 per clock and SM
-// (measured: 75 MFMA of layer 1 never ran under 16 us), so the two layers cost >= 25 us whatever the kernel; the job here is to
-// keep every SM's FP64 pipe busy without extra launches.  The z map is tiny (510 pixels at 1080p), so the output tile is small
-// -- 16 pixels x 32 channels, 32 x 4 tiles for 510 x 128 -- and K (9 taps x C_in) is split FOUR ways inside the block: 512
-// threads = 4 groups of 128, each group runs a quarter of the K steps on its own double-buffered shared-memory stage (named
-// barriers, no block-wide sync in the loop) with 2 x 2 outputs per thread; the groups' partial sums are added in fixed order
-// at the end (deterministic).  (The first build split the 9 taps over blockIdx.z and added the partials in a second launch:
-// 5 launches for the two layers where there are 2 now.)
+// ---- layers 0 and 1 (O1): direct implicit GEMM in fp64 on the FP64 TENSOR cores (mma.sync m8n8k4), ONE launch per layer.
+// The CUDA-core version of this kernel (2 x 2 outputs per thread, operands by LDS.128) took 27 + 16 us for 7 us of FP64 work
+// (61 DFMA per clock and SM measured, the same rate as DMMA), and clock64 stamps around its K steps did not move with a warm L2:
+// every LDS.128 delivers 512 bytes to a warp whatever the broadcast, 2 of them per 4 DFMA, and 16 warps saturate the 128 B/clk
+// shared-memory port (2.6 k cycles per 16-k step).  The m8n8k4 fragments need ONE 8-byte load per thread and operand for 256
+// FMAs of the warp: a fifth of the bytes (22 + 14 us).  What bounds it now is the operand traffic of so small a tile: 56 MB from
+// L2 per layer-1 launch, fetched in bursts by 2048 warps at once (a step's loads take 6-7 k cycles to come back); an L2
+// prefetch of the weights ahead of the predecessor wait changed nothing.
+// The z map is tiny (510 pixels at 1080p), so the output tile is small -- 16 pixels x 32 channels, 32 x 4 blocks for 510 x 128 --
+// and K (9 taps x C_in) is split over the block's 16 warps: each warp runs its share of the 16-k steps on its own shared-memory
+// stage (global -> registers one step ahead -> shared, __syncwarp only) and holds the whole tile's partial sums (2 x 4 fragments);
+// the partials are added in warp order at the end (deterministic).
 // ZIN: the input is the int16 hyper-latent itself, planar [n][c_z][pz] (layer 0), converted on load.
 // Epilogue: + bias, ReLU; layer 1 also adds the context branch q (R23), writes the 2-term bf16 split hi | mid the tensor-core
 // head reads, and this block's share of sum_c v^2 per pixel (xnorm2[m][n-tile]; the head adds the shares in order).
-constexpr int DM = 16, DN = 32, DK = 16, DG = 4;
-constexpr size_t kDirectSmem = size_t(DG) * 2 * DK * (DM + 2 + DN) * sizeof(double);      // 51.2 KB: dynamic
+constexpr int DM = 16, DN = 32, DK = 16, DW = 16;
+constexpr int kAS = 20, kBS = 36;           // row strides (doubles) of the A [k][pixel] and B [k][n] stages: = 4 (mod 16), so the 16 8-byte
+                                            // fragment loads of a half-warp (4 k rows x 4 columns) fall into 16 different bank pairs
+constexpr int kStageD = DK * kAS + DK * kBS;                                  // 896 doubles per warp
+constexpr size_t kDirectSmem = size_t(DW) * kStageD * sizeof(double);         // 112 KB: dynamic
+static_assert(DM * DN <= kStageD, "a warp's partial tile fits its own stage");
+
+__device__ __forceinline__ void dmma884(double (&d)[2], double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
+}
 
 template <bool ZIN>
-__global__ void __launch_bounds__(128 * DG) hyper_conv_direct_kernel(const void *__restrict__ in_raw, const double *__restrict__ wt,
-                                                                     const double *__restrict__ bias, int n_img, int hz, int wz, int c_in,
-                                                                     int n_out, double *__restrict__ out, const double *__restrict__ addend,
-                                                                     bf16 *__restrict__ xs, float *__restrict__ xnorm2)
+__global__ void __launch_bounds__(32 * DW) hyper_conv_direct_kernel(const void *__restrict__ in_raw, const double *__restrict__ wt,
+                                                                    const double *__restrict__ bias, int n_img, int hz, int wz, int c_in,
+                                                                    int n_out, double *__restrict__ out, const double *__restrict__ addend,
+                                                                    bf16 *__restrict__ xs, float *__restrict__ xnorm2)
 {
     extern __shared__ __align__(16) double direct_smem[];
-    double (*As)[2][DK][DM + 2] = reinterpret_cast<double (*)[2][DK][DM + 2]>(direct_smem);
-    double (*Bs)[2][DK][DN] = reinterpret_cast<double (*)[2][DK][DN]>(direct_smem + size_t(DG) * 2 * DK * (DM + 2));
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // (the bias does not depend on the predecessor grid: requested before the wait for it)
+    const double bias_o = blockIdx.y * DN + lane < n_out ? bias[blockIdx.y * DN + lane] : 0.0;
     asm volatile("griddepcontrol.wait;" ::: "memory");              // PDL: launched early, the predecessor's output is complete from here on
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    double *As = direct_smem + size_t(warp) * kStageD, *Bs = As + DK * kAS;
     const int pz = hz * wz;
     const int M = n_img * pz;
     const int m0 = blockIdx.x * DM, n0 = blockIdx.y * DN;
-    const int grp = threadIdx.x >> 7, tid = threadIdx.x & 127;
-    const int ty = tid >> 4, tx = tid & 15;                         // pixels 2 ty, 2 ty + 1; channels 2 tx, 2 tx + 1
-    // loaders (per group): A 16 px x 16 k (2 consecutive k per thread), B 16 k x 32 n (4 consecutive n per thread)
-    const int a_pix = tid >> 3, a_k = (tid & 7) * 2;
+    // loaders (per warp): A 16 px x 16 k (8 consecutive k per lane), B 16 k x 32 n (16 consecutive n per lane)
+    const int a_pix = lane >> 1, a_k = (lane & 1) * 8;
     const int gm = m0 + a_pix;
     const int a_img = gm < M ? gm / pz : 0, a_p = gm < M ? gm % pz : 0;
     const int a_y = a_p / wz, a_x = a_p % wz;
-    const int b_k = tid >> 3, b_n = (tid & 7) * 4;
-    const bool b_ok = n0 + b_n < n_out;                             // n_out % 4 == 0
+    const int b_k = lane >> 1, b_n = (lane & 1) * 16;
+    const bool b_ok = n0 + b_n < n_out;                             // n_out % 16 == 0
     const int ksteps_per_tap = c_in / DK;
     const int total_steps = 9 * ksteps_per_tap;
-    const int s_lo = total_steps * grp / DG, s_hi = total_steps * (grp + 1) / DG;     // this group's K steps
+    const int s_lo = total_steps * warp / DW, s_hi = total_steps * (warp + 1) / DW;   // this warp's K steps
     const double *in = static_cast<const double *>(in_raw);
     const int16_t *zin = static_cast<const int16_t *>(in_raw);
 
-    double ra[2];
-    double2 rb[2];
+    double ra[8];
+    double2 rb[8];
     auto gload = [&](int step) {
         const int tap = step / ksteps_per_tap, k0 = (step % ksteps_per_tap) * DK;
         const int yy = a_y + tap / 3 - 1, xx = a_x + tap % 3 - 1;
-        ra[0] = ra[1] = 0.0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) ra[j] = 0.0;
         if (gm < M && yy >= 0 && yy < hz && xx >= 0 && xx < wz) {
             if (ZIN) {
-                const long long o = ((long long)a_img * c_in + k0 + a_k) * pz + (long long)yy * wz + xx;
-                ra[0] = double(zin[o]); ra[1] = double(zin[o + pz]);
+                const int16_t *src = zin + ((long long)a_img * c_in + k0 + a_k) * pz + (long long)yy * wz + xx;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) ra[j] = double(src[(long long)j * pz]);
             } else {
-                const double2 v = *reinterpret_cast<const double2 *>(in + ((long long)a_img * pz + (long long)yy * wz + xx) * c_in + k0 + a_k);
-                ra[0] = v.x; ra[1] = v.y;
+                const double2 *src = reinterpret_cast<const double2 *>(in + ((long long)a_img * pz + (long long)yy * wz + xx) * c_in + k0 + a_k);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) { const double2 v = src[j]; ra[2 * j] = v.x; ra[2 * j + 1] = v.y; }
             }
         }
-        rb[0] = rb[1] = make_double2(0.0, 0.0);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) rb[j] = make_double2(0.0, 0.0);
         if (b_ok) {
             const double2 *src = reinterpret_cast<const double2 *>(wt + ((long long)tap * c_in + k0 + b_k) * n_out + n0 + b_n);
-            rb[0] = src[0]; rb[1] = src[1];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) rb[j] = src[j];
         }
     };
-    auto sstore = [&](int buf) {
-        As[grp][buf][a_k][a_pix] = ra[0]; As[grp][buf][a_k + 1][a_pix] = ra[1];
-        *reinterpret_cast<double2 *>(&Bs[grp][buf][b_k][b_n]) = rb[0];
-        *reinterpret_cast<double2 *>(&Bs[grp][buf][b_k][b_n + 2]) = rb[1];
+    auto sstore = [&]() {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) As[(a_k + j) * kAS + a_pix] = ra[j];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) *reinterpret_cast<double2 *>(&Bs[b_k * kBS + b_n + 2 * j]) = rb[j];
     };
-    auto group_sync = [&]() { asm volatile("bar.sync %0, 128;" ::"r"(grp + 1) : "memory"); };
 
-    double acc[2][2] = {};
-    if (s_lo < s_hi) {
-        gload(s_lo);
-        sstore(0);
-    }
-    group_sync();
+    double acc[2][4][2] = {};                                       // fragment (mt, nt): rows 8 mt + lane / 4, columns 8 nt + 2 (lane % 4) + {0, 1}
+    const int fk = lane & 3, fr = lane >> 2;
+    if (s_lo < s_hi) gload(s_lo);
     for (int step = s_lo; step < s_hi; ++step) {
-        const int buf = (step - s_lo) & 1;
+        __syncwarp();                                               // the previous step's fragment loads are done
+        sstore();
+        __syncwarp();
         if (step + 1 < s_hi) gload(step + 1);
 #pragma unroll
-        for (int k = 0; k < DK; ++k) {
-            const double2 a = *reinterpret_cast<const double2 *>(&As[grp][buf][k][ty * 2]);
-            const double2 b = *reinterpret_cast<const double2 *>(&Bs[grp][buf][k][tx * 2]);
-            acc[0][0] = fma(a.x, b.x, acc[0][0]); acc[0][1] = fma(a.x, b.y, acc[0][1]);
-            acc[1][0] = fma(a.y, b.x, acc[1][0]); acc[1][1] = fma(a.y, b.y, acc[1][1]);
+        for (int k4 = 0; k4 < DK / 4; ++k4) {
+            double a[2], b[4];
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) a[mt] = As[(4 * k4 + fk) * kAS + 8 * mt + fr];
+#pragma unroll
+            for (int nt = 0; nt < 4; ++nt) b[nt] = Bs[(4 * k4 + fk) * kBS + 8 * nt + fr];
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < 4; ++nt) dmma884(acc[mt][nt], a[mt], b[nt]);
         }
-        if (step + 1 < s_hi) sstore(buf ^ 1);
-        group_sync();
     }
-    // fixed-order reduction over the K groups: groups 1.. park their partial sums in their own (now idle) B stage
-    double *red = &Bs[grp][0][0][0];
-    if (grp > 0) {
-        red[tid] = acc[0][0]; red[128 + tid] = acc[0][1];           // 512 of the group's 2 x 16 x 32 doubles
-        red[256 + tid] = acc[1][0]; red[384 + tid] = acc[1][1];
-    }
+    // fixed-order reduction over the warps: every warp parks its partial tile [pixel][channel] in its own (now idle) stage
+    __syncwarp();
+#pragma unroll
+    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < 4; ++nt)
+            *reinterpret_cast<double2 *>(&As[(8 * mt + fr) * DN + 8 * nt + 2 * fk]) = make_double2(acc[mt][nt][0], acc[mt][nt][1]);
     __syncthreads();
-    if (grp > 0) return;
+    // one output per thread: warp = pixel of the tile, lane = channel
+    const int m = m0 + warp, o = n0 + lane;
+    double v = 0.0;
 #pragma unroll
-    for (int g2 = 1; g2 < DG; ++g2) {
-        const double *r2 = &Bs[g2][0][0][0];
-        acc[0][0] += r2[tid]; acc[0][1] += r2[128 + tid]; acc[1][0] += r2[256 + tid]; acc[1][1] += r2[384 + tid];
+    for (int w2 = 0; w2 < DW; ++w2) v += direct_smem[size_t(w2) * kStageD + warp * DN + lane];
+    double ss = 0.0;
+    if (m < M && o < n_out) {
+        v += bias_o;
+        v = v > 0.0 ? v : 0.0;
+        const long long e = (long long)m * n_out + o;
+        if (addend) v += addend[e];                                 // s = x2 + q (R23)
+        out[e] = v;
+        if (xs) {
+            const bf16 hi = __double2bfloat16(v);
+            xs[(long long)m * 2 * n_out + o] = hi;
+            xs[(long long)m * 2 * n_out + n_out + o] = __double2bfloat16(v - double(__bfloat162float(hi)));
+        }
+        ss = v * v;
     }
-
+    if (xnorm2) {                                                   // the warp holds pixel m's 32 channels of this n tile
 #pragma unroll
-    for (int i = 0; i < 2; ++i) {
-        const int m = m0 + ty * 2 + i;                              // uniform per half-warp; every lane joins the shuffles
-        double ss = 0.0;
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            const int o = n0 + tx * 2 + j;
-            if (m < M && o < n_out) {
-                double v = acc[i][j] + bias[o];
-                v = v > 0.0 ? v : 0.0;
-                const long long e = (long long)m * n_out + o;
-                if (addend) v += addend[e];                         // s = x2 + q (R23)
-                out[e] = v;
-                if (xs) {
-                    const bf16 hi = __double2bfloat16(v);
-                    xs[(long long)m * 2 * n_out + o] = hi;
-                    xs[(long long)m * 2 * n_out + n_out + o] = __double2bfloat16(v - double(__bfloat162float(hi)));
-                }
-                ss = fma(v, v, ss);
-            }
-        }
-        if (xnorm2) {                                               // the 16 lanes tx = 0..15 of this half-warp hold pixel m's 32 channels
-#pragma unroll
-            for (int o = 8; o > 0; o >>= 1) ss += __shfl_xor_sync(0xFFFFFFFFu, ss, o);
-            if (tx == 0 && m < M) xnorm2[(long long)m * gridDim.y + blockIdx.y] = float(ss);
-        }
+        for (int d = 16; d > 0; d >>= 1) ss += __shfl_xor_sync(0xFFFFFFFFu, ss, d);
+        if (lane == 0 && m < M) xnorm2[(long long)m * gridDim.y + blockIdx.y] = float(ss);
     }
 }
 
@@ -424,7 +435,7 @@ template <typename... KArgs, typename... Args>
 static cudaError_t launch_direct(void (*kern)(KArgs...), dim3 grid, LaunchStream st, Args &&...args)      // 2-D grid + dynamic smem + PDL
 {
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = grid; cfg.blockDim = dim3(128 * DG); cfg.dynamicSmemBytes = kDirectSmem; cfg.stream = st.s;
+    cfg.gridDim = grid; cfg.blockDim = dim3(32 * DW); cfg.dynamicSmemBytes = kDirectSmem; cfg.stream = st.s;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
@@ -438,7 +449,7 @@ cudaError_t launch_hyper_conv(const HyperLayer &L, const void *in, bool in_is_z,
                               bf16 *xs, float *xnorm2, const double *addend)
 {
     const int M = n_img * hz * wz;
-    if (L.c_in % DK == 0 && L.n % 4 == 0) {
+    if (L.c_in % DK == 0 && L.n % 16 == 0) {
         dim3 grid((M + DM - 1) / DM, (L.n + DN - 1) / DN);
         if (in_is_z)
             return launch_direct(hyper_conv_direct_kernel<true>, grid, st, in, L.w, L.bias, n_img, hz, wz, L.c_in, L.n, out, addend, xs, xnorm2);
