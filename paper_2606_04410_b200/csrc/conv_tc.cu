@@ -911,7 +911,7 @@ cudaError_t configure_conv_tc_kernels()
 {
     cudaError_t e = cudaSuccess;
     auto set = [&](auto kern) { if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); };
-    set(conv_halo_pair_kernel<EPI_PS2>); set(conv_halo_pair_kernel<EPI_HEAD>);
+    set(conv_halo_pair_kernel<EPI_PS2>); set(conv_halo_pair_kernel<EPI_HEAD>); set(conv_halo_pair_kernel<EPI_MU>);
     set(conv_halo_kernel<EPI_NHWC, true>); set(conv_halo_kernel<EPI_NHWC, false>);
     set(conv_halo_kernel<EPI_PS2, true>); set(conv_halo_kernel<EPI_PS2, false>);
     set(conv_halo_kernel<EPI_HEAD, false>);
@@ -925,7 +925,7 @@ cudaError_t configure_conv_tc_kernels()
 cudaError_t launch_conv_halo_pair(const ConvLayer &L, const ConvProblem &P, const CUtensorMap &tmap_halo, const EpiParams &E, int num_sms,
                                   LaunchStream st, bool transposed)
 {
-    if (L.taps != 9 || !L.has_half_map || (E.mode != EPI_PS2 && E.mode != EPI_HEAD)) return cudaErrorInvalidValue;
+    if (L.taps != 9 || !L.has_half_map || (E.mode != EPI_PS2 && E.mode != EPI_HEAD && E.mode != EPI_MU)) return cudaErrorInvalidValue;
     TcParams p{};
     p.H = P.H; p.W = P.W;
     p.xpose = transposed ? 1 : 0;
@@ -954,6 +954,7 @@ cudaError_t launch_conv_halo_pair(const ConvLayer &L, const ConvProblem &P, cons
     const size_t smem = 1024 + size_t(na) * kHaloStage + size_t(nb) * bh_bytes + 256 + 16 * size_t(nb) + 16 * size_t(na);
     const int clusters = p.total_tiles < num_sms / 2 ? p.total_tiles : num_sms / 2;
     if (E.mode == EPI_HEAD) return launch_pdl(conv_halo_pair_kernel<EPI_HEAD>, 2 * clusters, kThreads, smem, st, 2, tmap_halo, L.tmap_w_half, p, nb, na);
+    if (E.mode == EPI_MU) return launch_pdl(conv_halo_pair_kernel<EPI_MU>, 2 * clusters, kThreads, smem, st, 2, tmap_halo, L.tmap_w_half, p, nb, na);
     return launch_pdl(conv_halo_pair_kernel<EPI_PS2>, 2 * clusters, kThreads, smem, st, 2, tmap_halo, L.tmap_w_half, p, nb, na);
 }
 

@@ -22,7 +22,7 @@ cudaError_t conv(ufnvc_handle *h, const ConvLayer &L, const ConvProblem &P, cons
 {
     if (launches) ++*launches;
     if (L.use_tc && L.taps == 9 && am.halo_ok && !h->force_generic && h->use_pair_conv && L.has_half_map &&
-        E.mode == EPI_PS2 && P.W > 8)
+        (E.mode == EPI_PS2 || E.mode == EPI_MU) && P.W > 8)
         return launch_conv_halo_pair(L, P, am.halo_t ? am.tm_halo_t : am.tm_halo, E, h->num_sms, st, am.halo_t);
     if (L.use_tc && L.taps == 9 && am.halo_ok && !h->force_generic)
         return launch_conv_halo(L, P, am.tm_halo, E, h->num_sms, st);
@@ -327,7 +327,13 @@ extern "C" int ufnvc_load_weights(ufnvc_handle *h, const void *blob_host, size_t
         ok = ok && tc_make_weight_tmap(h->ctx_fold, err, fold_bn) && tc_make_weight_tmap(h->ctx_out, err);
         for (auto &tb : h->ctx_blocks) ok = ok && tc_make_weight_tmap(tb.pw1, err) && tc_make_weight_tmap(tb.pw2, err);
     }
-    for (int k = 0; k < 3 && c.mu_steps == 4; ++k) ok = ok && tc_make_weight_tmap(h->mu_net[k], err);
+    // progressive means: three small 3x3 convs in a row on the latent map -- n tiles of 64 on the CTA-pair kernel when that puts a
+    // unit on (nearly) every pair instead of one 128-wide tile on half of the SMs
+    for (int k = 0; k < 3 && c.mu_steps == 4; ++k) {
+        const long pairs = ((long(h->h + 15) / 16) * ((h->w + 7) / 8) + 1) / 2 * h->max_chunks;
+        const int mu_bn = (h->mu_net[k].n_pad % 64 == 0 && pairs * (h->mu_net[k].n_pad / 64) <= h->num_sms / 2 + 8) ? 64 : 0;
+        ok = ok && tc_make_weight_tmap(h->mu_net[k], err, mu_bn);
+    }
     if (!ok) return fail(h, UFNVC_E_CUDA, err);
     const int n = h->max_chunks, T = c.T;
     if (h->hybrid_head) ok = make_act_map(h, h->am_xs, h->xs, n, h->h_z, h->w_z, 2 * c.c_hyper, false, 1);
