@@ -329,9 +329,11 @@ namespace {
 // the 122 GB/s per SM the tensor core would consume (measured: tensor pipe 42 % active, L2 throughput 21 %).  A pair of
 // CTAs on one TPC runs ONE M = 256 MMA over both d tiles; each CTA stores only HALF of every weight tile (N/2 rows), so
 // the bytes per SM and per tile drop to 512 KB and a ring stage now lasts a whole GEMM1 or GEMM2 chunk (1024 tensor
-// cycles).  The leader CTA (rank 0) issues all MMAs; both CTAs run their own TMA producer and their own 8 epilogue
-// warps.  Barriers the MMA thread waits on live in the leader (the peer signals them through the cluster window);
-// barriers signalled by tcgen05.commit are multicast to both CTAs.
+// cycles).  The pair's leader CTA (even cluster rank) issues all MMAs; both CTAs run their own producers and epilogue warps.
+// Barriers the MMA thread waits on live in the leader (the peer signals them through the cluster window); barriers signalled
+// by tcgen05.commit are multicast to both CTAs.  Warps of a CTA: 0 weight producer, 1 MMA issuer + TMEM allocator, 2..5 GELU
+// (one per TMEM lane quadrant = scheduler), 6..13 output drain (two per quadrant), 14 relay and 15 input-tile producer (see
+// the cluster-of-two-pairs note in the kernel).
 // TMH = true: the GELU'd hidden chunk goes back into TMEM (bf16, over the fp32 columns it came from) and GEMM2 reads its
 // A operand from there: no 64 KB Hs buffer (the weight ring grows from 3 to 5 stages), and per tile 256 KB of st.shared
 // plus 256 KB of A-operand reads leave the shared-memory port, which TMA writes + MMA operand reads had saturated.
